@@ -1,0 +1,476 @@
+"""Pins for the CPU oracle: every oracle function is checked against something OTHER than itself
+(closed forms, impulse responses, the adjoint identity, brute-force Python loops, the float64
+routines of torch/numpy, invariants).  The paper prints no numeric worked example (all figures
+are images), so no paper-printed values exist to pin to -- see DESIGN.md.
+CPU only: `-m "not gpu"`.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2108_12430_b200 import specs as S
+from paper_2108_12430_b200 import synth
+
+RNG = np.random.default_rng(1234)
+
+
+# ------------------------------------------------------------------------------ D1 snapshot
+
+@pytest.mark.parametrize("W,S,C", [(512, 64, 22), (48, 7, 3), (10, 10, 1), (33, 1, 2), (64, 3, 5)])
+def test_snapshot_equals_slicing_of_zero_prefixed_stream(W, S, C):
+    """state <- previous snapshot updated by floor(fs/r) strictly new samples.
+    Pin: snapshot_t == last W samples of (zeros(W) ++ all samples so far), bit-exact, including
+    warm-up and S not dividing W."""
+    n_up = 3 * (W // S) + 5
+    x = RNG.standard_normal((C, n_up * S)).astype(np.float32)
+    padded = np.concatenate([np.zeros((C, W), np.float32), x], axis=1)
+    for t in range(n_up):
+        snap, first = oracle.snapshot(x[:, :(t + 1) * S], t, S, W)
+        end = W + (t + 1) * S
+        assert first == (t + 1) * S - W
+        assert np.array_equal(snap.view(np.uint32), padded[:, end - W:end].view(np.uint32))
+
+
+def test_snapshot_is_shift_by_stride_of_previous():
+    """PAPER.md:172 (Fig. 13): consecutive snapshots overlap in all but S samples."""
+    W, S, C = 96, 8, 4
+    x = RNG.standard_normal((C, 40 * S)).astype(np.float32)
+    prev, _ = oracle.snapshot(x[:, :S], 0, S, W)
+    for t in range(1, 40):
+        cur, _ = oracle.snapshot(x[:, :(t + 1) * S], t, S, W)
+        assert np.array_equal(cur[:, :W - S], prev[:, S:])
+        assert np.array_equal(cur[:, W - S:], x[:, t * S:(t + 1) * S])
+        prev = cur
+
+
+# -------------------------------------------------------------------------------- D2 conv1d
+
+def _brute_conv1d(x, w, b, s, pL, pR):
+    Cout, Cin, K = w.shape
+    L = x.shape[1]
+    Lout = (L + pL + pR - K) // s + 1
+    xp = [[0.0] * (pL + L + pR) for _ in range(Cin)]
+    for ci in range(Cin):
+        for i in range(L):
+            xp[ci][pL + i] = float(x[ci, i])
+    y = np.zeros((Cout, Lout))
+    for co in range(Cout):
+        for l in range(Lout):
+            acc = float(b[co])
+            for ci in range(Cin):
+                for j in range(K):
+                    acc += float(w[co, ci, j]) * xp[ci][s * l + j]
+            y[co, l] = acc
+    return y
+
+
+@pytest.mark.parametrize("Cin,Cout,L,K,s,pL,pR", [(1, 1, 16, 7, 2, 3, 3), (2, 2, 19, 7, 2, 3, 3),
+                                                  (2, 1, 12, 8, 1, 3, 4), (1, 2, 9, 3, 1, 0, 0)])
+def test_conv1d_brute_force(Cin, Cout, L, K, s, pL, pR):
+    x = RNG.standard_normal((Cin, L)); w = RNG.standard_normal((Cout, Cin, K)); b = RNG.standard_normal(Cout)
+    y = oracle.conv1d(x, w, b, s, pL, pR)
+    assert np.allclose(y, _brute_conv1d(x, w, b, s, pL, pR), rtol=0, atol=1e-13)
+
+
+def test_conv1d_impulse_reproduces_reversed_kernel():
+    """A unit impulse at l0 in channel ci gives y[co][l] = w[co][ci][l0 + pL - s*l] + b[co]:
+    the kernel appears reversed along l (every s-th tap for stride s)."""
+    Cin, Cout, L, K, pL, pR = 3, 4, 40, 7, 3, 3
+    w = RNG.standard_normal((Cout, Cin, K)); b = RNG.standard_normal(Cout)
+    for s in (1, 2):
+        for ci in range(Cin):
+            for l0 in (0, 1, 17, 18, L - 1):
+                x = np.zeros((Cin, L)); x[ci, l0] = 1.0
+                y = oracle.conv1d(x, w, b, s, pL, pR)
+                for co in range(Cout):
+                    for l in range(y.shape[1]):
+                        j = l0 + pL - s * l
+                        exp = b[co] + (w[co, ci, j] if 0 <= j < K else 0.0)
+                        assert y[co, l] == pytest.approx(exp, abs=1e-15)
+
+
+@pytest.mark.parametrize("s,pL,pR,K", [(2, 3, 3, 7), (1, 3, 4, 8), (3, 1, 2, 5)])
+def test_conv1d_matches_torch_float64(s, pL, pR, K):
+    Cin, Cout, L = 5, 6, 67
+    x = RNG.standard_normal((Cin, L)); w = RNG.standard_normal((Cout, Cin, K)); b = RNG.standard_normal(Cout)
+    xt = torch.nn.functional.pad(torch.from_numpy(x)[None], (pL, pR))
+    ref = torch.nn.functional.conv1d(xt, torch.from_numpy(w), torch.from_numpy(b), stride=s)[0].numpy()
+    assert np.allclose(oracle.conv1d(x, w, b, s, pL, pR), ref, rtol=0, atol=1e-12)
+
+
+def test_conv1d_linearity_and_shift_equivariance():
+    Cin, Cout, L, K, s = 3, 2, 64, 7, 2
+    w = RNG.standard_normal((Cout, Cin, K))
+    x1 = RNG.standard_normal((Cin, L)); x2 = RNG.standard_normal((Cin, L))
+    f = lambda x: oracle.conv1d(x, w, None, s, 3, 3)
+    assert np.allclose(f(2.5 * x1 - x2), 2.5 * f(x1) - f(x2), atol=1e-12)
+    xs = np.zeros_like(x1); xs[:, s * 3:] = x1[:, :-s * 3]        # shift input by 3*s samples
+    y, ys = f(x1), f(xs)
+    assert np.allclose(ys[:, 3 + 2:-2], y[:, 2:-3 - 2], atol=1e-12)   # away from the edges
+
+
+# ------------------------------------------------------------------------ D3 conv_transpose1d
+
+def test_convt_impulse_reproduces_kernel_unreversed():
+    """Impulse at l0 in channel ci -> y[co][s*l0 + j - p] = w[ci][co][j] (+ bias)."""
+    Cin, Cout, L, K, s, p, op = 3, 2, 12, 7, 2, 3, 1
+    w = RNG.standard_normal((Cin, Cout, K)); b = RNG.standard_normal(Cout)
+    for ci in range(Cin):
+        for l0 in (0, 1, 6, L - 1):
+            x = np.zeros((Cin, L)); x[ci, l0] = 1.0
+            y = oracle.conv_transpose1d(x, w, b, s, p, op)
+            assert y.shape == (Cout, 2 * L)
+            exp = np.tile(b[:, None], (1, 2 * L))
+            for j in range(K):
+                m = s * l0 + j - p
+                if 0 <= m < 2 * L:
+                    exp[:, m] += w[ci, :, j]
+            assert np.allclose(y, exp, atol=1e-15)
+
+
+@pytest.mark.parametrize("s,p,op,K", [(2, 3, 1, 7), (1, 0, 0, 3), (3, 2, 2, 7)])
+def test_convt_is_adjoint_of_conv(s, p, op, K):
+    """<Conv(x; w), y> == <x, ConvT(y; w)> with zero bias pins every index convention of D3
+    against D2 (which is pinned by brute force and impulses) with no reference implementation."""
+    Ca, Cb, Lb = 4, 3, 11                      # ConvT: Cb channels, length Lb -> Ca channels
+    w = RNG.standard_normal((Cb, Ca, K))       # ConvT weight [Cin=Cb][Cout=Ca][K]
+    yv = RNG.standard_normal((Cb, Lb))
+    z = oracle.conv_transpose1d(yv, w, None, s, p, op)          # [Ca][La]
+    La = z.shape[1]
+    x = RNG.standard_normal((Ca, La))
+    # The forward conv whose adjoint this is: weight [Cout=Cb][Cin=Ca][K], stride s, pad p; it maps
+    # length La to floor((La + 2p - K)/s) + 1 = Lb when La = (Lb-1)s - 2p + K + op and op < s.
+    cx = oracle.conv1d(x, w, None, s, p, p)
+    assert cx.shape == (Cb, Lb)
+    assert float(np.sum(cx * yv)) == pytest.approx(float(np.sum(x * z)), rel=1e-12, abs=1e-12)
+
+
+def test_convt_matches_torch_float64():
+    Cin, Cout, L, K, s, p, op = 5, 4, 23, 7, 2, 3, 1
+    x = RNG.standard_normal((Cin, L)); w = RNG.standard_normal((Cin, Cout, K)); b = RNG.standard_normal(Cout)
+    ref = torch.nn.functional.conv_transpose1d(torch.from_numpy(x)[None], torch.from_numpy(w),
+                                               torch.from_numpy(b), stride=s, padding=p,
+                                               output_padding=op)[0].numpy()
+    assert np.allclose(oracle.conv_transpose1d(x, w, b, s, p, op), ref, rtol=0, atol=1e-12)
+
+
+def test_convt_polyphase_split_matches_scatter_definition():
+    """D3 for s=2, K=7, p=3, op=1: even outputs m=2q use taps j in {1,3,5} at l = q + (3-j)/2, odd
+    outputs m=2q+1 use j in {0,2,4,6} at l = q + (4-j)/2.  (The split the CUDA path is built on is
+    derived here from the definition, independently of any kernel.)"""
+    Cin, Cout, L = 3, 2, 16
+    x = RNG.standard_normal((Cin, L)); w = RNG.standard_normal((Cin, Cout, 7)); b = RNG.standard_normal(Cout)
+    y = oracle.conv_transpose1d(x, w, b, 2, 3, 1)
+    exp = np.zeros((Cout, 2 * L))
+    for co in range(Cout):
+        for q in range(L):
+            e = b[co]; o = b[co]
+            for ci in range(Cin):
+                for j in (1, 3, 5):
+                    l = q + (3 - j) // 2
+                    if 0 <= l < L:
+                        e += w[ci, co, j] * x[ci, l]
+                for j in (0, 2, 4, 6):
+                    l = q + (4 - j) // 2
+                    if 0 <= l < L:
+                        o += w[ci, co, j] * x[ci, l]
+            exp[co, 2 * q] = e; exp[co, 2 * q + 1] = o
+    assert np.allclose(y, exp, atol=1e-13)
+
+
+# ---------------------------------------------------------------------------- D4 BatchNorm fold
+
+@pytest.mark.parametrize("kind", [S.KIND_CONV, S.KIND_CONVT])
+def test_bn_fold_equals_unfolded(kind):
+    Cin, Cout, K, L = 4, 5, 7, 20
+    shape = (Cout, Cin, K) if kind == S.KIND_CONV else (Cin, Cout, K)
+    w = RNG.standard_normal(shape); b = RNG.standard_normal(Cout)
+    g = RNG.uniform(0.5, 1.5, Cout); be = RNG.uniform(-0.1, 0.1, Cout)
+    mu = 0.1 * RNG.standard_normal(Cout); var = RNG.uniform(0.5, 1.5, Cout); eps = 1e-5
+    x = RNG.standard_normal((Cin, L))
+    conv = (lambda w_, b_: oracle.conv1d(x, w_, b_, 2, 3, 3)) if kind == S.KIND_CONV else \
+           (lambda w_, b_: oracle.conv_transpose1d(x, w_, b_, 2, 3, 1))
+    unfolded = oracle.batchnorm(conv(w, b), g, be, mu, var, eps)
+    wf, bf = oracle.bn_fold(kind, w, b, g, be, mu, var, eps)
+    assert np.allclose(conv(wf, bf), unfolded, rtol=0, atol=1e-12)
+    # and against the textbook formula evaluated by numpy
+    z = conv(w, b)
+    assert np.allclose(unfolded, g[:, None] * (z - mu[:, None]) / np.sqrt(var[:, None] + eps) + be[:, None], atol=1e-13)
+
+
+# ---------------------------------------------------------------------------- D5/D6 small ops
+
+def test_activations_pool_gap_dense_sigmoid_brute_force():
+    x = RNG.standard_normal((3, 22))
+    assert np.allclose(oracle.activation(x, S.ACT_TANH), np.tanh(x), atol=1e-15)
+    assert np.array_equal(oracle.activation(x, S.ACT_RELU), np.maximum(x, 0.0))
+    assert np.array_equal(oracle.activation(x, S.ACT_NONE), x)
+    mp = oracle.maxpool1d(x, 4)
+    assert mp.shape == (3, 5)
+    for c in range(3):
+        for q in range(5):
+            assert mp[c, q] == max(x[c, 4 * q + i] for i in range(4))
+    assert np.allclose(oracle.gap(x), [sum(x[c]) / 22 for c in range(3)], atol=1e-15)
+    w = RNG.standard_normal((4, 3)); b = RNG.standard_normal(4); v = RNG.standard_normal(3)
+    assert np.allclose(oracle.dense(v, w, b), [sum(w[o, i] * v[i] for i in range(3)) + b[o] for o in range(4)], atol=1e-14)
+    for z in (-30.0, -1.0, 0.0, 0.3, 12.0):
+        assert oracle.sigmoid(z) == pytest.approx(1.0 / (1.0 + math.exp(-z)), abs=1e-16)
+    assert oracle.sigmoid(0.0) == 0.5
+
+
+def test_relu_maxpool_bias_commute_exactly():
+    """A19: all three are monotone, so the epilogue order is free."""
+    x = RNG.standard_normal((4, 32)); b = RNG.standard_normal(4)
+    a = oracle.maxpool1d(oracle.activation(x + b[:, None], S.ACT_RELU), 4)
+    c = oracle.activation(oracle.maxpool1d(x, 4) + b[:, None], S.ACT_RELU)
+    assert np.array_equal(a, c)
+
+
+# ------------------------------------------------------------------------------- rounding (A9)
+
+def test_round_storage_matches_library_casts_and_tie_rules():
+    v32 = np.concatenate([RNG.standard_normal(4000), RNG.standard_normal(500) * 1e-3,
+                          RNG.standard_normal(500) * 300.0]).astype(np.float32)
+    got = oracle.round_storage(v32.astype(np.float64), oracle.DT_BF16)
+    ref = torch.from_numpy(v32).to(torch.bfloat16).to(torch.float64).numpy()
+    assert np.array_equal(got, ref)
+    got16 = oracle.round_storage(v32.astype(np.float64), oracle.DT_FP16)
+    assert np.array_equal(got16, v32.astype(np.float16).astype(np.float64))
+    v64 = RNG.standard_normal(4000) * 3.0
+    assert np.array_equal(oracle.round_storage(v64, oracle.DT_FP32), v64.astype(np.float32).astype(np.float64))
+    assert np.array_equal(oracle.round_storage(v64, oracle.DT_FP16), v64.astype(np.float16).astype(np.float64))
+    # ties go to even; values are exact in double
+    r = lambda x, d: float(oracle.round_storage(np.array([x]), d)[0])
+    assert r(1 + 2**-8, oracle.DT_BF16) == 1.0
+    assert r(1 + 3 * 2**-8, oracle.DT_BF16) == 1 + 2**-6
+    assert r(1 + 2**-8 + 2**-30, oracle.DT_BF16) == 1 + 2**-7     # just above the tie: up (no double rounding)
+    assert r(1 + 2**-11, oracle.DT_FP16) == 1.0
+    assert r(-(1 + 3 * 2**-11), oracle.DT_FP16) == -(1 + 2**-9)
+    assert r(0.0, oracle.DT_BF16) == 0.0
+
+
+# -------------------------------------------------------------- whole-autoencoder index pin
+
+def test_autoencoder_indexing_closed_form_through_all_layers():
+    """Identity activation + centre-tap delta kernels on one channel path: each encoder layer keeps
+    x[2l], each decoder layer zero-stuffs, so output[m] = x[m] if 2^d | m else 0 (d = depth)."""
+    widths = [21, 8, 16, 32]
+    layers = S.deepclean_layers(widths, bn=False)
+    layers = [S.ConvSpec(l.kind, l.cin, l.cout, l.k, l.stride, l.pad_l, l.pad_r, S.ACT_NONE) for l in layers]
+    prepared = []
+    for l in layers:
+        w = np.zeros(l.wshape()); w[0, 0, 3] = 1.0      # channel 0 -> channel 0, centre tap
+        prepared.append((w, np.zeros(l.cout)))
+    W = 128
+    x = RNG.standard_normal((21, W))
+    p = oracle.deepclean_forward(x, layers, prepared)
+    exp = np.where(np.arange(W) % 8 == 0, x[0], 0.0)
+    assert p.shape == (W,)
+    assert np.array_equal(p, exp)
+
+
+def test_deepclean_forward_matches_torch_float64_model():
+    """Library special case: the same stack built from torch's float64 conv routines."""
+    cfg = S.config_c0()
+    params = synth.deepclean_params(7, cfg.dc_layers)
+    prepared = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.dc_layers, params)]
+    x = RNG.standard_normal((21, 512))
+    p = oracle.deepclean_forward(x, cfg.dc_layers, prepared)
+    h = torch.from_numpy(x)[None]
+    for l, (w, b) in zip(cfg.dc_layers, prepared):
+        wt, bt = torch.from_numpy(w), torch.from_numpy(b)
+        if l.kind == S.KIND_CONV:
+            h = torch.nn.functional.conv1d(h, wt, bt, stride=2, padding=3)
+        else:
+            h = torch.nn.functional.conv_transpose1d(h, wt, bt, stride=2, padding=3, output_padding=1)
+        if l.act == S.ACT_TANH:
+            h = torch.tanh(h)
+    assert np.allclose(p, h[0, 0].numpy(), rtol=0, atol=1e-12)
+    assert 0.05 < float(np.sqrt(np.mean(p * p))) < 20.0
+
+
+def test_kaiming_init_keeps_preactivations_order_one():
+    """A7's rationale: with gain 5/3 the tanh layers are genuinely non-linear."""
+    cfg = S.config_c0()
+    params = synth.deepclean_params(0, cfg.dc_layers)
+    prepared = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.dc_layers, params)]
+    x = synth.white_channels(0, 21, 512).astype(np.float64)
+    _, acts = oracle.deepclean_forward(x, cfg.dc_layers, prepared, return_all=True)
+    for l, a in zip(cfg.dc_layers[:-1], acts[:-1]):
+        rms = float(np.sqrt(np.mean(a * a)))
+        assert 0.25 < rms < 1.0, rms          # tanh output RMS: O(1) pre-activations
+
+
+# ------------------------------------------------------------------------------ D7 Hann OLA
+
+def test_hann_is_periodic_and_shifted_copies_sum_to_k_over_2():
+    for W, k in [(512, 8), (64, 2), (96, 3), (32768, 32), (30, 5)]:
+        w = oracle.hann(W)
+        assert w[0] == 0.0 and w[W - 1] > 0.0
+        assert np.allclose(w, [0.5 - 0.5 * math.cos(2 * math.pi * n / W) for n in range(W)], atol=1e-15)
+        Sx = W // k
+        tot = sum(w[i * Sx:(i + 1) * Sx] for i in range(k))
+        assert np.allclose(tot, k / 2.0, atol=1e-9)
+
+
+def _stream_oracle(W, S_, n_up, dc_fn=None, agg=oracle.AGG_HANN_OLA, delta=0):
+    """StreamOracle with 1 detector (1 witness row + strain row) whose DeepClean is replaced by a
+    caller-supplied prediction function of the snapshot (to pin aggregation on its own)."""
+    so = oracle.StreamOracle(2, W, S_, [([0], 1)], [(None, None)], None, agg=agg, delta=delta, max_updates=n_up)
+    return so
+
+
+def test_ola_constant_prediction_reproduces_constant(monkeypatch):
+    """north_star: 'a constant window through the Hann overlap-add reproduces the constant'."""
+    W, S_, n_up, c = 64, 8, 30, 0.37
+    monkeypatch.setattr(oracle, "deepclean_forward", lambda x, layers, prepared: np.full(W, c))
+    so = _stream_oracle(W, S_, n_up)
+    x = RNG.standard_normal((2, n_up * S_)).astype(np.float32)
+    for t in range(n_up):
+        out = so.update(x[:, t * S_:(t + 1) * S_])
+        first = out["first_index"]
+        valid = (np.arange(W) + first) >= 0
+        assert np.allclose(out["nhat_running"][0][valid], c, atol=1e-14)
+        assert np.allclose(out["nhat_running"][0][~valid], 0.0)
+        assert np.allclose(out["cleaned_running"][0][valid], x[1, max(first, 0):first + W].astype(np.float64) - c, atol=1e-14)
+        if first >= 0:
+            assert np.allclose(out["nhat_final"][0], c, atol=1e-14)
+
+
+def test_ola_consistent_predictions_reproduce_signal_and_finality(monkeypatch):
+    """(iv) if every window predicts the same underlying g[a], nhat == g exactly; (v) a sample is
+    final after update floor(a/S) + k - 1 and never changes afterwards; (iii) wsum follows the
+    closed form of A11: wsum_t at window position n = Cs[n] - Cs[n + (t+1)S]."""
+    W, S_, n_up = 48, 6, 26
+    k = W // S_
+    g = RNG.standard_normal(n_up * S_ + W)
+    state = {"t": -1}
+
+    def fake(x, layers, prepared):
+        state["t"] += 1
+        first = (state["t"] + 1) * S_ - W
+        return np.array([g[first + n + W] for n in range(W)])       # g indexed with offset W
+
+    monkeypatch.setattr(oracle, "deepclean_forward", fake)
+    so = _stream_oracle(W, S_, n_up)
+    x = RNG.standard_normal((2, n_up * S_)).astype(np.float32)
+    w = oracle.hann(W)
+    Cs = np.zeros(2 * W + n_up * S_ + 1)
+    for m in range(W):
+        Cs[m] = sum(w[m + j * S_] for j in range(k) if m + j * S_ < W)
+    finals = {}
+    history = {}
+    for t in range(n_up):
+        out = so.update(x[:, t * S_:(t + 1) * S_])
+        first = out["first_index"]
+        for n in range(W):
+            a = first + n
+            if a < 0:
+                continue
+            assert out["nhat_running"][0][n] == pytest.approx(g[a + W], abs=1e-12)
+            assert so.wsum[0][a] == pytest.approx(Cs[n] - Cs[min(n + (t + 1) * S_, len(Cs) - 1)], abs=1e-12)
+            history.setdefault(a, []).append((t, out["nhat_running"][0][n]))
+        if first >= 0:
+            for i in range(S_):
+                finals[first + i] = (t, out["nhat_final"][0][i])
+    for a, (t_final, v) in finals.items():
+        assert t_final == a // S_ + k - 1
+        assert history[a][-1][0] == t_final and history[a][-1][1] == v     # last time it was touched
+
+
+def test_last_stride_mode_keeps_most_recent_samples(monkeypatch):
+    """'predicted segments keep only their most recent floor(fs/r) samples';
+    PAPER.md:186: with aggregation latency delta the kept span ends delta samples before the edge."""
+    W, S_, n_up = 40, 5, 20
+    preds = []
+
+    def fake(x, layers, prepared):
+        p = RNG.standard_normal(W); preds.append(p); return p
+
+    monkeypatch.setattr(oracle, "deepclean_forward", fake)
+    for delta in (0, 10):
+        preds.clear()
+        so = _stream_oracle(W, S_, n_up, agg=oracle.AGG_LAST_STRIDE, delta=delta)
+        x = RNG.standard_normal((2, n_up * S_)).astype(np.float32)
+        for t in range(n_up):
+            out = so.update(x[:, t * S_:(t + 1) * S_])
+            a0 = (t + 1) * S_ - S_ - delta
+            exp_n = preds[-1][W - S_ - delta:W - delta]
+            if a0 >= 0:
+                assert np.array_equal(out["nhat_final"][0], exp_n)
+                assert np.allclose(out["cleaned_final"][0], x[1, a0:a0 + S_].astype(np.float64) - exp_n, atol=1e-15)
+
+
+def test_subtraction_zero_network_returns_strain_bit_exact_and_bias_only_shifts():
+    cfg = S.config_c0()
+    st = cfg.stream
+    zero = [(np.zeros(l.wshape()), np.zeros(l.cout)) for l in cfg.dc_layers]
+    rows = [(st.witness_rows(0), st.strain_row(0))]
+    x = synth.white_channels(3, st.channels, 12 * st.stride)
+    so = oracle.StreamOracle(st.channels, st.window, st.stride, rows, [(cfg.dc_layers, zero)], max_updates=12)
+    cbias = 0.125
+    biased = [(w.copy(), b.copy()) for w, b in zero]
+    biased[-1][1][:] = cbias
+    so_b = oracle.StreamOracle(st.channels, st.window, st.stride, rows, [(cfg.dc_layers, biased)], max_updates=12)
+    for t in range(12):
+        new = x[:, t * st.stride:(t + 1) * st.stride]
+        out = so.update(new); outb = so_b.update(new)
+        first = out["first_index"]
+        lo = max(first, 0)
+        exp = x[st.strain_row(0), lo:first + st.window]
+        got = out["cleaned_running"][0][lo - first:]
+        assert np.array_equal(got.astype(np.float32).view(np.uint32), exp.view(np.uint32))
+        assert np.allclose(outb["cleaned_running"][0][lo - first:], exp.astype(np.float64) - cbias, atol=1e-15)
+
+
+# ------------------------------------------------------------------------------ classifier
+
+def test_all_zero_classifier_scores_one_half():
+    cfg = S.config_c2()
+    pc = [(np.zeros(l.wshape()), np.zeros(l.cout)) for l in cfg.bbh_convs]
+    pd = [(np.zeros((64, 128)), np.zeros(64)), (np.zeros((1, 64)), np.zeros(1))]
+    x = synth.bbh_windows(2, 2, 512)[0]
+    assert oracle.bbh_forward(x, cfg.bbh_convs, pc, pd) == 0.5
+
+
+def test_bbh_forward_matches_torch_float64_model():
+    cfg = S.config_c2()
+    cp, dp = synth.bbh_params(9, cfg.bbh_convs, cfg.bbh_dense)
+    pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    x = synth.bbh_windows(2, 2, 1024)[0].astype(np.float64)
+    score = oracle.bbh_forward(x, cfg.bbh_convs, pc, pd)
+    h = torch.from_numpy(x)[None]
+    for (w, b) in pc:
+        h = torch.nn.functional.pad(h, (3, 4))
+        h = torch.relu(torch.nn.functional.conv1d(h, torch.from_numpy(w), torch.from_numpy(b)))
+        h = torch.nn.functional.max_pool1d(h, 4)
+    assert h.shape == (1, 128, 16)
+    v = h.mean(dim=2)[0]
+    v = torch.relu(torch.from_numpy(pd[0][0]) @ v + torch.from_numpy(pd[0][1]))
+    z = torch.from_numpy(pd[1][0]) @ v + torch.from_numpy(pd[1][1])
+    assert score == pytest.approx(float(torch.sigmoid(z)[0]), abs=1e-13)
+    assert 0.0 < score < 1.0
+
+
+def test_classifier_window_reads_zero_before_stream_start():
+    """A12/D8: a classifier window reaching before a = 0 reads cleaned[a<0] = 0."""
+    cfg = S.config_small_ensemble(1)
+    st = cfg.stream
+    rows = [(st.witness_rows(d), st.strain_row(d)) for d in range(2)]
+    zero = [(np.zeros(l.wshape()), np.zeros(l.cout)) for l in cfg.dc_layers]
+    cp, dp = synth.bbh_params(1, cfg.bbh_convs, cfg.bbh_dense)
+    pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    so = oracle.StreamOracle(st.channels, st.window, st.stride, rows, [(cfg.dc_layers, zero)] * 2,
+                             (cfg.bbh_convs, pc, pd, cfg.bbh_len), max_updates=3)
+    x = synth.white_channels(4, st.channels, 3 * st.stride)
+    out = so.update(x[:, :st.stride])
+    xin = out["bbh_input"]
+    assert xin.shape == (2, cfg.bbh_len)
+    assert np.all(xin[:, :cfg.bbh_len - st.stride] == 0.0)
+    for d in range(2):
+        assert np.array_equal(xin[d, cfg.bbh_len - st.stride:].astype(np.float32), x[st.strain_row(d), :st.stride])
