@@ -1,0 +1,189 @@
+/*
+ * gwstream.h -- C ABI of the B200-native streaming inference engine for the hot path of
+ * arXiv:2108.12430 ("Hardware-accelerated Inference for Real-Time Gravitational-Wave Astronomy").
+ *
+ * The interface follows the paper's statement of the problem (section B.1):
+ *   "Inference requests are made to this model providing a floor(fs/r)-sized stream of strictly
+ *    new samples that are used to update the state to a new snapshot, which is then passed to
+ *    downstream static models."
+ * and the ensemble order of PAPER.md:76 (Fig. 4) / :212: snapshotter -> one DeepClean per detector
+ * -> aggregation + subtraction -> BBHnet on the cleaned strain of both detectors.
+ *
+ * Conventions
+ *  - Plain C, opaque handles, no exceptions.  Every call returns 0 (GW_OK) or a negative code;
+ *    gw_last_error() returns a thread-local description of the last failure on this thread.
+ *  - "dev" pointers are CUDA device pointers on the current device, "host" pointers are host
+ *    memory.  The caller owns every buffer it passes; the engine owns all persistent state (rings,
+ *    overlap-add accumulators, activations, weights -- parameters are COPIED at create time).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
+ *    enqueued on it and is asynchronous unless stated.  One handle is used from one host thread at
+ *    a time, and by one CUDA stream at a time.
+ *  - Per update the calls must come in this order:
+ *        gw_stream_update -> gw_deepclean_forward -> gw_cleaned_strain -> gw_bbh_score
+ *    (or one gw_step).  Anything else returns GW_ESTATE.  Results of update t are a pure function
+ *    of all samples through update t.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns GW_ECUDA.
+ *
+ * Layouts are row-major with the last index fastest, written [a][b][c].
+ * n = n_streams, C = channels, W = window, S = stride (both in samples), D = detectors.
+ */
+#ifndef GWSTREAM_H
+#define GWSTREAM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { GW_OK = 0, GW_EINVAL = -1, GW_ESTATE = -2, GW_ENOMEM = -3, GW_ECUDA = -4 };
+enum { GW_BF16 = 0, GW_FP16 = 1 };                       /* storage/multiply type; accumulation is fp32 */
+enum { GW_CONV = 0, GW_CONVT = 1 };                      /* Conv1d | ConvTranspose1d */
+enum { GW_ACT_NONE = 0, GW_ACT_TANH = 1, GW_ACT_RELU = 2 };
+enum { GW_FINAL = 0, GW_RUNNING = 1 };                   /* gw_cleaned_strain output selection */
+enum { GW_AGG_HANN_OLA = 0, GW_AGG_LAST_STRIDE = 1 };    /* aggregation of overlapping predictions */
+enum { GW_IMPL_UMMA = 0, GW_IMPL_SIMT = 1 };             /* conv GEMM implementation (SIMT = debug cross-check) */
+
+typedef struct gw_stream gw_stream;
+typedef struct gw_deepclean gw_deepclean;
+typedef struct gw_bbh gw_bbh;
+typedef struct gw_pipeline gw_pipeline;
+
+/* One convolution layer, parameters in HOST memory, fp32, unfolded.
+ *  kind GW_CONV : y[co][l] = b[co] + sum_ci sum_j w[co][ci][j] x[ci][stride*l + j - pad_l], zero
+ *                 padding pad_l / pad_r; w is [cout][cin][k].
+ *  kind GW_CONVT: the adjoint, y[co][m] = b[co] + sum_ci sum_{l,j: stride*l + j - pad_l = m}
+ *                 w[ci][co][j] x[ci][l]; pad_l = padding, pad_r = output_padding; w is [cin][cout][k].
+ *  BatchNorm (inference): if bn_gamma != NULL, z -> gamma (z - mean)/sqrt(var + eps) + beta is
+ *  applied between the convolution and the activation; it is folded into w and b in double
+ *  precision at create time (BASELINE.json configs[1]: "folded BatchNorm").
+ *  pool: MaxPool1d(pool, stride pool) after the activation (1 = none).
+ *  Supported by the tensor-core path: GW_CONV with k odd, stride 2, pad_l = pad_r = k/2 (DeepClean
+ *  encoder); GW_CONVT with k odd, stride 2, pad_l = k/2, pad_r = 1 (decoder); GW_CONV with stride 1,
+ *  pad_l + pad_r = k - 1, pool 4 (classifier).  Other shapes return GW_EINVAL. */
+typedef struct {
+    int kind, cin, cout, k, stride, pad_l, pad_r, act, pool;
+    const float *w, *b;
+    const float *bn_gamma, *bn_beta, *bn_mean, *bn_var;
+    float bn_eps;
+} gw_conv_layer;
+
+/* DeepClean stage: one network PER DETECTOR ("two DeepClean instances").
+ *  layers[d*n_layers + i] is layer i of detector d; the last layer must have cout = 1.
+ *  witness_rows[d*n_witness + c] / strain_row[d]: rows of the snapshot ring (one
+ *  snapshotter holds all data sources and hands slices to each model).
+ *  agg: GW_AGG_HANN_OLA (periodic-Hann overlap-add normalised by the summed window; needs
+ *  window % stride == 0 and window/stride >= 2) or GW_AGG_LAST_STRIDE (each
+ *  prediction keeps only its most recent `stride` samples).
+ *  delta: aggregation-latency offset in samples: the classifier window and the
+ *  LAST_STRIDE span end `delta` samples before the newest sample.  0 <= delta <= window - stride. */
+typedef struct {
+    int n_det, n_layers, n_witness;
+    const gw_conv_layer *layers;
+    const int *witness_rows;
+    const int *strain_row;
+    int agg, delta;
+} gw_dc_spec;
+
+/* BBH classifier: conv blocks (conv -> ReLU -> max-pool) on the D cleaned
+ * strains, global average pooling, dense layers (ReLU between, none after the last), sigmoid.
+ *  dense_w[i] is [dense_dims[i+1]][dense_dims[i]] fp32 host, dense_b[i] is [dense_dims[i+1]];
+ *  dense_dims[0] = cout of the last conv, dense_dims[n_dense] = 1.  n_dense must be 2.
+ *  length: classifier window L_b in samples (multiple of 64, <= 4096 and <= window). */
+typedef struct {
+    int n_convs;
+    const gw_conv_layer *convs;
+    int n_dense;
+    const int *dense_dims;
+    const float *const *dense_w;
+    const float *const *dense_b;
+    int length;
+} gw_bbh_spec;
+
+const char *gw_last_error(void);
+
+/* Number of CUDA kernels this library has launched (or captured into a graph and replayed) on
+ * behalf of the calling process so far; used by bench.py for "gpu_launches". */
+int64_t gw_kernel_launches(void);
+
+/* Select the conv GEMM implementation for handles created AFTER this call.  GW_IMPL_UMMA
+ * (default): tcgen05/TMEM/TMA.  GW_IMPL_SIMT: a slow CUDA-core kernel over the same operand
+ * layout, kept only to bisect tensor-core bugs in tests.  Both are CUDA; neither is a fallback. */
+int gw_set_conv_impl(int impl);
+
+/* ---- snapshotter -------------------------------------------------------------
+ * gw_stream_create: zeroed ring state [n][C][W] fp32 on the current device, sample counter 0.
+ *   Requires n >= 1, C >= 1, fs >= 1, 1 <= S <= W.
+ * gw_stream_update: new_samples_dev is [n][C][S] fp32, strictly new samples; appends them and
+ *   advances the counter by S.  128-bit path when S % 4 == 0 and W % 4 == 0, scalar otherwise.
+ * gw_stream_snapshot (test hook): writes the time-ordered snapshot [n][C][W] to out_dev and, if
+ *   first_index_host != NULL, the absolute index (t+1)S - W of its first sample (negative during
+ *   warm-up; samples before the stream start read as 0).  Synchronises `stream`.
+ * gw_stream_count: samples per channel appended so far (host-side mirror of the device counter). */
+int gw_stream_create(gw_stream **out, int n_streams, int channels, int fs, int window, int stride);
+int gw_stream_destroy(gw_stream *s);
+int gw_stream_update(gw_stream *s, const float *new_samples_dev, void *stream);
+int gw_stream_snapshot(gw_stream *s, float *out_dev, int64_t *first_index_host, void *stream);
+int64_t gw_stream_count(const gw_stream *s);
+
+/* ---- DeepClean ------------------------------------------------------------------
+ * gw_deepclean_create: folds BatchNorm, rounds weights RN-even to `dtype`, builds the GEMM
+ *   operands and TMA descriptors, allocates activations and aggregation state.  The stream must
+ *   outlive the handle.  Must be created before the stream's first update.
+ * gw_deepclean_forward: gathers the current window of every (stream, detector), converts it to
+ *   `dtype` channels-last, runs all layers; the raw prediction p_t [n][D][W] fp32 stays inside.
+ * gw_deepclean_noise (test hook): copies p_t to out_dev [n][D][W].
+ * gw_cleaned_strain: aggregates p_t into the running noise estimate (Hann overlap-add + window
+ *   normalisation, or LAST_STRIDE), subtracts it from the strain and writes to out_dev
+ *   (may be NULL):  GW_FINAL   -> [n][D][S], the S samples that became final with this update
+ *                                 (absolute index (t+1)S - W ...; LAST_STRIDE: (t+1)S - S - delta ...)
+ *                   GW_RUNNING -> [n][D][W], the running-normalised cleaned window.
+ *   Samples with negative absolute index are written as 0.
+ * gw_noise_estimate (test hook): the running noise estimate nhat over the current window,
+ *   [n][D][W] (0 where no prediction covers the sample).  Valid after gw_cleaned_strain. */
+int gw_deepclean_create(gw_deepclean **out, gw_stream *s, const gw_dc_spec *spec, int dtype);
+int gw_deepclean_destroy(gw_deepclean *dc);
+int gw_deepclean_forward(gw_deepclean *dc, void *stream);
+int gw_deepclean_noise(gw_deepclean *dc, float *out_dev, void *stream);
+int gw_cleaned_strain(gw_deepclean *dc, float *out_dev, int mode, void *stream);
+int gw_noise_estimate(gw_deepclean *dc, float *out_dev, void *stream);
+/* test hook: copy the activations after layer `layer` (0-based) as stored, 16-bit channels-last
+ * [n][D][L_layer][C_padded]; *rows / *cols (host, may be NULL) receive L_layer and C_padded. */
+int gw_deepclean_activation(gw_deepclean *dc, int layer, void *out_dev, int64_t out_bytes,
+                            int *rows, int *cols, void *stream);
+
+/* ---- BBH classifier ---------------------------------------------------------------
+ * gw_bbh_create: dc may be NULL for a stateless batch classifier (gw_bbh_score_batch only), in
+ *   which case n_det detectors and max_batch windows are assumed.
+ * gw_bbh_score: scores_dev [n] fp32 in (0,1), on the window
+ *   [(t+1)S - delta - L_b, (t+1)S - delta) of the running cleaned strain of this update.
+ * gw_bbh_score_batch: stateless; windows_dev [B][D][L_b] fp32, scores_dev [B]; B <= max_batch. */
+int gw_bbh_create(gw_bbh **out, gw_deepclean *dc, const gw_bbh_spec *spec, int dtype, int n_det,
+                  int max_batch);
+int gw_bbh_destroy(gw_bbh *b);
+int gw_bbh_score(gw_bbh *b, float *scores_dev, void *stream);
+int gw_bbh_score_batch(gw_bbh *b, const float *windows_dev, int batch, float *scores_dev, void *stream);
+
+/* ---- one update as one CUDA-graph replay (north_star (5)) ----------------------------------------
+ * gw_pipeline_create: ties the three stages (bbh may be NULL).  The first gw_step captures
+ *   update -> forward -> cleaned(GW_FINAL) -> score into a CUDA graph; later steps replay it (the ring
+ *   head lives in device memory, so the graph is replayed unchanged).
+ * gw_step: device buffers.  new_samples_dev [n][C][S]; scores_dev [n] (ignored without bbh);
+ *   cleaned_final_dev [n][D][S].  The three pointers must be the same on every call of one
+ *   pipeline (they are baked into the graph); otherwise GW_EINVAL.
+ * gw_step_host: HOST buffers; copies new samples host->device, replays the graph, copies scores
+ *   and final cleaned samples device->host, and synchronises.  Pinned host memory makes the copies
+ *   asynchronous; pageable memory works but is slower. */
+int gw_pipeline_create(gw_pipeline **out, gw_stream *s, gw_deepclean *dc, gw_bbh *bbh);
+int gw_pipeline_destroy(gw_pipeline *p);
+int gw_step(gw_pipeline *p, const float *new_samples_dev, float *scores_dev, float *cleaned_final_dev,
+            void *stream);
+int gw_step_host(gw_pipeline *p, const float *new_samples_host, float *scores_host,
+                 float *cleaned_final_host, void *stream);
+/* number of kernel nodes in the captured graph (0 before the first gw_step) */
+int gw_pipeline_graph_nodes(const gw_pipeline *p);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWSTREAM_H */

@@ -226,13 +226,24 @@ def conv_layer(x, layer, w, b) -> np.ndarray:
     return y
 
 
-def deepclean_forward(x, layers: Sequence, prepared: Sequence, return_all: bool = False):
+def deepclean_forward(x, layers: Sequence, prepared: Sequence, return_all: bool = False,
+                      act_dtype: Optional[int] = None):
     """x [n_witness][W] -> predicted noise p [W] (DeepClean takes the witness
-    channels and predicts the noise in the strain).  prepared[i] = prepare_conv(layers[i], ...)."""
+    channels and predicts the noise in the strain).  prepared[i] = prepare_conv(layers[i], ...).
+
+    act_dtype (DIAGNOSTIC ONLY, not the oracle of record): when given, the input and every
+    inter-layer activation are rounded RN-even to that storage type, i.e. the result an exact
+    machine would get if it had to store activations in 16 bits.  It separates the storage
+    rounding that any 16-bit implementation must incur from implementation error (DESIGN.md,
+    "Error budget")."""
     h = _d(x)
+    if act_dtype is not None:
+        h = round_storage(h, act_dtype)
     acts = []
-    for layer, (w, b) in zip(layers, prepared):
+    for i, (layer, (w, b)) in enumerate(zip(layers, prepared)):
         h = conv_layer(h, layer, w, b)
+        if act_dtype is not None and i < len(layers) - 1:
+            h = round_storage(h, act_dtype)
         if return_all:
             acts.append(h)
     assert h.shape[0] == 1

@@ -1,0 +1,345 @@
+"""Thin ctypes binding over libgwstream.so (include/gwstream.h).  Argument marshalling only:
+every step of the path runs in the library's CUDA kernels.  torch is used for device memory and
+streams.  There is no fallback: if the library (or a CUDA device) is missing, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Sequence
+
+import numpy as np
+
+from . import specs as S
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgwstream.so")
+
+GW_OK, GW_EINVAL, GW_ESTATE, GW_ENOMEM, GW_ECUDA = 0, -1, -2, -3, -4
+GW_BF16, GW_FP16 = 0, 1
+GW_FINAL, GW_RUNNING = 0, 1
+GW_IMPL_UMMA, GW_IMPL_SIMT = 0, 1
+
+EXPORTS = [
+    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl",
+    "gw_stream_create", "gw_stream_destroy", "gw_stream_update", "gw_stream_snapshot", "gw_stream_count",
+    "gw_deepclean_create", "gw_deepclean_destroy", "gw_deepclean_forward", "gw_deepclean_noise",
+    "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
+    "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
+    "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_pipeline_graph_nodes",
+]
+
+_FP = C.POINTER(C.c_float)
+
+
+class _ConvLayer(C.Structure):
+    _fields_ = [("kind", C.c_int), ("cin", C.c_int), ("cout", C.c_int), ("k", C.c_int), ("stride", C.c_int),
+                ("pad_l", C.c_int), ("pad_r", C.c_int), ("act", C.c_int), ("pool", C.c_int),
+                ("w", _FP), ("b", _FP), ("bn_gamma", _FP), ("bn_beta", _FP), ("bn_mean", _FP), ("bn_var", _FP),
+                ("bn_eps", C.c_float)]
+
+
+class _DcSpec(C.Structure):
+    _fields_ = [("n_det", C.c_int), ("n_layers", C.c_int), ("n_witness", C.c_int),
+                ("layers", C.POINTER(_ConvLayer)), ("witness_rows", C.POINTER(C.c_int)),
+                ("strain_row", C.POINTER(C.c_int)), ("agg", C.c_int), ("delta", C.c_int)]
+
+
+class _BbhSpec(C.Structure):
+    _fields_ = [("n_convs", C.c_int), ("convs", C.POINTER(_ConvLayer)), ("n_dense", C.c_int),
+                ("dense_dims", C.POINTER(C.c_int)), ("dense_w", C.POINTER(_FP)), ("dense_b", C.POINTER(_FP)),
+                ("length", C.c_int)]
+
+
+class GwError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"gwstream error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libgwstream.so; raises (loudly) when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2108_12430_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i, i64 = C.c_void_p, C.c_int, C.c_int64
+        L.gw_last_error.restype = C.c_char_p
+        L.gw_kernel_launches.restype = i64
+        L.gw_set_conv_impl.argtypes = [i]
+        L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
+        L.gw_stream_destroy.argtypes = [vp]
+        L.gw_stream_update.argtypes = [vp, vp, vp]
+        L.gw_stream_snapshot.argtypes = [vp, vp, C.POINTER(i64), vp]
+        L.gw_stream_count.argtypes = [vp]
+        L.gw_stream_count.restype = i64
+        L.gw_deepclean_create.argtypes = [C.POINTER(vp), vp, C.POINTER(_DcSpec), i]
+        L.gw_deepclean_destroy.argtypes = [vp]
+        L.gw_deepclean_forward.argtypes = [vp, vp]
+        L.gw_deepclean_noise.argtypes = [vp, vp, vp]
+        L.gw_cleaned_strain.argtypes = [vp, vp, i, vp]
+        L.gw_noise_estimate.argtypes = [vp, vp, vp]
+        L.gw_deepclean_activation.argtypes = [vp, i, vp, i64, C.POINTER(i), C.POINTER(i), vp]
+        L.gw_bbh_create.argtypes = [C.POINTER(vp), vp, C.POINTER(_BbhSpec), i, i, i]
+        L.gw_bbh_destroy.argtypes = [vp]
+        L.gw_bbh_score.argtypes = [vp, vp, vp]
+        L.gw_bbh_score_batch.argtypes = [vp, vp, i, vp, vp]
+        L.gw_pipeline_create.argtypes = [C.POINTER(vp), vp, vp, vp]
+        L.gw_pipeline_destroy.argtypes = [vp]
+        L.gw_step.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_step_host.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_pipeline_graph_nodes.argtypes = [vp]
+        _lib = L
+    return _lib
+
+
+def _check(rc: int) -> None:
+    if rc != GW_OK:
+        raise GwError(rc, lib().gw_last_error().decode())
+
+
+def kernel_launches() -> int:
+    return int(lib().gw_kernel_launches())
+
+
+def set_conv_impl(impl: int) -> None:
+    _check(lib().gw_set_conv_impl(impl))
+
+
+def _fp(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(_FP)
+
+
+def _stream_ptr(stream) -> C.c_void_p:
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _ptr(t) -> C.c_void_p:
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _marshal_layers(layer_specs: Sequence[S.ConvSpec], params: Sequence[Dict[str, np.ndarray]], keep: list):
+    arr = (_ConvLayer * len(layer_specs))()
+    for i, (l, p) in enumerate(zip(layer_specs, params)):
+        w = np.ascontiguousarray(p["w"], dtype=np.float32)
+        b = np.ascontiguousarray(p["b"], dtype=np.float32)
+        assert w.shape == l.wshape(), (w.shape, l.wshape())
+        keep += [w, b]
+        a = arr[i]
+        a.kind, a.cin, a.cout, a.k, a.stride = l.kind, l.cin, l.cout, l.k, l.stride
+        a.pad_l, a.pad_r, a.act, a.pool = l.pad_l, l.pad_r, l.act, l.pool
+        a.w, a.b = _fp(w), _fp(b)
+        if l.bn:
+            bn = [np.ascontiguousarray(p[k], dtype=np.float32) for k in ("bn_gamma", "bn_beta", "bn_mean", "bn_var")]
+            keep += bn
+            a.bn_gamma, a.bn_beta, a.bn_mean, a.bn_var = (_fp(x) for x in bn)
+            a.bn_eps = float(p["bn_eps"])
+    return arr
+
+
+class Stream:
+    """Snapshotter state for n independent streams."""
+
+    def __init__(self, spec: S.StreamSpec):
+        self.spec = spec
+        self.h = C.c_void_p()
+        _check(lib().gw_stream_create(C.byref(self.h), spec.n_streams, spec.channels, spec.fs, spec.window, spec.stride))
+
+    def update(self, new_samples, stream=None) -> None:
+        """new_samples: CUDA float32 tensor [n][C][S], contiguous."""
+        sp = self.spec
+        assert new_samples.is_cuda and new_samples.is_contiguous() and new_samples.dtype.is_floating_point
+        assert tuple(new_samples.shape) == (sp.n_streams, sp.channels, sp.stride), tuple(new_samples.shape)
+        _check(lib().gw_stream_update(self.h, _ptr(new_samples), _stream_ptr(stream)))
+
+    def snapshot(self, stream=None):
+        import torch
+        sp = self.spec
+        out = torch.empty((sp.n_streams, sp.channels, sp.window), dtype=torch.float32, device="cuda")
+        first = C.c_int64(0)
+        _check(lib().gw_stream_snapshot(self.h, _ptr(out), C.byref(first), _stream_ptr(stream)))
+        return out, int(first.value)
+
+    def count(self) -> int:
+        return int(lib().gw_stream_count(self.h))
+
+    def close(self) -> None:
+        if self.h:
+            lib().gw_stream_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class DeepClean:
+    """One DeepClean network per detector over a Stream."""
+
+    def __init__(self, stream: Stream, layers: Sequence[S.ConvSpec], params_per_det: Sequence[Sequence[Dict]],
+                 dtype: int = GW_BF16, agg: int = S.AGG_HANN_OLA, delta: int = 0):
+        sp = stream.spec
+        self.stream, self.layers, self.dtype = stream, list(layers), dtype
+        keep: list = []
+        n_det = len(params_per_det)
+        assert n_det == sp.n_det
+        flat_specs = list(layers) * n_det
+        flat_params = [p for det in params_per_det for p in det]
+        arr = _marshal_layers(flat_specs, flat_params, keep)
+        wit = (C.c_int * (n_det * sp.n_witness))(*[r for d in range(n_det) for r in sp.witness_rows(d)])
+        srow = (C.c_int * n_det)(*[sp.strain_row(d) for d in range(n_det)])
+        spec = _DcSpec(n_det, len(layers), sp.n_witness, arr, wit, srow, agg, delta)
+        self.h = C.c_void_p()
+        _check(lib().gw_deepclean_create(C.byref(self.h), stream.h, C.byref(spec), dtype))
+
+    def forward(self, stream=None) -> None:
+        _check(lib().gw_deepclean_forward(self.h, _stream_ptr(stream)))
+
+    def noise(self, stream=None):
+        import torch
+        sp = self.stream.spec
+        out = torch.empty((sp.n_streams, sp.n_det, sp.window), dtype=torch.float32, device="cuda")
+        _check(lib().gw_deepclean_noise(self.h, _ptr(out), _stream_ptr(stream)))
+        return out
+
+    def cleaned(self, mode: int = GW_FINAL, stream=None):
+        import torch
+        sp = self.stream.spec
+        n = sp.stride if mode == GW_FINAL else sp.window
+        out = torch.empty((sp.n_streams, sp.n_det, n), dtype=torch.float32, device="cuda")
+        _check(lib().gw_cleaned_strain(self.h, _ptr(out), mode, _stream_ptr(stream)))
+        return out
+
+    def noise_estimate(self, stream=None):
+        import torch
+        sp = self.stream.spec
+        out = torch.empty((sp.n_streams, sp.n_det, sp.window), dtype=torch.float32, device="cuda")
+        _check(lib().gw_noise_estimate(self.h, _ptr(out), _stream_ptr(stream)))
+        return out
+
+    def activation(self, layer: int, stream=None):
+        """Stored activations after `layer` (-1 = the gathered window): [n][D][L][C_padded], 16-bit."""
+        import torch
+        sp = self.stream.spec
+        rows, cols = C.c_int(0), C.c_int(0)
+        _check(lib().gw_deepclean_activation(self.h, layer, None, 0, C.byref(rows), C.byref(cols), _stream_ptr(stream)))
+        tdt = torch.bfloat16 if self.dtype == GW_BF16 else torch.float16
+        out = torch.empty((sp.n_streams, sp.n_det, rows.value, cols.value), dtype=tdt, device="cuda")
+        _check(lib().gw_deepclean_activation(self.h, layer, _ptr(out), out.numel() * 2, None, None, _stream_ptr(stream)))
+        return out
+
+    def close(self) -> None:
+        if self.h:
+            lib().gw_deepclean_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Bbh:
+    """BBH classifier, attached to a DeepClean stage or stateless."""
+
+    def __init__(self, dc: Optional[DeepClean], convs: Sequence[S.ConvSpec], conv_params, dense_params,
+                 length: int, dtype: int = GW_BF16, n_det: int = 2, max_batch: int = 256):
+        keep: list = []
+        arr = _marshal_layers(convs, conv_params, keep)
+        dims = [dense_params[0]["w"].shape[1]] + [p["w"].shape[0] for p in dense_params]
+        dims_c = (C.c_int * len(dims))(*dims)
+        ws = [np.ascontiguousarray(p["w"], dtype=np.float32) for p in dense_params]
+        bs = [np.ascontiguousarray(p["b"], dtype=np.float32) for p in dense_params]
+        keep += ws + bs
+        w_c = (_FP * len(ws))(*[_fp(w) for w in ws])
+        b_c = (_FP * len(bs))(*[_fp(b) for b in bs])
+        spec = _BbhSpec(len(convs), arr, len(dense_params), dims_c, w_c, b_c, length)
+        self.dc, self.length, self.n_det, self.max_batch = dc, length, n_det, max_batch
+        self.h = C.c_void_p()
+        _check(lib().gw_bbh_create(C.byref(self.h), dc.h if dc is not None else None, C.byref(spec), dtype,
+                                   n_det, max_batch))
+
+    def score(self, stream=None):
+        import torch
+        out = torch.empty((self.dc.stream.spec.n_streams,), dtype=torch.float32, device="cuda")
+        _check(lib().gw_bbh_score(self.h, _ptr(out), _stream_ptr(stream)))
+        return out
+
+    def score_batch(self, windows, stream=None):
+        import torch
+        assert windows.is_cuda and windows.is_contiguous() and windows.dtype == torch.float32
+        B = windows.shape[0]
+        assert tuple(windows.shape[1:]) == (self.n_det, self.length)
+        out = torch.empty((B,), dtype=torch.float32, device="cuda")
+        _check(lib().gw_bbh_score_batch(self.h, _ptr(windows), B, _ptr(out), _stream_ptr(stream)))
+        return out
+
+    def close(self) -> None:
+        if self.h:
+            lib().gw_bbh_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Pipeline:
+    """update -> forward -> cleaned -> score as one CUDA-graph replay per stride."""
+
+    def __init__(self, stream: Stream, dc: DeepClean, bbh: Optional[Bbh]):
+        self.stream, self.dc, self.bbh = stream, dc, bbh
+        self.h = C.c_void_p()
+        _check(lib().gw_pipeline_create(C.byref(self.h), stream.h, dc.h, bbh.h if bbh is not None else None))
+
+    def step(self, new_samples, scores, cleaned_final, stream=None) -> None:
+        """All CUDA float32 tensors: new [n][C][S], scores [n], cleaned_final [n][D][S]."""
+        _check(lib().gw_step(self.h, _ptr(new_samples), _ptr(scores), _ptr(cleaned_final), _stream_ptr(stream)))
+
+    def step_host(self, new_samples, scores, cleaned_final, stream=None) -> None:
+        """Host tensors / numpy float32 arrays (pinned for asynchronous copies)."""
+        def hp(a):
+            if a is None:
+                return C.c_void_p(0)
+            return C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
+        _check(lib().gw_step_host(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)))
+
+    def graph_nodes(self) -> int:
+        return int(lib().gw_pipeline_graph_nodes(self.h))
+
+    def close(self) -> None:
+        if self.h:
+            lib().gw_pipeline_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def build_ensemble(cfg: S.Config, dc_params_per_det, bbh_params=None, dtype: int = GW_BF16,
+                   agg: int = S.AGG_HANN_OLA, delta: int = 0):
+    """Convenience: Stream + DeepClean (+ Bbh) + Pipeline for a specs.Config."""
+    st = Stream(cfg.stream)
+    dc = DeepClean(st, cfg.dc_layers, dc_params_per_det, dtype, agg, delta)
+    bbh = None
+    if bbh_params is not None:
+        cp, dp = bbh_params
+        bbh = Bbh(dc, cfg.bbh_convs, cp, dp, cfg.bbh_len, dtype)
+    pipe = Pipeline(st, dc, bbh)
+    return st, dc, bbh, pipe

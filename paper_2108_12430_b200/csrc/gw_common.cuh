@@ -1,0 +1,85 @@
+// gw_common.cuh -- shared declarations of the CUDA path (engine-internal, not part of the ABI).
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gw {
+
+constexpr int kMaxSeg = 48;        // K segments (64 elements each) per conv GEMM
+constexpr int kTileM = 128;        // UMMA M: one TMEM lane per output row
+constexpr int kSegK = 64;          // 64 x 16-bit = one 128-byte swizzle row
+
+enum { FMT_FP16 = 0, FMT_BF16 = 1 };                       // UMMA instruction-descriptor encoding
+enum { EPI_STORE = 0, EPI_POOL = 1, EPI_POOL_HEAD = 2 };
+enum { ACT_NONE = 0, ACT_TANH = 1, ACT_RELU = 2 };
+
+// One convolution layer expressed as   D[m][n] = sum_s  A[m + shift_s][col_s .. col_s+64) . B[n][64 s .. 64 s+64)
+// where A is a 2-D view [rows][cols] of a channels-last activation tensor per batch item (rows out
+// of range read as zero = the layer's zero padding) and B is the per-detector weight matrix.
+struct ConvGemmParams {
+    CUtensorMap tmA;               // 3-D (cols, rows, batch), box (64, 128, 1), SWIZZLE_128B
+    CUtensorMap tmB;               // 3-D (K = 64 n_seg, N, n_det), box (64, N, 1), SWIZZLE_128B
+    const void* A;                 // raw pointers of the same operands (SIMT cross-check kernel)
+    const void* B;
+    int a_rows, a_cols;            // A view per batch item
+    int M;                         // output rows per batch item
+    int N;                         // GEMM N, multiple of 32, <= 256
+    int n_seg;
+    int n_det;                     // weight set = batch % n_det
+    int fmt;                       // FMT_*
+    int epi, act;
+    const float* bias;             // [n_det][N]
+    void* out;                     // EPI_STORE: [batch][M][N]; EPI_POOL: [batch][M/2][N/2], 16-bit
+    // EPI_POOL_HEAD: global average pool over the M/2 pooled rows, dense head, sigmoid
+    const float *hw1, *hb1, *hw2, *hb2;   // [hidden][N/2], [hidden], [hidden], [1]
+    int head_hidden;
+    float* scores;                 // [batch]
+    float* pooled_dbg;             // optional [batch][M/2][N/2] fp32 (SIMT path scratch)
+    int8_t seg_shift[kMaxSeg];
+    int16_t seg_col[kMaxSeg];
+};
+
+struct GemmLaunch {
+    ConvGemmParams p;
+    int batch;
+    int stages;
+    int smem_bytes;
+};
+
+void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st);
+void launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st);
+int conv_gemm_smem_bytes(int N, int stages);
+cudaError_t conv_gemm_prepare();   // opt-in shared-memory attribute
+
+// ---- bandwidth / CUDA-core kernels (gw_kernels.cu) -------------------------------------------
+void launch_append(float* ring, const float* new_samples, long long* count, unsigned* ticket, int n_rows,
+                   int W, int S, cudaStream_t st);
+void launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st);
+void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
+                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st);
+void launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
+                        int L, int cpad, int K, int pad, int fmt, cudaStream_t st);
+struct AggParams {
+    const float* pred;         // [n][D][W]
+    float* acc;                // [n][D][W] ring over absolute index mod W
+    const float* ring;         // snapshot ring [n][C][W]
+    const long long* count;
+    const int* strain_rows;    // [D]
+    const float* hann;         // [W]
+    const float* inv_wsum;     // [W]  1 / sum of the Hann weights covering window position n
+    float* final_out;          // [n][D][S] or null
+    float* running_out;        // [n][D][W] or null
+    float* nhat_out;           // [n][D][W] or null (test hook)
+    float* clf_in;             // [n][D][Lb] or null
+    int n_streams, n_det, channels, W, S, Lb, delta, agg;
+};
+void launch_aggregate(const AggParams& a, cudaStream_t st);
+void launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
+                      int cout, int cpad, int K, int pad_l, int pool, int fmt, cudaStream_t st);
+
+extern long long g_kernel_launches;
+
+}  // namespace gw

@@ -1,0 +1,858 @@
+// gw_engine.cu -- host side of libgwstream: the C ABI of include/gwstream.h, parameter preparation
+// (BatchNorm fold, rounding to the storage type, GEMM operand construction), TMA descriptors, the
+// per-update launch sequence and its CUDA-graph capture.  No arithmetic of the per-update path runs on
+// the host; everything here is one-time setup or launch plumbing.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/gwstream.h"
+#include "gw_common.cuh"
+
+using namespace gw;
+
+// ------------------------------------------------------------------------------------ errors
+static thread_local std::string g_err;
+static int g_conv_impl = GW_IMPL_UMMA;
+
+static int fail(int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+#define CU_TRY(expr)                                                                              \
+    do {                                                                                          \
+        cudaError_t _e = (expr);                                                                  \
+        if (_e != cudaSuccess)                                                                    \
+            return fail(_e == cudaErrorMemoryAllocation ? GW_ENOMEM : GW_ECUDA, "%s: %s", #expr,  \
+                        cudaGetErrorString(_e));                                                  \
+    } while (0)
+
+extern "C" const char* gw_last_error(void) { return g_err.c_str(); }
+extern "C" int64_t gw_kernel_launches(void) { return g_kernel_launches; }
+extern "C" int gw_set_conv_impl(int impl) {
+    if (impl != GW_IMPL_UMMA && impl != GW_IMPL_SIMT) return fail(GW_EINVAL, "unknown conv impl %d", impl);
+    g_conv_impl = impl;
+    return GW_OK;
+}
+
+static int check_device() {
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n == 0) return fail(GW_ECUDA, "no CUDA device (%s); gwstream has no CPU fallback",
+                                                cudaGetErrorString(e));
+    return GW_OK;
+}
+
+// ------------------------------------------------------------------------- TMA descriptor encode
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static PFN_encodeTiled g_encode = nullptr;
+
+static int get_encode() {
+    if (g_encode) return GW_OK;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess || fn == nullptr || qres != cudaDriverEntryPointSuccess)
+        return fail(GW_ECUDA, "cuTensorMapEncodeTiled not available: %s", cudaGetErrorString(e));
+    g_encode = reinterpret_cast<PFN_encodeTiled>(fn);
+    return GW_OK;
+}
+
+// 3-D tensor of 16-bit elements, dims (d0 fastest, d1, d2), strides in elements, box (64, box1, 1), 128B swizzle.
+static int make_tmap(CUtensorMap* tm, const void* base, int fmt, uint64_t d0, uint64_t d1, uint64_t d2,
+                     uint64_t stride1, uint64_t stride2, uint32_t box1) {
+    if (int rc = get_encode()) return rc;
+    cuuint64_t dims[3] = {d0, d1, d2};
+    cuuint64_t strides[2] = {stride1 * 2, stride2 * 2};
+    cuuint32_t box[3] = {static_cast<cuuint32_t>(kSegK), box1, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = g_encode(tm, fmt == FMT_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3,
+                          const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(GW_ECUDA, "cuTensorMapEncodeTiled failed (%d) dims %llu,%llu,%llu", (int)r,
+                                       (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)d2);
+    return GW_OK;
+}
+
+// --------------------------------------------------------------------- storage-type rounding (host)
+// Round a double straight to the 16-bit storage grid, nearest-even, and return the 16-bit pattern.
+// p = significand bits incl. the hidden one, emin = smallest normal exponent.
+static uint16_t to_storage_bits(double v, int fmt) {
+    const int p = fmt == FMT_BF16 ? 8 : 11;
+    const int emin = fmt == FMT_BF16 ? -126 : -14;
+    float f;
+    if (v == 0.0 || !isfinite(v)) {
+        f = static_cast<float>(v);
+    } else {
+        int e = ilogb(v);
+        if (e < emin) e = emin;
+        const int sh = e - (p - 1);                   // exponent of one unit in the last place
+        const double q = scalbn(v, -sh);              // exact
+        double fl = floor(q);
+        const double diff = q - fl;
+        if (diff > 0.5 || (diff == 0.5 && fmod(fl, 2.0) != 0.0)) fl += 1.0;
+        f = static_cast<float>(scalbn(fl, sh));       // exactly representable in float
+    }
+    if (fmt == FMT_BF16) {
+        uint32_t u;
+        memcpy(&u, &f, 4);
+        return static_cast<uint16_t>(u >> 16);        // low 16 bits are zero by construction
+    }
+    __half h = __float2half_rn(f);                    // exact: f is on the fp16 grid (or overflows to inf)
+    uint16_t b;
+    memcpy(&b, &h, 2);
+    return b;
+}
+static double storage_to_double(uint16_t b, int fmt) {
+    if (fmt == FMT_BF16) {
+        uint32_t u = static_cast<uint32_t>(b) << 16;
+        float f;
+        memcpy(&f, &u, 4);
+        return f;
+    }
+    __half h;
+    memcpy(&h, &b, 2);
+    return __half2float(h);
+}
+
+// ------------------------------------------------------------------------------ folded host layer
+struct HostLayer {
+    int kind, cin, cout, k, stride, pad_l, pad_r, act, pool;
+    std::vector<double> w, b;                        // BatchNorm folded, double
+    double W(int o, int i, int j) const {            // weight connecting input channel i to output channel o, tap j
+        return kind == GW_CONV ? w[(static_cast<size_t>(o) * cin + i) * k + j] : w[(static_cast<size_t>(i) * cout + o) * k + j];
+    }
+};
+
+static int fold_layer(const gw_conv_layer& L, HostLayer& H) {
+    if (L.cin < 1 || L.cout < 1 || L.k < 1 || L.k > 9 || !L.w || !L.b) return fail(GW_EINVAL, "bad conv layer");
+    H.kind = L.kind; H.cin = L.cin; H.cout = L.cout; H.k = L.k; H.stride = L.stride;
+    H.pad_l = L.pad_l; H.pad_r = L.pad_r; H.act = L.act; H.pool = L.pool < 1 ? 1 : L.pool;
+    const size_t nw = static_cast<size_t>(L.cin) * L.cout * L.k;
+    H.w.resize(nw); H.b.resize(L.cout);
+    for (size_t i = 0; i < nw; ++i) H.w[i] = L.w[i];
+    for (int c = 0; c < L.cout; ++c) H.b[c] = L.b[c];
+    if (L.bn_gamma) {
+        if (!L.bn_beta || !L.bn_mean || !L.bn_var) return fail(GW_EINVAL, "incomplete BatchNorm parameters");
+        for (int co = 0; co < L.cout; ++co) {
+            const double g = static_cast<double>(L.bn_gamma[co]) / sqrt(static_cast<double>(L.bn_var[co]) + static_cast<double>(L.bn_eps));
+            for (int ci = 0; ci < L.cin; ++ci)
+                for (int j = 0; j < L.k; ++j) {
+                    const size_t idx = L.kind == GW_CONV ? (static_cast<size_t>(co) * L.cin + ci) * L.k + j
+                                                         : (static_cast<size_t>(ci) * L.cout + co) * L.k + j;
+                    H.w[idx] *= g;
+                }
+            H.b[co] = (H.b[co] - static_cast<double>(L.bn_mean[co])) * g + static_cast<double>(L.bn_beta[co]);
+        }
+    }
+    return GW_OK;
+}
+
+static int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// ------------------------------------------------------------------------------------ handles
+struct gw_stream {
+    int n, C, fs, W, S;
+    float* ring = nullptr;
+    long long* d_count = nullptr;
+    unsigned* d_ticket = nullptr;
+    int64_t updates = 0;
+    gw_deepclean* dc = nullptr;
+};
+
+enum GemmKind { GK_ENC, GK_DEC, GK_BBH };
+
+struct GemmLayer {
+    GemmLaunch g;
+    void* d_B = nullptr;
+    float* d_bias = nullptr;
+    int impl = GW_IMPL_UMMA;
+};
+
+struct gw_deepclean {
+    gw_stream* s = nullptr;
+    int n_det = 0, n_layers = 0, n_wit = 0, agg = 0, delta = 0, fmt = FMT_BF16;
+    int batch = 0;
+    std::vector<HostLayer> host;                 // [n_det * n_layers]
+    std::vector<GemmLayer> gemm;                 // layers 0 .. n_layers-2
+    std::vector<void*> act;                      // act[0] = gathered window, act[i+1] = output of layer i
+    std::vector<int> act_rows, act_cols;
+    float* d_wt_final = nullptr;                 // [n_det][K][cpad]
+    float* d_b_final = nullptr;                  // [n_det]
+    int final_K = 0, final_pad = 0, final_cpad = 0, final_L = 0;
+    float* pred = nullptr;                       // [batch][W]
+    float* acc = nullptr;                        // [batch][W]
+    float* nhat = nullptr;                       // [batch][W] (test hook, allocated lazily)
+    float* d_hann = nullptr;
+    float* d_inv_wsum = nullptr;
+    int* d_rows_map = nullptr;
+    int* d_strain_rows = nullptr;
+    float* final_buf = nullptr;                  // [batch][S]
+    float* clf_in = nullptr;                     // owned by the attached gw_bbh
+    int Lb = 0;
+    gw_bbh* bbh = nullptr;
+    int64_t forward_for = 0, cleaned_for = 0;
+};
+
+struct gw_bbh {
+    gw_deepclean* dc = nullptr;
+    int n_det = 0, batch = 0, fmt = FMT_BF16, L = 0;
+    HostLayer c1;
+    float* d_w1 = nullptr;                       // first conv, fp32 (rounded to the storage grid)
+    float* d_b1 = nullptr;
+    int c1_cpad = 0;
+    std::vector<GemmLayer> gemm;
+    std::vector<void*> act;
+    float* in_buf = nullptr;                     // [batch][n_det][L]
+    float *d_hw1 = nullptr, *d_hb1 = nullptr, *d_hw2 = nullptr, *d_hb2 = nullptr;
+    float* pooled_dbg = nullptr;
+    float* scores_buf = nullptr;
+    int64_t scored_for = 0;
+};
+
+struct gw_pipeline {
+    gw_stream* s = nullptr;
+    gw_deepclean* dc = nullptr;
+    gw_bbh* bbh = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    int nodes = 0;
+    const float* cap_in = nullptr;
+    float* cap_scores = nullptr;
+    float* cap_final = nullptr;
+    float *d_in = nullptr, *d_scores = nullptr, *d_final = nullptr;   // staging for gw_step_host
+};
+
+// ------------------------------------------------------------------------------ GEMM layer build
+// Builds B (weights in segment order), bias, the segment table and both tensor maps for one layer.
+// tap(a, par, r): index j of the filter tap that connects A-view row shift a, column half `par`
+// (position parity inside a pair row; always 0 for GK_DEC) to output column half r; <0 or >=k: none.
+static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, int n_det, int fmt, const void* in,
+                            int in_L, int cin_p, void* out, int cout_p, int batch, int epi) {
+    const HostLayer& H0 = dets[0];
+    ConvGemmParams& p = gl.g.p;
+    memset(&p, 0, sizeof p);
+    const int halves_in = gk == GK_DEC ? 1 : 2;       // A view packs position pairs?
+    const int halves_out = gk == GK_ENC ? 1 : 2;      // N packs (even | odd) outputs?
+    p.a_cols = halves_in * cin_p;
+    p.a_rows = in_L / halves_in;
+    p.M = p.a_rows;
+    p.N = halves_out * cout_p;
+    p.n_det = n_det;
+    p.fmt = fmt;
+    p.epi = epi;
+    p.act = H0.act;
+    if (p.N > 256 || p.N % 32) return fail(GW_EINVAL, "GEMM N = %d unsupported (must be a multiple of 32, <= 256)", p.N);
+    if (p.a_cols % kSegK) return fail(GW_EINVAL, "A view width %d not a multiple of 64", p.a_cols);
+    auto tap = [&](int a, int par, int r) -> int {
+        switch (gk) {
+            case GK_ENC: return 2 * a + par + H0.pad_l;               // x index 2l + j - pad = 2(l+a) + par
+            case GK_DEC: return ((r + H0.pad_l - 2 * a));             // m = 2l + j - pad, m = 2q + r, l = q + a
+            default:     return 2 * a + par - r + H0.pad_l;           // x index (2m + r) + j - pad = 2(m+a) + par
+        }
+    };
+    // segment table
+    int n_seg = 0;
+    std::vector<int> seg_a, seg_cb;
+    for (int a = -8; a <= 8; ++a)
+        for (int cb = 0; cb < p.a_cols / kSegK; ++cb) {
+            bool any = false;
+            for (int kk = 0; kk < kSegK && !any; ++kk) {
+                const int col = cb * kSegK + kk, par = col / cin_p, ci = col % cin_p;
+                if (ci >= H0.cin) continue;
+                for (int r = 0; r < halves_out; ++r) {
+                    const int j = tap(a, par, r);
+                    if (j >= 0 && j < H0.k) any = true;
+                }
+            }
+            if (any) { seg_a.push_back(a); seg_cb.push_back(cb); ++n_seg; }
+        }
+    if (n_seg > kMaxSeg) return fail(GW_EINVAL, "layer needs %d K segments (max %d)", n_seg, kMaxSeg);
+    p.n_seg = n_seg;
+    for (int s = 0; s < n_seg; ++s) { p.seg_shift[s] = static_cast<int8_t>(seg_a[s]); p.seg_col[s] = static_cast<int16_t>(seg_cb[s] * kSegK); }
+    // weights and bias
+    const size_t ktot = static_cast<size_t>(n_seg) * kSegK;
+    std::vector<uint16_t> B(static_cast<size_t>(n_det) * p.N * ktot, 0);
+    std::vector<float> bias(static_cast<size_t>(n_det) * p.N, 0.f);
+    for (int d = 0; d < n_det; ++d) {
+        const HostLayer& H = dets[d];
+        for (int r = 0; r < halves_out; ++r)
+            for (int co = 0; co < H.cout; ++co) {
+                const int n = r * cout_p + co;
+                bias[static_cast<size_t>(d) * p.N + n] = static_cast<float>(H.b[co]);
+                for (int s = 0; s < n_seg; ++s)
+                    for (int kk = 0; kk < kSegK; ++kk) {
+                        const int col = seg_cb[s] * kSegK + kk, par = col / cin_p, ci = col % cin_p;
+                        if (ci >= H.cin) continue;
+                        const int j = tap(seg_a[s], par, r);
+                        if (j < 0 || j >= H.k) continue;
+                        B[(static_cast<size_t>(d) * p.N + n) * ktot + static_cast<size_t>(s) * kSegK + kk] =
+                            to_storage_bits(H.W(co, ci, j), fmt);
+                    }
+            }
+    }
+    CU_TRY(cudaMalloc(&gl.d_B, B.size() * 2));
+    CU_TRY(cudaMemcpy(gl.d_B, B.data(), B.size() * 2, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMalloc(&gl.d_bias, bias.size() * 4));
+    CU_TRY(cudaMemcpy(gl.d_bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
+    p.A = in; p.B = gl.d_B; p.bias = gl.d_bias; p.out = out;
+    if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows, batch, p.a_cols, static_cast<uint64_t>(p.a_rows) * p.a_cols, kTileM)) return rc;
+    if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.N)) return rc;
+    gl.g.batch = batch;
+    const int stage_bytes = kTileM * 128 + p.N * 128;
+    int stages = (200 * 1024) / stage_bytes;
+    if (stages > 6) stages = 6;
+    if (stages > n_seg) stages = n_seg;
+    if (stages < 1) stages = 1;
+    gl.g.stages = stages;
+    gl.g.smem_bytes = conv_gemm_smem_bytes(p.N, stages);
+    gl.impl = g_conv_impl;
+    return GW_OK;
+}
+
+static void run_gemm(const GemmLayer& gl, cudaStream_t st) {
+    if (gl.impl == GW_IMPL_UMMA) launch_conv_gemm_umma(gl.g, st);
+    else launch_conv_gemm_simt(gl.g, st);
+}
+
+static void free_gemm(GemmLayer& gl) {
+    cudaFree(gl.d_B); cudaFree(gl.d_bias);
+    gl.d_B = nullptr; gl.d_bias = nullptr;
+}
+
+// =============================================================================== snapshotter
+extern "C" int gw_stream_create(gw_stream** out, int n_streams, int channels, int fs, int window, int stride) {
+    if (!out) return fail(GW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (n_streams < 1 || channels < 1 || fs < 1 || window < 1 || stride < 1 || stride > window)
+        return fail(GW_EINVAL, "gw_stream_create: need n_streams, channels, fs >= 1 and 1 <= stride <= window");
+    if (int rc = check_device()) return rc;
+    gw_stream* s = new gw_stream();
+    s->n = n_streams; s->C = channels; s->fs = fs; s->W = window; s->S = stride;
+    const size_t bytes = static_cast<size_t>(n_streams) * channels * window * sizeof(float);
+    cudaError_t e = cudaMalloc(&s->ring, bytes);
+    if (e == cudaSuccess) e = cudaMemset(s->ring, 0, bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_count, sizeof(long long));
+    if (e == cudaSuccess) e = cudaMemset(s->d_count, 0, sizeof(long long));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_ticket, sizeof(unsigned));
+    if (e == cudaSuccess) e = cudaMemset(s->d_ticket, 0, sizeof(unsigned));
+    if (e != cudaSuccess) {
+        cudaFree(s->ring); cudaFree(s->d_count); cudaFree(s->d_ticket);
+        delete s;
+        return fail(e == cudaErrorMemoryAllocation ? GW_ENOMEM : GW_ECUDA, "gw_stream_create: %s", cudaGetErrorString(e));
+    }
+    *out = s;
+    return GW_OK;
+}
+
+extern "C" int gw_stream_destroy(gw_stream* s) {
+    if (!s) return GW_OK;
+    cudaFree(s->ring); cudaFree(s->d_count); cudaFree(s->d_ticket);
+    delete s;
+    return GW_OK;
+}
+
+static int stream_update_checked(gw_stream* s) {
+    if (s->dc && s->dc->cleaned_for != s->updates)
+        return fail(GW_ESTATE, "gw_stream_update: update %lld has not been through gw_deepclean_forward + gw_cleaned_strain",
+                    (long long)s->updates);
+    return GW_OK;
+}
+static void stream_update_enqueue(gw_stream* s, const float* src, cudaStream_t st) {
+    launch_append(s->ring, src, s->d_count, s->d_ticket, s->n * s->C, s->W, s->S, st);
+}
+
+extern "C" int gw_stream_update(gw_stream* s, const float* new_samples_dev, void* stream) {
+    if (!s || !new_samples_dev) return fail(GW_EINVAL, "gw_stream_update: NULL argument");
+    if (int rc = stream_update_checked(s)) return rc;
+    stream_update_enqueue(s, new_samples_dev, static_cast<cudaStream_t>(stream));
+    CU_TRY(cudaGetLastError());
+    s->updates += 1;
+    return GW_OK;
+}
+
+extern "C" int gw_stream_snapshot(gw_stream* s, float* out_dev, int64_t* first_index_host, void* stream) {
+    if (!s || !out_dev) return fail(GW_EINVAL, "gw_stream_snapshot: NULL argument");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    launch_snapshot(s->ring, out_dev, s->d_count, s->n * s->C, s->W, st);
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaStreamSynchronize(st));
+    if (first_index_host) *first_index_host = s->updates * static_cast<int64_t>(s->S) - s->W;
+    return GW_OK;
+}
+
+extern "C" int64_t gw_stream_count(const gw_stream* s) { return s ? s->updates * static_cast<int64_t>(s->S) : 0; }
+
+// ================================================================================= DeepClean
+static int validate_dc_layer(const HostLayer& H, bool last) {
+    if (H.stride != 2 || (H.k & 1) == 0) return fail(GW_EINVAL, "DeepClean layers need stride 2 and odd k");
+    if (H.kind == GW_CONV && (H.pad_l != H.k / 2 || H.pad_r != H.k / 2)) return fail(GW_EINVAL, "Conv1d needs pad = k/2");
+    if (H.kind == GW_CONVT && (H.pad_l != H.k / 2 || H.pad_r != 1)) return fail(GW_EINVAL, "ConvTranspose1d needs padding k/2, output_padding 1");
+    if (H.pool != 1) return fail(GW_EINVAL, "DeepClean layers have no pooling");
+    if (last && (H.kind != GW_CONVT || H.cout != 1 || H.act != GW_ACT_NONE))
+        return fail(GW_EINVAL, "last DeepClean layer must be a linear ConvTranspose1d with one output channel");
+    return GW_OK;
+}
+
+extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
+    if (!dc) return GW_OK;
+    for (auto& g : dc->gemm) free_gemm(g);
+    for (void* a : dc->act) cudaFree(a);
+    cudaFree(dc->d_wt_final); cudaFree(dc->d_b_final); cudaFree(dc->pred); cudaFree(dc->acc); cudaFree(dc->nhat);
+    cudaFree(dc->d_hann); cudaFree(dc->d_inv_wsum); cudaFree(dc->d_rows_map); cudaFree(dc->d_strain_rows);
+    cudaFree(dc->final_buf);
+    if (dc->s && dc->s->dc == dc) dc->s->dc = nullptr;
+    delete dc;
+    return GW_OK;
+}
+
+static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spec) {
+    const int W = s->W, S = s->S;
+    const int nl = spec->n_layers, nd = spec->n_det;
+    dc->host.resize(static_cast<size_t>(nd) * nl);
+    for (int d = 0; d < nd; ++d)
+        for (int i = 0; i < nl; ++i) {
+            if (int rc = fold_layer(spec->layers[d * nl + i], dc->host[d * nl + i])) return rc;
+            const HostLayer &H = dc->host[d * nl + i], &H0 = dc->host[i];
+            if (int rc = validate_dc_layer(H, i == nl - 1)) return rc;
+            if (H.kind != H0.kind || H.cin != H0.cin || H.cout != H0.cout || H.k != H0.k || H.act != H0.act)
+                return fail(GW_EINVAL, "detectors must share the layer shapes");
+        }
+    if (dc->host[0].cin != spec->n_witness) return fail(GW_EINVAL, "first layer cin != n_witness");
+    // padded channel counts: consumer decides (pair views need multiples of 32, ConvT inputs multiples of 64)
+    std::vector<int> cpad(nl + 1);
+    for (int i = 0; i <= nl; ++i) {
+        const int c = i == 0 ? dc->host[0].cin : dc->host[i - 1].cout;
+        if (i == nl) { cpad[i] = 1; break; }
+        const bool gemm_consumer = i < nl - 1;
+        cpad[i] = round_up(c, (gemm_consumer && dc->host[i].kind == GW_CONVT) ? 64 : 32);
+    }
+    // lengths
+    std::vector<int> len(nl + 1);
+    len[0] = W;
+    for (int i = 0; i < nl; ++i) {
+        const HostLayer& H = dc->host[i];
+        if (H.kind == GW_CONV) {
+            if (len[i] % 2) return fail(GW_EINVAL, "window length must be divisible by 2^(number of encoder layers)");
+            len[i + 1] = len[i] / 2;
+        } else {
+            len[i + 1] = len[i] * 2;
+        }
+        if (i > 0 && dc->host[i].cin != dc->host[i - 1].cout) return fail(GW_EINVAL, "layer %d cin mismatch", i);
+    }
+    if (len[nl] != W) return fail(GW_EINVAL, "network output length %d != window %d", len[nl], W);
+    const int batch = s->n * nd;
+    dc->batch = batch;
+    dc->act.assign(nl, nullptr);
+    dc->act_rows.assign(nl, 0); dc->act_cols.assign(nl, 0);
+    for (int i = 0; i < nl; ++i) {                  // act[i] = input of layer i
+        dc->act_rows[i] = len[i]; dc->act_cols[i] = cpad[i];
+        const size_t bytes = static_cast<size_t>(batch) * len[i] * cpad[i] * 2;
+        CU_TRY(cudaMalloc(&dc->act[i], bytes));
+        CU_TRY(cudaMemset(dc->act[i], 0, bytes));
+    }
+    dc->gemm.resize(nl - 1);
+    std::vector<HostLayer> per_det(nd);
+    for (int i = 0; i < nl - 1; ++i) {
+        for (int d = 0; d < nd; ++d) per_det[d] = dc->host[d * nl + i];
+        const GemmKind gk = dc->host[i].kind == GW_CONV ? GK_ENC : GK_DEC;
+        if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, dc->act[i], len[i], cpad[i],
+                                      dc->act[i + 1], cpad[i + 1], batch, EPI_STORE))
+            return rc;
+    }
+    // final layer on CUDA cores: wt[d][j][ci] fp32 holding storage-rounded weights
+    {
+        const HostLayer& H = dc->host[nl - 1];
+        dc->final_K = H.k; dc->final_pad = H.pad_l; dc->final_cpad = cpad[nl - 1]; dc->final_L = len[nl - 1];
+        std::vector<float> wt(static_cast<size_t>(nd) * H.k * cpad[nl - 1], 0.f), bf(nd);
+        for (int d = 0; d < nd; ++d) {
+            const HostLayer& Hd = dc->host[d * nl + nl - 1];
+            for (int j = 0; j < H.k; ++j)
+                for (int ci = 0; ci < H.cin; ++ci)
+                    wt[(static_cast<size_t>(d) * H.k + j) * cpad[nl - 1] + ci] =
+                        static_cast<float>(storage_to_double(to_storage_bits(Hd.W(0, ci, j), dc->fmt), dc->fmt));
+            bf[d] = static_cast<float>(Hd.b[0]);
+        }
+        CU_TRY(cudaMalloc(&dc->d_wt_final, wt.size() * 4));
+        CU_TRY(cudaMemcpy(dc->d_wt_final, wt.data(), wt.size() * 4, cudaMemcpyHostToDevice));
+        CU_TRY(cudaMalloc(&dc->d_b_final, bf.size() * 4));
+        CU_TRY(cudaMemcpy(dc->d_b_final, bf.data(), bf.size() * 4, cudaMemcpyHostToDevice));
+    }
+    const size_t wbytes = static_cast<size_t>(batch) * W * sizeof(float);
+    CU_TRY(cudaMalloc(&dc->pred, wbytes));
+    CU_TRY(cudaMemset(dc->pred, 0, wbytes));
+    CU_TRY(cudaMalloc(&dc->acc, wbytes));
+    CU_TRY(cudaMemset(dc->acc, 0, wbytes));
+    CU_TRY(cudaMalloc(&dc->final_buf, static_cast<size_t>(batch) * S * sizeof(float)));
+    // periodic Hann window and the reciprocal of the summed weights covering window position n:
+    // wsum[n] = sum_{i >= 0, n + iS < W} w[n + iS]  (every sample with absolute index >= 0 has exactly
+    // these windows over it, during warm-up as well: older windows would only add samples < 0).
+    {
+        std::vector<double> w(W);
+        const double pi = 3.14159265358979323846;
+        for (int n = 0; n < W; ++n) w[n] = 0.5 - 0.5 * cos(2.0 * pi * n / W);
+        std::vector<float> wf(W), inv(W);
+        for (int n = 0; n < W; ++n) {
+            double sum = 0.0;
+            for (int m = n; m < W; m += S) sum += w[m];
+            wf[n] = static_cast<float>(w[n]);
+            inv[n] = sum > 0.0 ? static_cast<float>(1.0 / sum) : 0.f;
+        }
+        CU_TRY(cudaMalloc(&dc->d_hann, W * 4));
+        CU_TRY(cudaMemcpy(dc->d_hann, wf.data(), W * 4, cudaMemcpyHostToDevice));
+        CU_TRY(cudaMalloc(&dc->d_inv_wsum, W * 4));
+        CU_TRY(cudaMemcpy(dc->d_inv_wsum, inv.data(), W * 4, cudaMemcpyHostToDevice));
+    }
+    CU_TRY(cudaMalloc(&dc->d_rows_map, static_cast<size_t>(nd) * spec->n_witness * sizeof(int)));
+    CU_TRY(cudaMemcpy(dc->d_rows_map, spec->witness_rows, static_cast<size_t>(nd) * spec->n_witness * sizeof(int), cudaMemcpyHostToDevice));
+    CU_TRY(cudaMalloc(&dc->d_strain_rows, nd * sizeof(int)));
+    CU_TRY(cudaMemcpy(dc->d_strain_rows, spec->strain_row, nd * sizeof(int), cudaMemcpyHostToDevice));
+    CU_TRY(conv_gemm_prepare());
+    return GW_OK;
+}
+
+extern "C" int gw_deepclean_create(gw_deepclean** out, gw_stream* s, const gw_dc_spec* spec, int dtype) {
+    if (!out) return fail(GW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!s || !spec || !spec->layers || !spec->witness_rows || !spec->strain_row) return fail(GW_EINVAL, "gw_deepclean_create: NULL argument");
+    if (dtype != GW_BF16 && dtype != GW_FP16) return fail(GW_EINVAL, "dtype must be GW_BF16 or GW_FP16");
+    if (spec->n_det < 1 || spec->n_layers < 2 || spec->n_witness < 1) return fail(GW_EINVAL, "bad DeepClean spec");
+    if (s->dc) return fail(GW_ESTATE, "stream already has a DeepClean stage");
+    if (s->updates != 0) return fail(GW_ESTATE, "DeepClean must be created before the first update");
+    if (spec->agg != GW_AGG_HANN_OLA && spec->agg != GW_AGG_LAST_STRIDE) return fail(GW_EINVAL, "unknown aggregation mode");
+    if (spec->agg == GW_AGG_HANN_OLA && (s->W % s->S != 0 || s->W / s->S < 2))
+        return fail(GW_EINVAL, "Hann overlap-add needs window %% stride == 0 and window/stride >= 2");
+    if (spec->delta < 0 || spec->delta > s->W - s->S) return fail(GW_EINVAL, "delta out of range");
+    for (int d = 0; d < spec->n_det; ++d) {
+        if (spec->strain_row[d] < 0 || spec->strain_row[d] >= s->C) return fail(GW_EINVAL, "strain row out of range");
+        for (int c = 0; c < spec->n_witness; ++c)
+            if (spec->witness_rows[d * spec->n_witness + c] < 0 || spec->witness_rows[d * spec->n_witness + c] >= s->C)
+                return fail(GW_EINVAL, "witness row out of range");
+    }
+    if (int rc = check_device()) return rc;
+    gw_deepclean* dc = new gw_deepclean();
+    dc->s = s; dc->n_det = spec->n_det; dc->n_layers = spec->n_layers; dc->n_wit = spec->n_witness;
+    dc->agg = spec->agg; dc->delta = spec->delta;
+    dc->fmt = dtype == GW_BF16 ? FMT_BF16 : FMT_FP16;
+    int rc = deepclean_build(dc, s, spec);
+    if (rc != GW_OK) { std::string keep = g_err; gw_deepclean_destroy(dc); g_err = keep; return rc; }
+    s->dc = dc;
+    *out = dc;
+    return GW_OK;
+}
+
+static void deepclean_forward_enqueue(gw_deepclean* dc, cudaStream_t st) {
+    gw_stream* s = dc->s;
+    launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
+                  dc->act_cols[0], dc->fmt, st);
+    for (auto& g : dc->gemm) run_gemm(g, st);
+    launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
+                       dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
+}
+
+extern "C" int gw_deepclean_forward(gw_deepclean* dc, void* stream) {
+    if (!dc) return fail(GW_EINVAL, "gw_deepclean_forward: NULL handle");
+    if (dc->s->updates == 0 || dc->forward_for == dc->s->updates)
+        return fail(GW_ESTATE, "gw_deepclean_forward: no new update to run on");
+    deepclean_forward_enqueue(dc, static_cast<cudaStream_t>(stream));
+    CU_TRY(cudaGetLastError());
+    dc->forward_for = dc->s->updates;
+    return GW_OK;
+}
+
+extern "C" int gw_deepclean_noise(gw_deepclean* dc, float* out_dev, void* stream) {
+    if (!dc || !out_dev) return fail(GW_EINVAL, "gw_deepclean_noise: NULL argument");
+    if (dc->forward_for == 0) return fail(GW_ESTATE, "gw_deepclean_noise: no forward pass yet");
+    CU_TRY(cudaMemcpyAsync(out_dev, dc->pred, static_cast<size_t>(dc->batch) * dc->s->W * 4, cudaMemcpyDeviceToDevice,
+                           static_cast<cudaStream_t>(stream)));
+    return GW_OK;
+}
+
+extern "C" int gw_deepclean_activation(gw_deepclean* dc, int layer, void* out_dev, int64_t out_bytes, int* rows,
+                                       int* cols, void* stream) {
+    if (!dc || layer < -1 || layer >= dc->n_layers - 1) return fail(GW_EINVAL, "gw_deepclean_activation: bad layer");
+    const int i = layer + 1;
+    if (rows) *rows = dc->act_rows[i];
+    if (cols) *cols = dc->act_cols[i];
+    const int64_t bytes = static_cast<int64_t>(dc->batch) * dc->act_rows[i] * dc->act_cols[i] * 2;
+    if (out_dev) {
+        if (out_bytes < bytes) return fail(GW_EINVAL, "output buffer too small (%lld < %lld)", (long long)out_bytes, (long long)bytes);
+        CU_TRY(cudaMemcpyAsync(out_dev, dc->act[i], bytes, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+    }
+    return GW_OK;
+}
+
+static void cleaned_enqueue(gw_deepclean* dc, float* final_out, float* running_out, float* nhat_out, cudaStream_t st) {
+    gw_stream* s = dc->s;
+    AggParams a;
+    a.pred = dc->pred; a.acc = dc->acc; a.ring = s->ring; a.count = s->d_count; a.strain_rows = dc->d_strain_rows;
+    a.hann = dc->d_hann; a.inv_wsum = dc->d_inv_wsum;
+    a.final_out = final_out; a.running_out = running_out; a.nhat_out = nhat_out; a.clf_in = dc->clf_in;
+    a.n_streams = s->n; a.n_det = dc->n_det; a.channels = s->C; a.W = s->W; a.S = s->S; a.Lb = dc->Lb;
+    a.delta = dc->delta; a.agg = dc->agg;
+    launch_aggregate(a, st);
+}
+
+extern "C" int gw_cleaned_strain(gw_deepclean* dc, float* out_dev, int mode, void* stream) {
+    if (!dc) return fail(GW_EINVAL, "gw_cleaned_strain: NULL handle");
+    if (mode != GW_FINAL && mode != GW_RUNNING) return fail(GW_EINVAL, "gw_cleaned_strain: bad mode");
+    if (dc->forward_for != dc->s->updates || dc->cleaned_for == dc->s->updates)
+        return fail(GW_ESTATE, "gw_cleaned_strain: call gw_deepclean_forward for this update first (once)");
+    if (!dc->nhat) {
+        const size_t wbytes = static_cast<size_t>(dc->batch) * dc->s->W * sizeof(float);
+        CU_TRY(cudaMalloc(&dc->nhat, wbytes));
+        CU_TRY(cudaMemset(dc->nhat, 0, wbytes));
+    }
+    cleaned_enqueue(dc, mode == GW_FINAL ? out_dev : nullptr, mode == GW_RUNNING ? out_dev : nullptr, dc->nhat,
+                    static_cast<cudaStream_t>(stream));
+    CU_TRY(cudaGetLastError());
+    dc->cleaned_for = dc->s->updates;
+    return GW_OK;
+}
+
+extern "C" int gw_noise_estimate(gw_deepclean* dc, float* out_dev, void* stream) {
+    if (!dc || !out_dev) return fail(GW_EINVAL, "gw_noise_estimate: NULL argument");
+    if (!dc->nhat || dc->cleaned_for == 0) return fail(GW_ESTATE, "gw_noise_estimate: call gw_cleaned_strain first");
+    CU_TRY(cudaMemcpyAsync(out_dev, dc->nhat, static_cast<size_t>(dc->batch) * dc->s->W * 4, cudaMemcpyDeviceToDevice,
+                           static_cast<cudaStream_t>(stream)));
+    return GW_OK;
+}
+
+// ================================================================================ classifier
+extern "C" int gw_bbh_destroy(gw_bbh* b) {
+    if (!b) return GW_OK;
+    for (auto& g : b->gemm) free_gemm(g);
+    for (void* a : b->act) cudaFree(a);
+    cudaFree(b->d_w1); cudaFree(b->d_b1); cudaFree(b->in_buf);
+    cudaFree(b->d_hw1); cudaFree(b->d_hb1); cudaFree(b->d_hw2); cudaFree(b->d_hb2);
+    cudaFree(b->pooled_dbg); cudaFree(b->scores_buf);
+    if (b->dc && b->dc->bbh == b) { b->dc->bbh = nullptr; b->dc->clf_in = nullptr; b->dc->Lb = 0; }
+    delete b;
+    return GW_OK;
+}
+
+static int upload(float** dst, const float* src, size_t n) {
+    CU_TRY(cudaMalloc(dst, n * 4));
+    CU_TRY(cudaMemcpy(*dst, src, n * 4, cudaMemcpyHostToDevice));
+    return GW_OK;
+}
+
+static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
+    const int nc = spec->n_convs;
+    std::vector<HostLayer> H(nc);
+    int L = spec->length;
+    for (int i = 0; i < nc; ++i) {
+        if (int rc = fold_layer(spec->convs[i], H[i])) return rc;
+        if (H[i].kind != GW_CONV || H[i].stride != 1 || H[i].pad_l + H[i].pad_r != H[i].k - 1 || H[i].pool != 4 ||
+            H[i].act != GW_ACT_RELU)
+            return fail(GW_EINVAL, "classifier blocks must be Conv1d stride 1 'same' padding + ReLU + MaxPool(4)");
+        if (i > 0 && H[i].cin != H[i - 1].cout) return fail(GW_EINVAL, "classifier block %d cin mismatch", i);
+    }
+    if (H[0].cin != b->n_det) return fail(GW_EINVAL, "first classifier block cin must equal the number of detectors");
+    if (spec->n_dense != 2 || spec->dense_dims[0] != H[nc - 1].cout || spec->dense_dims[2] != 1)
+        return fail(GW_EINVAL, "dense head must be cout -> hidden -> 1");
+    const int hidden = spec->dense_dims[1];
+    if (hidden < 1 || hidden > 128) return fail(GW_EINVAL, "dense hidden width must be in [1,128]");
+    // first block on CUDA cores
+    b->c1 = H[0];
+    b->c1_cpad = round_up(H[0].cout, 32);
+    {
+        std::vector<float> w(H[0].w.size()), bb(H[0].cout);
+        for (size_t i = 0; i < w.size(); ++i) w[i] = static_cast<float>(storage_to_double(to_storage_bits(H[0].w[i], b->fmt), b->fmt));
+        for (int c = 0; c < H[0].cout; ++c) bb[c] = static_cast<float>(H[0].b[c]);
+        if (int rc = upload(&b->d_w1, w.data(), w.size())) return rc;
+        if (int rc = upload(&b->d_b1, bb.data(), bb.size())) return rc;
+    }
+    CU_TRY(cudaMalloc(&b->in_buf, static_cast<size_t>(b->batch) * b->n_det * L * 4));
+    CU_TRY(cudaMemset(b->in_buf, 0, static_cast<size_t>(b->batch) * b->n_det * L * 4));
+    CU_TRY(cudaMalloc(&b->scores_buf, static_cast<size_t>(b->batch) * 4));
+    // activations: act[i] = input of block i+1 = pooled output of block i
+    b->act.assign(nc - 1, nullptr);
+    std::vector<int> len(nc), cp(nc);
+    int l = L;
+    for (int i = 0; i < nc - 1; ++i) {
+        l /= 4;
+        len[i] = l; cp[i] = round_up(H[i].cout, 32);
+        CU_TRY(cudaMalloc(&b->act[i], static_cast<size_t>(b->batch) * l * cp[i] * 2));
+        CU_TRY(cudaMemset(b->act[i], 0, static_cast<size_t>(b->batch) * l * cp[i] * 2));
+    }
+    if (int rc = upload(&b->d_hw1, spec->dense_w[0], static_cast<size_t>(hidden) * spec->dense_dims[0])) return rc;
+    if (int rc = upload(&b->d_hb1, spec->dense_b[0], hidden)) return rc;
+    if (int rc = upload(&b->d_hw2, spec->dense_w[1], hidden)) return rc;
+    if (int rc = upload(&b->d_hb2, spec->dense_b[1], 1)) return rc;
+    b->gemm.resize(nc - 1);
+    for (int i = 1; i < nc; ++i) {
+        const bool last = i == nc - 1;
+        const int cout_p = round_up(H[i].cout, 32);
+        if (last && len[i - 1] / 2 > kTileM) return fail(GW_EINVAL, "classifier window too long for the fused head");
+        if (last && cout_p != H[i].cout) return fail(GW_EINVAL, "last classifier block cout must be a multiple of 32");
+        if (len[i - 1] % 4) return fail(GW_EINVAL, "classifier length must be divisible by 4^blocks");
+        GemmLayer& gl = b->gemm[i - 1];
+        if (int rc = build_gemm_layer(gl, GK_BBH, &H[i], 1, b->fmt, b->act[i - 1], len[i - 1], cp[i - 1],
+                                      last ? nullptr : b->act[i], cout_p, b->batch, last ? EPI_POOL_HEAD : EPI_POOL))
+            return rc;
+        if (last) {
+            ConvGemmParams& p = gl.g.p;
+            p.hw1 = b->d_hw1; p.hb1 = b->d_hb1; p.hw2 = b->d_hw2; p.hb2 = b->d_hb2; p.head_hidden = hidden;
+            p.scores = b->scores_buf;
+            CU_TRY(cudaMalloc(&b->pooled_dbg, static_cast<size_t>(b->batch) * (p.M / 2) * (p.N / 2) * 4));
+            p.pooled_dbg = b->pooled_dbg;
+            // the head stages [64][N/2+1] + N/2 + hidden floats in the (free) pipeline shared memory
+            const int need = (64 * (p.N / 2 + 1) + p.N / 2 + hidden) * 4 + 1024;
+            if (gl.g.smem_bytes < need) gl.g.smem_bytes = need;
+        }
+    }
+    CU_TRY(conv_gemm_prepare());
+    return GW_OK;
+}
+
+extern "C" int gw_bbh_create(gw_bbh** out, gw_deepclean* dc, const gw_bbh_spec* spec, int dtype, int n_det, int max_batch) {
+    if (!out) return fail(GW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!spec || !spec->convs || !spec->dense_dims || !spec->dense_w || !spec->dense_b) return fail(GW_EINVAL, "gw_bbh_create: NULL argument");
+    if (dtype != GW_BF16 && dtype != GW_FP16) return fail(GW_EINVAL, "dtype must be GW_BF16 or GW_FP16");
+    if (spec->n_convs < 2) return fail(GW_EINVAL, "classifier needs at least 2 conv blocks");
+    if (spec->length < 64 || spec->length % 64) return fail(GW_EINVAL, "classifier length must be a multiple of 64");
+    if (dc) {
+        if (dc->bbh) return fail(GW_ESTATE, "DeepClean stage already has a classifier");
+        if (spec->length + dc->delta > dc->s->W) return fail(GW_EINVAL, "classifier window + delta exceeds the snapshot window");
+        n_det = dc->n_det; max_batch = dc->s->n;
+    } else if (n_det < 1 || max_batch < 1) {
+        return fail(GW_EINVAL, "stateless classifier needs n_det >= 1 and max_batch >= 1");
+    }
+    if (int rc = check_device()) return rc;
+    gw_bbh* b = new gw_bbh();
+    b->dc = dc; b->n_det = n_det; b->batch = max_batch; b->L = spec->length;
+    b->fmt = dtype == GW_BF16 ? FMT_BF16 : FMT_FP16;
+    int rc = bbh_build(b, spec);
+    if (rc != GW_OK) { std::string keep = g_err; b->dc = nullptr; gw_bbh_destroy(b); g_err = keep; return rc; }
+    if (dc) { dc->bbh = b; dc->clf_in = b->in_buf; dc->Lb = b->L; }
+    *out = b;
+    return GW_OK;
+}
+
+static void bbh_enqueue(gw_bbh* b, const float* in, int batch, cudaStream_t st) {
+    launch_bbh_conv1(in, b->d_w1, b->d_b1, b->act[0], batch, b->n_det, b->L, b->c1.cout, b->c1_cpad, b->c1.k,
+                     b->c1.pad_l, b->c1.pool, b->fmt, st);
+    for (auto& g : b->gemm) {
+        GemmLayer gl = g;
+        gl.g.batch = batch;
+        run_gemm(gl, st);
+    }
+}
+
+extern "C" int gw_bbh_score(gw_bbh* b, float* scores_dev, void* stream) {
+    if (!b || !scores_dev) return fail(GW_EINVAL, "gw_bbh_score: NULL argument");
+    if (!b->dc) return fail(GW_ESTATE, "gw_bbh_score: stateless classifier; use gw_bbh_score_batch");
+    if (b->dc->cleaned_for != b->dc->s->updates || b->dc->cleaned_for == 0 || b->scored_for == b->dc->s->updates)
+        return fail(GW_ESTATE, "gw_bbh_score: call gw_cleaned_strain for this update first (once)");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    bbh_enqueue(b, b->in_buf, b->batch, st);
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaMemcpyAsync(scores_dev, b->scores_buf, static_cast<size_t>(b->batch) * 4, cudaMemcpyDeviceToDevice, st));
+    b->scored_for = b->dc->s->updates;
+    return GW_OK;
+}
+
+extern "C" int gw_bbh_score_batch(gw_bbh* b, const float* windows_dev, int batch, float* scores_dev, void* stream) {
+    if (!b || !windows_dev || !scores_dev) return fail(GW_EINVAL, "gw_bbh_score_batch: NULL argument");
+    if (batch < 1 || batch > b->batch) return fail(GW_EINVAL, "batch %d outside [1, %d]", batch, b->batch);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    bbh_enqueue(b, windows_dev, batch, st);
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaMemcpyAsync(scores_dev, b->scores_buf, static_cast<size_t>(batch) * 4, cudaMemcpyDeviceToDevice, st));
+    return GW_OK;
+}
+
+// ================================================================================== pipeline
+extern "C" int gw_pipeline_create(gw_pipeline** out, gw_stream* s, gw_deepclean* dc, gw_bbh* bbh) {
+    if (!out) return fail(GW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!s || !dc || dc->s != s || (bbh && bbh->dc != dc)) return fail(GW_EINVAL, "gw_pipeline_create: stages do not belong together");
+    gw_pipeline* p = new gw_pipeline();
+    p->s = s; p->dc = dc; p->bbh = bbh;
+    *out = p;
+    return GW_OK;
+}
+
+extern "C" int gw_pipeline_destroy(gw_pipeline* p) {
+    if (!p) return GW_OK;
+    if (p->exec) cudaGraphExecDestroy(p->exec);
+    if (p->graph) cudaGraphDestroy(p->graph);
+    cudaFree(p->d_in); cudaFree(p->d_scores); cudaFree(p->d_final);
+    delete p;
+    return GW_OK;
+}
+
+extern "C" int gw_pipeline_graph_nodes(const gw_pipeline* p) { return p ? p->nodes : 0; }
+
+static int pipeline_capture(gw_pipeline* p, const float* in, float* scores, float* fin, cudaStream_t st) {
+    if (p->exec) { cudaGraphExecDestroy(p->exec); p->exec = nullptr; }
+    if (p->graph) { cudaGraphDestroy(p->graph); p->graph = nullptr; }
+    const long long before = g_kernel_launches;
+    CU_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+    stream_update_enqueue(p->s, in, st);
+    deepclean_forward_enqueue(p->dc, st);
+    cleaned_enqueue(p->dc, fin, nullptr, nullptr, st);
+    if (p->bbh) {
+        bbh_enqueue(p->bbh, p->bbh->in_buf, p->bbh->batch, st);
+        cudaMemcpyAsync(scores, p->bbh->scores_buf, static_cast<size_t>(p->bbh->batch) * 4, cudaMemcpyDeviceToDevice, st);
+    }
+    cudaError_t e = cudaStreamEndCapture(st, &p->graph);
+    p->nodes = static_cast<int>(g_kernel_launches - before);
+    g_kernel_launches = before;                         // captured, not launched
+    if (e != cudaSuccess) return fail(GW_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+    CU_TRY(cudaGraphInstantiate(&p->exec, p->graph, 0));
+    p->cap_in = in; p->cap_scores = scores; p->cap_final = fin;
+    return GW_OK;
+}
+
+extern "C" int gw_step(gw_pipeline* p, const float* new_samples_dev, float* scores_dev, float* cleaned_final_dev, void* stream) {
+    if (!p || !new_samples_dev || !cleaned_final_dev || (p->bbh && !scores_dev)) return fail(GW_EINVAL, "gw_step: NULL argument");
+    if (int rc = stream_update_checked(p->s)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!p->exec || p->cap_in != new_samples_dev || p->cap_scores != scores_dev || p->cap_final != cleaned_final_dev) {
+        if (st == nullptr) return fail(GW_EINVAL, "gw_step needs a non-default stream (graph capture)");
+        if (int rc = pipeline_capture(p, new_samples_dev, scores_dev, cleaned_final_dev, st)) return rc;
+    }
+    CU_TRY(cudaGraphLaunch(p->exec, st));
+    g_kernel_launches += p->nodes;
+    p->s->updates += 1;
+    p->dc->forward_for = p->dc->cleaned_for = p->s->updates;
+    if (p->bbh) p->bbh->scored_for = p->s->updates;
+    return GW_OK;
+}
+
+extern "C" int gw_step_host(gw_pipeline* p, const float* new_samples_host, float* scores_host, float* cleaned_final_host, void* stream) {
+    if (!p || !new_samples_host || !cleaned_final_host || (p->bbh && !scores_host)) return fail(GW_EINVAL, "gw_step_host: NULL argument");
+    gw_stream* s = p->s;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t in_bytes = static_cast<size_t>(s->n) * s->C * s->S * 4;
+    const size_t fin_bytes = static_cast<size_t>(p->dc->batch) * s->S * 4;
+    const size_t sc_bytes = static_cast<size_t>(s->n) * 4;
+    if (!p->d_in) {
+        CU_TRY(cudaMalloc(&p->d_in, in_bytes));
+        CU_TRY(cudaMalloc(&p->d_final, fin_bytes));
+        CU_TRY(cudaMalloc(&p->d_scores, sc_bytes));
+    }
+    CU_TRY(cudaMemcpyAsync(p->d_in, new_samples_host, in_bytes, cudaMemcpyHostToDevice, st));
+    if (int rc = gw_step(p, p->d_in, p->d_scores, p->d_final, stream)) return rc;
+    CU_TRY(cudaMemcpyAsync(cleaned_final_host, p->d_final, fin_bytes, cudaMemcpyDeviceToHost, st));
+    if (p->bbh) CU_TRY(cudaMemcpyAsync(scores_host, p->d_scores, sc_bytes, cudaMemcpyDeviceToHost, st));
+    CU_TRY(cudaStreamSynchronize(st));
+    return GW_OK;
+}

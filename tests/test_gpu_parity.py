@@ -1,0 +1,254 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+Bars (north_star): snapshots and indices bit-exact; network outputs relative L2 <= 1e-2 and every
+element |d| <= 2e-2 RMS(oracle output); classifier scores |d| <= 5e-3."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2108_12430_b200 import binding as gw
+from paper_2108_12430_b200 import specs as S
+from paper_2108_12430_b200 import synth
+from tests import util
+
+pytestmark = pytest.mark.gpu
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# ------------------------------------------------------------------------------- a1 snapshot
+@pytest.mark.parametrize("n,C,W,S", [(1, 22, 512, 64), (3, 5, 96, 7), (2, 44, 4096, 512), (2, 3, 10, 10),
+                                      (1, 2, 33, 1), (4, 4, 64, 12), (1, 22, 32768, 1024)])
+def test_snapshot_bit_exact(n, C, W, S_):
+    spec = S.StreamSpec(n, 1, 512, W, S_, n_witness=C - 1)
+    st = gw.Stream(spec)
+    n_up = min(3 * (W // S_) + 3, 40)
+    x = np.random.default_rng(11).standard_normal((n, C, n_up * S_)).astype(np.float32)
+    xd = _dev(x)
+    for t in range(n_up):
+        st.update(xd[:, :, t * S_:(t + 1) * S_].contiguous())
+        if t % 3 == 0 or t == n_up - 1:
+            snap, first = st.snapshot()
+            snap = snap.cpu().numpy()
+            for i in range(n):
+                ref, first_ref = oracle.snapshot(x[i][:, :(t + 1) * S_], t, S_, W)
+                assert first == first_ref
+                assert np.array_equal(snap[i].view(np.uint32), ref.view(np.uint32)), (t, i)
+    assert st.count() == n_up * S_
+
+
+# --------------------------------------------------------------------- DeepClean streaming (C0)
+def _run_streaming(cfg, dtype, n_up, white, agg=S.AGG_HANN_OLA, delta=0, check_scores=True, impl=gw.GW_IMPL_UMMA,
+                   use_graph=False):
+    gw.set_conv_impl(impl)
+    try:
+        st_spec = cfg.stream
+        dc_params, bbh_params = util.make_params(cfg)
+        x = synth.multi_stream(cfg.seed, st_spec, n_up * st_spec.stride, white=white)
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, agg, delta)
+    finally:
+        gw.set_conv_impl(gw.GW_IMPL_UMMA)
+    oracles = [util.make_stream_oracle(cfg, dc_params, bbh_params, dtype, n_up, agg, delta)
+               for _ in range(st_spec.n_streams)]
+    xd = _dev(x)
+    stats = {"pred": 0.0, "nhat": 0.0, "score": 0.0}
+    et = util.elem_tol(dtype)
+    cs = torch.cuda.Stream()
+    scores_d = torch.zeros(st_spec.n_streams, device="cuda")
+    final_d = torch.zeros((st_spec.n_streams, st_spec.n_det, st_spec.stride), device="cuda")
+    for t in range(n_up):
+        new = xd[:, :, t * st_spec.stride:(t + 1) * st_spec.stride].contiguous()
+        if use_graph:
+            with torch.cuda.stream(cs):
+                pipe.step(new, scores_d, final_d, cs)
+            cs.synchronize()
+            final = final_d.cpu().numpy()
+            scores = scores_d.cpu().numpy() if bbh is not None else None
+            pred = dc.noise().cpu().numpy()
+            running = nhat = None
+        else:
+            stream.update(new)
+            dc.forward()
+            pred = dc.noise().cpu().numpy()
+            running = dc.cleaned(gw.GW_RUNNING).cpu().numpy()
+            nhat = dc.noise_estimate().cpu().numpy()
+            scores = bbh.score().cpu().numpy() if bbh is not None else None
+            final = None
+        for i, orc in enumerate(oracles):
+            ref = orc.update(x[i][:, t * st_spec.stride:(t + 1) * st_spec.stride])
+            for d in range(st_spec.n_det):
+                tag = f"update {t} stream {i} det {d}"
+                _, w1 = util.check_network_output(pred[i, d], ref["pred"][d], "pred " + tag, elem=et)
+                stats["pred"] = max(stats["pred"], w1)
+                rms_n = ref["pred"][d]
+                if nhat is not None:
+                    _, w2 = util.check_network_output(nhat[i, d], ref["nhat_running"][d], "nhat " + tag, rms_ref=rms_n, elem=et)
+                    stats["nhat"] = max(stats["nhat"], w2)
+                    # reading A22: cleaned is judged against RMS(noise estimate), not against the strain
+                    util.check_network_output(running[i, d], ref["cleaned_running"][d], "cleaned " + tag, rms_ref=rms_n, elem=et)
+                if final is not None:
+                    util.check_network_output(final[i, d], ref["cleaned_final"][d], "final " + tag, rms_ref=rms_n, elem=et)
+            if scores is not None and check_scores:
+                assert abs(float(scores[i]) - ref["score"]) <= util.SCORE_ABS, (t, i, float(scores[i]), ref["score"])
+                stats["score"] = max(stats["score"], abs(float(scores[i]) - ref["score"]))
+    return stats
+
+
+@pytest.mark.parametrize("dtype", [gw.GW_BF16, gw.GW_FP16])
+def test_c0_streaming_deepclean_matches_oracle(dtype):
+    """configs[0]: 1 stream, 21 witnesses + strain, W=512, S=64, 32 updates, N(0,1) samples."""
+    cfg = S.config_c0()
+    stats = _run_streaming(cfg, dtype, cfg.n_updates, white=True)
+    print("C0 worst |d|/RMS:", stats)
+
+
+def test_c0_simt_cross_check_matches_oracle():
+    cfg = S.config_c0()
+    _run_streaming(cfg, gw.GW_BF16, 10, white=True, impl=gw.GW_IMPL_SIMT)
+
+
+def test_c0_last_stride_mode_and_latency_offset():
+    """PAPER.md:182 causal aggregation, PAPER.md:186 aggregation latency delta."""
+    cfg = S.config_c0()
+    _run_streaming(cfg, gw.GW_BF16, 14, white=True, agg=S.AGG_LAST_STRIDE, delta=0)
+    _run_streaming(cfg, gw.GW_BF16, 14, white=True, agg=S.AGG_LAST_STRIDE, delta=96)
+    _run_streaming(cfg, gw.GW_BF16, 14, white=True, agg=S.AGG_HANN_OLA, delta=128)
+
+
+# ------------------------------------------------------------------------ layer-by-layer check
+@pytest.mark.parametrize("dtype", [gw.GW_FP16, gw.GW_BF16])
+def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype):
+    """The full C1 network (21->32->64->128->256 and back, folded BatchNorm) on a 4096-sample window:
+    every stored activation against the oracle's, several M tiles and all channel widths."""
+    cfg = S.Config("C1-short", S.StreamSpec(2, 1, 4096, 4096, 512), S.config_c1().dc_layers, seed=1)
+    dc_params, _ = util.make_params(cfg)
+    dc_params2 = [dc_params[0]]
+    st = gw.Stream(cfg.stream)
+    dc = gw.DeepClean(st, cfg.dc_layers, dc_params2, dtype)
+    od, et = util.oracle_dtype(dtype), util.elem_tol(dtype)
+    n_up = 8
+    x = synth.multi_stream(3, cfg.stream, n_up * 512)
+    xd = _dev(x)
+    for t in range(n_up):
+        st.update(xd[:, :, t * 512:(t + 1) * 512].contiguous())
+        dc.forward()
+        dc.cleaned(gw.GW_FINAL)
+    prepared = [oracle.prepare_conv(l, p, od) for l, p in zip(cfg.dc_layers, dc_params2[0])]
+    for i in range(2):
+        snap, _ = oracle.snapshot(x[i], n_up - 1, 512, 4096)
+        ref_p, acts = oracle.deepclean_forward(snap[cfg.stream.witness_rows(0)].astype(np.float64), cfg.dc_layers,
+                                               prepared, return_all=True)
+        for li, (layer, ref) in enumerate(zip(cfg.dc_layers[:-1], acts[:-1])):
+            got = dc.activation(li).float().cpu().numpy()[i, 0]          # [L][Cp]
+            assert got.shape[0] == ref.shape[1]
+            assert np.all(got[:, layer.cout:] == 0.0), "padded channels must stay zero"
+            util.check_network_output(got[:, :layer.cout].T, ref, f"layer {li} stream {i}", elem=et)
+        pred = dc.noise().cpu().numpy()[i, 0]
+        util.check_network_output(pred, ref_p, f"prediction stream {i}", elem=et)
+        # against the storage-rounded oracle (diagnostic): what is left is implementation error only
+        # (fp32 accumulation order, hardware tanh, rounding flips it causes), far below the storage floor
+        ref_r = oracle.deepclean_forward(snap[cfg.stream.witness_rows(0)].astype(np.float64), cfg.dc_layers,
+                                         prepared, act_dtype=od)
+        util.check_network_output(pred, ref_r, f"prediction vs storage-rounded oracle, stream {i}",
+                                  elem=1.5e-2, rel_l2=3e-3)
+
+
+# ----------------------------------------------------------------------------- classifier (C2)
+@pytest.mark.parametrize("length,batch", [(4096, 24), (1024, 5)])
+def test_bbh_batch_matches_oracle(length, batch):
+    cfg = S.config_c2()
+    cp, dp = synth.bbh_params(202, cfg.bbh_convs, cfg.bbh_dense)
+    bbh = gw.Bbh(None, cfg.bbh_convs, cp, dp, length, gw.GW_BF16, n_det=2, max_batch=32)
+    x = synth.bbh_windows(2, batch, length)
+    got = bbh.score_batch(_dev(x)).cpu().numpy()
+    pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    ref = np.array([oracle.bbh_forward(x[i], cfg.bbh_convs, pc, pd) for i in range(batch)])
+    assert np.max(np.abs(got - ref)) <= util.SCORE_ABS, (got, ref)
+    assert np.std(ref) > 1e-3, "scores should not be degenerate"
+
+
+# -------------------------------------------------------------------- end-to-end small ensemble
+@pytest.mark.parametrize("dtype", [gw.GW_BF16, gw.GW_FP16])
+def test_small_ensemble_eager_matches_oracle(dtype):
+    cfg = S.config_small_ensemble(2)
+    stats = _run_streaming(cfg, dtype, cfg.n_updates, white=False)
+    print("ensemble worst:", stats)
+
+
+def test_small_ensemble_graph_matches_oracle_and_eager():
+    cfg = S.config_small_ensemble(2)
+    _run_streaming(cfg, gw.GW_BF16, cfg.n_updates, white=False, use_graph=True)
+
+
+def test_results_do_not_depend_on_batching():
+    """updates are serial per stream, streams are independent: stream i's results are
+    bit-identical whether it runs alone or batched with others."""
+    cfg2 = S.config_small_ensemble(3)
+    dc_params, bbh_params = util.make_params(cfg2)
+    x = synth.multi_stream(cfg2.seed, cfg2.stream, 6 * cfg2.stream.stride)
+    outs = {}
+    for which in ("all", 0, 2):
+        if which == "all":
+            cfg, xs = cfg2, x
+        else:
+            cfg, xs = S.config_small_ensemble(1), x[which:which + 1]
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, gw.GW_BF16)
+        xd = _dev(xs)
+        res = []
+        for t in range(6):
+            stream.update(xd[:, :, t * cfg.stream.stride:(t + 1) * cfg.stream.stride].contiguous())
+            dc.forward()
+            res.append((dc.cleaned(gw.GW_FINAL).cpu().numpy(), bbh.score().cpu().numpy()))
+        outs[which] = res
+    for which in (0, 2):
+        for t in range(6):
+            assert np.array_equal(outs["all"][t][0][which], outs[which][t][0][0])
+            assert outs["all"][t][1][which] == outs[which][t][1][0]
+
+
+def test_zero_network_returns_strain_bit_exact():
+    cfg = S.config_c0()
+    zero = [[{"w": np.zeros(l.wshape(), np.float32), "b": np.zeros(l.cout, np.float32)} for l in cfg.dc_layers]]
+    st = gw.Stream(cfg.stream)
+    dc = gw.DeepClean(st, cfg.dc_layers, zero, gw.GW_BF16)
+    x = synth.multi_stream(9, cfg.stream, 12 * 64, white=True)
+    xd = _dev(x)
+    for t in range(12):
+        st.update(xd[:, :, t * 64:(t + 1) * 64].contiguous())
+        dc.forward()
+        run = dc.cleaned(gw.GW_RUNNING).cpu().numpy()[0, 0]
+        first = (t + 1) * 64 - 512
+        lo = max(first, 0)
+        exp = x[0, cfg.stream.strain_row(0), lo:first + 512]
+        assert np.array_equal(run[lo - first:].view(np.uint32), exp.view(np.uint32))
+        assert np.all(run[:lo - first] == 0.0)
+
+
+def test_call_order_is_enforced():
+    cfg = S.config_c0()
+    dc_params, _ = util.make_params(cfg)
+    st = gw.Stream(cfg.stream)
+    dc = gw.DeepClean(st, cfg.dc_layers, dc_params, gw.GW_BF16)
+    new = torch.zeros((1, 22, 64), device="cuda")
+    with pytest.raises(gw.GwError) as e:
+        dc.forward()
+    assert e.value.code == gw.GW_ESTATE
+    st.update(new)
+    with pytest.raises(gw.GwError) as e:
+        st.update(new)
+    assert e.value.code == gw.GW_ESTATE
+    with pytest.raises(gw.GwError) as e:
+        dc.cleaned()
+    assert e.value.code == gw.GW_ESTATE
+    dc.forward()
+    with pytest.raises(gw.GwError) as e:
+        dc.forward()
+    assert e.value.code == gw.GW_ESTATE
+    dc.cleaned()
+    with pytest.raises(gw.GwError) as e:
+        dc.cleaned()
+    assert e.value.code == gw.GW_ESTATE
+    st.update(new)
