@@ -169,8 +169,9 @@ int gw_bbh_score_batch(gw_bbh *b, const float *windows_dev, int batch, float *sc
  *   update -> forward -> cleaned(GW_FINAL) -> score into a CUDA graph; later steps replay it (the ring
  *   head lives in device memory, so the graph is replayed unchanged).
  * gw_step: device buffers.  new_samples_dev [n][C][S]; scores_dev [n] (ignored without bbh);
- *   cleaned_final_dev [n][D][S].  The three pointers must be the same on every call of one
- *   pipeline (they are baked into the graph); otherwise GW_EINVAL.
+ *   cleaned_final_dev [n][D][S].  The pointers are baked into the graph: a different
+ *   new_samples_dev is a cheap node-parameter update, different output pointers re-capture.
+ *   `stream` must not be the legacy default stream.
  * gw_step_host: HOST buffers; copies new samples host->device, replays the graph, copies scores
  *   and final cleaned samples device->host, and synchronises.  Pinned host memory makes the copies
  *   asynchronous; pageable memory works but is slower. */
@@ -180,6 +181,15 @@ int gw_step(gw_pipeline *p, const float *new_samples_dev, float *scores_dev, flo
             void *stream);
 int gw_step_host(gw_pipeline *p, const float *new_samples_host, float *scores_host,
                  float *cleaned_final_host, void *stream);
+/* Profiling aid for bench.py: one update launched EAGERLY (same kernels, no graph) with a CUDA event
+ * after every kernel on `stream`; synchronises.  ms_out[i] (i < min(*n_out, max_kernels)) is the device
+ * time of kernel i, gw_profile_label(p, i) its name ("append", "gather", "gemm.dc0", ... "aggregate",
+ * "bbh_conv1", "gemm.bbh1", ...), gw_profile_flops(p, i) its algorithmic FLOPs (real channels and taps
+ * only, whole batch; 0 for non-GEMM kernels).  Counts as one update of the stream. */
+int gw_step_profile(gw_pipeline *p, const float *new_samples_dev, float *scores_dev, float *cleaned_final_dev,
+                    void *stream, int max_kernels, float *ms_out, int *n_out);
+const char *gw_profile_label(const gw_pipeline *p, int i);
+double gw_profile_flops(const gw_pipeline *p, int i);
 /* number of kernel nodes in the captured graph (0 before the first gw_step) */
 int gw_pipeline_graph_nodes(const gw_pipeline *p);
 

@@ -27,6 +27,7 @@ EXPORTS = [
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
     "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_pipeline_graph_nodes",
+    "gw_step_profile", "gw_profile_label", "gw_profile_flops",
 ]
 
 _FP = C.POINTER(C.c_float)
@@ -94,6 +95,11 @@ def lib():
         L.gw_step.argtypes = [vp, vp, vp, vp, vp]
         L.gw_step_host.argtypes = [vp, vp, vp, vp, vp]
         L.gw_pipeline_graph_nodes.argtypes = [vp]
+        L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_float), C.POINTER(i)]
+        L.gw_profile_label.argtypes = [vp, i]
+        L.gw_profile_label.restype = C.c_char_p
+        L.gw_profile_flops.argtypes = [vp, i]
+        L.gw_profile_flops.restype = C.c_double
         _lib = L
     return _lib
 
@@ -316,6 +322,15 @@ class Pipeline:
                 return C.c_void_p(0)
             return C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
         _check(lib().gw_step_host(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)))
+
+    def step_profile(self, new_samples, scores, cleaned_final, stream=None):
+        """One eager update with a CUDA event after each kernel -> [(label, ms, algorithmic flops)]."""
+        ms = (C.c_float * 64)()
+        n = C.c_int(0)
+        _check(lib().gw_step_profile(self.h, _ptr(new_samples), _ptr(scores), _ptr(cleaned_final),
+                                     _stream_ptr(stream), 64, ms, C.byref(n)))
+        return [(lib().gw_profile_label(self.h, i).decode(), float(ms[i]), float(lib().gw_profile_flops(self.h, i)))
+                for i in range(min(n.value, 64))]
 
     def graph_nodes(self) -> int:
         return int(lib().gw_pipeline_graph_nodes(self.h))

@@ -57,6 +57,7 @@ cudaError_t conv_gemm_prepare();   // opt-in shared-memory attribute
 // ---- bandwidth / CUDA-core kernels (gw_kernels.cu) -------------------------------------------
 void launch_append(float* ring, const float* new_samples, long long* count, unsigned* ticket, int n_rows,
                    int W, int S, cudaStream_t st);
+bool is_append_kernel(const void* func);   // identifies the a1 node of a captured graph
 void launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st);
 void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
                    int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st);

@@ -164,6 +164,27 @@ static int fold_layer(const gw_conv_layer& L, HostLayer& H) {
 
 static int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
+// Per-launch CUDA-event profiler (gw_step_profile): when armed, every enqueue helper drops an event
+// after each kernel it launches.
+struct Prof {
+    std::vector<cudaEvent_t> ev;
+    std::vector<std::string> labels;
+    int n = 0;
+};
+static Prof* g_prof = nullptr;
+static void prof_mark(const char* label, cudaStream_t st) {
+    if (!g_prof) return;
+    if (g_prof->n >= static_cast<int>(g_prof->ev.size())) {
+        cudaEvent_t e;
+        cudaEventCreate(&e);
+        g_prof->ev.push_back(e);
+        g_prof->labels.push_back("");
+    }
+    cudaEventRecord(g_prof->ev[g_prof->n], st);
+    g_prof->labels[g_prof->n] = label;
+    g_prof->n += 1;
+}
+
 // ------------------------------------------------------------------------------------ handles
 struct gw_stream {
     int n, C, fs, W, S;
@@ -181,6 +202,8 @@ struct GemmLayer {
     void* d_B = nullptr;
     float* d_bias = nullptr;
     int impl = GW_IMPL_UMMA;
+    std::string name;                            // profiler label, e.g. "gemm.dc3"
+    double flops = 0.0;                          // algorithmic FLOPs per batch item (real channels and taps only)
 };
 
 struct gw_deepclean {
@@ -230,11 +253,13 @@ struct gw_pipeline {
     gw_bbh* bbh = nullptr;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
+    cudaGraphNode_t append_node = nullptr;
     int nodes = 0;
     const float* cap_in = nullptr;
     float* cap_scores = nullptr;
     float* cap_final = nullptr;
     float *d_in = nullptr, *d_scores = nullptr, *d_final = nullptr;   // staging for gw_step_host
+    Prof prof;
 };
 
 // ------------------------------------------------------------------------------ GEMM layer build
@@ -327,6 +352,7 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
 static void run_gemm(const GemmLayer& gl, cudaStream_t st) {
     if (gl.impl == GW_IMPL_UMMA) launch_conv_gemm_umma(gl.g, st);
     else launch_conv_gemm_simt(gl.g, st);
+    prof_mark(gl.name.c_str(), st);
 }
 
 static void free_gemm(GemmLayer& gl) {
@@ -374,6 +400,7 @@ static int stream_update_checked(gw_stream* s) {
 }
 static void stream_update_enqueue(gw_stream* s, const float* src, cudaStream_t st) {
     launch_append(s->ring, src, s->d_count, s->d_ticket, s->n * s->C, s->W, s->S, st);
+    prof_mark("append", st);
 }
 
 extern "C" int gw_stream_update(gw_stream* s, const float* new_samples_dev, void* stream) {
@@ -473,6 +500,11 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, dc->act[i], len[i], cpad[i],
                                       dc->act[i + 1], cpad[i + 1], batch, EPI_STORE))
             return rc;
+        dc->gemm[i].name = "gemm.dc" + std::to_string(i);
+        // useful MACs: every (input position, tap, cin, cout) product of the layer definition
+        const HostLayer& H = dc->host[i];
+        const double lin = len[i];
+        dc->gemm[i].flops = 2.0 * (H.kind == GW_CONV ? lin / 2 : lin) * H.k * H.cin * H.cout;
     }
     // final layer on CUDA cores: wt[d][j][ci] fp32 holding storage-rounded weights
     {
@@ -559,9 +591,11 @@ static void deepclean_forward_enqueue(gw_deepclean* dc, cudaStream_t st) {
     gw_stream* s = dc->s;
     launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
                   dc->act_cols[0], dc->fmt, st);
+    prof_mark("gather", st);
     for (auto& g : dc->gemm) run_gemm(g, st);
     launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
                        dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
+    prof_mark("final_convt", st);
 }
 
 extern "C" int gw_deepclean_forward(gw_deepclean* dc, void* stream) {
@@ -605,6 +639,7 @@ static void cleaned_enqueue(gw_deepclean* dc, float* final_out, float* running_o
     a.n_streams = s->n; a.n_det = dc->n_det; a.channels = s->C; a.W = s->W; a.S = s->S; a.Lb = dc->Lb;
     a.delta = dc->delta; a.agg = dc->agg;
     launch_aggregate(a, st);
+    prof_mark("aggregate", st);
 }
 
 extern "C" int gw_cleaned_strain(gw_deepclean* dc, float* out_dev, int mode, void* stream) {
@@ -705,6 +740,8 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
         if (int rc = build_gemm_layer(gl, GK_BBH, &H[i], 1, b->fmt, b->act[i - 1], len[i - 1], cp[i - 1],
                                       last ? nullptr : b->act[i], cout_p, b->batch, last ? EPI_POOL_HEAD : EPI_POOL))
             return rc;
+        gl.name = "gemm.bbh" + std::to_string(i);
+        gl.flops = 2.0 * len[i - 1] * H[i].k * H[i].cin * H[i].cout;
         if (last) {
             ConvGemmParams& p = gl.g.p;
             p.hw1 = b->d_hw1; p.hb1 = b->d_hb1; p.hw2 = b->d_hw2; p.hb2 = b->d_hb2; p.head_hidden = hidden;
@@ -748,6 +785,7 @@ extern "C" int gw_bbh_create(gw_bbh** out, gw_deepclean* dc, const gw_bbh_spec* 
 static void bbh_enqueue(gw_bbh* b, const float* in, int batch, cudaStream_t st) {
     launch_bbh_conv1(in, b->d_w1, b->d_b1, b->act[0], batch, b->n_det, b->L, b->c1.cout, b->c1_cpad, b->c1.k,
                      b->c1.pad_l, b->c1.pool, b->fmt, st);
+    prof_mark("bbh_conv1", st);
     for (auto& g : b->gemm) {
         GemmLayer gl = g;
         gl.g.batch = batch;
@@ -794,6 +832,7 @@ extern "C" int gw_pipeline_destroy(gw_pipeline* p) {
     if (p->exec) cudaGraphExecDestroy(p->exec);
     if (p->graph) cudaGraphDestroy(p->graph);
     cudaFree(p->d_in); cudaFree(p->d_scores); cudaFree(p->d_final);
+    for (cudaEvent_t e : p->prof.ev) cudaEventDestroy(e);
     delete p;
     return GW_OK;
 }
@@ -818,6 +857,33 @@ static int pipeline_capture(gw_pipeline* p, const float* in, float* scores, floa
     if (e != cudaSuccess) return fail(GW_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
     CU_TRY(cudaGraphInstantiate(&p->exec, p->graph, 0));
     p->cap_in = in; p->cap_scores = scores; p->cap_final = fin;
+    // remember the append node: a new input pointer is then a parameter update, not a re-capture
+    p->append_node = nullptr;
+    size_t n_nodes = 0;
+    CU_TRY(cudaGraphGetNodes(p->graph, nullptr, &n_nodes));
+    std::vector<cudaGraphNode_t> nodes(n_nodes);
+    CU_TRY(cudaGraphGetNodes(p->graph, nodes.data(), &n_nodes));
+    for (cudaGraphNode_t nd : nodes) {
+        cudaGraphNodeType ty;
+        CU_TRY(cudaGraphNodeGetType(nd, &ty));
+        if (ty != cudaGraphNodeTypeKernel) continue;
+        cudaKernelNodeParams kp;
+        CU_TRY(cudaGraphKernelNodeGetParams(nd, &kp));
+        if (is_append_kernel(kp.func)) { p->append_node = nd; break; }
+    }
+    return GW_OK;
+}
+
+static int pipeline_set_input(gw_pipeline* p, const float* in) {
+    cudaKernelNodeParams kp;
+    CU_TRY(cudaGraphKernelNodeGetParams(p->append_node, &kp));
+    void* args[7];
+    for (int i = 0; i < 7; ++i) args[i] = kp.kernelParams[i];
+    const float* src = in;
+    args[1] = &src;                                     // k_append(ring, src, count, ticket, n_rows, W, S)
+    kp.kernelParams = args;
+    CU_TRY(cudaGraphExecKernelNodeSetParams(p->exec, p->append_node, &kp));
+    p->cap_in = in;
     return GW_OK;
 }
 
@@ -825,9 +891,12 @@ extern "C" int gw_step(gw_pipeline* p, const float* new_samples_dev, float* scor
     if (!p || !new_samples_dev || !cleaned_final_dev || (p->bbh && !scores_dev)) return fail(GW_EINVAL, "gw_step: NULL argument");
     if (int rc = stream_update_checked(p->s)) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (!p->exec || p->cap_in != new_samples_dev || p->cap_scores != scores_dev || p->cap_final != cleaned_final_dev) {
+    if (!p->exec || p->cap_scores != scores_dev || p->cap_final != cleaned_final_dev ||
+        (p->cap_in != new_samples_dev && !p->append_node)) {
         if (st == nullptr) return fail(GW_EINVAL, "gw_step needs a non-default stream (graph capture)");
         if (int rc = pipeline_capture(p, new_samples_dev, scores_dev, cleaned_final_dev, st)) return rc;
+    } else if (p->cap_in != new_samples_dev) {
+        if (int rc = pipeline_set_input(p, new_samples_dev)) return rc;
     }
     CU_TRY(cudaGraphLaunch(p->exec, st));
     g_kernel_launches += p->nodes;
@@ -835,6 +904,51 @@ extern "C" int gw_step(gw_pipeline* p, const float* new_samples_dev, float* scor
     p->dc->forward_for = p->dc->cleaned_for = p->s->updates;
     if (p->bbh) p->bbh->scored_for = p->s->updates;
     return GW_OK;
+}
+
+// One update, launched eagerly (no graph) with a CUDA event after every kernel; synchronises.
+extern "C" int gw_step_profile(gw_pipeline* p, const float* new_samples_dev, float* scores_dev, float* cleaned_final_dev,
+                               void* stream, int max_kernels, float* ms_out, int* n_out) {
+    if (!p || !new_samples_dev || !cleaned_final_dev || !ms_out || !n_out || (p->bbh && !scores_dev))
+        return fail(GW_EINVAL, "gw_step_profile: NULL argument");
+    if (int rc = stream_update_checked(p->s)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Prof& pr = p->prof;
+    pr.n = 0;
+    g_prof = &pr;
+    prof_mark("begin", st);
+    stream_update_enqueue(p->s, new_samples_dev, st);
+    deepclean_forward_enqueue(p->dc, st);
+    cleaned_enqueue(p->dc, cleaned_final_dev, nullptr, nullptr, st);
+    if (p->bbh) {
+        bbh_enqueue(p->bbh, p->bbh->in_buf, p->bbh->batch, st);
+        cudaMemcpyAsync(scores_dev, p->bbh->scores_buf, static_cast<size_t>(p->bbh->batch) * 4, cudaMemcpyDeviceToDevice, st);
+    }
+    g_prof = nullptr;
+    CU_TRY(cudaGetLastError());
+    CU_TRY(cudaStreamSynchronize(st));
+    p->s->updates += 1;
+    p->dc->forward_for = p->dc->cleaned_for = p->s->updates;
+    if (p->bbh) p->bbh->scored_for = p->s->updates;
+    const int nk = pr.n - 1;
+    *n_out = nk;
+    for (int i = 0; i < nk && i < max_kernels; ++i) CU_TRY(cudaEventElapsedTime(&ms_out[i], pr.ev[i], pr.ev[i + 1]));
+    return GW_OK;
+}
+
+extern "C" const char* gw_profile_label(const gw_pipeline* p, int i) {
+    if (!p || i < 0 || i + 1 >= p->prof.n) return "";
+    return p->prof.labels[i + 1].c_str();
+}
+
+// Algorithmic FLOPs of kernel i of the last profiled step (0 for non-GEMM kernels): real channels and
+// taps only, summed over the batch.
+extern "C" double gw_profile_flops(const gw_pipeline* p, int i) {
+    if (!p) return 0.0;
+    const std::string lab = gw_profile_label(p, i);
+    for (auto& g : p->dc->gemm) if (g.name == lab) return g.flops * p->dc->batch;
+    if (p->bbh) for (auto& g : p->bbh->gemm) if (g.name == lab) return g.flops * p->bbh->batch;
+    return 0.0;
 }
 
 extern "C" int gw_step_host(gw_pipeline* p, const float* new_samples_host, float* scores_host, float* cleaned_final_host, void* stream) {

@@ -86,6 +86,10 @@ void launch_append(float* ring, const float* new_samples, long long* count, unsi
     ++g_kernel_launches;
 }
 
+bool is_append_kernel(const void* func) {
+    return func == reinterpret_cast<const void*>(&k_append<4>) || func == reinterpret_cast<const void*>(&k_append<1>);
+}
+
 // Test hook: time-ordered read-out of the ring, out[row][n] = ring[row][(count + n) mod W].
 __global__ void __launch_bounds__(256) k_snapshot(const float* __restrict__ ring, float* __restrict__ out,
                                                   const long long* count, int n_rows, int W) {

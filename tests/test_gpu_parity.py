@@ -19,7 +19,7 @@ def _dev(a):
 
 
 # ------------------------------------------------------------------------------- a1 snapshot
-@pytest.mark.parametrize("n,C,W,S", [(1, 22, 512, 64), (3, 5, 96, 7), (2, 44, 4096, 512), (2, 3, 10, 10),
+@pytest.mark.parametrize("n,C,W,S_", [(1, 22, 512, 64), (3, 5, 96, 7), (2, 44, 4096, 512), (2, 3, 10, 10),
                                       (1, 2, 33, 1), (4, 4, 64, 12), (1, 22, 32768, 1024)])
 def test_snapshot_bit_exact(n, C, W, S_):
     spec = S.StreamSpec(n, 1, 512, W, S_, n_witness=C - 1)
@@ -92,6 +92,7 @@ def _run_streaming(cfg, dtype, n_up, white, agg=S.AGG_HANN_OLA, delta=0, check_s
                     util.check_network_output(final[i, d], ref["cleaned_final"][d], "final " + tag, rms_ref=rms_n, elem=et)
             if scores is not None and check_scores:
                 assert abs(float(scores[i]) - ref["score"]) <= util.SCORE_ABS, (t, i, float(scores[i]), ref["score"])
+                assert abs(util.logit(scores[i]) - util.logit(ref["score"])) <= util.LOGIT_ABS, (t, i, float(scores[i]), ref["score"])
                 stats["score"] = max(stats["score"], abs(float(scores[i]) - ref["score"]))
     return stats
 
@@ -144,22 +145,26 @@ def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype):
             got = dc.activation(li).float().cpu().numpy()[i, 0]          # [L][Cp]
             assert got.shape[0] == ref.shape[1]
             assert np.all(got[:, layer.cout:] == 0.0), "padded channels must stay zero"
-            util.check_network_output(got[:, :layer.cout].T, ref, f"layer {li} stream {i}", elem=et)
+            # internal activations carry their own storage rounding on top of the propagated error; an
+            # indexing bug would be O(1), so bf16 layers get a loose per-element bar here (outputs: `et`)
+            util.check_network_output(got[:, :layer.cout].T, ref, f"layer {li} stream {i}",
+                                      elem=1e-1 if dtype == gw.GW_BF16 else et)
         pred = dc.noise().cpu().numpy()[i, 0]
         util.check_network_output(pred, ref_p, f"prediction stream {i}", elem=et)
         # against the storage-rounded oracle (diagnostic): what is left is implementation error only
         # (fp32 accumulation order, hardware tanh, rounding flips it causes), far below the storage floor
         ref_r = oracle.deepclean_forward(snap[cfg.stream.witness_rows(0)].astype(np.float64), cfg.dc_layers,
                                          prepared, act_dtype=od)
-        util.check_network_output(pred, ref_r, f"prediction vs storage-rounded oracle, stream {i}",
-                                  elem=1.5e-2, rel_l2=3e-3)
+        r = util.check_network_output(pred, ref_r, f"prediction vs storage-rounded oracle, stream {i}",
+                                      elem=et, rel_l2=3e-3)   # a rare rounding flip costs one full ulp
+        print(f"dtype {dtype} stream {i}: vs storage-rounded oracle rel L2 {r[0]:.2e}, worst/RMS {r[1]:.2e}")
 
 
 # ----------------------------------------------------------------------------- classifier (C2)
 @pytest.mark.parametrize("length,batch", [(4096, 24), (1024, 5)])
 def test_bbh_batch_matches_oracle(length, batch):
     cfg = S.config_c2()
-    cp, dp = synth.bbh_params(202, cfg.bbh_convs, cfg.bbh_dense)
+    cp, dp = util.centred_bbh_params(202, cfg.bbh_convs, cfg.bbh_dense, length)
     bbh = gw.Bbh(None, cfg.bbh_convs, cp, dp, length, gw.GW_BF16, n_det=2, max_batch=32)
     x = synth.bbh_windows(2, batch, length)
     got = bbh.score_batch(_dev(x)).cpu().numpy()
@@ -167,7 +172,10 @@ def test_bbh_batch_matches_oracle(length, batch):
     pd = [oracle.prepare_dense(p) for p in dp]
     ref = np.array([oracle.bbh_forward(x[i], cfg.bbh_convs, pc, pd) for i in range(batch)])
     assert np.max(np.abs(got - ref)) <= util.SCORE_ABS, (got, ref)
-    assert np.std(ref) > 1e-3, "scores should not be degenerate"
+    assert np.max(np.abs(util.logit(got) - util.logit(ref))) <= util.LOGIT_ABS, (got, ref)
+    assert 0.2 < np.mean(ref) < 0.8 and np.std(ref) > 1e-2, "scores should not be degenerate"
+    print("bbh scores: max |d| %.2e, max |d logit| %.2e, ref range %.3f..%.3f" % (
+        np.max(np.abs(got - ref)), np.max(np.abs(util.logit(got) - util.logit(ref))), ref.min(), ref.max()))
 
 
 # -------------------------------------------------------------------- end-to-end small ensemble

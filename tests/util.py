@@ -32,10 +32,33 @@ def oracle_dtype(dtype: int) -> int:
     return oracle.DT_BF16 if dtype == 0 else oracle.DT_FP16
 
 
+LOGIT_ABS = 2e-2      # |d score| <= 5e-3 at the steepest point of the sigmoid <=> |d logit| <= 2e-2
+
+
+def centred_bbh_params(seed: int, convs, dense, length: int, dtype: int = 0):
+    """Random classifier weights put every score near sigmoid(-4), where the 5e-3 score bar would
+    accept almost anything.  Shift the last dense bias (a parameter, i.e. an input handed to both
+    sides) so that the oracle's mean logit over a few noise windows is 0: scores then spread around
+    0.5, where the bar bites."""
+    cp, dp = synth.bbh_params(seed, convs, dense)
+    od = oracle_dtype(dtype)
+    pc = [oracle.prepare_conv(l, p, od) for l, p in zip(convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    x = synth.bbh_windows(seed + 1, 4, length)
+    mean_logit = float(np.mean([oracle.bbh_forward(x[i], convs, pc, pd, return_logit=True) for i in range(4)]))
+    dp[-1]["b"] = (dp[-1]["b"] - np.float32(mean_logit)).astype(np.float32)
+    return cp, dp
+
+
+def logit(p):
+    p = np.asarray(p, dtype=np.float64)
+    return np.log(p / (1.0 - p))
+
+
 def make_params(cfg: S.Config):
     st = cfg.stream
     dc = [synth.deepclean_params(cfg.seed * 100 + d, cfg.dc_layers) for d in range(st.n_det)] if cfg.dc_layers else []
-    bbh = synth.bbh_params(cfg.seed * 100 + 50, cfg.bbh_convs, cfg.bbh_dense) if cfg.bbh_convs else None
+    bbh = centred_bbh_params(cfg.seed * 100 + 50, cfg.bbh_convs, cfg.bbh_dense, cfg.bbh_len) if cfg.bbh_convs else None
     return dc, bbh
 
 
