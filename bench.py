@@ -236,6 +236,13 @@ def run_native(args):
     ds_per_step = sp.n_streams * sp.stride / FS
     value = world * K * ds_per_step / (ms_total / 1e3)
 
+    if args.timed_only:
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K,
+                              "warmup": W_, "ms_per_step": ms_total / K, "gpu_launches": int(launches),
+                              "note": "--timed-only run (profiling aid), not a bench line"}), flush=True)
+        return
+
     # per-update latency: launch -> stream sync, host clock, one sample per update
     lat = []
     for _ in range(min(max(K, 50), 400)):
@@ -336,6 +343,8 @@ def main():
     ap.add_argument("--stride", type=int, default=512)
     ap.add_argument("--dtype", default="fp16", choices=["fp16", "bf16"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--timed-only", action="store_true",
+                    help="only the warm-up and the timed region (for short runs under ncu); prints a reduced line")
     ap.add_argument("--reference-budget", type=float, default=150.0,
                     help="--impl reference stops after this many seconds of oracle time (a bounded sample)")
     args = ap.parse_args()

@@ -16,11 +16,16 @@ enum { FMT_FP16 = 0, FMT_BF16 = 1 };                       // UMMA instruction-d
 enum { EPI_STORE = 0, EPI_POOL = 1, EPI_POOL_HEAD = 2 };
 enum { ACT_NONE = 0, ACT_TANH = 1, ACT_RELU = 2 };
 
-// One convolution layer expressed as   D[m][n] = sum_s  A[m + shift_s][col_s .. col_s+64) . B[n][64 s .. 64 s+64)
-// where A is a 2-D view [rows][cols] of a channels-last activation tensor per batch item (rows out
-// of range read as zero = the layer's zero padding) and B is the per-detector weight matrix.
+constexpr int kMaxCb = 8;          // 64-column blocks of the A view (a_cols <= 512)
+constexpr int kMaxShift = 6;       // distinct row shifts of one layer
+
+// One convolution layer expressed as
+//     D[m][n] = sum over segments (cb, a):  A[m + a][64 cb .. 64 cb + 64) . B[n][64 s .. 64 s + 64),  s = seg_of[cb][a - a_min]
+// where A is a 2-D view [rows][cols] of a channels-last activation tensor per batch item (rows out of
+// range read as zero = the layer's zero padding) and B is the per-detector weight matrix whose K order
+// is the segment order (cb outer, shift inner).
 struct ConvGemmParams {
-    CUtensorMap tmA;               // 3-D (cols, rows, batch), box (64, 128, 1), SWIZZLE_128B
+    CUtensorMap tmA;               // 3-D (cols, rows, batch), box (64, slab_rows, 1), SWIZZLE_128B
     CUtensorMap tmB;               // 3-D (K = 64 n_seg, N, n_det), box (64, N, 1), SWIZZLE_128B
     const void* A;                 // raw pointers of the same operands (SIMT cross-check kernel)
     const void* B;
@@ -31,6 +36,11 @@ struct ConvGemmParams {
     int n_det;                     // weight set = batch % n_det
     int fmt;                       // FMT_*
     int epi, act;
+    int n_cb, a_min, n_shift;      // column blocks, first row shift, number of row shifts
+    int slab_rows;                 // 128 + n_shift - 1: rows of A one output tile needs
+    int b_resident;                // 1: all of B lives in shared memory for the CTA's lifetime
+    int sa_stages, sb_stages;      // A-slab ring depth, B ring depth (streaming mode)
+    int tiles_m;                   // ceil(M / 128)
     const float* bias;             // [n_det][N]
     void* out;                     // EPI_STORE: [batch][M][N]; EPI_POOL: [batch][M/2][N/2], 16-bit
     // EPI_POOL_HEAD: global average pool over the M/2 pooled rows, dense head, sigmoid
@@ -38,20 +48,22 @@ struct ConvGemmParams {
     int head_hidden;
     float* scores;                 // [batch]
     float* pooled_dbg;             // optional [batch][M/2][N/2] fp32 (SIMT path scratch)
-    int8_t seg_shift[kMaxSeg];
+    int8_t seg_of[kMaxCb][kMaxShift];     // B K-block of segment (cb, shift), -1 if the segment is empty
+    int8_t seg_shift[kMaxSeg];     // per segment s: row shift, first column (SIMT kernel)
     int16_t seg_col[kMaxSeg];
 };
 
 struct GemmLaunch {
     ConvGemmParams p;
-    int batch;
-    int stages;
+    int batch;                     // n_items * n_det
     int smem_bytes;
+    int grid;                      // persistent CTAs (multiple of n_det)
 };
 
 void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st);
 void launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st);
-int conv_gemm_smem_bytes(int N, int stages);
+// Chooses resident/streaming B, ring depths and the shared-memory size for a layer; false if it cannot fit.
+bool conv_gemm_plan(GemmLaunch& g, int sm_count);
 cudaError_t conv_gemm_prepare();   // opt-in shared-memory attribute
 
 // ---- bandwidth / CUDA-core kernels (gw_kernels.cu) -------------------------------------------

@@ -1,19 +1,25 @@
 // gw_conv_gemm.cu -- every Conv1d / ConvTranspose1d layer with enough channels as an implicit GEMM on
-// the 5th-generation tensor cores (tcgen05.mma, accumulator in TMEM, operands staged by TMA).
+// the 5th-generation tensor cores (tcgen05.mma, accumulators in TMEM, operands staged by TMA).
 //
-//   D[m][n] = sum_s  A[m + shift_s][col_s .. col_s + 64) . B[n][64 s .. 64 s + 64)
+//   D[m][n] = sum over segments (cb, a):  A[m + a][64 cb .. 64 cb + 64) . B[n][64 s .. 64 s + 64)
 //
 // A is a 2-D view of the channels-last input activation of one (stream, detector):
 //   stride-2 Conv1d (encoder):   rows = L/2 position pairs, cols = 2 Cin (even | odd position)
 //   stride-2 ConvTranspose1d:    rows = L positions,        cols = Cin; N = (even | odd output) x Cout
 //   stride-1 Conv1d + pool 4:    rows = L/2 position pairs, cols = 2 Cin; N = (even | odd output) x Cout
-// so every tap is a row-shifted rectangular tile that one TMA box load fetches, and the layer's zero
-// padding is TMA's out-of-bounds fill (the batch index is the third tensor dimension, so a shifted
-// tile never bleeds into the neighbouring window).  B is the per-detector weight matrix, K-major,
-// built on the host at create time.
+// so every filter tap is a ROW-SHIFTED rectangular tile of the same matrix.  One output tile of 128 rows
+// therefore needs a slab of 128 + (shifts - 1) input rows per 64-column block; the slab is fetched ONCE by
+// one TMA box load (the layer's zero padding is TMA's out-of-bounds fill; the batch index is the third
+// tensor dimension, so a slab never bleeds into the neighbouring window) and every tap's MMA reads it
+// through a shared-memory descriptor whose start address is advanced by whole 128-byte rows.
 //
-// Warp roles (192 threads): warp 0 = TMA producer (+ TMEM alloc/dealloc), warp 1 = MMA issuer (one
-// thread), warps 2..5 = epilogue (TMEM -> registers -> bias/activation/pool -> 16-bit global).
+// The kernel is persistent and warp-specialised (320 threads, one CTA per SM):
+//   warp 0    TMA producer: A slabs (ring of sa_stages), B K-blocks (resident once, or a ring of sb_stages)
+//   warp 1    MMA issuer (one thread): tcgen05.mma into one of TWO TMEM accumulator stages
+//   warps 2-9 epilogue: TMEM -> registers -> bias / activation / pool / head -> 16-bit global, overlapping
+//             the next stage's MMAs
+// CTA c serves detector c % n_det (each detector has its own weights) and walks that detector's tiles
+// with stride gridDim.x / n_det.
 #include <stdio.h>
 
 #include "gw_common.cuh"
@@ -21,16 +27,64 @@
 
 namespace gw {
 
-constexpr int kGemmThreads = 192;
-constexpr int kABytes = kTileM * 128;   // 128 rows x 128 bytes
+constexpr int kEpiWarps = 8;
+constexpr int kGemmThreads = 64 + kEpiWarps * 32;   // producer warp, MMA warp, 8 epilogue warps
+constexpr int kAccCols = 256;                        // TMEM columns of one accumulator stage
+constexpr int kSmemBudget = 225 * 1024;
+constexpr int kFixedSmem = 1024 /*alignment slack*/ + 1024 /*bias*/ + 1024 /*barriers, tmem slot*/;
 
-int conv_gemm_smem_bytes(int N, int stages) { return stages * (kABytes + N * 128) + 1024 /*align*/ + 256 /*barriers*/; }
+__host__ __device__ __forceinline__ int slab_bytes_of(int slab_rows) { return (slab_rows * 128 + 1023) & ~1023; }
+__host__ __device__ __forceinline__ int head_scratch_bytes(int N, int hidden) {
+    return ((64 * (N / 2 + 1) + N / 2 + hidden) * 4 + 1023) & ~1023;
+}
+
+bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
+    ConvGemmParams& p = g.p;
+    const int b_block = p.N * 128;
+    const int sl = slab_bytes_of(p.slab_rows);
+    const int fixed = kFixedSmem + (p.epi == EPI_POOL_HEAD ? head_scratch_bytes(p.N, p.head_hidden) : 0);
+    int b_bytes;
+    if (p.n_seg * b_block <= 132 * 1024 && fixed + p.n_seg * b_block + 2 * sl <= kSmemBudget) {
+        p.b_resident = 1; p.sb_stages = 0; b_bytes = p.n_seg * b_block;
+    } else {
+        p.b_resident = 0;
+        p.sb_stages = p.n_seg < 4 ? p.n_seg : 4;
+        while (p.sb_stages > 1 && fixed + p.sb_stages * b_block + 2 * sl > kSmemBudget) p.sb_stages--;
+        b_bytes = p.sb_stages * b_block;
+    }
+    int sa = (kSmemBudget - fixed - b_bytes) / sl;
+    if (sa < 2) return false;
+    if (sa > 8) sa = 8;
+    p.sa_stages = sa;
+    g.smem_bytes = fixed + b_bytes + sa * sl;
+    g.grid = sm_count - sm_count % p.n_det;
+    return true;
+}
+
+template <int ACT>
+__device__ __forceinline__ float act_apply_t(float v) {
+    if (ACT == ACT_TANH) {
+        const float e = __expf(2.f * v);
+        return 1.f - __fdividef(2.f, 1.f + e);
+    }
+    if (ACT == ACT_RELU) return fmaxf(v, 0.f);
+    return v;
+}
+template <int FMT>
+__device__ __forceinline__ uint32_t pack_pair_t(float a, float b) {
+    if (FMT == FMT_BF16) {
+        __nv_bfloat162 v = __floats2bfloat162_rn(a, b);
+        return *reinterpret_cast<uint32_t*>(&v);
+    }
+    __half2 v = __floats2half2_rn(a, b);
+    return *reinterpret_cast<uint32_t*>(&v);
+}
 
 __device__ __forceinline__ float act_apply(float v, int act) {
     if (act == ACT_TANH) {
         // tanh(v) = 1 - 2/(1 + e^{2v}): two MUFU ops (ex2, rcp), absolute error ~1e-7.  The one-op
         // tanh.approx.f32 (relative error 2^-11) is as large as a bf16 rounding step and 4x an fp16 one,
-        // and it flips ~10% of the storage roundings; the epilogue is not the bottleneck.
+        // and it flips ~10% of the storage roundings.
         const float e = __expf(2.f * v);
         return 1.f - __fdividef(2.f, 1.f + e);
     }
@@ -47,39 +101,63 @@ __device__ __forceinline__ uint32_t pack_pair(float a, float b, int fmt) {
     return *reinterpret_cast<uint32_t*>(&v);
 }
 
+// Row-shifted operand views: a descriptor whose start address is advanced by whole 128-byte rows inside
+// a 1024-byte aligned SWIZZLE_128B slab needs NO base-offset (bits 49-51 stay 0): the tensor core
+// derives the swizzle phase from the absolute shared-memory address bits, exactly as TMA did when it
+// wrote the slab.  Measured on B200: base_offset = 0 matches the oracle, base_offset = (addr >> 7) & 7
+// gives garbage (profiles/r01_notes.md).
+
+// EPI / ACT / FMT are compile-time so that the per-element epilogue loop is straight-line code the
+// compiler can unroll and interleave (with run-time branches inside it, each element's MUFU latency
+// chain was exposed: ~120 cycles per element with only four epilogue warps to hide it).
+//
+// One accumulator stage is kAccCols = 256 TMEM columns and holds G = 256 / N consecutive output tiles
+// (EPI_STORE; G = 1 for the pooled epilogues), so that thin layers (N = 32, 64) hand over 8 or 4 tiles
+// per mbarrier round trip instead of one.  Two stages (512 columns) double-buffer MMA against epilogue.
+template <int EPI, int ACT, int FMT>
 __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid_constant__ ConvGemmParams p,
-                                                                    int stages) {
+                                                                    int n_items) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int b_bytes = p.N * 128;
-    const int stage_bytes = kABytes + b_bytes;
-    uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + stages * stage_bytes);
-    uint64_t* empty_bar = full_bar + stages;
-    uint64_t* tmem_full_bar = empty_bar + stages;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_full_bar + 1);
+    const int b_block = p.N * 128;
+    const int sl = slab_bytes_of(p.slab_rows);
+    const int sa = p.sa_stages, sb = p.sb_stages;
+    uint8_t* smem_b = smem;
+    uint8_t* smem_a = smem_b + (p.b_resident ? p.n_seg : sb) * b_block;
+    uint8_t* after_a = smem_a + sa * sl;
+    float* bias_s = reinterpret_cast<float*>(after_a);                       // [N]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(after_a + 1024);
+    uint64_t* a_full = bars;                 // [sa]
+    uint64_t* a_empty = a_full + 8;          // [sa]
+    uint64_t* b_full = a_empty + 8;          // [sb]
+    uint64_t* b_empty = b_full + 4;          // [sb]
+    uint64_t* bres_bar = b_empty + 4;        // [1]
+    uint64_t* tmem_full = bres_bar + 1;      // [2]
+    uint64_t* tmem_empty = tmem_full + 2;    // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+    float* head_s = reinterpret_cast<float*>(after_a + 2048);                // EPI_POOL_HEAD scratch
 
     const int warp = threadIdx.x / 32;
     const int lane = threadIdx.x % 32;
-    const int m0 = blockIdx.x * kTileM;
-    const int batch = blockIdx.y;
-    const int det = batch % p.n_det;
-
-    uint32_t tmem_cols = 32;
-    while (tmem_cols < static_cast<uint32_t>(p.N)) tmem_cols <<= 1;
+    const int det = blockIdx.x % p.n_det;
+    const int worker = blockIdx.x / p.n_det;
+    const int n_workers = gridDim.x / p.n_det;
+    const int G = (EPI == EPI_STORE) ? kAccCols / p.N : 1;                   // tiles per accumulator stage
+    const int spi = (p.tiles_m + G - 1) / G;                                 // super-tiles per batch item
+    const int total = n_items * spi;
 
     if (warp == 0) {
         if (lane == 0) {
             tma_prefetch_desc(&p.tmA);
             tma_prefetch_desc(&p.tmB);
-            for (int i = 0; i < stages; ++i) {
-                mbar_init(&full_bar[i], 1);
-                mbar_init(&empty_bar[i], 1);
-            }
-            mbar_init(tmem_full_bar, 1);
+            for (int i = 0; i < sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
+            for (int i = 0; i < sb; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
+            mbar_init(bres_bar, 1);
+            for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full[i], 1); mbar_init(&tmem_empty[i], kEpiWarps); }
             fence_barrier_init();
         }
         __syncwarp();
-        tmem_alloc(tmem_slot, tmem_cols);
+        tmem_alloc(tmem_slot, 2 * kAccCols);
     }
     tc_fence_before();
     __syncthreads();
@@ -87,152 +165,305 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const uint32_t tmem_base = *tmem_slot;
 
     if (warp == 0) {
+        // ------------------------------------------------------------------------ TMA producer
         if (lane == 0) {
-            for (int s = 0; s < p.n_seg; ++s) {
-                const int stage = s % stages;
-                const uint32_t phase = (s / stages) & 1;
-                mbar_wait(&empty_bar[stage], phase ^ 1);
-                mbar_arrive_expect_tx(&full_bar[stage], stage_bytes);
-                uint8_t* a_dst = smem + stage * stage_bytes;
-                tma_load_3d(a_dst, &p.tmA, &full_bar[stage], p.seg_col[s], m0 + p.seg_shift[s], batch);
-                tma_load_3d(a_dst + kABytes, &p.tmB, &full_bar[stage], s * kSegK, 0, det);
+            if (p.b_resident) {
+                mbar_arrive_expect_tx(bres_bar, p.n_seg * b_block);
+                for (int s = 0; s < p.n_seg; ++s) tma_load_3d(smem_b + s * b_block, &p.tmB, bres_bar, s * kSegK, 0, det);
+            }
+            int ia = 0, ib = 0;
+            for (int u = worker; u < total; u += n_workers) {
+                const int batch = (u / spi) * p.n_det + det;
+                for (int g = 0; g < G; ++g) {
+                    const int mt = (u % spi) * G + g;
+                    if (mt >= p.tiles_m) break;
+                    const int m0 = mt * kTileM;
+                    for (int cb = 0; cb < p.n_cb; ++cb) {
+                        const int stage = ia % sa;
+                        mbar_wait(&a_empty[stage], ((ia / sa) & 1) ^ 1);
+                        mbar_arrive_expect_tx(&a_full[stage], p.slab_rows * 128);
+                        tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min, batch);
+                        ++ia;
+                        if (!p.b_resident) {
+                            for (int sh = 0; sh < p.n_shift; ++sh) {
+                                const int s = p.seg_of[cb][sh];
+                                if (s < 0) continue;
+                                const int bs = ib % sb;
+                                mbar_wait(&b_empty[bs], ((ib / sb) & 1) ^ 1);
+                                mbar_arrive_expect_tx(&b_full[bs], b_block);
+                                tma_load_3d(smem_b + bs * b_block, &p.tmB, &b_full[bs], s * kSegK, 0, det);
+                                ++ib;
+                            }
+                        }
+                    }
+                }
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            const uint32_t idesc = umma_idesc_f16(p.fmt, kTileM, p.N);
-            for (int s = 0; s < p.n_seg; ++s) {
-                const int stage = s % stages;
-                const uint32_t phase = (s / stages) & 1;
-                mbar_wait(&full_bar[stage], phase);
-                tc_fence_after();
-                const uint32_t a_addr = smem_u32(smem + stage * stage_bytes);
-                const uint64_t adesc = umma_smem_desc_sw128(a_addr);
-                const uint64_t bdesc = umma_smem_desc_sw128(a_addr + kABytes);
+        // -------------------------------------------------------------------------- MMA issuer
+        // The whole warp walks the loops (warp-uniform control flow keeps descriptors in uniform
+        // registers); one elected lane issues the MMAs and commits.  The issue cost per MMA has to stay
+        // well under the MMA's own 16..128 cycles, so with resident weights ONE elected block issues every
+        // shift of a slab (up to 6 x 4 MMAs) between one barrier wait and one commit; which shifts exist
+        // for column block cb is a 6-bit field of the register `shmask`.
+        const uint32_t idesc = umma_idesc_f16(FMT, kTileM, p.N);
+        if (p.b_resident) mbar_wait(bres_bar, 0);
+        const uint32_t smem_a_u32 = smem_u32(smem_a), smem_b_u32 = smem_u32(smem_b);
+        const bool resident = p.b_resident != 0;
+        const int n_cb = p.n_cb, n_shift = p.n_shift;
+        const uint32_t b_step = static_cast<uint32_t>(b_block) >> 4;       // descriptor units per B K-block
+        unsigned long long shmask = 0;
+        for (int cb = 0; cb < n_cb; ++cb)
+            for (int sh = 0; sh < n_shift; ++sh)
+                if (p.seg_of[cb][sh] >= 0) shmask |= 1ull << (cb * kMaxShift + sh);
+        int it = 0;
+        int stage = 0; uint32_t a_phase = 0;            // A ring position
+        int bs = 0; uint32_t b_phase = 0;               // B ring position (streaming mode)
+        for (int u = worker; u < total; u += n_workers, ++it) {
+            const int acc = it & 1;
+            mbar_wait(&tmem_empty[acc], ((it >> 1) & 1) ^ 1);
+            tc_fence_after();
+            const int g_end = min(G, p.tiles_m - (u % spi) * G);
+            for (int g = 0; g < g_end; ++g) {
+                const uint32_t d_tmem = tmem_base + acc * kAccCols + g * p.N;
+                uint32_t accumulate = 0;
+                uint32_t b_lo = umma_desc_lo(smem_b_u32);                  // resident: block 0 of B
+                for (int cb = 0; cb < n_cb; ++cb) {
+                    const uint32_t m = static_cast<uint32_t>(shmask >> (cb * kMaxShift)) & ((1u << kMaxShift) - 1);
+                    mbar_wait(&a_full[stage], a_phase);
+                    tc_fence_after();
+                    const uint32_t a_lo = umma_desc_lo(smem_a_u32 + stage * sl);
+                    if (resident) {
+                        if (elect_one()) {
+                            uint32_t acc_flag = accumulate, bl = b_lo;
+                            for (int sh = 0; sh < n_shift; ++sh) {
+                                if (!((m >> sh) & 1u)) continue;
+                                const uint32_t a_lo_s = a_lo + 8u * sh;    // +128 bytes = one slab row
 #pragma unroll
-                for (int k = 0; k < kSegK / 16; ++k) {
-                    // advance 16 elements = 32 bytes along K inside the 128-byte swizzle row: +2 in the
-                    // (addr >> 4) field of the descriptor
-                    umma_f16(tmem_base, adesc + 2 * k, bdesc + 2 * k, idesc, (s | k) != 0 ? 1u : 0u);
+                                for (int k = 0; k < kSegK / 16; ++k)       // +32 bytes along K: +2 in (addr >> 4)
+                                    umma_f16(d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, acc_flag | k);
+                                acc_flag = 1;
+                                bl += b_step;
+                            }
+                            umma_commit(&a_empty[stage]);                  // slab free once these MMAs retire
+                        }
+                        __syncwarp();
+                        b_lo += b_step * __popc(m);
+                    } else {
+                        for (int sh = 0; sh < n_shift; ++sh) {
+                            if (!((m >> sh) & 1u)) continue;
+                            mbar_wait(&b_full[bs], b_phase);
+                            tc_fence_after();
+                            const uint32_t bl = umma_desc_lo(smem_b_u32 + bs * b_block);
+                            const uint32_t a_lo_s = a_lo + 8u * sh;
+                            const bool last = (m >> (sh + 1)) == 0;
+                            if (elect_one()) {
+#pragma unroll
+                                for (int k = 0; k < kSegK / 16; ++k)
+                                    umma_f16(d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, accumulate | k);
+                                umma_commit(&b_empty[bs]);
+                                if (last) umma_commit(&a_empty[stage]);
+                            }
+                            __syncwarp();
+                            accumulate = 1;
+                            if (++bs == sb) { bs = 0; b_phase ^= 1; }
+                        }
+                    }
+                    accumulate = 1;
+                    if (++stage == sa) { stage = 0; a_phase ^= 1; }
                 }
-                umma_commit(&empty_bar[stage]);        // frees the smem slot when these MMAs retire
             }
-            umma_commit(tmem_full_bar);                // accumulator complete
+            if (elect_one()) umma_commit(&tmem_full[acc]);                 // accumulator stage complete
+            __syncwarp();
         }
     } else {
-        // ------------------------------------------------------------------ epilogue warps 2..5
-        const int quad = warp % 4;                     // TMEM lane quadrant this warp may read
+        // ------------------------------------------------------------- epilogue warps 2..9 (8 warps)
+        const int quad = warp % 4;                             // TMEM lane quadrant this warp may read
+        const int hsel = (warp - 2) / 4;                       // which half of the 32-column chunks
         const int row_in_tile = quad * 32 + lane;
-        const int row = m0 + row_in_tile;
-        mbar_wait(tmem_full_bar, 0);
-        tc_fence_after();
-        const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16);
-        const float* bias = p.bias + static_cast<size_t>(det) * p.N;
-        if (p.epi == EPI_STORE) {
-            uint16_t* orow = reinterpret_cast<uint16_t*>(p.out) + (static_cast<size_t>(batch) * p.M + row) * p.N;
-            for (int c0 = 0; c0 < p.N; c0 += 32) {
-                uint32_t r[32];
-                tmem_ld_32x32(taddr + c0, r);
-                tmem_ld_wait();
-                if (row < p.M) {
-                    uint32_t o[16];
+        const int et = threadIdx.x - 64;                       // 0..255
+        for (int i = et; i < p.N; i += kEpiWarps * 32) bias_s[i] = __ldg(p.bias + static_cast<size_t>(det) * p.N + i);
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        // the four 32-column chunks this warp owns in every stage: tile-in-stage g and first column col0
+        int ch_g[4], ch_col[4];
+        const uint32_t bias_u32 = smem_u32(bias_s);
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const float v0 = act_apply(__uint_as_float(r[2 * j]) + __ldg(bias + c0 + 2 * j), p.act);
-                        const float v1 = act_apply(__uint_as_float(r[2 * j + 1]) + __ldg(bias + c0 + 2 * j + 1), p.act);
-                        o[j] = pack_pair(v0, v1, p.fmt);
+        for (int i = 0; i < 4; ++i) {
+            const int c = hsel + 4 * (i / 2) + 2 * (i % 2);
+            ch_g[i] = (32 * c) / p.N;
+            ch_col[i] = (32 * c) % p.N;
+        }
+        int it = 0;
+        for (int u = worker; u < total; u += n_workers, ++it) {
+            const int acc = it & 1;
+            const int batch = (u / spi) * p.n_det + det;
+            mbar_wait(&tmem_full[acc], (it >> 1) & 1);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * kAccCols;
+            if (EPI == EPI_STORE) {
+                // 8 chunks of 32 columns per stage; this warp takes chunks hsel, hsel+2, ... two at a time
+                for (int cp = 0; cp < 2; ++cp) {
+                    const int ca = hsel + 4 * cp, cbk = hsel + 4 * cp + 2;     // chunk indices
+                    uint32_t ra[32], rb[32];
+                    tmem_ld_32x32(taddr + 32 * ca, ra);
+                    tmem_ld_32x32(taddr + 32 * cbk, rb);
+                    float4 bia[2][8];                          // bias of both chunks, fetched under the TMEM latency
+#pragma unroll
+                    for (int which = 0; which < 2; ++which)
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) bia[which][j] = lds_f4(bias_u32 + 4u * (ch_col[2 * cp + which] + 4 * j));
+                    tmem_ld_wait();
+                    if (cp == 1) {                             // last reads of this stage: hand it back
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&tmem_empty[acc]);
                     }
-                    uint4* dst = reinterpret_cast<uint4*>(orow + c0);
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) dst[j] = make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
-                }
-            }
-        } else {
-            // conv (stride 1) + bias + ReLU + MaxPool(4): row m holds outputs 2m (cols [0,N/2)) and 2m+1
-            // (cols [N/2,N)); pooled row q = m/2 is the max over both halves of rows 2q and 2q+1.
-            const int half = p.N / 2;
-            const int Mq = p.M / 2;
-            float* pool_s = reinterpret_cast<float*>(smem);             // [64][half+1] fp32, pipeline smem is free now
-            const int pstride = half + 1;
-            for (int c0 = 0; c0 < half; c0 += 32) {
-                uint32_t re[32], ro[32];
-                tmem_ld_32x32(taddr + c0, re);
-                tmem_ld_32x32(taddr + half + c0, ro);
-                tmem_ld_wait();
-                float v[32];
+                    for (int which = 0; which < 2; ++which) {
+                        const uint32_t* r = which == 0 ? ra : rb;
+                        const int g = ch_g[2 * cp + which];
+                        const int col0 = ch_col[2 * cp + which];
+                        const int mt = (u % spi) * G + g;
+                        const int row = mt * kTileM + row_in_tile;
+                        if (g < G && mt < p.tiles_m && row < p.M) {
+                            uint32_t o[16];
 #pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    const float bj = __ldg(bias + c0 + j);
-                    float m = fmaxf(__uint_as_float(re[j]) + bj, __uint_as_float(ro[j]) + bj);
-                    m = (row < p.M) ? fmaxf(m, 0.f) : 0.f;               // ReLU; rows past the end contribute 0
-                    const float other = __shfl_xor_sync(0xffffffffu, m, 1);
-                    v[j] = fmaxf(m, other);
-                }
-                if ((lane & 1) == 0 && row < p.M) {
-                    const int q = row / 2;
-                    if (p.epi == EPI_POOL) {
-                        uint16_t* orow = reinterpret_cast<uint16_t*>(p.out) + (static_cast<size_t>(batch) * Mq + q) * half + c0;
-                        uint4* dst = reinterpret_cast<uint4*>(orow);
+                            for (int j = 0; j < 8; ++j) {
+                                const float4 b4 = bia[which][j];
+                                const float v0 = act_apply_t<ACT>(__uint_as_float(r[4 * j]) + b4.x);
+                                const float v1 = act_apply_t<ACT>(__uint_as_float(r[4 * j + 1]) + b4.y);
+                                const float v2 = act_apply_t<ACT>(__uint_as_float(r[4 * j + 2]) + b4.z);
+                                const float v3 = act_apply_t<ACT>(__uint_as_float(r[4 * j + 3]) + b4.w);
+                                o[2 * j] = pack_pair_t<FMT>(v0, v1);
+                                o[2 * j + 1] = pack_pair_t<FMT>(v2, v3);
+                            }
+                            uint16_t* orow = reinterpret_cast<uint16_t*>(p.out) + (static_cast<size_t>(batch) * p.M + row) * p.N + col0;
+                            uint4* dst = reinterpret_cast<uint4*>(orow);
 #pragma unroll
-                        for (int j = 0; j < 4; ++j)
-                            dst[j] = make_uint4(pack_pair(v[8 * j], v[8 * j + 1], p.fmt), pack_pair(v[8 * j + 2], v[8 * j + 3], p.fmt),
-                                                pack_pair(v[8 * j + 4], v[8 * j + 5], p.fmt), pack_pair(v[8 * j + 6], v[8 * j + 7], p.fmt));
-                    } else {
-                        float* prow = pool_s + (row_in_tile / 2) * pstride + c0;
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) prow[j] = v[j];
+                            for (int j = 0; j < 4; ++j) dst[j] = make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]);
+                        }
                     }
                 }
-            }
-            if (p.epi == EPI_POOL_HEAD) {
-                // global average pool over the Mq pooled rows, dense(half -> hidden) + ReLU,
-                // dense(hidden -> 1), sigmoid: fused into this (last) conv block's epilogue.
-                float* gap_s = pool_s + 64 * pstride;                    // [half]
-                float* hid_s = gap_s + half;                             // [hidden]
-                const int et = threadIdx.x - 64;                         // 0..127 among the epilogue threads
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                for (int c = et; c < half; c += 128) {
-                    float s = 0.f;
-                    for (int q = 0; q < Mq; ++q) s += pool_s[q * pstride + c];
-                    gap_s[c] = s / static_cast<float>(Mq);
-                }
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                for (int hrow = et; hrow < p.head_hidden; hrow += 128) {
-                    float s = __ldg(p.hb1 + hrow);
-                    const float* wr = p.hw1 + static_cast<size_t>(hrow) * half;
-                    for (int c = 0; c < half; ++c) s = fmaf(__ldg(wr + c), gap_s[c], s);
-                    hid_s[hrow] = fmaxf(s, 0.f);
-                }
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                if (et < 32) {
-                    float s = 0.f;
-                    for (int i = et; i < p.head_hidden; i += 32) s = fmaf(__ldg(p.hw2 + i), hid_s[i], s);
+            } else {
+                // conv (stride 1) + bias + ReLU + MaxPool(4): row m holds outputs 2m (cols [0,N/2)) and 2m+1
+                // (cols [N/2,N)); pooled row q = m/2 is the max over both halves of rows 2q and 2q+1.
+                const int m0 = (u % spi) * kTileM;
+                const int row = m0 + row_in_tile;
+                const int half = p.N / 2;
+                const int Mq = p.M / 2;
+                const int pstride = half + 1;
+                float* pool_s = head_s;                        // [64][half+1] fp32 (EPI_POOL_HEAD only)
+                const int n_chunks = half / 32;
+                for (int ci = hsel; ci < n_chunks; ci += 2) {
+                    const int c0 = ci * 32;
+                    uint32_t re[32], ro[32];
+                    tmem_ld_32x32(taddr + c0, re);
+                    tmem_ld_32x32(taddr + half + c0, ro);
+                    tmem_ld_wait();
+                    float v[32];
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-                    if (et == 0) {
-                        const float z = s + __ldg(p.hb2);
-                        p.scores[batch] = 1.f / (1.f + __expf(-z));
+                    for (int j = 0; j < 32; ++j) {
+                        const float bj = bias_s[c0 + j];
+                        float m = fmaxf(__uint_as_float(re[j]) + bj, __uint_as_float(ro[j]) + bj);
+                        m = (row < p.M) ? fmaxf(m, 0.f) : 0.f;               // ReLU; rows past the end contribute 0
+                        const float other = __shfl_xor_sync(0xffffffffu, m, 1);
+                        v[j] = fmaxf(m, other);
                     }
+                    if ((lane & 1) == 0 && row < p.M) {
+                        const int q = row / 2;
+                        if (EPI == EPI_POOL) {
+                            uint16_t* orow = reinterpret_cast<uint16_t*>(p.out) + (static_cast<size_t>(batch) * Mq + q) * half + c0;
+                            uint4* dst = reinterpret_cast<uint4*>(orow);
+#pragma unroll
+                            for (int j = 0; j < 4; ++j)
+                                dst[j] = make_uint4(pack_pair_t<FMT>(v[8 * j], v[8 * j + 1]), pack_pair_t<FMT>(v[8 * j + 2], v[8 * j + 3]),
+                                                    pack_pair_t<FMT>(v[8 * j + 4], v[8 * j + 5]), pack_pair_t<FMT>(v[8 * j + 6], v[8 * j + 7]));
+                        } else {
+                            float* prow = pool_s + (row_in_tile / 2) * pstride + c0;
+#pragma unroll
+                            for (int j = 0; j < 32; ++j) prow[j] = v[j];
+                        }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tmem_empty[acc]);
+                if (EPI == EPI_POOL_HEAD) {
+                    // global average pool over the Mq pooled rows, dense(half -> hidden) + ReLU,
+                    // dense(hidden -> 1), sigmoid: fused into this (last) conv block's epilogue.
+                    float* gap_s = pool_s + 64 * pstride;                    // [half]
+                    float* hid_s = gap_s + half;                             // [hidden]
+                    asm volatile("bar.sync 1, 256;" ::: "memory");
+                    for (int c = et; c < half; c += kEpiWarps * 32) {
+                        float s = 0.f;
+                        for (int q = 0; q < Mq; ++q) s += pool_s[q * pstride + c];
+                        gap_s[c] = s / static_cast<float>(Mq);
+                    }
+                    asm volatile("bar.sync 1, 256;" ::: "memory");
+                    for (int hrow = et; hrow < p.head_hidden; hrow += kEpiWarps * 32) {
+                        float s = __ldg(p.hb1 + hrow);
+                        const float* wr = p.hw1 + static_cast<size_t>(hrow) * half;
+                        for (int c = 0; c < half; ++c) s = fmaf(__ldg(wr + c), gap_s[c], s);
+                        hid_s[hrow] = fmaxf(s, 0.f);
+                    }
+                    asm volatile("bar.sync 1, 256;" ::: "memory");
+                    if (et < 32) {
+                        float s = 0.f;
+                        for (int i = et; i < p.head_hidden; i += 32) s = fmaf(__ldg(p.hw2 + i), hid_s[i], s);
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+                        if (et == 0) {
+                            const float z = s + __ldg(p.hb2);
+                            p.scores[batch] = 1.f / (1.f + __expf(-z));
+                        }
+                    }
+                    asm volatile("bar.sync 1, 256;" ::: "memory");           // scratch is reused by the next tile
                 }
             }
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem_base, tmem_cols);
+    if (warp == 0) tmem_dealloc(tmem_base, 2 * kAccCols);
+}
+
+typedef void (*GemmKernel)(const ConvGemmParams, int);
+
+static GemmKernel pick_kernel(int epi, int act, int fmt) {
+#define GW_PICK(E, A)                                                                                         \
+    if (epi == E && act == A) return fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16> : k_conv_gemm_umma<E, A, FMT_FP16>;
+    GW_PICK(EPI_STORE, ACT_TANH)
+    GW_PICK(EPI_STORE, ACT_NONE)
+    GW_PICK(EPI_STORE, ACT_RELU)
+    GW_PICK(EPI_POOL, ACT_RELU)
+    GW_PICK(EPI_POOL_HEAD, ACT_RELU)
+#undef GW_PICK
+    return nullptr;
 }
 
 static bool g_prepared = false;
 cudaError_t conv_gemm_prepare() {
     if (g_prepared) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(k_conv_gemm_umma, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    if (e == cudaSuccess) g_prepared = true;
-    return e;
+    const int epis[5] = {EPI_STORE, EPI_STORE, EPI_STORE, EPI_POOL, EPI_POOL_HEAD};
+    const int acts[5] = {ACT_TANH, ACT_NONE, ACT_RELU, ACT_RELU, ACT_RELU};
+    for (int i = 0; i < 5; ++i)
+        for (int fmt = 0; fmt < 2; ++fmt) {
+            cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel(epis[i], acts[i], fmt)),
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+            if (e != cudaSuccess) return e;
+        }
+    g_prepared = true;
+    return cudaSuccess;
 }
 
 void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
-    dim3 grid((g.p.M + kTileM - 1) / kTileM, g.batch);
-    k_conv_gemm_umma<<<grid, kGemmThreads, g.smem_bytes, st>>>(g.p, g.stages);
+    const int n_items = g.batch / g.p.n_det;
+    const int total = n_items * g.p.tiles_m;                 // tiles per detector
+    int workers = g.grid / g.p.n_det;
+    if (workers > total) workers = total;
+    GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt);
+    if (!k) { fprintf(stderr, "gwstream: no conv GEMM kernel for epi %d act %d\n", g.p.epi, g.p.act); return; }
+    k<<<workers * g.p.n_det, kGemmThreads, g.smem_bytes, st>>>(g.p, n_items);
     ++g_kernel_launches;
 }
 

@@ -7,6 +7,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <string>
@@ -267,7 +268,7 @@ struct gw_pipeline {
 // tap(a, par, r): index j of the filter tap that connects A-view row shift a, column half `par`
 // (position parity inside a pair row; always 0 for GK_DEC) to output column half r; <0 or >=k: none.
 static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, int n_det, int fmt, const void* in,
-                            int in_L, int cin_p, void* out, int cout_p, int batch, int epi) {
+                            int in_L, int cin_p, void* out, int cout_p, int batch, int epi, int head_hidden = 0) {
     const HostLayer& H0 = dets[0];
     ConvGemmParams& p = gl.g.p;
     memset(&p, 0, sizeof p);
@@ -290,11 +291,13 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
             default:     return 2 * a + par - r + H0.pad_l;           // x index (2m + r) + j - pad = 2(m+a) + par
         }
     };
-    // segment table
-    int n_seg = 0;
+    // segment table, ordered column block outer / row shift inner (the order the kernel issues MMAs in)
+    int n_seg = 0, a_lo = 99, a_hi = -99;
     std::vector<int> seg_a, seg_cb;
-    for (int a = -8; a <= 8; ++a)
-        for (int cb = 0; cb < p.a_cols / kSegK; ++cb) {
+    p.n_cb = p.a_cols / kSegK;
+    if (p.n_cb > kMaxCb) return fail(GW_EINVAL, "A view width %d too wide", p.a_cols);
+    for (int cb = 0; cb < p.n_cb; ++cb)
+        for (int a = -8; a <= 8; ++a) {
             bool any = false;
             for (int kk = 0; kk < kSegK && !any; ++kk) {
                 const int col = cb * kSegK + kk, par = col / cin_p, ci = col % cin_p;
@@ -304,11 +307,25 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
                     if (j >= 0 && j < H0.k) any = true;
                 }
             }
-            if (any) { seg_a.push_back(a); seg_cb.push_back(cb); ++n_seg; }
+            if (any) {
+                seg_a.push_back(a); seg_cb.push_back(cb); ++n_seg;
+                if (a < a_lo) a_lo = a;
+                if (a > a_hi) a_hi = a;
+            }
         }
-    if (n_seg > kMaxSeg) return fail(GW_EINVAL, "layer needs %d K segments (max %d)", n_seg, kMaxSeg);
+    if (n_seg > kMaxSeg || n_seg < 1) return fail(GW_EINVAL, "layer needs %d K segments (max %d)", n_seg, kMaxSeg);
     p.n_seg = n_seg;
-    for (int s = 0; s < n_seg; ++s) { p.seg_shift[s] = static_cast<int8_t>(seg_a[s]); p.seg_col[s] = static_cast<int16_t>(seg_cb[s] * kSegK); }
+    p.a_min = a_lo;
+    p.n_shift = a_hi - a_lo + 1;
+    if (p.n_shift > kMaxShift) return fail(GW_EINVAL, "layer needs %d row shifts (max %d)", p.n_shift, kMaxShift);
+    p.slab_rows = kTileM + p.n_shift - 1;
+    p.tiles_m = (p.M + kTileM - 1) / kTileM;
+    memset(p.seg_of, 0xff, sizeof p.seg_of);
+    for (int s = 0; s < n_seg; ++s) {
+        p.seg_shift[s] = static_cast<int8_t>(seg_a[s]);
+        p.seg_col[s] = static_cast<int16_t>(seg_cb[s] * kSegK);
+        p.seg_of[seg_cb[s]][seg_a[s] - a_lo] = static_cast<int8_t>(s);
+    }
     // weights and bias
     const size_t ktot = static_cast<size_t>(n_seg) * kSegK;
     std::vector<uint16_t> B(static_cast<size_t>(n_det) * p.N * ktot, 0);
@@ -335,16 +352,14 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     CU_TRY(cudaMalloc(&gl.d_bias, bias.size() * 4));
     CU_TRY(cudaMemcpy(gl.d_bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
     p.A = in; p.B = gl.d_B; p.bias = gl.d_bias; p.out = out;
-    if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows, batch, p.a_cols, static_cast<uint64_t>(p.a_rows) * p.a_cols, kTileM)) return rc;
+    if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows, batch, p.a_cols, static_cast<uint64_t>(p.a_rows) * p.a_cols, p.slab_rows)) return rc;
     if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.N)) return rc;
     gl.g.batch = batch;
-    const int stage_bytes = kTileM * 128 + p.N * 128;
-    int stages = (200 * 1024) / stage_bytes;
-    if (stages > 6) stages = 6;
-    if (stages > n_seg) stages = n_seg;
-    if (stages < 1) stages = 1;
-    gl.g.stages = stages;
-    gl.g.smem_bytes = conv_gemm_smem_bytes(p.N, stages);
+    p.head_hidden = head_hidden;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (!conv_gemm_plan(gl.g, sms)) return fail(GW_EINVAL, "conv GEMM layer does not fit in shared memory");
     gl.impl = g_conv_impl;
     return GW_OK;
 }
@@ -702,7 +717,8 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
         return fail(GW_EINVAL, "dense head must be cout -> hidden -> 1");
     const int hidden = spec->dense_dims[1];
     if (hidden < 1 || hidden > 128) return fail(GW_EINVAL, "dense hidden width must be in [1,128]");
-    // first block on CUDA cores
+    // first block on CUDA cores (its cin * k taps live in registers)
+    if (H[0].cin * H[0].k > 32) return fail(GW_EINVAL, "first classifier block: cin * k must be <= 32");
     b->c1 = H[0];
     b->c1_cpad = round_up(H[0].cout, 32);
     {
@@ -738,7 +754,8 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
         if (len[i - 1] % 4) return fail(GW_EINVAL, "classifier length must be divisible by 4^blocks");
         GemmLayer& gl = b->gemm[i - 1];
         if (int rc = build_gemm_layer(gl, GK_BBH, &H[i], 1, b->fmt, b->act[i - 1], len[i - 1], cp[i - 1],
-                                      last ? nullptr : b->act[i], cout_p, b->batch, last ? EPI_POOL_HEAD : EPI_POOL))
+                                      last ? nullptr : b->act[i], cout_p, b->batch, last ? EPI_POOL_HEAD : EPI_POOL,
+                                      last ? hidden : 0))
             return rc;
         gl.name = "gemm.bbh" + std::to_string(i);
         gl.flops = 2.0 * len[i - 1] * H[i].k * H[i].cin * H[i].cout;
@@ -748,9 +765,6 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
             p.scores = b->scores_buf;
             CU_TRY(cudaMalloc(&b->pooled_dbg, static_cast<size_t>(b->batch) * (p.M / 2) * (p.N / 2) * 4));
             p.pooled_dbg = b->pooled_dbg;
-            // the head stages [64][N/2+1] + N/2 + hidden floats in the (free) pipeline shared memory
-            const int need = (64 * (p.N / 2 + 1) + p.N / 2 + hidden) * 4 + 1024;
-            if (gl.g.smem_bytes < need) gl.g.smem_bytes = need;
         }
     }
     CU_TRY(conv_gemm_prepare());

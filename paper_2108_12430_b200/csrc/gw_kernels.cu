@@ -314,45 +314,64 @@ void launch_aggregate(const AggParams& a, cudaStream_t st) {
 // x: [batch][cin][L] fp32; w: [cout][cin][K] fp32 (already rounded to the storage type);
 // out: [batch][L/pool][cpad] 16-bit channels-last, channels >= cout zero.
 // ---------------------------------------------------------------------------------------------
+constexpr int kC1Q = 64;          // pooled positions per block
+constexpr int kC1MaxTaps = 32;    // cin * K held in registers per lane
+
 __global__ void __launch_bounds__(256) k_bbh_conv1(const float* __restrict__ x, const float* __restrict__ w,
                                                    const float* __restrict__ bias, void* __restrict__ out,
                                                    int cin, int L, int cout, int cpad, int K, int pad_l,
                                                    int pool, int fmt) {
+    extern __shared__ float xs[];                       // [cin][kC1Q * pool + K - 1] input tile with halo
     const int b = blockIdx.y;
     const int Lq = L / pool;
-    const int c = threadIdx.x % 32 + blockIdx.z * 32;
-    const int q = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
-    if (q >= Lq) return;
-    float best = 0.f;                                   // ReLU output is >= 0
-    if (c < cout) {
-        const float bc = __ldg(bias + c);
+    const int q0 = blockIdx.x * kC1Q;
+    const int span = kC1Q * pool + K - 1;
+    const int l0 = q0 * pool - pad_l;                   // first input position of the tile
+    for (int i = threadIdx.x; i < cin * span; i += blockDim.x) {
+        const int ci = i / span, l = l0 + i % span;
+        xs[i] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+    }
+    const int lane = threadIdx.x % 32, wrp = threadIdx.x / 32;
+    const int c = lane + blockIdx.z * 32;
+    float wr[kC1MaxTaps];
+#pragma unroll
+    for (int i = 0; i < kC1MaxTaps; ++i) wr[i] = (c < cout && i < cin * K) ? __ldg(w + static_cast<size_t>(c) * cin * K + i) : 0.f;
+    const float bc = c < cout ? __ldg(bias + c) : 0.f;
+    int off[kC1MaxTaps];                                // tap t reads xs[off[t] + position]
+#pragma unroll
+    for (int t = 0; t < kC1MaxTaps; ++t) off[t] = (t / K) * span + t % K;
+    const int n_taps = cin * K;
+    __syncthreads();
+    const int q_per_warp = kC1Q / 8;
+    for (int qi = 0; qi < q_per_warp; ++qi) {
+        const int ql = wrp * q_per_warp + qi;           // pooled position inside the tile
+        const int q = q0 + ql;
+        if (q >= Lq) break;
+        float best = 0.f;                               // ReLU output is >= 0
         for (int i = 0; i < pool; ++i) {
-            const int l = q * pool + i;
             float acc = bc;
-            for (int ci = 0; ci < cin; ++ci) {
-                const float* xr = x + (static_cast<size_t>(b) * cin + ci) * L;
-                const float* wr = w + (static_cast<size_t>(c) * cin + ci) * K;
-                for (int j = 0; j < K; ++j) {
-                    const int idx = l + j - pad_l;
-                    if (idx >= 0 && idx < L) acc = fmaf(__ldg(wr + j), __ldg(xr + idx), acc);
-                }
+#pragma unroll
+            for (int t = 0; t < kC1MaxTaps; ++t) {
+                if (t < n_taps) acc = fmaf(wr[t], xs[off[t] + ql * pool + i], acc);   // warp-broadcast read
             }
             best = fmaxf(best, acc);
         }
-    }
-    const float other = __shfl_down_sync(0xffffffffu, best, 1);
-    if ((threadIdx.x & 1) == 0) {
-        uint32_t* dst = reinterpret_cast<uint32_t*>(reinterpret_cast<uint16_t*>(out) +
-                                                    (static_cast<size_t>(b) * Lq + q) * cpad + c);
-        *dst = pack16(best, other, fmt);
+        if (c >= cout) best = 0.f;
+        const float other = __shfl_down_sync(0xffffffffu, best, 1);
+        if ((lane & 1) == 0) {
+            uint32_t* dst = reinterpret_cast<uint32_t*>(reinterpret_cast<uint16_t*>(out) +
+                                                        (static_cast<size_t>(b) * Lq + q) * cpad + c);
+            *dst = pack16(best, other, fmt);
+        }
     }
 }
 
 void launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
                       int cout, int cpad, int K, int pad_l, int pool, int fmt, cudaStream_t st) {
     const int Lq = L / pool;
-    dim3 grid((Lq + 7) / 8, batch, cpad / 32);
-    k_bbh_conv1<<<grid, 256, 0, st>>>(x, w, b, out, n_det, L, cout, cpad, K, pad_l, pool, fmt);
+    dim3 grid((Lq + kC1Q - 1) / kC1Q, batch, cpad / 32);
+    const size_t smem = static_cast<size_t>(n_det) * (kC1Q * pool + K - 1) * sizeof(float);
+    k_bbh_conv1<<<grid, 256, smem, st>>>(x, w, b, out, n_det, L, cout, cpad, K, pad_l, pool, fmt);
     ++g_kernel_launches;
 }
 

@@ -131,6 +131,19 @@ __device__ __forceinline__ uint64_t umma_smem_desc_sw128(uint32_t smem_addr) {
     return d;
 }
 
+// The same descriptor split into its address-dependent low word and its constant high word, so that an
+// issue loop only adds to a 32-bit value.
+__device__ __forceinline__ uint32_t umma_desc_lo(uint32_t smem_addr) { return ((smem_addr & 0x3FFFF) >> 4) | (1u << 16); }
+__device__ __forceinline__ uint64_t umma_desc_make(uint32_t lo) {
+    constexpr uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);
+    return (static_cast<uint64_t>(hi) << 32) | lo;
+}
+__device__ __forceinline__ float4 lds_f4(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 // Instruction descriptor for kind::f16: D fp32, A/B both `fmt` (0 fp16, 1 bf16), both K-major.
 // Bits: [4,6) D fmt = 1 (F32), [7,10) A fmt, [10,13) B fmt, [15] A major = 0, [16] B major = 0,
 // [17,23) N>>3, [24,29) M>>4.
