@@ -29,7 +29,14 @@ struct ConvGemmParams {
     CUtensorMap tmB;               // 3-D (K = 64 n_seg, N, n_det), box (64, N, 1), SWIZZLE_128B
     const void* A;                 // raw pointers of the same operands (SIMT cross-check kernel)
     const void* B;
-    int a_rows, a_cols;            // A view per batch item
+    int a_rows, a_cols;            // A view per batch item (logical rows: out-of-range rows read as zero)
+    int a_rows_tm;                 // rows per batch item of the underlying tensor (= a_rows, or 2 a_rows for a mirror ring)
+    // Mirror-ring source (first DeepClean layer): the window is rows [off, off + a_rows) of a ring that holds
+    // every sample twice (slots i and i + W), off = (*a_count mod a_ring_W) / a_ring_div, read on the device so
+    // that a captured graph replays unchanged.  Rows outside [0, a_rows) are zeroed in shared memory after the
+    // TMA load (the ring holds real samples there, not padding).  a_count == nullptr: plain activation tensor.
+    const long long* a_count;
+    int a_ring_W, a_ring_div;
     int M;                         // output rows per batch item
     int N;                         // GEMM N, multiple of 32, <= 256
     int n_seg;
@@ -70,7 +77,11 @@ cudaError_t conv_gemm_prepare();   // opt-in shared-memory attribute
 void launch_append(float* ring, const float* new_samples, long long* count, unsigned* ticket, int n_rows,
                    int W, int S, cudaStream_t st);
 bool is_append_kernel(const void* func);   // identifies the a1 node of a captured graph
+bool is_ring16_append_kernel(const void* func);
 void launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st);
+void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
+                          int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
+                          cudaStream_t st);
 void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
                    int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st);
 void launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,

@@ -172,6 +172,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 for (int s = 0; s < p.n_seg; ++s) tma_load_3d(smem_b + s * b_block, &p.tmB, bres_bar, s * kSegK, 0, det);
             }
             int ia = 0, ib = 0;
+            // mirror-ring source: the window starts at ring row (count mod W) / div (see ConvGemmParams)
+            const int row_off = p.a_count ? static_cast<int>((*p.a_count % p.a_ring_W) / p.a_ring_div) : 0;
             for (int u = worker; u < total; u += n_workers) {
                 const int batch = (u / spi) * p.n_det + det;
                 for (int g = 0; g < G; ++g) {
@@ -182,7 +184,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                         const int stage = ia % sa;
                         mbar_wait(&a_empty[stage], ((ia / sa) & 1) ^ 1);
                         mbar_arrive_expect_tx(&a_full[stage], p.slab_rows * 128);
-                        tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min, batch);
+                        tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min + row_off, batch);
                         ++ia;
                         if (!p.b_resident) {
                             for (int sh = 0; sh < p.n_shift; ++sh) {
@@ -210,6 +212,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         if (p.b_resident) mbar_wait(bres_bar, 0);
         const uint32_t smem_a_u32 = smem_u32(smem_a), smem_b_u32 = smem_u32(smem_b);
         const bool resident = p.b_resident != 0;
+        const bool ring = p.a_count != nullptr;
         const int n_cb = p.n_cb, n_shift = p.n_shift;
         const uint32_t b_step = static_cast<uint32_t>(b_block) >> 4;       // descriptor units per B K-block
         unsigned long long shmask = 0;
@@ -232,6 +235,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     const uint32_t m = static_cast<uint32_t>(shmask >> (cb * kMaxShift)) & ((1u << kMaxShift) - 1);
                     mbar_wait(&a_full[stage], a_phase);
                     tc_fence_after();
+                    if (ring) {
+                        // window-edge zero padding: slab rows whose logical row is outside [0, M) hold
+                        // neighbouring ring samples; clear them (whole 128-byte rows: swizzle-agnostic)
+                        const int lo = ((u % spi) * G + g) * kTileM + p.a_min;
+                        if (lo < 0 || lo + p.slab_rows > p.a_rows) {
+                            uint8_t* slab = smem_a + stage * sl;
+                            for (int idx = lane; idx < p.slab_rows * 8; idx += 32) {
+                                const int lr = lo + (idx >> 3);
+                                if (lr < 0 || lr >= p.a_rows)
+                                    *reinterpret_cast<uint4*>(slab + (idx >> 3) * 128 + (idx & 7) * 16) = make_uint4(0, 0, 0, 0);
+                            }
+                            fence_proxy_async();
+                            __syncwarp();
+                        }
+                    }
                     const uint32_t a_lo = umma_desc_lo(smem_a_u32 + stage * sl);
                     if (resident) {
                         if (elect_one()) {
@@ -478,11 +496,12 @@ __device__ __forceinline__ float ld16v(const void* p, size_t i, int fmt) {
 
 __device__ float simt_dot(const ConvGemmParams& p, int batch, int det, int m, int n) {
     float acc = 0.f;
+    const int row_off = p.a_count ? static_cast<int>((*p.a_count % p.a_ring_W) / p.a_ring_div) : 0;
     const size_t ktot = static_cast<size_t>(p.n_seg) * kSegK;
     for (int s = 0; s < p.n_seg; ++s) {
         const int r = m + p.seg_shift[s];
         if (r < 0 || r >= p.a_rows) continue;
-        const size_t abase = (static_cast<size_t>(batch) * p.a_rows + r) * p.a_cols + p.seg_col[s];
+        const size_t abase = (static_cast<size_t>(batch) * p.a_rows_tm + row_off + r) * p.a_cols + p.seg_col[s];
         const size_t bbase = (static_cast<size_t>(det) * p.N + n) * ktot + static_cast<size_t>(s) * kSegK;
         for (int k = 0; k < kSegK; ++k) acc = fmaf(ld16v(p.A, abase + k, p.fmt), ld16v(p.B, bbase + k, p.fmt), acc);
     }

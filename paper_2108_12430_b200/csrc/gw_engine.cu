@@ -213,7 +213,9 @@ struct gw_deepclean {
     int batch = 0;
     std::vector<HostLayer> host;                 // [n_det * n_layers]
     std::vector<GemmLayer> gemm;                 // layers 0 .. n_layers-2
-    std::vector<void*> act;                      // act[0] = gathered window, act[i+1] = output of layer i
+    void* ring16 = nullptr;                      // mirror ring [batch][2W][cpad0], 16-bit (when `mirror`)
+    bool mirror = false;                         // first layer reads the window from ring16 (no per-update gather)
+    std::vector<void*> act;                      // act[0] = gathered window (null when `mirror`), act[i+1] = output of layer i
     std::vector<int> act_rows, act_cols;
     float* d_wt_final = nullptr;                 // [n_det][K][cpad]
     float* d_b_final = nullptr;                  // [n_det]
@@ -254,7 +256,8 @@ struct gw_pipeline {
     gw_bbh* bbh = nullptr;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
-    cudaGraphNode_t append_node = nullptr;
+    cudaGraphNode_t append_node = nullptr;       // the two kernels that read the caller's new-sample buffer
+    cudaGraphNode_t ring16_node = nullptr;
     int nodes = 0;
     const float* cap_in = nullptr;
     float* cap_scores = nullptr;
@@ -268,7 +271,8 @@ struct gw_pipeline {
 // tap(a, par, r): index j of the filter tap that connects A-view row shift a, column half `par`
 // (position parity inside a pair row; always 0 for GK_DEC) to output column half r; <0 or >=k: none.
 static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, int n_det, int fmt, const void* in,
-                            int in_L, int cin_p, void* out, int cout_p, int batch, int epi, int head_hidden = 0) {
+                            int in_L, int cin_p, void* out, int cout_p, int batch, int epi, int head_hidden = 0,
+                            const long long* ring_count = nullptr, int ring_W = 0) {
     const HostLayer& H0 = dets[0];
     ConvGemmParams& p = gl.g.p;
     memset(&p, 0, sizeof p);
@@ -276,6 +280,10 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     const int halves_out = gk == GK_ENC ? 1 : 2;      // N packs (even | odd) outputs?
     p.a_cols = halves_in * cin_p;
     p.a_rows = in_L / halves_in;
+    p.a_rows_tm = ring_count ? 2 * p.a_rows : p.a_rows;     // mirror ring: every sample stored twice
+    p.a_count = ring_count;
+    p.a_ring_W = ring_W;
+    p.a_ring_div = halves_in;
     p.M = p.a_rows;
     p.N = halves_out * cout_p;
     p.n_det = n_det;
@@ -352,7 +360,7 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     CU_TRY(cudaMalloc(&gl.d_bias, bias.size() * 4));
     CU_TRY(cudaMemcpy(gl.d_bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
     p.A = in; p.B = gl.d_B; p.bias = gl.d_bias; p.out = out;
-    if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows, batch, p.a_cols, static_cast<uint64_t>(p.a_rows) * p.a_cols, p.slab_rows)) return rc;
+    if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows_tm, batch, p.a_cols, static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, p.slab_rows)) return rc;
     if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.N)) return rc;
     gl.g.batch = batch;
     p.head_hidden = head_hidden;
@@ -407,6 +415,8 @@ extern "C" int gw_stream_destroy(gw_stream* s) {
     return GW_OK;
 }
 
+static void ring16_append_enqueue(gw_deepclean* dc, const float* src, cudaStream_t st);
+
 static int stream_update_checked(gw_stream* s) {
     if (s->dc && s->dc->cleaned_for != s->updates)
         return fail(GW_ESTATE, "gw_stream_update: update %lld has not been through gw_deepclean_forward + gw_cleaned_strain",
@@ -416,6 +426,7 @@ static int stream_update_checked(gw_stream* s) {
 static void stream_update_enqueue(gw_stream* s, const float* src, cudaStream_t st) {
     launch_append(s->ring, src, s->d_count, s->d_ticket, s->n * s->C, s->W, s->S, st);
     prof_mark("append", st);
+    if (s->dc) ring16_append_enqueue(s->dc, src, st);
 }
 
 extern "C" int gw_stream_update(gw_stream* s, const float* new_samples_dev, void* stream) {
@@ -445,8 +456,8 @@ static int validate_dc_layer(const HostLayer& H, bool last) {
     if (H.kind == GW_CONV && (H.pad_l != H.k / 2 || H.pad_r != H.k / 2)) return fail(GW_EINVAL, "Conv1d needs pad = k/2");
     if (H.kind == GW_CONVT && (H.pad_l != H.k / 2 || H.pad_r != 1)) return fail(GW_EINVAL, "ConvTranspose1d needs padding k/2, output_padding 1");
     if (H.pool != 1) return fail(GW_EINVAL, "DeepClean layers have no pooling");
-    if (last && (H.kind != GW_CONVT || H.cout != 1 || H.act != GW_ACT_NONE))
-        return fail(GW_EINVAL, "last DeepClean layer must be a linear ConvTranspose1d with one output channel");
+    if (last && (H.kind != GW_CONVT || H.cout != 1 || H.act != GW_ACT_NONE || H.k > 7))
+        return fail(GW_EINVAL, "last DeepClean layer must be a linear ConvTranspose1d with one output channel, k <= 7");
     return GW_OK;
 }
 
@@ -454,6 +465,7 @@ extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
     if (!dc) return GW_OK;
     for (auto& g : dc->gemm) free_gemm(g);
     for (void* a : dc->act) cudaFree(a);
+    cudaFree(dc->ring16);
     cudaFree(dc->d_wt_final); cudaFree(dc->d_b_final); cudaFree(dc->pred); cudaFree(dc->acc); cudaFree(dc->nhat);
     cudaFree(dc->d_hann); cudaFree(dc->d_inv_wsum); cudaFree(dc->d_rows_map); cudaFree(dc->d_strain_rows);
     cudaFree(dc->final_buf);
@@ -501,19 +513,26 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     dc->batch = batch;
     dc->act.assign(nl, nullptr);
     dc->act_rows.assign(nl, 0); dc->act_cols.assign(nl, 0);
+    // The 16-bit mirror ring replaces the per-update gather when window positions pair up with ring slots
+    // (even stride => even head) and the first layer is a Conv1d; otherwise the window is re-gathered.
+    dc->mirror = (S % 2 == 0) && (W % 2 == 0) && dc->host[0].kind == GW_CONV;
     for (int i = 0; i < nl; ++i) {                  // act[i] = input of layer i
         dc->act_rows[i] = len[i]; dc->act_cols[i] = cpad[i];
-        const size_t bytes = static_cast<size_t>(batch) * len[i] * cpad[i] * 2;
-        CU_TRY(cudaMalloc(&dc->act[i], bytes));
-        CU_TRY(cudaMemset(dc->act[i], 0, bytes));
+        size_t bytes = static_cast<size_t>(batch) * len[i] * cpad[i] * 2;
+        void** dst = &dc->act[i];
+        if (i == 0 && dc->mirror) { bytes *= 2; dst = &dc->ring16; }
+        CU_TRY(cudaMalloc(dst, bytes));
+        CU_TRY(cudaMemset(*dst, 0, bytes));
     }
     dc->gemm.resize(nl - 1);
     std::vector<HostLayer> per_det(nd);
     for (int i = 0; i < nl - 1; ++i) {
         for (int d = 0; d < nd; ++d) per_det[d] = dc->host[d * nl + i];
         const GemmKind gk = dc->host[i].kind == GW_CONV ? GK_ENC : GK_DEC;
-        if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, dc->act[i], len[i], cpad[i],
-                                      dc->act[i + 1], cpad[i + 1], batch, EPI_STORE))
+        const bool from_ring = i == 0 && dc->mirror;
+        if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, from_ring ? dc->ring16 : dc->act[i],
+                                      len[i], cpad[i], dc->act[i + 1], cpad[i + 1], batch, EPI_STORE, 0,
+                                      from_ring ? s->d_count : nullptr, from_ring ? W : 0))
             return rc;
         dc->gemm[i].name = "gemm.dc" + std::to_string(i);
         // useful MACs: every (input position, tap, cin, cout) product of the layer definition
@@ -602,11 +621,22 @@ extern "C" int gw_deepclean_create(gw_deepclean** out, gw_stream* s, const gw_dc
     return GW_OK;
 }
 
+// a2, incremental: convert this update's S new witness samples into the mirror ring (after k_append).
+static void ring16_append_enqueue(gw_deepclean* dc, const float* src, cudaStream_t st) {
+    if (!dc->mirror) return;
+    gw_stream* s = dc->s;
+    launch_ring16_append(src, dc->ring16, s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, s->S,
+                         dc->act_cols[0], dc->fmt, st);
+    prof_mark("ring16_append", st);
+}
+
 static void deepclean_forward_enqueue(gw_deepclean* dc, cudaStream_t st) {
     gw_stream* s = dc->s;
-    launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
-                  dc->act_cols[0], dc->fmt, st);
-    prof_mark("gather", st);
+    if (!dc->mirror) {
+        launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
+                      dc->act_cols[0], dc->fmt, st);
+        prof_mark("gather", st);
+    }
     for (auto& g : dc->gemm) run_gemm(g, st);
     launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
                        dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
@@ -640,7 +670,15 @@ extern "C" int gw_deepclean_activation(gw_deepclean* dc, int layer, void* out_de
     const int64_t bytes = static_cast<int64_t>(dc->batch) * dc->act_rows[i] * dc->act_cols[i] * 2;
     if (out_dev) {
         if (out_bytes < bytes) return fail(GW_EINVAL, "output buffer too small (%lld < %lld)", (long long)out_bytes, (long long)bytes);
-        CU_TRY(cudaMemcpyAsync(out_dev, dc->act[i], bytes, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+        if (i == 0 && dc->mirror) {
+            // the window is the contiguous row range [h, h + W) of each batch item's mirror ring
+            const size_t row_b = static_cast<size_t>(dc->act_cols[0]) * 2, W = dc->s->W;
+            const size_t h = static_cast<size_t>((dc->s->updates * static_cast<int64_t>(dc->s->S)) % dc->s->W);
+            CU_TRY(cudaMemcpy2DAsync(out_dev, W * row_b, static_cast<const uint8_t*>(dc->ring16) + h * row_b, 2 * W * row_b,
+                                     W * row_b, dc->batch, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+        } else {
+            CU_TRY(cudaMemcpyAsync(out_dev, dc->act[i], bytes, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+        }
     }
     return GW_OK;
 }
@@ -718,7 +756,8 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
     const int hidden = spec->dense_dims[1];
     if (hidden < 1 || hidden > 128) return fail(GW_EINVAL, "dense hidden width must be in [1,128]");
     // first block on CUDA cores (its cin * k taps live in registers)
-    if (H[0].cin * H[0].k > 32) return fail(GW_EINVAL, "first classifier block: cin * k must be <= 32");
+    if (H[0].cin > 4 || H[0].k > 8 || H[0].pad_l > 4 || H[0].k - 1 - H[0].pad_l > 4)
+        return fail(GW_EINVAL, "first classifier block: needs cin <= 4, k <= 8, pad_l <= 4, pad_r <= 4");
     b->c1 = H[0];
     b->c1_cpad = round_up(H[0].cout, 32);
     {
@@ -873,6 +912,7 @@ static int pipeline_capture(gw_pipeline* p, const float* in, float* scores, floa
     p->cap_in = in; p->cap_scores = scores; p->cap_final = fin;
     // remember the append node: a new input pointer is then a parameter update, not a re-capture
     p->append_node = nullptr;
+    p->ring16_node = nullptr;
     size_t n_nodes = 0;
     CU_TRY(cudaGraphGetNodes(p->graph, nullptr, &n_nodes));
     std::vector<cudaGraphNode_t> nodes(n_nodes);
@@ -883,20 +923,29 @@ static int pipeline_capture(gw_pipeline* p, const float* in, float* scores, floa
         if (ty != cudaGraphNodeTypeKernel) continue;
         cudaKernelNodeParams kp;
         CU_TRY(cudaGraphKernelNodeGetParams(nd, &kp));
-        if (is_append_kernel(kp.func)) { p->append_node = nd; break; }
+        if (is_append_kernel(kp.func)) p->append_node = nd;
+        if (is_ring16_append_kernel(kp.func)) p->ring16_node = nd;
     }
     return GW_OK;
 }
 
-static int pipeline_set_input(gw_pipeline* p, const float* in) {
+static int set_node_src(gw_pipeline* p, cudaGraphNode_t node, int n_args, int src_arg, const float* in) {
     cudaKernelNodeParams kp;
-    CU_TRY(cudaGraphKernelNodeGetParams(p->append_node, &kp));
-    void* args[7];
-    for (int i = 0; i < 7; ++i) args[i] = kp.kernelParams[i];
+    CU_TRY(cudaGraphKernelNodeGetParams(node, &kp));
+    void* args[16];
+    for (int i = 0; i < n_args; ++i) args[i] = kp.kernelParams[i];
     const float* src = in;
-    args[1] = &src;                                     // k_append(ring, src, count, ticket, n_rows, W, S)
+    args[src_arg] = &src;
     kp.kernelParams = args;
-    CU_TRY(cudaGraphExecKernelNodeSetParams(p->exec, p->append_node, &kp));
+    CU_TRY(cudaGraphExecKernelNodeSetParams(p->exec, node, &kp));
+    return GW_OK;
+}
+
+static int pipeline_set_input(gw_pipeline* p, const float* in) {
+    // k_append(ring, src, count, ticket, n_rows, W, S); k_ring16_append(src, ring16, count, rows_map, ... 11 args)
+    if (int rc = set_node_src(p, p->append_node, 7, 1, in)) return rc;
+    if (p->ring16_node)
+        if (int rc = set_node_src(p, p->ring16_node, 11, 0, in)) return rc;
     p->cap_in = in;
     return GW_OK;
 }

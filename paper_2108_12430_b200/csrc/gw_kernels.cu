@@ -175,77 +175,211 @@ void launch_gather(const float* ring, void* xw, const long long* count, const in
 }
 
 // ---------------------------------------------------------------------------------------------
+// a2 (incremental form)  16-bit witness "mirror ring": [n*D][2W][cpad] channels-last.  Only the S new
+// samples of each witness channel are converted (RN-even) per update; sample with ring slot i is stored
+// at rows i and i + W, so the current window is always the CONTIGUOUS row range [h, h + W),
+// h = count mod W, and the first conv layer reads it straight through TMA (no per-update re-gather of
+// the whole window: that was 1.24 GB of traffic per step for 23 MB of new samples at n = 128).
+// Runs after k_append, so *count already includes this update's S samples.
+// src: [n][C][S] fp32.  Same 32-channel x 128-position transpose tile as k_gather.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_ring16_append(const float* __restrict__ src, void* __restrict__ ring16,
+                                                       const long long* count, const int* __restrict__ rows_map,
+                                                       int channels, int n_det, int n_wit, int W, int S, int cpad,
+                                                       int fmt) {
+    __shared__ float tile[32][kGatherPos + 1];
+    const int h0 = static_cast<int>((*count - S) % W);   // ring slot of this update's first sample
+    const int sd = blockIdx.y;
+    const int s = sd / n_det, d = sd % n_det;
+    const int cb = blockIdx.z * 32;
+    const int i0 = blockIdx.x * kGatherPos;
+    const int tid = threadIdx.x;
+    {
+        const int pos = tid % kGatherPos;
+        const int cg = tid / kGatherPos;
+        const int i = i0 + pos;
+#pragma unroll 4
+        for (int k = 0; k < 16; ++k) {
+            const int c = cb + cg * 16 + k;
+            float v = 0.f;
+            if (c < n_wit && i < S) {
+                const int row = s * channels + __ldg(rows_map + d * n_wit + c);
+                v = __ldg(src + static_cast<size_t>(row) * S + i);
+            }
+            tile[cg * 16 + k][pos] = v;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+        const int pos = it * 64 + tid / 4;
+        const int c0 = (tid % 4) * 8;
+        const int i = i0 + pos;
+        if (i < S) {
+            uint4 q;
+            q.x = pack16(tile[c0 + 0][pos], tile[c0 + 1][pos], fmt);
+            q.y = pack16(tile[c0 + 2][pos], tile[c0 + 3][pos], fmt);
+            q.z = pack16(tile[c0 + 4][pos], tile[c0 + 5][pos], fmt);
+            q.w = pack16(tile[c0 + 6][pos], tile[c0 + 7][pos], fmt);
+            int slot = h0 + i;
+            if (slot >= W) slot -= W;
+            uint16_t* dst = reinterpret_cast<uint16_t*>(ring16) + (static_cast<size_t>(sd) * 2 * W + slot) * cpad + cb + c0;
+            *reinterpret_cast<uint4*>(dst) = q;
+            *reinterpret_cast<uint4*>(dst + static_cast<size_t>(W) * cpad) = q;
+        }
+    }
+}
+
+bool is_ring16_append_kernel(const void* func) { return func == reinterpret_cast<const void*>(&k_ring16_append); }
+
+void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
+                          int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
+                          cudaStream_t st) {
+    dim3 grid((S + kGatherPos - 1) / kGatherPos, n_streams * n_det, cpad / 32);
+    k_ring16_append<<<grid, 256, 0, st>>>(new_samples, ring16, count, rows_map, channels, n_det, n_wit, W, S, cpad, fmt);
+    ++g_kernel_launches;
+}
+
+// ---------------------------------------------------------------------------------------------
 // a4' Final ConvTranspose1d (cout = 1, stride 2, pad = K/2, output_padding 1) on CUDA cores in
-// fp32: 7 x cin weights are far too thin for a tensor-core tile.  D3 of DESIGN.md:
+// fp32: K x cin weights are far too thin for a tensor-core tile.  D3 of DESIGN.md:
 //   y[2q + r] = b + sum_ci sum_{j : (r + pad - j) even} w[ci][j] x[q + (r + pad - j)/2][ci].
-// Each thread forms the K per-tap dot products t_j[l] of ONE input row l, the block exchanges them
-// through shared memory, then each thread emits the two outputs of its row.
-// x: [batch][L][cpad] 16-bit, wt: [n_det][K][cpad] fp32, pred: [batch][2L] fp32.
+// Phase 1: the per-tap dot products t_j[l] = sum_ci w[ci][j] x[l][ci] of every input row l of the tile.
+//   Four lanes share a row: each loads 8 channels with one 128-bit load (a warp request covers 512
+//   contiguous bytes) and holds the K x 8 weights of its channel octet in registers; the four partial
+//   sums are combined by a two-step reduce-scatter over shuffles (6 shuffles per row instead of 2K).
+// Phase 2: one thread per input row l emits outputs 2l and 2l + 1 from the t_j of rows l-1 .. l+2.
+// x: [batch][L][cpad] 16-bit, wt: [n_det][K][cpad] fp32, pred: [batch][2L] fp32.  K <= 8.
 // ---------------------------------------------------------------------------------------------
 constexpr int kFcThreads = 256;
 constexpr int kFcHalo = 4;
-constexpr int kFcMaxK = 9;
+constexpr int kFcRows = 256;                          // input rows per tile, halo included
+constexpr int kFcMaxK = 8;
 
-__global__ void __launch_bounds__(kFcThreads) k_final_convt(const void* __restrict__ x,
-                                                            const float* __restrict__ wt,
-                                                            const float* __restrict__ bias,
-                                                            float* __restrict__ pred, int n_det, int L, int cpad,
-                                                            int K, int pad, int fmt) {
-    extern __shared__ float sm[];
-    float* w_s = sm;                                  // [K][cpad]
-    float* t_s = sm + K * cpad;                       // [K][kFcThreads]
-    const int b = blockIdx.y;
-    const int det = b % n_det;
-    const int rows_out = kFcThreads - 2 * kFcHalo;
-    const int q0 = blockIdx.x * rows_out;
-    const int tid = threadIdx.x;
-    for (int i = tid; i < K * cpad; i += kFcThreads) w_s[i] = __ldg(wt + static_cast<size_t>(det) * K * cpad + i);
-    __syncthreads();
-    const int l = q0 - kFcHalo + tid;
-    float t[kFcMaxK];
+__device__ __forceinline__ void fc_load_rows(uint4 (&raw)[4], const void* x, int b, int L, int cpad, int c0,
+                                             int l_first, int tid) {
 #pragma unroll
-    for (int j = 0; j < kFcMaxK; ++j) t[j] = 0.f;
-    if (l >= 0 && l < L) {
-        const uint4* row = reinterpret_cast<const uint4*>(reinterpret_cast<const uint16_t*>(x) +
-                                                          (static_cast<size_t>(b) * L + l) * cpad);
-        for (int c8 = 0; c8 < cpad / 8; ++c8) {
-            float f[8];
-            unpack16x8(__ldg(row + c8), f, fmt);
-#pragma unroll
-            for (int j = 0; j < kFcMaxK; ++j) {
-                if (j < K) {
-                    const float* wj = w_s + j * cpad + c8 * 8;
-#pragma unroll
-                    for (int e = 0; e < 8; ++e) t[j] = fmaf(wj[e], f[e], t[j]);
-                }
-            }
-        }
+    for (int ps = 0; ps < 4; ++ps) {
+        const int l = l_first + ps * 64 + (tid >> 2);
+        raw[ps] = make_uint4(0, 0, 0, 0);
+        if (l >= 0 && l < L)
+            raw[ps] = __ldg(reinterpret_cast<const uint4*>(reinterpret_cast<const uint16_t*>(x) +
+                                                           (static_cast<size_t>(b) * L + l) * cpad + c0));
     }
+}
+
+// Persistent: block k serves detector k % n_det (its weights stay in registers) and walks that detector's
+// (batch item, tile) pairs; the next tile's rows are in flight while the current one is reduced.
+__global__ void __launch_bounds__(kFcThreads, 2) k_final_convt(const void* __restrict__ x,
+                                                               const float* __restrict__ wt,
+                                                               const float* __restrict__ bias,
+                                                               float* __restrict__ pred, int n_items, int n_det,
+                                                               int L, int cpad, int K, int pad, int fmt) {
+    __shared__ float t_s[2][kFcMaxK][kFcRows + 4];
+    const int det = blockIdx.x % n_det;
+    const int worker = blockIdx.x / n_det, n_workers = gridDim.x / n_det;
+    const int rows_out = kFcRows - 2 * kFcHalo;
+    const int tiles = (L + rows_out - 1) / rows_out;
+    const int total = n_items * tiles;
+    const int tid = threadIdx.x;
+    const int sub = tid & 3;                           // which channel octet of a 32-channel group
+    const int b0 = sub & 1, b1 = sub >> 1;
+    const int n_cg = cpad / 32;
+    const float bias_d = __ldg(bias + det);
+    float wv[kFcMaxK][8];
 #pragma unroll
     for (int j = 0; j < kFcMaxK; ++j)
-        if (j < K) t_s[j * kFcThreads + tid] = t[j];
-    __syncthreads();
-    if (tid >= kFcHalo && tid < kFcThreads - kFcHalo && l < L) {
-        float y[2];
 #pragma unroll
-        for (int r = 0; r < 2; ++r) {
-            float acc = __ldg(bias + det);
-            for (int j = 0; j < K; ++j) {
-                const int e = r + pad - j;
-                if ((e & 1) == 0) acc += t_s[j * kFcThreads + tid + e / 2];   // e/2 exact: e is even
+        for (int e = 0; e < 8; ++e)
+            wv[j][e] = j < K ? __ldg(wt + (static_cast<size_t>(det) * K + j) * cpad + sub * 8 + e) : 0.f;
+    uint4 raw[4];
+    if (worker < total)
+        fc_load_rows(raw, x, (worker / tiles) * n_det + det, L, cpad, sub * 8, (worker % tiles) * rows_out - kFcHalo, tid);
+    int buf = 0;
+    for (int u = worker; u < total; u += n_workers, buf ^= 1) {
+        const int b = (u / tiles) * n_det + det;
+        const int q0 = (u % tiles) * rows_out;
+        float t[4][kFcMaxK];
+#pragma unroll
+        for (int ps = 0; ps < 4; ++ps)
+#pragma unroll
+            for (int j = 0; j < kFcMaxK; ++j) t[ps][j] = 0.f;
+        for (int cg = 0; cg < n_cg; ++cg) {
+            uint4 cur[4];
+#pragma unroll
+            for (int ps = 0; ps < 4; ++ps) cur[ps] = raw[ps];
+            // prefetch: the next channel group of this tile, or the first one of the next tile
+            if (cg + 1 < n_cg) {
+                fc_load_rows(raw, x, b, L, cpad, (cg + 1) * 32 + sub * 8, q0 - kFcHalo, tid);
+            } else if (u + n_workers < total) {
+                const int un = u + n_workers;
+                fc_load_rows(raw, x, (un / tiles) * n_det + det, L, cpad, sub * 8, (un % tiles) * rows_out - kFcHalo, tid);
             }
-            y[r] = acc;
+            if (n_cg > 1) {                            // wide final layers: weights change with the channel group
+#pragma unroll
+                for (int j = 0; j < kFcMaxK; ++j)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e)
+                        wv[j][e] = j < K ? __ldg(wt + (static_cast<size_t>(det) * K + j) * cpad + cg * 32 + sub * 8 + e) : 0.f;
+            }
+#pragma unroll
+            for (int ps = 0; ps < 4; ++ps) {
+                float f[8];
+                unpack16x8(cur[ps], f, fmt);
+#pragma unroll
+                for (int j = 0; j < kFcMaxK; ++j)
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) t[ps][j] = fmaf(wv[j][e], f[e], t[ps][j]);
+            }
         }
-        *reinterpret_cast<float2*>(pred + static_cast<size_t>(b) * 2 * L + 2 * l) = make_float2(y[0], y[1]);
+#pragma unroll
+        for (int ps = 0; ps < 4; ++ps) {
+            // reduce-scatter over the 4 lanes of a row: lane (b0, b1) ends with the full sums of taps 4 b0 + 2 b1 + {0, 1}
+            float uu[4], v[2];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float send = b0 ? t[ps][i] : t[ps][i + 4];
+                const float keep = b0 ? t[ps][i + 4] : t[ps][i];
+                uu[i] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+            }
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const float send = b1 ? uu[i] : uu[i + 2];
+                const float keep = b1 ? uu[i + 2] : uu[i];
+                v[i] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+            }
+            const int row = ps * 64 + (tid >> 2);
+            const int j0 = 4 * b0 + 2 * b1;
+            t_s[buf][j0][row] = v[0];
+            t_s[buf][j0 + 1][row] = v[1];
+        }
+        __syncthreads();                               // t_s[buf] complete; t_s[buf ^ 1] is rewritten only after the next barrier
+        const int l = q0 - kFcHalo + tid;
+        if (tid >= kFcHalo && tid < kFcRows - kFcHalo && l < L) {
+            float y[2];
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                float acc = bias_d;
+                for (int j = 0; j < K; ++j) {
+                    const int e = r + pad - j;
+                    if ((e & 1) == 0) acc += t_s[buf][j][tid + e / 2];   // e/2 exact: e is even
+                }
+                y[r] = acc;
+            }
+            *reinterpret_cast<float2*>(pred + static_cast<size_t>(b) * 2 * L + 2 * l) = make_float2(y[0], y[1]);
+        }
     }
 }
 
 void launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
                         int L, int cpad, int K, int pad, int fmt, cudaStream_t st) {
-    const int rows_out = kFcThreads - 2 * kFcHalo;
-    dim3 grid((L + rows_out - 1) / rows_out, batch);
-    const size_t smem = static_cast<size_t>(K) * (cpad + kFcThreads) * sizeof(float);
-    k_final_convt<<<grid, kFcThreads, smem, st>>>(x, wt, bias, pred, n_det, L, cpad, K, pad, fmt);
+    const int rows_out = kFcRows - 2 * kFcHalo;
+    const int n_items = batch / n_det;
+    const int total = n_items * ((L + rows_out - 1) / rows_out);
+    int workers = (148 * 2) / n_det;
+    if (workers > total) workers = total;
+    if (workers < 1) workers = 1;
+    k_final_convt<<<workers * n_det, kFcThreads, 0, st>>>(x, wt, bias, pred, n_items, n_det, L, cpad, K, pad, fmt);
     ++g_kernel_launches;
 }
 
@@ -308,54 +442,66 @@ void launch_aggregate(const AggParams& a, cudaStream_t st) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// a6' First classifier block (cin = number of detectors, K = 8): conv + bias + ReLU + MaxPool(pool)
-// on CUDA cores in fp32 (GEMM K would be 16: one MMA k-step, all epilogue).  One warp = 32 output
-// channels of one pooled position; x reads are warp broadcasts, the 64-byte output row is contiguous.
+// a6' First classifier block (cin = number of detectors, K <= 8): conv + bias + ReLU + MaxPool(4) on
+// CUDA cores in fp32 (as a GEMM its K would be 16: one MMA k-step and all epilogue).
+// lane = output channel (its cin x 8 taps live in registers), one warp = 32 channels of a run of pooled
+// positions.  The input tile starts at l0 = 4 q0 - pad_l, so pooled position q reads the 12 consecutive
+// floats xs[ci][4 (q - q0) .. +12) as three 128-bit warp-broadcast loads per input channel; conv output
+// 4q + i, tap j reads element i + j of that window.  The 64-byte output row of a warp is contiguous.
 // x: [batch][cin][L] fp32; w: [cout][cin][K] fp32 (already rounded to the storage type);
-// out: [batch][L/pool][cpad] 16-bit channels-last, channels >= cout zero.
+// out: [batch][L/4][cpad] 16-bit channels-last, channels >= cout zero.
+// Requires pool == 4, K <= 8, pad_l <= 4, K - 1 - pad_l <= 4, cin <= 4.
 // ---------------------------------------------------------------------------------------------
 constexpr int kC1Q = 64;          // pooled positions per block
-constexpr int kC1MaxTaps = 32;    // cin * K held in registers per lane
+constexpr int kC1MaxCin = 4;
+constexpr int kC1Span = kC1Q * 4 + 12;
 
 __global__ void __launch_bounds__(256) k_bbh_conv1(const float* __restrict__ x, const float* __restrict__ w,
                                                    const float* __restrict__ bias, void* __restrict__ out,
-                                                   int cin, int L, int cout, int cpad, int K, int pad_l,
-                                                   int pool, int fmt) {
-    extern __shared__ float xs[];                       // [cin][kC1Q * pool + K - 1] input tile with halo
+                                                   int cin, int L, int cout, int cpad, int K, int pad_l, int fmt) {
+    __shared__ __align__(16) float xs[kC1MaxCin][kC1Span];
     const int b = blockIdx.y;
-    const int Lq = L / pool;
+    const int Lq = L / 4;
     const int q0 = blockIdx.x * kC1Q;
-    const int span = kC1Q * pool + K - 1;
-    const int l0 = q0 * pool - pad_l;                   // first input position of the tile
-    for (int i = threadIdx.x; i < cin * span; i += blockDim.x) {
-        const int ci = i / span, l = l0 + i % span;
-        xs[i] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+    const int l0 = q0 * 4 - pad_l;                      // first input position of the tile
+    for (int i = threadIdx.x; i < cin * kC1Span; i += blockDim.x) {
+        const int ci = i / kC1Span, l = l0 + i % kC1Span;
+        xs[ci][i % kC1Span] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
     }
     const int lane = threadIdx.x % 32, wrp = threadIdx.x / 32;
     const int c = lane + blockIdx.z * 32;
-    float wr[kC1MaxTaps];
+    float wr[kC1MaxCin][8];
 #pragma unroll
-    for (int i = 0; i < kC1MaxTaps; ++i) wr[i] = (c < cout && i < cin * K) ? __ldg(w + static_cast<size_t>(c) * cin * K + i) : 0.f;
+    for (int ci = 0; ci < kC1MaxCin; ++ci)
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            wr[ci][j] = (c < cout && ci < cin && j < K) ? __ldg(w + (static_cast<size_t>(c) * cin + ci) * K + j) : 0.f;
     const float bc = c < cout ? __ldg(bias + c) : 0.f;
-    int off[kC1MaxTaps];                                // tap t reads xs[off[t] + position]
-#pragma unroll
-    for (int t = 0; t < kC1MaxTaps; ++t) off[t] = (t / K) * span + t % K;
-    const int n_taps = cin * K;
     __syncthreads();
-    const int q_per_warp = kC1Q / 8;
+    constexpr int q_per_warp = kC1Q / 8;
+#pragma unroll 2
     for (int qi = 0; qi < q_per_warp; ++qi) {
         const int ql = wrp * q_per_warp + qi;           // pooled position inside the tile
         const int q = q0 + ql;
         if (q >= Lq) break;
-        float best = 0.f;                               // ReLU output is >= 0
-        for (int i = 0; i < pool; ++i) {
-            float acc = bc;
+        float acc[4] = {bc, bc, bc, bc};
 #pragma unroll
-            for (int t = 0; t < kC1MaxTaps; ++t) {
-                if (t < n_taps) acc = fmaf(wr[t], xs[off[t] + ql * pool + i], acc);   // warp-broadcast read
+        for (int ci = 0; ci < kC1MaxCin; ++ci) {
+            if (ci < cin) {
+                float v[12];
+                const float4* src = reinterpret_cast<const float4*>(&xs[ci][4 * ql]);   // warp-broadcast
+#pragma unroll
+                for (int t = 0; t < 3; ++t) {
+                    const float4 f = src[t];
+                    v[4 * t] = f.x; v[4 * t + 1] = f.y; v[4 * t + 2] = f.z; v[4 * t + 3] = f.w;
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) acc[i] = fmaf(wr[ci][j], v[i + j], acc[i]);
             }
-            best = fmaxf(best, acc);
         }
+        float best = fmaxf(fmaxf(fmaxf(acc[0], acc[1]), fmaxf(acc[2], acc[3])), 0.f);   // max-pool, then ReLU
         if (c >= cout) best = 0.f;
         const float other = __shfl_down_sync(0xffffffffu, best, 1);
         if ((lane & 1) == 0) {
@@ -368,10 +514,10 @@ __global__ void __launch_bounds__(256) k_bbh_conv1(const float* __restrict__ x, 
 
 void launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
                       int cout, int cpad, int K, int pad_l, int pool, int fmt, cudaStream_t st) {
-    const int Lq = L / pool;
+    (void)pool;                                        // validated == 4 at create time
+    const int Lq = L / 4;
     dim3 grid((Lq + kC1Q - 1) / kC1Q, batch, cpad / 32);
-    const size_t smem = static_cast<size_t>(n_det) * (kC1Q * pool + K - 1) * sizeof(float);
-    k_bbh_conv1<<<grid, 256, smem, st>>>(x, w, b, out, n_det, L, cout, cpad, K, pad_l, pool, fmt);
+    k_bbh_conv1<<<grid, 256, 0, st>>>(x, w, b, out, n_det, L, cout, cpad, K, pad_l, fmt);
     ++g_kernel_launches;
 }
 

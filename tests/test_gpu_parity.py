@@ -105,6 +105,13 @@ def test_c0_streaming_deepclean_matches_oracle(dtype):
     print("C0 worst |d|/RMS:", stats)
 
 
+def test_odd_stride_uses_the_gather_path_and_matches_oracle():
+    """S odd: window positions do not pair up with ring slots, so the 16-bit mirror ring is off and the
+    window is re-gathered from the fp32 ring every update (strides down to 2-3 samples)."""
+    cfg = S.Config("C0-odd", S.StreamSpec(2, 1, 512, 120, 15), S.config_c0().dc_layers, seed=7)
+    _run_streaming(cfg, gw.GW_FP16, 20, white=True)
+
+
 def test_c0_simt_cross_check_matches_oracle():
     cfg = S.config_c0()
     _run_streaming(cfg, gw.GW_BF16, 10, white=True, impl=gw.GW_IMPL_SIMT)
