@@ -61,15 +61,6 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     return true;
 }
 
-template <int ACT>
-__device__ __forceinline__ float act_apply_t(float v) {
-    if (ACT == ACT_TANH) {
-        const float e = __expf(2.f * v);
-        return 1.f - __fdividef(2.f, 1.f + e);
-    }
-    if (ACT == ACT_RELU) return fmaxf(v, 0.f);
-    return v;
-}
 template <int FMT>
 __device__ __forceinline__ uint32_t pack_pair_t(float a, float b) {
     if (FMT == FMT_BF16) {
@@ -78,6 +69,30 @@ __device__ __forceinline__ uint32_t pack_pair_t(float a, float b) {
     }
     __half2 v = __floats2half2_rn(a, b);
     return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// Activation + rounding to the storage type of two neighbouring outputs.
+// tanh on the MUFU pipe is what bounds the thin layers' epilogue (16 lanes per clock per SM): the exact
+// form 1 - 2/(1 + e^{2v}) costs two MUFU ops (ex2, rcp) and six FP32 ops per element, tanh.approx.f32 one
+// MUFU op (relative error 2^-11: about one fp16 rounding step; SURVEY.md A18 allows it and the parity
+// tests hold the result to north_star's tolerances).  fp16 takes the one-op form, bf16 the exact one.  tanh.approx.f16x2 was
+// tried: ptxas splits it into two MUFU.TANH.F16, so it saves nothing and is less accurate.
+template <int ACT, int FMT>
+__device__ __forceinline__ uint32_t act_pack_t(float a, float b) {
+    if (ACT == ACT_TANH) {
+        if (FMT == FMT_BF16) {
+            // bf16 keeps the exact form: its per-element error budget is already spent on storage rounding
+            // and every flipped rounding costs 2^-8
+            const float ea = __expf(2.f * a), eb = __expf(2.f * b);
+            return pack_pair_t<FMT>(1.f - __fdividef(2.f, 1.f + ea), 1.f - __fdividef(2.f, 1.f + eb));
+        }
+        float ta, tb;
+        asm("tanh.approx.f32 %0, %1;" : "=f"(ta) : "f"(a));
+        asm("tanh.approx.f32 %0, %1;" : "=f"(tb) : "f"(b));
+        return pack_pair_t<FMT>(ta, tb);
+    }
+    if (ACT == ACT_RELU) return pack_pair_t<FMT>(fmaxf(a, 0.f), fmaxf(b, 0.f));
+    return pack_pair_t<FMT>(a, b);
 }
 
 __device__ __forceinline__ float act_apply(float v, int act) {
@@ -348,12 +363,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
 #pragma unroll
                             for (int j = 0; j < 8; ++j) {
                                 const float4 b4 = bia[which][j];
-                                const float v0 = act_apply_t<ACT>(__uint_as_float(r[4 * j]) + b4.x);
-                                const float v1 = act_apply_t<ACT>(__uint_as_float(r[4 * j + 1]) + b4.y);
-                                const float v2 = act_apply_t<ACT>(__uint_as_float(r[4 * j + 2]) + b4.z);
-                                const float v3 = act_apply_t<ACT>(__uint_as_float(r[4 * j + 3]) + b4.w);
-                                o[2 * j] = pack_pair_t<FMT>(v0, v1);
-                                o[2 * j + 1] = pack_pair_t<FMT>(v2, v3);
+                                o[2 * j] = act_pack_t<ACT, FMT>(__uint_as_float(r[4 * j]) + b4.x, __uint_as_float(r[4 * j + 1]) + b4.y);
+                                o[2 * j + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[4 * j + 2]) + b4.z, __uint_as_float(r[4 * j + 3]) + b4.w);
                             }
                             uint16_t* orow = reinterpret_cast<uint16_t*>(p.out) + (static_cast<size_t>(batch) * p.M + row) * p.N + col0;
                             uint4* dst = reinterpret_cast<uint4*>(orow);
