@@ -27,6 +27,7 @@ constexpr int kMaxShift = 6;       // distinct row shifts of one layer
 struct ConvGemmParams {
     CUtensorMap tmA;               // 3-D (cols, rows, batch), box (64, slab_rows, 1), SWIZZLE_128B
     CUtensorMap tmB;               // 3-D (K = 64 n_seg, N, n_det), box (64, N, 1), SWIZZLE_128B
+    CUtensorMap tmOut;             // EPI_STORE: 3-D (N, M, batch), box (min(N, 64), 32, 1), swizzle = box row (128B / 64B)
     const void* A;                 // raw pointers of the same operands (SIMT cross-check kernel)
     const void* B;
     int a_rows, a_cols;            // A view per batch item (logical rows: out-of-range rows read as zero)
@@ -47,6 +48,7 @@ struct ConvGemmParams {
     int slab_rows;                 // 128 + n_shift - 1: rows of A one output tile needs
     int b_resident;                // 1: all of B lives in shared memory for the CTA's lifetime
     int sa_stages, sb_stages;      // A-slab ring depth, B ring depth (streaming mode)
+    int out_bufs;                  // EPI_STORE: output staging buffers per epilogue warp (1 or 2)
     int tiles_m;                   // ceil(M / 128)
     const float* bias;             // [n_det][N]
     void* out;                     // EPI_STORE: [batch][M][N]; EPI_POOL: [batch][M/2][N/2], 16-bit

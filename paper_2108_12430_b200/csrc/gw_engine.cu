@@ -74,15 +74,17 @@ static int get_encode() {
 
 // 3-D tensor of 16-bit elements, dims (d0 fastest, d1, d2), strides in elements, box (64, box1, 1), 128B swizzle.
 static int make_tmap(CUtensorMap* tm, const void* base, int fmt, uint64_t d0, uint64_t d1, uint64_t d2,
-                     uint64_t stride1, uint64_t stride2, uint32_t box1) {
+                     uint64_t stride1, uint64_t stride2, uint32_t box1, uint32_t box0 = kSegK) {
     if (int rc = get_encode()) return rc;
     cuuint64_t dims[3] = {d0, d1, d2};
     cuuint64_t strides[2] = {stride1 * 2, stride2 * 2};
-    cuuint32_t box[3] = {static_cast<cuuint32_t>(kSegK), box1, 1};
+    cuuint32_t box[3] = {box0, box1, 1};
     cuuint32_t estr[3] = {1, 1, 1};
+    // the swizzle span equals the box row: 64 elements = 128 bytes, 32 elements = 64 bytes
+    const CUtensorMapSwizzle sw = box0 * 2 == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
     CUresult r = g_encode(tm, fmt == FMT_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3,
                           const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(GW_ECUDA, "cuTensorMapEncodeTiled failed (%d) dims %llu,%llu,%llu", (int)r,
                                        (unsigned long long)d0, (unsigned long long)d1, (unsigned long long)d2);
@@ -291,6 +293,8 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     p.epi = epi;
     p.act = H0.act;
     if (p.N > 256 || p.N % 32) return fail(GW_EINVAL, "GEMM N = %d unsupported (must be a multiple of 32, <= 256)", p.N);
+    if (epi == EPI_STORE && p.N != 32 && p.N != 64 && p.N != 128 && p.N != 256)
+        return fail(GW_EINVAL, "GEMM N = %d unsupported by the store epilogue (32, 64, 128 or 256)", p.N);
     if (p.a_cols % kSegK) return fail(GW_EINVAL, "A view width %d not a multiple of 64", p.a_cols);
     auto tap = [&](int a, int par, int r) -> int {
         switch (gk) {
@@ -362,6 +366,8 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     p.A = in; p.B = gl.d_B; p.bias = gl.d_bias; p.out = out;
     if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows_tm, batch, p.a_cols, static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, p.slab_rows)) return rc;
     if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.N)) return rc;
+    if (epi == EPI_STORE)   // output [batch][M][N]: one 32-row x min(N, 64)-column box per epilogue-warp store
+        if (int rc = make_tmap(&p.tmOut, out, fmt, p.N, p.M, batch, p.N, static_cast<uint64_t>(p.M) * p.N, 32, p.N >= 64 ? 64 : 32)) return rc;
     gl.g.batch = batch;
     p.head_hidden = head_hidden;
     int dev = 0, sms = 148;
