@@ -162,7 +162,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_empty + 2);
     float* head_s = reinterpret_cast<float*>(after_a + 2048);                // EPI_POOL_HEAD scratch
 
-    const int warp = threadIdx.x / 32;
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x / 32, 0);   // provably warp-uniform: role branches and
+                                                                      // everything under them use the uniform datapath
     const int lane = threadIdx.x % 32;
     const int det = blockIdx.x % p.n_det;
     const int worker = blockIdx.x / p.n_det;
@@ -187,7 +188,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
-    const uint32_t tmem_base = *tmem_slot;
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // uniform register
 
     if (warp == 0) {
         // ------------------------------------------------------------------------ TMA producer
@@ -228,11 +229,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         }
     } else if (warp == 1) {
         // -------------------------------------------------------------------------- MMA issuer
-        // The whole warp walks the loops (warp-uniform control flow keeps descriptors in uniform
-        // registers); one elected lane issues the MMAs and commits.  The issue cost per MMA has to stay
-        // well under the MMA's own 16..128 cycles, so with resident weights ONE elected block issues every
-        // shift of a slab (up to 6 x 4 MMAs) between one barrier wait and one commit; which shifts exist
-        // for column block cb is a 6-bit field of the register `shmask`.
+        // The whole warp walks the loops; one elected lane issues the MMAs and commits, selected by an
+        // instruction PREDICATE on the tcgen05 instruction itself (umma_f16_if), never by a branch: inside a
+        // divergent `if (elect)` block the compiler computes every descriptor in vector registers and moves
+        // it to uniform registers one R2UR at a time; clock64 stamps put that block at ~330 cycles fixed
+        // plus ~40 per MMA, which bounded every layer with N <= 128 (an MMA there executes in 16..64 cycles).
+        // Which shifts exist for column block cb is a 6-bit field of the register `shmask`.
         const uint32_t idesc = umma_idesc_f16(FMT, kTileM, p.N);
         if (p.b_resident) mbar_wait(bres_bar, 0);
         const uint32_t smem_a_u32 = smem_u32(smem_a), smem_b_u32 = smem_u32(smem_b);
@@ -244,6 +246,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         for (int cb = 0; cb < n_cb; ++cb)
             for (int sh = 0; sh < n_shift; ++sh)
                 if (p.seg_of[cb][sh] >= 0) shmask |= 1ull << (cb * kMaxShift + sh);
+        const uint32_t leader = elect_one() ? 1u : 0u;  // the one lane that issues (same lane every time)
         int it = 0;
         int stage = 0; uint32_t a_phase = 0;            // A ring position
         int bs = 0; uint32_t b_phase = 0;               // B ring position (streaming mode)
@@ -277,21 +280,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     }
                     const uint32_t a_lo = umma_desc_lo(smem_a_u32 + stage * sl);
                     if (resident) {
-                        if (elect_one()) {
-                            uint32_t acc_flag = accumulate, bl = b_lo;
-                            for (int sh = 0; sh < n_shift; ++sh) {
-                                if (!((m >> sh) & 1u)) continue;
-                                const uint32_t a_lo_s = a_lo + 8u * sh;    // +128 bytes = one slab row
+                        uint32_t acc_flag = accumulate, bl = b_lo;
+                        for (int sh = 0; sh < n_shift; ++sh) {
+                            if (!((m >> sh) & 1u)) continue;
+                            const uint32_t a_lo_s = a_lo + 8u * sh;        // +128 bytes = one slab row
 #pragma unroll
-                                for (int k = 0; k < kSegK / 16; ++k)       // +32 bytes along K: +2 in (addr >> 4)
-                                    umma_f16(d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, acc_flag | k);
-                                acc_flag = 1;
-                                bl += b_step;
-                            }
-                            umma_commit(&a_empty[stage]);                  // slab free once these MMAs retire
+                            for (int k = 0; k < kSegK / 16; ++k)           // +32 bytes along K: +2 in (addr >> 4)
+                                umma_f16_if(leader, d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, acc_flag | k);
+                            acc_flag = 1;
+                            bl += b_step;
                         }
-                        __syncwarp();
-                        b_lo += b_step * __popc(m);
+                        umma_commit_if(leader, &a_empty[stage]);           // slab free once these MMAs retire
+                        b_lo = bl;
                     } else {
                         for (int sh = 0; sh < n_shift; ++sh) {
                             if (!((m >> sh) & 1u)) continue;
@@ -300,14 +300,11 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             const uint32_t bl = umma_desc_lo(smem_b_u32 + bs * b_block);
                             const uint32_t a_lo_s = a_lo + 8u * sh;
                             const bool last = (m >> (sh + 1)) == 0;
-                            if (elect_one()) {
 #pragma unroll
-                                for (int k = 0; k < kSegK / 16; ++k)
-                                    umma_f16(d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, accumulate | k);
-                                umma_commit(&b_empty[bs]);
-                                if (last) umma_commit(&a_empty[stage]);
-                            }
-                            __syncwarp();
+                            for (int k = 0; k < kSegK / 16; ++k)
+                                umma_f16_if(leader, d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, accumulate | k);
+                            umma_commit_if(leader, &b_empty[bs]);
+                            if (last) umma_commit_if(leader, &a_empty[stage]);
                             accumulate = 1;
                             if (++bs == sb) { bs = 0; b_phase ^= 1; }
                         }
@@ -316,8 +313,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     if (++stage == sa) { stage = 0; a_phase ^= 1; }
                 }
             }
-            if (elect_one()) umma_commit(&tmem_full[acc]);                 // accumulator stage complete
-            __syncwarp();
+            umma_commit_if(leader, &tmem_full[acc]);                       // accumulator stage complete
         }
     } else {
         // ------------------------------------------------------------- epilogue warps 2..9 (8 warps)
