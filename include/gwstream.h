@@ -111,6 +111,12 @@ int64_t gw_kernel_launches(void);
  * layout, kept only to bisect tensor-core bugs in tests.  Both are CUDA; neither is a fallback. */
 int gw_set_conv_impl(int impl);
 
+/* Fuse the last tensor-core layer of DeepClean (ConvTranspose1d -> <= 32 channels, tanh) with the final
+ * 1-channel ConvTranspose1d (k = 7) into one kernel, for handles created AFTER this call (default 1).
+ * With 0 the activation between them is written to HBM and can be read with gw_deepclean_activation
+ * (test hook); with 1 that call returns GW_ESTATE for that layer.  Results agree within rounding. */
+int gw_set_fuse_tail(int on);
+
 /* ---- snapshotter -------------------------------------------------------------
  * gw_stream_create: zeroed ring state [n][C][W] fp32 on the current device, sample counter 0.
  *   Requires n >= 1, C >= 1, fs >= 1, 1 <= S <= W.

@@ -13,7 +13,7 @@ constexpr int kTileM = 128;        // UMMA M: one TMEM lane per output row
 constexpr int kSegK = 64;          // 64 x 16-bit = one 128-byte swizzle row
 
 enum { FMT_FP16 = 0, FMT_BF16 = 1 };                       // UMMA instruction-descriptor encoding
-enum { EPI_STORE = 0, EPI_POOL = 1, EPI_POOL_HEAD = 2 };
+enum { EPI_STORE = 0, EPI_POOL = 1, EPI_POOL_HEAD = 2, EPI_FINAL = 3 };
 enum { ACT_NONE = 0, ACT_TANH = 1, ACT_RELU = 2 };
 
 constexpr int kMaxCb = 8;          // 64-column blocks of the A view (a_cols <= 512)
@@ -49,7 +49,16 @@ struct ConvGemmParams {
     int b_resident;                // 1: all of B lives in shared memory for the CTA's lifetime
     int sa_stages, sb_stages;      // A-slab ring depth, B ring depth (streaming mode)
     int out_bufs;                  // EPI_STORE: output staging buffers per epilogue warp (1 or 2)
-    int tiles_m;                   // ceil(M / 128)
+    int tiles_m;                   // output tiles per batch item: ceil(M / tile_stride)
+    // Tile t covers output rows [t * tile_stride + tile_row0, ... + 128).  128 / 0 everywhere except
+    // EPI_FINAL, whose tiles overlap by one halo row on each side (126 / -1).
+    int tile_stride, tile_row0;
+    // EPI_FINAL: this layer (ConvTranspose1d -> 32 channels, tanh) and the network's last layer
+    // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel: the
+    // epilogue turns each accumulator row (positions 2m, 2m+1 x 32 channels) into 4 fp32 predictions.
+    const float* fin_w;            // [n_det][7][32] fp32 (storage-rounded weights, channels >= cin zero)
+    const float* fin_b;            // [n_det]
+    float* pred;                   // [batch][4 M] fp32
     const float* bias;             // [n_det][N]
     void* out;                     // EPI_STORE: [batch][M][N]; EPI_POOL: [batch][M/2][N/2], 16-bit
     // EPI_POOL_HEAD: global average pool over the M/2 pooled rows, dense head, sigmoid

@@ -32,6 +32,7 @@ constexpr int kGemmThreads = 64 + kEpiWarps * 32;   // producer warp, MMA warp, 
 constexpr int kAccCols = 256;                        // TMEM columns of one accumulator stage
 constexpr int kSmemBudget = 225 * 1024;
 constexpr int kFixedSmem = 1024 /*alignment slack*/ + 1024 /*bias*/ + 1024 /*barriers, tmem slot*/;
+constexpr int kFinalScratch = 2048;                  // EPI_FINAL: last-layer weights [7][32] fp32 + warp-edge exchange
 constexpr int kOutStage = kEpiWarps * 4096;          // output staging: 32 rows x 128 bytes per epilogue warp
 
 __host__ __device__ __forceinline__ int slab_bytes_of(int slab_rows) { return (slab_rows * 128 + 1023) & ~1023; }
@@ -51,7 +52,7 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
         p.out_bufs = (kFixedSmem + 2 * kOutStage + b_need + 4 * sl <= kSmemBudget) ? 2 : 1;
     }
     const int fixed = kFixedSmem + (p.epi == EPI_POOL_HEAD ? head_scratch_bytes(p.N, p.head_hidden) : 0) +
-                      p.out_bufs * kOutStage;
+                      (p.epi == EPI_FINAL ? kFinalScratch : 0) + p.out_bufs * kOutStage;
     int b_bytes;
     if (p.n_seg * b_block <= 132 * 1024 && fixed + p.n_seg * b_block + 2 * sl <= kSmemBudget) {
         p.b_resident = 1; p.sb_stages = 0; b_bytes = p.n_seg * b_block;
@@ -102,6 +103,19 @@ __device__ __forceinline__ uint32_t act_pack_t(float a, float b) {
     }
     if (ACT == ACT_RELU) return pack_pair_t<FMT>(fmaxf(a, 0.f), fmaxf(b, 0.f));
     return pack_pair_t<FMT>(a, b);
+}
+
+// The same activation on one value, kept in fp32 (EPI_FINAL feeds it straight into the last layer).
+template <int ACT, int FMT>
+__device__ __forceinline__ float act_f32_t(float a) {
+    if (ACT == ACT_TANH) {
+        if (FMT == FMT_BF16) return 1.f - __fdividef(2.f, 1.f + __expf(2.f * a));
+        float t;
+        asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(a));
+        return t;
+    }
+    if (ACT == ACT_RELU) return fmaxf(a, 0.f);
+    return a;
 }
 
 __device__ __forceinline__ float act_apply(float v, int act) {
@@ -168,7 +182,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int det = blockIdx.x % p.n_det;
     const int worker = blockIdx.x / p.n_det;
     const int n_workers = gridDim.x / p.n_det;
-    const int G = (EPI == EPI_STORE) ? kAccCols / p.N : 1;                   // tiles per accumulator stage
+    const int G = (EPI == EPI_STORE || EPI == EPI_FINAL) ? kAccCols / p.N : 1;                   // tiles per accumulator stage
     const int spi = (p.tiles_m + G - 1) / G;                                 // super-tiles per batch item
     const int total = n_items * spi;
 
@@ -205,7 +219,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 for (int g = 0; g < G; ++g) {
                     const int mt = (u % spi) * G + g;
                     if (mt >= p.tiles_m) break;
-                    const int m0 = mt * kTileM;
+                    const int m0 = mt * p.tile_stride + p.tile_row0;
                     for (int cb = 0; cb < p.n_cb; ++cb) {
                         const int stage = ia % sa;
                         mbar_wait(&a_empty[stage], ((ia / sa) & 1) ^ 1);
@@ -266,7 +280,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     if (ring) {
                         // window-edge zero padding: slab rows whose logical row is outside [0, M) hold
                         // neighbouring ring samples; clear them (whole 128-byte rows: swizzle-agnostic)
-                        const int lo = ((u % spi) * G + g) * kTileM + p.a_min;
+                        const int lo = ((u % spi) * G + g) * p.tile_stride + p.tile_row0 + p.a_min;
                         if (lo < 0 || lo + p.slab_rows > p.a_rows) {
                             uint8_t* slab = smem_a + stage * sl;
                             for (int idx = lane; idx < p.slab_rows * 8; idx += 32) {
@@ -332,6 +346,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             ch_g[i] = (32 * c) / p.N;
             ch_col[i] = (32 * c) % p.N;
         }
+        float fin_bias = 0.f;
+        if (EPI == EPI_FINAL) {
+            for (int i = et; i < 7 * 32; i += kEpiWarps * 32) head_s[i] = __ldg(p.fin_w + static_cast<size_t>(det) * 7 * 32 + i);
+            fin_bias = __ldg(p.fin_b + det);
+            asm volatile("bar.sync 1, 256;" ::: "memory");
+        }
+        const uint32_t fw_u32 = smem_u32(head_s);
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;   // + 32 KiB for the second buffer
         int ostep = 0;
         int it = 0;
@@ -405,6 +426,74 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             }
                         }
                         tma_store_commit();
+                    }
+                }
+            } else if (EPI == EPI_FINAL) {
+                // N = 64: accumulator row i of tile g is input position m = mt * 126 - 1 + i of this layer and
+                // holds its outputs x[2m][0..32) | x[2m+1][0..32).  The last layer (D3) is
+                //   y[2q]   = b + t1[q+1] + t3[q] + t5[q-1],   y[2q+1] = b + t0[q+2] + t2[q+1] + t4[q] + t6[q-1],
+                //   t_j[q] = sum_ci w[ci][j] tanh(x[q][ci])    (x = 0 outside the window),
+                // so a row needs t5, t6 of the previous row's odd position and t0, t1, t2 / t0 of the next row's
+                // even / odd position: lane shuffles inside a warp, a shared-memory exchange between the four
+                // warps of a tile, and one halo row on each side of the tile (rows 0 and 127 only feed their
+                // neighbours).  Warp (quad, hsel) takes rows [32 quad, +32) of tiles g = hsel, hsel + 2.
+                float* xch = head_s + 7 * 32;                          // after the weights [7][32]: [2 cp][2 hsel][4 quad][8]
+                for (int cp = 0; cp < 2; ++cp) {
+                    const int g = 2 * cp + hsel;
+                    const int mt = (u % spi) * G + g;
+                    uint32_t ra[32], rb[32];
+                    tmem_ld_32x32(taddr + 64 * g, ra);
+                    tmem_ld_32x32(taddr + 64 * g + 32, rb);
+                    tmem_ld_wait();
+                    if (cp == 1) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&tmem_empty[acc]);
+                    }
+                    float t0[7], t1[7];
+#pragma unroll
+                    for (int j = 0; j < 7; ++j) t0[j] = t1[j] = 0.f;
+#pragma unroll
+                    for (int c4 = 0; c4 < 8; ++c4) {
+                        const float4 be = lds_f4(bias_u32 + 16u * c4), bo = lds_f4(bias_u32 + 128u + 16u * c4);
+                        float xe[4], xo[4];
+                        xe[0] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4]) + be.x);
+                        xe[1] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4 + 1]) + be.y);
+                        xe[2] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4 + 2]) + be.z);
+                        xe[3] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4 + 3]) + be.w);
+                        xo[0] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4]) + bo.x);
+                        xo[1] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4 + 1]) + bo.y);
+                        xo[2] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4 + 2]) + bo.z);
+                        xo[3] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4 + 3]) + bo.w);
+#pragma unroll
+                        for (int j = 0; j < 7; ++j) {
+                            const float4 w = lds_f4(fw_u32 + 4u * (j * 32 + 4 * c4));      // warp-broadcast
+                            t0[j] = fmaf(w.x, xe[0], fmaf(w.y, xe[1], fmaf(w.z, xe[2], fmaf(w.w, xe[3], t0[j]))));
+                            t1[j] = fmaf(w.x, xo[0], fmaf(w.y, xo[1], fmaf(w.z, xo[2], fmaf(w.w, xo[3], t1[j]))));
+                        }
+                    }
+                    const int row = mt * p.tile_stride + p.tile_row0 + row_in_tile;
+                    const bool inside = mt < p.tiles_m && row >= 0 && row < p.M;
+                    if (!inside) {                                     // zero padding of the last layer's input
+#pragma unroll
+                        for (int j = 0; j < 7; ++j) t0[j] = t1[j] = 0.f;
+                    }
+                    float p5 = __shfl_up_sync(0xffffffffu, t1[5], 1), p6 = __shfl_up_sync(0xffffffffu, t1[6], 1);
+                    float n0 = __shfl_down_sync(0xffffffffu, t0[0], 1), n1 = __shfl_down_sync(0xffffffffu, t0[1], 1);
+                    float n2 = __shfl_down_sync(0xffffffffu, t0[2], 1), n3 = __shfl_down_sync(0xffffffffu, t1[0], 1);
+                    float* xw = xch + (cp * 8 + hsel * 4 + quad) * 8;
+                    if (lane == 0) { xw[0] = t0[0]; xw[1] = t0[1]; xw[2] = t0[2]; xw[3] = t1[0]; }
+                    if (lane == 31) { xw[4] = t1[5]; xw[5] = t1[6]; }
+                    asm volatile("bar.sync %0, 128;" ::"r"(2 + hsel) : "memory");
+                    if (lane == 0 && quad > 0) { p5 = xw[-8 + 4]; p6 = xw[-8 + 5]; }
+                    if (lane == 31 && quad < 3) { n0 = xw[8]; n1 = xw[8 + 1]; n2 = xw[8 + 2]; n3 = xw[8 + 3]; }
+                    if (inside && row_in_tile >= 1 && row_in_tile <= p.tile_stride) {
+                        float4 y;
+                        y.x = fin_bias + t1[1] + t0[3] + p5;
+                        y.y = fin_bias + n0 + t1[2] + t0[4] + p6;
+                        y.z = fin_bias + n1 + t1[3] + t0[5];
+                        y.w = fin_bias + n3 + n2 + t1[4] + t0[6];
+                        *reinterpret_cast<float4*>(p.pred + (static_cast<size_t>(batch) * p.M + row) * 4) = y;
                     }
                 }
             } else {
@@ -499,6 +588,7 @@ static GemmKernel pick_kernel(int epi, int act, int fmt) {
     GW_PICK(EPI_STORE, ACT_TANH)
     GW_PICK(EPI_STORE, ACT_NONE)
     GW_PICK(EPI_STORE, ACT_RELU)
+    GW_PICK(EPI_FINAL, ACT_TANH)
     GW_PICK(EPI_POOL, ACT_RELU)
     GW_PICK(EPI_POOL_HEAD, ACT_RELU)
 #undef GW_PICK
@@ -508,9 +598,9 @@ static GemmKernel pick_kernel(int epi, int act, int fmt) {
 static bool g_prepared = false;
 cudaError_t conv_gemm_prepare() {
     if (g_prepared) return cudaSuccess;
-    const int epis[5] = {EPI_STORE, EPI_STORE, EPI_STORE, EPI_POOL, EPI_POOL_HEAD};
-    const int acts[5] = {ACT_TANH, ACT_NONE, ACT_RELU, ACT_RELU, ACT_RELU};
-    for (int i = 0; i < 5; ++i)
+    const int epis[6] = {EPI_STORE, EPI_STORE, EPI_STORE, EPI_POOL, EPI_POOL_HEAD, EPI_FINAL};
+    const int acts[6] = {ACT_TANH, ACT_NONE, ACT_RELU, ACT_RELU, ACT_RELU, ACT_TANH};
+    for (int i = 0; i < 6; ++i)
         for (int fmt = 0; fmt < 2; ++fmt) {
             cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel(epis[i], acts[i], fmt)),
                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);

@@ -41,6 +41,11 @@ static int fail(int code, const char* fmt, ...) {
 
 extern "C" const char* gw_last_error(void) { return g_err.c_str(); }
 extern "C" int64_t gw_kernel_launches(void) { return g_kernel_launches; }
+static int g_fuse_tail = 1;
+extern "C" int gw_set_fuse_tail(int on) {
+    g_fuse_tail = on ? 1 : 0;
+    return GW_OK;
+}
 extern "C" int gw_set_conv_impl(int impl) {
     if (impl != GW_IMPL_UMMA && impl != GW_IMPL_SIMT) return fail(GW_EINVAL, "unknown conv impl %d", impl);
     g_conv_impl = impl;
@@ -217,6 +222,7 @@ struct gw_deepclean {
     std::vector<GemmLayer> gemm;                 // layers 0 .. n_layers-2
     void* ring16 = nullptr;                      // mirror ring [batch][2W][cpad0], 16-bit (when `mirror`)
     bool mirror = false;                         // first layer reads the window from ring16 (no per-update gather)
+    bool fused_tail = false;                     // last GEMM layer + final ConvTranspose1d run as one kernel (EPI_FINAL)
     std::vector<void*> act;                      // act[0] = gathered window (null when `mirror`), act[i+1] = output of layer i
     std::vector<int> act_rows, act_cols;
     float* d_wt_final = nullptr;                 // [n_det][K][cpad]
@@ -293,6 +299,7 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     p.epi = epi;
     p.act = H0.act;
     if (p.N > 256 || p.N % 32) return fail(GW_EINVAL, "GEMM N = %d unsupported (must be a multiple of 32, <= 256)", p.N);
+    if (epi == EPI_FINAL && p.N != 64) return fail(GW_EINVAL, "fused final layer needs GEMM N = 64, got %d", p.N);
     if (epi == EPI_STORE && p.N != 32 && p.N != 64 && p.N != 128 && p.N != 256)
         return fail(GW_EINVAL, "GEMM N = %d unsupported by the store epilogue (32, 64, 128 or 256)", p.N);
     if (p.a_cols % kSegK) return fail(GW_EINVAL, "A view width %d not a multiple of 64", p.a_cols);
@@ -331,7 +338,9 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     p.n_shift = a_hi - a_lo + 1;
     if (p.n_shift > kMaxShift) return fail(GW_EINVAL, "layer needs %d row shifts (max %d)", p.n_shift, kMaxShift);
     p.slab_rows = kTileM + p.n_shift - 1;
-    p.tiles_m = (p.M + kTileM - 1) / kTileM;
+    p.tile_stride = epi == EPI_FINAL ? kTileM - 2 : kTileM;     // EPI_FINAL: one halo row on each side
+    p.tile_row0 = epi == EPI_FINAL ? -1 : 0;
+    p.tiles_m = (p.M + p.tile_stride - 1) / p.tile_stride;
     memset(p.seg_of, 0xff, sizeof p.seg_of);
     for (int s = 0; s < n_seg; ++s) {
         p.seg_shift[s] = static_cast<int8_t>(seg_a[s]);
@@ -522,8 +531,17 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     // The 16-bit mirror ring replaces the per-update gather when window positions pair up with ring slots
     // (even stride => even head) and the first layer is a Conv1d; otherwise the window is re-gathered.
     dc->mirror = (S % 2 == 0) && (W % 2 == 0) && dc->host[0].kind == GW_CONV;
+    // The last GEMM layer (ConvTranspose1d -> <= 32 channels, tanh) and the final 1-channel ConvTranspose1d
+    // (k = 7) run as ONE kernel when they have the standard shape: the 16-bit activation between them is
+    // never written (at C3 that round trip is 2 x 1 MiB per detector-window, more than the layer's input).
+    {
+        const HostLayer &Hp = dc->host[nl - 2], &Hf = dc->host[nl - 1];
+        dc->fused_tail = g_fuse_tail && g_conv_impl == GW_IMPL_UMMA && nl >= 3 && Hp.kind == GW_CONVT &&
+                         Hp.act == GW_ACT_TANH && cpad[nl - 1] == 32 && Hf.k == 7 && Hf.pad_l == 3;
+    }
     for (int i = 0; i < nl; ++i) {                  // act[i] = input of layer i
         dc->act_rows[i] = len[i]; dc->act_cols[i] = cpad[i];
+        if (i == nl - 1 && dc->fused_tail) continue;  // never materialised
         size_t bytes = static_cast<size_t>(batch) * len[i] * cpad[i] * 2;
         void** dst = &dc->act[i];
         if (i == 0 && dc->mirror) { bytes *= 2; dst = &dc->ring16; }
@@ -536,8 +554,9 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         for (int d = 0; d < nd; ++d) per_det[d] = dc->host[d * nl + i];
         const GemmKind gk = dc->host[i].kind == GW_CONV ? GK_ENC : GK_DEC;
         const bool from_ring = i == 0 && dc->mirror;
+        const bool fin = i == nl - 2 && dc->fused_tail;
         if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, from_ring ? dc->ring16 : dc->act[i],
-                                      len[i], cpad[i], dc->act[i + 1], cpad[i + 1], batch, EPI_STORE, 0,
+                                      len[i], cpad[i], dc->act[i + 1], cpad[i + 1], batch, fin ? EPI_FINAL : EPI_STORE, 0,
                                       from_ring ? s->d_count : nullptr, from_ring ? W : 0))
             return rc;
         dc->gemm[i].name = "gemm.dc" + std::to_string(i);
@@ -545,6 +564,10 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         const HostLayer& H = dc->host[i];
         const double lin = len[i];
         dc->gemm[i].flops = 2.0 * (H.kind == GW_CONV ? lin / 2 : lin) * H.k * H.cin * H.cout;
+        if (fin) {                                   // the final layer's MACs run in this kernel too
+            const HostLayer& Hf = dc->host[nl - 1];
+            dc->gemm[i].flops += 2.0 * len[nl - 1] * Hf.k * Hf.cin * Hf.cout;
+        }
     }
     // final layer on CUDA cores: wt[d][j][ci] fp32 holding storage-rounded weights
     {
@@ -567,6 +590,10 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     const size_t wbytes = static_cast<size_t>(batch) * W * sizeof(float);
     CU_TRY(cudaMalloc(&dc->pred, wbytes));
     CU_TRY(cudaMemset(dc->pred, 0, wbytes));
+    if (dc->fused_tail) {
+        ConvGemmParams& p = dc->gemm[nl - 2].g.p;
+        p.fin_w = dc->d_wt_final; p.fin_b = dc->d_b_final; p.pred = dc->pred;
+    }
     CU_TRY(cudaMalloc(&dc->acc, wbytes));
     CU_TRY(cudaMemset(dc->acc, 0, wbytes));
     CU_TRY(cudaMalloc(&dc->final_buf, static_cast<size_t>(batch) * S * sizeof(float)));
@@ -644,9 +671,11 @@ static void deepclean_forward_enqueue(gw_deepclean* dc, cudaStream_t st) {
         prof_mark("gather", st);
     }
     for (auto& g : dc->gemm) run_gemm(g, st);
-    launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
-                       dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
-    prof_mark("final_convt", st);
+    if (!dc->fused_tail) {
+        launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
+                           dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
+        prof_mark("final_convt", st);
+    }
 }
 
 extern "C" int gw_deepclean_forward(gw_deepclean* dc, void* stream) {
@@ -671,6 +700,8 @@ extern "C" int gw_deepclean_activation(gw_deepclean* dc, int layer, void* out_de
                                        int* cols, void* stream) {
     if (!dc || layer < -1 || layer >= dc->n_layers - 1) return fail(GW_EINVAL, "gw_deepclean_activation: bad layer");
     const int i = layer + 1;
+    if (i == dc->n_layers - 1 && dc->fused_tail && out_dev)
+        return fail(GW_ESTATE, "layer %d's output is not materialised: it is fused with the final layer (gw_set_fuse_tail(0) to inspect it)", layer);
     if (rows) *rows = dc->act_rows[i];
     if (cols) *cols = dc->act_cols[i];
     const int64_t bytes = static_cast<int64_t>(dc->batch) * dc->act_rows[i] * dc->act_cols[i] * 2;

@@ -126,15 +126,26 @@ def test_c0_last_stride_mode_and_latency_offset():
 
 
 # ------------------------------------------------------------------------ layer-by-layer check
+@pytest.mark.parametrize("fuse", [False, True])
 @pytest.mark.parametrize("dtype", [gw.GW_FP16, gw.GW_BF16])
-def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype):
+def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype, fuse):
     """The full C1 network (21->32->64->128->256 and back, folded BatchNorm) on a 4096-sample window:
-    every stored activation against the oracle's, several M tiles and all channel widths."""
+    every stored activation against the oracle's, several M tiles and all channel widths.  fuse=True is
+    the production path (last tensor-core layer + final ConvTranspose1d in one kernel: the activation
+    between them is not materialised); fuse=False stores and checks that activation as well."""
     cfg = S.Config("C1-short", S.StreamSpec(2, 1, 4096, 4096, 512), S.config_c1().dc_layers, seed=1)
     dc_params, _ = util.make_params(cfg)
     dc_params2 = [dc_params[0]]
     st = gw.Stream(cfg.stream)
-    dc = gw.DeepClean(st, cfg.dc_layers, dc_params2, dtype)
+    gw.set_fuse_tail(fuse)
+    try:
+        dc = gw.DeepClean(st, cfg.dc_layers, dc_params2, dtype)
+    finally:
+        gw.set_fuse_tail(True)
+    if fuse:
+        with pytest.raises(gw.GwError) as e:
+            dc.activation(len(cfg.dc_layers) - 2)
+        assert e.value.code == gw.GW_ESTATE
     od, et = util.oracle_dtype(dtype), util.elem_tol(dtype)
     n_up = 8
     x = synth.multi_stream(3, cfg.stream, n_up * 512)
@@ -149,6 +160,8 @@ def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype):
         ref_p, acts = oracle.deepclean_forward(snap[cfg.stream.witness_rows(0)].astype(np.float64), cfg.dc_layers,
                                                prepared, return_all=True)
         for li, (layer, ref) in enumerate(zip(cfg.dc_layers[:-1], acts[:-1])):
+            if fuse and li == len(cfg.dc_layers) - 2:
+                continue
             got = dc.activation(li).float().cpu().numpy()[i, 0]          # [L][Cp]
             assert got.shape[0] == ref.shape[1]
             assert np.all(got[:, layer.cout:] == 0.0), "padded channels must stay zero"
