@@ -31,6 +31,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+from paper_2108_12430_b200 import shard               # noqa: E402
 from paper_2108_12430_b200 import specs as S          # noqa: E402
 from paper_2108_12430_b200 import synth               # noqa: E402
 
@@ -229,10 +230,7 @@ def run_native(args):
     launches = gw.kernel_launches() - launches0
     clocks = sampler.stop() if rank == 0 else None
     ms_total = ev0.elapsed_time(ev1)
-    if world > 1:
-        t = torch.tensor([ms_total], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = shard.max_over_ranks(ms_total, device="cuda")
     ds_per_step = sp.n_streams * sp.stride / FS
     value = world * K * ds_per_step / (ms_total / 1e3)
 
@@ -268,10 +266,7 @@ def run_native(args):
         pipe.step_host(chunks_h[step_no[0] % n_chunks], scores_h, final_h, cs); step_no[0] += 1
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = shard.max_over_ranks(e2e_s, device="cuda")
     h2d = sp.n_streams * sp.channels * sp.stride * 4
     d2h = sp.n_streams * 4 + sp.n_streams * sp.n_det * sp.stride * 4
     e2e = {"value": world * K * ds_per_step / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
