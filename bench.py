@@ -188,6 +188,10 @@ def run_native(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
+    if args.no_pdl:
+        gw.set_pdl(False)
+    if args.no_snake:
+        gw.set_snake(False)
     dtype = gw.GW_BF16 if args.dtype == "bf16" else gw.GW_FP16
     cfg = S.config_c3(args.streams, args.stride, WINDOW)
     sp = cfg.stream
@@ -304,10 +308,10 @@ def run_native(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        times, cores = oracle_rate(cfg, args.dtype, 2)
+        times, cores = oracle_rate(cfg, args.dtype, 200, budget_s=15.0)   # a bounded sample: ~15 s of oracle time
         sec = sum(times)
         cpu = {"value": len(times) * (sp.stride / FS) / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{len(times)} updates of one 2-detector stream of the same workload ({sec:.1f} s)"}
+               "sample": f"{len(times)} consecutive updates of one 2-detector stream of the same workload ({sec:.1f} s of oracle time)"}
 
     if rank == 0:
         line = {
@@ -338,6 +342,8 @@ def main():
     ap.add_argument("--stride", type=int, default=512)
     ap.add_argument("--dtype", default="fp16", choices=["fp16", "bf16"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-pdl", action="store_true", help="disable programmatic dependent launch (A/B aid)")
+    ap.add_argument("--no-snake", action="store_true", help="every layer walks its tiles forwards (A/B aid)")
     ap.add_argument("--timed-only", action="store_true",
                     help="only the warm-up and the timed region (for short runs under ncu); prints a reduced line")
     ap.add_argument("--reference-budget", type=float, default=150.0,

@@ -117,6 +117,17 @@ int gw_set_conv_impl(int impl);
  * (test hook); with 1 that call returns GW_ESTATE for that layer.  Results agree within rounding. */
 int gw_set_fuse_tail(int on);
 
+/* Programmatic dependent launch between the kernels of an update (default 1): each kernel is launched
+ * with the stream-serialization attribute and waits on the device (griddepcontrol.wait) before it touches
+ * what its predecessor wrote, so its prologue overlaps the predecessor's tail.  Takes effect for launches
+ * and graph captures made AFTER this call.  Results are identical either way. */
+int gw_set_pdl(int on);
+
+/* Alternate the direction in which consecutive DeepClean layers walk their (window, tile) work list, for
+ * handles created AFTER this call (default 1): a layer then starts on the activations its predecessor wrote
+ * last, which are still in L2.  Pure scheduling; results are bit-identical either way. */
+int gw_set_snake(int on);
+
 /* ---- snapshotter -------------------------------------------------------------
  * gw_stream_create: zeroed ring state [n][C][W] fp32 on the current device, sample counter 0.
  *   Requires n >= 1, C >= 1, fs >= 1, 1 <= S <= W.

@@ -21,7 +21,7 @@ GW_FINAL, GW_RUNNING = 0, 1
 GW_IMPL_UMMA, GW_IMPL_SIMT = 0, 1
 
 EXPORTS = [
-    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail",
+    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake",
     "gw_stream_create", "gw_stream_destroy", "gw_stream_update", "gw_stream_snapshot", "gw_stream_count",
     "gw_deepclean_create", "gw_deepclean_destroy", "gw_deepclean_forward", "gw_deepclean_noise",
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
@@ -74,6 +74,8 @@ def lib():
         L.gw_kernel_launches.restype = i64
         L.gw_set_conv_impl.argtypes = [i]
         L.gw_set_fuse_tail.argtypes = [i]
+        L.gw_set_pdl.argtypes = [i]
+        L.gw_set_snake.argtypes = [i]
         L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
         L.gw_stream_destroy.argtypes = [vp]
         L.gw_stream_update.argtypes = [vp, vp, vp]
@@ -121,6 +123,16 @@ def set_conv_impl(impl: int) -> None:
 def set_fuse_tail(on: bool) -> None:
     """Fused last-GEMM-layer + final ConvTranspose1d kernel for handles created after this call (default on)."""
     _check(lib().gw_set_fuse_tail(1 if on else 0))
+
+
+def set_pdl(on: bool) -> None:
+    """Programmatic dependent launch between the kernels of an update (default on)."""
+    _check(lib().gw_set_pdl(1 if on else 0))
+
+
+def set_snake(on: bool) -> None:
+    """Alternating traversal direction of consecutive DeepClean layers (L2 reuse; default on)."""
+    _check(lib().gw_set_snake(1 if on else 0))
 
 
 def _fp(a: Optional[np.ndarray]):

@@ -53,10 +53,15 @@ struct ConvGemmParams {
     // Tile t covers output rows [t * tile_stride + tile_row0, ... + 128).  128 / 0 everywhere except
     // EPI_FINAL, whose tiles overlap by one halo row on each side (126 / -1).
     int tile_stride, tile_row0;
+    // 1: walk the (batch item, tile) work list backwards.  Consecutive layers alternate direction, so a
+    // layer starts on the activations its predecessor wrote LAST -- the part still resident in the 126 MB L2.
+    int reverse;
     // EPI_FINAL: this layer (ConvTranspose1d -> 32 channels, tanh) and the network's last layer
-    // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel: the
-    // epilogue turns each accumulator row (positions 2m, 2m+1 x 32 channels) into 4 fp32 predictions.
-    const float* fin_w;            // [n_det][7][32] fp32 (storage-rounded weights, channels >= cin zero)
+    // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel.  The
+    // epilogue writes each activated accumulator row (positions 2m, 2m+1 x 32 channels = one 128-byte
+    // row) to a shared-memory tile in the swizzled K-major layout, and a SECOND chain of tcgen05.mma
+    // (M 128, N 16, K 3 x 64: rows m-1, m, m+1) turns it into the 4 predictions y[4m .. 4m+3].
+    CUtensorMap tmF;               // last layer as a B operand: 3-D (K = 3 x 64, N = 16, n_det), box (64, 16, 1)
     const float* fin_b;            // [n_det]
     float* pred;                   // [batch][4 M] fp32
     const float* bias;             // [n_det][N]
@@ -66,6 +71,9 @@ struct ConvGemmParams {
     int head_hidden;
     float* scores;                 // [batch]
     float* pooled_dbg;             // optional [batch][M/2][N/2] fp32 (SIMT path scratch)
+#ifdef GW_TRACE
+    long long* trace;              // [grid][16] cycle counters of the roles (diagnostic builds only)
+#endif
     int8_t seg_of[kMaxCb][kMaxShift];     // B K-block of segment (cb, shift), -1 if the segment is empty
     int8_t seg_shift[kMaxSeg];     // per segment s: row shift, first column (SIMT kernel)
     int16_t seg_col[kMaxSeg];
@@ -116,5 +124,6 @@ void launch_bbh_conv1(const float* x, const float* w, const float* b, void* out,
                       int cout, int cpad, int K, int pad_l, int pool, int fmt, cudaStream_t st);
 
 extern long long g_kernel_launches;
+extern int g_pdl;                  // 1: kernels of a step are launched with programmatic stream serialization
 
 }  // namespace gw

@@ -27,12 +27,28 @@
 
 namespace gw {
 
+// Diagnostic builds (GW_TRACE=1 python -m paper_2108_12430_b200.build): per-role cycle counters of where each
+// CTA waits, written to p.trace and printed by gw_step_profile.  Compiled out of the product build.
+#ifdef GW_TRACE
+#define TR_DECL long long tr_[8] = {0, 0, 0, 0, 0, 0, 0, 0}; const long long tr_t0 = clock64();
+#define TR_WAIT(slot, stmt) { const long long t_ = clock64(); stmt; tr_[slot] += clock64() - t_; }
+#define TR_FLUSH(base, n) if (lane == 0 && p.trace) { for (int i_ = 0; i_ < n; ++i_) p.trace[blockIdx.x * 16 + base + i_] = tr_[i_]; p.trace[blockIdx.x * 16 + base + n] = clock64() - tr_t0; }
+#else
+#define TR_DECL
+#define TR_WAIT(slot, stmt) stmt;
+#define TR_FLUSH(base, n)
+#endif
+
 constexpr int kEpiWarps = 8;
 constexpr int kGemmThreads = 64 + kEpiWarps * 32;   // producer warp, MMA warp, 8 epilogue warps
 constexpr int kAccCols = 256;                        // TMEM columns of one accumulator stage
 constexpr int kSmemBudget = 225 * 1024;
 constexpr int kFixedSmem = 1024 /*alignment slack*/ + 1024 /*bias*/ + 1024 /*barriers, tmem slot*/;
-constexpr int kFinalScratch = 2048;                  // EPI_FINAL: last-layer weights [7][32] fp32 + warp-edge exchange
+constexpr int kFinBlock = 16 * 128;                  // EPI_FINAL: one K block (64) of the last layer's B operand, N = 16 rows
+constexpr int kFinalScratch = 3 * kFinBlock;         // EPI_FINAL: last-layer B operand, 3 row shifts
+constexpr int kFinTile = kTileM * 128;               // EPI_FINAL: one activated tile, 128 rows x 128 bytes
+constexpr int kFinN = 16;                            // EPI_FINAL: N of the second MMA chain (4 real columns)
+constexpr int kFinCol = 128;                         // EPI_FINAL: TMEM column of the second chain's accumulators in a stage
 constexpr int kOutStage = kEpiWarps * 4096;          // output staging: 32 rows x 128 bytes per epilogue warp
 
 __host__ __device__ __forceinline__ int slab_bytes_of(int slab_rows) { return (slab_rows * 128 + 1023) & ~1023; }
@@ -47,6 +63,7 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     // EPI_STORE stages its output through shared memory for TMA stores: one 4 KiB buffer per epilogue warp,
     // two when the operands leave room (thin layers)
     p.out_bufs = 0;
+    if (p.epi == EPI_FINAL) p.out_bufs = 2;               // four activated tiles: [accumulator stage][tile in stage]
     if (p.epi == EPI_STORE) {
         const int b_need = p.n_seg * b_block <= 132 * 1024 ? p.n_seg * b_block : 4 * b_block;
         p.out_bufs = (kFixedSmem + 2 * kOutStage + b_need + 4 * sl <= kSmemBudget) ? 2 : 1;
@@ -174,7 +191,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     uint64_t* tmem_full = bres_bar + 1;      // [2]
     uint64_t* tmem_empty = tmem_full + 2;    // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+    uint64_t* stg_full = bars + 32;          // [2 stages][2 tiles] EPI_FINAL: activated tile written to shared memory
+    uint64_t* fin_full = stg_full + 4;       // [2][2]              EPI_FINAL: second MMA chain of that tile complete
     float* head_s = reinterpret_cast<float*>(after_a + 2048);                // EPI_POOL_HEAD scratch
+    uint8_t* smem_fin = after_a + 2048;                                      // EPI_FINAL: last layer's B operand (1024-aligned)
 
     const int warp = __shfl_sync(0xffffffffu, threadIdx.x / 32, 0);   // provably warp-uniform: role branches and
                                                                       // everything under them use the uniform datapath
@@ -182,7 +202,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int det = blockIdx.x % p.n_det;
     const int worker = blockIdx.x / p.n_det;
     const int n_workers = gridDim.x / p.n_det;
-    const int G = (EPI == EPI_STORE || EPI == EPI_FINAL) ? kAccCols / p.N : 1;                   // tiles per accumulator stage
+    const int G = EPI == EPI_STORE ? kAccCols / p.N : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
     const int spi = (p.tiles_m + G - 1) / G;                                 // super-tiles per batch item
     const int total = n_items * spi;
 
@@ -190,10 +210,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         if (lane == 0) {
             tma_prefetch_desc(&p.tmA);
             tma_prefetch_desc(&p.tmB);
+            if (EPI == EPI_FINAL) tma_prefetch_desc(&p.tmF);
             for (int i = 0; i < sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
             for (int i = 0; i < sb; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
             mbar_init(bres_bar, 1);
             for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full[i], 1); mbar_init(&tmem_empty[i], kEpiWarps); }
+            for (int i = 0; i < 4; ++i) { mbar_init(&stg_full[i], 4); mbar_init(&fin_full[i], 1); }
             fence_barrier_init();
         }
         __syncwarp();
@@ -203,18 +225,27 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);   // uniform register
+    // Programmatic dependent launch: the next kernel of the step may be scheduled onto SMs as this grid's
+    // CTAs retire (its prologue and weight loads overlap our tail); we ourselves touch nothing the previous
+    // kernel wrote before griddep_wait().  Weights and biases are constants of the engine.
+    griddep_launch_dependents();
 
     if (warp == 0) {
         // ------------------------------------------------------------------------ TMA producer
         if (lane == 0) {
             if (p.b_resident) {
-                mbar_arrive_expect_tx(bres_bar, p.n_seg * b_block);
+                mbar_arrive_expect_tx(bres_bar, p.n_seg * b_block + (EPI == EPI_FINAL ? kFinalScratch : 0));
                 for (int s = 0; s < p.n_seg; ++s) tma_load_3d(smem_b + s * b_block, &p.tmB, bres_bar, s * kSegK, 0, det);
+                if (EPI == EPI_FINAL)
+                    for (int s = 0; s < 3; ++s) tma_load_3d(smem_fin + s * kFinBlock, &p.tmF, bres_bar, s * kSegK, 0, det);
             }
+            griddep_wait();
             int ia = 0, ib = 0;
+            TR_DECL
             // mirror-ring source: the window starts at ring row (count mod W) / div (see ConvGemmParams)
             const int row_off = p.a_count ? static_cast<int>((*p.a_count % p.a_ring_W) / p.a_ring_div) : 0;
-            for (int u = worker; u < total; u += n_workers) {
+            for (int w = worker; w < total; w += n_workers) {
+                const int u = p.reverse ? total - 1 - w : w;
                 const int batch = (u / spi) * p.n_det + det;
                 for (int g = 0; g < G; ++g) {
                     const int mt = (u % spi) * G + g;
@@ -222,7 +253,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     const int m0 = mt * p.tile_stride + p.tile_row0;
                     for (int cb = 0; cb < p.n_cb; ++cb) {
                         const int stage = ia % sa;
-                        mbar_wait(&a_empty[stage], ((ia / sa) & 1) ^ 1);
+                        TR_WAIT(0, mbar_wait(&a_empty[stage], ((ia / sa) & 1) ^ 1))
                         mbar_arrive_expect_tx(&a_full[stage], p.slab_rows * 128);
                         tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min + row_off, batch);
                         ++ia;
@@ -231,7 +262,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                                 const int s = p.seg_of[cb][sh];
                                 if (s < 0) continue;
                                 const int bs = ib % sb;
-                                mbar_wait(&b_empty[bs], ((ib / sb) & 1) ^ 1);
+                                TR_WAIT(1, mbar_wait(&b_empty[bs], ((ib / sb) & 1) ^ 1))
                                 mbar_arrive_expect_tx(&b_full[bs], b_block);
                                 tma_load_3d(smem_b + bs * b_block, &p.tmB, &b_full[bs], s * kSegK, 0, det);
                                 ++ib;
@@ -240,6 +271,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     }
                 }
             }
+            TR_FLUSH(0, 2)
         }
     } else if (warp == 1) {
         // -------------------------------------------------------------------------- MMA issuer
@@ -262,11 +294,36 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 if (p.seg_of[cb][sh] >= 0) shmask |= 1ull << (cb * kMaxShift + sh);
         const uint32_t leader = elect_one() ? 1u : 0u;  // the one lane that issues (same lane every time)
         int it = 0;
+        TR_DECL
         int stage = 0; uint32_t a_phase = 0;            // A ring position
         int bs = 0; uint32_t b_phase = 0;               // B ring position (streaming mode)
-        for (int u = worker; u < total; u += n_workers, ++it) {
+        // EPI_FINAL: the second chain of super-tile `itp` (both tiles): D row i = rows i, i+1, i+2 of the
+        // activated tile (tile rows m-1, m, m+1 of output row m = i + 1) times the last layer's three K blocks.
+        const uint32_t idesc_fin = umma_idesc_f16(FMT, kTileM, kFinN);
+        const uint32_t fin_lo = umma_desc_lo(smem_u32(smem_fin));
+        const uint32_t stg_lo = umma_desc_lo(smem_u32(smem_out));
+        auto issue_final = [&](int itp) {
+            const int accp = itp & 1;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                TR_WAIT(3, mbar_wait(&stg_full[accp * 2 + h], (itp >> 1) & 1))
+                tc_fence_after();
+                const uint32_t d_fin = tmem_base + accp * kAccCols + kFinCol + h * kFinN;
+                const uint32_t a_t = stg_lo + static_cast<uint32_t>((accp * 2 + h) * kFinTile >> 4);
+#pragma unroll
+                for (int sh = 0; sh < 3; ++sh)
+#pragma unroll
+                    for (int k = 0; k < kSegK / 16; ++k)
+                        umma_f16_if(leader, d_fin, umma_desc_make(a_t + 8u * sh + 2 * k),
+                                    umma_desc_make(fin_lo + static_cast<uint32_t>(sh * kFinBlock >> 4) + 2 * k), idesc_fin,
+                                    (sh | k) ? 1u : 0u);
+                umma_commit_if(leader, &fin_full[accp * 2 + h]);
+            }
+        };
+        for (int w = worker; w < total; w += n_workers, ++it) {
+            const int u = p.reverse ? total - 1 - w : w;
             const int acc = it & 1;
-            mbar_wait(&tmem_empty[acc], ((it >> 1) & 1) ^ 1);
+            TR_WAIT(0, mbar_wait(&tmem_empty[acc], ((it >> 1) & 1) ^ 1))
             tc_fence_after();
             const int g_end = min(G, p.tiles_m - (u % spi) * G);
             for (int g = 0; g < g_end; ++g) {
@@ -275,7 +332,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 uint32_t b_lo = umma_desc_lo(smem_b_u32);                  // resident: block 0 of B
                 for (int cb = 0; cb < n_cb; ++cb) {
                     const uint32_t m = static_cast<uint32_t>(shmask >> (cb * kMaxShift)) & ((1u << kMaxShift) - 1);
-                    mbar_wait(&a_full[stage], a_phase);
+                    TR_WAIT(1, mbar_wait(&a_full[stage], a_phase))
                     tc_fence_after();
                     if (ring) {
                         // window-edge zero padding: slab rows whose logical row is outside [0, M) hold
@@ -309,7 +366,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     } else {
                         for (int sh = 0; sh < n_shift; ++sh) {
                             if (!((m >> sh) & 1u)) continue;
-                            mbar_wait(&b_full[bs], b_phase);
+                            TR_WAIT(2, mbar_wait(&b_full[bs], b_phase))
                             tc_fence_after();
                             const uint32_t bl = umma_desc_lo(smem_b_u32 + bs * b_block);
                             const uint32_t a_lo_s = a_lo + 8u * sh;
@@ -328,7 +385,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 }
             }
             umma_commit_if(leader, &tmem_full[acc]);                       // accumulator stage complete
+            if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);           // behind this stage's MMAs in the pipe
         }
+        if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);
+        TR_FLUSH(3, 4)
     } else {
         // ------------------------------------------------------------- epilogue warps 2..9 (8 warps)
         const int quad = warp % 4;                             // TMEM lane quadrant this warp may read
@@ -346,20 +406,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             ch_g[i] = (32 * c) / p.N;
             ch_col[i] = (32 * c) % p.N;
         }
-        float fin_bias = 0.f;
-        if (EPI == EPI_FINAL) {
-            for (int i = et; i < 7 * 32; i += kEpiWarps * 32) head_s[i] = __ldg(p.fin_w + static_cast<size_t>(det) * 7 * 32 + i);
-            fin_bias = __ldg(p.fin_b + det);
-            asm volatile("bar.sync 1, 256;" ::: "memory");
-        }
-        const uint32_t fw_u32 = smem_u32(head_s);
+        griddep_wait();                                        // before the first global store of this grid
+        const float fin_bias = EPI == EPI_FINAL ? __ldg(p.fin_b + det) : 0.f;
+        int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL: the tile whose second chain is in flight
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;   // + 32 KiB for the second buffer
         int ostep = 0;
         int it = 0;
-        for (int u = worker; u < total; u += n_workers, ++it) {
+        TR_DECL
+        for (int w = worker; w < total; w += n_workers, ++it) {
+            const int u = p.reverse ? total - 1 - w : w;
             const int acc = it & 1;
             const int batch = (u / spi) * p.n_det + det;
-            mbar_wait(&tmem_full[acc], (it >> 1) & 1);
+            TR_WAIT(0, mbar_wait(&tmem_full[acc], (it >> 1) & 1))
             tc_fence_after();
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * kAccCols;
             if (EPI == EPI_STORE) {
@@ -382,7 +440,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                         for (int j = 0; j < 8; ++j) bia[which][j] = lds_f4(bias_u32 + 4u * (ch_col[2 * cp + which] + 4 * j));
                     const uint32_t stg = stage_u32 + ((ostep % p.out_bufs) << 15);
                     if (lane == 0) {                           // the store that last read this buffer has drained it
-                        if (p.out_bufs == 2) tma_store_wait_read<1>(); else tma_store_wait_read<0>();
+                        TR_WAIT(1, if (p.out_bufs == 2) tma_store_wait_read<1>(); else tma_store_wait_read<0>())
                     }
                     ++ostep;
                     tmem_ld_wait();
@@ -429,73 +487,58 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     }
                 }
             } else if (EPI == EPI_FINAL) {
-                // N = 64: accumulator row i of tile g is input position m = mt * 126 - 1 + i of this layer and
-                // holds its outputs x[2m][0..32) | x[2m+1][0..32).  The last layer (D3) is
-                //   y[2q]   = b + t1[q+1] + t3[q] + t5[q-1],   y[2q+1] = b + t0[q+2] + t2[q+1] + t4[q] + t6[q-1],
-                //   t_j[q] = sum_ci w[ci][j] tanh(x[q][ci])    (x = 0 outside the window),
-                // so a row needs t5, t6 of the previous row's odd position and t0, t1, t2 / t0 of the next row's
-                // even / odd position: lane shuffles inside a warp, a shared-memory exchange between the four
-                // warps of a tile, and one halo row on each side of the tile (rows 0 and 127 only feed their
-                // neighbours).  Warp (quad, hsel) takes rows [32 quad, +32) of tiles g = hsel, hsel + 2.
-                float* xch = head_s + 7 * 32;                          // after the weights [7][32]: [2 cp][2 hsel][4 quad][8]
-                for (int cp = 0; cp < 2; ++cp) {
-                    const int g = 2 * cp + hsel;
-                    const int mt = (u % spi) * G + g;
-                    uint32_t ra[32], rb[32];
-                    tmem_ld_32x32(taddr + 64 * g, ra);
-                    tmem_ld_32x32(taddr + 64 * g + 32, rb);
-                    tmem_ld_wait();
-                    if (cp == 1) {
-                        tc_fence_before();
-                        __syncwarp();
-                        if (lane == 0) mbar_arrive(&tmem_empty[acc]);
-                    }
-                    float t0[7], t1[7];
+                // N = 64, two tiles per stage: accumulator row i of tile g is input position m = mt * 126 - 1 + i of
+                // this layer and holds its outputs x[2m][0..32) | x[2m+1][0..32) = one 128-byte row of the last
+                // layer's A operand.  Warp (quad, hsel) activates rows [32 quad, +32) of tile g = hsel, writes them
+                // (16-bit, zero outside the window = the last layer's padding) into the shared-memory tile
+                // [acc][hsel] in the swizzled K-major layout and hands the tile to the MMA warp; the last layer
+                //   y[4m + r] = b + sum_{a, par, ci} w[ci][r + 3 - 4a - 2 par] x[2(m + a) + par][ci],  a = -1, 0, 1,
+                // is then three row-shifted K blocks on the tensor core (D3).  The 4 results of the
+                // PREVIOUS tile are read back one iteration later, when its chain has long retired.
+                const int mt = (u % spi) * G + hsel;
+                uint32_t ra[32], rb[32];
+                tmem_ld_32x32(taddr + 64 * hsel, ra);
+                tmem_ld_32x32(taddr + 64 * hsel + 32, rb);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tmem_empty[acc]);
+                const int row = mt * p.tile_stride + p.tile_row0 + row_in_tile;
+                const bool inside = mt < p.tiles_m && row >= 0 && row < p.M;
+                const uint32_t tile_u32 = smem_u32(smem_out) + (acc * 2 + hsel) * kFinTile + quad * 4096;
 #pragma unroll
-                    for (int j = 0; j < 7; ++j) t0[j] = t1[j] = 0.f;
+                for (int which = 0; which < 2; ++which) {
+                    const uint32_t* r = which == 0 ? ra : rb;
 #pragma unroll
-                    for (int c4 = 0; c4 < 8; ++c4) {
-                        const float4 be = lds_f4(bias_u32 + 16u * c4), bo = lds_f4(bias_u32 + 128u + 16u * c4);
-                        float xe[4], xo[4];
-                        xe[0] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4]) + be.x);
-                        xe[1] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4 + 1]) + be.y);
-                        xe[2] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4 + 2]) + be.z);
-                        xe[3] = act_f32_t<ACT, FMT>(__uint_as_float(ra[4 * c4 + 3]) + be.w);
-                        xo[0] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4]) + bo.x);
-                        xo[1] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4 + 1]) + bo.y);
-                        xo[2] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4 + 2]) + bo.z);
-                        xo[3] = act_f32_t<ACT, FMT>(__uint_as_float(rb[4 * c4 + 3]) + bo.w);
+                    for (int jj = 0; jj < 4; ++jj) {
+                        uint32_t o[4];
 #pragma unroll
-                        for (int j = 0; j < 7; ++j) {
-                            const float4 w = lds_f4(fw_u32 + 4u * (j * 32 + 4 * c4));      // warp-broadcast
-                            t0[j] = fmaf(w.x, xe[0], fmaf(w.y, xe[1], fmaf(w.z, xe[2], fmaf(w.w, xe[3], t0[j]))));
-                            t1[j] = fmaf(w.x, xo[0], fmaf(w.y, xo[1], fmaf(w.z, xo[2], fmaf(w.w, xo[3], t1[j]))));
+                        for (int h = 0; h < 2; ++h) {
+                            const float4 b4 = lds_f4(bias_u32 + 4u * (32 * which + 8 * jj + 4 * h));
+                            o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
+                            o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
                         }
-                    }
-                    const int row = mt * p.tile_stride + p.tile_row0 + row_in_tile;
-                    const bool inside = mt < p.tiles_m && row >= 0 && row < p.M;
-                    if (!inside) {                                     // zero padding of the last layer's input
-#pragma unroll
-                        for (int j = 0; j < 7; ++j) t0[j] = t1[j] = 0.f;
-                    }
-                    float p5 = __shfl_up_sync(0xffffffffu, t1[5], 1), p6 = __shfl_up_sync(0xffffffffu, t1[6], 1);
-                    float n0 = __shfl_down_sync(0xffffffffu, t0[0], 1), n1 = __shfl_down_sync(0xffffffffu, t0[1], 1);
-                    float n2 = __shfl_down_sync(0xffffffffu, t0[2], 1), n3 = __shfl_down_sync(0xffffffffu, t1[0], 1);
-                    float* xw = xch + (cp * 8 + hsel * 4 + quad) * 8;
-                    if (lane == 0) { xw[0] = t0[0]; xw[1] = t0[1]; xw[2] = t0[2]; xw[3] = t1[0]; }
-                    if (lane == 31) { xw[4] = t1[5]; xw[5] = t1[6]; }
-                    asm volatile("bar.sync %0, 128;" ::"r"(2 + hsel) : "memory");
-                    if (lane == 0 && quad > 0) { p5 = xw[-8 + 4]; p6 = xw[-8 + 5]; }
-                    if (lane == 31 && quad < 3) { n0 = xw[8]; n1 = xw[8 + 1]; n2 = xw[8 + 2]; n3 = xw[8 + 3]; }
-                    if (inside && row_in_tile >= 1 && row_in_tile <= p.tile_stride) {
-                        float4 y;
-                        y.x = fin_bias + t1[1] + t0[3] + p5;
-                        y.y = fin_bias + n0 + t1[2] + t0[4] + p6;
-                        y.z = fin_bias + n1 + t1[3] + t0[5];
-                        y.w = fin_bias + n3 + n2 + t1[4] + t0[6];
-                        *reinterpret_cast<float4*>(p.pred + (static_cast<size_t>(batch) * p.M + row) * 4) = y;
+                        if (!inside) o[0] = o[1] = o[2] = o[3] = 0u;
+                        sts_u4(tile_u32 + lane * 128 + (((4 * which + jj) ^ (lane & 7)) << 4), o[0], o[1], o[2], o[3]);
                     }
                 }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&stg_full[acc * 2 + hsel]);
+                if (it > 0) {
+                    const int accp = acc ^ 1;
+                    TR_WAIT(2, mbar_wait(&fin_full[accp * 2 + hsel], ((it - 1) >> 1) & 1))
+                    tc_fence_after();
+                    uint32_t y[4];
+                    tmem_ld_32x4(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + hsel * kFinN, y);
+                    tmem_ld_wait();
+                    const int orow = prev_mt * p.tile_stride + row_in_tile;     // D row i = tile row i + 1
+                    if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M)
+                        *reinterpret_cast<float4*>(p.pred + (static_cast<size_t>(prev_batch) * p.M + orow) * 4) =
+                            make_float4(__uint_as_float(y[0]) + fin_bias, __uint_as_float(y[1]) + fin_bias,
+                                        __uint_as_float(y[2]) + fin_bias, __uint_as_float(y[3]) + fin_bias);
+                }
+                prev_batch = batch; prev_mt = mt;
             } else {
                 // conv (stride 1) + bias + ReLU + MaxPool(4): row m holds outputs 2m (cols [0,N/2)) and 2m+1
                 // (cols [N/2,N)); pooled row q = m/2 is the max over both halves of rows 2q and 2q+1.
@@ -573,6 +616,20 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 }
             }
         }
+        if (EPI == EPI_FINAL && it > 0) {                      // the last tile's second chain
+            const int accp = (it - 1) & 1;
+            mbar_wait(&fin_full[accp * 2 + hsel], ((it - 1) >> 1) & 1);
+            tc_fence_after();
+            uint32_t y[4];
+            tmem_ld_32x4(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + hsel * kFinN, y);
+            tmem_ld_wait();
+            const int orow = prev_mt * p.tile_stride + row_in_tile;
+            if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M)
+                *reinterpret_cast<float4*>(p.pred + (static_cast<size_t>(prev_batch) * p.M + orow) * 4) =
+                    make_float4(__uint_as_float(y[0]) + fin_bias, __uint_as_float(y[1]) + fin_bias,
+                                __uint_as_float(y[2]) + fin_bias, __uint_as_float(y[3]) + fin_bias);
+        }
+        if (warp == 2) { TR_FLUSH(8, 3) }
     }
     if (EPI == EPI_STORE && warp >= 2 && lane == 0) tma_store_wait_all<0>();   // staging buffers are still being read
     tc_fence_before();
@@ -595,6 +652,7 @@ static GemmKernel pick_kernel(int epi, int act, int fmt) {
     return nullptr;
 }
 
+int g_pdl = 1;                       // programmatic dependent launch between the kernels of a step
 static bool g_prepared = false;
 cudaError_t conv_gemm_prepare() {
     if (g_prepared) return cudaSuccess;
@@ -617,7 +675,17 @@ void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     if (workers > total) workers = total;
     GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt);
     if (!k) { fprintf(stderr, "gwstream: no conv GEMM kernel for epi %d act %d\n", g.p.epi, g.p.act); return; }
-    k<<<workers * g.p.n_det, kGemmThreads, g.smem_bytes, st>>>(g.p, n_items);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(workers * g.p.n_det);
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = g.smem_bytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = g_pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, k, g.p, n_items);
     ++g_kernel_launches;
 }
 

@@ -46,6 +46,15 @@ extern "C" int gw_set_fuse_tail(int on) {
     g_fuse_tail = on ? 1 : 0;
     return GW_OK;
 }
+static int g_snake = 1;
+extern "C" int gw_set_snake(int on) {
+    g_snake = on ? 1 : 0;
+    return GW_OK;
+}
+extern "C" int gw_set_pdl(int on) {
+    g_pdl = on ? 1 : 0;
+    return GW_OK;
+}
 extern "C" int gw_set_conv_impl(int impl) {
     if (impl != GW_IMPL_UMMA && impl != GW_IMPL_SIMT) return fail(GW_EINVAL, "unknown conv impl %d", impl);
     g_conv_impl = impl;
@@ -227,6 +236,7 @@ struct gw_deepclean {
     std::vector<int> act_rows, act_cols;
     float* d_wt_final = nullptr;                 // [n_det][K][cpad]
     float* d_b_final = nullptr;                  // [n_det]
+    void* d_fin_B = nullptr;                     // fused tail: last layer as a 16-bit B operand [n_det][16][3 x 64]
     int final_K = 0, final_pad = 0, final_cpad = 0, final_L = 0;
     float* pred = nullptr;                       // [batch][W]
     float* acc = nullptr;                        // [batch][W]
@@ -384,8 +394,34 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (!conv_gemm_plan(gl.g, sms)) return fail(GW_EINVAL, "conv GEMM layer does not fit in shared memory");
     gl.impl = g_conv_impl;
+#ifdef GW_TRACE
+    CU_TRY(cudaMalloc(&p.trace, 148 * 16 * 8));
+    CU_TRY(cudaMemset(p.trace, 0, 148 * 16 * 8));
+#endif
     return GW_OK;
 }
+
+#ifdef GW_TRACE
+// Diagnostic builds: mean over CTAs of the per-role wait counters of the last launch of a layer.
+static void trace_report(const GemmLayer& gl) {
+    const ConvGemmParams& p = gl.g.p;
+    if (!p.trace) return;
+    std::vector<long long> h(148 * 16);
+    cudaMemcpy(h.data(), p.trace, h.size() * 8, cudaMemcpyDeviceToHost);
+    double m[16] = {0};
+    int n = 0;
+    for (int b = 0; b < 148; ++b) {
+        if (h[b * 16 + 7] == 0) continue;
+        ++n;
+        for (int i = 0; i < 16; ++i) m[i] += static_cast<double>(h[b * 16 + i]);
+    }
+    if (!n) return;
+    for (double& v : m) v /= n;
+    fprintf(stderr, "[trace] %-10s N=%3d | producer: a_empty %7.0f b_empty %7.0f total %7.0f | mma: tmem_empty %7.0f a_full %7.0f "
+                    "b_full %7.0f stg_full %7.0f total %7.0f | epi(w2): tmem_full %7.0f store_rd %7.0f fin_full %7.0f total %7.0f\n",
+            gl.name.c_str(), p.N, m[0], m[1], m[2], m[3], m[4], m[5], m[6], m[7], m[8], m[9], m[10], m[11]);
+}
+#endif
 
 static void run_gemm(const GemmLayer& gl, cudaStream_t st) {
     if (gl.impl == GW_IMPL_UMMA) launch_conv_gemm_umma(gl.g, st);
@@ -481,7 +517,7 @@ extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
     for (auto& g : dc->gemm) free_gemm(g);
     for (void* a : dc->act) cudaFree(a);
     cudaFree(dc->ring16);
-    cudaFree(dc->d_wt_final); cudaFree(dc->d_b_final); cudaFree(dc->pred); cudaFree(dc->acc); cudaFree(dc->nhat);
+    cudaFree(dc->d_wt_final); cudaFree(dc->d_b_final); cudaFree(dc->d_fin_B); cudaFree(dc->pred); cudaFree(dc->acc); cudaFree(dc->nhat);
     cudaFree(dc->d_hann); cudaFree(dc->d_inv_wsum); cudaFree(dc->d_rows_map); cudaFree(dc->d_strain_rows);
     cudaFree(dc->final_buf);
     if (dc->s && dc->s->dc == dc) dc->s->dc = nullptr;
@@ -559,6 +595,7 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
                                       len[i], cpad[i], dc->act[i + 1], cpad[i + 1], batch, fin ? EPI_FINAL : EPI_STORE, 0,
                                       from_ring ? s->d_count : nullptr, from_ring ? W : 0))
             return rc;
+        dc->gemm[i].g.p.reverse = g_snake ? (i & 1) : 0;
         dc->gemm[i].name = "gemm.dc" + std::to_string(i);
         // useful MACs: every (input position, tap, cin, cout) product of the layer definition
         const HostLayer& H = dc->host[i];
@@ -591,8 +628,29 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     CU_TRY(cudaMalloc(&dc->pred, wbytes));
     CU_TRY(cudaMemset(dc->pred, 0, wbytes));
     if (dc->fused_tail) {
+        // The last layer as the B operand of a second MMA chain: N = 16 rows (r = 0..3 real: y[4m + r]),
+        // K = 3 row shifts (a = -1, 0, 1) x 64 columns (par x 32 + ci: x[2(m + a) + par][ci]); the tap that
+        // connects them is j = r + pad - 4a - 2 par (o = 2l + j - pad, D3).
+        const HostLayer& H = dc->host[nl - 1];
+        const int ktot = 3 * kSegK;
+        std::vector<uint16_t> FB(static_cast<size_t>(nd) * 16 * ktot, 0);
+        for (int d = 0; d < nd; ++d) {
+            const HostLayer& Hd = dc->host[d * nl + nl - 1];
+            for (int r = 0; r < 4; ++r)
+                for (int a = -1; a <= 1; ++a)
+                    for (int par = 0; par < 2; ++par) {
+                        const int j = r + H.pad_l - 4 * a - 2 * par;
+                        if (j < 0 || j >= H.k) continue;
+                        for (int ci = 0; ci < H.cin; ++ci)
+                            FB[(static_cast<size_t>(d) * 16 + r) * ktot + (a + 1) * kSegK + par * 32 + ci] =
+                                to_storage_bits(Hd.W(0, ci, j), dc->fmt);
+                    }
+        }
+        CU_TRY(cudaMalloc(&dc->d_fin_B, FB.size() * 2));
+        CU_TRY(cudaMemcpy(dc->d_fin_B, FB.data(), FB.size() * 2, cudaMemcpyHostToDevice));
         ConvGemmParams& p = dc->gemm[nl - 2].g.p;
-        p.fin_w = dc->d_wt_final; p.fin_b = dc->d_b_final; p.pred = dc->pred;
+        if (int rc = make_tmap(&p.tmF, dc->d_fin_B, dc->fmt, ktot, 16, nd, ktot, static_cast<uint64_t>(16) * ktot, 16)) return rc;
+        p.fin_b = dc->d_b_final; p.pred = dc->pred;
     }
     CU_TRY(cudaMalloc(&dc->acc, wbytes));
     CU_TRY(cudaMemset(dc->acc, 0, wbytes));
@@ -1030,6 +1088,10 @@ extern "C" int gw_step_profile(gw_pipeline* p, const float* new_samples_dev, flo
     p->s->updates += 1;
     p->dc->forward_for = p->dc->cleaned_for = p->s->updates;
     if (p->bbh) p->bbh->scored_for = p->s->updates;
+#ifdef GW_TRACE
+    for (auto& g : p->dc->gemm) trace_report(g);
+    if (p->bbh) for (auto& g : p->bbh->gemm) trace_report(g);
+#endif
     const int nk = pr.n - 1;
     *n_out = nk;
     for (int i = 0; i < nk && i < max_kernels; ++i) CU_TRY(cudaEventElapsedTime(&ms_out[i], pr.ev[i], pr.ev[i + 1]));
