@@ -40,7 +40,8 @@ namespace gw {
 #endif
 
 constexpr int kEpiWarps = 8;
-constexpr int kGemmThreads = 64 + kEpiWarps * 32;   // producer warp, MMA warp, 8 epilogue warps
+constexpr int kGemmThreads = 64 + kEpiWarps * 32 + 32;   // producer warp, MMA warp, 8 epilogue warps, second MMA warp
+constexpr int kMmaWarp2 = 2 + kEpiWarps;                  // warp index of the second MMA issuer
 constexpr int kAccCols = 256;                        // TMEM columns of one accumulator stage
 constexpr int kSmemBudget = 225 * 1024;
 constexpr int kFixedSmem = 1024 /*alignment slack*/ + 1024 /*bias*/ + 1024 /*barriers, tmem slot*/;
@@ -204,6 +205,15 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int n_workers = gridDim.x / p.n_det;
     const int G = EPI == EPI_STORE ? kAccCols / p.N : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
     const int spi = (p.tiles_m + G - 1) / G;                                 // super-tiles per batch item
+    // Two MMA-issuing warps share a stage when it holds several tiles (even tiles: warp 1, odd tiles: warp
+    // kMmaWarp2).  Below N = 128 an MMA is bound by its shared-memory operand read (32 + N/4 cycles, measured:
+    // profiles/r01_mma_rate_microbench.txt) and a single issuing warp ADDS ~30 cycles of descriptor arithmetic per
+    // instruction (GW_TRACE: 69 / 76 / 87 cycles per MMA at N = 32 / 64 / 128); two warps hide one behind the other.
+    // Each MMA warp owns its own sub-ring of A-slab stages (even tiles: stages [0, ring0), odd tiles: the rest): a
+    // stage whose fills alternate between two waiters could be one mbarrier phase ahead of one of them, and a
+    // parity wait cannot tell (TMA completions are unordered).
+    const int n_mma = (G >= 2 && p.b_resident && sa >= 4) ? 2 : 1;
+    const int ring0 = n_mma == 2 ? (sa + 1) / 2 : sa;                       // stages of sub-ring 0
     const int total = n_items * spi;
 
     if (warp == 0) {
@@ -214,7 +224,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             for (int i = 0; i < sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
             for (int i = 0; i < sb; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
             mbar_init(bres_bar, 1);
-            for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full[i], 1); mbar_init(&tmem_empty[i], kEpiWarps); }
+            for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full[i], n_mma); mbar_init(&tmem_empty[i], kEpiWarps); }
             for (int i = 0; i < 4; ++i) { mbar_init(&stg_full[i], 4); mbar_init(&fin_full[i], 1); }
             fence_barrier_init();
         }
@@ -240,7 +250,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     for (int s = 0; s < 3; ++s) tma_load_3d(smem_fin + s * kFinBlock, &p.tmF, bres_bar, s * kSegK, 0, det);
             }
             griddep_wait();
-            int ia = 0, ib = 0;
+            int ib = 0;
+            int rs0 = 0, rs1 = 0; uint32_t rp0 = 0, rp1 = 0;                 // position and phase in each sub-ring
             TR_DECL
             // mirror-ring source: the window starts at ring row (count mod W) / div (see ConvGemmParams)
             const int row_off = p.a_count ? static_cast<int>((*p.a_count % p.a_ring_W) / p.a_ring_div) : 0;
@@ -252,11 +263,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     if (mt >= p.tiles_m) break;
                     const int m0 = mt * p.tile_stride + p.tile_row0;
                     for (int cb = 0; cb < p.n_cb; ++cb) {
-                        const int stage = ia % sa;
-                        TR_WAIT(0, mbar_wait(&a_empty[stage], ((ia / sa) & 1) ^ 1))
+                        const bool second = n_mma == 2 && (g & 1);
+                        const int stage = second ? ring0 + rs1 : rs0;
+                        TR_WAIT(0, mbar_wait(&a_empty[stage], (second ? rp1 : rp0) ^ 1))
                         mbar_arrive_expect_tx(&a_full[stage], p.slab_rows * 128);
                         tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min + row_off, batch);
-                        ++ia;
+                        if (second) { if (++rs1 == sa - ring0) { rs1 = 0; rp1 ^= 1; } }
+                        else if (++rs0 == ring0) { rs0 = 0; rp0 ^= 1; }
                         if (!p.b_resident) {
                             for (int sh = 0; sh < p.n_shift; ++sh) {
                                 const int s = p.seg_of[cb][sh];
@@ -273,8 +286,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             }
             TR_FLUSH(0, 2)
         }
-    } else if (warp == 1) {
+    } else if (warp == 1 || (warp == kMmaWarp2 && n_mma == 2)) {
         // -------------------------------------------------------------------------- MMA issuer
+        const int mw = warp == 1 ? 0 : 1;
         // The whole warp walks the loops; one elected lane issues the MMAs and commits, selected by an
         // instruction PREDICATE on the tcgen05 instruction itself (umma_f16_if), never by a branch: inside a
         // divergent `if (elect)` block the compiler computes every descriptor in vector registers and moves
@@ -295,7 +309,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         const uint32_t leader = elect_one() ? 1u : 0u;  // the one lane that issues (same lane every time)
         int it = 0;
         TR_DECL
-        int stage = 0; uint32_t a_phase = 0;            // A ring position
+        const int ring_base = mw ? ring0 : 0, ring_size = mw ? sa - ring0 : ring0;
+        int stage = 0; uint32_t a_phase = 0;            // position in this warp's A sub-ring
         int bs = 0; uint32_t b_phase = 0;               // B ring position (streaming mode)
         // EPI_FINAL: the second chain of super-tile `itp` (both tiles): D row i = rows i, i+1, i+2 of the
         // activated tile (tile rows m-1, m, m+1 of output row m = i + 1) times the last layer's three K blocks.
@@ -306,6 +321,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             const int accp = itp & 1;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
+                if (n_mma == 2 && h != mw) continue;
                 TR_WAIT(3, mbar_wait(&stg_full[accp * 2 + h], (itp >> 1) & 1))
                 tc_fence_after();
                 const uint32_t d_fin = tmem_base + accp * kAccCols + kFinCol + h * kFinN;
@@ -327,19 +343,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             tc_fence_after();
             const int g_end = min(G, p.tiles_m - (u % spi) * G);
             for (int g = 0; g < g_end; ++g) {
+                if (n_mma == 2 && (g & 1) != mw) continue;                 // the other warp's tile
                 const uint32_t d_tmem = tmem_base + acc * kAccCols + g * p.N;
                 uint32_t accumulate = 0;
                 uint32_t b_lo = umma_desc_lo(smem_b_u32);                  // resident: block 0 of B
                 for (int cb = 0; cb < n_cb; ++cb) {
                     const uint32_t m = static_cast<uint32_t>(shmask >> (cb * kMaxShift)) & ((1u << kMaxShift) - 1);
-                    TR_WAIT(1, mbar_wait(&a_full[stage], a_phase))
+                    const int astage = ring_base + stage;
+                    TR_WAIT(1, mbar_wait(&a_full[astage], a_phase))
                     tc_fence_after();
                     if (ring) {
                         // window-edge zero padding: slab rows whose logical row is outside [0, M) hold
                         // neighbouring ring samples; clear them (whole 128-byte rows: swizzle-agnostic)
                         const int lo = ((u % spi) * G + g) * p.tile_stride + p.tile_row0 + p.a_min;
                         if (lo < 0 || lo + p.slab_rows > p.a_rows) {
-                            uint8_t* slab = smem_a + stage * sl;
+                            uint8_t* slab = smem_a + astage * sl;
                             for (int idx = lane; idx < p.slab_rows * 8; idx += 32) {
                                 const int lr = lo + (idx >> 3);
                                 if (lr < 0 || lr >= p.a_rows)
@@ -349,7 +367,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             __syncwarp();
                         }
                     }
-                    const uint32_t a_lo = umma_desc_lo(smem_a_u32 + stage * sl);
+                    const uint32_t a_lo = umma_desc_lo(smem_a_u32 + astage * sl);
                     if (resident) {
                         uint32_t acc_flag = accumulate, bl = b_lo;
                         for (int sh = 0; sh < n_shift; ++sh) {
@@ -361,7 +379,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             acc_flag = 1;
                             bl += b_step;
                         }
-                        umma_commit_if(leader, &a_empty[stage]);           // slab free once these MMAs retire
+                        umma_commit_if(leader, &a_empty[astage]);          // slab free once these MMAs retire
                         b_lo = bl;
                     } else {
                         for (int sh = 0; sh < n_shift; ++sh) {
@@ -375,21 +393,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             for (int k = 0; k < kSegK / 16; ++k)
                                 umma_f16_if(leader, d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, accumulate | k);
                             umma_commit_if(leader, &b_empty[bs]);
-                            if (last) umma_commit_if(leader, &a_empty[stage]);
+                            if (last) umma_commit_if(leader, &a_empty[astage]);
                             accumulate = 1;
                             if (++bs == sb) { bs = 0; b_phase ^= 1; }
                         }
                     }
                     accumulate = 1;
-                    if (++stage == sa) { stage = 0; a_phase ^= 1; }
+                    if (++stage == ring_size) { stage = 0; a_phase ^= 1; }
                 }
             }
             umma_commit_if(leader, &tmem_full[acc]);                       // accumulator stage complete
             if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);           // behind this stage's MMAs in the pipe
         }
         if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);
-        TR_FLUSH(3, 4)
-    } else {
+        if (mw == 0) { TR_FLUSH(3, 4) }
+    } else if (warp < kMmaWarp2) {
         // ------------------------------------------------------------- epilogue warps 2..9 (8 warps)
         const int quad = warp % 4;                             // TMEM lane quadrant this warp may read
         const int hsel = (warp - 2) / 4;                       // which half of the 32-column chunks
@@ -631,7 +649,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         }
         if (warp == 2) { TR_FLUSH(8, 3) }
     }
-    if (EPI == EPI_STORE && warp >= 2 && lane == 0) tma_store_wait_all<0>();   // staging buffers are still being read
+    if (EPI == EPI_STORE && warp >= 2 && warp < kMmaWarp2 && lane == 0) tma_store_wait_all<0>();   // staging buffers are still being read
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem_base, 2 * kAccCols);

@@ -63,8 +63,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
         if (clock64() - t0 > 4000000000LL) {   // ~2 s at 2 GHz
-            printf("gwstream: mbarrier wait timed out (block %d,%d thread %d)\n", blockIdx.x, blockIdx.y,
-                   threadIdx.x);
+            if (threadIdx.x % 32 == 0)
+                printf("gwstream: mbarrier wait timed out (block %d warp %d, barrier at +%u, parity %u)\n", blockIdx.x,
+                       threadIdx.x / 32, smem_u32(bar) & 1023u, parity);
             __trap();
         }
     }
