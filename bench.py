@@ -40,6 +40,8 @@ UNIT = "data-seconds/s"
 FS = 4096
 WINDOW = 32768
 SEG_SECONDS = 16          # looped device-resident input segment per stream (BASELINE.json configs[4])
+SWEEP_STREAMS = (1, 16, 128, 512)      # BASELINE.json configs[4]
+SWEEP_STRIDES = (256, 512, 1024)
 
 
 def log(*a):
@@ -192,10 +194,12 @@ def run_native(args):
         gw.set_pdl(False)
     if args.no_snake:
         gw.set_snake(False)
+    if args.no_2sm:
+        gw.set_two_sm(False)
     dtype = gw.GW_BF16 if args.dtype == "bf16" else gw.GW_FP16
     cfg = S.config_c3(args.streams, args.stride, WINDOW)
     sp = cfg.stream
-    n_chunks = SEG_SECONDS * FS // sp.stride
+    n_chunks = args.seg_seconds * FS // sp.stride
     dc_params, bbh_params = make_params(cfg)
     t0 = time.time()
     chunks_h = torch.from_numpy(make_input_chunks(cfg, n_chunks)).pin_memory()
@@ -247,7 +251,7 @@ def run_native(args):
 
     # per-update latency: launch -> stream sync, host clock, one sample per update
     lat = []
-    for _ in range(min(max(K, 50), 400)):
+    for _ in range(min(max(K, 50), 5000)):
         t0 = time.perf_counter()
         step()
         cs.synchronize()
@@ -305,6 +309,18 @@ def run_native(args):
                 "timing": "CUDA events after every launch, eager replay of the same step on the launch stream"}
     kernels = {k: {"ms": round(v[0], 4), **({"tflops": round(v[1] / (v[0] * 1e-3) / 1e12, 1)} if v[1] else {})}
                for k, v in prof.items()}
+    # bandwidth kernels: ALGORITHMIC bytes per step / event time
+    nd, nw = sp.n_det, sp.n_witness
+    hbm_bytes = {
+        "append": sp.n_streams * sp.channels * sp.stride * 8,                       # read new + write ring
+        "ring16_append": sp.n_streams * nd * sp.stride * (nw * 4 + 2 * 32 * 2),     # read fp32, write both mirror copies
+        "aggregate": sp.n_streams * nd * sp.window * 20,                            # p_t, acc r/w, strain, cleaned
+        "bbh_conv1": sp.n_streams * (nd * cfg.bbh_len * 4 + (cfg.bbh_len // 4) * 32 * 2),
+    }
+    for k, b in hbm_bytes.items():
+        if k in kernels and kernels[k]["ms"] > 0:
+            gbs = b / (kernels[k]["ms"] * 1e-3) / 1e9
+            kernels[k].update({"gbs": round(gbs, 1), "hbm_frac": round(gbs / pk["hbm_gbs"], 3)})
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -332,6 +348,30 @@ def run_native(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: n in {1, 16, 128, 512} x stride in {1/16, 1/8, 1/4 s} x {fp16, bf16}, one
+    process per point (a fresh engine and allocator each time)."""
+    rows = []
+    for dtype in ("fp16", "bf16"):
+        for n in SWEEP_STREAMS:
+            for stride in SWEEP_STRIDES:
+                cmd = [sys.executable, os.path.abspath(__file__), "--streams", str(n), "--stride", str(stride), "--dtype", dtype,
+                       "--steps", str(args.steps), "--warmup", str(args.warmup), "--no-cpu-baseline",
+                       "--seg-seconds", str(4 if n >= 512 else SEG_SECONDS)]
+                res = subprocess.run(cmd, capture_output=True, text=True)
+                line = res.stdout.strip().splitlines()[-1] if res.returncode == 0 and res.stdout.strip() else None
+                if line is None:
+                    log(f"sweep point n={n} S={stride} {dtype} failed:\n{res.stderr[-2000:]}")
+                    continue
+                with open(args.sweep, "a") as f:
+                    f.write(line + "\n")
+                d = json.loads(line)
+                rows.append((dtype, n, stride, d["value"], d["ms_per_step"], d["latency"]["p50_ms"], d["latency"]["p99_ms"],
+                             d["latency"]["realtime_budget_ms"], d["roofline"]["frac"], d["e2e"]["value"]))
+                log("%-5s n=%4d S=%5d  %9.1f data-s/s  %7.3f ms/step  p50 %7.3f  p99 %7.3f (budget %6.1f ms)  tensor %.3f  e2e %9.1f"
+                    % rows[-1])
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -344,12 +384,18 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pdl", action="store_true", help="disable programmatic dependent launch (A/B aid)")
     ap.add_argument("--no-snake", action="store_true", help="every layer walks its tiles forwards (A/B aid)")
+    ap.add_argument("--seg-seconds", type=int, default=SEG_SECONDS, help="length of the looped input segment per stream")
+    ap.add_argument("--sweep", metavar="FILE", help="run the configs[4] grid (n x stride x dtype), one bench line per "
+                                                    "point appended to FILE (JSON lines); prints a table to stderr")
+    ap.add_argument("--no-2sm", action="store_true", help="single-CTA kernel for the N=256 layers too (A/B aid)")
     ap.add_argument("--timed-only", action="store_true",
                     help="only the warm-up and the timed region (for short runs under ncu); prints a reduced line")
     ap.add_argument("--reference-budget", type=float, default=150.0,
                     help="--impl reference stops after this many seconds of oracle time (a bounded sample)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         args.warmup = min(args.warmup, 1)
         run_reference(args)
     else:

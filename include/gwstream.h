@@ -128,6 +128,12 @@ int gw_set_pdl(int on);
  * last, which are still in L2.  Pure scheduling; results are bit-identical either way. */
 int gw_set_snake(int on);
 
+/* CTA-pair conv GEMM (tcgen05 cta_group::2: two CTAs of a cluster share every streamed weight block, M = 256)
+ * for the layers whose weights do not fit in shared memory (GEMM N = 256), for handles created AFTER this call
+ * (default 1).  With 0 those layers run the single-CTA kernel.  The accumulation order of every output is the
+ * same, so results are bit-identical. */
+int gw_set_two_sm(int on);
+
 /* ---- snapshotter -------------------------------------------------------------
  * gw_stream_create: zeroed ring state [n][C][W] fp32 on the current device, sample counter 0.
  *   Requires n >= 1, C >= 1, fs >= 1, 1 <= S <= W.

@@ -21,7 +21,7 @@ GW_FINAL, GW_RUNNING = 0, 1
 GW_IMPL_UMMA, GW_IMPL_SIMT = 0, 1
 
 EXPORTS = [
-    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake",
+    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake", "gw_set_two_sm",
     "gw_stream_create", "gw_stream_destroy", "gw_stream_update", "gw_stream_snapshot", "gw_stream_count",
     "gw_deepclean_create", "gw_deepclean_destroy", "gw_deepclean_forward", "gw_deepclean_noise",
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
@@ -76,6 +76,7 @@ def lib():
         L.gw_set_fuse_tail.argtypes = [i]
         L.gw_set_pdl.argtypes = [i]
         L.gw_set_snake.argtypes = [i]
+        L.gw_set_two_sm.argtypes = [i]
         L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
         L.gw_stream_destroy.argtypes = [vp]
         L.gw_stream_update.argtypes = [vp, vp, vp]
@@ -133,6 +134,11 @@ def set_pdl(on: bool) -> None:
 def set_snake(on: bool) -> None:
     """Alternating traversal direction of consecutive DeepClean layers (L2 reuse; default on)."""
     _check(lib().gw_set_snake(1 if on else 0))
+
+
+def set_two_sm(on: bool) -> None:
+    """CTA-pair (cta_group::2) kernel for the N = 256 conv GEMM layers (default on)."""
+    _check(lib().gw_set_two_sm(1 if on else 0))
 
 
 def _fp(a: Optional[np.ndarray]):

@@ -56,6 +56,7 @@ struct ConvGemmParams {
     // 1: walk the (batch item, tile) work list backwards.  Consecutive layers alternate direction, so a
     // layer starts on the activations its predecessor wrote LAST -- the part still resident in the 126 MB L2.
     int reverse;
+    int two_sm;                    // 1: CTA-pair kernel (tcgen05 cta_group::2, M = 256), chosen by conv_gemm_plan
     // EPI_FINAL: this layer (ConvTranspose1d -> 32 channels, tanh) and the network's last layer
     // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel.  The
     // epilogue writes each activated accumulator row (positions 2m, 2m+1 x 32 channels = one 128-byte

@@ -61,6 +61,23 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     ConvGemmParams& p = g.p;
     const int b_block = p.N * 128;
     const int sl = slab_bytes_of(p.slab_rows);
+    if (p.two_sm) {
+        // CTA-pair kernel: N = 256 store layers with an even number of tiles; half weight blocks of 16 KiB
+        const int pairs = sm_count / 2;
+        bool ok = p.epi == EPI_STORE && p.N == 256 && p.a_count == nullptr && p.tiles_m % 2 == 0 && pairs >= p.n_det;
+        for (int ob = 2; ok && ob >= 1; --ob) {
+            const int fixed = kFixedSmem + ob * kOutStage;
+            const int sa = p.n_cb < 2 ? 2 : (p.n_cb > 8 ? 8 : p.n_cb);
+            int sb = (kSmemBudget - fixed - sa * sl) / (128 * 128);
+            if (sb > 8) sb = 8;
+            if (sb < 3) continue;
+            p.out_bufs = ob; p.b_resident = 0; p.sa_stages = sa; p.sb_stages = sb;
+            g.smem_bytes = fixed + sb * 128 * 128 + sa * sl;
+            g.grid = 2 * (pairs - pairs % p.n_det);
+            return true;
+        }
+        p.two_sm = 0;
+    }
     // EPI_STORE stages its output through shared memory for TMA stores: one 4 KiB buffer per epilogue warp,
     // two when the operands leave room (thin layers)
     p.out_bufs = 0;
@@ -655,6 +672,229 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     if (warp == 0) tmem_dealloc(tmem_base, 2 * kAccCols);
 }
 
+// ---------------------------------------------------------------------------------------------
+// CTA-pair variant for the layers whose weights do not fit in shared memory (GEMM N = 256, EPI_STORE).
+//
+// With one CTA per tile such a layer is bound by SHARED-MEMORY bandwidth, not by the tensor pipe: per
+// 128 x 256 x 896 tile the tensor core reads 56 x (4 KiB A + 8 KiB B), TMA writes 448 KiB of weights and 67 KiB
+// of slabs, the epilogue moves 128 KiB -- 1.3 MiB at 128 B/clk = 10.3 k cycles against 7.2 k cycles of math
+// (measured 13.5 k; profiles/r01_mma_rate_microbench.txt).  Here two CTAs of a cluster (one TPC) work on two
+// consecutive tiles as ONE tcgen05.mma.cta_group::2 of M = 256: each CTA loads its own A slab but only HALF of
+// every weight block (128 of the 256 rows of B), and the tensor cores of both SMs read both halves.  Weight
+// fills and weight reads per SM halve (1.3 MiB -> 0.85 MiB per tile).
+//
+// Roles per CTA (320 threads): warp 0 TMA producer (both CTAs; completion bytes are counted on the LEADER's
+// barriers), warp 1 MMA issuer (leader only; commits multicast to both CTAs), warps 2-9 epilogue (each CTA
+// drains its own 128 TMEM lanes; the peer's warps release the accumulator stage on the leader's barrier).
+// ---------------------------------------------------------------------------------------------
+constexpr int kGemm2Threads = 64 + kEpiWarps * 32;
+constexpr int kHalfB = 128 * 128;                    // half of one weight K block: 128 rows x 128 bytes
+
+template <int ACT, int FMT>
+__global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid_constant__ ConvGemmParams p, int n_items) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const int sl = slab_bytes_of(p.slab_rows);
+    const int sa = p.sa_stages, sb = p.sb_stages;
+    uint8_t* smem_out = smem;                                                // [out_bufs][8 warps][4 KiB]
+    uint8_t* smem_b = smem + p.out_bufs * kOutStage;                         // [sb][16 KiB]
+    uint8_t* smem_a = smem_b + sb * kHalfB;                                  // [sa][slab]
+    uint8_t* after_a = smem_a + sa * sl;
+    float* bias_s = reinterpret_cast<float*>(after_a);                       // [256]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(after_a + 1024);
+    uint64_t* a_full = bars;                 // [8]  leader's are used
+    uint64_t* a_empty = a_full + 8;          // [8]
+    uint64_t* b_full = a_empty + 8;          // [8]  leader's are used
+    uint64_t* b_empty = b_full + 8;          // [8]
+    uint64_t* tmem_full = b_empty + 8;       // [2]
+    uint64_t* tmem_empty = tmem_full + 2;    // [2]  leader's are used: 2 x 8 epilogue warps arrive
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_empty + 2);
+
+    const int warp = __shfl_sync(0xffffffffu, threadIdx.x / 32, 0);
+    const int lane = threadIdx.x % 32;
+    const uint32_t rank = cluster_ctarank();                                 // 0 = leader
+    const int cid = blockIdx.x / 2;
+    const int det = cid % p.n_det;
+    const int cworker = cid / p.n_det;
+    const int n_cw = (gridDim.x / 2) / p.n_det;
+    const int half_tiles = p.tiles_m / 2;                                    // tile pairs per batch item
+    const int total = n_items * half_tiles;
+
+    if (warp == 0) {
+        if (lane == 0) {
+            tma_prefetch_desc(&p.tmA);
+            tma_prefetch_desc(&p.tmB);
+            for (int i = 0; i < 8; ++i) {
+                mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1);
+                mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1);
+            }
+            for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full[i], 1); mbar_init(&tmem_empty[i], 2 * kEpiWarps); }
+            fence_barrier_init();
+        }
+        __syncwarp();
+        tmem_alloc_2sm(tmem_slot, 2 * kAccCols);
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();                          // both CTAs' barriers exist before anything arrives on them
+    tc_fence_after();
+    const uint32_t tmem_base = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+    griddep_launch_dependents();
+
+    if (warp == 0) {
+        // --------------------------------------------------------------- TMA producer (both CTAs)
+        griddep_wait();
+        const uint32_t lead_a_full = mapa_u32(smem_u32(a_full), 0), lead_b_full = mapa_u32(smem_u32(b_full), 0);
+        int stage = 0; uint32_t aph = 0;
+        int bs = 0; uint32_t bph = 0;
+        for (int w = cworker; w < total; w += n_cw) {
+            const int u = p.reverse ? total - 1 - w : w;
+            const int batch = (u / half_tiles) * p.n_det + det;
+            const int m0 = ((u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
+            for (int cb = 0; cb < p.n_cb; ++cb) {
+                mbar_wait(&a_empty[stage], aph ^ 1);
+                if (lane == 0) {
+                    if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.slab_rows * 128);
+                    tma_load_3d_2sm(smem_a + stage * sl, &p.tmA, lead_a_full + 8u * stage, cb * kSegK, m0 + p.a_min, batch);
+                }
+                if (++stage == sa) { stage = 0; aph ^= 1; }
+                for (int sh = 0; sh < p.n_shift; ++sh) {
+                    const int s = p.seg_of[cb][sh];
+                    if (s < 0) continue;
+                    mbar_wait(&b_empty[bs], bph ^ 1);
+                    if (lane == 0) {
+                        if (rank == 0) mbar_arrive_expect_tx(&b_full[bs], 2 * kHalfB);
+                        tma_load_3d_2sm(smem_b + bs * kHalfB, &p.tmB, lead_b_full + 8u * bs, s * kSegK, static_cast<int>(rank) * 128, det);
+                    }
+                    if (++bs == sb) { bs = 0; bph ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer (leader CTA)
+        if (rank == 0) {
+            const uint32_t idesc = umma_idesc_f16(FMT, 2 * kTileM, 256);
+            const uint32_t smem_a_u32 = smem_u32(smem_a), smem_b_u32 = smem_u32(smem_b);
+            const int n_cb = p.n_cb, n_shift = p.n_shift;
+            unsigned long long shmask = 0;
+            for (int cb = 0; cb < n_cb; ++cb)
+                for (int sh = 0; sh < n_shift; ++sh)
+                    if (p.seg_of[cb][sh] >= 0) shmask |= 1ull << (cb * kMaxShift + sh);
+            const uint32_t leader = elect_one() ? 1u : 0u;
+            int it = 0;
+            int stage = 0; uint32_t aph = 0;
+            int bs = 0; uint32_t bph = 0;
+            for (int w = cworker; w < total; w += n_cw, ++it) {
+                const int acc = it & 1;
+                mbar_wait(&tmem_empty[acc], ((it >> 1) & 1) ^ 1);
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + acc * kAccCols;
+                uint32_t accumulate = 0;
+                for (int cb = 0; cb < n_cb; ++cb) {
+                    const uint32_t m = static_cast<uint32_t>(shmask >> (cb * kMaxShift)) & ((1u << kMaxShift) - 1);
+                    mbar_wait(&a_full[stage], aph);
+                    tc_fence_after();
+                    const uint32_t a_lo = umma_desc_lo(smem_a_u32 + stage * sl);
+                    for (int sh = 0; sh < n_shift; ++sh) {
+                        if (!((m >> sh) & 1u)) continue;
+                        mbar_wait(&b_full[bs], bph);
+                        tc_fence_after();
+                        const uint32_t bl = umma_desc_lo(smem_b_u32 + bs * kHalfB);
+                        const uint32_t a_lo_s = a_lo + 8u * sh;
+#pragma unroll
+                        for (int k = 0; k < kSegK / 16; ++k)
+                            umma_f16_2sm_if(leader, d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, accumulate | k);
+                        umma_commit_2sm_if(leader, &b_empty[bs]);
+                        if ((m >> (sh + 1)) == 0) umma_commit_2sm_if(leader, &a_empty[stage]);
+                        accumulate = 1;
+                        if (++bs == sb) { bs = 0; bph ^= 1; }
+                    }
+                    if (++stage == sa) { stage = 0; aph ^= 1; }
+                }
+                umma_commit_2sm_if(leader, &tmem_full[acc]);
+            }
+        }
+    } else {
+        // ----------------------------------------------- epilogue warps 2..9 (both CTAs, own 128 TMEM lanes)
+        const int quad = warp % 4;
+        const int hsel = (warp - 2) / 4;
+        const int et = threadIdx.x - 64;
+        for (int i = et; i < 256; i += kEpiWarps * 32) bias_s[i] = __ldg(p.bias + static_cast<size_t>(det) * 256 + i);
+        asm volatile("bar.sync 1, 256;" ::: "memory");
+        const uint32_t bias_u32 = smem_u32(bias_s);
+        griddep_wait();
+        const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;
+        const uint32_t empty_addr[2] = {mapa_u32(smem_u32(&tmem_empty[0]), 0), mapa_u32(smem_u32(&tmem_empty[1]), 0)};
+        int ostep = 0;
+        int it = 0;
+        for (int w = cworker; w < total; w += n_cw, ++it) {
+            const int u = p.reverse ? total - 1 - w : w;
+            const int acc = it & 1;
+            const int batch = (u / half_tiles) * p.n_det + det;
+            const int mt = (u % half_tiles) * 2 + static_cast<int>(rank);
+            mbar_wait(&tmem_full[acc], (it >> 1) & 1);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * kAccCols;
+            for (int cp = 0; cp < 2; ++cp) {
+                const int col = 32 * (4 * cp + 2 * hsel);                    // 64 adjacent columns: two 32-column chunks
+                uint32_t ra[32], rb[32];
+                tmem_ld_32x32(taddr + col, ra);
+                tmem_ld_32x32(taddr + col + 32, rb);
+                float4 bia[2][8];
+#pragma unroll
+                for (int which = 0; which < 2; ++which)
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) bia[which][j] = lds_f4(bias_u32 + 4u * (col + 32 * which + 4 * j));
+                const uint32_t stg = stage_u32 + ((ostep % p.out_bufs) << 15);
+                if (lane == 0) {
+                    if (p.out_bufs == 2) tma_store_wait_read<1>(); else tma_store_wait_read<0>();
+                }
+                ++ostep;
+                tmem_ld_wait();
+                if (cp == 1) {                                               // stage drained: tell the leader's MMA warp
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive_cluster(empty_addr[acc]);
+                }
+                __syncwarp();
+#pragma unroll
+                for (int which = 0; which < 2; ++which) {
+                    const uint32_t* r = which == 0 ? ra : rb;
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {
+                        uint32_t o[4];
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const float4 b4 = bia[which][2 * jj + h];
+                            o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
+                            o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
+                        }
+                        sts_u4(stg + lane * 128 + (((4 * which + jj) ^ (lane & 7)) << 4), o[0], o[1], o[2], o[3]);
+                    }
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) {
+                    if (mt < p.tiles_m) tma_store_3d(&p.tmOut, stg, col, mt * kTileM + quad * 32, batch);
+                    tma_store_commit();
+                }
+            }
+        }
+        if (lane == 0) tma_store_wait_all<0>();
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();                          // the peer may still be reading this CTA's shared memory / TMEM
+    if (warp == 0) tmem_dealloc_2sm(tmem_base, 2 * kAccCols);
+}
+
+typedef void (*Gemm2Kernel)(const ConvGemmParams, int);
+static Gemm2Kernel pick_kernel_2sm(int act, int fmt) {
+    if (act == ACT_TANH) return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_TANH, FMT_BF16> : k_conv_gemm_2sm<ACT_TANH, FMT_FP16>;
+    if (act == ACT_RELU) return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_RELU, FMT_BF16> : k_conv_gemm_2sm<ACT_RELU, FMT_FP16>;
+    return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_NONE, FMT_BF16> : k_conv_gemm_2sm<ACT_NONE, FMT_FP16>;
+}
+
 typedef void (*GemmKernel)(const ConvGemmParams, int);
 
 static GemmKernel pick_kernel(int epi, int act, int fmt) {
@@ -682,6 +922,12 @@ cudaError_t conv_gemm_prepare() {
                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
             if (e != cudaSuccess) return e;
         }
+    for (int act = 0; act < 3; ++act)
+        for (int fmt = 0; fmt < 2; ++fmt) {
+            cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel_2sm(act, fmt)),
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+            if (e != cudaSuccess) return e;
+        }
     g_prepared = true;
     return cudaSuccess;
 }
@@ -693,6 +939,26 @@ void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     if (workers > total) workers = total;
     GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt);
     if (!k) { fprintf(stderr, "gwstream: no conv GEMM kernel for epi %d act %d\n", g.p.epi, g.p.act); return; }
+    if (g.p.two_sm) {
+        int cw = g.grid / 2 / g.p.n_det;                         // clusters per detector
+        const int units = n_items * (g.p.tiles_m / 2);
+        if (cw > units) cw = units;
+        cudaLaunchConfig_t cfg2 = {};
+        cfg2.gridDim = dim3(2 * cw * g.p.n_det);
+        cfg2.blockDim = dim3(kGemm2Threads);
+        cfg2.dynamicSmemBytes = g.smem_bytes;
+        cfg2.stream = st;
+        cudaLaunchAttribute at2[2];
+        at2[0].id = cudaLaunchAttributeClusterDimension;
+        at2[0].val.clusterDim.x = 2; at2[0].val.clusterDim.y = 1; at2[0].val.clusterDim.z = 1;
+        at2[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at2[1].val.programmaticStreamSerializationAllowed = g_pdl ? 1 : 0;
+        cfg2.attrs = at2;
+        cfg2.numAttrs = 2;
+        cudaLaunchKernelEx(&cfg2, pick_kernel_2sm(g.p.act, g.p.fmt), g.p, n_items);
+        ++g_kernel_launches;
+        return;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(workers * g.p.n_det);
     cfg.blockDim = dim3(kGemmThreads);

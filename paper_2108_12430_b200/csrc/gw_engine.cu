@@ -46,6 +46,11 @@ extern "C" int gw_set_fuse_tail(int on) {
     g_fuse_tail = on ? 1 : 0;
     return GW_OK;
 }
+static int g_two_sm = 1;
+extern "C" int gw_set_two_sm(int on) {
+    g_two_sm = on ? 1 : 0;
+    return GW_OK;
+}
 static int g_snake = 1;
 extern "C" int gw_set_snake(int on) {
     g_snake = on ? 1 : 0;
@@ -384,7 +389,6 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     CU_TRY(cudaMemcpy(gl.d_bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
     p.A = in; p.B = gl.d_B; p.bias = gl.d_bias; p.out = out;
     if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows_tm, batch, p.a_cols, static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, p.slab_rows)) return rc;
-    if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.N)) return rc;
     if (epi == EPI_STORE)   // output [batch][M][N]: one 32-row x min(N, 64)-column box per epilogue-warp store
         if (int rc = make_tmap(&p.tmOut, out, fmt, p.N, p.M, batch, p.N, static_cast<uint64_t>(p.M) * p.N, 32, p.N >= 64 ? 64 : 32)) return rc;
     gl.g.batch = batch;
@@ -392,7 +396,9 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    p.two_sm = g_two_sm;                               // a request: the plan keeps it only where the pair kernel applies
     if (!conv_gemm_plan(gl.g, sms)) return fail(GW_EINVAL, "conv GEMM layer does not fit in shared memory");
+    if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.two_sm ? 128 : p.N)) return rc;
     gl.impl = g_conv_impl;
 #ifdef GW_TRACE
     CU_TRY(cudaMalloc(&p.trace, 148 * 16 * 8));
