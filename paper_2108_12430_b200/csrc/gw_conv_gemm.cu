@@ -743,33 +743,60 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
 
     if (warp == 0) {
         // --------------------------------------------------------------- TMA producer (both CTAs)
+        // Two cursors.  The WEIGHT cursor walks the flat schedule (work item, segment 0 .. n_seg-1; segment order
+        // is issue order, `cbstart` marks the first segment of a column block) and blocks on b_empty.  The SLAB
+        // cursor runs ahead of it without blocking (a stage frees up a whole tile before its next use), and is
+        // only forced -- blocking -- to have issued slab (item, cb) before the first weight block of that column
+        // block (otherwise the weight ring could fill while the MMA warp waits for the slab).
         griddep_wait();
         const uint32_t lead_a_full = mapa_u32(smem_u32(a_full), 0), lead_b_full = mapa_u32(smem_u32(b_full), 0);
-        int stage = 0; uint32_t aph = 0;
-        int bs = 0; uint32_t bph = 0;
-        for (int w = cworker; w < total; w += n_cw) {
-            const int u = p.reverse ? total - 1 - w : w;
-            const int batch = (u / half_tiles) * p.n_det + det;
-            const int m0 = ((u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
+        unsigned long long cbstart = 0;
+        {
+            int sidx = 0;
             for (int cb = 0; cb < p.n_cb; ++cb) {
-                mbar_wait(&a_empty[stage], aph ^ 1);
-                if (lane == 0) {
-                    if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.slab_rows * 128);
-                    tma_load_3d_2sm(smem_a + stage * sl, &p.tmA, lead_a_full + 8u * stage, cb * kSegK, m0 + p.a_min, batch);
-                }
-                if (++stage == sa) { stage = 0; aph ^= 1; }
-                for (int sh = 0; sh < p.n_shift; ++sh) {
-                    const int s = p.seg_of[cb][sh];
-                    if (s < 0) continue;
-                    mbar_wait(&b_empty[bs], bph ^ 1);
-                    if (lane == 0) {
-                        if (rank == 0) mbar_arrive_expect_tx(&b_full[bs], 2 * kHalfB);
-                        tma_load_3d_2sm(smem_b + bs * kHalfB, &p.tmB, lead_b_full + 8u * bs, s * kSegK, static_cast<int>(rank) * 128, det);
-                    }
-                    if (++bs == sb) { bs = 0; bph ^= 1; }
-                }
+                bool first = true;
+                for (int sh = 0; sh < p.n_shift; ++sh)
+                    if (p.seg_of[cb][sh] >= 0) { if (first) cbstart |= 1ull << sidx; first = false; ++sidx; }
             }
         }
+        const int n_cb = p.n_cb, n_seg = p.n_seg;
+        int stage = 0; uint32_t aph = 0;
+        int bs = 0; uint32_t bph = 0;
+        int aw = cworker, acb = 0;                                           // slab cursor: work item, column block
+        int a_issued = 0, a_needed = 0;                                      // slabs issued / slabs the weight cursor requires
+        TR_DECL
+        auto slab_step = [&](bool block) -> bool {                           // issue the slab under the cursor, if it can be
+            if (aw >= total) return false;
+            if (block) { TR_WAIT(0, mbar_wait(&a_empty[stage], aph ^ 1)) }
+            else if (!__shfl_sync(0xffffffffu, mbar_test_wait(&a_empty[stage], aph ^ 1) ? 1 : 0, 0)) return false;
+            if (lane == 0) {
+                const int u = p.reverse ? total - 1 - aw : aw;
+                const int m0 = ((u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
+                if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.slab_rows * 128);
+                tma_load_3d_2sm(smem_a + stage * sl, &p.tmA, lead_a_full + 8u * stage, acb * kSegK, m0 + p.a_min,
+                                (u / half_tiles) * p.n_det + det);
+            }
+            if (++stage == sa) { stage = 0; aph ^= 1; }
+            if (++acb == n_cb) { acb = 0; aw += n_cw; }
+            ++a_issued;
+            return true;
+        };
+        for (int w = cworker; w < total; w += n_cw) {
+            for (int sg = 0; sg < n_seg; ++sg) {
+                if ((cbstart >> sg) & 1ull) {
+                    ++a_needed;
+                    while (a_issued < a_needed) slab_step(true);
+                }
+                while (slab_step(false)) {}
+                TR_WAIT(1, mbar_wait(&b_empty[bs], bph ^ 1))
+                if (lane == 0) {
+                    if (rank == 0) mbar_arrive_expect_tx(&b_full[bs], 2 * kHalfB);
+                    tma_load_3d_2sm(smem_b + bs * kHalfB, &p.tmB, lead_b_full + 8u * bs, sg * kSegK, static_cast<int>(rank) * 128, det);
+                }
+                if (++bs == sb) { bs = 0; bph ^= 1; }
+            }
+        }
+        TR_FLUSH(0, 2)
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer (leader CTA)
         if (rank == 0) {
@@ -782,22 +809,23 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
                     if (p.seg_of[cb][sh] >= 0) shmask |= 1ull << (cb * kMaxShift + sh);
             const uint32_t leader = elect_one() ? 1u : 0u;
             int it = 0;
+            TR_DECL
             int stage = 0; uint32_t aph = 0;
             int bs = 0; uint32_t bph = 0;
             for (int w = cworker; w < total; w += n_cw, ++it) {
                 const int acc = it & 1;
-                mbar_wait(&tmem_empty[acc], ((it >> 1) & 1) ^ 1);
+                TR_WAIT(0, mbar_wait(&tmem_empty[acc], ((it >> 1) & 1) ^ 1))
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * kAccCols;
                 uint32_t accumulate = 0;
                 for (int cb = 0; cb < n_cb; ++cb) {
                     const uint32_t m = static_cast<uint32_t>(shmask >> (cb * kMaxShift)) & ((1u << kMaxShift) - 1);
-                    mbar_wait(&a_full[stage], aph);
+                    TR_WAIT(1, mbar_wait(&a_full[stage], aph))
                     tc_fence_after();
                     const uint32_t a_lo = umma_desc_lo(smem_a_u32 + stage * sl);
                     for (int sh = 0; sh < n_shift; ++sh) {
                         if (!((m >> sh) & 1u)) continue;
-                        mbar_wait(&b_full[bs], bph);
+                        TR_WAIT(2, mbar_wait(&b_full[bs], bph))
                         tc_fence_after();
                         const uint32_t bl = umma_desc_lo(smem_b_u32 + bs * kHalfB);
                         const uint32_t a_lo_s = a_lo + 8u * sh;
@@ -813,6 +841,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
                 }
                 umma_commit_2sm_if(leader, &tmem_full[acc]);
             }
+            TR_FLUSH(3, 4)
         }
     } else {
         // ----------------------------------------------- epilogue warps 2..9 (both CTAs, own 128 TMEM lanes)
@@ -827,12 +856,13 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
         const uint32_t empty_addr[2] = {mapa_u32(smem_u32(&tmem_empty[0]), 0), mapa_u32(smem_u32(&tmem_empty[1]), 0)};
         int ostep = 0;
         int it = 0;
+        TR_DECL
         for (int w = cworker; w < total; w += n_cw, ++it) {
             const int u = p.reverse ? total - 1 - w : w;
             const int acc = it & 1;
             const int batch = (u / half_tiles) * p.n_det + det;
             const int mt = (u % half_tiles) * 2 + static_cast<int>(rank);
-            mbar_wait(&tmem_full[acc], (it >> 1) & 1);
+            TR_WAIT(0, mbar_wait(&tmem_full[acc], (it >> 1) & 1))
             tc_fence_after();
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * kAccCols;
             for (int cp = 0; cp < 2; ++cp) {
@@ -847,7 +877,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
                     for (int j = 0; j < 8; ++j) bia[which][j] = lds_f4(bias_u32 + 4u * (col + 32 * which + 4 * j));
                 const uint32_t stg = stage_u32 + ((ostep % p.out_bufs) << 15);
                 if (lane == 0) {
-                    if (p.out_bufs == 2) tma_store_wait_read<1>(); else tma_store_wait_read<0>();
+                    TR_WAIT(1, if (p.out_bufs == 2) tma_store_wait_read<1>(); else tma_store_wait_read<0>())
                 }
                 ++ostep;
                 tmem_ld_wait();
@@ -881,6 +911,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
             }
         }
         if (lane == 0) tma_store_wait_all<0>();
+        if (warp == 2) { TR_FLUSH(8, 3) }
     }
     tc_fence_before();
     __syncthreads();
