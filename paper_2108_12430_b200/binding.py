@@ -26,7 +26,7 @@ EXPORTS = [
     "gw_deepclean_create", "gw_deepclean_destroy", "gw_deepclean_forward", "gw_deepclean_noise",
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
-    "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_pipeline_graph_nodes",
+    "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_step_host_async", "gw_pipeline_graph_nodes",
     "gw_step_profile", "gw_profile_label", "gw_profile_flops",
 ]
 
@@ -98,6 +98,7 @@ def lib():
         L.gw_pipeline_destroy.argtypes = [vp]
         L.gw_step.argtypes = [vp, vp, vp, vp, vp]
         L.gw_step_host.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_step_host_async.argtypes = [vp, vp, vp, vp, vp]
         L.gw_pipeline_graph_nodes.argtypes = [vp]
         L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_float), C.POINTER(i)]
         L.gw_profile_label.argtypes = [vp, i]
@@ -346,6 +347,15 @@ class Pipeline:
                 return C.c_void_p(0)
             return C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
         _check(lib().gw_step_host(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)))
+
+    def step_host_async(self, new_samples, scores, cleaned_final, stream=None) -> None:
+        """step_host without the synchronisation: the input copy of this call overlaps the previous step's
+        kernels.  All three host buffers must stay untouched until `stream` is synchronised past the call."""
+        def hp(a):
+            if a is None:
+                return C.c_void_p(0)
+            return C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
+        _check(lib().gw_step_host_async(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)))
 
     def step_profile(self, new_samples, scores, cleaned_final, stream=None):
         """One eager update with a CUDA event after each kernel -> [(label, ms, algorithmic flops)]."""

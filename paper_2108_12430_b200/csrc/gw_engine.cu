@@ -286,6 +286,10 @@ struct gw_pipeline {
     float* cap_scores = nullptr;
     float* cap_final = nullptr;
     float *d_in = nullptr, *d_scores = nullptr, *d_final = nullptr;   // staging for gw_step_host
+    float* d_in2[2] = {nullptr, nullptr};        // gw_step_host_async: double-buffered input staging,
+    cudaStream_t copy_stream = nullptr;          // filled on an internal copy stream while the previous step computes
+    cudaEvent_t in_done[2] = {nullptr, nullptr}, in_free[2] = {nullptr, nullptr};
+    int64_t async_calls = 0;
     Prof prof;
 };
 
@@ -986,6 +990,12 @@ extern "C" int gw_pipeline_destroy(gw_pipeline* p) {
     if (p->exec) cudaGraphExecDestroy(p->exec);
     if (p->graph) cudaGraphDestroy(p->graph);
     cudaFree(p->d_in); cudaFree(p->d_scores); cudaFree(p->d_final);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(p->d_in2[i]);
+        if (p->in_done[i]) cudaEventDestroy(p->in_done[i]);
+        if (p->in_free[i]) cudaEventDestroy(p->in_free[i]);
+    }
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
     for (cudaEvent_t e : p->prof.ev) cudaEventDestroy(e);
     delete p;
     return GW_OK;
@@ -1117,6 +1127,44 @@ extern "C" double gw_profile_flops(const gw_pipeline* p, int i) {
     for (auto& g : p->dc->gemm) if (g.name == lab) return g.flops * p->dc->batch;
     if (p->bbh) for (auto& g : p->bbh->gemm) if (g.name == lab) return g.flops * p->bbh->batch;
     return 0.0;
+}
+
+// Throughput form of gw_step_host: does NOT synchronise, and the host->device copy of this call's samples
+// runs on an internal copy stream into one of two staging buffers, so it overlaps the previous step's kernels
+// (at C4 n=128 the copy is 11.5 MB, about a quarter of the step).  Results land in the host buffers in stream
+// order on `stream`; all host buffers of a call must stay valid until `stream` has been synchronised past it.
+extern "C" int gw_step_host_async(gw_pipeline* p, const float* new_samples_host, float* scores_host,
+                                  float* cleaned_final_host, void* stream) {
+    if (!p || !new_samples_host || !cleaned_final_host || (p->bbh && !scores_host))
+        return fail(GW_EINVAL, "gw_step_host_async: NULL argument");
+    gw_stream* s = p->s;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t in_bytes = static_cast<size_t>(s->n) * s->C * s->S * 4;
+    const size_t fin_bytes = static_cast<size_t>(p->dc->batch) * s->S * 4;
+    const size_t sc_bytes = static_cast<size_t>(s->n) * 4;
+    if (!p->copy_stream) {
+        CU_TRY(cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CU_TRY(cudaMalloc(&p->d_in2[i], in_bytes));
+            CU_TRY(cudaEventCreateWithFlags(&p->in_done[i], cudaEventDisableTiming));
+            CU_TRY(cudaEventCreateWithFlags(&p->in_free[i], cudaEventDisableTiming));
+        }
+    }
+    if (!p->d_final) {
+        CU_TRY(cudaMalloc(&p->d_final, fin_bytes));
+        CU_TRY(cudaMalloc(&p->d_scores, sc_bytes));
+    }
+    const int b = static_cast<int>(p->async_calls & 1);
+    if (p->async_calls >= 2) CU_TRY(cudaStreamWaitEvent(p->copy_stream, p->in_free[b], 0));   // step k-2 has read it
+    CU_TRY(cudaMemcpyAsync(p->d_in2[b], new_samples_host, in_bytes, cudaMemcpyHostToDevice, p->copy_stream));
+    CU_TRY(cudaEventRecord(p->in_done[b], p->copy_stream));
+    CU_TRY(cudaStreamWaitEvent(st, p->in_done[b], 0));
+    if (int rc = gw_step(p, p->d_in2[b], p->d_scores, p->d_final, stream)) return rc;
+    CU_TRY(cudaEventRecord(p->in_free[b], st));
+    CU_TRY(cudaMemcpyAsync(cleaned_final_host, p->d_final, fin_bytes, cudaMemcpyDeviceToHost, st));
+    if (p->bbh) CU_TRY(cudaMemcpyAsync(scores_host, p->d_scores, sc_bytes, cudaMemcpyDeviceToHost, st));
+    p->async_calls += 1;
+    return GW_OK;
 }
 
 extern "C" int gw_step_host(gw_pipeline* p, const float* new_samples_host, float* scores_host, float* cleaned_final_host, void* stream) {

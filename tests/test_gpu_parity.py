@@ -326,3 +326,40 @@ def test_full_size_c4_sampled_streams_match_oracle(dtype):
             j = {0: 0, 1: 77, 2: 127}[i % 3] if i not in sampled else i
             assert np.array_equal(pred[i], pred[j]), (t, i, j)
             assert np.array_equal(final[i], final[j]) and scores[i] == scores[j], (t, i, j)
+
+
+@pytest.mark.gpu
+def test_host_step_async_equals_device_step_bitwise():
+    """gw_step_host_async (double-buffered input staging on an internal copy stream) and gw_step_host deliver
+    exactly what gw_step computes from device-resident inputs."""
+    cfg = S.config_small_ensemble(3)
+    sp = cfg.stream
+    dc_params, bbh_params = util.make_params(cfg)
+    n_up = 7
+    x = synth.multi_stream(cfg.seed, sp, n_up * sp.stride)
+    outs = {}
+    for mode in ("device", "host", "async"):
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, gw.GW_FP16)
+        cs = torch.cuda.Stream()
+        res = []
+        if mode == "device":
+            xd = _dev(x)
+            sc = torch.zeros(sp.n_streams, device="cuda")
+            fin = torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda")
+            for t in range(n_up):
+                pipe.step(xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous(), sc, fin, cs)
+                cs.synchronize()
+                res.append((fin.cpu().numpy().copy(), sc.cpu().numpy().copy()))
+        else:
+            xin = [torch.from_numpy(np.ascontiguousarray(x[:, :, t * sp.stride:(t + 1) * sp.stride])).pin_memory() for t in range(n_up)]
+            sch = [torch.zeros(sp.n_streams).pin_memory() for _ in range(n_up)]
+            finh = [torch.zeros((sp.n_streams, sp.n_det, sp.stride)).pin_memory() for _ in range(n_up)]
+            for t in range(n_up):
+                (pipe.step_host if mode == "host" else pipe.step_host_async)(xin[t], sch[t], finh[t], cs)
+            cs.synchronize()
+            res = [(finh[t].numpy().copy(), sch[t].numpy().copy()) for t in range(n_up)]
+        outs[mode] = res
+    for mode in ("host", "async"):
+        for t in range(n_up):
+            assert np.array_equal(outs[mode][t][0], outs["device"][t][0]), (mode, t)
+            assert np.array_equal(outs[mode][t][1], outs["device"][t][1]), (mode, t)
