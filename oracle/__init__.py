@@ -337,3 +337,40 @@ class StreamOracle:
             out["bbh_input"] = xin
             out["score"] = bbh_forward(xin, convs, pc, pd)
         return out
+
+
+def offline_clean(x: np.ndarray, W: int, S: int, rows, dc) -> Dict[str, np.ndarray]:
+    """D9, offline / non-streaming mode ("adjacent frames ... in parallel",
+    :202 offline regime, :216 non-streaming ensemble): an archival segment x [C][T], T = W + (B-1) S, of ONE
+    stream is cut into the B windows [jS, jS + W) that lie inside it -- the same window grid as the streaming
+    path (D1), without the warm-up windows that reach before the segment -- every window goes through DeepClean
+    independently, and the predictions are combined by the same periodic-Hann overlap-add (D7), normalised by
+    the summed weights of the windows that actually cover a sample:
+
+        nhat[a] = sum_j w[a - jS] p_j[a - jS] / sum_j w[a - jS]   (j: jS <= a < jS + W, 0 <= j < B)
+        cleaned[d][a] = strain_d[a] - nhat_d[a]
+
+    A sample covered by all W/S windows gets exactly the streaming path's final value.  Sample 0 is covered
+    only at window position 0, where the periodic Hann weight is 0: its estimate is defined as 0.
+    Returns {"pred": [D][B][W], "nhat": [D][T], "cleaned": [D][T]} in float64."""
+    x = np.asarray(x)
+    C, T = x.shape
+    assert T >= W and (T - W) % S == 0
+    B = (T - W) // S + 1
+    w = hann(W)
+    ndet = len(rows)
+    pred = np.zeros((ndet, B, W), dtype=np.float64)
+    nhat = np.zeros((ndet, T), dtype=np.float64)
+    cleaned = np.zeros((ndet, T), dtype=np.float64)
+    for d, ((wit, strain), (layers, prepared)) in enumerate(zip(rows, dc)):
+        acc = np.zeros(T, dtype=np.float64)
+        wsum = np.zeros(T, dtype=np.float64)
+        for j in range(B):
+            p = deepclean_forward(x[wit, j * S:j * S + W], layers, prepared)
+            pred[d, j] = p
+            acc[j * S:j * S + W] += w * p
+            wsum[j * S:j * S + W] += w
+        ok = wsum > 0
+        nhat[d, ok] = acc[ok] / wsum[ok]
+        cleaned[d] = x[strain].astype(np.float64) - nhat[d]
+    return {"pred": pred, "nhat": nhat, "cleaned": cleaned}

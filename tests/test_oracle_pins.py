@@ -495,3 +495,65 @@ def test_bf16_activation_storage_alone_exceeds_the_elementwise_bar():
         out[dt] = (np.linalg.norm(d) / np.linalg.norm(ref), np.max(np.abs(d)) / np.sqrt(np.mean(ref * ref)))
     assert out[oracle.DT_BF16][0] < 1e-2 and out[oracle.DT_BF16][1] > 2e-2
     assert out[oracle.DT_FP16][0] < 2.5e-3 and out[oracle.DT_FP16][1] < 5e-3
+
+
+# ------------------------------------------------------------------ D9 offline mode
+def test_offline_interior_equals_streaming_finals_and_edges_follow_the_definition():
+    """The offline definition is pinned against the streaming one (itself pinned above): with the same window
+    grid, every sample covered by all W/S windows of the segment gets the streaming path's FINAL value; near the
+    segment's ends the estimate is the weighted mean over the covering windows, checked by brute force."""
+    cfg = S.config_c0()
+    sp = cfg.stream
+    W, St = sp.window, sp.stride
+    k = W // St
+    B = 12
+    T = W + (B - 1) * St
+    params = synth.deepclean_params(7, cfg.dc_layers)
+    prepared = [oracle.prepare_conv(l, p, oracle.DT_FP16) for l, p in zip(cfg.dc_layers, params)]
+    rows = [(sp.witness_rows(0), sp.strain_row(0))]
+    dc = [(cfg.dc_layers, prepared)]
+    x = synth.stream_channels(3, sp, T, white=True)
+    off = oracle.offline_clean(x, W, St, rows, dc)
+    # streaming over the same samples: update t sees window [(t+1)S - W, (t+1)S); sample a is final after
+    # update a // S + k - 1 and is emitted in that update's block of S final samples
+    n_up = T // St
+    so = oracle.StreamOracle(sp.channels, W, St, rows, dc, None, max_updates=n_up + 1)
+    finals = np.full(T, np.nan)
+    for t in range(n_up):
+        ref = so.update(x[:, t * St:(t + 1) * St])
+        a0 = (t + 1) * St - W
+        if a0 >= 0:
+            finals[a0:a0 + St] = ref["cleaned_final"][0]
+    # interior: covered by all k windows that lie inside the segment: a in [(k-1) S, T - (k-1) S)
+    lo, hi = (k - 1) * St, T - (k - 1) * St
+    assert hi > lo
+    assert np.allclose(off["cleaned"][0, lo:hi], finals[lo:hi], rtol=0, atol=1e-12)
+    # edges, brute force over covering windows
+    w = oracle.hann(W)
+    for a in (1, St - 1, St, 3 * St + 5, T - 1, T - St, T - 2 * St - 3):
+        num = den = 0.0
+        for j in range(B):
+            n = a - j * St
+            if 0 <= n < W:
+                num += w[n] * off["pred"][0, j, n]
+                den += w[n]
+        assert abs(off["nhat"][0, a] - num / den) <= 1e-12
+    assert off["nhat"][0, 0] == 0.0 and off["cleaned"][0, 0] == float(x[sp.strain_row(0), 0])
+
+
+def test_offline_constant_prediction_gives_the_constant():
+    """Bias-only network (all weights zero, last bias c): every window predicts c, so nhat = c wherever the
+    summed window is positive, whatever the coverage (closed form; north_star's constant-window pin)."""
+    cfg = S.config_c0()
+    sp = cfg.stream
+    params = synth.deepclean_params(9, cfg.dc_layers)
+    for p in params:
+        p["w"][...] = 0
+        p["b"][...] = 0
+    params[-1]["b"][...] = 0.375
+    prepared = [oracle.prepare_conv(l, p, oracle.DT_FP16) for l, p in zip(cfg.dc_layers, params)]
+    T = sp.window + 3 * sp.stride
+    x = synth.stream_channels(4, sp, T, white=True)
+    off = oracle.offline_clean(x, sp.window, sp.stride, [(sp.witness_rows(0), sp.strain_row(0))], [(cfg.dc_layers, prepared)])
+    assert np.allclose(off["nhat"][0, 1:], 0.375, rtol=0, atol=1e-15)
+    assert np.allclose(off["cleaned"][0, 1:], x[sp.strain_row(0), 1:].astype(np.float64) - 0.375, rtol=0, atol=1e-15)
