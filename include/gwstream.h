@@ -48,6 +48,7 @@ typedef struct gw_stream gw_stream;
 typedef struct gw_deepclean gw_deepclean;
 typedef struct gw_bbh gw_bbh;
 typedef struct gw_pipeline gw_pipeline;
+typedef struct gw_offline gw_offline;
 
 /* One convolution layer, parameters in HOST memory, fp32, unfolded.
  *  kind GW_CONV : y[co][l] = b[co] + sum_ci sum_j w[co][ci][j] x[ci][stride*l + j - pad_l], zero
@@ -222,6 +223,27 @@ const char *gw_profile_label(const gw_pipeline *p, int i);
 double gw_profile_flops(const gw_pipeline *p, int i);
 /* number of kernel nodes in the captured graph (0 before the first gw_step) */
 int gw_pipeline_graph_nodes(const gw_pipeline *p);
+
+/* ---- offline / non-streaming mode (PAPER.md:174 "adjacent frames ... in parallel", :202 offline regime, :216
+ * non-streaming ensemble; D9) ---------------------------------------------------
+ * One launch sequence cleans an ARCHIVAL segment of ONE stream: T = window + (n_windows - 1) * stride samples per
+ * channel are cut into the n_windows windows [j*stride, j*stride + window) (the streaming path's window grid
+ * without its warm-up windows), every window goes through DeepClean (same kernels as the streaming path, the
+ * windows folded into the GEMM M dimension), and the predictions are combined by the periodic-Hann overlap-add
+ * normalised by the summed weights of the windows that actually cover a sample; cleaned = strain - estimate.
+ * A sample covered by all window/stride windows is bit-identical to the streaming path's final value.
+ * gw_offline_create: spec as for gw_deepclean_create (agg and delta are ignored); window % stride == 0,
+ *   window/stride >= 2.  Owns all device state.  Errors: GW_EINVAL, GW_ENOMEM, GW_ECUDA.
+ * gw_offline_samples: T.
+ * gw_offline_run: samples_dev [channels][T] fp32, cleaned_dev [n_det][T] fp32, noise_dev [n_det][T] or NULL (the
+ *   estimate that was subtracted), all device pointers owned by the caller; asynchronous on `stream`.
+ * gw_offline_predictions (test hook): raw per-window predictions [n_windows][n_det][window] of the last run. */
+int gw_offline_create(gw_offline **out, const gw_dc_spec *spec, int channels, int fs, int window, int stride,
+                      int n_windows, int dtype);
+int gw_offline_destroy(gw_offline *o);
+int64_t gw_offline_samples(const gw_offline *o);
+int gw_offline_run(gw_offline *o, const float *samples_dev, float *cleaned_dev, float *noise_dev, void *stream);
+int gw_offline_predictions(gw_offline *o, float *out_dev, void *stream);
 
 #ifdef __cplusplus
 }

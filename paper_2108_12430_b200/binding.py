@@ -28,6 +28,7 @@ EXPORTS = [
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
     "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_step_host_async", "gw_pipeline_graph_nodes",
     "gw_step_profile", "gw_profile_label", "gw_profile_flops",
+    "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
 ]
 
 _FP = C.POINTER(C.c_float)
@@ -99,6 +100,12 @@ def lib():
         L.gw_step.argtypes = [vp, vp, vp, vp, vp]
         L.gw_step_host.argtypes = [vp, vp, vp, vp, vp]
         L.gw_step_host_async.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_offline_create.argtypes = [C.POINTER(vp), vp, i, i, i, i, i, i]
+        L.gw_offline_destroy.argtypes = [vp]
+        L.gw_offline_samples.argtypes = [vp]
+        L.gw_offline_samples.restype = i64
+        L.gw_offline_run.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_offline_predictions.argtypes = [vp, vp, vp]
         L.gw_pipeline_graph_nodes.argtypes = [vp]
         L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_float), C.POINTER(i)]
         L.gw_profile_label.argtypes = [vp, i]
@@ -377,6 +384,51 @@ class Pipeline:
     def __del__(self):
         try:
             self.close()
+        except Exception:
+            pass
+
+
+class Offline:
+    """Offline / non-streaming DeepClean (D9): `n_windows` consecutive windows of ONE stream's archival
+    segment per launch.  `spec` gives the per-stream shape (n_streams is ignored)."""
+
+    def __init__(self, spec: S.StreamSpec, layers: Sequence[S.ConvSpec], params_per_det: Sequence[Sequence[Dict]],
+                 n_windows: int, dtype: int = GW_BF16):
+        self.spec, self.n_windows = spec, n_windows
+        keep: list = []
+        n_det = len(params_per_det)
+        assert n_det == spec.n_det
+        arr = _marshal_layers(list(layers) * n_det, [p for det in params_per_det for p in det], keep)
+        wit = (C.c_int * (n_det * spec.n_witness))(*[r for d in range(n_det) for r in spec.witness_rows(d)])
+        srow = (C.c_int * n_det)(*[spec.strain_row(d) for d in range(n_det)])
+        dspec = _DcSpec(n_det, len(layers), spec.n_witness, arr, wit, srow, S.AGG_HANN_OLA, 0)
+        self.h = C.c_void_p()
+        _check(lib().gw_offline_create(C.byref(self.h), C.byref(dspec), spec.channels, spec.fs, spec.window, spec.stride,
+                                       n_windows, dtype))
+        self.samples = int(lib().gw_offline_samples(self.h))
+
+    def run(self, samples, cleaned=None, noise=None, stream=None):
+        """samples: CUDA float32 [C][T]; returns (cleaned [D][T], noise estimate [D][T])."""
+        import torch
+        assert tuple(samples.shape) == (self.spec.channels, self.samples) and samples.is_contiguous()
+        if cleaned is None:
+            cleaned = torch.empty((self.spec.n_det, self.samples), dtype=torch.float32, device="cuda")
+        if noise is None:
+            noise = torch.empty((self.spec.n_det, self.samples), dtype=torch.float32, device="cuda")
+        _check(lib().gw_offline_run(self.h, _ptr(samples), _ptr(cleaned), _ptr(noise), _stream_ptr(stream)))
+        return cleaned, noise
+
+    def predictions(self, stream=None):
+        import torch
+        out = torch.empty((self.n_windows, self.spec.n_det, self.spec.window), dtype=torch.float32, device="cuda")
+        _check(lib().gw_offline_predictions(self.h, _ptr(out), _stream_ptr(stream)))
+        return out
+
+    def __del__(self):
+        try:
+            if self.h:
+                lib().gw_offline_destroy(self.h)
+                self.h = C.c_void_p()
         except Exception:
             pass
 

@@ -103,7 +103,10 @@ void launch_ring16_append(const float* new_samples, void* ring16, const long lon
                           int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
                           cudaStream_t st);
 void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
-                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st);
+                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st, long long seg_T = 0,
+                   int seg_S = 0);
+void launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann, const double* cum,
+                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, cudaStream_t st);
 void launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
                         int L, int cpad, int K, int pad, int fmt, cudaStream_t st);
 struct AggParams {

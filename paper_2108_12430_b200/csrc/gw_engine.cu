@@ -235,6 +235,7 @@ struct gw_deepclean {
     std::vector<HostLayer> host;                 // [n_det * n_layers]
     std::vector<GemmLayer> gemm;                 // layers 0 .. n_layers-2
     void* ring16 = nullptr;                      // mirror ring [batch][2W][cpad0], 16-bit (when `mirror`)
+    bool offline = false;                        // owned by a gw_offline: windows of one archival segment, gather path
     bool mirror = false;                         // first layer reads the window from ring16 (no per-update gather)
     bool fused_tail = false;                     // last GEMM layer + final ConvTranspose1d run as one kernel (EPI_FINAL)
     std::vector<void*> act;                      // act[0] = gathered window (null when `mirror`), act[i+1] = output of layer i
@@ -576,7 +577,7 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     dc->act_rows.assign(nl, 0); dc->act_cols.assign(nl, 0);
     // The 16-bit mirror ring replaces the per-update gather when window positions pair up with ring slots
     // (even stride => even head) and the first layer is a Conv1d; otherwise the window is re-gathered.
-    dc->mirror = (S % 2 == 0) && (W % 2 == 0) && dc->host[0].kind == GW_CONV;
+    dc->mirror = !dc->offline && (S % 2 == 0) && (W % 2 == 0) && dc->host[0].kind == GW_CONV;
     // The last GEMM layer (ConvTranspose1d -> <= 32 channels, tanh) and the final 1-channel ConvTranspose1d
     // (k = 7) run as ONE kernel when they have the standard shape: the 16-bit activation between them is
     // never written (at C3 that round trip is 2 x 1 MiB per detector-window, more than the layer's input).
@@ -753,6 +754,99 @@ extern "C" int gw_deepclean_forward(gw_deepclean* dc, void* stream) {
     deepclean_forward_enqueue(dc, static_cast<cudaStream_t>(stream));
     CU_TRY(cudaGetLastError());
     dc->forward_for = dc->s->updates;
+    return GW_OK;
+}
+
+// ============================================================================ offline mode (D9)
+struct gw_offline {
+    gw_stream* s = nullptr;                      // shape carrier only (n = windows per launch); no ring
+    gw_deepclean* dc = nullptr;
+    double* d_cum = nullptr;                     // [W] summed Hann weights along each residue chain
+    int B = 0;
+    long long T = 0;
+};
+
+extern "C" int gw_offline_destroy(gw_offline* o) {
+    if (!o) return GW_OK;
+    if (o->dc) { o->dc->s = nullptr; gw_deepclean_destroy(o->dc); }
+    if (o->s) { cudaFree(o->s->d_count); cudaFree(o->s->d_ticket); delete o->s; }
+    cudaFree(o->d_cum);
+    delete o;
+    return GW_OK;
+}
+
+extern "C" int gw_offline_create(gw_offline** out, const gw_dc_spec* spec, int channels, int fs, int window, int stride,
+                                 int n_windows, int dtype) {
+    if (!out) return fail(GW_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!spec || !spec->layers || !spec->witness_rows || !spec->strain_row) return fail(GW_EINVAL, "gw_offline_create: NULL argument");
+    if (dtype != GW_BF16 && dtype != GW_FP16) return fail(GW_EINVAL, "dtype must be GW_BF16 or GW_FP16");
+    if (channels < 1 || fs < 1 || window < 1 || stride < 1 || n_windows < 1) return fail(GW_EINVAL, "gw_offline_create: bad shape");
+    if (window % stride != 0 || window / stride < 2) return fail(GW_EINVAL, "offline overlap-add needs window %% stride == 0 and window/stride >= 2");
+    if (spec->n_det < 1 || spec->n_layers < 2 || spec->n_witness < 1) return fail(GW_EINVAL, "bad DeepClean spec");
+    for (int d = 0; d < spec->n_det; ++d) {
+        if (spec->strain_row[d] < 0 || spec->strain_row[d] >= channels) return fail(GW_EINVAL, "strain row out of range");
+        for (int c = 0; c < spec->n_witness; ++c)
+            if (spec->witness_rows[d * spec->n_witness + c] < 0 || spec->witness_rows[d * spec->n_witness + c] >= channels)
+                return fail(GW_EINVAL, "witness row out of range");
+    }
+    if (int rc = check_device()) return rc;
+    gw_offline* o = new gw_offline();
+    o->B = n_windows;
+    o->T = static_cast<long long>(window) + static_cast<long long>(n_windows - 1) * stride;
+    o->s = new gw_stream();
+    o->s->n = n_windows; o->s->C = channels; o->s->fs = fs; o->s->W = window; o->s->S = stride;
+    gw_deepclean* dc = new gw_deepclean();
+    o->dc = dc;
+    dc->s = o->s; dc->n_det = spec->n_det; dc->n_layers = spec->n_layers; dc->n_wit = spec->n_witness;
+    dc->agg = GW_AGG_HANN_OLA; dc->delta = 0; dc->offline = true;
+    dc->fmt = dtype == GW_BF16 ? FMT_BF16 : FMT_FP16;
+    int rc = deepclean_build(dc, o->s, spec);
+    if (rc == GW_OK) {
+        std::vector<double> w(window), cum(window);
+        const double pi = 3.14159265358979323846;
+        for (int n = 0; n < window; ++n) w[n] = 0.5 - 0.5 * cos(2.0 * pi * n / window);
+        for (int n = 0; n < window; ++n) {
+            double sum = 0.0;
+            for (int m = n; m < window; m += stride) sum += w[m];      // the order of the streaming path's table
+            cum[n] = sum;
+        }
+        cudaError_t e = cudaMalloc(&o->d_cum, window * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemcpy(o->d_cum, cum.data(), window * sizeof(double), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) rc = fail(GW_ECUDA, "gw_offline_create: %s", cudaGetErrorString(e));
+    }
+    if (rc != GW_OK) { std::string keep = g_err; gw_offline_destroy(o); g_err = keep; return rc; }
+    *out = o;
+    return GW_OK;
+}
+
+extern "C" int64_t gw_offline_samples(const gw_offline* o) { return o ? o->T : 0; }
+
+extern "C" int gw_offline_run(gw_offline* o, const float* samples_dev, float* cleaned_dev, float* noise_dev, void* stream) {
+    if (!o || !samples_dev || !cleaned_dev) return fail(GW_EINVAL, "gw_offline_run: NULL argument");
+    gw_deepclean* dc = o->dc;
+    gw_stream* s = o->s;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    launch_gather(samples_dev, dc->act[0], nullptr, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, dc->act_cols[0],
+                  dc->fmt, st, o->T, s->S);
+    prof_mark("gather", st);
+    for (auto& g : dc->gemm) run_gemm(g, st);
+    if (!dc->fused_tail) {
+        launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
+                           dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
+    }
+    launch_ola_offline(dc->pred, samples_dev, dc->d_strain_rows, dc->d_hann, o->d_cum, cleaned_dev, noise_dev, o->B, dc->n_det,
+                       s->W, s->S, o->T, st);
+    CU_TRY(cudaGetLastError());
+    dc->forward_for += 1;                        // gw_deepclean_noise-style hooks see a completed pass
+    return GW_OK;
+}
+
+// Test hook: the raw per-window predictions [B][D][W] of the last gw_offline_run.
+extern "C" int gw_offline_predictions(gw_offline* o, float* out_dev, void* stream) {
+    if (!o || !out_dev) return fail(GW_EINVAL, "gw_offline_predictions: NULL argument");
+    CU_TRY(cudaMemcpyAsync(out_dev, o->dc->pred, static_cast<size_t>(o->dc->batch) * o->s->W * 4, cudaMemcpyDeviceToDevice,
+                           static_cast<cudaStream_t>(stream)));
     return GW_OK;
 }
 

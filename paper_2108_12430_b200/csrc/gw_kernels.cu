@@ -122,11 +122,14 @@ void launch_snapshot(const float* ring, float* out, const long long* count, int 
 // ---------------------------------------------------------------------------------------------
 constexpr int kGatherPos = 128;
 
+// Offline mode (seg_T > 0): the source is ONE stream's archival segment [channels][seg_T] and batch item `s` is
+// its window [s * seg_S, s * seg_S + W) -- no ring head, every item reads the same channel rows.
 __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, void* __restrict__ xw,
                                                 const long long* count, const int* __restrict__ rows_map,
-                                                int channels, int n_det, int n_wit, int W, int cpad, int fmt) {
+                                                int channels, int n_det, int n_wit, int W, int cpad, int fmt,
+                                                long long seg_T, int seg_S) {
     __shared__ float tile[32][kGatherPos + 1];
-    const int h = static_cast<int>(*count % W);
+    const int h = seg_T > 0 ? 0 : static_cast<int>(*count % W);
     const int sd = blockIdx.y;                       // stream * n_det + det
     const int s = sd / n_det, d = sd % n_det;
     const int cb = blockIdx.z * 32;                  // channel chunk
@@ -143,8 +146,9 @@ __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, 
             const int c = cb + cg * 16 + k;
             float v = 0.f;
             if (c < n_wit && n < W) {
-                const int row = s * channels + __ldg(rows_map + d * n_wit + c);
-                v = __ldg(ring + static_cast<size_t>(row) * W + slot);
+                const int mrow = __ldg(rows_map + d * n_wit + c);
+                v = seg_T > 0 ? __ldg(ring + static_cast<size_t>(mrow) * seg_T + static_cast<size_t>(s) * seg_S + n)
+                              : __ldg(ring + static_cast<size_t>(s * channels + mrow) * W + slot);
             }
             tile[cg * 16 + k][pos] = v;
         }
@@ -168,9 +172,10 @@ __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, 
 }
 
 void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
-                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st) {
+                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st, long long seg_T,
+                   int seg_S) {
     dim3 grid((W + kGatherPos - 1) / kGatherPos, n_streams * n_det, cpad / 32);
-    k_gather<<<grid, 256, 0, st>>>(ring, xw, count, rows_map, channels, n_det, n_wit, W, cpad, fmt);
+    k_gather<<<grid, 256, 0, st>>>(ring, xw, count, rows_map, channels, n_det, n_wit, W, cpad, fmt, seg_T, seg_S);
     ++g_kernel_launches;
 }
 
@@ -481,6 +486,46 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
         const int i = n - (W - a.delta - a.Lb);
         if (i >= 0 && i < a.Lb) *reinterpret_cast<float4*>(a.clf_in + static_cast<size_t>(sd) * a.Lb + i) = cleaned;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Offline mode (D9): overlap-add of the B windows [jS, jS + W) of one archival segment, gather form.  One
+// thread per output sample a: the covering windows j are visited in ascending order with the SAME fused
+// multiply-add chain as the streaming accumulator (acc = fma(w[n], p_j[n], acc) from 0), and the weight
+// sum comes from the same double table (cum[n] = sum_{i >= 0, n + iS < W} w[n + iS]), so a sample covered by
+// all W/S windows is bit-identical to the streaming path's final value.  pred: [B][D][W].
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_ola_offline(const float* __restrict__ pred, const float* __restrict__ seg,
+                                                     const int* __restrict__ strain_rows, const float* __restrict__ hann,
+                                                     const double* __restrict__ cum, float* __restrict__ cleaned,
+                                                     float* __restrict__ nhat_out, int B, int n_det, int W, int S,
+                                                     long long T) {
+    const long long a = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
+    const int d = blockIdx.y;
+    if (a >= T) return;
+    const int k = W / S;
+    const int q = static_cast<int>(a / S), r = static_cast<int>(a % S);
+    const int j_lo = q - k + 1 > 0 ? q - k + 1 : 0;
+    const int j_hi = q < B - 1 ? q : B - 1;
+    float acc = 0.f;
+    for (int j = j_lo; j <= j_hi; ++j) {
+        const int n = static_cast<int>(a - static_cast<long long>(j) * S);
+        acc = fmaf(__ldg(hann + n), __ldg(pred + (static_cast<size_t>(j) * n_det + d) * W + n), acc);
+    }
+    const int n_new = r + (q - j_hi) * S;                  // position in the newest covering window
+    const int n_past = r + (q - j_lo + 1) * S;             // first position of the chain NOT covered
+    const double sum = cum[n_new] - (n_past < W ? cum[n_past] : 0.0);
+    const float nhat = sum > 0.0 ? acc * static_cast<float>(1.0 / sum) : 0.f;
+    const float strain = __ldg(seg + static_cast<size_t>(__ldg(strain_rows + d)) * T + a);
+    cleaned[static_cast<size_t>(d) * T + a] = strain - nhat;
+    if (nhat_out) nhat_out[static_cast<size_t>(d) * T + a] = nhat;
+}
+
+void launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann, const double* cum,
+                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, cudaStream_t st) {
+    dim3 grid(static_cast<unsigned>((T + 255) / 256), n_det);
+    k_ola_offline<<<grid, 256, 0, st>>>(pred, seg, strain_rows, hann, cum, cleaned, nhat_out, B, n_det, W, S, T);
+    ++g_kernel_launches;
 }
 
 void launch_aggregate(const AggParams& a, cudaStream_t st) {

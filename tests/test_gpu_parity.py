@@ -363,3 +363,51 @@ def test_host_step_async_equals_device_step_bitwise():
         for t in range(n_up):
             assert np.array_equal(outs[mode][t][0], outs["device"][t][0]), (mode, t)
             assert np.array_equal(outs[mode][t][1], outs["device"][t][1]), (mode, t)
+
+
+# --------------------------------------------------------------- offline / non-streaming mode (D9)
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype", [gw.GW_FP16, gw.GW_BF16])
+def test_offline_matches_oracle_and_streaming_finals(dtype):
+    """B windows of one stream per launch: against the fp64 offline oracle (north_star tolerances on the raw
+    predictions and on the estimate), and -- a property that needs no oracle -- every sample covered by all W/S
+    windows is BIT-identical to the final value the streaming path emits for it."""
+    cfg = S.config_small_ensemble(1)                     # W = 2048, S = 256, k = 8, two detectors
+    sp = cfg.stream
+    W, St = sp.window, sp.stride
+    k = W // St
+    B = 21                                               # several tiles per window, odd count, ragged coverage at both ends
+    T = W + (B - 1) * St
+    dc_params, _ = util.make_params(cfg)
+    x = synth.stream_channels(cfg.seed + 40, sp, T)
+    off = gw.Offline(sp, cfg.dc_layers, dc_params, B, dtype)
+    assert off.samples == T
+    cleaned, noise = off.run(_dev(x))
+    torch.cuda.synchronize()
+    cleaned, noise, pred = cleaned.cpu().numpy(), noise.cpu().numpy(), off.predictions().cpu().numpy()
+    od = util.oracle_dtype(dtype)
+    rows = [(sp.witness_rows(d), sp.strain_row(d)) for d in range(sp.n_det)]
+    odc = [(cfg.dc_layers, [oracle.prepare_conv(l, p, od) for l, p in zip(cfg.dc_layers, dc_params[d])]) for d in range(sp.n_det)]
+    ref = oracle.offline_clean(x, W, St, rows, odc)
+    et = util.elem_tol(dtype)
+    for d in range(sp.n_det):
+        for j in (0, 1, B // 2, B - 1):
+            util.check_network_output(pred[j, d], ref["pred"][d, j], f"offline pred window {j} det {d}", elem=et)
+        rms_ref = ref["pred"][d]
+        util.check_network_output(noise[d], ref["nhat"][d], f"offline nhat det {d}", rms_ref=rms_ref, elem=et)
+        util.check_network_output(cleaned[d], ref["cleaned"][d], f"offline cleaned det {d}", rms_ref=rms_ref, elem=et)
+        assert noise[d, 0] == 0.0 and cleaned[d, 0] == x[sp.strain_row(d), 0]
+    # the streaming path over the same samples
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, None, dtype)
+    xd = _dev(x[None])
+    finals = np.full((sp.n_det, T), np.nan, dtype=np.float32)
+    for t in range(T // St):
+        stream.update(xd[:, :, t * St:(t + 1) * St].contiguous())
+        dc.forward()
+        f = dc.cleaned(gw.GW_FINAL).cpu().numpy()[0]
+        a0 = (t + 1) * St - W
+        if a0 >= 0:
+            finals[:, a0:a0 + St] = f
+    lo, hi = (k - 1) * St, T - (k - 1) * St
+    assert hi - lo >= 2 * St
+    assert np.array_equal(cleaned[:, lo:hi], finals[:, lo:hi])
