@@ -332,6 +332,33 @@ def run_native(args):
             gbs = b / (kernels[k]["ms"] * 1e-3) / 1e9
             kernels[k].update({"gbs": round(gbs, 1), "hbm_frac": round(gbs / pk["hbm_gbs"], 3)})
 
+    # offline / non-streaming mode (D9): the same number of detector-windows per launch, but all from ONE
+    # stream's archival segment (B = n windows advance the stream by B*S samples per launch)
+    offline = None
+    if not args.no_offline:
+        B = sp.n_streams
+        one = S.StreamSpec(1, sp.n_det, sp.fs, sp.window, sp.stride, sp.n_witness)
+        off = gw.Offline(one, cfg.dc_layers, dc_params, B, dtype)
+        seg = torch.from_numpy(synth.stream_channels(cfg.seed, one, off.samples)).cuda()
+        cl = torch.empty((sp.n_det, off.samples), device="cuda")
+        nz = torch.empty((sp.n_det, off.samples), device="cuda")
+        with torch.cuda.stream(cs):
+            for _ in range(3):
+                off.run(seg, cl, nz, cs)
+            o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            o0.record(cs)
+            n_off = max(10, min(K, 50))
+            for _ in range(n_off):
+                off.run(seg, cl, nz, cs)
+            o1.record(cs)
+        torch.cuda.synchronize()
+        off_ms = o0.elapsed_time(o1) / n_off
+        offline = {"windows_per_launch": B, "samples_per_launch": off.samples, "ms_per_launch": off_ms,
+                   "value": B * sp.stride / FS / (off_ms * 1e-3), "unit": UNIT,
+                   "what": "gw_offline_run on a device-resident segment of one 2-detector stream; value counts the B*S new "
+                           "samples a launch advances the stream by"}
+        del off, seg, cl, nz
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         times, cores = oracle_rate(cfg, args.dtype, 200, budget_s=15.0)   # a bounded sample: ~15 s of oracle time
@@ -351,7 +378,7 @@ def run_native(args):
                        "l2": f"inputs larger than L2: ring state {sp.n_streams * sp.channels * sp.window * 4 / 2**20:.0f} MiB "
                              "is re-read every step", "precision": f"{args.dtype} storage, fp32 accumulate"},
             "latency": latency, "e2e": e2e, "gpu_launches": int(launches), "graph_nodes": pipe.graph_nodes(),
-            "roofline": roofline, "kernels": kernels, "clocks": clocks, "cpu_baseline": cpu,
+            "roofline": roofline, "kernels": kernels, "clocks": clocks, "cpu_baseline": cpu, "offline": offline,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -366,7 +393,7 @@ def run_sweep(args):
         for n in SWEEP_STREAMS:
             for stride in SWEEP_STRIDES:
                 cmd = [sys.executable, os.path.abspath(__file__), "--streams", str(n), "--stride", str(stride), "--dtype", dtype,
-                       "--steps", str(args.steps), "--warmup", str(args.warmup), "--no-cpu-baseline",
+                       "--steps", str(args.steps), "--warmup", str(args.warmup), "--no-cpu-baseline", "--no-offline",
                        "--seg-seconds", str(4 if n >= 512 else SEG_SECONDS)]
                 res = subprocess.run(cmd, capture_output=True, text=True)
                 line = res.stdout.strip().splitlines()[-1] if res.returncode == 0 and res.stdout.strip() else None
@@ -398,6 +425,7 @@ def main():
     ap.add_argument("--sweep", metavar="FILE", help="run the configs[4] grid (n x stride x dtype), one bench line per "
                                                     "point appended to FILE (JSON lines); prints a table to stderr")
     ap.add_argument("--no-2sm", action="store_true", help="single-CTA kernel for the N=256 layers too (A/B aid)")
+    ap.add_argument("--no-offline", action="store_true", help="skip the offline-mode measurement")
     ap.add_argument("--timed-only", action="store_true",
                     help="only the warm-up and the timed region (for short runs under ncu); prints a reduced line")
     ap.add_argument("--reference-budget", type=float, default=150.0,

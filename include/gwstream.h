@@ -224,6 +224,19 @@ double gw_profile_flops(const gw_pipeline *p, int i);
 /* number of kernel nodes in the captured graph (0 before the first gw_step) */
 int gw_pipeline_graph_nodes(const gw_pipeline *p);
 
+/* ---- pre/post-processing at the edges of DeepClean (PAPER.md:198 "preprocesses", :212 "postprocessed"; the paper
+ * does not define them: reading A14 of DESIGN.md fixes per-channel standardisation) -------------------------------
+ * Witness c of detector d enters the network as (x - wit_mean[d*n_witness+c]) / wit_std[...] (applied in fp32
+ * when the sample is converted to the 16-bit storage type), and the aggregated estimate is subtracted from the
+ * strain as strain_std[d] * nhat + strain_mean[d] (gw_noise_estimate returns the rescaled estimate; the raw
+ * predictions of gw_deepclean_noise are unscaled).  Host arrays, copied; a NULL array means identity for that part;
+ * the default is identity everywhere, which is bit-exact with no processing at all.  wit_std must be > 0.
+ * gw_deepclean_set_scaling must precede the first update (GW_ESTATE otherwise: the state holds converted samples). */
+int gw_deepclean_set_scaling(gw_deepclean *dc, const float *wit_mean, const float *wit_std, const float *strain_mean,
+                             const float *strain_std);
+int gw_offline_set_scaling(gw_offline *o, const float *wit_mean, const float *wit_std, const float *strain_mean,
+                           const float *strain_std);
+
 /* ---- offline / non-streaming mode (PAPER.md:174 "adjacent frames ... in parallel", :202 offline regime, :216
  * non-streaming ensemble; D9) ---------------------------------------------------
  * One launch sequence cleans an ARCHIVAL segment of ONE stream: T = window + (n_windows - 1) * stride samples per

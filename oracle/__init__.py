@@ -281,7 +281,11 @@ class StreamOracle:
     """
 
     def __init__(self, channels: int, W: int, S: int, rows, dc, bbh=None, agg: int = AGG_HANN_OLA,
-                 delta: int = 0, max_updates: int = 64):
+                 delta: int = 0, max_updates: int = 64, scaling=None):
+        # scaling (reading A14): None or (wit_mean [D][n_wit], wit_std [D][n_wit],
+        # strain_mean [D], strain_std [D]): the network sees (x - mean) / std of every witness and the
+        # aggregated estimate is subtracted as strain_std * nhat + strain_mean.
+        self.scaling = scaling
         self.C, self.W, self.S = channels, W, S
         self.rows, self.dc, self.bbh, self.agg, self.delta = rows, dc, bbh, agg, delta
         self.T = max_updates * S
@@ -291,6 +295,20 @@ class StreamOracle:
         self.acc = np.zeros((ndet, self.T), dtype=np.float64)
         self.wsum = np.zeros((ndet, self.T), dtype=np.float64)
         self.w = hann(W)
+
+    def _cleaned(self, d: int, strain_all: np.ndarray, a0: int, a1: int):
+        """Estimate and cleaned strain of samples [a0, a1) of detector d (zeros before the stream start);
+        post-processing (A14): where an estimate exists it is rescaled to strain_std * nhat + strain_mean."""
+        nh = np.empty(a1 - a0); cl = np.empty(a1 - a0)
+        lib().gwo_cleaned(self.acc[d], self.wsum[d], strain_all, a0, a1, nh, cl)
+        if self.scaling is not None:
+            a = np.arange(a0, a1)
+            ok = (a >= 0) & (a < self.T)
+            has = np.zeros(a1 - a0, dtype=bool)
+            has[ok] = self.wsum[d][a[ok]] > 0
+            nh = np.where(has, float(self.scaling[3][d]) * nh + float(self.scaling[2][d]), nh)
+            cl = np.where(has, strain_all[np.clip(a, 0, self.T - 1)].astype(np.float64) - nh, cl)
+        return nh, cl
 
     def update(self, new: np.ndarray) -> Dict[str, np.ndarray]:
         """new [C][S] float32, strictly new samples.  Returns this update's results."""
@@ -304,7 +322,11 @@ class StreamOracle:
                "nhat_running": [], "cleaned_running": []}
         count = (t + 1) * S
         for d, ((wit, srow), (layers, prepared)) in enumerate(zip(self.rows, self.dc)):
-            p = deepclean_forward(snap[wit].astype(np.float64), layers, prepared)   # D2-D5
+            xin_d = snap[wit].astype(np.float64)
+            if self.scaling is not None:                                            # pre-processing (A14)
+                xin_d = (xin_d - _d(self.scaling[0])[d][:, None]) / _d(self.scaling[1])[d][:, None]
+                xin_d[:, :max(0, -first)] = 0.0      # before the stream start the network sees zeros (A12), not -mean/std
+            p = deepclean_forward(xin_d, layers, prepared)                          # D2-D5
             out["pred"].append(p)
             strain_all = np.ascontiguousarray(self.x[srow])
             if self.agg == AGG_HANN_OLA:                                            # D7
@@ -320,26 +342,22 @@ class StreamOracle:
                         self.wsum[d][a] = 1.0
                 acc, wsum = self.acc[d], self.wsum[d]
                 fin0 = a0
-            nh = np.empty(S); cl = np.empty(S)
-            lib().gwo_cleaned(acc, wsum, strain_all, fin0, fin0 + S, nh, cl)
+            nh, cl = self._cleaned(d, strain_all, fin0, fin0 + S)
             out["nhat_final"].append(nh); out["cleaned_final"].append(cl)
-            nhr = np.empty(W); clr = np.empty(W)
-            lib().gwo_cleaned(acc, wsum, strain_all, first, first + W, nhr, clr)
+            nhr, clr = self._cleaned(d, strain_all, first, first + W)
             out["nhat_running"].append(nhr); out["cleaned_running"].append(clr)
         if self.bbh is not None:                                                    # D8
             convs, pc, pd, Lb = self.bbh
             a1 = count - self.delta
             xin = np.zeros((len(self.rows), Lb), dtype=np.float64)
             for d, (wit, srow) in enumerate(self.rows):
-                nh = np.empty(Lb)
-                lib().gwo_cleaned(self.acc[d], self.wsum[d], np.ascontiguousarray(self.x[srow]),
-                                  a1 - Lb, a1, nh, xin[d])
+                _, xin[d] = self._cleaned(d, np.ascontiguousarray(self.x[srow]), a1 - Lb, a1)
             out["bbh_input"] = xin
             out["score"] = bbh_forward(xin, convs, pc, pd)
         return out
 
 
-def offline_clean(x: np.ndarray, W: int, S: int, rows, dc) -> Dict[str, np.ndarray]:
+def offline_clean(x: np.ndarray, W: int, S: int, rows, dc, scaling=None) -> Dict[str, np.ndarray]:
     """D9, offline / non-streaming mode ("adjacent frames ... in parallel",
     :202 offline regime, :216 non-streaming ensemble): an archival segment x [C][T], T = W + (B-1) S, of ONE
     stream is cut into the B windows [jS, jS + W) that lie inside it -- the same window grid as the streaming
@@ -366,11 +384,16 @@ def offline_clean(x: np.ndarray, W: int, S: int, rows, dc) -> Dict[str, np.ndarr
         acc = np.zeros(T, dtype=np.float64)
         wsum = np.zeros(T, dtype=np.float64)
         for j in range(B):
-            p = deepclean_forward(x[wit, j * S:j * S + W], layers, prepared)
+            xin = x[wit, j * S:j * S + W].astype(np.float64)
+            if scaling is not None:                       # pre-processing (A14), as in StreamOracle
+                xin = (xin - _d(scaling[0])[d][:, None]) / _d(scaling[1])[d][:, None]
+            p = deepclean_forward(xin, layers, prepared)
             pred[d, j] = p
             acc[j * S:j * S + W] += w * p
             wsum[j * S:j * S + W] += w
         ok = wsum > 0
         nhat[d, ok] = acc[ok] / wsum[ok]
+        if scaling is not None:                           # post-processing where an estimate exists
+            nhat[d, ok] = float(scaling[3][d]) * nhat[d, ok] + float(scaling[2][d])
         cleaned[d] = x[strain].astype(np.float64) - nhat[d]
     return {"pred": pred, "nhat": nhat, "cleaned": cleaned}

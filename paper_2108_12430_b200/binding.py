@@ -28,7 +28,7 @@ EXPORTS = [
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
     "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_step_host_async", "gw_pipeline_graph_nodes",
     "gw_step_profile", "gw_profile_label", "gw_profile_flops",
-    "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
+    "gw_deepclean_set_scaling", "gw_offline_set_scaling", "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
 ]
 
 _FP = C.POINTER(C.c_float)
@@ -100,6 +100,8 @@ def lib():
         L.gw_step.argtypes = [vp, vp, vp, vp, vp]
         L.gw_step_host.argtypes = [vp, vp, vp, vp, vp]
         L.gw_step_host_async.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_deepclean_set_scaling.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_offline_set_scaling.argtypes = [vp, vp, vp, vp, vp]
         L.gw_offline_create.argtypes = [C.POINTER(vp), vp, i, i, i, i, i, i]
         L.gw_offline_destroy.argtypes = [vp]
         L.gw_offline_samples.argtypes = [vp]
@@ -221,6 +223,13 @@ class Stream:
             pass
 
 
+def _scaling_args(*arrays):
+    keep = [None if a is None else np.ascontiguousarray(a, dtype=np.float32) for a in arrays]
+    ptrs = [C.c_void_p(0) if a is None else C.c_void_p(a.ctypes.data) for a in keep]
+    ptrs[0]._keep = keep                                  # the arrays outlive the call
+    return ptrs
+
+
 class DeepClean:
     """One DeepClean network per detector over a Stream."""
 
@@ -239,6 +248,11 @@ class DeepClean:
         spec = _DcSpec(n_det, len(layers), sp.n_witness, arr, wit, srow, agg, delta)
         self.h = C.c_void_p()
         _check(lib().gw_deepclean_create(C.byref(self.h), stream.h, C.byref(spec), dtype))
+
+    def set_scaling(self, wit_mean=None, wit_std=None, strain_mean=None, strain_std=None) -> None:
+        """Per-channel standardisation of the witnesses ([D][n_witness]) and rescaling of the estimate ([D]);
+        None = identity.  Before the first update."""
+        _check(lib().gw_deepclean_set_scaling(self.h, *_scaling_args(wit_mean, wit_std, strain_mean, strain_std)))
 
     def forward(self, stream=None) -> None:
         _check(lib().gw_deepclean_forward(self.h, _stream_ptr(stream)))
@@ -406,6 +420,9 @@ class Offline:
         _check(lib().gw_offline_create(C.byref(self.h), C.byref(dspec), spec.channels, spec.fs, spec.window, spec.stride,
                                        n_windows, dtype))
         self.samples = int(lib().gw_offline_samples(self.h))
+
+    def set_scaling(self, wit_mean=None, wit_std=None, strain_mean=None, strain_std=None) -> None:
+        _check(lib().gw_offline_set_scaling(self.h, *_scaling_args(wit_mean, wit_std, strain_mean, strain_std)))
 
     def run(self, samples, cleaned=None, noise=None, stream=None):
         """samples: CUDA float32 [C][T]; returns (cleaned [D][T], noise estimate [D][T])."""

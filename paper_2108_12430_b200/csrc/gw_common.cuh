@@ -101,12 +101,13 @@ bool is_ring16_append_kernel(const void* func);
 void launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st);
 void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
                           int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
-                          cudaStream_t st);
+                          const float* pre, cudaStream_t st);
 void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
-                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st, long long seg_T = 0,
-                   int seg_S = 0);
+                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, const float* pre, cudaStream_t st,
+                   long long seg_T = 0, int seg_S = 0);
 void launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann, const double* cum,
-                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, cudaStream_t st);
+                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, const float* post,
+                        cudaStream_t st);
 void launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
                         int L, int cpad, int K, int pad, int fmt, cudaStream_t st);
 struct AggParams {
@@ -117,6 +118,7 @@ struct AggParams {
     const int* strain_rows;    // [D]
     const float* hann;         // [W]
     const float* inv_wsum;     // [W]  1 / sum of the Hann weights covering window position n
+    const float* post;         // [D][2] post-processing of the estimate: (std, mean) of the strain (identity: 1, 0)
     float* final_out;          // [n][D][S] or null
     float* running_out;        // [n][D][W] or null
     float* nhat_out;           // [n][D][W] or null (test hook)

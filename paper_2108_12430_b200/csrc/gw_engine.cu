@@ -251,6 +251,8 @@ struct gw_deepclean {
     float* d_inv_wsum = nullptr;
     int* d_rows_map = nullptr;
     int* d_strain_rows = nullptr;
+    float* d_pre = nullptr;                      // [n_det][n_wit][2] witness standardisation (mean, 1/std); identity (0, 1)
+    float* d_post = nullptr;                     // [n_det][2] estimate back to strain units (std, mean); identity (1, 0)
     float* final_buf = nullptr;                  // [batch][S]
     float* clf_in = nullptr;                     // owned by the attached gw_bbh
     int Lb = 0;
@@ -530,6 +532,7 @@ extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
     cudaFree(dc->ring16);
     cudaFree(dc->d_wt_final); cudaFree(dc->d_b_final); cudaFree(dc->d_fin_B); cudaFree(dc->pred); cudaFree(dc->acc); cudaFree(dc->nhat);
     cudaFree(dc->d_hann); cudaFree(dc->d_inv_wsum); cudaFree(dc->d_rows_map); cudaFree(dc->d_strain_rows);
+    cudaFree(dc->d_pre); cudaFree(dc->d_post);
     cudaFree(dc->final_buf);
     if (dc->s && dc->s->dc == dc) dc->s->dc = nullptr;
     delete dc;
@@ -689,8 +692,48 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     CU_TRY(cudaMemcpy(dc->d_rows_map, spec->witness_rows, static_cast<size_t>(nd) * spec->n_witness * sizeof(int), cudaMemcpyHostToDevice));
     CU_TRY(cudaMalloc(&dc->d_strain_rows, nd * sizeof(int)));
     CU_TRY(cudaMemcpy(dc->d_strain_rows, spec->strain_row, nd * sizeof(int), cudaMemcpyHostToDevice));
+    {
+        std::vector<float> pre(static_cast<size_t>(nd) * spec->n_witness * 2), post(static_cast<size_t>(nd) * 2);
+        for (size_t i = 0; i < pre.size(); i += 2) { pre[i] = 0.f; pre[i + 1] = 1.f; }
+        for (size_t i = 0; i < post.size(); i += 2) { post[i] = 1.f; post[i + 1] = 0.f; }
+        CU_TRY(cudaMalloc(&dc->d_pre, pre.size() * 4));
+        CU_TRY(cudaMemcpy(dc->d_pre, pre.data(), pre.size() * 4, cudaMemcpyHostToDevice));
+        CU_TRY(cudaMalloc(&dc->d_post, post.size() * 4));
+        CU_TRY(cudaMemcpy(dc->d_post, post.data(), post.size() * 4, cudaMemcpyHostToDevice));
+    }
     CU_TRY(conv_gemm_prepare());
     return GW_OK;
+}
+
+// Pre/post-processing at the edges of DeepClean (PAPER.md:198 "preprocesses", :212 "postprocessed"; the paper
+// never defines them: DESIGN.md reading A14): witness c of detector d enters the network as
+// (x - wit_mean) / wit_std, and the aggregated estimate is subtracted as strain_std * nhat + strain_mean.
+static int set_scaling(gw_deepclean* dc, const float* wit_mean, const float* wit_std, const float* strain_mean,
+                       const float* strain_std) {
+    const int nd = dc->n_det, nw = dc->n_wit;
+    std::vector<float> pre(static_cast<size_t>(nd) * nw * 2), post(static_cast<size_t>(nd) * 2);
+    for (int i = 0; i < nd * nw; ++i) {
+        const double sd = wit_std ? wit_std[i] : 1.0;
+        if (!(sd > 0.0) || !isfinite(sd)) return fail(GW_EINVAL, "witness std must be finite and > 0");
+        pre[2 * i] = wit_mean ? wit_mean[i] : 0.f;
+        pre[2 * i + 1] = wit_std ? static_cast<float>(1.0 / sd) : 1.f;
+    }
+    for (int d = 0; d < nd; ++d) {
+        post[2 * d] = strain_std ? strain_std[d] : 1.f;
+        post[2 * d + 1] = strain_mean ? strain_mean[d] : 0.f;
+        if (!isfinite(post[2 * d]) || !isfinite(post[2 * d + 1])) return fail(GW_EINVAL, "strain scaling must be finite");
+    }
+    CU_TRY(cudaMemcpy(dc->d_pre, pre.data(), pre.size() * 4, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(dc->d_post, post.data(), post.size() * 4, cudaMemcpyHostToDevice));
+    return GW_OK;
+}
+
+extern "C" int gw_deepclean_set_scaling(gw_deepclean* dc, const float* wit_mean, const float* wit_std,
+                                        const float* strain_mean, const float* strain_std) {
+    if (!dc) return fail(GW_EINVAL, "gw_deepclean_set_scaling: NULL handle");
+    if (dc->s && dc->s->updates != 0)
+        return fail(GW_ESTATE, "gw_deepclean_set_scaling: must be called before the first update (the state holds converted samples)");
+    return set_scaling(dc, wit_mean, wit_std, strain_mean, strain_std);
 }
 
 extern "C" int gw_deepclean_create(gw_deepclean** out, gw_stream* s, const gw_dc_spec* spec, int dtype) {
@@ -728,7 +771,7 @@ static void ring16_append_enqueue(gw_deepclean* dc, const float* src, cudaStream
     if (!dc->mirror) return;
     gw_stream* s = dc->s;
     launch_ring16_append(src, dc->ring16, s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, s->S,
-                         dc->act_cols[0], dc->fmt, st);
+                         dc->act_cols[0], dc->fmt, dc->d_pre, st);
     prof_mark("ring16_append", st);
 }
 
@@ -736,7 +779,7 @@ static void deepclean_forward_enqueue(gw_deepclean* dc, cudaStream_t st) {
     gw_stream* s = dc->s;
     if (!dc->mirror) {
         launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
-                      dc->act_cols[0], dc->fmt, st);
+                      dc->act_cols[0], dc->fmt, dc->d_pre, st);
         prof_mark("gather", st);
     }
     for (auto& g : dc->gemm) run_gemm(g, st);
@@ -820,6 +863,12 @@ extern "C" int gw_offline_create(gw_offline** out, const gw_dc_spec* spec, int c
     return GW_OK;
 }
 
+extern "C" int gw_offline_set_scaling(gw_offline* o, const float* wit_mean, const float* wit_std, const float* strain_mean,
+                                      const float* strain_std) {
+    if (!o) return fail(GW_EINVAL, "gw_offline_set_scaling: NULL handle");
+    return set_scaling(o->dc, wit_mean, wit_std, strain_mean, strain_std);
+}
+
 extern "C" int64_t gw_offline_samples(const gw_offline* o) { return o ? o->T : 0; }
 
 extern "C" int gw_offline_run(gw_offline* o, const float* samples_dev, float* cleaned_dev, float* noise_dev, void* stream) {
@@ -828,7 +877,7 @@ extern "C" int gw_offline_run(gw_offline* o, const float* samples_dev, float* cl
     gw_stream* s = o->s;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     launch_gather(samples_dev, dc->act[0], nullptr, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, dc->act_cols[0],
-                  dc->fmt, st, o->T, s->S);
+                  dc->fmt, dc->d_pre, st, o->T, s->S);
     prof_mark("gather", st);
     for (auto& g : dc->gemm) run_gemm(g, st);
     if (!dc->fused_tail) {
@@ -836,7 +885,7 @@ extern "C" int gw_offline_run(gw_offline* o, const float* samples_dev, float* cl
                            dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
     }
     launch_ola_offline(dc->pred, samples_dev, dc->d_strain_rows, dc->d_hann, o->d_cum, cleaned_dev, noise_dev, o->B, dc->n_det,
-                       s->W, s->S, o->T, st);
+                       s->W, s->S, o->T, dc->d_post, st);
     CU_TRY(cudaGetLastError());
     dc->forward_for += 1;                        // gw_deepclean_noise-style hooks see a completed pass
     return GW_OK;
@@ -886,7 +935,7 @@ static void cleaned_enqueue(gw_deepclean* dc, float* final_out, float* running_o
     gw_stream* s = dc->s;
     AggParams a;
     a.pred = dc->pred; a.acc = dc->acc; a.ring = s->ring; a.count = s->d_count; a.strain_rows = dc->d_strain_rows;
-    a.hann = dc->d_hann; a.inv_wsum = dc->d_inv_wsum;
+    a.hann = dc->d_hann; a.inv_wsum = dc->d_inv_wsum; a.post = dc->d_post;
     a.final_out = final_out; a.running_out = running_out; a.nhat_out = nhat_out; a.clf_in = dc->clf_in;
     a.n_streams = s->n; a.n_det = dc->n_det; a.channels = s->C; a.W = s->W; a.S = s->S; a.Lb = dc->Lb;
     a.delta = dc->delta; a.agg = dc->agg;
@@ -1147,10 +1196,10 @@ static int set_node_src(gw_pipeline* p, cudaGraphNode_t node, int n_args, int sr
 }
 
 static int pipeline_set_input(gw_pipeline* p, const float* in) {
-    // k_append(ring, src, count, ticket, n_rows, W, S); k_ring16_append(src, ring16, count, rows_map, ... 11 args)
+    // k_append(ring, src, count, ticket, n_rows, W, S); k_ring16_append(src, ring16, count, rows_map, ... 12 args)
     if (int rc = set_node_src(p, p->append_node, 7, 1, in)) return rc;
     if (p->ring16_node)
-        if (int rc = set_node_src(p, p->ring16_node, 11, 0, in)) return rc;
+        if (int rc = set_node_src(p, p->ring16_node, 12, 0, in)) return rc;
     p->cap_in = in;
     return GW_OK;
 }

@@ -127,7 +127,7 @@ constexpr int kGatherPos = 128;
 __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, void* __restrict__ xw,
                                                 const long long* count, const int* __restrict__ rows_map,
                                                 int channels, int n_det, int n_wit, int W, int cpad, int fmt,
-                                                long long seg_T, int seg_S) {
+                                                long long seg_T, int seg_S, const float* __restrict__ pre) {
     __shared__ float tile[32][kGatherPos + 1];
     const int h = seg_T > 0 ? 0 : static_cast<int>(*count % W);
     const int sd = blockIdx.y;                       // stream * n_det + det
@@ -149,6 +149,9 @@ __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, 
                 const int mrow = __ldg(rows_map + d * n_wit + c);
                 v = seg_T > 0 ? __ldg(ring + static_cast<size_t>(mrow) * seg_T + static_cast<size_t>(s) * seg_S + n)
                               : __ldg(ring + static_cast<size_t>(s * channels + mrow) * W + slot);
+                const float2 ms = __ldg(reinterpret_cast<const float2*>(pre) + d * n_wit + c);   // (mean, 1/std)
+                v = (v - ms.x) * ms.y;
+                if (seg_T == 0 && *count - W + n < 0) v = 0.f;   // before the stream start the network sees zeros (A12)
             }
             tile[cg * 16 + k][pos] = v;
         }
@@ -172,10 +175,10 @@ __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, 
 }
 
 void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
-                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, cudaStream_t st, long long seg_T,
-                   int seg_S) {
+                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, const float* pre, cudaStream_t st,
+                   long long seg_T, int seg_S) {
     dim3 grid((W + kGatherPos - 1) / kGatherPos, n_streams * n_det, cpad / 32);
-    k_gather<<<grid, 256, 0, st>>>(ring, xw, count, rows_map, channels, n_det, n_wit, W, cpad, fmt, seg_T, seg_S);
+    k_gather<<<grid, 256, 0, st>>>(ring, xw, count, rows_map, channels, n_det, n_wit, W, cpad, fmt, seg_T, seg_S, pre);
     ++g_kernel_launches;
 }
 
@@ -191,7 +194,7 @@ void launch_gather(const float* ring, void* xw, const long long* count, const in
 __global__ void __launch_bounds__(256) k_ring16_append(const float* __restrict__ src, void* __restrict__ ring16,
                                                        const long long* count, const int* __restrict__ rows_map,
                                                        int channels, int n_det, int n_wit, int W, int S, int cpad,
-                                                       int fmt) {
+                                                       int fmt, const float* __restrict__ pre) {
     __shared__ float tile[32][kGatherPos + 1];
     const int h0 = static_cast<int>((*count - S) % W);   // ring slot of this update's first sample
     const int sd = blockIdx.y;
@@ -209,7 +212,8 @@ __global__ void __launch_bounds__(256) k_ring16_append(const float* __restrict__
             float v = 0.f;
             if (c < n_wit && i < S) {
                 const int row = s * channels + __ldg(rows_map + d * n_wit + c);
-                v = __ldg(src + static_cast<size_t>(row) * S + i);
+                const float2 ms = __ldg(reinterpret_cast<const float2*>(pre) + d * n_wit + c);   // (mean, 1/std)
+                v = (__ldg(src + static_cast<size_t>(row) * S + i) - ms.x) * ms.y;
             }
             tile[cg * 16 + k][pos] = v;
         }
@@ -239,9 +243,9 @@ bool is_ring16_append_kernel(const void* func) { return func == reinterpret_cast
 
 void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
                           int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
-                          cudaStream_t st) {
+                          const float* pre, cudaStream_t st) {
     dim3 grid((S + kGatherPos - 1) / kGatherPos, n_streams * n_det, cpad / 32);
-    k_ring16_append<<<grid, 256, 0, st>>>(new_samples, ring16, count, rows_map, channels, n_det, n_wit, W, S, cpad, fmt);
+    k_ring16_append<<<grid, 256, 0, st>>>(new_samples, ring16, count, rows_map, channels, n_det, n_wit, W, S, cpad, fmt, pre);
     ++g_kernel_launches;
 }
 
@@ -424,6 +428,8 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
             else if (n >= W - S - a.delta) { nhat = p; a.acc[wi + slot] = p; }
             else nhat = a.acc[wi + slot];
         }
+        if (a.agg == 0 || n < W - a.delta)                 // post-processing: estimate back to strain units
+            nhat = fmaf(__ldg(a.post + 2 * d), nhat, __ldg(a.post + 2 * d + 1));
         const float strain = __ldg(a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot);
         cleaned = strain - nhat;
     }
@@ -472,6 +478,10 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
             else if (n >= W - S - a.delta) { nhat = p; *accp = p; }
             else nhat = *accp;
         }
+        if (a.agg == 0 || n < W - a.delta) {               // post-processing: estimate back to strain units
+            const float ps = __ldg(a.post + 2 * d), pm = __ldg(a.post + 2 * d + 1);
+            nhat = make_float4(fmaf(ps, nhat.x, pm), fmaf(ps, nhat.y, pm), fmaf(ps, nhat.z, pm), fmaf(ps, nhat.w, pm));
+        }
         const float4 st4 = __ldg(reinterpret_cast<const float4*>(
             a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot));
         cleaned = make_float4(st4.x - nhat.x, st4.y - nhat.y, st4.z - nhat.z, st4.w - nhat.w);
@@ -499,7 +509,7 @@ __global__ void __launch_bounds__(256) k_ola_offline(const float* __restrict__ p
                                                      const int* __restrict__ strain_rows, const float* __restrict__ hann,
                                                      const double* __restrict__ cum, float* __restrict__ cleaned,
                                                      float* __restrict__ nhat_out, int B, int n_det, int W, int S,
-                                                     long long T) {
+                                                     long long T, const float* __restrict__ post) {
     const long long a = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x;
     const int d = blockIdx.y;
     if (a >= T) return;
@@ -515,16 +525,17 @@ __global__ void __launch_bounds__(256) k_ola_offline(const float* __restrict__ p
     const int n_new = r + (q - j_hi) * S;                  // position in the newest covering window
     const int n_past = r + (q - j_lo + 1) * S;             // first position of the chain NOT covered
     const double sum = cum[n_new] - (n_past < W ? cum[n_past] : 0.0);
-    const float nhat = sum > 0.0 ? acc * static_cast<float>(1.0 / sum) : 0.f;
+    const float nhat = sum > 0.0 ? fmaf(__ldg(post + 2 * d), acc * static_cast<float>(1.0 / sum), __ldg(post + 2 * d + 1)) : 0.f;
     const float strain = __ldg(seg + static_cast<size_t>(__ldg(strain_rows + d)) * T + a);
     cleaned[static_cast<size_t>(d) * T + a] = strain - nhat;
     if (nhat_out) nhat_out[static_cast<size_t>(d) * T + a] = nhat;
 }
 
 void launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann, const double* cum,
-                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, cudaStream_t st) {
+                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, const float* post,
+                        cudaStream_t st) {
     dim3 grid(static_cast<unsigned>((T + 255) / 256), n_det);
-    k_ola_offline<<<grid, 256, 0, st>>>(pred, seg, strain_rows, hann, cum, cleaned, nhat_out, B, n_det, W, S, T);
+    k_ola_offline<<<grid, 256, 0, st>>>(pred, seg, strain_rows, hann, cum, cleaned, nhat_out, B, n_det, W, S, T, post);
     ++g_kernel_launches;
 }
 

@@ -411,3 +411,77 @@ def test_offline_matches_oracle_and_streaming_finals(dtype):
     lo, hi = (k - 1) * St, T - (k - 1) * St
     assert hi - lo >= 2 * St
     assert np.array_equal(cleaned[:, lo:hi], finals[:, lo:hi])
+
+
+# ------------------------------------------------------- pre/post-processing (reading A14)
+def _scaling_for(sp, seed=0):
+    rng = np.random.default_rng(900 + seed)
+    return (rng.normal(0, 0.5, (sp.n_det, sp.n_witness)).astype(np.float32),
+            rng.uniform(0.5, 2.0, (sp.n_det, sp.n_witness)).astype(np.float32),
+            rng.normal(0, 0.3, sp.n_det).astype(np.float32), rng.uniform(0.5, 2.0, sp.n_det).astype(np.float32))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("stride", [256, 255])           # mirror-ring path / gather path (odd stride)
+def test_scaled_streaming_matches_oracle(stride):
+    cfg0 = S.config_small_ensemble(2)
+    sp = S.StreamSpec(2, 2, 4096, 2048, stride)          # 255 does not divide 2048: LAST_STRIDE aggregation there
+    cfg = S.Config("scaled", sp, cfg0.dc_layers, cfg0.bbh_convs, cfg0.bbh_dense, cfg0.bbh_len, 10, 5)
+    dtype = gw.GW_FP16
+    agg = S.AGG_HANN_OLA if stride == 256 else S.AGG_LAST_STRIDE
+    dc_params, bbh_params = util.make_params(cfg)
+    scaling = _scaling_for(sp)
+    n_up = 10
+    x = synth.multi_stream(cfg.seed, sp, n_up * sp.stride)
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, agg, 0)
+    dc.set_scaling(*scaling)
+    oracles = [util.make_stream_oracle(cfg, dc_params, bbh_params, dtype, n_up, agg, 0, scaling=scaling) for _ in range(sp.n_streams)]
+    xd = _dev(x)
+    for t in range(n_up):
+        stream.update(xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous())
+        dc.forward()
+        pred = dc.noise().cpu().numpy()
+        running = dc.cleaned(gw.GW_RUNNING).cpu().numpy()
+        nhat = dc.noise_estimate().cpu().numpy()
+        scores = bbh.score().cpu().numpy()
+        for i, orc in enumerate(oracles):
+            ref = orc.update(x[i][:, t * sp.stride:(t + 1) * sp.stride])
+            for d in range(sp.n_det):
+                tag = f"scaled update {t} stream {i} det {d}"
+                util.check_network_output(pred[i, d], ref["pred"][d], "pred " + tag)
+                rms_n = float(scaling[3][d]) * ref["pred"][d]          # the estimate's scale after rescaling
+                util.check_network_output(nhat[i, d], ref["nhat_running"][d], "nhat " + tag, rms_ref=rms_n)
+                util.check_network_output(running[i, d], ref["cleaned_running"][d], "cleaned " + tag, rms_ref=rms_n)
+            assert abs(float(scores[i]) - ref["score"]) <= util.SCORE_ABS
+    with pytest.raises(gw.GwError):
+        dc.set_scaling(*scaling)                        # after the first update: GW_ESTATE
+
+
+@pytest.mark.gpu
+def test_identity_scaling_is_bit_exact_and_offline_scaling_matches_oracle():
+    cfg = S.config_small_ensemble(1)
+    sp = cfg.stream
+    dc_params, _ = util.make_params(cfg)
+    B = 9
+    T = sp.window + (B - 1) * sp.stride
+    x = synth.stream_channels(77, sp, T)
+    outs = []
+    for ident in (False, True):
+        off = gw.Offline(sp, cfg.dc_layers, dc_params, B, gw.GW_FP16)
+        if ident:
+            off.set_scaling(np.zeros((sp.n_det, sp.n_witness)), np.ones((sp.n_det, sp.n_witness)), np.zeros(sp.n_det), np.ones(sp.n_det))
+        c, n = off.run(_dev(x))
+        outs.append((c.cpu().numpy(), n.cpu().numpy()))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    scaling = _scaling_for(sp, 1)
+    off = gw.Offline(sp, cfg.dc_layers, dc_params, B, gw.GW_FP16)
+    off.set_scaling(*scaling)
+    c, n = off.run(_dev(x))
+    c, n = c.cpu().numpy(), n.cpu().numpy()
+    rows = [(sp.witness_rows(d), sp.strain_row(d)) for d in range(sp.n_det)]
+    odc = [(cfg.dc_layers, [oracle.prepare_conv(l, p, oracle.DT_FP16) for l, p in zip(cfg.dc_layers, dc_params[d])]) for d in range(sp.n_det)]
+    ref = oracle.offline_clean(x, sp.window, sp.stride, rows, odc, scaling=scaling)
+    for d in range(sp.n_det):
+        rms_n = float(scaling[3][d]) * ref["pred"][d]
+        util.check_network_output(n[d], ref["nhat"][d], f"offline scaled nhat det {d}", rms_ref=rms_n)
+        util.check_network_output(c[d], ref["cleaned"][d], f"offline scaled cleaned det {d}", rms_ref=rms_n)

@@ -557,3 +557,43 @@ def test_offline_constant_prediction_gives_the_constant():
     off = oracle.offline_clean(x, sp.window, sp.stride, [(sp.witness_rows(0), sp.strain_row(0))], [(cfg.dc_layers, prepared)])
     assert np.allclose(off["nhat"][0, 1:], 0.375, rtol=0, atol=1e-15)
     assert np.allclose(off["cleaned"][0, 1:], x[sp.strain_row(0), 1:].astype(np.float64) - 0.375, rtol=0, atol=1e-15)
+
+
+# ------------------------------------------------ pre/post-processing (reading A14)
+def test_scaling_is_input_standardisation_and_affine_output():
+    """The scaled oracle is pinned against the unscaled one (pinned above): standardising the witnesses inside
+    equals feeding pre-standardised witnesses, and the estimate is the unscaled estimate mapped through
+    strain_std * nhat + strain_mean; identity scaling changes nothing at all."""
+    cfg = S.config_c0()
+    sp = cfg.stream
+    rng = np.random.default_rng(11)
+    params = synth.deepclean_params(21, cfg.dc_layers)
+    prepared = [oracle.prepare_conv(l, p, oracle.DT_FP16) for l, p in zip(cfg.dc_layers, params)]
+    rows = [(sp.witness_rows(0), sp.strain_row(0))]
+    dc = [(cfg.dc_layers, prepared)]
+    n_up = 11
+    x = synth.stream_channels(5, sp, n_up * sp.stride, white=True)
+    mu = rng.normal(0, 0.5, (1, sp.n_witness)); sd = rng.uniform(0.5, 2.0, (1, sp.n_witness))
+    smu = np.array([0.25]); ssd = np.array([1.75])
+    xs = x.astype(np.float64).copy()
+    xs[sp.witness_rows(0)] = (xs[sp.witness_rows(0)] - mu[0][:, None]) / sd[0][:, None]
+    a = oracle.StreamOracle(sp.channels, sp.window, sp.stride, rows, dc, None, max_updates=n_up, scaling=(mu, sd, smu, ssd))
+    b = oracle.StreamOracle(sp.channels, sp.window, sp.stride, rows, dc, None, max_updates=n_up)
+    tol = 1e-5                                        # b is fed the standardised witnesses rounded to float32 (its input type)
+    c = oracle.StreamOracle(sp.channels, sp.window, sp.stride, rows, dc, None, max_updates=n_up,
+                            scaling=(np.zeros_like(mu), np.ones_like(sd), np.zeros(1), np.ones(1)))
+    e = oracle.StreamOracle(sp.channels, sp.window, sp.stride, rows, dc, None, max_updates=n_up)
+    for t in range(n_up):
+        sl = slice(t * sp.stride, (t + 1) * sp.stride)
+        ra, rb = a.update(x[:, sl]), b.update(xs[:, sl].astype(np.float32))
+        assert np.allclose(ra["pred"][0], rb["pred"][0], rtol=0, atol=tol)
+        assert float(np.sqrt(np.mean(ra["pred"][0] ** 2))) > 0.05          # the comparison is not vacuous
+        assert np.allclose(ra["nhat_running"][0][ra["nhat_running"][0] != 0],
+                           (ssd[0] * rb["nhat_running"][0] + smu[0])[ra["nhat_running"][0] != 0], rtol=0, atol=tol)
+        first = (t + 1) * sp.stride - sp.window
+        n0 = max(0, -first)
+        strain = x[sp.strain_row(0), first + n0:first + sp.window].astype(np.float64)
+        assert np.allclose(ra["cleaned_running"][0][n0:], strain - ra["nhat_running"][0][n0:], rtol=0, atol=1e-12)
+        rc, re = c.update(x[:, sl]), e.update(x[:, sl])
+        for key in ("pred", "nhat_final", "cleaned_final", "nhat_running", "cleaned_running"):
+            assert np.array_equal(rc[key][0], re[key][0]), key

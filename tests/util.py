@@ -63,7 +63,7 @@ def make_params(cfg: S.Config):
 
 
 def make_stream_oracle(cfg: S.Config, dc_params, bbh_params, dtype: int, max_updates: int,
-                       agg: int = oracle.AGG_HANN_OLA, delta: int = 0):
+                       agg: int = oracle.AGG_HANN_OLA, delta: int = 0, scaling=None):
     st = cfg.stream
     od = oracle_dtype(dtype)
     rows = [(st.witness_rows(d), st.strain_row(d)) for d in range(st.n_det)]
@@ -75,7 +75,7 @@ def make_stream_oracle(cfg: S.Config, dc_params, bbh_params, dtype: int, max_upd
         bbh = (cfg.bbh_convs, [oracle.prepare_conv(l, p, od) for l, p in zip(cfg.bbh_convs, cp)],
                [oracle.prepare_dense(p) for p in dp], cfg.bbh_len)
     return oracle.StreamOracle(st.channels, st.window, st.stride, rows, dc, bbh, agg=agg, delta=delta,
-                               max_updates=max_updates)
+                               max_updates=max_updates, scaling=scaling)
 
 
 def check_network_output(got: np.ndarray, ref: np.ndarray, what: str, rms_ref: np.ndarray | None = None,
