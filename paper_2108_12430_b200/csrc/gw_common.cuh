@@ -37,6 +37,10 @@ struct ConvGemmParams {
     // that a captured graph replays unchanged.  Rows outside [0, a_rows) are zeroed in shared memory after the
     // TMA load (the ring holds real samples there, not padding).  a_count == nullptr: plain activation tensor.
     const long long* a_count;
+    // Offline source (a_4d = 1): tmA is 4-D (cols, rows, detector, window) over ONE stream's 16-bit segment
+    // [n_det][T][cpad]; window j is the overlapping row range starting S/2 rows after window j-1 (its stride in the
+    // tensor map), so no per-window copy exists and rows outside [0, a_rows) are still TMA's zero fill.
+    int a_4d;
     int a_ring_W, a_ring_div;
     int M;                         // output rows per batch item
     int N;                         // GEMM N, multiple of 32, <= 256

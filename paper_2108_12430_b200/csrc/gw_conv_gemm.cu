@@ -284,7 +284,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                         const int stage = second ? ring0 + rs1 : rs0;
                         TR_WAIT(0, mbar_wait(&a_empty[stage], (second ? rp1 : rp0) ^ 1))
                         mbar_arrive_expect_tx(&a_full[stage], p.slab_rows * 128);
-                        tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min + row_off, batch);
+                        if (p.a_4d) tma_load_4d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min, det, u / spi);
+                        else tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min + row_off, batch);
                         if (second) { if (++rs1 == sa - ring0) { rs1 = 0; rp1 ^= 1; } }
                         else if (++rs0 == ring0) { rs0 = 0; rp0 ^= 1; }
                         if (!p.b_resident) {

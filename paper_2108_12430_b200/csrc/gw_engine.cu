@@ -91,6 +91,21 @@ static int get_encode() {
     return GW_OK;
 }
 
+// 4-D tensor of 16-bit elements (offline first layer: cols, rows, detector, window), box (64, box1, 1, 1), 128B swizzle.
+static int make_tmap4(CUtensorMap* tm, const void* base, int fmt, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t d3,
+                      uint64_t stride1, uint64_t stride2, uint64_t stride3, uint32_t box1) {
+    if (int rc = get_encode()) return rc;
+    cuuint64_t dims[4] = {d0, d1, d2, d3};
+    cuuint64_t strides[3] = {stride1 * 2, stride2 * 2, stride3 * 2};
+    cuuint32_t box[4] = {kSegK, box1, 1, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = g_encode(tm, fmt == FMT_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 4,
+                          const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(GW_ECUDA, "cuTensorMapEncodeTiled (4-D) failed (%d)", (int)r);
+    return GW_OK;
+}
+
 // 3-D tensor of 16-bit elements, dims (d0 fastest, d1, d2), strides in elements, box (64, box1, 1), 128B swizzle.
 static int make_tmap(CUtensorMap* tm, const void* base, int fmt, uint64_t d0, uint64_t d1, uint64_t d2,
                      uint64_t stride1, uint64_t stride2, uint32_t box1, uint32_t box0 = kSegK) {
@@ -235,7 +250,10 @@ struct gw_deepclean {
     std::vector<HostLayer> host;                 // [n_det * n_layers]
     std::vector<GemmLayer> gemm;                 // layers 0 .. n_layers-2
     void* ring16 = nullptr;                      // mirror ring [batch][2W][cpad0], 16-bit (when `mirror`)
-    bool offline = false;                        // owned by a gw_offline: windows of one archival segment, gather path
+    bool offline = false;                        // owned by a gw_offline: windows of one archival segment
+    long long off_T = 0;                         // offline: samples per channel of the segment
+    void* seg16 = nullptr;                       // offline: 16-bit channels-last segment [n_det][T][cpad0]; the first layer
+                                                 // reads its overlapping windows straight from it (null: gather path)
     bool mirror = false;                         // first layer reads the window from ring16 (no per-update gather)
     bool fused_tail = false;                     // last GEMM layer + final ConvTranspose1d run as one kernel (EPI_FINAL)
     std::vector<void*> act;                      // act[0] = gathered window (null when `mirror`), act[i+1] = output of layer i
@@ -302,7 +320,7 @@ struct gw_pipeline {
 // (position parity inside a pair row; always 0 for GK_DEC) to output column half r; <0 or >=k: none.
 static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, int n_det, int fmt, const void* in,
                             int in_L, int cin_p, void* out, int cout_p, int batch, int epi, int head_hidden = 0,
-                            const long long* ring_count = nullptr, int ring_W = 0) {
+                            const long long* ring_count = nullptr, int ring_W = 0, long long seg_T = 0, int seg_S = 0) {
     const HostLayer& H0 = dets[0];
     ConvGemmParams& p = gl.g.p;
     memset(&p, 0, sizeof p);
@@ -395,7 +413,12 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     CU_TRY(cudaMalloc(&gl.d_bias, bias.size() * 4));
     CU_TRY(cudaMemcpy(gl.d_bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
     p.A = in; p.B = gl.d_B; p.bias = gl.d_bias; p.out = out;
-    if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows_tm, batch, p.a_cols, static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, p.slab_rows)) return rc;
+    if (seg_T > 0) {
+        // offline first layer: `in` = [n_det][seg_T][cin_p]; window j starts seg_S positions after window j - 1
+        p.a_4d = 1;
+        if (int rc = make_tmap4(&p.tmA, in, fmt, p.a_cols, p.a_rows, n_det, batch / n_det, p.a_cols,
+                                static_cast<uint64_t>(seg_T) * cin_p, static_cast<uint64_t>(seg_S) * cin_p, p.slab_rows)) return rc;
+    } else if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows_tm, batch, p.a_cols, static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, p.slab_rows)) return rc;
     if (epi == EPI_STORE)   // output [batch][M][N]: one 32-row x min(N, 64)-column box per epilogue-warp store
         if (int rc = make_tmap(&p.tmOut, out, fmt, p.N, p.M, batch, p.N, static_cast<uint64_t>(p.M) * p.N, 32, p.N >= 64 ? 64 : 32)) return rc;
     gl.g.batch = batch;
@@ -529,7 +552,7 @@ extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
     if (!dc) return GW_OK;
     for (auto& g : dc->gemm) free_gemm(g);
     for (void* a : dc->act) cudaFree(a);
-    cudaFree(dc->ring16);
+    cudaFree(dc->ring16); cudaFree(dc->seg16);
     cudaFree(dc->d_wt_final); cudaFree(dc->d_b_final); cudaFree(dc->d_fin_B); cudaFree(dc->pred); cudaFree(dc->acc); cudaFree(dc->nhat);
     cudaFree(dc->d_hann); cudaFree(dc->d_inv_wsum); cudaFree(dc->d_rows_map); cudaFree(dc->d_strain_rows);
     cudaFree(dc->d_pre); cudaFree(dc->d_post);
@@ -581,6 +604,10 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     // The 16-bit mirror ring replaces the per-update gather when window positions pair up with ring slots
     // (even stride => even head) and the first layer is a Conv1d; otherwise the window is re-gathered.
     dc->mirror = !dc->offline && (S % 2 == 0) && (W % 2 == 0) && dc->host[0].kind == GW_CONV;
+    // offline: the first layer reads overlapping windows of the converted segment through a 4-D tensor map when
+    // window starts fall on position pairs (even stride); otherwise every window is gathered (k_gather)
+    const bool direct_seg = dc->offline && (S % 2 == 0) && (W % 2 == 0) && dc->host[0].kind == GW_CONV &&
+                            g_conv_impl == GW_IMPL_UMMA;
     // The last GEMM layer (ConvTranspose1d -> <= 32 channels, tanh) and the final 1-channel ConvTranspose1d
     // (k = 7) run as ONE kernel when they have the standard shape: the 16-bit activation between them is
     // never written (at C3 that round trip is 2 x 1 MiB per detector-window, more than the layer's input).
@@ -595,6 +622,7 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         size_t bytes = static_cast<size_t>(batch) * len[i] * cpad[i] * 2;
         void** dst = &dc->act[i];
         if (i == 0 && dc->mirror) { bytes *= 2; dst = &dc->ring16; }
+        if (i == 0 && direct_seg) { bytes = static_cast<size_t>(nd) * dc->off_T * cpad[0] * 2; dst = &dc->seg16; }
         CU_TRY(cudaMalloc(dst, bytes));
         CU_TRY(cudaMemset(*dst, 0, bytes));
     }
@@ -605,9 +633,12 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         const GemmKind gk = dc->host[i].kind == GW_CONV ? GK_ENC : GK_DEC;
         const bool from_ring = i == 0 && dc->mirror;
         const bool fin = i == nl - 2 && dc->fused_tail;
-        if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, from_ring ? dc->ring16 : dc->act[i],
+        const bool from_seg = i == 0 && direct_seg;
+        if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt,
+                                      from_ring ? dc->ring16 : from_seg ? dc->seg16 : dc->act[i],
                                       len[i], cpad[i], dc->act[i + 1], cpad[i + 1], batch, fin ? EPI_FINAL : EPI_STORE, 0,
-                                      from_ring ? s->d_count : nullptr, from_ring ? W : 0))
+                                      from_ring ? s->d_count : nullptr, from_ring ? W : 0, from_seg ? dc->off_T : 0,
+                                      from_seg ? S : 0))
             return rc;
         dc->gemm[i].g.p.reverse = g_snake ? (i & 1) : 0;
         dc->gemm[i].name = "gemm.dc" + std::to_string(i);
@@ -842,7 +873,7 @@ extern "C" int gw_offline_create(gw_offline** out, const gw_dc_spec* spec, int c
     gw_deepclean* dc = new gw_deepclean();
     o->dc = dc;
     dc->s = o->s; dc->n_det = spec->n_det; dc->n_layers = spec->n_layers; dc->n_wit = spec->n_witness;
-    dc->agg = GW_AGG_HANN_OLA; dc->delta = 0; dc->offline = true;
+    dc->agg = GW_AGG_HANN_OLA; dc->delta = 0; dc->offline = true; dc->off_T = o->T;
     dc->fmt = dtype == GW_BF16 ? FMT_BF16 : FMT_FP16;
     int rc = deepclean_build(dc, o->s, spec);
     if (rc == GW_OK) {
@@ -876,8 +907,13 @@ extern "C" int gw_offline_run(gw_offline* o, const float* samples_dev, float* cl
     gw_deepclean* dc = o->dc;
     gw_stream* s = o->s;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    launch_gather(samples_dev, dc->act[0], nullptr, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, dc->act_cols[0],
-                  dc->fmt, dc->d_pre, st, o->T, s->S);
+    if (dc->seg16) {       // the whole segment as ONE "window" of length T: converts every sample once
+        launch_gather(samples_dev, dc->seg16, nullptr, dc->d_rows_map, 1, s->C, dc->n_det, dc->n_wit, static_cast<int>(o->T),
+                      dc->act_cols[0], dc->fmt, dc->d_pre, st, o->T, 0);
+    } else {
+        launch_gather(samples_dev, dc->act[0], nullptr, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, dc->act_cols[0],
+                      dc->fmt, dc->d_pre, st, o->T, s->S);
+    }
     prof_mark("gather", st);
     for (auto& g : dc->gemm) run_gemm(g, st);
     if (!dc->fused_tail) {

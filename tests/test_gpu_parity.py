@@ -485,3 +485,22 @@ def test_identity_scaling_is_bit_exact_and_offline_scaling_matches_oracle():
         rms_n = float(scaling[3][d]) * ref["pred"][d]
         util.check_network_output(n[d], ref["nhat"][d], f"offline scaled nhat det {d}", rms_ref=rms_n)
         util.check_network_output(c[d], ref["cleaned"][d], f"offline scaled cleaned det {d}", rms_ref=rms_n)
+
+
+@pytest.mark.gpu
+def test_offline_odd_stride_gather_path_matches_oracle():
+    """Odd stride: window starts do not fall on position pairs, so the offline first layer cannot read the
+    converted segment through the overlapping-window tensor map and every window is gathered instead."""
+    sp = S.StreamSpec(1, 1, 512, 120, 15)
+    layers = S.config_c0().dc_layers
+    params = [synth.deepclean_params(31, layers)]
+    B = 13
+    T = sp.window + (B - 1) * sp.stride
+    x = synth.stream_channels(32, sp, T, white=True)
+    off = gw.Offline(sp, layers, params, B, gw.GW_FP16)
+    c, n = off.run(_dev(x))
+    c, n = c.cpu().numpy(), n.cpu().numpy()
+    odc = [(layers, [oracle.prepare_conv(l, p, oracle.DT_FP16) for l, p in zip(layers, params[0])])]
+    ref = oracle.offline_clean(x, sp.window, sp.stride, [(sp.witness_rows(0), sp.strain_row(0))], odc)
+    util.check_network_output(n[0], ref["nhat"][0], "offline odd-stride nhat", rms_ref=ref["pred"][0])
+    util.check_network_output(c[0], ref["cleaned"][0], "offline odd-stride cleaned", rms_ref=ref["pred"][0])
