@@ -504,3 +504,65 @@ def test_offline_odd_stride_gather_path_matches_oracle():
     ref = oracle.offline_clean(x, sp.window, sp.stride, [(sp.witness_rows(0), sp.strain_row(0))], odc)
     util.check_network_output(n[0], ref["nhat"][0], "offline odd-stride nhat", rms_ref=ref["pred"][0])
     util.check_network_output(c[0], ref["cleaned"][0], "offline odd-stride cleaned", rms_ref=ref["pred"][0])
+
+
+# ------------------------------------------------------------------ C2 at full size, edge cases
+@pytest.mark.gpu
+def test_c2_full_batch_sampled_windows_match_oracle():
+    """BASELINE.json configs[2]: 256 windows x 2 detectors x 4096 samples, bf16.  The oracle scores sampled windows;
+    a property covers the rest: a window's score does not depend on its position in the batch (bit-exact)."""
+    cfg = S.config_c2()
+    L, batch = 4096, 256
+    cp, dp = util.centred_bbh_params(202, cfg.bbh_convs, cfg.bbh_dense, L)
+    bbh = gw.Bbh(None, cfg.bbh_convs, cp, dp, L, gw.GW_BF16, n_det=2, max_batch=batch)
+    x = synth.bbh_windows(2, batch, L)
+    got = bbh.score_batch(_dev(x)).cpu().numpy()
+    pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    for i in (0, 1, 2, 3, 77, 128, 129, 200, 254, 255):
+        ref = oracle.bbh_forward(x[i], cfg.bbh_convs, pc, pd)
+        assert abs(float(got[i]) - ref) <= util.SCORE_ABS, (i, float(got[i]), ref)
+    perm = np.random.default_rng(0).permutation(batch)
+    got_p = bbh.score_batch(_dev(x[perm])).cpu().numpy()
+    assert np.array_equal(got_p, got[perm])
+    with pytest.raises(gw.GwError):
+        bbh.score_batch(_dev(x[:0]))                    # empty batch: GW_EINVAL, nothing launched
+    one = bbh.score_batch(_dev(x[5:6])).cpu().numpy()   # batch of one
+    assert one[0] == got[5]
+
+
+@pytest.mark.gpu
+def test_degenerate_shapes():
+    """Stride = window (no overlap: LAST_STRIDE keeps the whole prediction), a single offline window (the estimate
+    is the prediction itself wherever the Hann weight is positive), and a single stream / single detector."""
+    layers = S.config_c0().dc_layers
+    params = [synth.deepclean_params(61, layers)]
+    od = [(layers, [oracle.prepare_conv(l, p, oracle.DT_FP16) for l, p in zip(layers, params[0])])]
+    # stride == window
+    sp = S.StreamSpec(1, 1, 512, 128, 128)
+    cfg = S.Config("k1", sp, layers, seed=8)
+    n_up = 4
+    x = synth.multi_stream(8, sp, n_up * sp.stride, white=True)
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, params, None, gw.GW_FP16, S.AGG_LAST_STRIDE, 0)
+    orc = oracle.StreamOracle(sp.channels, sp.window, sp.stride, [(sp.witness_rows(0), sp.strain_row(0))], od, None,
+                              agg=oracle.AGG_LAST_STRIDE, max_updates=n_up)
+    xd = _dev(x)
+    for t in range(n_up):
+        stream.update(xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous())
+        dc.forward()
+        fin = dc.cleaned(gw.GW_FINAL).cpu().numpy()[0, 0]
+        ref = orc.update(x[0][:, t * sp.stride:(t + 1) * sp.stride])
+        util.check_network_output(fin, ref["cleaned_final"][0], f"k=1 final update {t}", rms_ref=ref["pred"][0])
+    with pytest.raises(gw.GwError):                     # Hann overlap-add needs at least two windows over a sample
+        gw.build_ensemble(cfg, params, None, gw.GW_FP16, S.AGG_HANN_OLA, 0)
+    # one offline window
+    sp1 = S.StreamSpec(1, 1, 512, 128, 64)
+    x1 = synth.stream_channels(9, sp1, sp1.window, white=True)
+    off = gw.Offline(sp1, layers, params, 1, gw.GW_FP16)
+    c, n = off.run(_dev(x1))
+    p = off.predictions().cpu().numpy()[0, 0]
+    n = n.cpu().numpy()[0]
+    assert n[0] == 0.0
+    assert np.allclose(n[1:], p[1:], rtol=2e-6, atol=1e-7)      # w p / w, one rounding each way
+    ref = oracle.offline_clean(x1, sp1.window, sp1.stride, [(sp1.witness_rows(0), sp1.strain_row(0))], od)
+    util.check_network_output(c.cpu().numpy()[0], ref["cleaned"][0], "single offline window", rms_ref=ref["pred"][0])
