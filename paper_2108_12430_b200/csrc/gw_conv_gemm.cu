@@ -13,13 +13,16 @@
 // tensor dimension, so a slab never bleeds into the neighbouring window) and every tap's MMA reads it
 // through a shared-memory descriptor whose start address is advanced by whole 128-byte rows.
 //
-// The kernel is persistent and warp-specialised (320 threads, one CTA per SM):
-//   warp 0    TMA producer: A slabs (ring of sa_stages), B K-blocks (resident once, or a ring of sb_stages)
-//   warp 1    MMA issuer (one thread): tcgen05.mma into one of TWO TMEM accumulator stages
-//   warps 2-9 epilogue: TMEM -> registers -> bias / activation / pool / head -> 16-bit global, overlapping
-//             the next stage's MMAs
+// k_conv_gemm_umma is persistent and warp-specialised (352 threads, one CTA per SM):
+//   warp 0     TMA producer: A slabs (ring of sa_stages), B K-blocks (resident once, or a ring of sb_stages)
+//   warp 1     MMA issuer (one elected lane, predicated issue on the uniform datapath): tcgen05.mma into one of
+//              TWO TMEM accumulator stages; in EPI_FINAL also the second chain (the network's last layer)
+//   warp 10    second MMA issuer for stages that hold several tiles (odd tiles; its own A-slab sub-ring)
+//   warps 2-9  epilogue: TMEM -> registers -> bias / activation / pool / head -> swizzled shared-memory staging ->
+//              TMA store, overlapping the next stage's MMAs
 // CTA c serves detector c % n_det (each detector has its own weights) and walks that detector's tiles
-// with stride gridDim.x / n_det.
+// with stride gridDim.x / n_det.  k_conv_gemm_2sm (further down) is the CTA-pair variant for N = 256.
+// Kernels of a step are chained with programmatic dependent launch (griddepcontrol).
 #include <stdio.h>
 
 #include "gw_common.cuh"
