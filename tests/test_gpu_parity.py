@@ -566,3 +566,37 @@ def test_degenerate_shapes():
     assert np.allclose(n[1:], p[1:], rtol=2e-6, atol=1e-7)      # w p / w, one rounding each way
     ref = oracle.offline_clean(x1, sp1.window, sp1.stride, [(sp1.witness_rows(0), sp1.strain_row(0))], od)
     util.check_network_output(c.cpu().numpy()[0], ref["cleaned"][0], "single offline window", rms_ref=ref["pred"][0])
+
+
+@pytest.mark.gpu
+def test_c0_against_the_stored_oracle_values():
+    """The CUDA path against tests/golden/c0_oracle.txt (values written by the oracle alone, BASELINE.json
+    configs[0], fp16): the same bars as the live comparison, on numbers that cannot drift with the code under test."""
+    import os
+    recs = []
+    for line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "c0_oracle.txt")):
+        if not line.startswith("#") and line.strip():
+            k, t, i, v = line.split()
+            recs.append((k, int(t), int(i), float(v)))
+    cfg = S.config_c0()
+    sp = cfg.stream
+    params = [synth.deepclean_params(cfg.seed * 100, cfg.dc_layers)]
+    x = synth.multi_stream(cfg.seed, sp, cfg.n_updates * sp.stride, white=True)
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, params, None, gw.GW_FP16)
+    xd = _dev(x)
+    got = {}
+    rms = {}
+    for t in range(cfg.n_updates):
+        stream.update(xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous())
+        dc.forward()
+        pred = dc.noise().cpu().numpy()[0, 0]
+        running = dc.cleaned(gw.GW_RUNNING).cpu().numpy()[0, 0]
+        rms[t] = float(np.sqrt(np.mean(pred.astype(np.float64) ** 2)))
+        got[("pred", t)] = pred
+        got[("cleaned_running", t)] = running
+    checked = 0
+    for k, t, i, v in recs:
+        if (k, t) in got:
+            assert abs(float(got[(k, t)][i]) - v) <= util.ELEM_RMS * rms[t], (k, t, i, float(got[(k, t)][i]), v)
+            checked += 1
+    assert checked >= 40

@@ -5,6 +5,7 @@ are images), so no paper-printed values exist to pin to -- 
 CPU only: `-m "not gpu"`.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -597,3 +598,31 @@ def test_scaling_is_input_standardisation_and_affine_output():
         rc, re = c.update(x[:, sl]), e.update(x[:, sl])
         for key in ("pred", "nhat_final", "cleaned_final", "nhat_running", "cleaned_running"):
             assert np.array_equal(rc[key][0], re[key][0]), key
+
+
+# ---------------------------------------------------------------- stored oracle values (tests/golden)
+def _load_golden():
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "c0_oracle.txt")
+    recs = []
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        key, t, i, v = line.split()
+        recs.append((key, int(t), int(i), float(v)))
+    return recs
+
+
+def test_oracle_reproduces_the_stored_c0_values():
+    """tests/golden/c0_oracle.txt was written by tests/golden/make_golden.py from oracle/ alone (the paper prints no
+    values for this path).  The oracle must keep reproducing it: a change of its arithmetic has to show up here and
+    be justified against the paper."""
+    import importlib.util
+    spec = importlib.util.spec_from_file_location(
+        "make_golden", os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "make_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    now = {(k, t, i): v for k, t, i, v in mod.records()}
+    stored = _load_golden()
+    assert len(stored) == len(now) and len(stored) > 40
+    for k, t, i, v in stored:
+        assert abs(now[(k, t, i)] - v) <= 1e-13 * max(1.0, abs(v)), (k, t, i, now[(k, t, i)], v)
