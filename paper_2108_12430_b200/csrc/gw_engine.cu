@@ -1192,7 +1192,8 @@ static int pipeline_capture(gw_pipeline* p, const float* in, float* scores, floa
     cleaned_enqueue(p->dc, fin, nullptr, nullptr, st);
     if (p->bbh) {
         bbh_enqueue(p->bbh, p->bbh->in_buf, p->bbh->batch, st);
-        cudaMemcpyAsync(scores, p->bbh->scores_buf, static_cast<size_t>(p->bbh->batch) * 4, cudaMemcpyDeviceToDevice, st);
+        // cudaMemcpyDefault: `scores` may be the device alias of a pinned host buffer (gw_step_host_async)
+        cudaMemcpyAsync(scores, p->bbh->scores_buf, static_cast<size_t>(p->bbh->batch) * 4, cudaMemcpyDefault, st);
     }
     cudaError_t e = cudaStreamEndCapture(st, &p->graph);
     p->nodes = static_cast<int>(g_kernel_launches - before);
@@ -1338,10 +1339,22 @@ extern "C" int gw_step_host_async(gw_pipeline* p, const float* new_samples_host,
     CU_TRY(cudaMemcpyAsync(p->d_in2[b], new_samples_host, in_bytes, cudaMemcpyHostToDevice, p->copy_stream));
     CU_TRY(cudaEventRecord(p->in_done[b], p->copy_stream));
     CU_TRY(cudaStreamWaitEvent(st, p->in_done[b], 0));
-    if (int rc = gw_step(p, p->d_in2[b], p->d_scores, p->d_final, stream)) return rc;
-    CU_TRY(cudaEventRecord(p->in_free[b], st));
-    CU_TRY(cudaMemcpyAsync(cleaned_final_host, p->d_final, fin_bytes, cudaMemcpyDeviceToHost, st));
-    if (p->bbh) CU_TRY(cudaMemcpyAsync(scores_host, p->d_scores, sc_bytes, cudaMemcpyDeviceToHost, st));
+    // Pinned (mapped) host output buffers are written by the kernels themselves -- 0.5 MB of posted PCIe writes from
+    // the overlap-add kernel and n scores from the classifier head -- instead of by two copies behind the graph.
+    void *fin_alias = nullptr, *sc_alias = nullptr;
+    const bool direct = cudaHostGetDevicePointer(&fin_alias, cleaned_final_host, 0) == cudaSuccess &&
+                        (!p->bbh || cudaHostGetDevicePointer(&sc_alias, scores_host, 0) == cudaSuccess);
+    if (!direct) cudaGetLastError();             // pageable memory: clear the sticky-free error, use the copies
+    if (direct) {
+        if (int rc = gw_step(p, p->d_in2[b], p->bbh ? static_cast<float*>(sc_alias) : p->d_scores,
+                             static_cast<float*>(fin_alias), stream)) return rc;
+        CU_TRY(cudaEventRecord(p->in_free[b], st));
+    } else {
+        if (int rc = gw_step(p, p->d_in2[b], p->d_scores, p->d_final, stream)) return rc;
+        CU_TRY(cudaEventRecord(p->in_free[b], st));
+        CU_TRY(cudaMemcpyAsync(cleaned_final_host, p->d_final, fin_bytes, cudaMemcpyDeviceToHost, st));
+        if (p->bbh) CU_TRY(cudaMemcpyAsync(scores_host, p->d_scores, sc_bytes, cudaMemcpyDeviceToHost, st));
+    }
     p->async_calls += 1;
     return GW_OK;
 }
