@@ -310,6 +310,14 @@ class StreamOracle:
             cl = np.where(has, strain_all[np.clip(a, 0, self.T - 1)].astype(np.float64) - nh, cl)
         return nh, cl
 
+    def skip(self, new: np.ndarray) -> None:
+        """Append an update's samples WITHOUT computing it (tests that check a late block of a long stream: the
+        windows of later updates then hold the true history, while the overlap-add state lacks the skipped windows --
+        final values are valid again once W/S computed updates have passed, D7)."""
+        self.t += 1
+        assert (self.t + 1) * self.S <= self.T, "raise max_updates"
+        self.x[:, self.t * self.S:(self.t + 1) * self.S] = new
+
     def update(self, new: np.ndarray) -> Dict[str, np.ndarray]:
         """new [C][S] float32, strictly new samples.  Returns this update's results."""
         W, S = self.W, self.S

@@ -62,6 +62,7 @@ def _run_streaming(cfg, dtype, n_up, white, agg=S.AGG_HANN_OLA, delta=0, check_s
         new = xd[:, :, t * st_spec.stride:(t + 1) * st_spec.stride].contiguous()
         if use_graph:
             with torch.cuda.stream(cs):
+                cs.wait_stream(torch.cuda.current_stream())      # `new` was produced on torch's current stream
                 pipe.step(new, scores_d, final_d, cs)
             cs.synchronize()
             final = final_d.cpu().numpy()
@@ -310,6 +311,7 @@ def test_full_size_c4_sampled_streams_match_oracle(dtype):
     et = util.elem_tol(dtype)
     for t in range(n_up):
         new = xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous()
+        cs.wait_stream(torch.cuda.current_stream())
         pipe.step(new, scores_d, final_d, cs)
         cs.synchronize()
         pred = dc.noise().cpu().numpy()
@@ -347,7 +349,9 @@ def test_host_step_async_equals_device_step_bitwise():
             sc = torch.zeros(sp.n_streams, device="cuda")
             fin = torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda")
             for t in range(n_up):
-                pipe.step(xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous(), sc, fin, cs)
+                new = xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous()
+                cs.wait_stream(torch.cuda.current_stream())
+                pipe.step(new, sc, fin, cs)
                 cs.synchronize()
                 res.append((fin.cpu().numpy().copy(), sc.cpu().numpy().copy()))
         else:
@@ -600,3 +604,72 @@ def test_c0_against_the_stored_oracle_values():
             assert abs(float(got[(k, t)][i]) - v) <= util.ELEM_RMS * rms[t], (k, t, i, float(got[(k, t)][i]), v)
             checked += 1
     assert checked >= 40
+
+
+# ------------------------------------------------------- C1 and C3 at full size, long streams
+@pytest.mark.gpu
+def test_c1_full_rate_streaming_bf16_steady_state():
+    """BASELINE.json configs[1]: one stream, 21 witnesses, W = 32768, S = 1024 (k = 32), bf16, 40 updates: the first
+    updates (warm-up, partly-zero windows) and the 8 steady-state updates after all 32 overlapping windows exist."""
+    cfg = S.config_c1()
+    sp = cfg.stream
+    dtype = gw.GW_BF16
+    dc_params, _ = util.make_params(cfg)
+    n_up = 40
+    x = synth.multi_stream(cfg.seed, sp, n_up * sp.stride)
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, None, dtype)
+    orc = util.make_stream_oracle(cfg, dc_params, None, dtype, n_up)
+    xd = _dev(x)
+    et = util.elem_tol(dtype)
+    for t in range(n_up):
+        stream.update(xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous())
+        dc.forward()
+        pred = dc.noise().cpu().numpy()[0, 0]
+        final = dc.cleaned(gw.GW_FINAL).cpu().numpy()[0, 0]
+        ref = orc.update(x[0][:, t * sp.stride:(t + 1) * sp.stride])
+        if t < 3 or t >= 31:
+            util.check_network_output(pred, ref["pred"][0], f"C1 pred update {t}", elem=et)
+            util.check_network_output(final, ref["cleaned_final"][0], f"C1 final update {t}", rms_ref=ref["pred"][0], elem=et)
+
+
+@pytest.mark.gpu
+def test_c3_ten_minute_stream_first_and_late_blocks():
+    """BASELINE.json configs[3]: 2 detectors x 21 witnesses, W = 32768, S = 512 (k = 64), classifier on the last
+    second, 4800 updates = 10 min, through the CUDA graph.  Full chain (raw prediction, final cleaned samples, score)
+    against the oracle on the first 72 updates and on the last 72; the oracle skips the updates in between (its
+    overlap-add state is rebuilt over the 63 updates before the late block, which are computed but not compared)."""
+    cfg = S.config_c3(1)
+    sp = cfg.stream
+    dtype = gw.GW_FP16
+    k = sp.window // sp.stride
+    n_up, blk = 4800, 72
+    dc_params, bbh_params = util.make_params(cfg)
+    x = synth.multi_stream(cfg.seed, sp, n_up * sp.stride)
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype)
+    # [update][stream][channel][S], resident before the loop: every step's input is a contiguous view, no copies race
+    xc = torch.from_numpy(np.ascontiguousarray(x.reshape(1, sp.channels, n_up, sp.stride).transpose(2, 0, 1, 3))).cuda()
+    cs = torch.cuda.Stream()
+    scores_d = torch.zeros(1, device="cuda")
+    final_d = torch.zeros((1, sp.n_det, sp.stride), device="cuda")
+    torch.cuda.synchronize()
+    keep = {}
+    for t in range(n_up):
+        pipe.step(xc[t], scores_d, final_d, cs)
+        if t < blk or t >= n_up - blk:
+            cs.synchronize()
+            keep[t] = (dc.noise().cpu().numpy()[0], final_d.cpu().numpy()[0].copy(), float(scores_d.cpu()[0]))
+    cs.synchronize()
+    orc = util.make_stream_oracle(cfg, dc_params, bbh_params, dtype, n_up)
+    first_late = n_up - blk - (k - 1)
+    for t in range(n_up):
+        new = x[0][:, t * sp.stride:(t + 1) * sp.stride]
+        if blk <= t < first_late:
+            orc.skip(new)
+            continue
+        ref = orc.update(new)
+        if t in keep:
+            pred, final, score = keep[t]
+            for d in range(sp.n_det):
+                util.check_network_output(pred[d], ref["pred"][d], f"C3 pred update {t} det {d}")
+                util.check_network_output(final[d], ref["cleaned_final"][d], f"C3 final update {t} det {d}", rms_ref=ref["pred"][d])
+            assert abs(score - ref["score"]) <= util.SCORE_ABS, (t, score, ref["score"])
