@@ -324,6 +324,7 @@ def run_native(args):
     hbm_bytes = {
         "append": sp.n_streams * sp.channels * sp.stride * 8,                       # read new + write ring
         "ring16_append": sp.n_streams * nd * sp.stride * (nw * 4 + 2 * 32 * 2),     # read fp32, write both mirror copies
+        "snapshot_append": sp.n_streams * (sp.channels * sp.stride * 8 + nd * sp.stride * 2 * 32 * 2),  # a1 + a2 fused
         "aggregate": sp.n_streams * nd * sp.window * 20,                            # p_t, acc r/w, strain, cleaned
         "bbh_conv1": sp.n_streams * (nd * cfg.bbh_len * 4 + (cfg.bbh_len // 4) * 32 * 2),
     }

@@ -102,6 +102,10 @@ void launch_append(float* ring, const float* new_samples, long long* count, unsi
                    int W, int S, cudaStream_t st);
 bool is_append_kernel(const void* func);   // identifies the a1 node of a captured graph
 bool is_ring16_append_kernel(const void* func);
+bool is_snapshot_append_kernel(const void* func);   // the fused a1 + a2 kernel (src is argument 1)
+void launch_snapshot_append(float* ring, const float* new_samples, void* ring16, long long* count, unsigned* ticket,
+                            const int* rows_map, const float* pre, int n_streams, int channels, int n_det, int n_wit, int W,
+                            int S, int cpad, int fmt, cudaStream_t st);
 void launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st);
 void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
                           int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,

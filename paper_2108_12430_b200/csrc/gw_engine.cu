@@ -300,8 +300,9 @@ struct gw_pipeline {
     gw_bbh* bbh = nullptr;
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
-    cudaGraphNode_t append_node = nullptr;       // the two kernels that read the caller's new-sample buffer
+    cudaGraphNode_t append_node = nullptr;       // the kernels that read the caller's new-sample buffer
     cudaGraphNode_t ring16_node = nullptr;
+    bool append_fused = false;                   // append_node is k_snapshot_append (a1 + a2 in one kernel)
     int nodes = 0;
     const float* cap_in = nullptr;
     float* cap_scores = nullptr;
@@ -511,9 +512,16 @@ static int stream_update_checked(gw_stream* s) {
     return GW_OK;
 }
 static void stream_update_enqueue(gw_stream* s, const float* src, cudaStream_t st) {
+    gw_deepclean* dc = s->dc;
+    if (dc && dc->mirror && s->S % 4 == 0 && s->W % 4 == 0) {       // a1 + a2 in one launch
+        launch_snapshot_append(s->ring, src, dc->ring16, s->d_count, s->d_ticket, dc->d_rows_map, dc->d_pre, s->n, s->C,
+                               dc->n_det, dc->n_wit, s->W, s->S, dc->act_cols[0], dc->fmt, st);
+        prof_mark("snapshot_append", st);
+        return;
+    }
     launch_append(s->ring, src, s->d_count, s->d_ticket, s->n * s->C, s->W, s->S, st);
     prof_mark("append", st);
-    if (s->dc) ring16_append_enqueue(s->dc, src, st);
+    if (dc) ring16_append_enqueue(dc, src, st);
 }
 
 extern "C" int gw_stream_update(gw_stream* s, const float* new_samples_dev, void* stream) {
@@ -1214,7 +1222,8 @@ static int pipeline_capture(gw_pipeline* p, const float* in, float* scores, floa
         if (ty != cudaGraphNodeTypeKernel) continue;
         cudaKernelNodeParams kp;
         CU_TRY(cudaGraphKernelNodeGetParams(nd, &kp));
-        if (is_append_kernel(kp.func)) p->append_node = nd;
+        if (is_append_kernel(kp.func)) { p->append_node = nd; p->append_fused = false; }
+        if (is_snapshot_append_kernel(kp.func)) { p->append_node = nd; p->append_fused = true; }
         if (is_ring16_append_kernel(kp.func)) p->ring16_node = nd;
     }
     return GW_OK;
@@ -1234,6 +1243,12 @@ static int set_node_src(gw_pipeline* p, cudaGraphNode_t node, int n_args, int sr
 
 static int pipeline_set_input(gw_pipeline* p, const float* in) {
     // k_append(ring, src, count, ticket, n_rows, W, S); k_ring16_append(src, ring16, count, rows_map, ... 12 args)
+    // k_snapshot_append(ring, src, ring16, count, ticket, rows_map, pre, ... 14 args)
+    if (p->append_fused) {
+        if (int rc = set_node_src(p, p->append_node, 14, 1, in)) return rc;
+        p->cap_in = in;
+        return GW_OK;
+    }
     if (int rc = set_node_src(p, p->append_node, 7, 1, in)) return rc;
     if (p->ring16_node)
         if (int rc = set_node_src(p, p->ring16_node, 12, 0, in)) return rc;

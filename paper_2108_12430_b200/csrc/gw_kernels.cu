@@ -239,6 +239,102 @@ __global__ void __launch_bounds__(256) k_ring16_append(const float* __restrict__
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// a1 + a2 in ONE launch (the usual case: S, W multiples of 4 and the mirror ring in use): block (tile of 128
+// new samples, stream x detector) converts its detector's witness samples into the mirror ring exactly as
+// k_ring16_append does, and appends the fp32 ring rows r = d, d + n_det, ... of its stream exactly as
+// k_append<4> does (every ring row of the stream has one owner).  Both parts use the OLD counter; the last
+// block advances it.  One read of the new samples from HBM, one launch instead of two (each was a ~11 us,
+// latency-bound kernel for 23-28 MB at n = 128).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_snapshot_append(float* __restrict__ ring, const float* __restrict__ src,
+                                                         void* __restrict__ ring16, long long* count, unsigned* ticket,
+                                                         const int* __restrict__ rows_map, const float* __restrict__ pre,
+                                                         int channels, int n_det, int n_wit, int W, int S, int cpad,
+                                                         int fmt) {
+    __shared__ float tile[32][kGatherPos + 1];
+    const long long cnt = *count;
+    const int h0 = static_cast<int>(cnt % W);              // ring slot of this update's first sample
+    const int sd = blockIdx.y;
+    const int s = sd / n_det, d = sd % n_det;
+    const int i0 = blockIdx.x * kGatherPos;
+    const int tid = threadIdx.x;
+    // fp32 ring rows owned by this block: 32 float4 per row and tile
+    {
+        const int n_mine = (channels - d + n_det - 1) / n_det;
+        for (int idx = tid; idx < n_mine * 32; idx += 256) {
+            const int row = s * channels + d + (idx >> 5) * n_det;
+            const int i = i0 + (idx & 31) * 4;
+            if (i < S) {
+                int slot = h0 + i;
+                if (slot >= W) slot -= W;
+                *reinterpret_cast<float4*>(ring + static_cast<size_t>(row) * W + slot) =
+                    __ldg(reinterpret_cast<const float4*>(src + static_cast<size_t>(row) * S + i));
+            }
+        }
+    }
+    // 16-bit mirror ring, 32 channels at a time through the transpose tile
+    for (int cb = 0; cb < cpad; cb += 32) {
+        __syncthreads();
+        {
+            const int pos = tid % kGatherPos;
+            const int cg = tid / kGatherPos;
+            const int i = i0 + pos;
+#pragma unroll 4
+            for (int k = 0; k < 16; ++k) {
+                const int c = cb + cg * 16 + k;
+                float v = 0.f;
+                if (c < n_wit && i < S) {
+                    const int row = s * channels + __ldg(rows_map + d * n_wit + c);
+                    const float2 ms = __ldg(reinterpret_cast<const float2*>(pre) + d * n_wit + c);   // (mean, 1/std)
+                    v = (__ldg(src + static_cast<size_t>(row) * S + i) - ms.x) * ms.y;
+                }
+                tile[cg * 16 + k][pos] = v;
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const int pos = it * 64 + tid / 4;
+            const int c0 = (tid % 4) * 8;
+            const int i = i0 + pos;
+            if (i < S) {
+                uint4 q;
+                q.x = pack16(tile[c0 + 0][pos], tile[c0 + 1][pos], fmt);
+                q.y = pack16(tile[c0 + 2][pos], tile[c0 + 3][pos], fmt);
+                q.z = pack16(tile[c0 + 4][pos], tile[c0 + 5][pos], fmt);
+                q.w = pack16(tile[c0 + 6][pos], tile[c0 + 7][pos], fmt);
+                int slot = h0 + i;
+                if (slot >= W) slot -= W;
+                uint16_t* dst = reinterpret_cast<uint16_t*>(ring16) + (static_cast<size_t>(sd) * 2 * W + slot) * cpad + cb + c0;
+                *reinterpret_cast<uint4*>(dst) = q;
+                *reinterpret_cast<uint4*>(dst + static_cast<size_t>(W) * cpad) = q;
+            }
+        }
+    }
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) {
+        const unsigned t = atomicAdd(ticket, 1u);
+        if (t == gridDim.x * gridDim.y - 1) {
+            *count = cnt + S;
+            *ticket = 0;
+            __threadfence();
+        }
+    }
+}
+
+bool is_snapshot_append_kernel(const void* func) { return func == reinterpret_cast<const void*>(&k_snapshot_append); }
+
+void launch_snapshot_append(float* ring, const float* new_samples, void* ring16, long long* count, unsigned* ticket,
+                            const int* rows_map, const float* pre, int n_streams, int channels, int n_det, int n_wit, int W,
+                            int S, int cpad, int fmt, cudaStream_t st) {
+    dim3 grid((S + kGatherPos - 1) / kGatherPos, n_streams * n_det);
+    k_snapshot_append<<<grid, 256, 0, st>>>(ring, new_samples, ring16, count, ticket, rows_map, pre, channels, n_det, n_wit, W,
+                                            S, cpad, fmt);
+    ++g_kernel_launches;
+}
+
 bool is_ring16_append_kernel(const void* func) { return func == reinterpret_cast<const void*>(&k_ring16_append); }
 
 void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,

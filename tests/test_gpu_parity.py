@@ -77,8 +77,11 @@ def _run_streaming(cfg, dtype, n_up, white, agg=S.AGG_HANN_OLA, delta=0, check_s
             nhat = dc.noise_estimate().cpu().numpy()
             scores = bbh.score().cpu().numpy() if bbh is not None else None
             final = None
+        snap, first = stream.snapshot()                  # a1 with the DeepClean stage attached (fused a1 + a2 kernel)
+        snap = snap.cpu().numpy()
         for i, orc in enumerate(oracles):
             ref = orc.update(x[i][:, t * st_spec.stride:(t + 1) * st_spec.stride])
+            assert first == ref["first_index"] and np.array_equal(snap[i], ref["snapshot"]), ("snapshot", t, i)
             for d in range(st_spec.n_det):
                 tag = f"update {t} stream {i} det {d}"
                 _, w1 = util.check_network_output(pred[i, d], ref["pred"][d], "pred " + tag, elem=et)
