@@ -129,6 +129,13 @@ int gw_set_pdl(int on);
  * last, which are still in L2.  Pure scheduling; results are bit-identical either way. */
 int gw_set_snake(int on);
 
+/* Diagnostic: measured cycles per tcgen05.mma (cta_group::1, kind::f16, M = 128, K = 16, both operands in shared
+ * memory, SWIZZLE_128B) for GEMM N in {16, 32, 64, 128, 256} on the current device: one CTA issues 1024 MMAs back to
+ * back with a conv layer's descriptor pattern.  *issue_cycles = issue-loop time per MMA, *complete_cycles = time
+ * until the last one has retired, per MMA (host pointers).  Synchronises the device.  This is the number behind the
+ * shared-memory-operand roofline of the thin layers. */
+int gw_probe_mma_cycles(int N, float *issue_cycles, float *complete_cycles);
+
 /* CTA-pair conv GEMM (tcgen05 cta_group::2: two CTAs of a cluster share every streamed weight block, M = 256)
  * for the layers whose weights do not fit in shared memory (GEMM N = 256), for handles created AFTER this call
  * (default 1).  With 0 those layers run the single-CTA kernel.  The accumulation order of every output is the

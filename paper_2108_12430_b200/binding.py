@@ -21,7 +21,7 @@ GW_FINAL, GW_RUNNING = 0, 1
 GW_IMPL_UMMA, GW_IMPL_SIMT = 0, 1
 
 EXPORTS = [
-    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake", "gw_set_two_sm",
+    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake", "gw_probe_mma_cycles", "gw_set_two_sm",
     "gw_stream_create", "gw_stream_destroy", "gw_stream_update", "gw_stream_snapshot", "gw_stream_count",
     "gw_deepclean_create", "gw_deepclean_destroy", "gw_deepclean_forward", "gw_deepclean_noise",
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
@@ -77,6 +77,7 @@ def lib():
         L.gw_set_fuse_tail.argtypes = [i]
         L.gw_set_pdl.argtypes = [i]
         L.gw_set_snake.argtypes = [i]
+        L.gw_probe_mma_cycles.argtypes = [i, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.gw_set_two_sm.argtypes = [i]
         L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
         L.gw_stream_destroy.argtypes = [vp]
@@ -149,6 +150,25 @@ def set_snake(on: bool) -> None:
 def set_two_sm(on: bool) -> None:
     """CTA-pair (cta_group::2) kernel for the N = 256 conv GEMM layers (default on)."""
     _check(lib().gw_set_two_sm(1 if on else 0))
+
+
+def probe_mma_cycles(n_values=(16, 32, 64, 128, 256)):
+    """Diagnostic: {N: (issue cycles, completion cycles) per tcgen05.mma} measured on the current device.
+
+        python -c "from paper_2108_12430_b200 import binding as gw; gw.print_mma_probe()"
+    """
+    out = {}
+    for n in n_values:
+        a, b = C.c_float(0), C.c_float(0)
+        _check(lib().gw_probe_mma_cycles(int(n), C.byref(a), C.byref(b)))
+        out[int(n)] = (float(a.value), float(b.value))
+    return out
+
+
+def print_mma_probe() -> None:
+    for n, (issue, done) in probe_mma_cycles().items():
+        print(f"N={n:3d}: issue {issue:6.1f} clk/MMA, complete {done:6.1f} clk/MMA  (math floor {n // 2}, shared-memory "
+              f"operand read 32 + N/4 = {32 + n // 4})")
 
 
 def _fp(a: Optional[np.ndarray]):

@@ -95,6 +95,7 @@ void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st);
 void launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st);
 // Chooses resident/streaming B, ring depths and the shared-memory size for a layer; false if it cannot fit.
 bool conv_gemm_plan(GemmLaunch& g, int sm_count);
+cudaError_t probe_mma_cycles(int N, float* issue, float* complete);   // diagnostic: cycles per tcgen05.mma, N in {16..256}
 cudaError_t conv_gemm_prepare();   // opt-in shared-memory attribute
 
 // ---- bandwidth / CUDA-core kernels (gw_kernels.cu) -------------------------------------------

@@ -930,6 +930,88 @@ static Gemm2Kernel pick_kernel_2sm(int act, int fmt) {
     return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_NONE, FMT_BF16> : k_conv_gemm_2sm<ACT_NONE, FMT_FP16>;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Diagnostic (gw_probe_mma_cycles): cycles per tcgen05.mma.cta_group::1.kind::f16 (M = 128, K = 16, both operands in
+// shared memory, SWIZZLE_128B K-major) as a function of N, issued back to back by one warp of one CTA with the
+// descriptor pattern of a conv layer (four row shifts x four K steps).  This is the measurement behind the
+// shared-memory-operand roofline of DESIGN.md section 7: cycles = max(N/2, 32 + N/4).
+// ---------------------------------------------------------------------------------------------
+template <int N>
+__global__ void __launch_bounds__(128, 1) k_probe_mma(long long* out, int reps) {
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    __shared__ uint64_t bar;
+    __shared__ uint32_t slot;
+    const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
+    for (int i = threadIdx.x; i < 176 * 1024 / 4; i += 128) reinterpret_cast<uint32_t*>(smem)[i] = 0;
+    if (warp == 0) {
+        if (lane == 0) { mbar_init(&bar, 1); fence_barrier_init(); }
+        __syncwarp();
+        tmem_alloc(&slot, 512);
+    }
+    fence_proxy_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = slot;
+    if (warp == 1) {
+        const uint32_t idesc = umma_idesc_f16(FMT_FP16, kTileM, N);
+        const uint32_t a_lo = umma_desc_lo(smem_u32(smem));             // a slab of 131 rows
+        const uint32_t b_lo = umma_desc_lo(smem_u32(smem + 32768));     // four K blocks of N rows
+        const uint32_t leader = elect_one() ? 1u : 0u;
+        const long long t0 = clock64();
+        for (int r = 0; r < reps; ++r) {
+#pragma unroll
+            for (int sh = 0; sh < 4; ++sh)
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    umma_f16_if(leader, tmem + (r & 1) * 256, umma_desc_make(a_lo + 8u * sh + 2 * k),
+                                umma_desc_make(b_lo + static_cast<uint32_t>(sh * N * 128 >> 4) + 2 * k), idesc, 1u);
+        }
+        const long long t1 = clock64();
+        umma_commit_if(leader, &bar);
+        mbar_wait(&bar, 0);
+        const long long t2 = clock64();
+        if (lane == 0) { out[0] = t1 - t0; out[1] = t2 - t0; }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, 512);
+}
+
+template <int N>
+static cudaError_t probe_one(long long* d_out, int reps, float* issue, float* complete) {
+    cudaError_t e = cudaFuncSetAttribute(k_probe_mma<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 180 * 1024);
+    if (e != cudaSuccess) return e;
+    long long h[2] = {0, 0};
+    for (int it = 0; it < 2; ++it) {                       // second run: instruction cache and clocks warm
+        k_probe_mma<N><<<1, 128, 180 * 1024>>>(d_out, reps);
+        e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) return e;
+    }
+    e = cudaMemcpy(h, d_out, sizeof h, cudaMemcpyDeviceToHost);
+    *issue = static_cast<float>(h[0]) / (reps * 16.0f);
+    *complete = static_cast<float>(h[1]) / (reps * 16.0f);
+    return e;
+}
+
+cudaError_t probe_mma_cycles(int N, float* issue, float* complete) {
+    long long* d_out = nullptr;
+    cudaError_t e = cudaMalloc(&d_out, 16);
+    if (e != cudaSuccess) return e;
+    const int reps = 64;
+    switch (N) {
+        case 16: e = probe_one<16>(d_out, reps, issue, complete); break;
+        case 32: e = probe_one<32>(d_out, reps, issue, complete); break;
+        case 64: e = probe_one<64>(d_out, reps, issue, complete); break;
+        case 128: e = probe_one<128>(d_out, reps, issue, complete); break;
+        case 256: e = probe_one<256>(d_out, reps, issue, complete); break;
+        default: e = cudaErrorInvalidValue;
+    }
+    cudaFree(d_out);
+    return e;
+}
+
 typedef void (*GemmKernel)(const ConvGemmParams, int);
 
 static GemmKernel pick_kernel(int epi, int act, int fmt) {

@@ -74,6 +74,14 @@ static int check_device() {
     return GW_OK;
 }
 
+extern "C" int gw_probe_mma_cycles(int N, float* issue_cycles, float* complete_cycles) {
+    if (!issue_cycles || !complete_cycles) return fail(GW_EINVAL, "gw_probe_mma_cycles: NULL argument");
+    if (N != 16 && N != 32 && N != 64 && N != 128 && N != 256) return fail(GW_EINVAL, "gw_probe_mma_cycles: N must be 16, 32, 64, 128 or 256");
+    if (int rc = check_device()) return rc;
+    CU_TRY(probe_mma_cycles(N, issue_cycles, complete_cycles));
+    return GW_OK;
+}
+
 // ------------------------------------------------------------------------- TMA descriptor encode
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,

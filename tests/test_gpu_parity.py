@@ -676,3 +676,15 @@ def test_c3_ten_minute_stream_first_and_late_blocks():
                 util.check_network_output(pred[d], ref["pred"][d], f"C3 pred update {t} det {d}")
                 util.check_network_output(final[d], ref["cleaned_final"][d], f"C3 final update {t} det {d}", rms_ref=ref["pred"][d])
             assert abs(score - ref["score"]) <= util.SCORE_ABS, (t, score, ref["score"])
+
+
+@pytest.mark.gpu
+def test_mma_probe_reports_the_operand_read_law():
+    """gw_probe_mma_cycles: the measured cycles per tcgen05.mma follow max(N/2, 32 + N/4) within 15 % on this class of
+    device (the thin layers' shared-memory roofline in DESIGN.md rests on it); bad N is rejected."""
+    got = gw.probe_mma_cycles()
+    for n, (issue, done) in got.items():
+        law = max(n / 2, 32 + n / 4)
+        assert 0.85 * law <= done <= 1.15 * law, (n, issue, done, law)
+    with pytest.raises(gw.GwError):
+        gw.probe_mma_cycles((48,))
