@@ -347,13 +347,15 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 tc_fence_after();
                 const uint32_t d_fin = tmem_base + accp * kAccCols + kFinCol + h * kFinN;
                 const uint32_t a_t = stg_lo + static_cast<uint32_t>((accp * 2 + h) * kFinTile >> 4);
+                // shift 0 (row m-1) reaches the outputs only through its odd position (columns 32..63: K steps 2, 3):
+                // tap j = r + 3 + 4 - 2 par is valid for par = 1 alone, so K steps 0, 1 of that block are all zero
 #pragma unroll
                 for (int sh = 0; sh < 3; ++sh)
 #pragma unroll
-                    for (int k = 0; k < kSegK / 16; ++k)
+                    for (int k = (sh == 0 ? 2 : 0); k < kSegK / 16; ++k)
                         umma_f16_if(leader, d_fin, umma_desc_make(a_t + 8u * sh + 2 * k),
                                     umma_desc_make(fin_lo + static_cast<uint32_t>(sh * kFinBlock >> 4) + 2 * k), idesc_fin,
-                                    (sh | k) ? 1u : 0u);
+                                    (sh == 0 && k == 2) ? 0u : 1u);
                 umma_commit_if(leader, &fin_full[accp * 2 + h]);
             }
         };
