@@ -214,8 +214,9 @@ int gw_step_host(gw_pipeline *p, const float *new_samples_host, float *scores_ho
                  float *cleaned_final_host, void *stream);
 /* gw_step_host_async: the throughput form of gw_step_host (offline regime).  Same arguments; does
  * NOT synchronise.  The host->device copy of this call's samples runs on an internal copy stream into one of two
- * staging buffers and overlaps the previous step's kernels; scores and final cleaned samples are copied back in
- * stream order on `stream`.  Every host buffer passed to a call must stay valid (and, for the outputs, unread)
+ * staging buffers and overlaps the previous step's kernels; scores and final cleaned samples reach the host
+ * buffers in stream order on `stream` (pinned, mapped buffers are written by the kernels themselves; pageable ones
+ * through copies).  Every host buffer passed to a call must stay valid (and, for the outputs, unread)
  * until `stream` has been synchronised past that call.  Use pinned host memory. */
 int gw_step_host_async(gw_pipeline *p, const float *new_samples_host, float *scores_host,
                        float *cleaned_final_host, void *stream);
