@@ -688,3 +688,44 @@ def test_mma_probe_reports_the_operand_read_law():
         assert 0.85 * law <= done <= 1.15 * law, (n, issue, done, law)
     with pytest.raises(gw.GwError):
         gw.probe_mma_cycles((48,))
+
+
+@pytest.mark.gpu
+def test_handles_release_their_device_memory():
+    """Create / run / destroy every kind of handle a few times: free device memory returns to where it started
+    (the engine owns all persistent state, include/gwstream.h)."""
+    import gc
+    cfg = S.config_small_ensemble(2)
+    sp = cfg.stream
+    dc_params, bbh_params = util.make_params(cfg)
+    x = _dev(synth.multi_stream(cfg.seed, sp, 2 * sp.stride))
+    one = S.StreamSpec(1, sp.n_det, sp.fs, sp.window, sp.stride, sp.n_witness)
+    seg = _dev(synth.stream_channels(1, one, sp.window + 3 * sp.stride))
+    scores_h = torch.zeros(sp.n_streams).pin_memory()
+    final_h = torch.zeros((sp.n_streams, sp.n_det, sp.stride)).pin_memory()
+    xin = torch.from_numpy(np.ascontiguousarray(x[:, :, :sp.stride].cpu().numpy())).pin_memory()
+
+    def cycle():
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, gw.GW_FP16)
+        cs = torch.cuda.Stream()
+        sc = torch.zeros(sp.n_streams, device="cuda")
+        fin = torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda")
+        cs.wait_stream(torch.cuda.current_stream())
+        pipe.step(x[:, :, :sp.stride].contiguous(), sc, fin, cs)
+        pipe.step_host_async(xin, scores_h, final_h, cs)
+        cs.synchronize()
+        off = gw.Offline(one, cfg.dc_layers, dc_params, 4, gw.GW_FP16)
+        off.run(seg)
+        torch.cuda.synchronize()
+        for h in (pipe, bbh, dc, stream, off):
+            h.__del__()
+        del sc, fin
+
+    cycle()                                              # first cycle: CUDA module load, allocator pools
+    gc.collect(); torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(3):
+        cycle()
+    gc.collect(); torch.cuda.synchronize(); torch.cuda.empty_cache()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 < 8 * 2**20, (free0, free1)
