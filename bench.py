@@ -194,6 +194,8 @@ def run_native(args):
         gw.set_pdl(False)
     if args.no_snake:
         gw.set_snake(False)
+    if args.no_skip:
+        gw.set_skip_zeros(False)
     if args.no_2sm:
         gw.set_two_sm(False)
     dtype = gw.GW_BF16 if args.dtype == "bf16" else gw.GW_FP16
@@ -427,6 +429,7 @@ def main():
                                                     "point appended to FILE (JSON lines); prints a table to stderr")
     ap.add_argument("--no-2sm", action="store_true", help="single-CTA kernel for the N=256 layers too (A/B aid)")
     ap.add_argument("--no-offline", action="store_true", help="skip the offline-mode measurement")
+    ap.add_argument("--no-skip", action="store_true", help="issue the structurally empty MMAs too (A/B aid)")
     ap.add_argument("--timed-only", action="store_true",
                     help="only the warm-up and the timed region (for short runs under ncu); prints a reduced line")
     ap.add_argument("--reference-budget", type=float, default=150.0,

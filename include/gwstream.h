@@ -129,6 +129,11 @@ int gw_set_pdl(int on);
  * last, which are still in L2.  Pure scheduling; results are bit-identical either way. */
 int gw_set_snake(int on);
 
+/* Skip the structurally empty parts of the resident-weight conv GEMMs (K steps and halves of N that no filter tap
+ * reaches; such weight blocks are also kept at half size in shared memory), for handles created AFTER this call
+ * (default 1).  Only exact zeros are skipped: results are bit-identical. */
+int gw_set_skip_zeros(int on);
+
 /* Diagnostic: measured cycles per tcgen05.mma (cta_group::1, kind::f16, M = 128, K = 16, both operands in shared
  * memory, SWIZZLE_128B) for GEMM N in {16, 32, 64, 128, 256} on the current device: one CTA issues 1024 MMAs back to
  * back with a conv layer's descriptor pattern.  *issue_cycles = issue-loop time per MMA, *complete_cycles = time

@@ -21,7 +21,7 @@ GW_FINAL, GW_RUNNING = 0, 1
 GW_IMPL_UMMA, GW_IMPL_SIMT = 0, 1
 
 EXPORTS = [
-    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake", "gw_probe_mma_cycles", "gw_set_two_sm",
+    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake", "gw_set_skip_zeros", "gw_probe_mma_cycles", "gw_set_two_sm",
     "gw_stream_create", "gw_stream_destroy", "gw_stream_update", "gw_stream_snapshot", "gw_stream_count",
     "gw_deepclean_create", "gw_deepclean_destroy", "gw_deepclean_forward", "gw_deepclean_noise",
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
@@ -77,6 +77,7 @@ def lib():
         L.gw_set_fuse_tail.argtypes = [i]
         L.gw_set_pdl.argtypes = [i]
         L.gw_set_snake.argtypes = [i]
+        L.gw_set_skip_zeros.argtypes = [i]
         L.gw_probe_mma_cycles.argtypes = [i, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.gw_set_two_sm.argtypes = [i]
         L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
@@ -150,6 +151,11 @@ def set_snake(on: bool) -> None:
 def set_two_sm(on: bool) -> None:
     """CTA-pair (cta_group::2) kernel for the N = 256 conv GEMM layers (default on)."""
     _check(lib().gw_set_two_sm(1 if on else 0))
+
+
+def set_skip_zeros(on: bool) -> None:
+    """Skip structurally empty K steps / halves of N in the resident-weight conv GEMMs (default on)."""
+    _check(lib().gw_set_skip_zeros(1 if on else 0))
 
 
 def probe_mma_cycles(n_values=(16, 32, 64, 128, 256)):

@@ -79,6 +79,15 @@ struct ConvGemmParams {
 #ifdef GW_TRACE
     long long* trace;              // [grid][16] cycle counters of the roles (diagnostic builds only)
 #endif
+    // Structural zeros of the resident-weight path, one bit per (cb, shift) at position cb * kMaxShift + shift:
+    // mask_k2: K steps 0 and 1 of the segment hold no weight (a stride-2 Conv1d's outermost shift reaches one
+    //          position parity only) -> two MMAs instead of four;
+    // mask_nu: only the UPPER half of N holds weights (a ConvTranspose1d's outermost shift feeds odd outputs only)
+    //          -> MMAs of N/2 into the upper half of the accumulator, and the block is stored at half size.
+    // Skipped products are exact zeros: results do not change.  b_res_bytes = size of the resident weight image.
+    unsigned long long mask_k2, mask_nu;
+    int b_res_bytes;
+    CUtensorMap tmBh;              // the upper-half weight blocks: box (64, N/2, 1)
     int8_t seg_of[kMaxCb][kMaxShift];     // B K-block of segment (cb, shift), -1 if the segment is empty
     int8_t seg_shift[kMaxSeg];     // per segment s: row shift, first column (SIMT kernel)
     int16_t seg_col[kMaxSeg];

@@ -86,15 +86,22 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     p.out_bufs = 0;
     if (p.epi == EPI_FINAL) p.out_bufs = 2;               // four activated tiles: [accumulator stage][tile in stage]
     if (p.epi == EPI_STORE) {
-        const int b_need = p.n_seg * b_block <= 132 * 1024 ? p.n_seg * b_block : 4 * b_block;
+        int nh = 0;
+        for (unsigned long long m = p.mask_nu; m; m &= m - 1) ++nh;
+        const int rb = p.n_seg * b_block - nh * (b_block / 2);
+        const int b_need = rb <= 132 * 1024 ? rb : 4 * b_block;
         p.out_bufs = (kFixedSmem + 2 * kOutStage + b_need + 4 * sl <= kSmemBudget) ? 2 : 1;
     }
     const int fixed = kFixedSmem + (p.epi == EPI_POOL_HEAD ? head_scratch_bytes(p.N, p.head_hidden) : 0) +
                       (p.epi == EPI_FINAL ? kFinalScratch : 0) + p.out_bufs * kOutStage;
     int b_bytes;
-    if (p.n_seg * b_block <= 132 * 1024 && fixed + p.n_seg * b_block + 2 * sl <= kSmemBudget) {
-        p.b_resident = 1; p.sb_stages = 0; b_bytes = p.n_seg * b_block;
+    int n_half = 0;
+    for (unsigned long long m = p.mask_nu; m; m &= m - 1) ++n_half;
+    const int res_bytes = p.n_seg * b_block - n_half * (b_block / 2);      // upper-half-only blocks are stored at half size
+    if (res_bytes <= 132 * 1024 && fixed + res_bytes + 2 * sl <= kSmemBudget) {
+        p.b_resident = 1; p.sb_stages = 0; b_bytes = res_bytes; p.b_res_bytes = res_bytes;
     } else {
+        p.mask_k2 = 0; p.mask_nu = 0;                                      // streamed weights: every block in full
         p.b_resident = 0;
         p.sb_stages = p.n_seg < 4 ? p.n_seg : 4;
         while (p.sb_stages > 1 && fixed + p.sb_stages * b_block + 2 * sl > kSmemBudget) p.sb_stages--;
@@ -200,7 +207,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int sa = p.sa_stages, sb = p.sb_stages;
     uint8_t* smem_out = smem;                                                // [out_bufs][8 warps][4 KiB]
     uint8_t* smem_b = smem + p.out_bufs * kOutStage;
-    uint8_t* smem_a = smem_b + (p.b_resident ? p.n_seg : sb) * b_block;
+    uint8_t* smem_a = smem_b + (p.b_resident ? p.b_res_bytes : sb * b_block);
     uint8_t* after_a = smem_a + sa * sl;
     float* bias_s = reinterpret_cast<float*>(after_a);                       // [N]
     uint64_t* bars = reinterpret_cast<uint64_t*>(after_a + 1024);
@@ -264,8 +271,20 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         // ------------------------------------------------------------------------ TMA producer
         if (lane == 0) {
             if (p.b_resident) {
-                mbar_arrive_expect_tx(bres_bar, p.n_seg * b_block + (EPI == EPI_FINAL ? kFinalScratch : 0));
-                for (int s = 0; s < p.n_seg; ++s) tma_load_3d(smem_b + s * b_block, &p.tmB, bres_bar, s * kSegK, 0, det);
+                mbar_arrive_expect_tx(bres_bar, p.b_res_bytes + (EPI == EPI_FINAL ? kFinalScratch : 0));
+                int off = 0;                                   // blocks in issue order (cb outer, shift inner)
+                for (int cb = 0; cb < p.n_cb; ++cb)
+                    for (int sh = 0; sh < p.n_shift; ++sh) {
+                        const int s = p.seg_of[cb][sh];
+                        if (s < 0) continue;
+                        if ((p.mask_nu >> (cb * kMaxShift + sh)) & 1ull) {
+                            tma_load_3d(smem_b + off, &p.tmBh, bres_bar, s * kSegK, p.N / 2, det);
+                            off += b_block / 2;
+                        } else {
+                            tma_load_3d(smem_b + off, &p.tmB, bres_bar, s * kSegK, 0, det);
+                            off += b_block;
+                        }
+                    }
                 if (EPI == EPI_FINAL)
                     for (int s = 0; s < 3; ++s) tma_load_3d(smem_fin + s * kFinBlock, &p.tmF, bres_bar, s * kSegK, 0, det);
             }
@@ -323,6 +342,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         const bool ring = p.a_count != nullptr;
         const int n_cb = p.n_cb, n_shift = p.n_shift;
         const uint32_t b_step = static_cast<uint32_t>(b_block) >> 4;       // descriptor units per B K-block
+        const uint32_t idesc_half = umma_idesc_f16(FMT, kTileM, p.N / 2);
+        const unsigned long long mask_k2 = p.mask_k2, mask_nu = p.mask_nu;
         unsigned long long shmask = 0;
         for (int cb = 0; cb < n_cb; ++cb)
             for (int sh = 0; sh < n_shift; ++sh)
@@ -393,14 +414,27 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     const uint32_t a_lo = umma_desc_lo(smem_a_u32 + astage * sl);
                     if (resident) {
                         uint32_t acc_flag = accumulate, bl = b_lo;
+                        const uint32_t mk2 = static_cast<uint32_t>(mask_k2 >> (cb * kMaxShift)), mnu = static_cast<uint32_t>(mask_nu >> (cb * kMaxShift));
                         for (int sh = 0; sh < n_shift; ++sh) {
                             if (!((m >> sh) & 1u)) continue;
                             const uint32_t a_lo_s = a_lo + 8u * sh;        // +128 bytes = one slab row
+                            if ((mnu >> sh) & 1u) {                        // weights in the upper half of N only (half-size block)
 #pragma unroll
-                            for (int k = 0; k < kSegK / 16; ++k)           // +32 bytes along K: +2 in (addr >> 4)
-                                umma_f16_if(leader, d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, acc_flag | k);
+                                for (int k = 0; k < kSegK / 16; ++k)
+                                    umma_f16_if(leader, d_tmem + p.N / 2, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc_half, 1u);
+                                bl += b_step / 2;
+                            } else if ((mk2 >> sh) & 1u) {                 // K steps 0, 1 hold no weight
+#pragma unroll
+                                for (int k = 2; k < kSegK / 16; ++k)
+                                    umma_f16_if(leader, d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, acc_flag | (k - 2));
+                                bl += b_step;
+                            } else {
+#pragma unroll
+                                for (int k = 0; k < kSegK / 16; ++k)       // +32 bytes along K: +2 in (addr >> 4)
+                                    umma_f16_if(leader, d_tmem, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc, acc_flag | k);
+                                bl += b_step;
+                            }
                             acc_flag = 1;
-                            bl += b_step;
                         }
                         umma_commit_if(leader, &a_empty[astage]);          // slab free once these MMAs retire
                         b_lo = bl;

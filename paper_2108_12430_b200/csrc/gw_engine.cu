@@ -51,6 +51,11 @@ extern "C" int gw_set_two_sm(int on) {
     g_two_sm = on ? 1 : 0;
     return GW_OK;
 }
+static int g_skip_zeros = 1;
+extern "C" int gw_set_skip_zeros(int on) {
+    g_skip_zeros = on ? 1 : 0;
+    return GW_OK;
+}
 static int g_snake = 1;
 extern "C" int gw_set_snake(int on) {
     g_snake = on ? 1 : 0;
@@ -396,6 +401,25 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
         p.seg_col[s] = static_cast<int16_t>(seg_cb[s] * kSegK);
         p.seg_of[seg_cb[s]][seg_a[s] - a_lo] = static_cast<int8_t>(s);
     }
+    // structural zeros of each segment (which K steps / which half of N any filter tap reaches at all)
+    if (g_skip_zeros && epi != EPI_POOL && epi != EPI_POOL_HEAD) {
+        for (int s = 0; s < n_seg; ++s) {
+            bool k01 = false, lower = false, upper = false;
+            for (int kk = 0; kk < kSegK; ++kk) {
+                const int col = seg_cb[s] * kSegK + kk, par = col / cin_p, ci = col % cin_p;
+                if (ci >= H0.cin) continue;
+                for (int r = 0; r < halves_out; ++r) {
+                    const int j = tap(seg_a[s], par, r);
+                    if (j < 0 || j >= H0.k) continue;
+                    if (kk < 32) k01 = true;
+                    (r == 0 ? lower : upper) = true;
+                }
+            }
+            const unsigned long long bit = 1ull << (seg_cb[s] * kMaxShift + (seg_a[s] - a_lo));
+            if (halves_out == 2 && upper && !lower && s > 0 && (p.N / 2) % 16 == 0) p.mask_nu |= bit;   // never the tile's first MMA
+            else if (!k01) p.mask_k2 |= bit;
+        }
+    }
     // weights and bias
     const size_t ktot = static_cast<size_t>(n_seg) * kSegK;
     std::vector<uint16_t> B(static_cast<size_t>(n_det) * p.N * ktot, 0);
@@ -438,6 +462,8 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     p.two_sm = g_two_sm;                               // a request: the plan keeps it only where the pair kernel applies
     if (!conv_gemm_plan(gl.g, sms)) return fail(GW_EINVAL, "conv GEMM layer does not fit in shared memory");
     if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.two_sm ? 128 : p.N)) return rc;
+    if (p.mask_nu)
+        if (int rc = make_tmap(&p.tmBh, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.N / 2)) return rc;
     gl.impl = g_conv_impl;
 #ifdef GW_TRACE
     CU_TRY(cudaMalloc(&p.trace, 148 * 16 * 8));
