@@ -670,11 +670,15 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                         gap_s[c] = s / static_cast<float>(Mq);
                     }
                     asm volatile("bar.sync 1, 256;" ::: "memory");
-                    for (int hrow = et; hrow < p.head_hidden; hrow += kEpiWarps * 32) {
-                        float s = __ldg(p.hb1 + hrow);
+                    // one warp per hidden unit, lanes stride over the inputs: the weight row is read with coalesced
+                    // 128-byte requests (one thread per row walked 128 dependent, uncoalesced loads: ~15 us per launch)
+                    for (int hrow = warp - 2; hrow < p.head_hidden; hrow += kEpiWarps) {
                         const float* wr = p.hw1 + static_cast<size_t>(hrow) * half;
-                        for (int c = 0; c < half; ++c) s = fmaf(__ldg(wr + c), gap_s[c], s);
-                        hid_s[hrow] = fmaxf(s, 0.f);
+                        float s = 0.f;
+                        for (int c = lane; c < half; c += 32) s = fmaf(__ldg(wr + c), gap_s[c], s);
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+                        if (lane == 0) hid_s[hrow] = fmaxf(s + __ldg(p.hb1 + hrow), 0.f);
                     }
                     asm volatile("bar.sync 1, 256;" ::: "memory");
                     if (et < 32) {
