@@ -362,6 +362,33 @@ def run_native(args):
                            "samples a launch advances the stream by"}
         del off, seg, cl, nz
 
+    # the snapshotter alone at the paper's highest update rates ("the bottleneck in this
+    # pipeline is the streaming state update" at r = fs/3 and fs/2, i.e. strides of 3 and 2 samples; r = fs was not
+    # attempted there): one stream, 44 channels, W = 32768, a ring append of `stride` samples per update
+    snapshotter = None
+    if not args.no_offline:
+        snapshotter = {}
+        for st_small in (1, 2, 3, 16):
+            sps = S.StreamSpec(1, sp.n_det, sp.fs, sp.window, st_small, sp.n_witness)
+            ss = gw.Stream(sps)
+            new = torch.randn((1, sps.channels, st_small), device="cuda")
+            n_u = 2000
+            with torch.cuda.stream(cs):
+                for _ in range(50):
+                    ss.update(new, cs)
+                s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                s0.record(cs)
+                for _ in range(n_u):
+                    ss.update(new, cs)
+                s1.record(cs)
+            torch.cuda.synchronize()
+            us = 1e3 * s0.elapsed_time(s1) / n_u
+            snapshotter[f"stride_{st_small}"] = {"us_per_update": round(us, 3), "updates_per_s": round(1e6 / us),
+                                                 "realtime_rate_hz": FS / st_small}
+            ss.close()
+        snapshotter["what"] = ("gw_stream_update alone, eager launches of k_append on one stream, 2000 updates, CUDA events; "
+                               "real time needs realtime_rate_hz updates per second")
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         times, cores = oracle_rate(cfg, args.dtype, 200, budget_s=15.0)   # a bounded sample: ~15 s of oracle time
@@ -381,7 +408,7 @@ def run_native(args):
                        "l2": f"inputs larger than L2: ring state {sp.n_streams * sp.channels * sp.window * 4 / 2**20:.0f} MiB "
                              "is re-read every step", "precision": f"{args.dtype} storage, fp32 accumulate"},
             "latency": latency, "e2e": e2e, "gpu_launches": int(launches), "graph_nodes": pipe.graph_nodes(),
-            "roofline": roofline, "kernels": kernels, "clocks": clocks, "cpu_baseline": cpu, "offline": offline,
+            "roofline": roofline, "kernels": kernels, "clocks": clocks, "cpu_baseline": cpu, "offline": offline, "snapshotter": snapshotter,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
