@@ -33,6 +33,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     trace = ["-DGW_TRACE"] if os.environ.get("GW_TRACE") == "1" else []   # diagnostic build: per-role wait counters
+    if os.environ.get("GW_BF16_APPROX_TANH") == "1":                      # experiment: one-MUFU tanh for bf16 as well
+        trace.append("-DGW_BF16_APPROX_TANH")
     cmd = [nvcc] + NVCC_FLAGS + trace + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)

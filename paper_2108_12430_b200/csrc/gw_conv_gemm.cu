@@ -132,10 +132,15 @@ __device__ __forceinline__ uint32_t pack_pair_t(float a, float b) {
 // MUFU op (relative error 2^-11: about one fp16 rounding step; SURVEY.md A18 allows it and the parity
 // tests hold the result to north_star's tolerances).  fp16 takes the one-op form, bf16 the exact one.  tanh.approx.f16x2 was
 // tried: ptxas splits it into two MUFU.TANH.F16, so it saves nothing and is less accurate.
+#ifdef GW_BF16_APPROX_TANH
+constexpr bool kBf16ExactTanh = false;
+#else
+constexpr bool kBf16ExactTanh = true;
+#endif
 template <int ACT, int FMT>
 __device__ __forceinline__ uint32_t act_pack_t(float a, float b) {
     if (ACT == ACT_TANH) {
-        if (FMT == FMT_BF16) {
+        if (FMT == FMT_BF16 && kBf16ExactTanh) {
             // bf16 keeps the exact form: its per-element error budget is already spent on storage rounding
             // and every flipped rounding costs 2^-8
             const float ea = __expf(2.f * a), eb = __expf(2.f * b);
@@ -154,7 +159,7 @@ __device__ __forceinline__ uint32_t act_pack_t(float a, float b) {
 template <int ACT, int FMT>
 __device__ __forceinline__ float act_f32_t(float a) {
     if (ACT == ACT_TANH) {
-        if (FMT == FMT_BF16) return 1.f - __fdividef(2.f, 1.f + __expf(2.f * a));
+        if (FMT == FMT_BF16 && kBf16ExactTanh) return 1.f - __fdividef(2.f, 1.f + __expf(2.f * a));
         float t;
         asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(a));
         return t;
