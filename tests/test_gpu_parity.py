@@ -288,20 +288,20 @@ def test_call_order_is_enforced():
 
 # ------------------------------------------------- full size: the launch configuration bench.py times
 @pytest.mark.gpu
-@pytest.mark.parametrize("dtype", [gw.GW_FP16, gw.GW_BF16])
-def test_full_size_c4_sampled_streams_match_oracle(dtype):
-    """BASELINE.json configs[4] as bench.py runs it: n = 128 streams x 2 detectors, W = 32768, S = 512, one
+@pytest.mark.parametrize("dtype,n", [(gw.GW_FP16, 128), (gw.GW_BF16, 128), (gw.GW_FP16, 512)])
+def test_full_size_c4_sampled_streams_match_oracle(dtype, n):
+    """BASELINE.json configs[4] as bench.py runs it: n = 128 (and 512) streams x 2 detectors, W = 32768, S = 512, one
     CUDA-graph launch per stride -- every CTA of the persistent conv GEMMs walks many tiles, weight
     blocks stream through the pair-mode ring, both MMA warps and PDL are live.  The oracle checks sampled
     streams one by one (first, last and one in the middle); a property that holds at any size covers the
     rest: streams fed identical samples give bit-identical results wherever they sit in the batch."""
-    n, n_up = 128, 3
+    n_up = 3
     cfg = S.config_c3(n, 512, 32768)
     sp = cfg.stream
     dc_params, bbh_params = util.make_params(cfg)
     one = S.StreamSpec(1, sp.n_det, sp.fs, sp.window, sp.stride, sp.n_witness)
     base = [synth.stream_channels(cfg.seed + i, one, n_up * sp.stride) for i in range(3)]
-    sampled = {0: 0, 77: 1, 127: 2}                      # stream index -> which base signal it carries
+    sampled = {0: 0, 77: 1, n - 1: 2}                    # stream index -> which base signal it carries
     x = np.empty((n, sp.channels, n_up * sp.stride), dtype=np.float32)
     for i in range(n):
         x[i] = base[sampled.get(i, i % 3)]
@@ -328,7 +328,7 @@ def test_full_size_c4_sampled_streams_match_oracle(dtype):
                 util.check_network_output(final[i, d], ref["cleaned_final"][d], "final " + tag, rms_ref=ref["pred"][d], elem=et)
             assert abs(float(scores[i]) - ref["score"]) <= util.SCORE_ABS, (t, i, float(scores[i]), ref["score"])
         for i in range(n):                               # position in the batch does not matter
-            j = {0: 0, 1: 77, 2: 127}[i % 3] if i not in sampled else i
+            j = {0: 0, 1: 77, 2: n - 1}[i % 3] if i not in sampled else i
             assert np.array_equal(pred[i], pred[j]), (t, i, j)
             assert np.array_equal(final[i], final[j]) and scores[i] == scores[j], (t, i, j)
 
