@@ -60,6 +60,9 @@ struct ConvGemmParams {
     // 1: walk the (batch item, tile) work list backwards.  Consecutive layers alternate direction, so a
     // layer starts on the activations its predecessor wrote LAST -- the part still resident in the 126 MB L2.
     int reverse;
+    // EPI_STORE: tiles per accumulator stage (0 = as many as fit: 256 / N).  The plan lowers it when the launch has too
+    // few stages' worth of work to fill the persistent CTAs evenly (small stream counts: latency, wave quantisation).
+    int g_tiles;
     int two_sm;                    // 1: CTA-pair kernel (tcgen05 cta_group::2, M = 256), chosen by conv_gemm_plan
     // EPI_FINAL: this layer (ConvTranspose1d -> 32 channels, tanh) and the network's last layer
     // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel.  The

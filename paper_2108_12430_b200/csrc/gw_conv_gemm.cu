@@ -113,6 +113,18 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     p.sa_stages = sa;
     g.smem_bytes = fixed + b_bytes + sa * sl;
     g.grid = sm_count - sm_count % p.n_det;
+    // tiles per stage: when the whole launch is less than one wave of full stages (few streams: the latency
+    // regime), smaller units spread it over more CTAs -- the smallest unit count that still fits one wave wins.
+    // With more work than that the full stage stays (measured at n = 16: smaller units did not pay).
+    p.g_tiles = 0;
+    if (p.epi == EPI_STORE && g.batch > 0) {
+        const int n_items = g.batch / p.n_det, workers = g.grid / p.n_det;
+        for (int G = kAccCols / p.N; G >= 2; G /= 2) {
+            const long long units = static_cast<long long>(n_items) * ((p.tiles_m + G - 1) / G);
+            if (units > workers) break;
+            p.g_tiles = G;
+        }
+    }
     return true;
 }
 
@@ -235,7 +247,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int det = blockIdx.x % p.n_det;
     const int worker = blockIdx.x / p.n_det;
     const int n_workers = gridDim.x / p.n_det;
-    const int G = EPI == EPI_STORE ? kAccCols / p.N : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
+    const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / p.N) : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
     const int spi = (p.tiles_m + G - 1) / G;                                 // super-tiles per batch item
     // Two MMA-issuing warps share a stage when it holds several tiles (even tiles: warp 1, odd tiles: warp
     // kMmaWarp2).  Below N = 128 an MMA is bound by its shared-memory operand read (32 + N/4 cycles, measured:
@@ -1096,7 +1108,8 @@ cudaError_t conv_gemm_prepare() {
 
 void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     const int n_items = g.batch / g.p.n_det;
-    const int total = n_items * g.p.tiles_m;                 // tiles per detector
+    const int per_unit = g.p.epi == EPI_STORE ? (g.p.g_tiles ? g.p.g_tiles : kAccCols / g.p.N) : g.p.epi == EPI_FINAL ? 2 : 1;
+    const int total = n_items * ((g.p.tiles_m + per_unit - 1) / per_unit);   // work units per detector
     int workers = g.grid / g.p.n_det;
     if (workers > total) workers = total;
     GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt);
