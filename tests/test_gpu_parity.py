@@ -729,3 +729,41 @@ def test_handles_release_their_device_memory():
     gc.collect(); torch.cuda.synchronize(); torch.cuda.empty_cache()
     free1, _ = torch.cuda.mem_get_info()
     assert free0 - free1 < 8 * 2**20, (free0, free1)
+
+
+@pytest.mark.gpu
+def test_scheduling_switches_are_bit_identical():
+    """include/gwstream.h promises that gw_set_pdl / _snake / _two_sm / _skip_zeros change scheduling (or skip exact
+    zeros) only.  C3-shaped layers at full window length (the CTA-pair kernel needs an even number of 128-row tiles),
+    three streams so that CTAs walk several work items; every switch off in turn, compared bitwise with all on."""
+    cfg = S.config_c3(3, 512, 32768)
+    sp = cfg.stream
+    dc_params, bbh_params = util.make_params(cfg)
+    n_up = 2
+    xc = torch.from_numpy(np.ascontiguousarray(
+        synth.multi_stream(cfg.seed, sp, n_up * sp.stride).reshape(sp.n_streams, sp.channels, n_up, sp.stride).transpose(2, 0, 1, 3))).cuda()
+    switches = {"pdl": gw.set_pdl, "snake": gw.set_snake, "two_sm": gw.set_two_sm, "skip_zeros": gw.set_skip_zeros}
+
+    def run():
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, gw.GW_FP16)
+        cs = torch.cuda.Stream()
+        sc = torch.zeros(sp.n_streams, device="cuda")
+        fin = torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda")
+        torch.cuda.synchronize()
+        out = []
+        for t in range(n_up):
+            pipe.step(xc[t], sc, fin, cs)
+            cs.synchronize()
+            out.append((dc.noise().cpu().numpy(), fin.cpu().numpy().copy(), sc.cpu().numpy().copy()))
+        return out
+
+    base = run()
+    for name, setter in switches.items():
+        setter(False)
+        try:
+            got = run()
+        finally:
+            setter(True)
+        for t in range(n_up):
+            for a, b, what in zip(got[t], base[t], ("pred", "final", "scores")):
+                assert np.array_equal(a, b), (name, t, what)
