@@ -653,74 +653,88 @@ void launch_aggregate(const AggParams& a, cudaStream_t st) {
 // ---------------------------------------------------------------------------------------------
 // a6' First classifier block (cin = number of detectors, K <= 8): conv + bias + ReLU + MaxPool(4) on
 // CUDA cores in fp32 (as a GEMM its K would be 16: one MMA k-step and all epilogue).
-// lane = output channel (its cin x 8 taps live in registers), one warp = 32 channels of a run of pooled
-// positions.  The input tile starts at l0 = 4 q0 - pad_l, so pooled position q reads the 12 consecutive
-// floats xs[ci][4 (q - q0) .. +12) as three 128-bit warp-broadcast loads per input channel; conv output
-// 4q + i, tap j reads element i + j of that window.  The 64-byte output row of a warp is contiguous.
+// lane = pooled position, a warp = 32 pooled positions x 8 output channels: each lane keeps the 12 input samples
+// per input channel that its four conv outputs touch in registers (conflict-free 128-bit shared loads, 16 bytes
+// apart per lane) and the channel's cin x 8 taps arrive as warp-broadcast 128-bit shared loads, so a (position,
+// channel) pair costs its 16 x cin x ... FMAs and little else (lane = channel with broadcast inputs spent 137
+// instructions per 64 FMAs: the kernel was instruction-bound).  A lane stores its 8 channels as one 16-byte word.
 // x: [batch][cin][L] fp32; w: [cout][cin][K] fp32 (already rounded to the storage type);
 // out: [batch][L/4][cpad] 16-bit channels-last, channels >= cout zero.
-// Requires pool == 4, K <= 8, pad_l <= 4, K - 1 - pad_l <= 4, cin <= 4.
+// Requires pool == 4, K <= 8, pad_l <= 4, K - 1 - pad_l <= 4, cin <= 4, cpad == 32 per blockIdx.z.
 // ---------------------------------------------------------------------------------------------
-constexpr int kC1Q = 64;          // pooled positions per block
+constexpr int kC1Q = 64;          // pooled positions per tile: two position groups of 32 lanes
 constexpr int kC1MaxCin = 4;
 constexpr int kC1Span = kC1Q * 4 + 12;
 
-__global__ void __launch_bounds__(256) k_bbh_conv1(const float* __restrict__ x, const float* __restrict__ w,
-                                                   const float* __restrict__ bias, void* __restrict__ out,
-                                                   int cin, int L, int cout, int cpad, int K, int pad_l, int fmt) {
+// CIN is a template parameter so that the per-lane input window costs 12 CIN registers, not 48: four blocks per SM
+// (592 slots) then hold the 512 blocks of a 128-window launch in ONE wave.
+template <int CIN>
+__global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ x, const float* __restrict__ w,
+                                                      const float* __restrict__ bias, void* __restrict__ out,
+                                                      int L, int cout, int cpad, int K, int pad_l, int fmt) {
+    constexpr int cin = CIN;
     __shared__ __align__(16) float xs[kC1MaxCin][kC1Span];
+    __shared__ __align__(16) float ws[32][kC1MaxCin][8];      // this block's 32 channels, zero where unused
+    __shared__ float bs[32];
     const int b = blockIdx.y;
     const int Lq = L / 4;
     const int lane = threadIdx.x % 32, wrp = threadIdx.x / 32;
-    const int c = lane + blockIdx.z * 32;
-    float wr[kC1MaxCin][8];
-#pragma unroll
-    for (int ci = 0; ci < kC1MaxCin; ++ci)
-#pragma unroll
-        for (int j = 0; j < 8; ++j)
-            wr[ci][j] = (c < cout && ci < cin && j < K) ? __ldg(w + (static_cast<size_t>(c) * cin + ci) * K + j) : 0.f;
-    const float bc = c < cout ? __ldg(bias + c) : 0.f;
-    constexpr int q_per_warp = kC1Q / 8;
-    // a block keeps its 16 weights per lane in registers and walks several tiles of kC1Q pooled positions
-    for (int q0 = blockIdx.x * kC1Q; q0 < Lq; q0 += gridDim.x * kC1Q) {
-    const int l0 = q0 * 4 - pad_l;                      // first input position of the tile
-    __syncthreads();                                    // the previous tile has been consumed
-    for (int i = threadIdx.x; i < cin * kC1Span; i += blockDim.x) {
-        const int ci = i / kC1Span, l = l0 + i % kC1Span;
-        xs[ci][i % kC1Span] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+    const int cbase = blockIdx.z * 32;
+    for (int i = threadIdx.x; i < 32 * kC1MaxCin * 8; i += blockDim.x) {
+        const int c = cbase + i / (kC1MaxCin * 8), ci = (i / 8) % kC1MaxCin, j = i % 8;
+        (&ws[0][0][0])[i] = (c < cout && ci < cin && j < K) ? __ldg(w + (static_cast<size_t>(c) * cin + ci) * K + j) : 0.f;
     }
-    __syncthreads();
-#pragma unroll 2
-    for (int qi = 0; qi < q_per_warp; ++qi) {
-        const int ql = wrp * q_per_warp + qi;           // pooled position inside the tile
+    if (threadIdx.x < 32) bs[threadIdx.x] = cbase + threadIdx.x < cout ? __ldg(bias + cbase + threadIdx.x) : 0.f;
+    const int pg = wrp & 1;                               // position group: pooled positions [32 pg, +32) of the tile
+    const int cg = wrp >> 1;                              // channel group: channels [8 cg, +8) of the block's 32
+    for (int q0 = blockIdx.x * kC1Q; q0 < Lq; q0 += gridDim.x * kC1Q) {
+        const int l0 = q0 * 4 - pad_l;                    // first input position of the tile
+        __syncthreads();                                  // the previous tile has been consumed (and ws / bs are written)
+        for (int i = threadIdx.x; i < cin * kC1Span; i += blockDim.x) {
+            const int ci = i / kC1Span, l = l0 + i % kC1Span;
+            xs[ci][i % kC1Span] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+        }
+        __syncthreads();
+        const int ql = pg * 32 + lane;                    // pooled position inside the tile
         const int q = q0 + ql;
-        if (q >= Lq) break;
-        float acc[4] = {bc, bc, bc, bc};
+        float v[CIN][12];
 #pragma unroll
-        for (int ci = 0; ci < kC1MaxCin; ++ci) {
-            if (ci < cin) {
-                float v[12];
-                const float4* src = reinterpret_cast<const float4*>(&xs[ci][4 * ql]);   // warp-broadcast
+        for (int ci = 0; ci < CIN; ++ci) {
+            {
+                const float4* src = reinterpret_cast<const float4*>(&xs[ci][4 * ql]);
 #pragma unroll
                 for (int t = 0; t < 3; ++t) {
                     const float4 f = src[t];
-                    v[4 * t] = f.x; v[4 * t + 1] = f.y; v[4 * t + 2] = f.z; v[4 * t + 3] = f.w;
+                    v[ci][4 * t] = f.x; v[ci][4 * t + 1] = f.y; v[ci][4 * t + 2] = f.z; v[ci][4 * t + 3] = f.w;
                 }
-#pragma unroll
-                for (int j = 0; j < 8; ++j)
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) acc[i] = fmaf(wr[ci][j], v[i + j], acc[i]);
             }
         }
-        float best = fmaxf(fmaxf(fmaxf(acc[0], acc[1]), fmaxf(acc[2], acc[3])), 0.f);   // max-pool, then ReLU
-        if (c >= cout) best = 0.f;
-        const float other = __shfl_down_sync(0xffffffffu, best, 1);
-        if ((lane & 1) == 0) {
-            uint32_t* dst = reinterpret_cast<uint32_t*>(reinterpret_cast<uint16_t*>(out) +
-                                                        (static_cast<size_t>(b) * Lq + q) * cpad + c);
-            *dst = pack16(best, other, fmt);
+        float res[8];
+#pragma unroll
+        for (int cc = 0; cc < 8; ++cc) {
+            const int c = cg * 8 + cc;
+            const float bc = bs[c];
+            float acc[4] = {bc, bc, bc, bc};
+#pragma unroll
+            for (int ci = 0; ci < CIN; ++ci) {
+                {
+                    const float4 w0 = *reinterpret_cast<const float4*>(&ws[c][ci][0]);   // warp-broadcast
+                    const float4 w1 = *reinterpret_cast<const float4*>(&ws[c][ci][4]);
+                    const float wr[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+#pragma unroll
+                    for (int j = 0; j < 8; ++j)
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) acc[i] = fmaf(wr[j], v[ci][i + j], acc[i]);
+                }
+            }
+            res[cc] = fmaxf(fmaxf(fmaxf(acc[0], acc[1]), fmaxf(acc[2], acc[3])), 0.f);   // max-pool, then ReLU
         }
-    }
+        if (q < Lq) {
+            uint4 o;
+            o.x = pack16(res[0], res[1], fmt); o.y = pack16(res[2], res[3], fmt);
+            o.z = pack16(res[4], res[5], fmt); o.w = pack16(res[6], res[7], fmt);
+            *reinterpret_cast<uint4*>(reinterpret_cast<uint16_t*>(out) + (static_cast<size_t>(b) * Lq + q) * cpad + cbase + cg * 8) = o;
+        }
     }
 }
 
@@ -731,7 +745,12 @@ void launch_bbh_conv1(const float* x, const float* w, const float* b, void* out,
     int tiles = (Lq + kC1Q - 1) / kC1Q;
     if (static_cast<long long>(tiles) * batch >= 148 * 8) tiles = (tiles + 3) / 4;   // enough blocks: four tiles per block
     dim3 grid(tiles, batch, cpad / 32);
-    k_bbh_conv1<<<grid, 256, 0, st>>>(x, w, b, out, n_det, L, cout, cpad, K, pad_l, fmt);
+    switch (n_det) {                                   // cin = number of detectors (validated <= 4 at create time)
+        case 1: k_bbh_conv1<1><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
+        case 2: k_bbh_conv1<2><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
+        case 3: k_bbh_conv1<3><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
+        default: k_bbh_conv1<4><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
+    }
     ++g_kernel_launches;
 }
 
