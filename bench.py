@@ -358,6 +358,7 @@ def run_native(args):
         off_ms = o0.elapsed_time(o1) / n_off
         offline = {"windows_per_launch": B, "samples_per_launch": off.samples, "ms_per_launch": off_ms,
                    "value": B * sp.stride / FS / (off_ms * 1e-3), "unit": UNIT,
+                   "tflops_whole_launch": round(sum(v[1] for k, v in prof.items() if k.startswith("gemm.dc")) / (off_ms * 1e-3) / 1e12, 1),
                    "what": "gw_offline_run on a device-resident segment of one 2-detector stream; value counts the B*S new "
                            "samples a launch advances the stream by"}
         del off, seg, cl, nz
