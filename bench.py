@@ -304,6 +304,7 @@ def run_native(args):
             a = prof.setdefault(label, [0.0, 0.0])
             a[0] += ms / n_prof
             a[1] = fl
+    smem_bytes = pipe.profile_smem_bytes()
     pk = peaks()
     gemm_ms = sum(v[0] for k, v in prof.items() if k.startswith("gemm."))
     gemm_fl = sum(v[1] for k, v in prof.items() if k.startswith("gemm."))
@@ -334,6 +335,15 @@ def run_native(args):
         if k in kernels and kernels[k]["ms"] > 0:
             gbs = b / (kernels[k]["ms"] * 1e-3) / 1e9
             kernels[k].update({"gbs": round(gbs, 1), "hbm_frac": round(gbs / pk["hbm_gbs"], 3)})
+    # conv GEMMs against the shared-memory operand roofline: traffic by the engine's accounting
+    # (MMA operand reads + TMA fills + epilogue staging) over 128 B/clk per SM at the SM clock sampled under load
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1700.0
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    smem_peak_gbs = sms * 128 * sm_mhz * 1e6 / 1e9
+    for k, b in smem_bytes.items():
+        if k in kernels and kernels[k]["ms"] > 0:
+            gbs = b / (kernels[k]["ms"] * 1e-3) / 1e9
+            kernels[k].update({"smem_gbs": round(gbs, 1), "smem_frac": round(gbs / smem_peak_gbs, 3)})
 
     # offline / non-streaming mode (D9): the same number of detector-windows per launch, but all from ONE
     # stream's archival segment (B = n windows advance the stream by B*S samples per launch)
@@ -409,7 +419,7 @@ def run_native(args):
                        "l2": f"inputs larger than L2: ring state {sp.n_streams * sp.channels * sp.window * 4 / 2**20:.0f} MiB "
                              "is re-read every step", "precision": f"{args.dtype} storage, fp32 accumulate"},
             "latency": latency, "e2e": e2e, "gpu_launches": int(launches), "graph_nodes": pipe.graph_nodes(),
-            "roofline": roofline, "kernels": kernels, "clocks": clocks, "cpu_baseline": cpu, "offline": offline, "snapshotter": snapshotter,
+            "roofline": roofline, "smem_peak_gbs": round(smem_peak_gbs, 1), "kernels": kernels, "clocks": clocks, "cpu_baseline": cpu, "offline": offline, "snapshotter": snapshotter,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -234,6 +234,10 @@ int gw_step_profile(gw_pipeline *p, const float *new_samples_dev, float *scores_
                     void *stream, int max_kernels, float *ms_out, int *n_out);
 const char *gw_profile_label(const gw_pipeline *p, int i);
 double gw_profile_flops(const gw_pipeline *p, int i);
+/* Shared-memory traffic (bytes, all SMs) of conv GEMM kernel i of the last profiled step by the accounting of
+ * DESIGN.md section 7 (MMA operand reads + TMA fills + epilogue staging); 0 for other kernels.  Against
+ * 128 B/clk x SMs x SM clock it is the roofline the thin layers are bound by. */
+double gw_profile_smem_bytes(const gw_pipeline *p, int i);
 /* number of kernel nodes in the captured graph (0 before the first gw_step) */
 int gw_pipeline_graph_nodes(const gw_pipeline *p);
 

@@ -27,7 +27,7 @@ EXPORTS = [
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
     "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_step_host_async", "gw_pipeline_graph_nodes",
-    "gw_step_profile", "gw_profile_label", "gw_profile_flops",
+    "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes",
     "gw_deepclean_set_scaling", "gw_offline_set_scaling", "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
 ]
 
@@ -116,6 +116,8 @@ def lib():
         L.gw_profile_label.restype = C.c_char_p
         L.gw_profile_flops.argtypes = [vp, i]
         L.gw_profile_flops.restype = C.c_double
+        L.gw_profile_smem_bytes.argtypes = [vp, i]
+        L.gw_profile_smem_bytes.restype = C.c_double
         _lib = L
     return _lib
 
@@ -412,6 +414,18 @@ class Pipeline:
                                      _stream_ptr(stream), 64, ms, C.byref(n)))
         return [(lib().gw_profile_label(self.h, i).decode(), float(ms[i]), float(lib().gw_profile_flops(self.h, i)))
                 for i in range(min(n.value, 64))]
+
+    def profile_smem_bytes(self):
+        """{label: shared-memory traffic in bytes} of the conv GEMM kernels of the last step_profile."""
+        out = {}
+        for i in range(64):
+            lab = lib().gw_profile_label(self.h, i).decode()
+            if not lab:
+                break
+            b = float(lib().gw_profile_smem_bytes(self.h, i))
+            if b > 0:
+                out[lab] = b
+        return out
 
     def graph_nodes(self) -> int:
         return int(lib().gw_pipeline_graph_nodes(self.h))

@@ -1358,6 +1358,36 @@ extern "C" double gw_profile_flops(const gw_pipeline* p, int i) {
     return 0.0;
 }
 
+// Shared-memory traffic of one launch of a conv GEMM layer, summed over all SMs, by the accounting of DESIGN.md
+// section 7: per 128-row tile the tensor core reads 4 KiB of A plus 32 N bytes of B per MMA (half of B per SM in the
+// CTA-pair kernel), TMA writes the A slabs (and, when weights are streamed, the weight blocks) and the epilogue
+// writes its staged output once and TMA reads it once.  Divided by 128 B/clk/SM x SMs x clock it gives the
+// shared-memory roofline the thin layers sit on.
+static double gemm_smem_bytes(const GemmLayer& gl, int batch) {
+    const ConvGemmParams& p = gl.g.p;
+    const int n_items = batch / p.n_det;
+    int n_half = 0, n_k2 = 0;
+    for (unsigned long long m = p.mask_nu; m; m &= m - 1) ++n_half;
+    for (unsigned long long m = p.mask_k2; m; m &= m - 1) ++n_k2;
+    const double b_per_mma = 32.0 * p.N * (p.two_sm ? 0.5 : 1.0);
+    double mma = 4.0 * (p.n_seg - n_half - n_k2) * (4096.0 + b_per_mma)             // full segments: four K steps
+               + 4.0 * n_half * (4096.0 + b_per_mma / 2) + 2.0 * n_k2 * (4096.0 + b_per_mma);
+    double fill = static_cast<double>(p.n_cb) * p.slab_rows * 128.0;
+    if (!p.b_resident) fill += static_cast<double>(p.n_seg) * p.N * 128.0 * (p.two_sm ? 0.5 : 1.0);
+    double epi = 0.0;
+    if (p.epi == EPI_STORE) epi = 2.0 * 128.0 * p.N * 2.0;                            // staged once, read once by the TMA store
+    if (p.epi == EPI_FINAL) { epi = 128.0 * 128.0; mma += 10.0 * (4096.0 + 32.0 * 16); }   // activated tile + second chain
+    return (mma + fill + epi) * static_cast<double>(p.tiles_m) * n_items * p.n_det;
+}
+
+extern "C" double gw_profile_smem_bytes(const gw_pipeline* p, int i) {
+    if (!p) return 0.0;
+    const std::string lab = gw_profile_label(p, i);
+    for (auto& g : p->dc->gemm) if (g.name == lab) return gemm_smem_bytes(g, p->dc->batch);
+    if (p->bbh) for (auto& g : p->bbh->gemm) if (g.name == lab) return gemm_smem_bytes(g, p->bbh->batch);
+    return 0.0;
+}
+
 // Throughput form of gw_step_host: does NOT synchronise, and the host->device copy of this call's samples
 // runs on an internal copy stream into one of two staging buffers, so it overlaps the previous step's kernels
 // (at C4 n=128 the copy is 11.5 MB, about a quarter of the step).  Results land in the host buffers in stream
