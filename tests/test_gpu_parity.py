@@ -175,13 +175,36 @@ def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype, fuse):
                                       elem=1e-1 if dtype == gw.GW_BF16 else et)
         pred = dc.noise().cpu().numpy()[i, 0]
         util.check_network_output(pred, ref_p, f"prediction stream {i}", elem=et)
-        # against the storage-rounded oracle (diagnostic): what is left is implementation error only
-        # (fp32 accumulation order, hardware tanh, rounding flips it causes), far below the storage floor
-        ref_r = oracle.deepclean_forward(snap[cfg.stream.witness_rows(0)].astype(np.float64), cfg.dc_layers,
-                                         prepared, act_dtype=od)
+        # Against the storage-rounded oracle what is left is implementation error only (fp32 accumulation order,
+        # hardware tanh, the rounding flips they cause): the storage-format floor argument does not apply here, so
+        # BOTH dtypes are held to north_star's per-element bar (2e-2 RMS) and to a 3e-3 relative-L2 bar.
+        xin = snap[cfg.stream.witness_rows(0)].astype(np.float64)
+        ref_r, acts_r = oracle.deepclean_forward(xin, cfg.dc_layers, prepared, act_dtype=od, return_all=True)
         r = util.check_network_output(pred, ref_r, f"prediction vs storage-rounded oracle, stream {i}",
-                                      elem=et, rel_l2=3e-3)   # a rare rounding flip costs one full ulp
-        print(f"dtype {dtype} stream {i}: vs storage-rounded oracle rel L2 {r[0]:.2e}, worst/RMS {r[1]:.2e}")
+                                      elem=util.ELEM_RMS, rel_l2=3e-3)
+        worst_layer = 0.0
+        for li, (layer, ref) in enumerate(zip(cfg.dc_layers[:-1], acts_r[:-1])):
+            if fuse and li == len(cfg.dc_layers) - 2:
+                continue
+            got = dc.activation(li).float().cpu().numpy()[i, 0]
+            # stored 16-bit values: a rounding that flips costs one unit in the last place of the value's binade (bf16:
+            # 2^-8 = 3.9e-3 for |v| in [0.5, 1), i.e. ~1.3e-2 of a layer RMS of 0.3), and flips propagate; the bar for
+            # the STORED layers is therefore two such units (bf16 4e-2 RMS, fp16 5e-3 RMS), still 2.5x tighter than the
+            # 1e-1 used against the unrounded oracle above; the fp32 prediction itself is held to 2e-2 RMS.
+            _, wl = util.check_network_output(got[:, :layer.cout].T, ref, f"layer {li} vs storage-rounded oracle, stream {i}",
+                                              elem=4e-2 if dtype == gw.GW_BF16 else 5e-3, rel_l2=3e-3)
+            worst_layer = max(worst_layer, wl)
+        # total error against the model with UNROUNDED fp64 weights (reported: weight quantisation is part of the model
+        # by reading A9, so this is context, not a bar; only a loose sanity bound is asserted)
+        unr = [util.unrounded_conv(l, p) for l, p in zip(cfg.dc_layers, dc_params2[0])]
+        ref_u = oracle.deepclean_forward(xin, cfg.dc_layers, unr)
+        du = pred - ref_u
+        rel_u = float(np.linalg.norm(du) / np.linalg.norm(ref_u))
+        worst_u = float(np.max(np.abs(du)) / np.sqrt(np.mean(ref_u ** 2)))
+        assert rel_u <= 5e-2
+        print(f"dtype {'bf16' if dtype == gw.GW_BF16 else 'fp16'} fuse {fuse} stream {i}: vs storage-rounded oracle rel L2 "
+              f"{r[0]:.2e}, worst/RMS {r[1]:.2e} (layers: worst/RMS {worst_layer:.2e}); vs fp64-weight model rel L2 {rel_u:.2e}, "
+              f"worst/RMS {worst_u:.2e}")
 
 
 # ----------------------------------------------------------------------------- classifier (C2)
@@ -213,6 +236,26 @@ def test_small_ensemble_eager_matches_oracle(dtype):
 def test_small_ensemble_graph_matches_oracle_and_eager():
     cfg = S.config_small_ensemble(2)
     _run_streaming(cfg, gw.GW_BF16, cfg.n_updates, white=False, use_graph=True)
+
+
+@pytest.mark.parametrize("agg", [S.AGG_HANN_OLA, S.AGG_LAST_STRIDE])
+@pytest.mark.parametrize("delta", [256, 788, 131])
+def test_small_ensemble_latency_offset_scores_match_oracle(agg, delta):
+    """D8 with delta > 0 WITH the classifier attached: the window the classifier scores ends `delta`
+    samples before the newest sample (delta = S, 3S + 20, and 131: not a multiple of 4, which takes the scalar
+    aggregation kernel).  Scores, running estimate and running cleaned strain against the oracle, both aggregation
+    modes; the oracle's own window arithmetic is pinned by direct slicing in tests/test_oracle_pins.py."""
+    cfg = S.config_small_ensemble(2)
+    assert cfg.bbh_len + delta <= cfg.stream.window
+    stats = _run_streaming(cfg, gw.GW_FP16, cfg.n_updates, white=False, agg=agg, delta=delta)
+    print(f"delta={delta} agg={agg}: worst", stats)
+
+
+def test_small_ensemble_latency_offset_through_the_graph():
+    """The same through gw_step (the captured graph bakes delta into the aggregation node)."""
+    cfg = S.config_small_ensemble(2)
+    _run_streaming(cfg, gw.GW_FP16, cfg.n_updates, white=False, agg=S.AGG_HANN_OLA, delta=512, use_graph=True)
+    _run_streaming(cfg, gw.GW_FP16, cfg.n_updates, white=False, agg=S.AGG_LAST_STRIDE, delta=256, use_graph=True)
 
 
 def test_results_do_not_depend_on_batching():
@@ -288,49 +331,77 @@ def test_call_order_is_enforced():
 
 # ------------------------------------------------- full size: the launch configuration bench.py times
 @pytest.mark.gpu
-@pytest.mark.parametrize("dtype,n", [(gw.GW_FP16, 128), (gw.GW_BF16, 128), (gw.GW_FP16, 512)])
-def test_full_size_c4_sampled_streams_match_oracle(dtype, n):
+@pytest.mark.parametrize("dtype,n,full_chain", [(gw.GW_FP16, 128, True), (gw.GW_BF16, 128, False), (gw.GW_FP16, 512, False)])
+def test_full_size_c4_sampled_streams_match_oracle(dtype, n, full_chain):
     """BASELINE.json configs[4] as bench.py runs it: n = 128 (and 512) streams x 2 detectors, W = 32768, S = 512, one
-    CUDA-graph launch per stride -- every CTA of the persistent conv GEMMs walks many tiles, weight
-    blocks stream through the pair-mode ring, both MMA warps and PDL are live.  The oracle checks sampled
-    streams one by one (first, last and one in the middle); a property that holds at any size covers the
-    rest: streams fed identical samples give bit-identical results wherever they sit in the batch."""
-    n_up = 3
+    CUDA-graph launch per stride -- every CTA of the persistent conv GEMMs walks many tiles, weight blocks stream
+    through the pair-mode ring, both MMA warps and PDL are live -- compared with the oracle on FULLY POPULATED windows:
+    the engine is pre-rolled through W/S = 64 updates (the sampled oracles only record those samples, oracle.skip), then
+    the raw predictions of three sampled streams (first, middle, last) are checked on 3 further updates.  With
+    full_chain (n = 128, fp16) the oracle of stream 0 is run through ALL 72 updates instead, so that its overlap-add
+    state is complete: final cleaned samples and classifier scores are then checked on the 8 steady-state updates as
+    well as on the warm-up ones.  A property that holds at any size covers the unsampled streams: streams fed identical
+    samples give bit-identical results wherever they sit in the batch."""
     cfg = S.config_c3(n, 512, 32768)
     sp = cfg.stream
+    k = sp.window // sp.stride
+    n_cmp = 8 if full_chain else 3
+    n_up = k + n_cmp
     dc_params, bbh_params = util.make_params(cfg)
     one = S.StreamSpec(1, sp.n_det, sp.fs, sp.window, sp.stride, sp.n_witness)
-    base = [synth.stream_channels(cfg.seed + i, one, n_up * sp.stride) for i in range(3)]
+    base = np.stack([synth.stream_channels(cfg.seed + i, one, n_up * sp.stride) for i in range(3)])
     sampled = {0: 0, 77: 1, n - 1: 2}                    # stream index -> which base signal it carries
-    x = np.empty((n, sp.channels, n_up * sp.stride), dtype=np.float32)
-    for i in range(n):
-        x[i] = base[sampled.get(i, i % 3)]
+    which = np.array([sampled.get(i, i % 3) for i in range(n)])
     stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype)
     oracles = {i: util.make_stream_oracle(S.config_c3(1, 512, 32768), dc_params, bbh_params, dtype, n_up) for i in sampled}
-    xd = _dev(x)
+    base_d = _dev(base)
+    which_d = torch.from_numpy(which).cuda()
     cs = torch.cuda.Stream()
     scores_d = torch.zeros(n, device="cuda")
     final_d = torch.zeros((n, sp.n_det, sp.stride), device="cuda")
     et = util.elem_tol(dtype)
+    worst = {"pred": 0.0, "final": 0.0, "score": 0.0}
     for t in range(n_up):
-        new = xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous()
+        new = base_d[:, :, t * sp.stride:(t + 1) * sp.stride][which_d].contiguous()     # [n][C][S]
         cs.wait_stream(torch.cuda.current_stream())
         pipe.step(new, scores_d, final_d, cs)
         cs.synchronize()
+        compare_all = t >= k
+        for i, orc in oracles.items():
+            xs = base[sampled[i]][:, t * sp.stride:(t + 1) * sp.stride]
+            chain = full_chain and i == 0
+            if not compare_all and not chain:
+                orc.skip(xs)                             # zero oracle cost: only records the samples
+        if not compare_all and not full_chain:
+            continue
         pred = dc.noise().cpu().numpy()
         final = final_d.cpu().numpy()
         scores = scores_d.cpu().numpy()
         for i, orc in oracles.items():
-            ref = orc.update(x[i][:, t * sp.stride:(t + 1) * sp.stride])
+            chain = full_chain and i == 0
+            if not compare_all and not chain:
+                continue
+            if chain and not compare_all and t % 8 != 7 and t > 2:
+                orc.update(base[sampled[i]][:, t * sp.stride:(t + 1) * sp.stride])   # state only (warm-up updates are sampled)
+                continue
+            ref = orc.update(base[sampled[i]][:, t * sp.stride:(t + 1) * sp.stride])
             for d in range(sp.n_det):
                 tag = f"full size update {t} stream {i} det {d}"
-                util.check_network_output(pred[i, d], ref["pred"][d], "pred " + tag, elem=et)
-                util.check_network_output(final[i, d], ref["cleaned_final"][d], "final " + tag, rms_ref=ref["pred"][d], elem=et)
-            assert abs(float(scores[i]) - ref["score"]) <= util.SCORE_ABS, (t, i, float(scores[i]), ref["score"])
-        for i in range(n):                               # position in the batch does not matter (PAPER.md:174)
-            j = {0: 0, 1: 77, 2: n - 1}[i % 3] if i not in sampled else i
-            assert np.array_equal(pred[i], pred[j]), (t, i, j)
-            assert np.array_equal(final[i], final[j]) and scores[i] == scores[j], (t, i, j)
+                _, w1 = util.check_network_output(pred[i, d], ref["pred"][d], "pred " + tag, elem=et)
+                worst["pred"] = max(worst["pred"], w1)
+                if chain:                                # overlap-add state complete: finals and scores are meaningful
+                    _, w2 = util.check_network_output(final[i, d], ref["cleaned_final"][d], "final " + tag, rms_ref=ref["pred"][d], elem=et)
+                    worst["final"] = max(worst["final"], w2)
+            if chain:
+                assert abs(float(scores[i]) - ref["score"]) <= util.SCORE_ABS, (t, i, float(scores[i]), ref["score"])
+                worst["score"] = max(worst["score"], abs(float(scores[i]) - ref["score"]))
+        if compare_all:
+            for i in range(n):                           # position in the batch does not matter (PAPER.md:174)
+                j = {0: 0, 1: 77, 2: n - 1}[which[i]]
+                assert np.array_equal(pred[i], pred[j]), (t, i, j)
+                assert np.array_equal(final[i], final[j]) and scores[i] == scores[j], (t, i, j)
+    print(f"full size n={n} dtype={'bf16' if dtype == gw.GW_BF16 else 'fp16'}: fully populated windows, worst |d|/RMS "
+          f"pred {worst['pred']:.3e} final {worst['final']:.3e}, worst |d score| {worst['score']:.2e}")
 
 
 @pytest.mark.gpu
@@ -624,6 +695,7 @@ def test_c1_full_rate_streaming_bf16_steady_state():
     orc = util.make_stream_oracle(cfg, dc_params, None, dtype, n_up)
     xd = _dev(x)
     et = util.elem_tol(dtype)
+    worst = worst_l2 = 0.0
     for t in range(n_up):
         stream.update(xd[:, :, t * sp.stride:(t + 1) * sp.stride].contiguous())
         dc.forward()
@@ -631,8 +703,13 @@ def test_c1_full_rate_streaming_bf16_steady_state():
         final = dc.cleaned(gw.GW_FINAL).cpu().numpy()[0, 0]
         ref = orc.update(x[0][:, t * sp.stride:(t + 1) * sp.stride])
         if t < 3 or t >= 31:
-            util.check_network_output(pred, ref["pred"][0], f"C1 pred update {t}", elem=et)
+            r = util.check_network_output(pred, ref["pred"][0], f"C1 pred update {t}", elem=et)
             util.check_network_output(final, ref["cleaned_final"][0], f"C1 final update {t}", rms_ref=ref["pred"][0], elem=et)
+            worst = max(worst, r[1]); worst_l2 = max(worst_l2, r[0])
+    # reported, not asserted: north_star's per-element bar (2e-2 RMS) against the UNROUNDED-activation fp64 oracle is out
+    # of reach of any bf16-storage implementation (tests/test_oracle_pins.py::test_bf16_activation_storage_alone_...)
+    print(f"C1 bf16 vs fp64 oracle: worst |d|/RMS {worst:.3e} ({'meets' if worst <= util.ELEM_RMS else 'MISSES'} north_star's "
+          f"2e-2; asserted bar {et}), worst rel L2 {worst_l2:.3e} (bar {util.REL_L2})")
 
 
 @pytest.mark.gpu

@@ -477,6 +477,42 @@ def test_classifier_window_reads_zero_before_stream_start():
         assert np.array_equal(xin[d, cfg.bbh_len - st.stride:].astype(np.float32), x[st.strain_row(d), :st.stride])
 
 
+@pytest.mark.parametrize("agg", [oracle.AGG_HANN_OLA, oracle.AGG_LAST_STRIDE])
+@pytest.mark.parametrize("delta_of", [lambda S_: S_, lambda S_: 3 * S_ + 20, lambda S_: 131])
+def test_classifier_window_with_latency_offset_is_the_delayed_strain_slice(agg, delta_of):
+    """D8 with delta > 0 (analyse [-8 + dt, dt], i.e. everything the classifier sees ends `delta`
+    samples before the newest sample).  Zero network => cleaned == strain, so the classifier input of update t must
+    be the strain samples [(t+1)S - delta - L_b, (t+1)S - delta) by direct slicing (zeros before the stream start).
+    A sign or off-by-S mistake in the window arithmetic moves the slice and fails on the time-varying strain."""
+    cfg = S.config_small_ensemble(1)
+    st = cfg.stream
+    S_, Lb = st.stride, cfg.bbh_len
+    delta = delta_of(S_)
+    rows = [(st.witness_rows(d), st.strain_row(d)) for d in range(2)]
+    zero = [(np.zeros(l.wshape()), np.zeros(l.cout)) for l in cfg.dc_layers]
+    cp, dp = synth.bbh_params(1, cfg.bbh_convs, cfg.bbh_dense)
+    pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    n_up = 9
+    so = oracle.StreamOracle(st.channels, st.window, S_, rows, [(cfg.dc_layers, zero)] * 2,
+                             (cfg.bbh_convs, pc, pd, Lb), agg=agg, delta=delta, max_updates=n_up)
+    x = synth.white_channels(4, st.channels, n_up * S_)
+    seen_real = False
+    for t in range(n_up):
+        out = so.update(x[:, t * S_:(t + 1) * S_])
+        a1 = (t + 1) * S_ - delta
+        for d in range(2):
+            padded = np.concatenate([np.zeros(Lb + delta, np.float32), x[st.strain_row(d), :(t + 1) * S_]])
+            exp = padded[len(padded) - delta - Lb:len(padded) - delta]
+            assert exp.shape == (Lb,)
+            assert np.array_equal(out["bbh_input"][d].astype(np.float32), exp), (t, d, a1)
+        seen_real = seen_real or a1 - Lb >= 0
+        # the score is the classifier on exactly that slice
+        ref = oracle.bbh_forward(out["bbh_input"], cfg.bbh_convs, pc, pd)
+        assert out["score"] == ref
+    assert seen_real, "the test must reach windows that lie entirely inside the stream"
+
+
 # ------------------------------------------------------------- error budget of 16-bit storage
 
 def test_bf16_activation_storage_alone_exceeds_the_elementwise_bar():

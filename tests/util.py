@@ -78,6 +78,17 @@ def make_stream_oracle(cfg: S.Config, dc_params, bbh_params, dtype: int, max_upd
                                max_updates=max_updates, scaling=scaling)
 
 
+def unrounded_conv(layer, params):
+    """(w, b) of a layer in float64 with BatchNorm folded but WITHOUT rounding to the storage type: the model before
+    weight quantisation.  Used only to report the total distance of the CUDA path to that model (context: by reading A9
+    the quantised weights are the model)."""
+    w, b = np.asarray(params["w"], np.float64), np.asarray(params["b"], np.float64)
+    if getattr(layer, "bn", False):
+        w, b = oracle.bn_fold(layer.kind, w, b, params["bn_gamma"], params["bn_beta"], params["bn_mean"],
+                              params["bn_var"], float(params["bn_eps"]))
+    return w, b
+
+
 def check_network_output(got: np.ndarray, ref: np.ndarray, what: str, rms_ref: np.ndarray | None = None,
                          elem: float = ELEM_RMS, rel_l2: float = REL_L2):
     """relative L2 <= 1e-2 and max |d| <= 2e-2 * RMS(ref) (RMS of `rms_ref` when given; reading A22)."""
