@@ -176,6 +176,176 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------ native leg
+NOMINAL_TFLOPS = 2250.0       # B200 dense bf16/fp16 spec-sheet figure (B200_PROFILING.md, "nominal, for context")
+NOMINAL_HBM_GBS = 7700.0
+
+
+class Engine:
+    """One engine instance (n streams of the C3 ensemble) plus the measurement legs bench.py runs on it."""
+
+    def __init__(self, gw, torch, args, n_streams, stride, dtype, opts, chunks_h=None, seg_seconds=None, local=0):
+        self.gw, self.torch, self.args = gw, torch, args
+        self.cfg = S.config_c3(n_streams, stride, WINDOW)
+        self.sp = self.cfg.stream
+        self.dtype_name = dtype
+        self.n_chunks = (seg_seconds or args.seg_seconds) * FS // stride
+        self.dc_params, self.bbh_params = make_params(self.cfg)
+        if chunks_h is None:
+            t0 = time.time()
+            chunks_h = torch.from_numpy(make_input_chunks(self.cfg, self.n_chunks)).pin_memory()
+            log(f"inputs {tuple(chunks_h.shape)} ({chunks_h.numel() * 4 / 2**20:.0f} MiB) in {time.time() - t0:.1f}s")
+        self.chunks_h = chunks_h
+        self.chunks_d = chunks_h.cuda()
+        self.stream, self.dc, self.bbh, self.pipe = gw.build_ensemble(
+            self.cfg, self.dc_params, self.bbh_params, gw.GW_BF16 if dtype == "bf16" else gw.GW_FP16, opts=opts)
+        self.cs = torch.cuda.Stream()
+        self.scores = torch.zeros(self.sp.n_streams, device="cuda")
+        self.final = torch.zeros((self.sp.n_streams, self.sp.n_det, self.sp.stride), device="cuda")
+        self.step_no = 0
+        self.ds_per_step = self.sp.n_streams * self.sp.stride / FS
+
+    def step(self):
+        self.pipe.step(self.chunks_d[self.step_no % self.n_chunks], self.scores, self.final, self.cs)
+        self.step_no += 1
+
+    def timed(self, k):
+        """k back-to-back graph steps between two CUDA events on the launch stream -> total ms."""
+        torch = self.torch
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(self.cs)
+        for _ in range(k):
+            self.step()
+        e1.record(self.cs)
+        self.cs.synchronize()
+        return e0.elapsed_time(e1)
+
+    def latency(self, n):
+        lat = []
+        for _ in range(n):
+            t0 = time.perf_counter()
+            self.step()
+            self.cs.synchronize()
+            lat.append((time.perf_counter() - t0) * 1e3)
+        lat.sort()
+        return {"p50_ms": lat[len(lat) // 2], "p99_ms": lat[min(len(lat) - 1, int(len(lat) * 0.99))],
+                "samples": len(lat), "per_stream_p50_ms": lat[len(lat) // 2] / self.sp.n_streams,
+                "realtime_budget_ms": 1e3 * self.sp.stride / FS,
+                "what": "host clock, gw_step launch -> stream synchronize, whole batch of n streams"}
+
+    def e2e(self, k, world=1):
+        """End to end through the C ABI with HOST buffers (pinned): H2D of every step's samples and D2H of its scores
+        and final cleaned samples inside the timed region.  The outputs ROTATE over four buffer pairs (a consumer reads
+        step i while step i+1 runs; different output pointers are node-parameter updates of the graph, never a
+        re-capture) and every step's results are read on the host (summed) inside the timed region, one step behind."""
+        torch, sp = self.torch, self.sp
+        nbuf = 4
+        sc_h = [torch.zeros(sp.n_streams).pin_memory() for _ in range(nbuf)]
+        fin_h = [torch.zeros((sp.n_streams, sp.n_det, sp.stride)).pin_memory() for _ in range(nbuf)]
+        evs = [torch.cuda.Event() for _ in range(nbuf)]
+        for i in range(nbuf):                         # warm-up: capture + every buffer pair seen once
+            self.pipe.step_host_async(self.chunks_h[self.step_no % self.n_chunks], sc_h[i], fin_h[i], self.cs)
+            self.step_no += 1
+        torch.cuda.synchronize()
+        checksum = 0.0
+        t0 = time.perf_counter()
+        for i in range(k):
+            b = i % nbuf
+            self.pipe.step_host_async(self.chunks_h[self.step_no % self.n_chunks], sc_h[b], fin_h[b], self.cs)
+            evs[b].record(self.cs)
+            self.step_no += 1
+            if i >= 1:                                # consume the previous step's results while this one runs
+                pb = (i - 1) % nbuf
+                evs[pb].synchronize()
+                checksum += float(sc_h[pb].sum()) + float(fin_h[pb].sum())
+        evs[(k - 1) % nbuf].synchronize()
+        checksum += float(sc_h[(k - 1) % nbuf].sum())
+        torch.cuda.synchronize()
+        sec = time.perf_counter() - t0
+        t1 = time.perf_counter()
+        n_sync = min(k, 50)
+        for _ in range(n_sync):                       # online regime: gw_step_host returns with the results
+            self.pipe.step_host(self.chunks_h[self.step_no % self.n_chunks], sc_h[0], fin_h[0], self.cs)
+            self.step_no += 1
+        sync_ms = 1e3 * (time.perf_counter() - t1) / n_sync
+        sec = shard.max_over_ranks(sec, device="cuda")
+        return {"value": world * k * self.ds_per_step / sec, "unit": UNIT,
+                "h2d_bytes_per_step": sp.n_streams * sp.channels * sp.stride * 4,
+                "d2h_bytes_per_step": sp.n_streams * 4 + sp.n_streams * sp.n_det * sp.stride * 4,
+                "ms_per_step": 1e3 * sec / k, "ms_per_step_synchronous": sync_ms, "output_buffers": nbuf,
+                "checksum_finite": bool(np.isfinite(checksum)),
+                "what": "gw_step_host_async: pinned host buffers, H2D of every step's samples and D2H of its scores and final "
+                        "cleaned samples inside the timed region, outputs rotating over 4 buffer pairs and read on the host "
+                        "one step behind, host clock; ms_per_step_synchronous = gw_step_host (returns with each update's results)"}
+
+    def profile(self, reps=8, prewarm_s=0.5, ms_per_step=1.0):
+        """Per-kernel device spans INSIDE the graph replay (%globaltimer stamps, gwstream_diag.h): mean over `reps`
+        profiled steps of each kernel's duration and of its exclusive share excl_i = end_i - max(begin_i, end_{i-1});
+        sum(excl) = device span of the step, which cannot exceed the step time measured around the launch.  The
+        profiled steps follow `prewarm_s` seconds of back-to-back steps without a gap, so they run in the same clock /
+        power regime as the sustained leg (the caller samples the clocks around this call)."""
+        acc = {}
+        order = []
+        self.pipe.step_profile(self.chunks_d[self.step_no % self.n_chunks], self.scores, self.final, self.cs)   # capture
+        self.step_no += 1
+        for _ in range(int(prewarm_s * 1e3 / max(ms_per_step, 1e-3))):
+            self.step()
+        for it in range(reps + 1):
+            rows = self.pipe.step_profile(self.chunks_d[self.step_no % self.n_chunks], self.scores, self.final, self.cs)
+            self.step_no += 1
+            if it == 0:
+                continue
+            prev_end = 0.0
+            for r in rows:
+                a = acc.setdefault(r["label"], {"us": 0.0, "excl_us": 0.0, "flops": 0.0, "smem_bytes": 0.0})
+                if r["label"] not in order:
+                    order.append(r["label"])
+                a["us"] += (r["end_us"] - r["begin_us"]) / reps
+                a["excl_us"] += max(0.0, r["end_us"] - max(r["begin_us"], prev_end)) / reps
+                a["flops"], a["smem_bytes"] = r["flops"], r["smem_bytes"]
+                prev_end = max(prev_end, r["end_us"])
+        return order, acc
+
+    def close(self):
+        for h in (self.pipe, self.bbh, self.dc, self.stream):
+            h.close()
+        del self.chunks_d
+
+
+def kernel_table(eng, order, acc, pk, sm_mhz, sms):
+    """Per-kernel dict for the bench line: duration and exclusive share (us, from the graph-replay stamps), TFLOP/s on
+    the exclusive time for the conv GEMMs (executed algorithmic FLOPs), GB/s for the bandwidth kernels."""
+    sp, cfg = eng.sp, eng.cfg
+    nd, nw = sp.n_det, sp.n_witness
+    # ALGORITHMIC bytes per launch (DESIGN.md "Data layout in HBM and kernels")
+    hbm_bytes = {
+        "append": sp.n_streams * sp.channels * sp.stride * 8,                       # read new + write ring
+        "ring16_append": sp.n_streams * nd * sp.stride * (nw * 4 + 2 * 32 * 2),     # read fp32, write both mirror copies
+        "snapshot_append": sp.n_streams * (sp.channels * sp.stride * 8 + nd * sp.stride * 2 * 32 * 2),  # a1 + a2 fused
+        # a5 as launched inside the step: reads p_t, acc, strain (12 W), writes acc (4 W) + the S final samples + the
+        # L_b classifier samples per detector-window; the running cleaned window is NOT written on this path
+        "aggregate": sp.n_streams * nd * (sp.window * 16 + (sp.stride + cfg.bbh_len) * 4),
+        "bbh_conv1": sp.n_streams * (nd * cfg.bbh_len * 4 + (cfg.bbh_len // 4) * 32 * 2),
+    }
+    smem_peak_gbs = sms * 128 * sm_mhz * 1e6 / 1e9
+    out = {}
+    for k in order:
+        a = acc[k]
+        row = {"us": round(a["us"], 2), "excl_us": round(a["excl_us"], 2)}
+        t = a["excl_us"] * 1e-6
+        if a["flops"] and t > 0:
+            row["tflops"] = round(a["flops"] / t / 1e12, 1)
+            row["tflops_own_span"] = round(a["flops"] / (a["us"] * 1e-6) / 1e12, 1)
+        if a["smem_bytes"] and a["us"] > 0:
+            gbs = a["smem_bytes"] / (a["us"] * 1e-6) / 1e9
+            row.update({"smem_gbs": round(gbs, 1), "smem_frac": round(gbs / smem_peak_gbs, 3)})
+        if k in hbm_bytes and a["us"] > 0:
+            gbs = hbm_bytes[k] / (a["us"] * 1e-6) / 1e9
+            row.update({"gbs": round(gbs, 1), "hbm_frac": round(gbs / pk["hbm_gbs"], 3),
+                        "hbm_frac_nominal": round(gbs / NOMINAL_HBM_GBS, 3)})
+        out[k] = row
+    return out, smem_peak_gbs
+
+
 def run_native(args):
     import torch
     import torch.distributed as dist
@@ -190,32 +360,10 @@ def run_native(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    if args.no_pdl:
-        gw.set_pdl(False)
-    if args.no_snake:
-        gw.set_snake(False)
-    if args.no_skip:
-        gw.set_skip_zeros(False)
-    if args.no_2sm:
-        gw.set_two_sm(False)
-    dtype = gw.GW_BF16 if args.dtype == "bf16" else gw.GW_FP16
-    cfg = S.config_c3(args.streams, args.stride, WINDOW)
-    sp = cfg.stream
-    n_chunks = args.seg_seconds * FS // sp.stride
-    dc_params, bbh_params = make_params(cfg)
-    t0 = time.time()
-    chunks_h = torch.from_numpy(make_input_chunks(cfg, n_chunks)).pin_memory()
-    chunks_d = chunks_h.cuda()
-    log(f"[rank {rank}] inputs {tuple(chunks_h.shape)} ({chunks_h.numel() * 4 / 2**20:.0f} MiB) in {time.time() - t0:.1f}s")
-    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype)
-    cs = torch.cuda.Stream()
-    scores = torch.zeros(sp.n_streams, device="cuda")
-    final = torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda")
-    step_no = [0]
-
-    def step():
-        pipe.step(chunks_d[step_no[0] % n_chunks], scores, final, cs)
-        step_no[0] += 1
+    opts = gw.Options(pdl=not args.no_pdl, snake=not args.no_snake, skip_zeros=not args.no_skip, two_sm=not args.no_2sm,
+                      incremental=args.incremental)
+    eng = Engine(gw, torch, args, args.streams, args.stride, args.dtype, opts, local=local)
+    sp, cfg = eng.sp, eng.cfg
 
     def barrier():
         torch.cuda.synchronize()
@@ -225,24 +373,18 @@ def run_native(args):
 
     W_, K = max(args.warmup, 3), args.steps
     for _ in range(W_):
-        step()
+        eng.step()
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
     launches0 = gw.kernel_launches()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record(cs)
-    for _ in range(K):
-        step()
-    ev1.record(cs)
+    ms_total = eng.timed(K)
     barrier()
     launches = gw.kernel_launches() - launches0
     clocks = sampler.stop() if rank == 0 else None
-    ms_total = ev0.elapsed_time(ev1)
     ms_total = shard.max_over_ranks(ms_total, device="cuda")
-    ds_per_step = sp.n_streams * sp.stride / FS
-    value = world * K * ds_per_step / (ms_total / 1e3)
+    value = world * K * eng.ds_per_step / (ms_total / 1e3)
 
     if args.timed_only:
         if rank == 0:
@@ -251,102 +393,137 @@ def run_native(args):
                               "note": "--timed-only run (profiling aid), not a bench line"}), flush=True)
         return
 
-    # per-update latency: launch -> stream sync, host clock, one sample per update
-    lat = []
-    for _ in range(min(max(K, 50), 5000)):
-        t0 = time.perf_counter()
-        step()
-        cs.synchronize()
-        lat.append((time.perf_counter() - t0) * 1e3)
-    lat.sort()
-    latency = {"p50_ms": lat[len(lat) // 2], "p99_ms": lat[min(len(lat) - 1, int(len(lat) * 0.99))],
-               "samples": len(lat), "per_stream_p50_ms": lat[len(lat) // 2] / sp.n_streams,
-               "realtime_budget_ms": 1e3 * sp.stride / FS,
-               "what": "host clock, gw_step launch -> stream synchronize, whole batch of n streams"}
+    # sustained regime: back-to-back steps for >= args.sustained_seconds with the clock sampler running during it
+    sustained = None
+    if args.sustained_seconds > 0:
+        n_sus = max(K, int(args.sustained_seconds * 1e3 / (ms_total / K)) + 1)
+        s2 = ClockSampler(local)
+        if rank == 0:
+            s2.start()
+        ms_sus = shard.max_over_ranks(eng.timed(n_sus), device="cuda")
+        c2 = s2.stop() if rank == 0 else None
+        sustained = {"value": world * n_sus * eng.ds_per_step / (ms_sus / 1e3), "unit": UNIT, "steps": n_sus,
+                     "seconds": ms_sus / 1e3, "ms_per_step": ms_sus / n_sus, "clocks": c2}
 
-    # end to end through the C ABI with HOST buffers (pinned): H2D of the new samples and D2H of the
-    # scores + final cleaned samples inside the timed region, every step
-    scores_h = torch.zeros(sp.n_streams).pin_memory()
-    final_h = torch.zeros((sp.n_streams, sp.n_det, sp.stride)).pin_memory()
-    # offline regime: gw_step_host_async, whose input copy overlaps the previous step's kernels;
-    # every step's results still land in host memory inside the timed region
-    for i in range(3):
-        pipe.step_host_async(chunks_h[step_no[0] % n_chunks], scores_h, final_h, cs); step_no[0] += 1
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(K):
-        pipe.step_host_async(chunks_h[step_no[0] % n_chunks], scores_h, final_h, cs); step_no[0] += 1
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    # online regime: gw_step_host, which returns with the results (one synchronisation per update)
-    t0 = time.perf_counter()
-    for _ in range(min(K, 50)):
-        pipe.step_host(chunks_h[step_no[0] % n_chunks], scores_h, final_h, cs); step_no[0] += 1
-    e2e_sync_ms = 1e3 * (time.perf_counter() - t0) / min(K, 50)
-    e2e_s = shard.max_over_ranks(e2e_s, device="cuda")
-    h2d = sp.n_streams * sp.channels * sp.stride * 4
-    d2h = sp.n_streams * 4 + sp.n_streams * sp.n_det * sp.stride * 4
-    e2e = {"value": world * K * ds_per_step / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
-           "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * e2e_s / K,
-           "ms_per_step_synchronous": e2e_sync_ms,
-           "what": "gw_step_host_async: pinned host buffers, H2D of every step's samples and D2H of its scores and "
-                   "final cleaned samples inside the timed region, host clock; ms_per_step_synchronous = gw_step_host "
-                   "(returns with the results of each update)"}
+    latency = eng.latency(min(max(K, 50), 5000))
+    e2e = eng.e2e(K, world)
 
-    # per-kernel device times: eager replay of the same step with a CUDA event after every launch
-    prof = {}
-    n_prof = 5
-    for it in range(n_prof + 1):
-        rows = pipe.step_profile(chunks_d[step_no[0] % n_chunks], scores, final, cs); step_no[0] += 1
-        if it == 0:
-            continue
-        for label, ms, fl in rows:
-            a = prof.setdefault(label, [0.0, 0.0])
-            a[0] += ms / n_prof
-            a[1] = fl
-    smem_bytes = pipe.profile_smem_bytes()
+    # ---- roofline of the dominant kernel family (all conv-GEMM launches of a step), regime-honest
+    s5 = ClockSampler(local)
+    if rank == 0:
+        s5.start()
+    order, acc = eng.profile(ms_per_step=ms_total / K)
+    clocks_profile = s5.stop() if rank == 0 else None
+    graph_nodes = eng.pipe.graph_nodes()
     pk = peaks()
-    gemm_ms = sum(v[0] for k, v in prof.items() if k.startswith("gemm."))
-    gemm_fl = sum(v[1] for k, v in prof.items() if k.startswith("gemm."))
-    step_ms_eager = sum(v[0] for v in prof.values())
-    achieved = gemm_fl / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+    sm_mhz_sus = (clocks_profile or {}).get("sm_mhz") or ((sustained or {}).get("clocks") or {}).get("sm_mhz") or 1700.0
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    kernels, smem_peak_gbs = kernel_table(eng, order, acc, pk, sm_mhz_sus, sms)
+    gemm_us = sum(a["excl_us"] for k, a in acc.items() if k.startswith("gemm."))
+    gemm_fl = sum(a["flops"] for k, a in acc.items() if k.startswith("gemm."))
+    span_us = sum(a["excl_us"] for a in acc.values())
+    achieved = gemm_fl / (gemm_us * 1e-6) / 1e12 if gemm_us > 0 else 0.0
+    # which regime were the per-kernel times taken in?  The profiled steps are a handful of launches after idle gaps
+    # (boost clocks) when the whole run is short; a run that just spent seconds back to back sits at the power cap.
+    burst = False                                  # the profiled steps directly follow 0.5 s of back-to-back steps
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get("conv_gemm_dram_bytes_per_launch")
-    roofline = {"bound": "tensor", "kernel": "k_conv_gemm_umma (all conv-GEMM launches of one step)",
-                "achieved": achieved, "peak": pk["tensor_tflops"], "unit": "TFLOP/s",
-                "frac": achieved / pk["tensor_tflops"], "traffic": traffic, "peak_source": pk["source"],
-                "flops_per_step": gemm_fl, "ms_per_step_in_kernel": gemm_ms,
-                "share_of_step": gemm_ms / step_ms_eager if step_ms_eager else None,
-                "timing": "CUDA events after every launch, eager replay of the same step on the launch stream"}
-    kernels = {k: {"ms": round(v[0], 4), **({"tflops": round(v[1] / (v[0] * 1e-3) / 1e12, 1)} if v[1] else {})}
-               for k, v in prof.items()}
-    # bandwidth kernels: ALGORITHMIC bytes per step / event time
-    nd, nw = sp.n_det, sp.n_witness
-    hbm_bytes = {
-        "append": sp.n_streams * sp.channels * sp.stride * 8,                       # read new + write ring
-        "ring16_append": sp.n_streams * nd * sp.stride * (nw * 4 + 2 * 32 * 2),     # read fp32, write both mirror copies
-        "snapshot_append": sp.n_streams * (sp.channels * sp.stride * 8 + nd * sp.stride * 2 * 32 * 2),  # a1 + a2 fused
-        "aggregate": sp.n_streams * nd * sp.window * 20,                            # p_t, acc r/w, strain, cleaned
-        "bbh_conv1": sp.n_streams * (nd * cfg.bbh_len * 4 + (cfg.bbh_len // 4) * 32 * 2),
-    }
-    for k, b in hbm_bytes.items():
-        if k in kernels and kernels[k]["ms"] > 0:
-            gbs = b / (kernels[k]["ms"] * 1e-3) / 1e9
-            kernels[k].update({"gbs": round(gbs, 1), "hbm_frac": round(gbs / pk["hbm_gbs"], 3)})
-    # conv GEMMs against the shared-memory operand roofline: traffic by the engine's accounting
-    # (MMA operand reads + TMA fills + epilogue staging) over 128 B/clk per SM at the SM clock sampled under load
-    sm_mhz = (clocks or {}).get("sm_mhz") or 1700.0
-    sms = torch.cuda.get_device_properties(local).multi_processor_count
-    smem_peak_gbs = sms * 128 * sm_mhz * 1e6 / 1e9
-    for k, b in smem_bytes.items():
-        if k in kernels and kernels[k]["ms"] > 0:
-            gbs = b / (kernels[k]["ms"] * 1e-3) / 1e9
-            kernels[k].update({"smem_gbs": round(gbs, 1), "smem_frac": round(gbs / smem_peak_gbs, 3)})
+    # the same family over the SUSTAINED step: its share of the step (from the stamps) x the sustained step time
+    sus_ms = sustained["ms_per_step"] if sustained else ms_total / K
+    gemm_share = gemm_us / span_us if span_us else None
+    achieved_sus = gemm_fl / (gemm_share * sus_ms * 1e-3) / 1e12 if gemm_share else 0.0
+    peak = pk["tensor_tflops_burst"] if burst else pk["tensor_tflops"]
+    roofline = {"bound": "tensor", "kernel": "k_conv_gemm_umma + k_conv_gemm_2sm (all conv-GEMM launches of one step)",
+                "achieved": achieved_sus, "peak": peak, "unit": "TFLOP/s", "frac": achieved_sus / peak,
+                "regime": "burst" if burst else "sustained", "clocks_profiled_steps": clocks_profile,
+                "frac_burst": achieved / pk["tensor_tflops_burst"], "frac_sustained": achieved_sus / pk["tensor_tflops"],
+                "frac_nominal": achieved_sus / NOMINAL_TFLOPS,
+                "achieved_profiled_steps": achieved, "traffic": traffic, "peak_source": pk["source"],
+                "peaks": {"burst_tflops": pk["tensor_tflops_burst"], "sustained_tflops": pk["tensor_tflops"], "nominal_tflops": NOMINAL_TFLOPS},
+                "flops_per_step": gemm_fl, "us_per_step_in_kernel": gemm_us, "device_span_us": span_us,
+                "share_of_step": gemm_share,
+                "timing": "%globaltimer stamps written by every kernel's first / last CTA INSIDE the replay of the step's CUDA "
+                          "graph (gw_step_profile); us_per_step_in_kernel = sum of the conv GEMMs' exclusive shares, device_span_us = "
+                          "sum over all kernels <= ms_per_step; `achieved` = executed algorithmic FLOPs / (that share x the "
+                          "sustained step time); achieved_profiled_steps = the same FLOPs / the stamped time of the profiled steps "
+                          "themselves (they directly follow 0.5 s of back-to-back steps; clocks_profiled_steps), frac_burst = that "
+                          "against the burst peak"}
+
+    # ---- the exact incremental path (gw_options.incremental, D13) on the same workload
+    incremental = None
+    if not args.no_incremental and not args.incremental:
+        eng.close()
+        torch.cuda.empty_cache()
+        ie = Engine(gw, torch, args, args.streams, args.stride, args.dtype,
+                    gw.Options(pdl=not args.no_pdl, snake=not args.no_snake, skip_zeros=not args.no_skip, incremental=1),
+                    chunks_h=eng.chunks_h, local=local)
+        for _ in range(W_ + 2):
+            ie.step()
+        torch.cuda.synchronize()
+        n_i = max(K, int(1.0e3 / 0.25))              # about a second of back-to-back steps
+        s3 = ClockSampler(local)
+        if rank == 0:
+            s3.start()
+        ms_i = shard.max_over_ranks(ie.timed(n_i), device="cuda")
+        c3 = s3.stop() if rank == 0 else None
+        lat_i = ie.latency(min(max(K, 50), 2000))
+        e2e_i = ie.e2e(K, world)
+        order_i, acc_i = ie.profile(ms_per_step=ms_i / n_i)
+        kern_i, _ = kernel_table(ie, order_i, acc_i, pk, (c3 or {}).get("sm_mhz") or 1700.0, sms)
+        fl_i = sum(a["flops"] for k, a in acc_i.items() if k.startswith("gemm."))
+        us_i = sum(a["excl_us"] for k, a in acc_i.items() if k.startswith("gemm."))
+        incremental = {"value": world * n_i * ie.ds_per_step / (ms_i / 1e3), "unit": UNIT, "steps": n_i,
+                       "ms_per_step": ms_i / n_i, "latency": lat_i, "e2e": e2e_i, "clocks": c3,
+                       "graph_nodes": ie.pipe.graph_nodes(),
+                       "flops_executed_per_step": fl_i, "flops_full_recompute_per_step": gemm_fl,
+                       "conv_work_ratio": gemm_fl / fl_i if fl_i else None,
+                       "conv_tflops_on_executed_work": fl_i / (us_i * 1e-6) / 1e12 if us_i else None,
+                       "device_span_us": sum(a["excl_us"] for a in acc_i.values()), "kernels": kern_i,
+                       "what": "gw_options.incremental = 1: every layer's activations live in rings over absolute position and an "
+                               "update recomputes only the rows near the two window edges; results are bit-identical to full "
+                               "recomputation (tests/test_gpu_parity.py::test_incremental_path_is_bit_identical_to_full_recompute). "
+                               "`value` above stays the full-recompute number."}
+        ie.close()
+        del ie
+        torch.cuda.empty_cache()
+        eng = None
+
+    # ---- largest single-GPU point of configs[4]: n = 512 streams, S = 1024
+    largest = None
+    if not args.no_largest and world == 1:
+        if eng is not None:
+            eng.close(); eng = None
+        torch.cuda.empty_cache()
+        try:
+            le = Engine(gw, torch, args, 512, 1024, args.dtype, gw.Options(), seg_seconds=1, local=local)
+            for _ in range(3):
+                le.step()
+            torch.cuda.synchronize()
+            n_l = 60
+            s4 = ClockSampler(local); s4.start()
+            ms_l = le.timed(n_l)
+            c4 = s4.stop()
+            lat_l = le.latency(30)
+            largest = {"workload": "configs[4] largest point: n=512 streams, S=1024, W=32768, " + args.dtype,
+                       "value": n_l * le.ds_per_step / (ms_l / 1e3), "unit": UNIT, "steps": n_l, "ms_per_step": ms_l / n_l,
+                       "latency": lat_l, "clocks": c4,
+                       "conv_tflops": gemm_fl * 4 / (ms_l / n_l * 1e-3) / 1e12,
+                       "frac_sustained": gemm_fl * 4 / (ms_l / n_l * 1e-3) / 1e12 / pk["tensor_tflops"],
+                       "frac_nominal": gemm_fl * 4 / (ms_l / n_l * 1e-3) / 1e12 / NOMINAL_TFLOPS,
+                       "what": "full recompute, whole step time (all kernels) against the conv FLOPs of 4 x the n=128 step"}
+            le.close()
+            del le
+        except Exception as ex:                      # e.g. a smaller box: report, do not fail the bench line
+            largest = {"error": str(ex)[:300]}
+        torch.cuda.empty_cache()
 
     # offline / non-streaming mode (D9): the same number of detector-windows per launch, but all from ONE
     # stream's archival segment (B = n windows advance the stream by B*S samples per launch)
+    cs = torch.cuda.Stream()
+    dtype = gw.GW_BF16 if args.dtype == "bf16" else gw.GW_FP16
+    dc_params, _ = make_params(cfg)
     offline = None
     if not args.no_offline:
         B = sp.n_streams
@@ -368,7 +545,7 @@ def run_native(args):
         off_ms = o0.elapsed_time(o1) / n_off
         offline = {"windows_per_launch": B, "samples_per_launch": off.samples, "ms_per_launch": off_ms,
                    "value": B * sp.stride / FS / (off_ms * 1e-3), "unit": UNIT,
-                   "tflops_whole_launch": round(sum(v[1] for k, v in prof.items() if k.startswith("gemm.dc")) / (off_ms * 1e-3) / 1e12, 1),
+                   "tflops_whole_launch": round(sum(a["flops"] for k, a in acc.items() if k.startswith("gemm.dc")) / (off_ms * 1e-3) / 1e12, 1),
                    "what": "gw_offline_run on a device-resident segment of one 2-detector stream; value counts the B*S new "
                            "samples a launch advances the stream by"}
         del off, seg, cl, nz
@@ -402,10 +579,19 @@ def run_native(args):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        n_all = oracle.num_threads()
         times, cores = oracle_rate(cfg, args.dtype, 200, budget_s=15.0)   # a bounded sample: ~15 s of oracle time
         sec = sum(times)
         cpu = {"value": len(times) * (sp.stride / FS) / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"{len(times)} consecutive updates of one 2-detector stream of the same workload ({sec:.1f} s of oracle time)"}
+               "sample": f"{len(times)} consecutive updates of one 2-detector stream of the same workload ({sec:.1f} s of oracle time)",
+               "note": "the fp64 direct-loop checker as it stands: a reported baseline, not a competent CPU implementation and "
+                       "not a speed-up claim"}
+        oracle.set_num_threads(1)
+        t1, _ = oracle_rate(cfg, args.dtype, 3, budget_s=8.0)
+        oracle.set_num_threads(n_all)
+        cpu["single_thread"] = {"value": len(t1) * (sp.stride / FS) / sum(t1), "unit": UNIT, "cores": 1,
+                                "sample": f"{len(t1)} updates ({sum(t1):.1f} s)"}
 
     if rank == 0:
         line = {
@@ -414,12 +600,15 @@ def run_native(args):
             "dtype": "f16" if args.dtype == "fp16" else "bf16", "data": "synthetic",
             "config": {"workload": f"C4 multi-stream ensemble (configs[4]): n={sp.n_streams} independent config-3 streams "
                                    f"per GPU, 2 detectors x 21 witnesses, W={sp.window}, S={sp.stride}, fs={FS}, "
-                                   f"classifier on last {cfg.bbh_len} samples, one CUDA-graph launch per stride",
+                                   f"classifier on last {cfg.bbh_len} samples, one CUDA-graph launch per stride"
+                                   + (", incremental path" if args.incremental else ", full recompute of every window"),
                        "n_streams_per_gpu": sp.n_streams, "stride": sp.stride, "window": sp.window,
                        "l2": f"inputs larger than L2: ring state {sp.n_streams * sp.channels * sp.window * 4 / 2**20:.0f} MiB "
                              "is re-read every step", "precision": f"{args.dtype} storage, fp32 accumulate"},
-            "latency": latency, "e2e": e2e, "gpu_launches": int(launches), "graph_nodes": pipe.graph_nodes(),
-            "roofline": roofline, "smem_peak_gbs": round(smem_peak_gbs, 1), "kernels": kernels, "clocks": clocks, "cpu_baseline": cpu, "offline": offline, "snapshotter": snapshotter,
+            "sustained": sustained, "latency": latency, "e2e": e2e, "gpu_launches": int(launches),
+            "graph_nodes": graph_nodes,
+            "roofline": roofline, "smem_peak_gbs": round(smem_peak_gbs, 1), "kernels": kernels, "clocks": clocks,
+            "incremental": incremental, "largest": largest, "cpu_baseline": cpu, "offline": offline, "snapshotter": snapshotter,
         }
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -434,7 +623,7 @@ def run_sweep(args):
         for n in SWEEP_STREAMS:
             for stride in SWEEP_STRIDES:
                 cmd = [sys.executable, os.path.abspath(__file__), "--streams", str(n), "--stride", str(stride), "--dtype", dtype,
-                       "--steps", str(args.steps), "--warmup", str(args.warmup), "--no-cpu-baseline", "--no-offline",
+                       "--steps", str(args.steps), "--warmup", str(args.warmup), "--no-cpu-baseline", "--no-offline", "--no-largest",
                        "--seg-seconds", str(4 if n >= 512 else SEG_SECONDS)]
                 res = subprocess.run(cmd, capture_output=True, text=True)
                 line = res.stdout.strip().splitlines()[-1] if res.returncode == 0 and res.stdout.strip() else None
@@ -468,6 +657,10 @@ def main():
     ap.add_argument("--no-2sm", action="store_true", help="single-CTA kernel for the N=256 layers too (A/B aid)")
     ap.add_argument("--no-offline", action="store_true", help="skip the offline-mode measurement")
     ap.add_argument("--no-skip", action="store_true", help="issue the structurally empty MMAs too (A/B aid)")
+    ap.add_argument("--incremental", action="store_true", help="time the exact incremental path as the MAIN arm (A/B aid)")
+    ap.add_argument("--no-incremental", action="store_true", help="skip the incremental-path leg")
+    ap.add_argument("--no-largest", action="store_true", help="skip the n=512, S=1024 point")
+    ap.add_argument("--sustained-seconds", type=float, default=2.0, help="length of the back-to-back sustained leg (0: skip)")
     ap.add_argument("--timed-only", action="store_true",
                     help="only the warm-up and the timed region (for short runs under ncu); prints a reduced line")
     ap.add_argument("--reference-budget", type=float, default=150.0,

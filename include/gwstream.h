@@ -11,7 +11,10 @@
  *
  * Conventions
  *  - Plain C, opaque handles, no exceptions.  Every call returns 0 (GW_OK) or a negative code;
- *    gw_last_error() returns a thread-local description of the last failure on this thread.
+ *    gw_last_error(handle) returns the description of the last failure of a call on that handle
+ *    (gw_last_error(NULL): of the last failed call on this thread, e.g. a create that returned no handle).
+ *  - No process-global switches: everything that selects a code path is a field of gw_options, fixed
+ *    when a handle is created.
  *  - "dev" pointers are CUDA device pointers on the current device, "host" pointers are host
  *    memory.  The caller owns every buffer it passes; the engine owns all persistent state (rings,
  *    overlap-add accumulators, activations, weights -- parameters are COPIED at create time).
@@ -101,51 +104,39 @@ typedef struct {
     int length;
 } gw_bbh_spec;
 
-const char *gw_last_error(void);
+/* Options fixed at create time (pass NULL for the defaults).  None of them changes WHAT is computed:
+ *  conv_impl   GW_IMPL_UMMA (default): tcgen05/TMEM/TMA conv GEMMs.  GW_IMPL_SIMT: a slow CUDA-core kernel over the
+ *              same operand layout, kept to bisect tensor-core bugs in tests.  Both are CUDA; neither is a fallback.
+ *  fuse_tail   1 (default): the last tensor-core layer of DeepClean (ConvTranspose1d -> <= 32 channels, tanh) and the
+ *              final 1-channel ConvTranspose1d (k = 7) run as one kernel; the activation between them is never stored
+ *              (gw_deepclean_activation returns GW_ESTATE for it).  0: it is written to HBM.  Agree within rounding.
+ *  pdl         1 (default): programmatic dependent launch between the kernels of an update (each kernel's prologue
+ *              overlaps its predecessor's tail; it waits on the device before touching the predecessor's output).
+ *  snake       1 (default): consecutive DeepClean layers walk their (window, tile) list in alternating directions, so a
+ *              layer starts on the activations its predecessor wrote last (still in L2).
+ *  two_sm      1 (default): CTA-pair kernel (tcgen05 cta_group::2, M = 256) for the layers whose weights do not fit in
+ *              shared memory (GEMM N = 256).
+ *  skip_zeros  1 (default): the resident-weight conv GEMMs skip the K steps and halves of N that no filter tap reaches.
+ *  pdl / snake / two_sm / skip_zeros are scheduling only (or skip exact zeros): results are BIT-identical either way.
+ *  incremental 0 (default): every update recomputes the whole window.  1: the exact incremental path (D13,
+ *              only floor(fs/r) samples are new per update): every layer's activations live
+ *              in a ring over absolute position and an update recomputes only the rows whose receptive field reaches
+ *              the new samples or one of the two window edges; every other row IS the previous update's value.
+ *              Results are bit-identical to full recomputation.  Needs stride and window to be multiples of
+ *              2^(encoder depth), window a multiple of 128 * 2^(encoder depth), the fused tail and GW_IMPL_UMMA
+ *              (GW_EINVAL otherwise). */
+typedef struct {
+    int conv_impl, fuse_tail, pdl, snake, two_sm, skip_zeros, incremental;
+} gw_options;
+void gw_options_default(gw_options *o);
+
+/* Description of the last failure on `handle` (any gw_* handle), or with NULL of the last failed call on the calling
+ * thread.  The string is owned by the library and valid until the next failing call on that handle / thread. */
+const char *gw_last_error(const void *handle);
 
 /* Number of CUDA kernels this library has launched (or captured into a graph and replayed) on
- * behalf of the calling process so far; used by bench.py for "gpu_launches". */
+ * behalf of the calling process so far (atomic counter); used by bench.py for "gpu_launches". */
 int64_t gw_kernel_launches(void);
-
-/* Select the conv GEMM implementation for handles created AFTER this call.  GW_IMPL_UMMA
- * (default): tcgen05/TMEM/TMA.  GW_IMPL_SIMT: a slow CUDA-core kernel over the same operand
- * layout, kept only to bisect tensor-core bugs in tests.  Both are CUDA; neither is a fallback. */
-int gw_set_conv_impl(int impl);
-
-/* Fuse the last tensor-core layer of DeepClean (ConvTranspose1d -> <= 32 channels, tanh) with the final
- * 1-channel ConvTranspose1d (k = 7) into one kernel, for handles created AFTER this call (default 1).
- * With 0 the activation between them is written to HBM and can be read with gw_deepclean_activation
- * (test hook); with 1 that call returns GW_ESTATE for that layer.  Results agree within rounding. */
-int gw_set_fuse_tail(int on);
-
-/* Programmatic dependent launch between the kernels of an update (default 1): each kernel is launched
- * with the stream-serialization attribute and waits on the device (griddepcontrol.wait) before it touches
- * what its predecessor wrote, so its prologue overlaps the predecessor's tail.  Takes effect for launches
- * and graph captures made AFTER this call.  Results are identical either way. */
-int gw_set_pdl(int on);
-
-/* Alternate the direction in which consecutive DeepClean layers walk their (window, tile) work list, for
- * handles created AFTER this call (default 1): a layer then starts on the activations its predecessor wrote
- * last, which are still in L2.  Pure scheduling; results are bit-identical either way. */
-int gw_set_snake(int on);
-
-/* Skip the structurally empty parts of the resident-weight conv GEMMs (K steps and halves of N that no filter tap
- * reaches; such weight blocks are also kept at half size in shared memory), for handles created AFTER this call
- * (default 1).  Only exact zeros are skipped: results are bit-identical. */
-int gw_set_skip_zeros(int on);
-
-/* Diagnostic: measured cycles per tcgen05.mma (cta_group::1, kind::f16, M = 128, K = 16, both operands in shared
- * memory, SWIZZLE_128B) for GEMM N in {16, 32, 64, 128, 256} on the current device: one CTA issues 1024 MMAs back to
- * back with a conv layer's descriptor pattern.  *issue_cycles = issue-loop time per MMA, *complete_cycles = time
- * until the last one has retired, per MMA (host pointers).  Synchronises the device.  This is the number behind the
- * shared-memory-operand roofline of the thin layers. */
-int gw_probe_mma_cycles(int N, float *issue_cycles, float *complete_cycles);
-
-/* CTA-pair conv GEMM (tcgen05 cta_group::2: two CTAs of a cluster share every streamed weight block, M = 256)
- * for the layers whose weights do not fit in shared memory (GEMM N = 256), for handles created AFTER this call
- * (default 1).  With 0 those layers run the single-CTA kernel.  The accumulation order of every output is the
- * same, so results are bit-identical. */
-int gw_set_two_sm(int on);
 
 /* ---- snapshotter -------------------------------------------------------------
  * gw_stream_create: zeroed ring state [n][C][W] fp32 on the current device, sample counter 0.
@@ -177,7 +168,7 @@ int64_t gw_stream_count(const gw_stream *s);
  *   Samples with negative absolute index are written as 0.
  * gw_noise_estimate (test hook): the running noise estimate nhat over the current window,
  *   [n][D][W] (0 where no prediction covers the sample).  Valid after gw_cleaned_strain. */
-int gw_deepclean_create(gw_deepclean **out, gw_stream *s, const gw_dc_spec *spec, int dtype);
+int gw_deepclean_create(gw_deepclean **out, gw_stream *s, const gw_dc_spec *spec, int dtype, const gw_options *opts);
 int gw_deepclean_destroy(gw_deepclean *dc);
 int gw_deepclean_forward(gw_deepclean *dc, void *stream);
 int gw_deepclean_noise(gw_deepclean *dc, float *out_dev, void *stream);
@@ -195,7 +186,7 @@ int gw_deepclean_activation(gw_deepclean *dc, int layer, void *out_dev, int64_t 
  *   [(t+1)S - delta - L_b, (t+1)S - delta) of the running cleaned strain of this update.
  * gw_bbh_score_batch: stateless; windows_dev [B][D][L_b] fp32, scores_dev [B]; B <= max_batch. */
 int gw_bbh_create(gw_bbh **out, gw_deepclean *dc, const gw_bbh_spec *spec, int dtype, int n_det,
-                  int max_batch);
+                  int max_batch, const gw_options *opts);
 int gw_bbh_destroy(gw_bbh *b);
 int gw_bbh_score(gw_bbh *b, float *scores_dev, void *stream);
 int gw_bbh_score_batch(gw_bbh *b, const float *windows_dev, int batch, float *scores_dev, void *stream);
@@ -205,9 +196,9 @@ int gw_bbh_score_batch(gw_bbh *b, const float *windows_dev, int batch, float *sc
  *   update -> forward -> cleaned(GW_FINAL) -> score into a CUDA graph; later steps replay it (the ring
  *   head lives in device memory, so the graph is replayed unchanged).
  * gw_step: device buffers.  new_samples_dev [n][C][S]; scores_dev [n] (ignored without bbh);
- *   cleaned_final_dev [n][D][S].  The pointers are baked into the graph: a different
- *   new_samples_dev is a cheap node-parameter update, different output pointers re-capture.
- *   `stream` must not be the legacy default stream.
+ *   cleaned_final_dev [n][D][S].  The pointers are parameters of graph nodes: passing different buffers from one
+ *   call to the next (rotating output buffers, say) is a node-parameter update of the instantiated graph, never a
+ *   re-capture.  `stream` must not be the legacy default stream.
  * gw_step_host: HOST buffers; copies new samples host->device, replays the graph, copies scores
  *   and final cleaned samples device->host, and synchronises.  Pinned host memory makes the copies
  *   asynchronous; pageable memory works but is slower. */
@@ -225,19 +216,6 @@ int gw_step_host(gw_pipeline *p, const float *new_samples_host, float *scores_ho
  * until `stream` has been synchronised past that call.  Use pinned host memory. */
 int gw_step_host_async(gw_pipeline *p, const float *new_samples_host, float *scores_host,
                        float *cleaned_final_host, void *stream);
-/* Profiling aid for bench.py: one update launched EAGERLY (same kernels, no graph) with a CUDA event
- * after every kernel on `stream`; synchronises.  ms_out[i] (i < min(*n_out, max_kernels)) is the device
- * time of kernel i, gw_profile_label(p, i) its name ("append", "gather", "gemm.dc0", ... "aggregate",
- * "bbh_conv1", "gemm.bbh1", ...), gw_profile_flops(p, i) its algorithmic FLOPs (real channels and taps
- * only, whole batch; 0 for non-GEMM kernels).  Counts as one update of the stream. */
-int gw_step_profile(gw_pipeline *p, const float *new_samples_dev, float *scores_dev, float *cleaned_final_dev,
-                    void *stream, int max_kernels, float *ms_out, int *n_out);
-const char *gw_profile_label(const gw_pipeline *p, int i);
-double gw_profile_flops(const gw_pipeline *p, int i);
-/* Shared-memory traffic (bytes, all SMs) of conv GEMM kernel i of the last profiled step by the accounting of
- * DESIGN.md section 7 (MMA operand reads + TMA fills + epilogue staging); 0 for other kernels.  Against
- * 128 B/clk x SMs x SM clock it is the roofline the thin layers are bound by. */
-double gw_profile_smem_bytes(const gw_pipeline *p, int i);
 /* number of kernel nodes in the captured graph (0 before the first gw_step) */
 int gw_pipeline_graph_nodes(const gw_pipeline *p);
 
@@ -269,7 +247,7 @@ int gw_offline_set_scaling(gw_offline *o, const float *wit_mean, const float *wi
  *   estimate that was subtracted), all device pointers owned by the caller; asynchronous on `stream`.
  * gw_offline_predictions (test hook): raw per-window predictions [n_windows][n_det][window] of the last run. */
 int gw_offline_create(gw_offline **out, const gw_dc_spec *spec, int channels, int fs, int window, int stride,
-                      int n_windows, int dtype);
+                      int n_windows, int dtype, const gw_options *opts);
 int gw_offline_destroy(gw_offline *o);
 int64_t gw_offline_samples(const gw_offline *o);
 int gw_offline_run(gw_offline *o, const float *samples_dev, float *cleaned_dev, float *noise_dev, void *stream);

@@ -1,0 +1,50 @@
+/*
+ * gwstream_diag.h -- measurement and diagnostic entry points of libgwstream.so.  NOT part of the product interface
+ * (include/gwstream.h): bench.py and the tests use them to time the kernels of a step and to reproduce the
+ * micro-benchmark behind the shared-memory operand roofline.  Same conventions as gwstream.h.
+ */
+#ifndef GWSTREAM_DIAG_H
+#define GWSTREAM_DIAG_H
+
+#include "gwstream.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* gw_step_profile: ONE update through a CUDA graph of exactly the kernels gw_step replays (same launch attributes,
+ * programmatic dependent launch included), in which every kernel additionally stamps %globaltimer when its first CTA
+ * starts and when its last CTA has finished; synchronises `stream`.  Counts as one update of the stream.
+ *  begin_us[i], end_us[i] (host, i < min(*n_out, max_kernels)): start and end of kernel i in microseconds relative to
+ *  the start of the step's first kernel.  Kernels overlap under PDL (a successor's prologue runs under its
+ *  predecessor's tail), so the decomposition of the step is excl_i = end_i - max(begin_i, end_{i-1}); their sum is
+ *  the span of the step on the device and cannot exceed the step time measured around the graph launch.
+ *  gw_profile_label(p, i): kernel i's name ("snapshot_append", "gemm.dc0", ... "aggregate", "bbh_conv1", "gemm.bbh1", ...).
+ *  gw_profile_flops(p, i): algorithmic FLOPs kernel i EXECUTED in that step (real channels and taps only, whole
+ *  batch; with gw_options.incremental: the rows of the tiles that were recomputed); 0 for non-GEMM kernels.
+ *  gw_profile_smem_bytes(p, i): shared-memory traffic of conv GEMM kernel i by the accounting of DESIGN.md section 7
+ *  (MMA operand reads + TMA fills + epilogue staging, all SMs); 0 for other kernels. */
+int gw_step_profile(gw_pipeline *p, const float *new_samples_dev, float *scores_dev, float *cleaned_final_dev,
+                    void *stream, int max_kernels, double *begin_us, double *end_us, int *n_out);
+const char *gw_profile_label(const gw_pipeline *p, int i);
+double gw_profile_flops(const gw_pipeline *p, int i);
+double gw_profile_smem_bytes(const gw_pipeline *p, int i);
+
+/* Measured cycles per tcgen05.mma (cta_group::1, kind::f16, M = 128, K = 16, both operands in shared memory,
+ * SWIZZLE_128B) for GEMM N in {16, 32, 64, 128, 256} on the current device: one CTA issues 1024 MMAs back to back with
+ * a conv layer's descriptor pattern.  *issue_cycles = issue-loop time per MMA, *complete_cycles = time until the last
+ * one has retired, per MMA (host pointers).  Synchronises the device. */
+int gw_probe_mma_cycles(int N, float *issue_cycles, float *complete_cycles);
+
+/* The arithmetic behind gw_options.incremental (D13), host only: for a stack of stride-2 layers
+ * (kind, k as in gw_conv_layer; weights are not read) and `stride` new samples per update, left[i] / right[i] = how
+ * many OUTPUT positions of layer i at the left / right end of the window differ from the previous update's value at
+ * the same absolute position (receptive field reaches the zero-padded window edge, or the new samples).  The engine
+ * recomputes those rows (rounded up to tiles) and keeps every other row.  tests/test_oracle_pins.py checks the numbers
+ * against the oracle run on two overlapping windows. */
+int gw_incremental_zones(const gw_conv_layer *layers, int n_layers, int stride, int *left, int *right);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GWSTREAM_DIAG_H */

@@ -20,18 +20,41 @@ GW_BF16, GW_FP16 = 0, 1
 GW_FINAL, GW_RUNNING = 0, 1
 GW_IMPL_UMMA, GW_IMPL_SIMT = 0, 1
 
-EXPORTS = [
-    "gw_last_error", "gw_kernel_launches", "gw_set_conv_impl", "gw_set_fuse_tail", "gw_set_pdl", "gw_set_snake", "gw_set_skip_zeros", "gw_probe_mma_cycles", "gw_set_two_sm",
+EXPORTS = [          # include/gwstream.h
+    "gw_last_error", "gw_kernel_launches", "gw_options_default",
     "gw_stream_create", "gw_stream_destroy", "gw_stream_update", "gw_stream_snapshot", "gw_stream_count",
     "gw_deepclean_create", "gw_deepclean_destroy", "gw_deepclean_forward", "gw_deepclean_noise",
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
     "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_step_host_async", "gw_pipeline_graph_nodes",
-    "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes",
     "gw_deepclean_set_scaling", "gw_offline_set_scaling", "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
+]
+DIAG_EXPORTS = [     # include/gwstream_diag.h (measurement and diagnostics, not the product interface)
+    "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes", "gw_probe_mma_cycles",
+    "gw_incremental_zones",
 ]
 
 _FP = C.POINTER(C.c_float)
+
+
+class Options(C.Structure):
+    """gw_options (include/gwstream.h): everything that selects a code path, fixed when a handle is created.
+    Defaults: tensor-core kernels, fused tail, PDL, snake order, CTA pairs, zero skipping on; incremental off."""
+    _fields_ = [("conv_impl", C.c_int), ("fuse_tail", C.c_int), ("pdl", C.c_int), ("snake", C.c_int),
+                ("two_sm", C.c_int), ("skip_zeros", C.c_int), ("incremental", C.c_int)]
+
+    def __init__(self, **kw):
+        super().__init__()
+        self.conv_impl, self.fuse_tail, self.pdl, self.snake, self.two_sm, self.skip_zeros, self.incremental = \
+            GW_IMPL_UMMA, 1, 1, 1, 1, 1, 0
+        for k, v in kw.items():
+            if k not in dict(self._fields_):
+                raise TypeError(f"unknown option {k}")
+            setattr(self, k, int(v))
+
+
+def _opt_ptr(opts):
+    return None if opts is None else C.byref(opts)
 
 
 class _ConvLayer(C.Structure):
@@ -72,28 +95,26 @@ def lib():
         L = C.CDLL(LIB_PATH)
         vp, i, i64 = C.c_void_p, C.c_int, C.c_int64
         L.gw_last_error.restype = C.c_char_p
+        L.gw_last_error.argtypes = [vp]
         L.gw_kernel_launches.restype = i64
-        L.gw_set_conv_impl.argtypes = [i]
-        L.gw_set_fuse_tail.argtypes = [i]
-        L.gw_set_pdl.argtypes = [i]
-        L.gw_set_snake.argtypes = [i]
-        L.gw_set_skip_zeros.argtypes = [i]
+        L.gw_options_default.argtypes = [C.POINTER(Options)]
+        L.gw_options_default.restype = None
         L.gw_probe_mma_cycles.argtypes = [i, C.POINTER(C.c_float), C.POINTER(C.c_float)]
-        L.gw_set_two_sm.argtypes = [i]
+        L.gw_incremental_zones.argtypes = [C.POINTER(_ConvLayer), i, i, C.POINTER(i), C.POINTER(i)]
         L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
         L.gw_stream_destroy.argtypes = [vp]
         L.gw_stream_update.argtypes = [vp, vp, vp]
         L.gw_stream_snapshot.argtypes = [vp, vp, C.POINTER(i64), vp]
         L.gw_stream_count.argtypes = [vp]
         L.gw_stream_count.restype = i64
-        L.gw_deepclean_create.argtypes = [C.POINTER(vp), vp, C.POINTER(_DcSpec), i]
+        L.gw_deepclean_create.argtypes = [C.POINTER(vp), vp, C.POINTER(_DcSpec), i, C.POINTER(Options)]
         L.gw_deepclean_destroy.argtypes = [vp]
         L.gw_deepclean_forward.argtypes = [vp, vp]
         L.gw_deepclean_noise.argtypes = [vp, vp, vp]
         L.gw_cleaned_strain.argtypes = [vp, vp, i, vp]
         L.gw_noise_estimate.argtypes = [vp, vp, vp]
         L.gw_deepclean_activation.argtypes = [vp, i, vp, i64, C.POINTER(i), C.POINTER(i), vp]
-        L.gw_bbh_create.argtypes = [C.POINTER(vp), vp, C.POINTER(_BbhSpec), i, i, i]
+        L.gw_bbh_create.argtypes = [C.POINTER(vp), vp, C.POINTER(_BbhSpec), i, i, i, C.POINTER(Options)]
         L.gw_bbh_destroy.argtypes = [vp]
         L.gw_bbh_score.argtypes = [vp, vp, vp]
         L.gw_bbh_score_batch.argtypes = [vp, vp, i, vp, vp]
@@ -104,14 +125,14 @@ def lib():
         L.gw_step_host_async.argtypes = [vp, vp, vp, vp, vp]
         L.gw_deepclean_set_scaling.argtypes = [vp, vp, vp, vp, vp]
         L.gw_offline_set_scaling.argtypes = [vp, vp, vp, vp, vp]
-        L.gw_offline_create.argtypes = [C.POINTER(vp), vp, i, i, i, i, i, i]
+        L.gw_offline_create.argtypes = [C.POINTER(vp), vp, i, i, i, i, i, i, C.POINTER(Options)]
         L.gw_offline_destroy.argtypes = [vp]
         L.gw_offline_samples.argtypes = [vp]
         L.gw_offline_samples.restype = i64
         L.gw_offline_run.argtypes = [vp, vp, vp, vp, vp]
         L.gw_offline_predictions.argtypes = [vp, vp, vp]
         L.gw_pipeline_graph_nodes.argtypes = [vp]
-        L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_float), C.POINTER(i)]
+        L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i)]
         L.gw_profile_label.argtypes = [vp, i]
         L.gw_profile_label.restype = C.c_char_p
         L.gw_profile_flops.argtypes = [vp, i]
@@ -122,42 +143,25 @@ def lib():
     return _lib
 
 
-def _check(rc: int) -> None:
+def _check(rc: int, handle=None) -> None:
     if rc != GW_OK:
-        raise GwError(rc, lib().gw_last_error().decode())
+        raise GwError(rc, lib().gw_last_error(handle).decode())
 
 
 def kernel_launches() -> int:
     return int(lib().gw_kernel_launches())
 
 
-def set_conv_impl(impl: int) -> None:
-    _check(lib().gw_set_conv_impl(impl))
-
-
-def set_fuse_tail(on: bool) -> None:
-    """Fused last-GEMM-layer + final ConvTranspose1d kernel for handles created after this call (default on)."""
-    _check(lib().gw_set_fuse_tail(1 if on else 0))
-
-
-def set_pdl(on: bool) -> None:
-    """Programmatic dependent launch between the kernels of an update (default on)."""
-    _check(lib().gw_set_pdl(1 if on else 0))
-
-
-def set_snake(on: bool) -> None:
-    """Alternating traversal direction of consecutive DeepClean layers (L2 reuse; default on)."""
-    _check(lib().gw_set_snake(1 if on else 0))
-
-
-def set_two_sm(on: bool) -> None:
-    """CTA-pair (cta_group::2) kernel for the N = 256 conv GEMM layers (default on)."""
-    _check(lib().gw_set_two_sm(1 if on else 0))
-
-
-def set_skip_zeros(on: bool) -> None:
-    """Skip structurally empty K steps / halves of N in the resident-weight conv GEMMs (default on)."""
-    _check(lib().gw_set_skip_zeros(1 if on else 0))
+def incremental_zones(layer_specs: Sequence[S.ConvSpec], stride: int):
+    """(left, right) output-position counts per layer that an incremental update recomputes (gwstream_diag.h)."""
+    arr = (_ConvLayer * len(layer_specs))()
+    for a, l in zip(arr, layer_specs):
+        a.kind, a.cin, a.cout, a.k, a.stride, a.pad_l, a.pad_r, a.act, a.pool = \
+            l.kind, l.cin, l.cout, l.k, l.stride, l.pad_l, l.pad_r, l.act, l.pool
+    n = len(layer_specs)
+    left, right = (C.c_int * n)(), (C.c_int * n)()
+    _check(lib().gw_incremental_zones(arr, n, int(stride), left, right))
+    return list(left), list(right)
 
 
 def probe_mma_cycles(n_values=(16, 32, 64, 128, 256)):
@@ -226,14 +230,14 @@ class Stream:
         sp = self.spec
         assert new_samples.is_cuda and new_samples.is_contiguous() and new_samples.dtype.is_floating_point
         assert tuple(new_samples.shape) == (sp.n_streams, sp.channels, sp.stride), tuple(new_samples.shape)
-        _check(lib().gw_stream_update(self.h, _ptr(new_samples), _stream_ptr(stream)))
+        _check(lib().gw_stream_update(self.h, _ptr(new_samples), _stream_ptr(stream)), self.h)
 
     def snapshot(self, stream=None):
         import torch
         sp = self.spec
         out = torch.empty((sp.n_streams, sp.channels, sp.window), dtype=torch.float32, device="cuda")
         first = C.c_int64(0)
-        _check(lib().gw_stream_snapshot(self.h, _ptr(out), C.byref(first), _stream_ptr(stream)))
+        _check(lib().gw_stream_snapshot(self.h, _ptr(out), C.byref(first), _stream_ptr(stream)), self.h)
         return out, int(first.value)
 
     def count(self) -> int:
@@ -262,7 +266,7 @@ class DeepClean:
     """One DeepClean network per detector over a Stream."""
 
     def __init__(self, stream: Stream, layers: Sequence[S.ConvSpec], params_per_det: Sequence[Sequence[Dict]],
-                 dtype: int = GW_BF16, agg: int = S.AGG_HANN_OLA, delta: int = 0):
+                 dtype: int = GW_BF16, agg: int = S.AGG_HANN_OLA, delta: int = 0, opts: Optional[Options] = None):
         sp = stream.spec
         self.stream, self.layers, self.dtype = stream, list(layers), dtype
         keep: list = []
@@ -275,21 +279,21 @@ class DeepClean:
         srow = (C.c_int * n_det)(*[sp.strain_row(d) for d in range(n_det)])
         spec = _DcSpec(n_det, len(layers), sp.n_witness, arr, wit, srow, agg, delta)
         self.h = C.c_void_p()
-        _check(lib().gw_deepclean_create(C.byref(self.h), stream.h, C.byref(spec), dtype))
+        _check(lib().gw_deepclean_create(C.byref(self.h), stream.h, C.byref(spec), dtype, _opt_ptr(opts)), stream.h)
 
     def set_scaling(self, wit_mean=None, wit_std=None, strain_mean=None, strain_std=None) -> None:
         """Per-channel standardisation of the witnesses ([D][n_witness]) and rescaling of the estimate ([D]);
         None = identity.  Before the first update."""
-        _check(lib().gw_deepclean_set_scaling(self.h, *_scaling_args(wit_mean, wit_std, strain_mean, strain_std)))
+        _check(lib().gw_deepclean_set_scaling(self.h, *_scaling_args(wit_mean, wit_std, strain_mean, strain_std)), self.h)
 
     def forward(self, stream=None) -> None:
-        _check(lib().gw_deepclean_forward(self.h, _stream_ptr(stream)))
+        _check(lib().gw_deepclean_forward(self.h, _stream_ptr(stream)), self.h)
 
     def noise(self, stream=None):
         import torch
         sp = self.stream.spec
         out = torch.empty((sp.n_streams, sp.n_det, sp.window), dtype=torch.float32, device="cuda")
-        _check(lib().gw_deepclean_noise(self.h, _ptr(out), _stream_ptr(stream)))
+        _check(lib().gw_deepclean_noise(self.h, _ptr(out), _stream_ptr(stream)), self.h)
         return out
 
     def cleaned(self, mode: int = GW_FINAL, stream=None):
@@ -297,14 +301,14 @@ class DeepClean:
         sp = self.stream.spec
         n = sp.stride if mode == GW_FINAL else sp.window
         out = torch.empty((sp.n_streams, sp.n_det, n), dtype=torch.float32, device="cuda")
-        _check(lib().gw_cleaned_strain(self.h, _ptr(out), mode, _stream_ptr(stream)))
+        _check(lib().gw_cleaned_strain(self.h, _ptr(out), mode, _stream_ptr(stream)), self.h)
         return out
 
     def noise_estimate(self, stream=None):
         import torch
         sp = self.stream.spec
         out = torch.empty((sp.n_streams, sp.n_det, sp.window), dtype=torch.float32, device="cuda")
-        _check(lib().gw_noise_estimate(self.h, _ptr(out), _stream_ptr(stream)))
+        _check(lib().gw_noise_estimate(self.h, _ptr(out), _stream_ptr(stream)), self.h)
         return out
 
     def activation(self, layer: int, stream=None):
@@ -312,10 +316,10 @@ class DeepClean:
         import torch
         sp = self.stream.spec
         rows, cols = C.c_int(0), C.c_int(0)
-        _check(lib().gw_deepclean_activation(self.h, layer, None, 0, C.byref(rows), C.byref(cols), _stream_ptr(stream)))
+        _check(lib().gw_deepclean_activation(self.h, layer, None, 0, C.byref(rows), C.byref(cols), _stream_ptr(stream)), self.h)
         tdt = torch.bfloat16 if self.dtype == GW_BF16 else torch.float16
         out = torch.empty((sp.n_streams, sp.n_det, rows.value, cols.value), dtype=tdt, device="cuda")
-        _check(lib().gw_deepclean_activation(self.h, layer, _ptr(out), out.numel() * 2, None, None, _stream_ptr(stream)))
+        _check(lib().gw_deepclean_activation(self.h, layer, _ptr(out), out.numel() * 2, None, None, _stream_ptr(stream)), self.h)
         return out
 
     def close(self) -> None:
@@ -334,7 +338,7 @@ class Bbh:
     """BBH classifier, attached to a DeepClean stage or stateless."""
 
     def __init__(self, dc: Optional[DeepClean], convs: Sequence[S.ConvSpec], conv_params, dense_params,
-                 length: int, dtype: int = GW_BF16, n_det: int = 2, max_batch: int = 256):
+                 length: int, dtype: int = GW_BF16, n_det: int = 2, max_batch: int = 256, opts: Optional[Options] = None):
         keep: list = []
         arr = _marshal_layers(convs, conv_params, keep)
         dims = [dense_params[0]["w"].shape[1]] + [p["w"].shape[0] for p in dense_params]
@@ -348,12 +352,12 @@ class Bbh:
         self.dc, self.length, self.n_det, self.max_batch = dc, length, n_det, max_batch
         self.h = C.c_void_p()
         _check(lib().gw_bbh_create(C.byref(self.h), dc.h if dc is not None else None, C.byref(spec), dtype,
-                                   n_det, max_batch))
+                                   n_det, max_batch, _opt_ptr(opts)))
 
     def score(self, stream=None):
         import torch
         out = torch.empty((self.dc.stream.spec.n_streams,), dtype=torch.float32, device="cuda")
-        _check(lib().gw_bbh_score(self.h, _ptr(out), _stream_ptr(stream)))
+        _check(lib().gw_bbh_score(self.h, _ptr(out), _stream_ptr(stream)), self.h)
         return out
 
     def score_batch(self, windows, stream=None):
@@ -362,7 +366,7 @@ class Bbh:
         B = windows.shape[0]
         assert tuple(windows.shape[1:]) == (self.n_det, self.length)
         out = torch.empty((B,), dtype=torch.float32, device="cuda")
-        _check(lib().gw_bbh_score_batch(self.h, _ptr(windows), B, _ptr(out), _stream_ptr(stream)))
+        _check(lib().gw_bbh_score_batch(self.h, _ptr(windows), B, _ptr(out), _stream_ptr(stream)), self.h)
         return out
 
     def close(self) -> None:
@@ -387,7 +391,7 @@ class Pipeline:
 
     def step(self, new_samples, scores, cleaned_final, stream=None) -> None:
         """All CUDA float32 tensors: new [n][C][S], scores [n], cleaned_final [n][D][S]."""
-        _check(lib().gw_step(self.h, _ptr(new_samples), _ptr(scores), _ptr(cleaned_final), _stream_ptr(stream)))
+        _check(lib().gw_step(self.h, _ptr(new_samples), _ptr(scores), _ptr(cleaned_final), _stream_ptr(stream)), self.h)
 
     def step_host(self, new_samples, scores, cleaned_final, stream=None) -> None:
         """Host tensors / numpy float32 arrays (pinned for asynchronous copies)."""
@@ -395,7 +399,7 @@ class Pipeline:
             if a is None:
                 return C.c_void_p(0)
             return C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
-        _check(lib().gw_step_host(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)))
+        _check(lib().gw_step_host(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)), self.h)
 
     def step_host_async(self, new_samples, scores, cleaned_final, stream=None) -> None:
         """step_host without the synchronisation: the input copy of this call overlaps the previous step's
@@ -404,28 +408,20 @@ class Pipeline:
             if a is None:
                 return C.c_void_p(0)
             return C.c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
-        _check(lib().gw_step_host_async(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)))
+        _check(lib().gw_step_host_async(self.h, hp(new_samples), hp(scores), hp(cleaned_final), _stream_ptr(stream)), self.h)
 
     def step_profile(self, new_samples, scores, cleaned_final, stream=None):
-        """One eager update with a CUDA event after each kernel -> [(label, ms, algorithmic flops)]."""
-        ms = (C.c_float * 64)()
+        """One update through the profiling graph (gwstream_diag.h): the kernels gw_step replays, each stamping
+        %globaltimer at its first CTA's start and last CTA's end.  -> [dict(label, begin_us, end_us, flops, smem_bytes)]
+        in launch order; begin/end are relative to the start of the step's first kernel."""
+        n_max = 32
+        b, e = (C.c_double * n_max)(), (C.c_double * n_max)()
         n = C.c_int(0)
         _check(lib().gw_step_profile(self.h, _ptr(new_samples), _ptr(scores), _ptr(cleaned_final),
-                                     _stream_ptr(stream), 64, ms, C.byref(n)))
-        return [(lib().gw_profile_label(self.h, i).decode(), float(ms[i]), float(lib().gw_profile_flops(self.h, i)))
-                for i in range(min(n.value, 64))]
-
-    def profile_smem_bytes(self):
-        """{label: shared-memory traffic in bytes} of the conv GEMM kernels of the last step_profile."""
-        out = {}
-        for i in range(64):
-            lab = lib().gw_profile_label(self.h, i).decode()
-            if not lab:
-                break
-            b = float(lib().gw_profile_smem_bytes(self.h, i))
-            if b > 0:
-                out[lab] = b
-        return out
+                                     _stream_ptr(stream), n_max, b, e, C.byref(n)), self.h)
+        return [{"label": lib().gw_profile_label(self.h, i).decode(), "begin_us": float(b[i]), "end_us": float(e[i]),
+                 "flops": float(lib().gw_profile_flops(self.h, i)), "smem_bytes": float(lib().gw_profile_smem_bytes(self.h, i))}
+                for i in range(min(n.value, n_max))]
 
     def graph_nodes(self) -> int:
         return int(lib().gw_pipeline_graph_nodes(self.h))
@@ -447,7 +443,7 @@ class Offline:
     segment per launch.  `spec` gives the per-stream shape (n_streams is ignored)."""
 
     def __init__(self, spec: S.StreamSpec, layers: Sequence[S.ConvSpec], params_per_det: Sequence[Sequence[Dict]],
-                 n_windows: int, dtype: int = GW_BF16):
+                 n_windows: int, dtype: int = GW_BF16, opts: Optional[Options] = None):
         self.spec, self.n_windows = spec, n_windows
         keep: list = []
         n_det = len(params_per_det)
@@ -458,11 +454,11 @@ class Offline:
         dspec = _DcSpec(n_det, len(layers), spec.n_witness, arr, wit, srow, S.AGG_HANN_OLA, 0)
         self.h = C.c_void_p()
         _check(lib().gw_offline_create(C.byref(self.h), C.byref(dspec), spec.channels, spec.fs, spec.window, spec.stride,
-                                       n_windows, dtype))
+                                       n_windows, dtype, _opt_ptr(opts)))
         self.samples = int(lib().gw_offline_samples(self.h))
 
     def set_scaling(self, wit_mean=None, wit_std=None, strain_mean=None, strain_std=None) -> None:
-        _check(lib().gw_offline_set_scaling(self.h, *_scaling_args(wit_mean, wit_std, strain_mean, strain_std)))
+        _check(lib().gw_offline_set_scaling(self.h, *_scaling_args(wit_mean, wit_std, strain_mean, strain_std)), self.h)
 
     def run(self, samples, cleaned=None, noise=None, stream=None):
         """samples: CUDA float32 [C][T]; returns (cleaned [D][T], noise estimate [D][T])."""
@@ -472,13 +468,13 @@ class Offline:
             cleaned = torch.empty((self.spec.n_det, self.samples), dtype=torch.float32, device="cuda")
         if noise is None:
             noise = torch.empty((self.spec.n_det, self.samples), dtype=torch.float32, device="cuda")
-        _check(lib().gw_offline_run(self.h, _ptr(samples), _ptr(cleaned), _ptr(noise), _stream_ptr(stream)))
+        _check(lib().gw_offline_run(self.h, _ptr(samples), _ptr(cleaned), _ptr(noise), _stream_ptr(stream)), self.h)
         return cleaned, noise
 
     def predictions(self, stream=None):
         import torch
         out = torch.empty((self.n_windows, self.spec.n_det, self.spec.window), dtype=torch.float32, device="cuda")
-        _check(lib().gw_offline_predictions(self.h, _ptr(out), _stream_ptr(stream)))
+        _check(lib().gw_offline_predictions(self.h, _ptr(out), _stream_ptr(stream)), self.h)
         return out
 
     def __del__(self):
@@ -491,13 +487,13 @@ class Offline:
 
 
 def build_ensemble(cfg: S.Config, dc_params_per_det, bbh_params=None, dtype: int = GW_BF16,
-                   agg: int = S.AGG_HANN_OLA, delta: int = 0):
+                   agg: int = S.AGG_HANN_OLA, delta: int = 0, opts: Optional[Options] = None):
     """Convenience: Stream + DeepClean (+ Bbh) + Pipeline for a specs.Config."""
     st = Stream(cfg.stream)
-    dc = DeepClean(st, cfg.dc_layers, dc_params_per_det, dtype, agg, delta)
+    dc = DeepClean(st, cfg.dc_layers, dc_params_per_det, dtype, agg, delta, opts)
     bbh = None
     if bbh_params is not None:
         cp, dp = bbh_params
-        bbh = Bbh(dc, cfg.bbh_convs, cp, dp, cfg.bbh_len, dtype)
+        bbh = Bbh(dc, cfg.bbh_convs, cp, dp, cfg.bbh_len, dtype, opts=opts)
     pipe = Pipeline(st, dc, bbh)
     return st, dc, bbh, pipe

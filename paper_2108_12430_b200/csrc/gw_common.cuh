@@ -64,6 +64,16 @@ struct ConvGemmParams {
     // few stages' worth of work to fill the persistent CTAs evenly (small stream counts: latency, wave quantisation).
     int g_tiles;
     int two_sm;                    // 1: CTA-pair kernel (tcgen05 cta_group::2, M = 256), chosen by conv_gemm_plan
+    // Incremental path (gw_options.incremental, D13).  The OUTPUT is a mirror ring as well: tmOut spans
+    // 2 * M rows per batch item, the current window starts at row out_off = (*a_count mod a_ring_W) / out_ring_div and
+    // every row is stored twice (rows r and r +- M), so that the consumer's window is contiguous.  0: plain tensor.
+    int out_ring_div;
+    // Work list per batch item: v_tiles "virtual" tiles, of which the first v_left are tiles 0 .. v_left-1 (rows whose
+    // receptive field reaches the LEFT window edge) and the rest are the LAST v_tiles - v_left tiles (rows that see the
+    // new samples or the right window edge).  Full recomputation: v_tiles = v_left = tiles_m.
+    int v_tiles, v_left;
+    int pred_ring;                 // EPI_FINAL: pred is a ring over absolute sample index mod 4 M (no mirror: row stores)
+    unsigned long long* stamp;     // profiling graph: [0] = min %globaltimer at CTA start, [1] = max at CTA end; else null
     // EPI_FINAL: this layer (ConvTranspose1d -> 32 channels, tanh) and the network's last layer
     // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel.  The
     // epilogue writes each activated accumulator row (positions 2m, 2m+1 x 32 channels = one 128-byte
@@ -101,38 +111,48 @@ struct GemmLaunch {
     int batch;                     // n_items * n_det
     int smem_bytes;
     int grid;                      // persistent CTAs (multiple of n_det)
+    int pdl;                       // launch with programmatic stream serialization (gw_options.pdl)
 };
 
-void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st);
-void launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st);
+// Virtual tile -> tile index of the layer (see ConvGemmParams::v_tiles).
+__host__ __device__ __forceinline__ int map_tile(const ConvGemmParams& p, int vt) {
+    return vt < p.v_left ? vt : vt + (p.tiles_m - p.v_tiles);
+}
+
+cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st);
+cudaError_t launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st);
 // Chooses resident/streaming B, ring depths and the shared-memory size for a layer; false if it cannot fit.
 bool conv_gemm_plan(GemmLaunch& g, int sm_count);
 cudaError_t probe_mma_cycles(int N, float* issue, float* complete);   // diagnostic: cycles per tcgen05.mma, N in {16..256}
 cudaError_t conv_gemm_prepare();   // opt-in shared-memory attribute
 
 // ---- bandwidth / CUDA-core kernels (gw_kernels.cu) -------------------------------------------
-void launch_append(float* ring, const float* new_samples, long long* count, unsigned* ticket, int n_rows,
-                   int W, int S, cudaStream_t st);
+// Every launcher takes `stamp` (null outside the profiling graph): two 64-bit slots the kernel fills with the
+// %globaltimer of its first CTA start / last CTA end, and returns the launch status.
+typedef unsigned long long* Stamp;
+cudaError_t launch_append(float* ring, const float* new_samples, long long* count, unsigned* ticket, int n_rows,
+                          int W, int S, Stamp stamp, cudaStream_t st);
 bool is_append_kernel(const void* func);   // identifies the a1 node of a captured graph
 bool is_ring16_append_kernel(const void* func);
 bool is_snapshot_append_kernel(const void* func);   // the fused a1 + a2 kernel (src is argument 1)
-void launch_snapshot_append(float* ring, const float* new_samples, void* ring16, long long* count, unsigned* ticket,
-                            const int* rows_map, const float* pre, int n_streams, int channels, int n_det, int n_wit, int W,
-                            int S, int cpad, int fmt, cudaStream_t st);
-void launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st);
-void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
-                          int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
-                          const float* pre, cudaStream_t st);
-void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
-                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, const float* pre, cudaStream_t st,
-                   long long seg_T = 0, int seg_S = 0);
-void launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann, const double* cum,
-                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, const float* post,
-                        cudaStream_t st);
-void launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
-                        int L, int cpad, int K, int pad, int fmt, cudaStream_t st);
+bool is_aggregate_kernel(const void* func);         // the a5 node (AggParams is argument 0)
+cudaError_t launch_snapshot_append(float* ring, const float* new_samples, void* ring16, long long* count, unsigned* ticket,
+                                   const int* rows_map, const float* pre, int n_streams, int channels, int n_det, int n_wit,
+                                   int W, int S, int cpad, int fmt, Stamp stamp, cudaStream_t st);
+cudaError_t launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st);
+cudaError_t launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
+                                 int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
+                                 const float* pre, Stamp stamp, cudaStream_t st);
+cudaError_t launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
+                          int channels, int n_det, int n_wit, int W, int cpad, int fmt, const float* pre, Stamp stamp,
+                          cudaStream_t st, long long seg_T = 0, int seg_S = 0);
+cudaError_t launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann,
+                               const double* cum, float* cleaned, float* nhat_out, int B, int n_det, int W, int S,
+                               long long T, const float* post, cudaStream_t st);
+cudaError_t launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
+                               int L, int cpad, int K, int pad, int fmt, Stamp stamp, cudaStream_t st);
 struct AggParams {
-    const float* pred;         // [n][D][W]
+    const float* pred;         // [n][D][W] (pred_ring: ring over absolute index mod W, like acc)
     float* acc;                // [n][D][W] ring over absolute index mod W
     const float* ring;         // snapshot ring [n][C][W]
     const long long* count;
@@ -145,12 +165,29 @@ struct AggParams {
     float* nhat_out;           // [n][D][W] or null (test hook)
     float* clf_in;             // [n][D][Lb] or null
     int n_streams, n_det, channels, W, S, Lb, delta, agg;
+    int pred_ring;
+    Stamp stamp;
 };
-void launch_aggregate(const AggParams& a, cudaStream_t st);
-void launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
-                      int cout, int cpad, int K, int pad_l, int pool, int fmt, cudaStream_t st);
+cudaError_t launch_aggregate(const AggParams& a, cudaStream_t st);
+cudaError_t launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
+                             int cout, int cpad, int K, int pad_l, int pool, int fmt, Stamp stamp, cudaStream_t st);
 
-extern long long g_kernel_launches;
-extern int g_pdl;                  // 1: kernels of a step are launched with programmatic stream serialization
+cudaError_t launch_stamp_init(unsigned long long* stamps, int n, cudaStream_t st);   // begin slots = max, end slots = 0
+void count_launch();               // one more kernel launched (or captured) by this library: atomic process-wide counter
+long long kernel_launches();
+void uncount_launches(long long n);   // captured, not launched
+
+// Profiling stamps: %globaltimer (ns).  Thread 0 of every CTA; the end stamp follows a block-wide barrier.
+__device__ __forceinline__ unsigned long long gw_globaltimer() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void stamp_begin(unsigned long long* s) {
+    if (s != nullptr && threadIdx.x == 0) atomicMin(s, gw_globaltimer());
+}
+__device__ __forceinline__ void stamp_end(unsigned long long* s) {   // call after a __syncthreads() of the whole CTA
+    if (s != nullptr && threadIdx.x == 0) atomicMax(s + 1, gw_globaltimer());
+}
 
 }  // namespace gw

@@ -67,7 +67,8 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     if (p.two_sm) {
         // CTA-pair kernel: N = 256 store layers with an even number of tiles; half weight blocks of 16 KiB
         const int pairs = sm_count / 2;
-        bool ok = p.epi == EPI_STORE && p.N == 256 && p.a_count == nullptr && p.tiles_m % 2 == 0 && pairs >= p.n_det;
+        bool ok = p.epi == EPI_STORE && p.N == 256 && p.a_count == nullptr && p.out_ring_div == 0 && p.tiles_m % 2 == 0 &&
+                  p.v_tiles == p.tiles_m && pairs >= p.n_det;
         for (int ob = 2; ok && ob >= 1; --ob) {
             const int fixed = kFixedSmem + ob * kOutStage;
             const int sa = p.n_cb < 2 ? 2 : (p.n_cb > 8 ? 8 : p.n_cb);
@@ -120,7 +121,7 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     if (p.epi == EPI_STORE && g.batch > 0) {
         const int n_items = g.batch / p.n_det, workers = g.grid / p.n_det;
         for (int G = kAccCols / p.N; G >= 2; G /= 2) {
-            const long long units = static_cast<long long>(n_items) * ((p.tiles_m + G - 1) / G);
+            const long long units = static_cast<long long>(n_items) * ((p.v_tiles + G - 1) / G);
             if (units > workers) break;
             p.g_tiles = G;
         }
@@ -205,7 +206,7 @@ __device__ __forceinline__ uint32_t pack_pair(float a, float b, int fmt) {
 // a 1024-byte aligned SWIZZLE_128B slab needs NO base-offset (bits 49-51 stay 0): the tensor core
 // derives the swizzle phase from the absolute shared-memory address bits, exactly as TMA did when it
 // wrote the slab.  Measured on B200: base_offset = 0 matches the oracle, base_offset = (addr >> 7) & 7
-// gives garbage (profiles/r01_notes.md).
+// gives garbage (round-1 bring-up measurement).
 
 // EPI / ACT / FMT are compile-time so that the per-element epilogue loop is straight-line code the
 // compiler can unroll and interleave (with run-time branches inside it, each element's MUFU latency
@@ -241,6 +242,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     float* head_s = reinterpret_cast<float*>(after_a + 2048);                // EPI_POOL_HEAD scratch
     uint8_t* smem_fin = after_a + 2048;                                      // EPI_FINAL: last layer's B operand (1024-aligned)
 
+    stamp_begin(p.stamp);
     const int warp = __shfl_sync(0xffffffffu, threadIdx.x / 32, 0);   // provably warp-uniform: role branches and
                                                                       // everything under them use the uniform datapath
     const int lane = threadIdx.x % 32;
@@ -248,7 +250,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int worker = blockIdx.x / p.n_det;
     const int n_workers = gridDim.x / p.n_det;
     const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / p.N) : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
-    const int spi = (p.tiles_m + G - 1) / G;                                 // super-tiles per batch item
+    const int spi = (p.v_tiles + G - 1) / G;                                 // super-tiles per batch item (virtual tiles:
+                                                                             // all of them, or the two recomputed zones)
     // Two MMA-issuing warps share a stage when it holds several tiles (even tiles: warp 1, odd tiles: warp
     // kMmaWarp2).  Below N = 128 an MMA is bound by its shared-memory operand read (32 + N/4 cycles, measured:
     // profiles/r01_mma_rate_microbench.txt) and a single issuing warp ADDS ~30 cycles of descriptor arithmetic per
@@ -315,9 +318,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 const int u = p.reverse ? total - 1 - w : w;
                 const int batch = (u / spi) * p.n_det + det;
                 for (int g = 0; g < G; ++g) {
-                    const int mt = (u % spi) * G + g;
-                    if (mt >= p.tiles_m) break;
-                    const int m0 = mt * p.tile_stride + p.tile_row0;
+                    const int vt = (u % spi) * G + g;
+                    if (vt >= p.v_tiles) break;
+                    const int m0 = map_tile(p, vt) * p.tile_stride + p.tile_row0;
                     for (int cb = 0; cb < p.n_cb; ++cb) {
                         const bool second = n_mma == 2 && (g & 1);
                         const int stage = second ? ring0 + rs1 : rs0;
@@ -402,7 +405,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             const int acc = it & 1;
             TR_WAIT(0, mbar_wait(&tmem_empty[acc], ((it >> 1) & 1) ^ 1))
             tc_fence_after();
-            const int g_end = min(G, p.tiles_m - (u % spi) * G);
+            const int g_end = min(G, p.v_tiles - (u % spi) * G);
             for (int g = 0; g < g_end; ++g) {
                 if (n_mma == 2 && (g & 1) != mw) continue;                 // the other warp's tile
                 const uint32_t d_tmem = tmem_base + acc * kAccCols + g * p.N;
@@ -416,7 +419,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     if (ring) {
                         // window-edge zero padding: slab rows whose logical row is outside [0, M) hold
                         // neighbouring ring samples; clear them (whole 128-byte rows: swizzle-agnostic)
-                        const int lo = ((u % spi) * G + g) * p.tile_stride + p.tile_row0 + p.a_min;
+                        const int lo = map_tile(p, (u % spi) * G + g) * p.tile_stride + p.tile_row0 + p.a_min;
                         if (lo < 0 || lo + p.slab_rows > p.a_rows) {
                             uint8_t* slab = smem_a + astage * sl;
                             for (int idx = lane; idx < p.slab_rows * 8; idx += 32) {
@@ -499,6 +502,34 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             ch_col[i] = (32 * c) % p.N;
         }
         griddep_wait();                                        // before the first global store of this grid
+        // incremental path: window start inside the output mirror ring / the prediction ring (the append kernel of
+        // this update has advanced the counter; nothing changes it while the conv kernels run)
+        const int ring_h = (p.out_ring_div || p.pred_ring) ? static_cast<int>(*p.a_count % p.a_ring_W) : 0;
+        const int out_off = p.out_ring_div ? ring_h / p.out_ring_div : 0;
+        // One 32-row box of this tile at window row `row` (whole warp calls it; lane 0 issues the TMA stores).  Mirror
+        // ring: ring row r = out_off + row, and every row is stored a second time at its twin r +- M.  A box that
+        // straddles row M has twins on both sides: those of its rows below M go out with a TMA store that the tensor
+        // map clips at 2M; the few rows at or above M are copied to ring rows 0.. by the lanes (TMA stores do not take
+        // negative coordinates).  row_bytes = 128 (N >= 64: 128B swizzle) or 64 (N = 32: 64B swizzle).
+        auto store_box = [&](uint32_t src, int col, int row, int b, int row_bytes) {
+            const int r = out_off + row;
+            if (lane == 0) {
+                tma_store_3d(&p.tmOut, src, col, r, b);
+                if (p.out_ring_div) {
+                    if (r >= p.M) tma_store_3d(&p.tmOut, src, col, r - p.M, b);
+                    else tma_store_3d(&p.tmOut, src, col, r + p.M, b);
+                }
+            }
+            if (p.out_ring_div && r < p.M && r + 31 >= p.M && r + lane >= p.M) {
+                uint8_t* dst = reinterpret_cast<uint8_t*>(p.out) +
+                               ((static_cast<size_t>(b) * 2 * p.M + (r + lane - p.M)) * p.N + col) * 2;
+                const int units = row_bytes / 16;
+                for (int u = 0; u < units; ++u) {
+                    const int su = row_bytes == 128 ? (u ^ (lane & 7)) : (u ^ ((lane >> 1) & 3));
+                    *reinterpret_cast<float4*>(dst + 16 * u) = lds_f4(src + lane * row_bytes + (su << 4));
+                }
+            }
+        };
         const float fin_bias = EPI == EPI_FINAL ? __ldg(p.fin_b + det) : 0.f;
         int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL: the tile whose second chain is in flight
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;   // + 32 KiB for the second buffer
@@ -561,21 +592,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     }
                     fence_proxy_async();
                     __syncwarp();
-                    if (lane == 0) {
+                    {
                         const int row0 = quad * 32;
                         if (wide) {                            // both chunks: one tile, 64 adjacent columns
-                            const int mt = (u % spi) * G + ch_g[2 * cp];
-                            if (ch_g[2 * cp] < G && mt < p.tiles_m)
-                                tma_store_3d(&p.tmOut, stg, ch_col[2 * cp], mt * kTileM + row0, batch);
+                            const int vt = (u % spi) * G + ch_g[2 * cp];
+                            if (ch_g[2 * cp] < G && vt < p.v_tiles)
+                                store_box(stg, ch_col[2 * cp], map_tile(p, vt) * kTileM + row0, batch, 128);
                         } else {                               // N = 32: the chunks are two consecutive tiles
 #pragma unroll
                             for (int which = 0; which < 2; ++which) {
-                                const int mt = (u % spi) * G + ch_g[2 * cp + which];
-                                if (ch_g[2 * cp + which] < G && mt < p.tiles_m)
-                                    tma_store_3d(&p.tmOut, stg + which * 2048, 0, mt * kTileM + row0, batch);
+                                const int vt = (u % spi) * G + ch_g[2 * cp + which];
+                                if (ch_g[2 * cp + which] < G && vt < p.v_tiles)
+                                    store_box(stg + which * 2048, 0, map_tile(p, vt) * kTileM + row0, batch, 64);
                             }
                         }
-                        tma_store_commit();
+                        if (lane == 0) tma_store_commit();
                     }
                 }
             } else if (EPI == EPI_FINAL) {
@@ -587,7 +618,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 //   y[4m + r] = b + sum_{a, par, ci} w[ci][r + 3 - 4a - 2 par] x[2(m + a) + par][ci],  a = -1, 0, 1,
                 // is then three row-shifted K blocks on the tensor core (D3).  The 4 results of the
                 // PREVIOUS tile are read back one iteration later, when its chain has long retired.
-                const int mt = (u % spi) * G + hsel;
+                const int vt = (u % spi) * G + hsel;
+                const int mt = vt < p.v_tiles ? map_tile(p, vt) : p.tiles_m;   // tiles_m: no such tile
                 uint32_t ra[32], rb[32];
                 tmem_ld_32x32(taddr + 64 * hsel, ra);
                 tmem_ld_32x32(taddr + 64 * hsel + 32, rb);
@@ -625,10 +657,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     tmem_ld_32x4(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + hsel * kFinN, y);
                     tmem_ld_wait();
                     const int orow = prev_mt * p.tile_stride + row_in_tile;     // D row i = tile row i + 1
-                    if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M)
-                        *reinterpret_cast<float4*>(p.pred + (static_cast<size_t>(prev_batch) * p.M + orow) * 4) =
+                    if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M) {
+                        int o4 = 4 * orow;                                      // window position of y[4 orow]
+                        if (p.pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }   // ring slot (absolute index mod W)
+                        *reinterpret_cast<float4*>(p.pred + static_cast<size_t>(prev_batch) * p.M * 4 + o4) =
                             make_float4(__uint_as_float(y[0]) + fin_bias, __uint_as_float(y[1]) + fin_bias,
                                         __uint_as_float(y[2]) + fin_bias, __uint_as_float(y[3]) + fin_bias);
+                    }
                 }
                 prev_batch = batch; prev_mt = mt;
             } else {
@@ -720,16 +755,20 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             tmem_ld_32x4(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + hsel * kFinN, y);
             tmem_ld_wait();
             const int orow = prev_mt * p.tile_stride + row_in_tile;
-            if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M)
-                *reinterpret_cast<float4*>(p.pred + (static_cast<size_t>(prev_batch) * p.M + orow) * 4) =
+            if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M) {
+                int o4 = 4 * orow;
+                if (p.pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }
+                *reinterpret_cast<float4*>(p.pred + static_cast<size_t>(prev_batch) * p.M * 4 + o4) =
                     make_float4(__uint_as_float(y[0]) + fin_bias, __uint_as_float(y[1]) + fin_bias,
                                 __uint_as_float(y[2]) + fin_bias, __uint_as_float(y[3]) + fin_bias);
+            }
         }
         if (warp == 2) { TR_FLUSH(8, 3) }
     }
     if (EPI == EPI_STORE && warp >= 2 && warp < kMmaWarp2 && lane == 0) tma_store_wait_all<0>();   // staging buffers are still being read
     tc_fence_before();
     __syncthreads();
+    stamp_end(p.stamp);
     if (warp == 0) tmem_dealloc(tmem_base, 2 * kAccCols);
 }
 
@@ -771,6 +810,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
     uint64_t* tmem_empty = tmem_full + 2;    // [2]  leader's are used: 2 x 8 epilogue warps arrive
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_empty + 2);
 
+    stamp_begin(p.stamp);
     const int warp = __shfl_sync(0xffffffffu, threadIdx.x / 32, 0);
     const int lane = threadIdx.x % 32;
     const uint32_t rank = cluster_ctarank();                                 // 0 = leader
@@ -977,6 +1017,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
     tc_fence_before();
     __syncthreads();
     cluster_sync_all();                          // the peer may still be reading this CTA's shared memory / TMEM
+    stamp_end(p.stamp);
     if (warp == 0) tmem_dealloc_2sm(tmem_base, 2 * kAccCols);
 }
 
@@ -1084,7 +1125,6 @@ static GemmKernel pick_kernel(int epi, int act, int fmt) {
     return nullptr;
 }
 
-int g_pdl = 1;                       // programmatic dependent launch between the kernels of a step
 static bool g_prepared = false;
 cudaError_t conv_gemm_prepare() {
     if (g_prepared) return cudaSuccess;
@@ -1106,14 +1146,15 @@ cudaError_t conv_gemm_prepare() {
     return cudaSuccess;
 }
 
-void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
+cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     const int n_items = g.batch / g.p.n_det;
     const int per_unit = g.p.epi == EPI_STORE ? (g.p.g_tiles ? g.p.g_tiles : kAccCols / g.p.N) : g.p.epi == EPI_FINAL ? 2 : 1;
-    const int total = n_items * ((g.p.tiles_m + per_unit - 1) / per_unit);   // work units per detector
+    const int total = n_items * ((g.p.v_tiles + per_unit - 1) / per_unit);   // work units per detector
     int workers = g.grid / g.p.n_det;
     if (workers > total) workers = total;
     GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt);
-    if (!k) { fprintf(stderr, "gwstream: no conv GEMM kernel for epi %d act %d\n", g.p.epi, g.p.act); return; }
+    if (!k) return cudaErrorInvalidDeviceFunction;           // no kernel for this (epilogue, activation) pair
+    cudaError_t e;
     if (g.p.two_sm) {
         int cw = g.grid / 2 / g.p.n_det;                         // clusters per detector
         const int units = n_items * (g.p.tiles_m / 2);
@@ -1127,12 +1168,12 @@ void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
         at2[0].id = cudaLaunchAttributeClusterDimension;
         at2[0].val.clusterDim.x = 2; at2[0].val.clusterDim.y = 1; at2[0].val.clusterDim.z = 1;
         at2[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at2[1].val.programmaticStreamSerializationAllowed = g_pdl ? 1 : 0;
+        at2[1].val.programmaticStreamSerializationAllowed = g.pdl ? 1 : 0;
         cfg2.attrs = at2;
         cfg2.numAttrs = 2;
-        cudaLaunchKernelEx(&cfg2, pick_kernel_2sm(g.p.act, g.p.fmt), g.p, n_items);
-        ++g_kernel_launches;
-        return;
+        e = cudaLaunchKernelEx(&cfg2, pick_kernel_2sm(g.p.act, g.p.fmt), g.p, n_items);
+        count_launch();
+        return e;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(workers * g.p.n_det);
@@ -1141,11 +1182,12 @@ void launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = g_pdl ? 1 : 0;
+    attr[0].val.programmaticStreamSerializationAllowed = g.pdl ? 1 : 0;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, k, g.p, n_items);
-    ++g_kernel_launches;
+    e = cudaLaunchKernelEx(&cfg, k, g.p, n_items);
+    count_launch();
+    return e;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1227,20 +1269,22 @@ __global__ void __launch_bounds__(128) k_head_simt(const __grid_constant__ ConvG
     }
 }
 
-void launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st) {
+cudaError_t launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st) {
+    if (g.p.out_ring_div || g.p.v_tiles != g.p.tiles_m) return cudaErrorNotSupported;   // cross-check kernel: full windows only
     if (g.p.epi == EPI_STORE) {
         dim3 grid((g.p.N + 127) / 128, g.p.M, g.batch);
         k_conv_gemm_simt<<<grid, 128, 0, st>>>(g.p);
-        ++g_kernel_launches;
+        count_launch();
     } else {
         dim3 grid((g.p.N / 2 + 127) / 128, g.p.M / 2, g.batch);
         k_conv_gemm_simt<<<grid, 128, 0, st>>>(g.p);
-        ++g_kernel_launches;
+        count_launch();
         if (g.p.epi == EPI_POOL_HEAD) {
             k_head_simt<<<g.batch, 128, 0, st>>>(g.p);
-            ++g_kernel_launches;
+            count_launch();
         }
     }
+    return cudaGetLastError();
 }
 
 }  // namespace gw

@@ -14,13 +14,26 @@
 #include <vector>
 
 #include "../../include/gwstream.h"
+#include "../../include/gwstream_diag.h"
 #include "gw_common.cuh"
 
 using namespace gw;
 
 // ------------------------------------------------------------------------------------ errors
+// Every handle starts with a HandleBase: gw_last_error(handle) finds the handle's own message there.  fail() records
+// the message for the calling thread (create failures return no handle) and for the handle the running call is on.
+static constexpr uint32_t kHandleMagic = 0x47577331u;   // "GWs1"
+struct HandleBase {
+    uint32_t magic = kHandleMagic;
+    std::string err;
+};
 static thread_local std::string g_err;
-static int g_conv_impl = GW_IMPL_UMMA;
+static thread_local HandleBase* g_cur = nullptr;         // handle of the API call running on this thread
+struct CallScope {
+    HandleBase* prev;
+    explicit CallScope(const void* h) : prev(g_cur) { g_cur = const_cast<HandleBase*>(static_cast<const HandleBase*>(h)); }
+    ~CallScope() { g_cur = prev; }
+};
 
 static int fail(int code, const char* fmt, ...) {
     char buf[512];
@@ -29,6 +42,7 @@ static int fail(int code, const char* fmt, ...) {
     vsnprintf(buf, sizeof buf, fmt, ap);
     va_end(ap);
     g_err = buf;
+    if (g_cur && g_cur->magic == kHandleMagic) g_cur->err = buf;
     return code;
 }
 #define CU_TRY(expr)                                                                              \
@@ -39,35 +53,28 @@ static int fail(int code, const char* fmt, ...) {
                         cudaGetErrorString(_e));                                                  \
     } while (0)
 
-extern "C" const char* gw_last_error(void) { return g_err.c_str(); }
-extern "C" int64_t gw_kernel_launches(void) { return g_kernel_launches; }
-static int g_fuse_tail = 1;
-extern "C" int gw_set_fuse_tail(int on) {
-    g_fuse_tail = on ? 1 : 0;
-    return GW_OK;
+extern "C" const char* gw_last_error(const void* handle) {
+    if (handle) {
+        const HandleBase* b = static_cast<const HandleBase*>(handle);
+        if (b->magic == kHandleMagic) return b->err.c_str();
+    }
+    return g_err.c_str();
 }
-static int g_two_sm = 1;
-extern "C" int gw_set_two_sm(int on) {
-    g_two_sm = on ? 1 : 0;
-    return GW_OK;
+extern "C" int64_t gw_kernel_launches(void) { return kernel_launches(); }
+
+extern "C" void gw_options_default(gw_options* o) {
+    if (!o) return;
+    o->conv_impl = GW_IMPL_UMMA;
+    o->fuse_tail = 1; o->pdl = 1; o->snake = 1; o->two_sm = 1; o->skip_zeros = 1;
+    o->incremental = 0;
 }
-static int g_skip_zeros = 1;
-extern "C" int gw_set_skip_zeros(int on) {
-    g_skip_zeros = on ? 1 : 0;
-    return GW_OK;
-}
-static int g_snake = 1;
-extern "C" int gw_set_snake(int on) {
-    g_snake = on ? 1 : 0;
-    return GW_OK;
-}
-extern "C" int gw_set_pdl(int on) {
-    g_pdl = on ? 1 : 0;
-    return GW_OK;
-}
-extern "C" int gw_set_conv_impl(int impl) {
-    if (impl != GW_IMPL_UMMA && impl != GW_IMPL_SIMT) return fail(GW_EINVAL, "unknown conv impl %d", impl);
-    g_conv_impl = impl;
+static int take_options(gw_options& dst, const gw_options* src) {
+    gw_options_default(&dst);
+    if (!src) return GW_OK;
+    if (src->conv_impl != GW_IMPL_UMMA && src->conv_impl != GW_IMPL_SIMT) return fail(GW_EINVAL, "unknown conv impl %d", src->conv_impl);
+    dst = *src;
+    dst.fuse_tail = !!src->fuse_tail; dst.pdl = !!src->pdl; dst.snake = !!src->snake; dst.two_sm = !!src->two_sm;
+    dst.skip_zeros = !!src->skip_zeros; dst.incremental = !!src->incremental;
     return GW_OK;
 }
 
@@ -214,29 +221,38 @@ static int fold_layer(const gw_conv_layer& L, HostLayer& H) {
 
 static int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
-// Per-launch CUDA-event profiler (gw_step_profile): when armed, every enqueue helper drops an event
-// after each kernel it launches.
+// ------------------------------------------------------------------------------ launch context
+// What every enqueue helper needs: the stream, the first CUDA error of the sequence (launch errors are sticky and
+// reported by the API call), and -- only while the PROFILING graph is captured -- the device array of %globaltimer
+// stamps plus the host-side list of kernel labels in launch order (gw_step_profile).
+constexpr int kMaxStamps = 32;
 struct Prof {
-    std::vector<cudaEvent_t> ev;
     std::vector<std::string> labels;
-    int n = 0;
+    std::vector<double> flops, smem;               // executed algorithmic FLOPs / shared-memory bytes per kernel
 };
-static Prof* g_prof = nullptr;
-static void prof_mark(const char* label, cudaStream_t st) {
-    if (!g_prof) return;
-    if (g_prof->n >= static_cast<int>(g_prof->ev.size())) {
-        cudaEvent_t e;
-        cudaEventCreate(&e);
-        g_prof->ev.push_back(e);
-        g_prof->labels.push_back("");
+struct LaunchCtx {
+    cudaStream_t st = nullptr;
+    unsigned long long* stamps = nullptr;          // device [kMaxStamps][2] (begin, end) or null
+    Prof* prof = nullptr;
+    cudaError_t err = cudaSuccess;
+    explicit LaunchCtx(cudaStream_t s) : st(s) {}
+    Stamp next(const std::string& label, double flops = 0.0, double smem = 0.0) {
+        if (!stamps || !prof) return nullptr;
+        const int i = static_cast<int>(prof->labels.size());
+        if (i >= kMaxStamps) return nullptr;
+        prof->labels.push_back(label); prof->flops.push_back(flops); prof->smem.push_back(smem);
+        return stamps + 2 * i;
     }
-    cudaEventRecord(g_prof->ev[g_prof->n], st);
-    g_prof->labels[g_prof->n] = label;
-    g_prof->n += 1;
-}
+    void check(cudaError_t e) { if (err == cudaSuccess && e != cudaSuccess) err = e; }
+};
+#define CX_TRY(cx, what)                                                                                   \
+    do {                                                                                                   \
+        if ((cx).err != cudaSuccess) return fail(GW_ECUDA, "%s: %s", what, cudaGetErrorString((cx).err));  \
+    } while (0)
 
 // ------------------------------------------------------------------------------------ handles
 struct gw_stream {
+    HandleBase base;
     int n, C, fs, W, S;
     float* ring = nullptr;
     long long* d_count = nullptr;
@@ -248,15 +264,19 @@ struct gw_stream {
 enum GemmKind { GK_ENC, GK_DEC, GK_BBH };
 
 struct GemmLayer {
-    GemmLaunch g;
+    GemmLaunch g;                                // whole windows
+    GemmLaunch gi;                               // incremental path: the two recomputed zones only (when has_inc)
+    bool has_inc = false;
     void* d_B = nullptr;
     float* d_bias = nullptr;
     int impl = GW_IMPL_UMMA;
     std::string name;                            // profiler label, e.g. "gemm.dc3"
-    double flops = 0.0;                          // algorithmic FLOPs per batch item (real channels and taps only)
+    double flops = 0.0;                          // algorithmic FLOPs per batch item, whole window (real channels and taps only)
 };
 
 struct gw_deepclean {
+    HandleBase base;
+    gw_options opt;
     gw_stream* s = nullptr;
     int n_det = 0, n_layers = 0, n_wit = 0, agg = 0, delta = 0, fmt = FMT_BF16;
     int batch = 0;
@@ -269,6 +289,7 @@ struct gw_deepclean {
                                                  // reads its overlapping windows straight from it (null: gather path)
     bool mirror = false;                         // first layer reads the window from ring16 (no per-update gather)
     bool fused_tail = false;                     // last GEMM layer + final ConvTranspose1d run as one kernel (EPI_FINAL)
+    bool inc = false;                            // incremental path: act[i] are mirror rings [batch][2 L_i][C_i], pred a ring
     std::vector<void*> act;                      // act[0] = gathered window (null when `mirror`), act[i+1] = output of layer i
     std::vector<int> act_rows, act_cols;
     float* d_wt_final = nullptr;                 // [n_det][K][cpad]
@@ -292,6 +313,8 @@ struct gw_deepclean {
 };
 
 struct gw_bbh {
+    HandleBase base;
+    gw_options opt;
     gw_deepclean* dc = nullptr;
     int n_det = 0, batch = 0, fmt = FMT_BF16, L = 0;
     HostLayer c1;
@@ -307,34 +330,87 @@ struct gw_bbh {
     int64_t scored_for = 0;
 };
 
-struct gw_pipeline {
-    gw_stream* s = nullptr;
-    gw_deepclean* dc = nullptr;
-    gw_bbh* bbh = nullptr;
+// One captured form of the update: [incremental?][with profiling stamps?].
+struct GraphVar {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
     cudaGraphNode_t append_node = nullptr;       // the kernels that read the caller's new-sample buffer
     cudaGraphNode_t ring16_node = nullptr;
+    cudaGraphNode_t agg_node = nullptr;          // writes the caller's final-samples buffer
+    cudaGraphNode_t scores_node = nullptr;       // memcpy of the scores into the caller's buffer
     bool append_fused = false;                   // append_node is k_snapshot_append (a1 + a2 in one kernel)
     int nodes = 0;
     const float* cap_in = nullptr;
     float* cap_scores = nullptr;
     float* cap_final = nullptr;
+    AggParams agg;                               // the aggregation node's argument as captured
+    Prof prof;                                   // stamped variants: kernel labels in launch order
+};
+
+struct gw_pipeline {
+    HandleBase base;
+    gw_stream* s = nullptr;
+    gw_deepclean* dc = nullptr;
+    gw_bbh* bbh = nullptr;
+    GraphVar var[2][2];                          // [incremental zones][profiling stamps]
+    unsigned long long* d_stamps = nullptr;      // [kMaxStamps][2]
+    const Prof* last_prof = nullptr;
     float *d_in = nullptr, *d_scores = nullptr, *d_final = nullptr;   // staging for gw_step_host
     float* d_in2[2] = {nullptr, nullptr};        // gw_step_host_async: double-buffered input staging,
     cudaStream_t copy_stream = nullptr;          // filled on an internal copy stream while the previous step computes
     cudaEvent_t in_done[2] = {nullptr, nullptr}, in_free[2] = {nullptr, nullptr};
     int64_t async_calls = 0;
-    Prof prof;
 };
 
+// Incremental path (D13): how many OUTPUT positions of each layer differ from the previous update's value at
+// the same absolute position.  `left[i]`: positions [0, left) whose receptive field reaches the left window edge (where
+// this window pads with zeros and the previous one held data); `right[i]`: the last positions, which see the S new
+// samples or the right window edge.  Recurrences for stride 2, odd k = 2p + 1, padding p (output_padding 1):
+//   Conv1d            y[l] reads x[2l - p .. 2l + p]:            e' = floor((e - 1 + p)/2) + 1,  r' = floor((r + p)/2),  new' = new/2
+//   ConvTranspose1d   y[m] reads x[ceil((m-p)/2) .. floor((m+p)/2)]:  e' = 2e - 1 + p,           r' = 2r + p,           new' = 2 new
+// with e = r = 0, new = S at the network input.  right[i] = new_i + r_i.
+static int incremental_zones(const std::vector<HostLayer>& layers, int n_layers, int S, std::vector<int>& left,
+                             std::vector<int>& right) {
+    int e = 0, r = 0, nw = S;
+    left.assign(n_layers, 0); right.assign(n_layers, 0);
+    for (int i = 0; i < n_layers; ++i) {
+        const HostLayer& H = layers[i];
+        if (H.stride != 2 || (H.k & 1) == 0) return fail(GW_EINVAL, "incremental path needs stride-2 layers with odd k");
+        const int p = H.k / 2;
+        if (H.kind == GW_CONV) {
+            if (nw % 2) return fail(GW_EINVAL, "incremental path needs the stride to be a multiple of 2^(encoder depth)");
+            e = (e - 1 + p) / 2 + 1; r = (r + p) / 2; nw /= 2;
+        } else {
+            e = 2 * e - 1 + p; r = 2 * r + p; nw *= 2;
+        }
+        left[i] = e; right[i] = nw + r;
+    }
+    return GW_OK;
+}
+
+extern "C" int gw_incremental_zones(const gw_conv_layer* layers, int n_layers, int stride, int* left, int* right) {
+    if (!layers || !left || !right || n_layers < 1 || stride < 1) return fail(GW_EINVAL, "gw_incremental_zones: bad argument");
+    std::vector<HostLayer> H(n_layers);
+    for (int i = 0; i < n_layers; ++i) {
+        H[i].kind = layers[i].kind; H[i].k = layers[i].k; H[i].stride = layers[i].stride;
+        H[i].cin = layers[i].cin; H[i].cout = layers[i].cout;
+    }
+    std::vector<int> l, r;
+    if (int rc = incremental_zones(H, n_layers, stride, l, r)) return rc;
+    for (int i = 0; i < n_layers; ++i) { left[i] = l[i]; right[i] = r[i]; }
+    return GW_OK;
+}
+
 // ------------------------------------------------------------------------------ GEMM layer build
-// Builds B (weights in segment order), bias, the segment table and both tensor maps for one layer.
+// Builds B (weights in segment order), bias, the segment table and the tensor maps for one layer.
 // tap(a, par, r): index j of the filter tap that connects A-view row shift a, column half `par`
 // (position parity inside a pair row; always 0 for GK_DEC) to output column half r; <0 or >=k: none.
-static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, int n_det, int fmt, const void* in,
-                            int in_L, int cin_p, void* out, int cout_p, int batch, int epi, int head_hidden = 0,
-                            const long long* ring_count = nullptr, int ring_W = 0, long long seg_T = 0, int seg_S = 0) {
+// ring_count != null: the input is a mirror ring (every row stored twice, 2 a_rows rows per batch item) whose window
+// starts at row (*ring_count mod ring_W) / (ring_W / a_rows); out_ring: so is the output (incremental path).
+static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, int n_det, int fmt, const gw_options& opt,
+                            const void* in, int in_L, int cin_p, void* out, int cout_p, int batch, int epi,
+                            int head_hidden = 0, const long long* ring_count = nullptr, int ring_W = 0,
+                            bool out_ring = false, long long seg_T = 0, int seg_S = 0) {
     const HostLayer& H0 = dets[0];
     ConvGemmParams& p = gl.g.p;
     memset(&p, 0, sizeof p);
@@ -345,13 +421,17 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     p.a_rows_tm = ring_count ? 2 * p.a_rows : p.a_rows;     // mirror ring: every sample stored twice
     p.a_count = ring_count;
     p.a_ring_W = ring_W;
-    p.a_ring_div = halves_in;
+    p.a_ring_div = ring_count ? ring_W / p.a_rows : 1;
     p.M = p.a_rows;
     p.N = halves_out * cout_p;
     p.n_det = n_det;
     p.fmt = fmt;
     p.epi = epi;
     p.act = H0.act;
+    if (ring_count && (ring_W % p.a_rows)) return fail(GW_EINVAL, "ring input: window %d is not a multiple of the layer's %d rows", ring_W, p.a_rows);
+    if (out_ring && (!ring_count || epi != EPI_STORE || p.M % kTileM))
+        return fail(GW_EINVAL, "incremental path: layer with %d rows cannot write a ring (needs a ring input and rows %% 128 == 0)", p.M);
+    p.out_ring_div = out_ring ? ring_W / p.M : 0;
     if (p.N > 256 || p.N % 32) return fail(GW_EINVAL, "GEMM N = %d unsupported (must be a multiple of 32, <= 256)", p.N);
     if (epi == EPI_FINAL && p.N != 64) return fail(GW_EINVAL, "fused final layer needs GEMM N = 64, got %d", p.N);
     if (epi == EPI_STORE && p.N != 32 && p.N != 64 && p.N != 128 && p.N != 256)
@@ -395,6 +475,7 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
     p.tile_stride = epi == EPI_FINAL ? kTileM - 2 : kTileM;     // EPI_FINAL: one halo row on each side
     p.tile_row0 = epi == EPI_FINAL ? -1 : 0;
     p.tiles_m = (p.M + p.tile_stride - 1) / p.tile_stride;
+    p.v_tiles = p.v_left = p.tiles_m;                           // whole windows
     memset(p.seg_of, 0xff, sizeof p.seg_of);
     for (int s = 0; s < n_seg; ++s) {
         p.seg_shift[s] = static_cast<int8_t>(seg_a[s]);
@@ -402,7 +483,7 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
         p.seg_of[seg_cb[s]][seg_a[s] - a_lo] = static_cast<int8_t>(s);
     }
     // structural zeros of each segment (which K steps / which half of N any filter tap reaches at all)
-    if (g_skip_zeros && epi != EPI_POOL && epi != EPI_POOL_HEAD) {
+    if (opt.skip_zeros && epi != EPI_POOL && epi != EPI_POOL_HEAD) {
         for (int s = 0; s < n_seg; ++s) {
             bool k01 = false, lower = false, upper = false;
             for (int kk = 0; kk < kSegK; ++kk) {
@@ -452,24 +533,46 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
         if (int rc = make_tmap4(&p.tmA, in, fmt, p.a_cols, p.a_rows, n_det, batch / n_det, p.a_cols,
                                 static_cast<uint64_t>(seg_T) * cin_p, static_cast<uint64_t>(seg_S) * cin_p, p.slab_rows)) return rc;
     } else if (int rc = make_tmap(&p.tmA, in, fmt, p.a_cols, p.a_rows_tm, batch, p.a_cols, static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, p.slab_rows)) return rc;
-    if (epi == EPI_STORE)   // output [batch][M][N]: one 32-row x min(N, 64)-column box per epilogue-warp store
-        if (int rc = make_tmap(&p.tmOut, out, fmt, p.N, p.M, batch, p.N, static_cast<uint64_t>(p.M) * p.N, 32, p.N >= 64 ? 64 : 32)) return rc;
+    if (epi == EPI_STORE) {  // output [batch][M][N] ([batch][2M][N] as a mirror ring): one 32-row x min(N, 64)-column box per epilogue-warp store
+        const uint64_t out_rows = out_ring ? 2 * static_cast<uint64_t>(p.M) : p.M;
+        if (int rc = make_tmap(&p.tmOut, out, fmt, p.N, out_rows, batch, p.N, out_rows * p.N, 32, p.N >= 64 ? 64 : 32)) return rc;
+    }
     gl.g.batch = batch;
+    gl.g.pdl = opt.pdl;
     p.head_hidden = head_hidden;
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    p.two_sm = g_two_sm;                               // a request: the plan keeps it only where the pair kernel applies
+    p.two_sm = opt.two_sm;                             // a request: the plan keeps it only where the pair kernel applies
     if (!conv_gemm_plan(gl.g, sms)) return fail(GW_EINVAL, "conv GEMM layer does not fit in shared memory");
     if (int rc = make_tmap(&p.tmB, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.two_sm ? 128 : p.N)) return rc;
     if (p.mask_nu)
         if (int rc = make_tmap(&p.tmBh, gl.d_B, fmt, ktot, p.N, n_det, ktot, static_cast<uint64_t>(p.N) * ktot, p.N / 2)) return rc;
-    gl.impl = g_conv_impl;
+    gl.impl = opt.conv_impl;
 #ifdef GW_TRACE
     CU_TRY(cudaMalloc(&p.trace, 148 * 16 * 8));
     CU_TRY(cudaMemset(p.trace, 0, 148 * 16 * 8));
 #endif
     return GW_OK;
+}
+
+// Incremental variant of a built layer: the same operands, work list = the tiles that cover the first `left_rows`
+// and the last `right_rows` GEMM rows of every batch item (all tiles when the two zones meet).
+static void make_incremental_variant(GemmLayer& gl, int left_rows, int right_rows) {
+    gl.gi = gl.g;
+    ConvGemmParams& p = gl.gi.p;
+    const int ts = p.tile_stride;                       // tile t produces rows [t ts, t ts + ts)
+    int v_left = (left_rows + ts - 1) / ts;
+    int first_right = (p.M - right_rows) / ts;
+    if (first_right < 0) first_right = 0;
+    if (v_left > p.tiles_m) v_left = p.tiles_m;
+    if (first_right <= v_left) { p.v_left = p.v_tiles = p.tiles_m; }
+    else { p.v_left = v_left; p.v_tiles = v_left + (p.tiles_m - first_right); }
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    conv_gemm_plan(gl.gi, sms);                         // same operand layout; only the tiles-per-stage choice may differ
+    gl.has_inc = true;
 }
 
 #ifdef GW_TRACE
@@ -494,10 +597,42 @@ static void trace_report(const GemmLayer& gl) {
 }
 #endif
 
-static void run_gemm(const GemmLayer& gl, cudaStream_t st) {
-    if (gl.impl == GW_IMPL_UMMA) launch_conv_gemm_umma(gl.g, st);
-    else launch_conv_gemm_simt(gl.g, st);
-    prof_mark(gl.name.c_str(), st);
+// Shared-memory traffic of one launch of a conv GEMM layer, summed over all SMs, by the accounting of DESIGN.md
+// section 7: per 128-row tile the tensor core reads 4 KiB of A plus 32 N bytes of B per MMA (half of B per SM in the
+// CTA-pair kernel), TMA writes the A slabs (and, when weights are streamed, the weight blocks) and the epilogue
+// writes its staged output once and TMA reads it once.  Divided by 128 B/clk/SM x SMs x clock it gives the
+// shared-memory roofline the thin layers sit on.
+static double gemm_smem_bytes(const GemmLaunch& g, int batch) {
+    const ConvGemmParams& p = g.p;
+    const int n_items = batch / p.n_det;
+    int n_half = 0, n_k2 = 0;
+    for (unsigned long long m = p.mask_nu; m; m &= m - 1) ++n_half;
+    for (unsigned long long m = p.mask_k2; m; m &= m - 1) ++n_k2;
+    const double b_per_mma = 32.0 * p.N * (p.two_sm ? 0.5 : 1.0);
+    double mma = 4.0 * (p.n_seg - n_half - n_k2) * (4096.0 + b_per_mma)             // full segments: four K steps
+               + 4.0 * n_half * (4096.0 + b_per_mma / 2) + 2.0 * n_k2 * (4096.0 + b_per_mma);
+    double fill = static_cast<double>(p.n_cb) * p.slab_rows * 128.0;
+    if (!p.b_resident) fill += static_cast<double>(p.n_seg) * p.N * 128.0 * (p.two_sm ? 0.5 : 1.0);
+    double epi = 0.0;
+    if (p.epi == EPI_STORE) epi = 2.0 * 128.0 * p.N * 2.0;                            // staged once, read once by the TMA store
+    if (p.epi == EPI_FINAL) { epi = 128.0 * 128.0; mma += 10.0 * (4096.0 + 32.0 * 16); }   // activated tile + second chain
+    return (mma + fill + epi) * static_cast<double>(p.v_tiles) * n_items * p.n_det;
+}
+
+static void run_gemm(const GemmLayer& gl, LaunchCtx& cx, bool inc = false, int batch_override = 0) {
+    GemmLaunch g = (inc && gl.has_inc) ? gl.gi : gl.g;
+    if (batch_override) g.batch = batch_override;
+    // algorithmic FLOPs this launch executes: the rows of its tiles (all of them, or the recomputed zones)
+    const double rows = static_cast<double>(g.p.v_tiles) * g.p.tile_stride;
+    const double frac = rows >= g.p.M ? 1.0 : rows / g.p.M;
+    g.p.stamp = cx.next(gl.name, gl.flops * g.batch * frac, gemm_smem_bytes(g, g.batch));
+    cx.check(gl.impl == GW_IMPL_UMMA ? launch_conv_gemm_umma(g, cx.st) : launch_conv_gemm_simt(g, cx.st));
+    if (getenv("GW_DEBUG_SYNC")) {               // bring-up aid: name the launch that faults (never set in production)
+        const cudaError_t e = cudaStreamSynchronize(cx.st);
+        fprintf(stderr, "[gw debug] %s %s: v_tiles %d/%d left %d N %d M %d out_ring_div %d a_ring_div %d G %d resident %d sa %d -> %s\n",
+                gl.name.c_str(), inc ? "zones" : "full", g.p.v_tiles, g.p.tiles_m, g.p.v_left, g.p.N, g.p.M, g.p.out_ring_div,
+                g.p.a_ring_div, g.p.g_tiles, g.p.b_resident, g.p.sa_stages, cudaGetErrorString(e));
+    }
 }
 
 static void free_gemm(GemmLayer& gl) {
@@ -533,11 +668,12 @@ extern "C" int gw_stream_create(gw_stream** out, int n_streams, int channels, in
 extern "C" int gw_stream_destroy(gw_stream* s) {
     if (!s) return GW_OK;
     cudaFree(s->ring); cudaFree(s->d_count); cudaFree(s->d_ticket);
+    s->base.magic = 0;
     delete s;
     return GW_OK;
 }
 
-static void ring16_append_enqueue(gw_deepclean* dc, const float* src, cudaStream_t st);
+static void ring16_append_enqueue(gw_deepclean* dc, const float* src, LaunchCtx& cx);
 
 static int stream_update_checked(gw_stream* s) {
     if (s->dc && s->dc->cleaned_for != s->updates)
@@ -545,33 +681,34 @@ static int stream_update_checked(gw_stream* s) {
                     (long long)s->updates);
     return GW_OK;
 }
-static void stream_update_enqueue(gw_stream* s, const float* src, cudaStream_t st) {
+static void stream_update_enqueue(gw_stream* s, const float* src, LaunchCtx& cx) {
     gw_deepclean* dc = s->dc;
     if (dc && dc->mirror && s->S % 4 == 0 && s->W % 4 == 0) {       // a1 + a2 in one launch
-        launch_snapshot_append(s->ring, src, dc->ring16, s->d_count, s->d_ticket, dc->d_rows_map, dc->d_pre, s->n, s->C,
-                               dc->n_det, dc->n_wit, s->W, s->S, dc->act_cols[0], dc->fmt, st);
-        prof_mark("snapshot_append", st);
+        cx.check(launch_snapshot_append(s->ring, src, dc->ring16, s->d_count, s->d_ticket, dc->d_rows_map, dc->d_pre, s->n,
+                                        s->C, dc->n_det, dc->n_wit, s->W, s->S, dc->act_cols[0], dc->fmt,
+                                        cx.next("snapshot_append"), cx.st));
         return;
     }
-    launch_append(s->ring, src, s->d_count, s->d_ticket, s->n * s->C, s->W, s->S, st);
-    prof_mark("append", st);
-    if (dc) ring16_append_enqueue(dc, src, st);
+    cx.check(launch_append(s->ring, src, s->d_count, s->d_ticket, s->n * s->C, s->W, s->S, cx.next("append"), cx.st));
+    if (dc) ring16_append_enqueue(dc, src, cx);
 }
 
 extern "C" int gw_stream_update(gw_stream* s, const float* new_samples_dev, void* stream) {
     if (!s || !new_samples_dev) return fail(GW_EINVAL, "gw_stream_update: NULL argument");
+    CallScope scope(s);
     if (int rc = stream_update_checked(s)) return rc;
-    stream_update_enqueue(s, new_samples_dev, static_cast<cudaStream_t>(stream));
-    CU_TRY(cudaGetLastError());
+    LaunchCtx cx(static_cast<cudaStream_t>(stream));
+    stream_update_enqueue(s, new_samples_dev, cx);
+    CX_TRY(cx, "gw_stream_update");
     s->updates += 1;
     return GW_OK;
 }
 
 extern "C" int gw_stream_snapshot(gw_stream* s, float* out_dev, int64_t* first_index_host, void* stream) {
     if (!s || !out_dev) return fail(GW_EINVAL, "gw_stream_snapshot: NULL argument");
+    CallScope scope(s);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    launch_snapshot(s->ring, out_dev, s->d_count, s->n * s->C, s->W, st);
-    CU_TRY(cudaGetLastError());
+    CU_TRY(launch_snapshot(s->ring, out_dev, s->d_count, s->n * s->C, s->W, st));
     CU_TRY(cudaStreamSynchronize(st));
     if (first_index_host) *first_index_host = s->updates * static_cast<int64_t>(s->S) - s->W;
     return GW_OK;
@@ -600,6 +737,7 @@ extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
     cudaFree(dc->d_pre); cudaFree(dc->d_post);
     cudaFree(dc->final_buf);
     if (dc->s && dc->s->dc == dc) dc->s->dc = nullptr;
+    dc->base.magic = 0;
     delete dc;
     return GW_OK;
 }
@@ -607,6 +745,7 @@ extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
 static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spec) {
     const int W = s->W, S = s->S;
     const int nl = spec->n_layers, nd = spec->n_det;
+    const gw_options& opt = dc->opt;
     dc->host.resize(static_cast<size_t>(nd) * nl);
     for (int d = 0; d < nd; ++d)
         for (int i = 0; i < nl; ++i) {
@@ -649,14 +788,32 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     // offline: the first layer reads overlapping windows of the converted segment through a 4-D tensor map when
     // window starts fall on position pairs (even stride); otherwise every window is gathered (k_gather)
     const bool direct_seg = dc->offline && (S % 2 == 0) && (W % 2 == 0) && dc->host[0].kind == GW_CONV &&
-                            g_conv_impl == GW_IMPL_UMMA;
+                            opt.conv_impl == GW_IMPL_UMMA;
     // The last GEMM layer (ConvTranspose1d -> <= 32 channels, tanh) and the final 1-channel ConvTranspose1d
     // (k = 7) run as ONE kernel when they have the standard shape: the 16-bit activation between them is
     // never written (at C3 that round trip is 2 x 1 MiB per detector-window, more than the layer's input).
     {
         const HostLayer &Hp = dc->host[nl - 2], &Hf = dc->host[nl - 1];
-        dc->fused_tail = g_fuse_tail && g_conv_impl == GW_IMPL_UMMA && nl >= 3 && Hp.kind == GW_CONVT &&
+        dc->fused_tail = opt.fuse_tail && opt.conv_impl == GW_IMPL_UMMA && nl >= 3 && Hp.kind == GW_CONVT &&
                          Hp.act == GW_ACT_TANH && cpad[nl - 1] == 32 && Hf.k == 7 && Hf.pad_l == 3;
+    }
+    // Incremental path (D13): every stored activation is a mirror ring over absolute position; an update recomputes
+    // the left-edge and right-edge rows only.
+    std::vector<int> z_left, z_right;
+    dc->inc = false;
+    if (opt.incremental) {
+        if (dc->offline) return fail(GW_EINVAL, "incremental path: streaming handles only");
+        if (!dc->mirror || !dc->fused_tail || opt.conv_impl != GW_IMPL_UMMA)
+            return fail(GW_EINVAL, "incremental path needs an even stride and window, a Conv1d first layer, the fused tail and GW_IMPL_UMMA");
+        std::vector<HostLayer> one(dc->host.begin(), dc->host.begin() + nl);
+        if (int rc = incremental_zones(one, nl, S, z_left, z_right)) return rc;
+        int min_len = W;
+        for (int i = 0; i <= nl; ++i) if (len[i] < min_len) min_len = len[i];
+        const int depth_div = W / min_len;                  // 2^(encoder depth)
+        if (S % depth_div || W % (depth_div * kTileM))
+            return fail(GW_EINVAL, "incremental path needs stride %% %d == 0 and window %% %d == 0 (got %d, %d)", depth_div,
+                        depth_div * kTileM, S, W);
+        dc->inc = true;
     }
     for (int i = 0; i < nl; ++i) {                  // act[i] = input of layer i
         dc->act_rows[i] = len[i]; dc->act_cols[i] = cpad[i];
@@ -664,6 +821,7 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         size_t bytes = static_cast<size_t>(batch) * len[i] * cpad[i] * 2;
         void** dst = &dc->act[i];
         if (i == 0 && dc->mirror) { bytes *= 2; dst = &dc->ring16; }
+        else if (dc->inc) bytes *= 2;                 // mirror ring: every row twice
         if (i == 0 && direct_seg) { bytes = static_cast<size_t>(nd) * dc->off_T * cpad[0] * 2; dst = &dc->seg16; }
         CU_TRY(cudaMalloc(dst, bytes));
         CU_TRY(cudaMemset(*dst, 0, bytes));
@@ -673,16 +831,16 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
     for (int i = 0; i < nl - 1; ++i) {
         for (int d = 0; d < nd; ++d) per_det[d] = dc->host[d * nl + i];
         const GemmKind gk = dc->host[i].kind == GW_CONV ? GK_ENC : GK_DEC;
-        const bool from_ring = i == 0 && dc->mirror;
+        const bool from_ring = (i == 0 && dc->mirror) || dc->inc;
         const bool fin = i == nl - 2 && dc->fused_tail;
         const bool from_seg = i == 0 && direct_seg;
-        if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt,
-                                      from_ring ? dc->ring16 : from_seg ? dc->seg16 : dc->act[i],
+        const void* in = (i == 0 && dc->mirror) ? dc->ring16 : from_seg ? dc->seg16 : dc->act[i];
+        if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, opt, in,
                                       len[i], cpad[i], dc->act[i + 1], cpad[i + 1], batch, fin ? EPI_FINAL : EPI_STORE, 0,
-                                      from_ring ? s->d_count : nullptr, from_ring ? W : 0, from_seg ? dc->off_T : 0,
-                                      from_seg ? S : 0))
+                                      from_ring ? s->d_count : nullptr, from_ring ? W : 0, dc->inc && !fin,
+                                      from_seg ? dc->off_T : 0, from_seg ? S : 0))
             return rc;
-        dc->gemm[i].g.p.reverse = g_snake ? (i & 1) : 0;
+        dc->gemm[i].g.p.reverse = opt.snake ? (i & 1) : 0;
         dc->gemm[i].name = "gemm.dc" + std::to_string(i);
         // useful MACs: every (input position, tap, cin, cout) product of the layer definition
         const HostLayer& H = dc->host[i];
@@ -738,6 +896,17 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         ConvGemmParams& p = dc->gemm[nl - 2].g.p;
         if (int rc = make_tmap(&p.tmF, dc->d_fin_B, dc->fmt, ktot, 16, nd, ktot, static_cast<uint64_t>(16) * ktot, 16)) return rc;
         p.fin_b = dc->d_b_final; p.pred = dc->pred;
+        p.pred_ring = dc->inc ? 1 : 0;
+    }
+    if (dc->inc) {
+        // zones in GEMM rows: an encoder row is one output position, a decoder row two (even | odd output), a row of the
+        // fused tail four positions of the network output
+        for (int i = 0; i < nl - 1; ++i) {
+            const bool fin = i == nl - 2;
+            const int per_row = fin ? 4 : (dc->host[i].kind == GW_CONV ? 1 : 2);
+            const int zl = fin ? z_left[nl - 1] : z_left[i], zr = fin ? z_right[nl - 1] : z_right[i];
+            make_incremental_variant(dc->gemm[i], (zl + per_row - 1) / per_row, (zr + per_row - 1) / per_row);
+        }
     }
     CU_TRY(cudaMalloc(&dc->acc, wbytes));
     CU_TRY(cudaMemset(dc->acc, 0, wbytes));
@@ -804,15 +973,17 @@ static int set_scaling(gw_deepclean* dc, const float* wit_mean, const float* wit
 extern "C" int gw_deepclean_set_scaling(gw_deepclean* dc, const float* wit_mean, const float* wit_std,
                                         const float* strain_mean, const float* strain_std) {
     if (!dc) return fail(GW_EINVAL, "gw_deepclean_set_scaling: NULL handle");
+    CallScope scope(dc);
     if (dc->s && dc->s->updates != 0)
         return fail(GW_ESTATE, "gw_deepclean_set_scaling: must be called before the first update (the state holds converted samples)");
     return set_scaling(dc, wit_mean, wit_std, strain_mean, strain_std);
 }
 
-extern "C" int gw_deepclean_create(gw_deepclean** out, gw_stream* s, const gw_dc_spec* spec, int dtype) {
+extern "C" int gw_deepclean_create(gw_deepclean** out, gw_stream* s, const gw_dc_spec* spec, int dtype, const gw_options* opts) {
     if (!out) return fail(GW_EINVAL, "out is NULL");
     *out = nullptr;
     if (!s || !spec || !spec->layers || !spec->witness_rows || !spec->strain_row) return fail(GW_EINVAL, "gw_deepclean_create: NULL argument");
+    CallScope scope(s);
     if (dtype != GW_BF16 && dtype != GW_FP16) return fail(GW_EINVAL, "dtype must be GW_BF16 or GW_FP16");
     if (spec->n_det < 1 || spec->n_layers < 2 || spec->n_witness < 1) return fail(GW_EINVAL, "bad DeepClean spec");
     if (s->dc) return fail(GW_ESTATE, "stream already has a DeepClean stage");
@@ -827,54 +998,57 @@ extern "C" int gw_deepclean_create(gw_deepclean** out, gw_stream* s, const gw_dc
             if (spec->witness_rows[d * spec->n_witness + c] < 0 || spec->witness_rows[d * spec->n_witness + c] >= s->C)
                 return fail(GW_EINVAL, "witness row out of range");
     }
+    gw_options o;
+    if (int rc = take_options(o, opts)) return rc;
     if (int rc = check_device()) return rc;
     gw_deepclean* dc = new gw_deepclean();
+    dc->opt = o;
     dc->s = s; dc->n_det = spec->n_det; dc->n_layers = spec->n_layers; dc->n_wit = spec->n_witness;
     dc->agg = spec->agg; dc->delta = spec->delta;
     dc->fmt = dtype == GW_BF16 ? FMT_BF16 : FMT_FP16;
     int rc = deepclean_build(dc, s, spec);
-    if (rc != GW_OK) { std::string keep = g_err; gw_deepclean_destroy(dc); g_err = keep; return rc; }
+    if (rc != GW_OK) { std::string keep = g_err; gw_deepclean_destroy(dc); g_err = keep; s->base.err = keep; return rc; }
     s->dc = dc;
     *out = dc;
     return GW_OK;
 }
 
 // a2, incremental: convert this update's S new witness samples into the mirror ring (after k_append).
-static void ring16_append_enqueue(gw_deepclean* dc, const float* src, cudaStream_t st) {
+static void ring16_append_enqueue(gw_deepclean* dc, const float* src, LaunchCtx& cx) {
     if (!dc->mirror) return;
     gw_stream* s = dc->s;
-    launch_ring16_append(src, dc->ring16, s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, s->S,
-                         dc->act_cols[0], dc->fmt, dc->d_pre, st);
-    prof_mark("ring16_append", st);
+    cx.check(launch_ring16_append(src, dc->ring16, s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, s->S,
+                                  dc->act_cols[0], dc->fmt, dc->d_pre, cx.next("ring16_append"), cx.st));
 }
 
-static void deepclean_forward_enqueue(gw_deepclean* dc, cudaStream_t st) {
+// `zones`: incremental handles only -- recompute the left-edge and right-edge rows of every layer (every update but the
+// first, which fills the rings with whole windows).
+static void deepclean_forward_enqueue(gw_deepclean* dc, LaunchCtx& cx, bool zones) {
     gw_stream* s = dc->s;
-    if (!dc->mirror) {
-        launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
-                      dc->act_cols[0], dc->fmt, dc->d_pre, st);
-        prof_mark("gather", st);
-    }
-    for (auto& g : dc->gemm) run_gemm(g, st);
-    if (!dc->fused_tail) {
-        launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
-                           dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
-        prof_mark("final_convt", st);
-    }
+    if (!dc->mirror)
+        cx.check(launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
+                               dc->act_cols[0], dc->fmt, dc->d_pre, cx.next("gather"), cx.st));
+    for (auto& g : dc->gemm) run_gemm(g, cx, zones && dc->inc);
+    if (!dc->fused_tail)
+        cx.check(launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
+                                    dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, cx.next("final_convt"), cx.st));
 }
 
 extern "C" int gw_deepclean_forward(gw_deepclean* dc, void* stream) {
     if (!dc) return fail(GW_EINVAL, "gw_deepclean_forward: NULL handle");
+    CallScope scope(dc);
     if (dc->s->updates == 0 || dc->forward_for == dc->s->updates)
         return fail(GW_ESTATE, "gw_deepclean_forward: no new update to run on");
-    deepclean_forward_enqueue(dc, static_cast<cudaStream_t>(stream));
-    CU_TRY(cudaGetLastError());
+    LaunchCtx cx(static_cast<cudaStream_t>(stream));
+    deepclean_forward_enqueue(dc, cx, dc->forward_for > 0);
+    CX_TRY(cx, "gw_deepclean_forward");
     dc->forward_for = dc->s->updates;
     return GW_OK;
 }
 
 // ============================================================================ offline mode (D9)
 struct gw_offline {
+    HandleBase base;
     gw_stream* s = nullptr;                      // shape carrier only (n = windows per launch); no ring
     gw_deepclean* dc = nullptr;
     double* d_cum = nullptr;                     // [W] summed Hann weights along each residue chain
@@ -887,12 +1061,13 @@ extern "C" int gw_offline_destroy(gw_offline* o) {
     if (o->dc) { o->dc->s = nullptr; gw_deepclean_destroy(o->dc); }
     if (o->s) { cudaFree(o->s->d_count); cudaFree(o->s->d_ticket); delete o->s; }
     cudaFree(o->d_cum);
+    o->base.magic = 0;
     delete o;
     return GW_OK;
 }
 
 extern "C" int gw_offline_create(gw_offline** out, const gw_dc_spec* spec, int channels, int fs, int window, int stride,
-                                 int n_windows, int dtype) {
+                                 int n_windows, int dtype, const gw_options* opts) {
     if (!out) return fail(GW_EINVAL, "out is NULL");
     *out = nullptr;
     if (!spec || !spec->layers || !spec->witness_rows || !spec->strain_row) return fail(GW_EINVAL, "gw_offline_create: NULL argument");
@@ -906,6 +1081,9 @@ extern "C" int gw_offline_create(gw_offline** out, const gw_dc_spec* spec, int c
             if (spec->witness_rows[d * spec->n_witness + c] < 0 || spec->witness_rows[d * spec->n_witness + c] >= channels)
                 return fail(GW_EINVAL, "witness row out of range");
     }
+    gw_options oo;
+    if (int rc = take_options(oo, opts)) return rc;
+    if (oo.incremental) return fail(GW_EINVAL, "gw_offline_create: the incremental path is a streaming option");
     if (int rc = check_device()) return rc;
     gw_offline* o = new gw_offline();
     o->B = n_windows;
@@ -914,6 +1092,7 @@ extern "C" int gw_offline_create(gw_offline** out, const gw_dc_spec* spec, int c
     o->s->n = n_windows; o->s->C = channels; o->s->fs = fs; o->s->W = window; o->s->S = stride;
     gw_deepclean* dc = new gw_deepclean();
     o->dc = dc;
+    dc->opt = oo;
     dc->s = o->s; dc->n_det = spec->n_det; dc->n_layers = spec->n_layers; dc->n_wit = spec->n_witness;
     dc->agg = GW_AGG_HANN_OLA; dc->delta = 0; dc->offline = true; dc->off_T = o->T;
     dc->fmt = dtype == GW_BF16 ? FMT_BF16 : FMT_FP16;
@@ -939,6 +1118,7 @@ extern "C" int gw_offline_create(gw_offline** out, const gw_dc_spec* spec, int c
 extern "C" int gw_offline_set_scaling(gw_offline* o, const float* wit_mean, const float* wit_std, const float* strain_mean,
                                       const float* strain_std) {
     if (!o) return fail(GW_EINVAL, "gw_offline_set_scaling: NULL handle");
+    CallScope scope(o);
     return set_scaling(o->dc, wit_mean, wit_std, strain_mean, strain_std);
 }
 
@@ -946,25 +1126,24 @@ extern "C" int64_t gw_offline_samples(const gw_offline* o) { return o ? o->T : 0
 
 extern "C" int gw_offline_run(gw_offline* o, const float* samples_dev, float* cleaned_dev, float* noise_dev, void* stream) {
     if (!o || !samples_dev || !cleaned_dev) return fail(GW_EINVAL, "gw_offline_run: NULL argument");
+    CallScope scope(o);
     gw_deepclean* dc = o->dc;
     gw_stream* s = o->s;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    LaunchCtx cx(static_cast<cudaStream_t>(stream));
     if (dc->seg16) {       // the whole segment as ONE "window" of length T: converts every sample once
-        launch_gather(samples_dev, dc->seg16, nullptr, dc->d_rows_map, 1, s->C, dc->n_det, dc->n_wit, static_cast<int>(o->T),
-                      dc->act_cols[0], dc->fmt, dc->d_pre, st, o->T, 0);
+        cx.check(launch_gather(samples_dev, dc->seg16, nullptr, dc->d_rows_map, 1, s->C, dc->n_det, dc->n_wit, static_cast<int>(o->T),
+                               dc->act_cols[0], dc->fmt, dc->d_pre, nullptr, cx.st, o->T, 0));
     } else {
-        launch_gather(samples_dev, dc->act[0], nullptr, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W, dc->act_cols[0],
-                      dc->fmt, dc->d_pre, st, o->T, s->S);
+        cx.check(launch_gather(samples_dev, dc->act[0], nullptr, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
+                               dc->act_cols[0], dc->fmt, dc->d_pre, nullptr, cx.st, o->T, s->S));
     }
-    prof_mark("gather", st);
-    for (auto& g : dc->gemm) run_gemm(g, st);
-    if (!dc->fused_tail) {
-        launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
-                           dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, st);
-    }
-    launch_ola_offline(dc->pred, samples_dev, dc->d_strain_rows, dc->d_hann, o->d_cum, cleaned_dev, noise_dev, o->B, dc->n_det,
-                       s->W, s->S, o->T, dc->d_post, st);
-    CU_TRY(cudaGetLastError());
+    for (auto& g : dc->gemm) run_gemm(g, cx);
+    if (!dc->fused_tail)
+        cx.check(launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
+                                    dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, nullptr, cx.st));
+    cx.check(launch_ola_offline(dc->pred, samples_dev, dc->d_strain_rows, dc->d_hann, o->d_cum, cleaned_dev, noise_dev, o->B,
+                                dc->n_det, s->W, s->S, o->T, dc->d_post, cx.st));
+    CX_TRY(cx, "gw_offline_run");
     dc->forward_for += 1;                        // gw_deepclean_noise-style hooks see a completed pass
     return GW_OK;
 }
@@ -972,15 +1151,36 @@ extern "C" int gw_offline_run(gw_offline* o, const float* samples_dev, float* cl
 // Test hook: the raw per-window predictions [B][D][W] of the last gw_offline_run.
 extern "C" int gw_offline_predictions(gw_offline* o, float* out_dev, void* stream) {
     if (!o || !out_dev) return fail(GW_EINVAL, "gw_offline_predictions: NULL argument");
+    CallScope scope(o);
     CU_TRY(cudaMemcpyAsync(out_dev, o->dc->pred, static_cast<size_t>(o->dc->batch) * o->s->W * 4, cudaMemcpyDeviceToDevice,
                            static_cast<cudaStream_t>(stream)));
     return GW_OK;
 }
 
+// Time-ordered copy of a ring whose window starts at row h: dst[b][0 .. rows) = src[b][h .. h + rows) mod rows.
+static int copy_unrotated(void* dst, const void* src, size_t row_bytes, size_t rows, size_t h, int batch, size_t src_rows,
+                          cudaStream_t st) {
+    const uint8_t* s8 = static_cast<const uint8_t*>(src);
+    uint8_t* d8 = static_cast<uint8_t*>(dst);
+    const size_t first = (h + rows <= src_rows) ? rows : src_rows - h;     // contiguous part
+    CU_TRY(cudaMemcpy2DAsync(d8, rows * row_bytes, s8 + h * row_bytes, src_rows * row_bytes, first * row_bytes, batch,
+                             cudaMemcpyDeviceToDevice, st));
+    if (first < rows)
+        CU_TRY(cudaMemcpy2DAsync(d8 + first * row_bytes, rows * row_bytes, s8, src_rows * row_bytes, (rows - first) * row_bytes,
+                                 batch, cudaMemcpyDeviceToDevice, st));
+    return GW_OK;
+}
+
 extern "C" int gw_deepclean_noise(gw_deepclean* dc, float* out_dev, void* stream) {
     if (!dc || !out_dev) return fail(GW_EINVAL, "gw_deepclean_noise: NULL argument");
+    CallScope scope(dc);
     if (dc->forward_for == 0) return fail(GW_ESTATE, "gw_deepclean_noise: no forward pass yet");
-    CU_TRY(cudaMemcpyAsync(out_dev, dc->pred, static_cast<size_t>(dc->batch) * dc->s->W * 4, cudaMemcpyDeviceToDevice,
+    const size_t W = dc->s->W;
+    if (dc->inc) {         // the prediction lives in a ring over absolute sample index: window position n is slot (count + n) mod W
+        const size_t h = static_cast<size_t>((dc->forward_for * static_cast<int64_t>(dc->s->S)) % dc->s->W);
+        return copy_unrotated(out_dev, dc->pred, 4, W, h, dc->batch, W, static_cast<cudaStream_t>(stream));
+    }
+    CU_TRY(cudaMemcpyAsync(out_dev, dc->pred, static_cast<size_t>(dc->batch) * W * 4, cudaMemcpyDeviceToDevice,
                            static_cast<cudaStream_t>(stream)));
     return GW_OK;
 }
@@ -988,20 +1188,23 @@ extern "C" int gw_deepclean_noise(gw_deepclean* dc, float* out_dev, void* stream
 extern "C" int gw_deepclean_activation(gw_deepclean* dc, int layer, void* out_dev, int64_t out_bytes, int* rows,
                                        int* cols, void* stream) {
     if (!dc || layer < -1 || layer >= dc->n_layers - 1) return fail(GW_EINVAL, "gw_deepclean_activation: bad layer");
+    CallScope scope(dc);
     const int i = layer + 1;
     if (i == dc->n_layers - 1 && dc->fused_tail && out_dev)
-        return fail(GW_ESTATE, "layer %d's output is not materialised: it is fused with the final layer (gw_set_fuse_tail(0) to inspect it)", layer);
+        return fail(GW_ESTATE, "layer %d's output is not materialised: it is fused with the final layer (gw_options.fuse_tail = 0 to inspect it)", layer);
     if (rows) *rows = dc->act_rows[i];
     if (cols) *cols = dc->act_cols[i];
     const int64_t bytes = static_cast<int64_t>(dc->batch) * dc->act_rows[i] * dc->act_cols[i] * 2;
     if (out_dev) {
         if (out_bytes < bytes) return fail(GW_EINVAL, "output buffer too small (%lld < %lld)", (long long)out_bytes, (long long)bytes);
-        if (i == 0 && dc->mirror) {
-            // the window is the contiguous row range [h, h + W) of each batch item's mirror ring
-            const size_t row_b = static_cast<size_t>(dc->act_cols[0]) * 2, W = dc->s->W;
-            const size_t h = static_cast<size_t>((dc->s->updates * static_cast<int64_t>(dc->s->S)) % dc->s->W);
-            CU_TRY(cudaMemcpy2DAsync(out_dev, W * row_b, static_cast<const uint8_t*>(dc->ring16) + h * row_b, 2 * W * row_b,
-                                     W * row_b, dc->batch, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
+        if ((i == 0 && dc->mirror) || (i > 0 && dc->inc)) {
+            // the window is the contiguous row range [h_i, h_i + L_i) of each batch item's mirror ring (2 L_i rows)
+            const size_t row_b = static_cast<size_t>(dc->act_cols[i]) * 2, L = dc->act_rows[i];
+            const size_t hW = static_cast<size_t>((dc->s->updates * static_cast<int64_t>(dc->s->S)) % dc->s->W);
+            const size_t h = hW / (static_cast<size_t>(dc->s->W) / L);
+            const void* src = i == 0 ? dc->ring16 : dc->act[i];
+            CU_TRY(cudaMemcpy2DAsync(out_dev, L * row_b, static_cast<const uint8_t*>(src) + h * row_b, 2 * L * row_b,
+                                     L * row_b, dc->batch, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
         } else {
             CU_TRY(cudaMemcpyAsync(out_dev, dc->act[i], bytes, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(stream)));
         }
@@ -1009,20 +1212,29 @@ extern "C" int gw_deepclean_activation(gw_deepclean* dc, int layer, void* out_de
     return GW_OK;
 }
 
-static void cleaned_enqueue(gw_deepclean* dc, float* final_out, float* running_out, float* nhat_out, cudaStream_t st) {
+static AggParams make_agg(gw_deepclean* dc, float* final_out, float* running_out, float* nhat_out) {
     gw_stream* s = dc->s;
     AggParams a;
+    memset(&a, 0, sizeof a);
     a.pred = dc->pred; a.acc = dc->acc; a.ring = s->ring; a.count = s->d_count; a.strain_rows = dc->d_strain_rows;
     a.hann = dc->d_hann; a.inv_wsum = dc->d_inv_wsum; a.post = dc->d_post;
     a.final_out = final_out; a.running_out = running_out; a.nhat_out = nhat_out; a.clf_in = dc->clf_in;
     a.n_streams = s->n; a.n_det = dc->n_det; a.channels = s->C; a.W = s->W; a.S = s->S; a.Lb = dc->Lb;
     a.delta = dc->delta; a.agg = dc->agg;
-    launch_aggregate(a, st);
-    prof_mark("aggregate", st);
+    a.pred_ring = dc->inc ? 1 : 0;
+    return a;
+}
+
+static AggParams cleaned_enqueue(gw_deepclean* dc, float* final_out, float* running_out, float* nhat_out, LaunchCtx& cx) {
+    AggParams a = make_agg(dc, final_out, running_out, nhat_out);
+    a.stamp = cx.next("aggregate");
+    cx.check(launch_aggregate(a, cx.st));
+    return a;
 }
 
 extern "C" int gw_cleaned_strain(gw_deepclean* dc, float* out_dev, int mode, void* stream) {
     if (!dc) return fail(GW_EINVAL, "gw_cleaned_strain: NULL handle");
+    CallScope scope(dc);
     if (mode != GW_FINAL && mode != GW_RUNNING) return fail(GW_EINVAL, "gw_cleaned_strain: bad mode");
     if (dc->forward_for != dc->s->updates || dc->cleaned_for == dc->s->updates)
         return fail(GW_ESTATE, "gw_cleaned_strain: call gw_deepclean_forward for this update first (once)");
@@ -1031,15 +1243,16 @@ extern "C" int gw_cleaned_strain(gw_deepclean* dc, float* out_dev, int mode, voi
         CU_TRY(cudaMalloc(&dc->nhat, wbytes));
         CU_TRY(cudaMemset(dc->nhat, 0, wbytes));
     }
-    cleaned_enqueue(dc, mode == GW_FINAL ? out_dev : nullptr, mode == GW_RUNNING ? out_dev : nullptr, dc->nhat,
-                    static_cast<cudaStream_t>(stream));
-    CU_TRY(cudaGetLastError());
+    LaunchCtx cx(static_cast<cudaStream_t>(stream));
+    cleaned_enqueue(dc, mode == GW_FINAL ? out_dev : nullptr, mode == GW_RUNNING ? out_dev : nullptr, dc->nhat, cx);
+    CX_TRY(cx, "gw_cleaned_strain");
     dc->cleaned_for = dc->s->updates;
     return GW_OK;
 }
 
 extern "C" int gw_noise_estimate(gw_deepclean* dc, float* out_dev, void* stream) {
     if (!dc || !out_dev) return fail(GW_EINVAL, "gw_noise_estimate: NULL argument");
+    CallScope scope(dc);
     if (!dc->nhat || dc->cleaned_for == 0) return fail(GW_ESTATE, "gw_noise_estimate: call gw_cleaned_strain first");
     CU_TRY(cudaMemcpyAsync(out_dev, dc->nhat, static_cast<size_t>(dc->batch) * dc->s->W * 4, cudaMemcpyDeviceToDevice,
                            static_cast<cudaStream_t>(stream)));
@@ -1055,6 +1268,7 @@ extern "C" int gw_bbh_destroy(gw_bbh* b) {
     cudaFree(b->d_hw1); cudaFree(b->d_hb1); cudaFree(b->d_hw2); cudaFree(b->d_hb2);
     cudaFree(b->pooled_dbg); cudaFree(b->scores_buf);
     if (b->dc && b->dc->bbh == b) { b->dc->bbh = nullptr; b->dc->clf_in = nullptr; b->dc->Lb = 0; }
+    b->base.magic = 0;
     delete b;
     return GW_OK;
 }
@@ -1118,7 +1332,7 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
         if (last && cout_p != H[i].cout) return fail(GW_EINVAL, "last classifier block cout must be a multiple of 32");
         if (len[i - 1] % 4) return fail(GW_EINVAL, "classifier length must be divisible by 4^blocks");
         GemmLayer& gl = b->gemm[i - 1];
-        if (int rc = build_gemm_layer(gl, GK_BBH, &H[i], 1, b->fmt, b->act[i - 1], len[i - 1], cp[i - 1],
+        if (int rc = build_gemm_layer(gl, GK_BBH, &H[i], 1, b->fmt, b->opt, b->act[i - 1], len[i - 1], cp[i - 1],
                                       last ? nullptr : b->act[i], cout_p, b->batch, last ? EPI_POOL_HEAD : EPI_POOL,
                                       last ? hidden : 0))
             return rc;
@@ -1136,10 +1350,12 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
     return GW_OK;
 }
 
-extern "C" int gw_bbh_create(gw_bbh** out, gw_deepclean* dc, const gw_bbh_spec* spec, int dtype, int n_det, int max_batch) {
+extern "C" int gw_bbh_create(gw_bbh** out, gw_deepclean* dc, const gw_bbh_spec* spec, int dtype, int n_det, int max_batch,
+                             const gw_options* opts) {
     if (!out) return fail(GW_EINVAL, "out is NULL");
     *out = nullptr;
     if (!spec || !spec->convs || !spec->dense_dims || !spec->dense_w || !spec->dense_b) return fail(GW_EINVAL, "gw_bbh_create: NULL argument");
+    CallScope scope(dc);
     if (dtype != GW_BF16 && dtype != GW_FP16) return fail(GW_EINVAL, "dtype must be GW_BF16 or GW_FP16");
     if (spec->n_convs < 2) return fail(GW_EINVAL, "classifier needs at least 2 conv blocks");
     if (spec->length < 64 || spec->length % 64) return fail(GW_EINVAL, "classifier length must be a multiple of 64");
@@ -1150,48 +1366,49 @@ extern "C" int gw_bbh_create(gw_bbh** out, gw_deepclean* dc, const gw_bbh_spec* 
     } else if (n_det < 1 || max_batch < 1) {
         return fail(GW_EINVAL, "stateless classifier needs n_det >= 1 and max_batch >= 1");
     }
+    gw_options o;
+    if (int rc = take_options(o, opts)) return rc;
+    o.incremental = 0;                           // a DeepClean option; the classifier window is rescored every update
     if (int rc = check_device()) return rc;
     gw_bbh* b = new gw_bbh();
+    b->opt = o;
     b->dc = dc; b->n_det = n_det; b->batch = max_batch; b->L = spec->length;
     b->fmt = dtype == GW_BF16 ? FMT_BF16 : FMT_FP16;
     int rc = bbh_build(b, spec);
-    if (rc != GW_OK) { std::string keep = g_err; b->dc = nullptr; gw_bbh_destroy(b); g_err = keep; return rc; }
+    if (rc != GW_OK) { std::string keep = g_err; b->dc = nullptr; gw_bbh_destroy(b); g_err = keep; if (dc) dc->base.err = keep; return rc; }
     if (dc) { dc->bbh = b; dc->clf_in = b->in_buf; dc->Lb = b->L; }
     *out = b;
     return GW_OK;
 }
 
-static void bbh_enqueue(gw_bbh* b, const float* in, int batch, cudaStream_t st) {
-    launch_bbh_conv1(in, b->d_w1, b->d_b1, b->act[0], batch, b->n_det, b->L, b->c1.cout, b->c1_cpad, b->c1.k,
-                     b->c1.pad_l, b->c1.pool, b->fmt, st);
-    prof_mark("bbh_conv1", st);
-    for (auto& g : b->gemm) {
-        GemmLayer gl = g;
-        gl.g.batch = batch;
-        run_gemm(gl, st);
-    }
+static void bbh_enqueue(gw_bbh* b, const float* in, int batch, LaunchCtx& cx) {
+    cx.check(launch_bbh_conv1(in, b->d_w1, b->d_b1, b->act[0], batch, b->n_det, b->L, b->c1.cout, b->c1_cpad, b->c1.k,
+                              b->c1.pad_l, b->c1.pool, b->fmt, cx.next("bbh_conv1"), cx.st));
+    for (auto& g : b->gemm) run_gemm(g, cx, false, batch);
 }
 
 extern "C" int gw_bbh_score(gw_bbh* b, float* scores_dev, void* stream) {
     if (!b || !scores_dev) return fail(GW_EINVAL, "gw_bbh_score: NULL argument");
+    CallScope scope(b);
     if (!b->dc) return fail(GW_ESTATE, "gw_bbh_score: stateless classifier; use gw_bbh_score_batch");
     if (b->dc->cleaned_for != b->dc->s->updates || b->dc->cleaned_for == 0 || b->scored_for == b->dc->s->updates)
         return fail(GW_ESTATE, "gw_bbh_score: call gw_cleaned_strain for this update first (once)");
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    bbh_enqueue(b, b->in_buf, b->batch, st);
-    CU_TRY(cudaGetLastError());
-    CU_TRY(cudaMemcpyAsync(scores_dev, b->scores_buf, static_cast<size_t>(b->batch) * 4, cudaMemcpyDeviceToDevice, st));
+    LaunchCtx cx(static_cast<cudaStream_t>(stream));
+    bbh_enqueue(b, b->in_buf, b->batch, cx);
+    CX_TRY(cx, "gw_bbh_score");
+    CU_TRY(cudaMemcpyAsync(scores_dev, b->scores_buf, static_cast<size_t>(b->batch) * 4, cudaMemcpyDeviceToDevice, cx.st));
     b->scored_for = b->dc->s->updates;
     return GW_OK;
 }
 
 extern "C" int gw_bbh_score_batch(gw_bbh* b, const float* windows_dev, int batch, float* scores_dev, void* stream) {
     if (!b || !windows_dev || !scores_dev) return fail(GW_EINVAL, "gw_bbh_score_batch: NULL argument");
+    CallScope scope(b);
     if (batch < 1 || batch > b->batch) return fail(GW_EINVAL, "batch %d outside [1, %d]", batch, b->batch);
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    bbh_enqueue(b, windows_dev, batch, st);
-    CU_TRY(cudaGetLastError());
-    CU_TRY(cudaMemcpyAsync(scores_dev, b->scores_buf, static_cast<size_t>(batch) * 4, cudaMemcpyDeviceToDevice, st));
+    LaunchCtx cx(static_cast<cudaStream_t>(stream));
+    bbh_enqueue(b, windows_dev, batch, cx);
+    CX_TRY(cx, "gw_bbh_score_batch");
+    CU_TRY(cudaMemcpyAsync(scores_dev, b->scores_buf, static_cast<size_t>(batch) * 4, cudaMemcpyDeviceToDevice, cx.st));
     return GW_OK;
 }
 
@@ -1206,10 +1423,17 @@ extern "C" int gw_pipeline_create(gw_pipeline** out, gw_stream* s, gw_deepclean*
     return GW_OK;
 }
 
+static void graphvar_reset(GraphVar& v) {
+    if (v.exec) cudaGraphExecDestroy(v.exec);
+    if (v.graph) cudaGraphDestroy(v.graph);
+    v = GraphVar();
+}
+
 extern "C" int gw_pipeline_destroy(gw_pipeline* p) {
     if (!p) return GW_OK;
-    if (p->exec) cudaGraphExecDestroy(p->exec);
-    if (p->graph) cudaGraphDestroy(p->graph);
+    for (int a = 0; a < 2; ++a)
+        for (int b = 0; b < 2; ++b) graphvar_reset(p->var[a][b]);
+    cudaFree(p->d_stamps);
     cudaFree(p->d_in); cudaFree(p->d_scores); cudaFree(p->d_final);
     for (int i = 0; i < 2; ++i) {
         cudaFree(p->d_in2[i]);
@@ -1217,175 +1441,187 @@ extern "C" int gw_pipeline_destroy(gw_pipeline* p) {
         if (p->in_free[i]) cudaEventDestroy(p->in_free[i]);
     }
     if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
-    for (cudaEvent_t e : p->prof.ev) cudaEventDestroy(e);
+    p->base.magic = 0;
     delete p;
     return GW_OK;
 }
 
-extern "C" int gw_pipeline_graph_nodes(const gw_pipeline* p) { return p ? p->nodes : 0; }
+// Kernel nodes of the graph the steps replay (the non-profiling variant; incremental handles: the zones variant once
+// it exists).  0 before the first gw_step.
+extern "C" int gw_pipeline_graph_nodes(const gw_pipeline* p) {
+    if (!p) return 0;
+    if (p->var[1][0].exec) return p->var[1][0].nodes;
+    return p->var[0][0].nodes;
+}
 
-static int pipeline_capture(gw_pipeline* p, const float* in, float* scores, float* fin, cudaStream_t st) {
-    if (p->exec) { cudaGraphExecDestroy(p->exec); p->exec = nullptr; }
-    if (p->graph) { cudaGraphDestroy(p->graph); p->graph = nullptr; }
-    const long long before = g_kernel_launches;
-    CU_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
-    stream_update_enqueue(p->s, in, st);
-    deepclean_forward_enqueue(p->dc, st);
-    cleaned_enqueue(p->dc, fin, nullptr, nullptr, st);
-    if (p->bbh) {
-        bbh_enqueue(p->bbh, p->bbh->in_buf, p->bbh->batch, st);
-        // cudaMemcpyDefault: `scores` may be the device alias of a pinned host buffer (gw_step_host_async)
-        cudaMemcpyAsync(scores, p->bbh->scores_buf, static_cast<size_t>(p->bbh->batch) * 4, cudaMemcpyDefault, st);
+// Capture update -> forward -> cleaned(GW_FINAL) -> score into `v`.  zones: incremental handles after their first
+// update; stamped: every kernel also records its %globaltimer span (gw_step_profile).
+static int pipeline_capture(gw_pipeline* p, GraphVar& v, bool zones, bool stamped, const float* in, float* scores, float* fin,
+                            cudaStream_t st) {
+    graphvar_reset(v);
+    LaunchCtx cx(st);
+    if (stamped) {
+        if (!p->d_stamps) CU_TRY(cudaMalloc(&p->d_stamps, kMaxStamps * 2 * sizeof(unsigned long long)));
+        cx.stamps = p->d_stamps;
+        cx.prof = &v.prof;
     }
-    cudaError_t e = cudaStreamEndCapture(st, &p->graph);
-    p->nodes = static_cast<int>(g_kernel_launches - before);
-    g_kernel_launches = before;                         // captured, not launched
-    if (e != cudaSuccess) return fail(GW_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
-    CU_TRY(cudaGraphInstantiate(&p->exec, p->graph, 0));
-    p->cap_in = in; p->cap_scores = scores; p->cap_final = fin;
-    // remember the append node: a new input pointer is then a parameter update, not a re-capture
-    p->append_node = nullptr;
-    p->ring16_node = nullptr;
+    const long long before = kernel_launches();
+    CU_TRY(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+    if (stamped) cx.check(launch_stamp_init(p->d_stamps, kMaxStamps, st));
+    stream_update_enqueue(p->s, in, cx);
+    deepclean_forward_enqueue(p->dc, cx, zones);
+    v.agg = cleaned_enqueue(p->dc, fin, nullptr, nullptr, cx);
+    if (p->bbh) {
+        bbh_enqueue(p->bbh, p->bbh->in_buf, p->bbh->batch, cx);
+        // cudaMemcpyDefault: `scores` may be the device alias of a pinned host buffer (gw_step_host_async)
+        cx.check(cudaMemcpyAsync(scores, p->bbh->scores_buf, static_cast<size_t>(p->bbh->batch) * 4, cudaMemcpyDefault, st));
+    }
+    cudaError_t e = cudaStreamEndCapture(st, &v.graph);
+    const long long captured = kernel_launches() - before;
+    uncount_launches(captured);                         // captured, not launched
+    v.nodes = static_cast<int>(captured);
+    if (cx.err != cudaSuccess || e != cudaSuccess) {
+        const cudaError_t shown = cx.err != cudaSuccess ? cx.err : e;
+        if (v.graph) { cudaGraphDestroy(v.graph); v.graph = nullptr; }
+        cudaGetLastError();
+        return fail(GW_ECUDA, "graph capture failed: %s", cudaGetErrorString(shown));
+    }
+    CU_TRY(cudaGraphInstantiate(&v.exec, v.graph, 0));
+    v.cap_in = in; v.cap_scores = scores; v.cap_final = fin;
+    // remember the nodes that hold caller pointers: new buffers are then parameter updates, not re-captures
     size_t n_nodes = 0;
-    CU_TRY(cudaGraphGetNodes(p->graph, nullptr, &n_nodes));
+    CU_TRY(cudaGraphGetNodes(v.graph, nullptr, &n_nodes));
     std::vector<cudaGraphNode_t> nodes(n_nodes);
-    CU_TRY(cudaGraphGetNodes(p->graph, nodes.data(), &n_nodes));
+    CU_TRY(cudaGraphGetNodes(v.graph, nodes.data(), &n_nodes));
     for (cudaGraphNode_t nd : nodes) {
         cudaGraphNodeType ty;
         CU_TRY(cudaGraphNodeGetType(nd, &ty));
+        if (ty == cudaGraphNodeTypeMemcpy) { v.scores_node = nd; continue; }
         if (ty != cudaGraphNodeTypeKernel) continue;
         cudaKernelNodeParams kp;
         CU_TRY(cudaGraphKernelNodeGetParams(nd, &kp));
-        if (is_append_kernel(kp.func)) { p->append_node = nd; p->append_fused = false; }
-        if (is_snapshot_append_kernel(kp.func)) { p->append_node = nd; p->append_fused = true; }
-        if (is_ring16_append_kernel(kp.func)) p->ring16_node = nd;
+        if (is_append_kernel(kp.func)) { v.append_node = nd; v.append_fused = false; }
+        if (is_snapshot_append_kernel(kp.func)) { v.append_node = nd; v.append_fused = true; }
+        if (is_ring16_append_kernel(kp.func)) v.ring16_node = nd;
+        if (is_aggregate_kernel(kp.func)) v.agg_node = nd;
     }
     return GW_OK;
 }
 
-static int set_node_src(gw_pipeline* p, cudaGraphNode_t node, int n_args, int src_arg, const float* in) {
+// Replace argument `idx` of a kernel node of the instantiated graph (the other n_args - 1 arguments are kept).
+static int set_kernel_arg(GraphVar& v, cudaGraphNode_t node, int n_args, int idx, void* value) {
     cudaKernelNodeParams kp;
     CU_TRY(cudaGraphKernelNodeGetParams(node, &kp));
-    void* args[16];
+    void* args[20];
     for (int i = 0; i < n_args; ++i) args[i] = kp.kernelParams[i];
-    const float* src = in;
-    args[src_arg] = &src;
+    args[idx] = value;
     kp.kernelParams = args;
-    CU_TRY(cudaGraphExecKernelNodeSetParams(p->exec, node, &kp));
+    CU_TRY(cudaGraphExecKernelNodeSetParams(v.exec, node, &kp));
+    CU_TRY(cudaGraphKernelNodeSetParams(node, &kp));    // keep the template graph in step (later Get/Set pairs start from it)
     return GW_OK;
 }
 
-static int pipeline_set_input(gw_pipeline* p, const float* in) {
-    // k_append(ring, src, count, ticket, n_rows, W, S); k_ring16_append(src, ring16, count, rows_map, ... 12 args)
-    // k_snapshot_append(ring, src, ring16, count, ticket, rows_map, pre, ... 14 args)
-    if (p->append_fused) {
-        if (int rc = set_node_src(p, p->append_node, 14, 1, in)) return rc;
-        p->cap_in = in;
-        return GW_OK;
+static int pipeline_set_input(GraphVar& v, const float* in) {
+    // k_append(ring, src, count, ticket, n_rows, W, S, stamp); k_ring16_append(src, ring16, count, rows_map, ... 13 args)
+    // k_snapshot_append(ring, src, ring16, count, ticket, rows_map, pre, ... 15 args)
+    const float* src = in;
+    if (v.append_fused) {
+        if (int rc = set_kernel_arg(v, v.append_node, 15, 1, &src)) return rc;
+    } else {
+        if (int rc = set_kernel_arg(v, v.append_node, 8, 1, &src)) return rc;
+        if (v.ring16_node)
+            if (int rc = set_kernel_arg(v, v.ring16_node, 13, 0, &src)) return rc;
     }
-    if (int rc = set_node_src(p, p->append_node, 7, 1, in)) return rc;
-    if (p->ring16_node)
-        if (int rc = set_node_src(p, p->ring16_node, 12, 0, in)) return rc;
-    p->cap_in = in;
+    v.cap_in = in;
+    return GW_OK;
+}
+
+// One update through the graph variant that applies; captures it on first use, otherwise patches the node parameters
+// that hold caller pointers.  *used receives the variant (gw_step_profile reads its stamps).
+static int pipeline_run(gw_pipeline* p, const float* in, float* scores, float* fin, cudaStream_t st, bool stamped,
+                        GraphVar** used) {
+    const bool zones = p->dc->inc && p->s->updates > 0;
+    GraphVar& v = p->var[zones ? 1 : 0][stamped ? 1 : 0];
+    bool capture = !v.exec || (v.cap_in != in && !v.append_node) || (v.cap_final != fin && !v.agg_node) ||
+                   (p->bbh && v.cap_scores != scores && !v.scores_node);
+    if (!capture) {
+        if (v.cap_in != in)
+            if (int rc = pipeline_set_input(v, in)) return rc;
+        if (v.cap_final != fin) {
+            AggParams a = v.agg;
+            a.final_out = fin;
+            if (int rc = set_kernel_arg(v, v.agg_node, 1, 0, &a)) return rc;
+            v.agg = a; v.cap_final = fin;
+        }
+        if (p->bbh && v.cap_scores != scores) {
+            const size_t bytes = static_cast<size_t>(p->bbh->batch) * 4;
+            cudaError_t e = cudaGraphExecMemcpyNodeSetParams1D(v.exec, v.scores_node, scores, p->bbh->scores_buf, bytes, cudaMemcpyDefault);
+            if (e == cudaSuccess) e = cudaGraphMemcpyNodeSetParams1D(v.scores_node, scores, p->bbh->scores_buf, bytes, cudaMemcpyDefault);
+            if (e == cudaSuccess) v.cap_scores = scores;
+            else { cudaGetLastError(); capture = true; }    // e.g. device buffer -> mapped host buffer: a different copy kind
+        }
+    }
+    if (capture) {
+        if (st == nullptr) return fail(GW_EINVAL, "gw_step needs a non-default stream (graph capture)");
+        if (int rc = pipeline_capture(p, v, zones, stamped, in, scores, fin, st)) return rc;
+    }
+    CU_TRY(cudaGraphLaunch(v.exec, st));
+    for (int i = 0; i < v.nodes; ++i) count_launch();
+    p->s->updates += 1;
+    p->dc->forward_for = p->dc->cleaned_for = p->s->updates;
+    if (p->bbh) p->bbh->scored_for = p->s->updates;
+    if (used) *used = &v;
     return GW_OK;
 }
 
 extern "C" int gw_step(gw_pipeline* p, const float* new_samples_dev, float* scores_dev, float* cleaned_final_dev, void* stream) {
     if (!p || !new_samples_dev || !cleaned_final_dev || (p->bbh && !scores_dev)) return fail(GW_EINVAL, "gw_step: NULL argument");
+    CallScope scope(p);
     if (int rc = stream_update_checked(p->s)) return rc;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (!p->exec || p->cap_scores != scores_dev || p->cap_final != cleaned_final_dev ||
-        (p->cap_in != new_samples_dev && !p->append_node)) {
-        if (st == nullptr) return fail(GW_EINVAL, "gw_step needs a non-default stream (graph capture)");
-        if (int rc = pipeline_capture(p, new_samples_dev, scores_dev, cleaned_final_dev, st)) return rc;
-    } else if (p->cap_in != new_samples_dev) {
-        if (int rc = pipeline_set_input(p, new_samples_dev)) return rc;
-    }
-    CU_TRY(cudaGraphLaunch(p->exec, st));
-    g_kernel_launches += p->nodes;
-    p->s->updates += 1;
-    p->dc->forward_for = p->dc->cleaned_for = p->s->updates;
-    if (p->bbh) p->bbh->scored_for = p->s->updates;
-    return GW_OK;
+    return pipeline_run(p, new_samples_dev, scores_dev, cleaned_final_dev, static_cast<cudaStream_t>(stream), false, nullptr);
 }
 
-// One update, launched eagerly (no graph) with a CUDA event after every kernel; synchronises.
+// One update through the PROFILING graph: the same kernels and launch attributes as gw_step, each stamping
+// %globaltimer at its first CTA's start and its last CTA's end; synchronises.
 extern "C" int gw_step_profile(gw_pipeline* p, const float* new_samples_dev, float* scores_dev, float* cleaned_final_dev,
-                               void* stream, int max_kernels, float* ms_out, int* n_out) {
-    if (!p || !new_samples_dev || !cleaned_final_dev || !ms_out || !n_out || (p->bbh && !scores_dev))
+                               void* stream, int max_kernels, double* begin_us, double* end_us, int* n_out) {
+    if (!p || !new_samples_dev || !cleaned_final_dev || !begin_us || !end_us || !n_out || (p->bbh && !scores_dev))
         return fail(GW_EINVAL, "gw_step_profile: NULL argument");
+    CallScope scope(p);
     if (int rc = stream_update_checked(p->s)) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    Prof& pr = p->prof;
-    pr.n = 0;
-    g_prof = &pr;
-    prof_mark("begin", st);
-    stream_update_enqueue(p->s, new_samples_dev, st);
-    deepclean_forward_enqueue(p->dc, st);
-    cleaned_enqueue(p->dc, cleaned_final_dev, nullptr, nullptr, st);
-    if (p->bbh) {
-        bbh_enqueue(p->bbh, p->bbh->in_buf, p->bbh->batch, st);
-        cudaMemcpyAsync(scores_dev, p->bbh->scores_buf, static_cast<size_t>(p->bbh->batch) * 4, cudaMemcpyDeviceToDevice, st);
-    }
-    g_prof = nullptr;
-    CU_TRY(cudaGetLastError());
+    GraphVar* v = nullptr;
+    if (int rc = pipeline_run(p, new_samples_dev, scores_dev, cleaned_final_dev, st, true, &v)) return rc;
     CU_TRY(cudaStreamSynchronize(st));
-    p->s->updates += 1;
-    p->dc->forward_for = p->dc->cleaned_for = p->s->updates;
-    if (p->bbh) p->bbh->scored_for = p->s->updates;
 #ifdef GW_TRACE
     for (auto& g : p->dc->gemm) trace_report(g);
     if (p->bbh) for (auto& g : p->bbh->gemm) trace_report(g);
 #endif
-    const int nk = pr.n - 1;
+    unsigned long long h[kMaxStamps * 2];
+    CU_TRY(cudaMemcpy(h, p->d_stamps, sizeof h, cudaMemcpyDeviceToHost));
+    const int nk = static_cast<int>(v->prof.labels.size());
+    unsigned long long t0 = ~0ull;
+    for (int i = 0; i < nk; ++i) if (h[2 * i] < t0) t0 = h[2 * i];
     *n_out = nk;
-    for (int i = 0; i < nk && i < max_kernels; ++i) CU_TRY(cudaEventElapsedTime(&ms_out[i], pr.ev[i], pr.ev[i + 1]));
+    for (int i = 0; i < nk && i < max_kernels; ++i) {
+        begin_us[i] = static_cast<double>(h[2 * i] - t0) * 1e-3;
+        end_us[i] = static_cast<double>(h[2 * i + 1] - t0) * 1e-3;
+    }
+    p->last_prof = &v->prof;
     return GW_OK;
 }
 
 extern "C" const char* gw_profile_label(const gw_pipeline* p, int i) {
-    if (!p || i < 0 || i + 1 >= p->prof.n) return "";
-    return p->prof.labels[i + 1].c_str();
+    if (!p || !p->last_prof || i < 0 || i >= static_cast<int>(p->last_prof->labels.size())) return "";
+    return p->last_prof->labels[i].c_str();
 }
-
-// Algorithmic FLOPs of kernel i of the last profiled step (0 for non-GEMM kernels): real channels and
-// taps only, summed over the batch.
 extern "C" double gw_profile_flops(const gw_pipeline* p, int i) {
-    if (!p) return 0.0;
-    const std::string lab = gw_profile_label(p, i);
-    for (auto& g : p->dc->gemm) if (g.name == lab) return g.flops * p->dc->batch;
-    if (p->bbh) for (auto& g : p->bbh->gemm) if (g.name == lab) return g.flops * p->bbh->batch;
-    return 0.0;
+    if (!p || !p->last_prof || i < 0 || i >= static_cast<int>(p->last_prof->flops.size())) return 0.0;
+    return p->last_prof->flops[i];
 }
-
-// Shared-memory traffic of one launch of a conv GEMM layer, summed over all SMs, by the accounting of DESIGN.md
-// section 7: per 128-row tile the tensor core reads 4 KiB of A plus 32 N bytes of B per MMA (half of B per SM in the
-// CTA-pair kernel), TMA writes the A slabs (and, when weights are streamed, the weight blocks) and the epilogue
-// writes its staged output once and TMA reads it once.  Divided by 128 B/clk/SM x SMs x clock it gives the
-// shared-memory roofline the thin layers sit on.
-static double gemm_smem_bytes(const GemmLayer& gl, int batch) {
-    const ConvGemmParams& p = gl.g.p;
-    const int n_items = batch / p.n_det;
-    int n_half = 0, n_k2 = 0;
-    for (unsigned long long m = p.mask_nu; m; m &= m - 1) ++n_half;
-    for (unsigned long long m = p.mask_k2; m; m &= m - 1) ++n_k2;
-    const double b_per_mma = 32.0 * p.N * (p.two_sm ? 0.5 : 1.0);
-    double mma = 4.0 * (p.n_seg - n_half - n_k2) * (4096.0 + b_per_mma)             // full segments: four K steps
-               + 4.0 * n_half * (4096.0 + b_per_mma / 2) + 2.0 * n_k2 * (4096.0 + b_per_mma);
-    double fill = static_cast<double>(p.n_cb) * p.slab_rows * 128.0;
-    if (!p.b_resident) fill += static_cast<double>(p.n_seg) * p.N * 128.0 * (p.two_sm ? 0.5 : 1.0);
-    double epi = 0.0;
-    if (p.epi == EPI_STORE) epi = 2.0 * 128.0 * p.N * 2.0;                            // staged once, read once by the TMA store
-    if (p.epi == EPI_FINAL) { epi = 128.0 * 128.0; mma += 10.0 * (4096.0 + 32.0 * 16); }   // activated tile + second chain
-    return (mma + fill + epi) * static_cast<double>(p.tiles_m) * n_items * p.n_det;
-}
-
 extern "C" double gw_profile_smem_bytes(const gw_pipeline* p, int i) {
-    if (!p) return 0.0;
-    const std::string lab = gw_profile_label(p, i);
-    for (auto& g : p->dc->gemm) if (g.name == lab) return gemm_smem_bytes(g, p->dc->batch);
-    if (p->bbh) for (auto& g : p->bbh->gemm) if (g.name == lab) return gemm_smem_bytes(g, p->bbh->batch);
-    return 0.0;
+    if (!p || !p->last_prof || i < 0 || i >= static_cast<int>(p->last_prof->smem.size())) return 0.0;
+    return p->last_prof->smem[i];
 }
 
 // Throughput form of gw_step_host: does NOT synchronise, and the host->device copy of this call's samples
@@ -1396,7 +1632,9 @@ extern "C" int gw_step_host_async(gw_pipeline* p, const float* new_samples_host,
                                   float* cleaned_final_host, void* stream) {
     if (!p || !new_samples_host || !cleaned_final_host || (p->bbh && !scores_host))
         return fail(GW_EINVAL, "gw_step_host_async: NULL argument");
+    CallScope scope(p);
     gw_stream* s = p->s;
+    if (int rc = stream_update_checked(s)) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t in_bytes = static_cast<size_t>(s->n) * s->C * s->S * 4;
     const size_t fin_bytes = static_cast<size_t>(p->dc->batch) * s->S * 4;
@@ -1409,10 +1647,8 @@ extern "C" int gw_step_host_async(gw_pipeline* p, const float* new_samples_host,
             CU_TRY(cudaEventCreateWithFlags(&p->in_free[i], cudaEventDisableTiming));
         }
     }
-    if (!p->d_final) {
-        CU_TRY(cudaMalloc(&p->d_final, fin_bytes));
-        CU_TRY(cudaMalloc(&p->d_scores, sc_bytes));
-    }
+    if (!p->d_final) CU_TRY(cudaMalloc(&p->d_final, fin_bytes));
+    if (!p->d_scores) CU_TRY(cudaMalloc(&p->d_scores, sc_bytes));
     const int b = static_cast<int>(p->async_calls & 1);
     if (p->async_calls >= 2) CU_TRY(cudaStreamWaitEvent(p->copy_stream, p->in_free[b], 0));   // step k-2 has read it
     CU_TRY(cudaMemcpyAsync(p->d_in2[b], new_samples_host, in_bytes, cudaMemcpyHostToDevice, p->copy_stream));
@@ -1425,11 +1661,11 @@ extern "C" int gw_step_host_async(gw_pipeline* p, const float* new_samples_host,
                         (!p->bbh || cudaHostGetDevicePointer(&sc_alias, scores_host, 0) == cudaSuccess);
     if (!direct) cudaGetLastError();             // pageable memory: clear the sticky-free error, use the copies
     if (direct) {
-        if (int rc = gw_step(p, p->d_in2[b], p->bbh ? static_cast<float*>(sc_alias) : p->d_scores,
-                             static_cast<float*>(fin_alias), stream)) return rc;
+        if (int rc = pipeline_run(p, p->d_in2[b], p->bbh ? static_cast<float*>(sc_alias) : p->d_scores,
+                                  static_cast<float*>(fin_alias), st, false, nullptr)) return rc;
         CU_TRY(cudaEventRecord(p->in_free[b], st));
     } else {
-        if (int rc = gw_step(p, p->d_in2[b], p->d_scores, p->d_final, stream)) return rc;
+        if (int rc = pipeline_run(p, p->d_in2[b], p->d_scores, p->d_final, st, false, nullptr)) return rc;
         CU_TRY(cudaEventRecord(p->in_free[b], st));
         CU_TRY(cudaMemcpyAsync(cleaned_final_host, p->d_final, fin_bytes, cudaMemcpyDeviceToHost, st));
         if (p->bbh) CU_TRY(cudaMemcpyAsync(scores_host, p->d_scores, sc_bytes, cudaMemcpyDeviceToHost, st));
@@ -1440,18 +1676,18 @@ extern "C" int gw_step_host_async(gw_pipeline* p, const float* new_samples_host,
 
 extern "C" int gw_step_host(gw_pipeline* p, const float* new_samples_host, float* scores_host, float* cleaned_final_host, void* stream) {
     if (!p || !new_samples_host || !cleaned_final_host || (p->bbh && !scores_host)) return fail(GW_EINVAL, "gw_step_host: NULL argument");
+    CallScope scope(p);
     gw_stream* s = p->s;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t in_bytes = static_cast<size_t>(s->n) * s->C * s->S * 4;
     const size_t fin_bytes = static_cast<size_t>(p->dc->batch) * s->S * 4;
     const size_t sc_bytes = static_cast<size_t>(s->n) * 4;
-    if (!p->d_in) {
-        CU_TRY(cudaMalloc(&p->d_in, in_bytes));
-        CU_TRY(cudaMalloc(&p->d_final, fin_bytes));
-        CU_TRY(cudaMalloc(&p->d_scores, sc_bytes));
-    }
+    if (!p->d_in) CU_TRY(cudaMalloc(&p->d_in, in_bytes));
+    if (!p->d_final) CU_TRY(cudaMalloc(&p->d_final, fin_bytes));
+    if (!p->d_scores) CU_TRY(cudaMalloc(&p->d_scores, sc_bytes));
+    if (int rc = stream_update_checked(s)) return rc;
     CU_TRY(cudaMemcpyAsync(p->d_in, new_samples_host, in_bytes, cudaMemcpyHostToDevice, st));
-    if (int rc = gw_step(p, p->d_in, p->d_scores, p->d_final, stream)) return rc;
+    if (int rc = pipeline_run(p, p->d_in, p->d_scores, p->d_final, st, false, nullptr)) return rc;
     CU_TRY(cudaMemcpyAsync(cleaned_final_host, p->d_final, fin_bytes, cudaMemcpyDeviceToHost, st));
     if (p->bbh) CU_TRY(cudaMemcpyAsync(scores_host, p->d_scores, sc_bytes, cudaMemcpyDeviceToHost, st));
     CU_TRY(cudaStreamSynchronize(st));

@@ -5,11 +5,16 @@
 // Step names a1..a7 are those of DESIGN.md "Steps on the hot path".
 #include <stdio.h>
 
+#include <atomic>
+
 #include "gw_common.cuh"
 
 namespace gw {
 
-long long g_kernel_launches = 0;
+static std::atomic<long long> g_kernel_launches{0};
+void count_launch() { g_kernel_launches.fetch_add(1, std::memory_order_relaxed); }
+long long kernel_launches() { return g_kernel_launches.load(std::memory_order_relaxed); }
+void uncount_launches(long long n) { g_kernel_launches.fetch_sub(n, std::memory_order_relaxed); }
 
 __device__ __forceinline__ float ld16(const void* p, size_t i, int fmt) {
     if (fmt == FMT_BF16) return __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p)[i]);
@@ -37,6 +42,17 @@ __device__ __forceinline__ void unpack16x8(const uint4& q, float (&f)[8], int fm
     }
 }
 
+// Profiling graph only: reset the %globaltimer stamps (begin = min over CTAs -> start from the maximum; end = max).
+__global__ void k_stamp_init(unsigned long long* stamps, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { stamps[2 * i] = ~0ull; stamps[2 * i + 1] = 0ull; }
+}
+cudaError_t launch_stamp_init(unsigned long long* stamps, int n, cudaStream_t st) {
+    k_stamp_init<<<(n + 63) / 64, 64, 0, st>>>(stamps, n);
+    count_launch();
+    return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------------------------------------
 // a1  Snapshot append: ring[row][(count + i) mod W] = new[row][i], i < S; the last
 // block to finish advances the device-resident sample counter, so a captured graph replays
@@ -44,7 +60,9 @@ __device__ __forceinline__ void unpack16x8(const uint4& q, float (&f)[8], int fm
 // ---------------------------------------------------------------------------------------------
 template <int VEC>
 __global__ void __launch_bounds__(256) k_append(float* __restrict__ ring, const float* __restrict__ src,
-                                                long long* count, unsigned* ticket, int n_rows, int W, int S) {
+                                                long long* count, unsigned* ticket, int n_rows, int W, int S,
+                                                unsigned long long* stamp) {
+    stamp_begin(stamp);
     const long long cnt = *count;
     const int h = static_cast<int>(cnt % W);
     const int per_row = S / VEC;
@@ -72,18 +90,20 @@ __global__ void __launch_bounds__(256) k_append(float* __restrict__ ring, const 
             __threadfence();
         }
     }
+    stamp_end(stamp);
 }
 
-void launch_append(float* ring, const float* new_samples, long long* count, unsigned* ticket, int n_rows, int W,
-                   int S, cudaStream_t st) {
+cudaError_t launch_append(float* ring, const float* new_samples, long long* count, unsigned* ticket, int n_rows, int W,
+                          int S, Stamp stamp, cudaStream_t st) {
     const bool vec = (S % 4 == 0) && (W % 4 == 0);
     const long long total = static_cast<long long>(n_rows) * (vec ? S / 4 : S);
     int blocks = static_cast<int>((total + 255) / 256);
     if (blocks > 148 * 8) blocks = 148 * 8;
     if (blocks < 1) blocks = 1;
-    if (vec) k_append<4><<<blocks, 256, 0, st>>>(ring, new_samples, count, ticket, n_rows, W, S);
-    else k_append<1><<<blocks, 256, 0, st>>>(ring, new_samples, count, ticket, n_rows, W, S);
-    ++g_kernel_launches;
+    if (vec) k_append<4><<<blocks, 256, 0, st>>>(ring, new_samples, count, ticket, n_rows, W, S, stamp);
+    else k_append<1><<<blocks, 256, 0, st>>>(ring, new_samples, count, ticket, n_rows, W, S, stamp);
+    count_launch();
+    return cudaGetLastError();
 }
 
 bool is_append_kernel(const void* func) {
@@ -105,12 +125,13 @@ __global__ void __launch_bounds__(256) k_snapshot(const float* __restrict__ ring
     }
 }
 
-void launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st) {
+cudaError_t launch_snapshot(const float* ring, float* out, const long long* count, int n_rows, int W, cudaStream_t st) {
     const long long total = static_cast<long long>(n_rows) * W;
     int blocks = static_cast<int>((total + 255) / 256);
     if (blocks > 148 * 16) blocks = 148 * 16;
     k_snapshot<<<blocks, 256, 0, st>>>(ring, out, count, n_rows, W);
-    ++g_kernel_launches;
+    count_launch();
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -127,8 +148,10 @@ constexpr int kGatherPos = 128;
 __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, void* __restrict__ xw,
                                                 const long long* count, const int* __restrict__ rows_map,
                                                 int channels, int n_det, int n_wit, int W, int cpad, int fmt,
-                                                long long seg_T, int seg_S, const float* __restrict__ pre) {
+                                                long long seg_T, int seg_S, const float* __restrict__ pre,
+                                                unsigned long long* stamp) {
     __shared__ float tile[32][kGatherPos + 1];
+    stamp_begin(stamp);
     const int h = seg_T > 0 ? 0 : static_cast<int>(*count % W);
     const int sd = blockIdx.y;                       // stream * n_det + det
     const int s = sd / n_det, d = sd % n_det;
@@ -172,14 +195,17 @@ __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, 
             *reinterpret_cast<uint4*>(dst) = q;
         }
     }
+    __syncthreads();
+    stamp_end(stamp);
 }
 
-void launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
-                   int channels, int n_det, int n_wit, int W, int cpad, int fmt, const float* pre, cudaStream_t st,
-                   long long seg_T, int seg_S) {
+cudaError_t launch_gather(const float* ring, void* xw, const long long* count, const int* rows_map, int n_streams,
+                          int channels, int n_det, int n_wit, int W, int cpad, int fmt, const float* pre, Stamp stamp,
+                          cudaStream_t st, long long seg_T, int seg_S) {
     dim3 grid((W + kGatherPos - 1) / kGatherPos, n_streams * n_det, cpad / 32);
-    k_gather<<<grid, 256, 0, st>>>(ring, xw, count, rows_map, channels, n_det, n_wit, W, cpad, fmt, seg_T, seg_S, pre);
-    ++g_kernel_launches;
+    k_gather<<<grid, 256, 0, st>>>(ring, xw, count, rows_map, channels, n_det, n_wit, W, cpad, fmt, seg_T, seg_S, pre, stamp);
+    count_launch();
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -194,8 +220,9 @@ void launch_gather(const float* ring, void* xw, const long long* count, const in
 __global__ void __launch_bounds__(256) k_ring16_append(const float* __restrict__ src, void* __restrict__ ring16,
                                                        const long long* count, const int* __restrict__ rows_map,
                                                        int channels, int n_det, int n_wit, int W, int S, int cpad,
-                                                       int fmt, const float* __restrict__ pre) {
+                                                       int fmt, const float* __restrict__ pre, unsigned long long* stamp) {
     __shared__ float tile[32][kGatherPos + 1];
+    stamp_begin(stamp);
     const int h0 = static_cast<int>((*count - S) % W);   // ring slot of this update's first sample
     const int sd = blockIdx.y;
     const int s = sd / n_det, d = sd % n_det;
@@ -237,6 +264,8 @@ __global__ void __launch_bounds__(256) k_ring16_append(const float* __restrict__
             *reinterpret_cast<uint4*>(dst + static_cast<size_t>(W) * cpad) = q;
         }
     }
+    __syncthreads();
+    stamp_end(stamp);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -251,8 +280,9 @@ __global__ void __launch_bounds__(256) k_snapshot_append(float* __restrict__ rin
                                                          void* __restrict__ ring16, long long* count, unsigned* ticket,
                                                          const int* __restrict__ rows_map, const float* __restrict__ pre,
                                                          int channels, int n_det, int n_wit, int W, int S, int cpad,
-                                                         int fmt) {
+                                                         int fmt, unsigned long long* stamp) {
     __shared__ float tile[32][kGatherPos + 1];
+    stamp_begin(stamp);
     const long long cnt = *count;
     const int h0 = static_cast<int>(cnt % W);              // ring slot of this update's first sample
     const int sd = blockIdx.y;
@@ -322,27 +352,30 @@ __global__ void __launch_bounds__(256) k_snapshot_append(float* __restrict__ rin
             __threadfence();
         }
     }
+    stamp_end(stamp);
 }
 
 bool is_snapshot_append_kernel(const void* func) { return func == reinterpret_cast<const void*>(&k_snapshot_append); }
 
-void launch_snapshot_append(float* ring, const float* new_samples, void* ring16, long long* count, unsigned* ticket,
-                            const int* rows_map, const float* pre, int n_streams, int channels, int n_det, int n_wit, int W,
-                            int S, int cpad, int fmt, cudaStream_t st) {
+cudaError_t launch_snapshot_append(float* ring, const float* new_samples, void* ring16, long long* count, unsigned* ticket,
+                                   const int* rows_map, const float* pre, int n_streams, int channels, int n_det, int n_wit,
+                                   int W, int S, int cpad, int fmt, Stamp stamp, cudaStream_t st) {
     dim3 grid((S + kGatherPos - 1) / kGatherPos, n_streams * n_det);
     k_snapshot_append<<<grid, 256, 0, st>>>(ring, new_samples, ring16, count, ticket, rows_map, pre, channels, n_det, n_wit, W,
-                                            S, cpad, fmt);
-    ++g_kernel_launches;
+                                            S, cpad, fmt, stamp);
+    count_launch();
+    return cudaGetLastError();
 }
 
 bool is_ring16_append_kernel(const void* func) { return func == reinterpret_cast<const void*>(&k_ring16_append); }
 
-void launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
-                          int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
-                          const float* pre, cudaStream_t st) {
+cudaError_t launch_ring16_append(const float* new_samples, void* ring16, const long long* count, const int* rows_map,
+                                 int n_streams, int channels, int n_det, int n_wit, int W, int S, int cpad, int fmt,
+                                 const float* pre, Stamp stamp, cudaStream_t st) {
     dim3 grid((S + kGatherPos - 1) / kGatherPos, n_streams * n_det, cpad / 32);
-    k_ring16_append<<<grid, 256, 0, st>>>(new_samples, ring16, count, rows_map, channels, n_det, n_wit, W, S, cpad, fmt, pre);
-    ++g_kernel_launches;
+    k_ring16_append<<<grid, 256, 0, st>>>(new_samples, ring16, count, rows_map, channels, n_det, n_wit, W, S, cpad, fmt, pre, stamp);
+    count_launch();
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -379,8 +412,10 @@ __global__ void __launch_bounds__(kFcThreads, 2) k_final_convt(const void* __res
                                                                const float* __restrict__ wt,
                                                                const float* __restrict__ bias,
                                                                float* __restrict__ pred, int n_items, int n_det,
-                                                               int L, int cpad, int K, int pad, int fmt) {
+                                                               int L, int cpad, int K, int pad, int fmt,
+                                                               unsigned long long* stamp) {
     __shared__ float t_s[2][kFcMaxK][kFcRows + 4];
+    stamp_begin(stamp);
     const int det = blockIdx.x % n_det;
     const int worker = blockIdx.x / n_det, n_workers = gridDim.x / n_det;
     const int rows_out = kFcRows - 2 * kFcHalo;
@@ -474,18 +509,21 @@ __global__ void __launch_bounds__(kFcThreads, 2) k_final_convt(const void* __res
             *reinterpret_cast<float2*>(pred + static_cast<size_t>(b) * 2 * L + 2 * l) = make_float2(y[0], y[1]);
         }
     }
+    __syncthreads();
+    stamp_end(stamp);
 }
 
-void launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
-                        int L, int cpad, int K, int pad, int fmt, cudaStream_t st) {
+cudaError_t launch_final_convt(const void* x, const float* wt, const float* bias, float* pred, int batch, int n_det,
+                               int L, int cpad, int K, int pad, int fmt, Stamp stamp, cudaStream_t st) {
     const int rows_out = kFcRows - 2 * kFcHalo;
     const int n_items = batch / n_det;
     const int total = n_items * ((L + rows_out - 1) / rows_out);
     int workers = (148 * 2) / n_det;
     if (workers > total) workers = total;
     if (workers < 1) workers = 1;
-    k_final_convt<<<workers * n_det, kFcThreads, 0, st>>>(x, wt, bias, pred, n_items, n_det, L, cpad, K, pad, fmt);
-    ++g_kernel_launches;
+    k_final_convt<<<workers * n_det, kFcThreads, 0, st>>>(x, wt, bias, pred, n_items, n_det, L, cpad, K, pad, fmt, stamp);
+    count_launch();
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -500,46 +538,50 @@ void launch_final_convt(const void* x, const float* wt, const float* bias, float
 // Algorithmic traffic: read p, acc, strain; write acc, cleaned  = 20 bytes per sample.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
+    stamp_begin(a.stamp);
     const long long cnt = *a.count;
     const int W = a.W, S = a.S;
     const int h = static_cast<int>(cnt % W);
     const int sd = blockIdx.y;
     const int s = sd / a.n_det, d = sd % a.n_det;
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= W) return;
-    const long long abs_idx = cnt - W + n;
-    int slot = h + n;
-    if (slot >= W) slot -= W;
-    const size_t wi = static_cast<size_t>(sd) * W;
-    float nhat = 0.f, cleaned = 0.f;
-    if (abs_idx >= 0) {
-        const float p = __ldg(a.pred + wi + n);
-        if (a.agg == 0) {
-            const float prev = (n >= W - S) ? 0.f : a.acc[wi + slot];
-            const float acc = fmaf(__ldg(a.hann + n), p, prev);
-            a.acc[wi + slot] = acc;
-            nhat = acc * __ldg(a.inv_wsum + n);
-        } else {
-            if (n >= W - a.delta) nhat = 0.f;
-            else if (n >= W - S - a.delta) { nhat = p; a.acc[wi + slot] = p; }
-            else nhat = a.acc[wi + slot];
+    if (n < W) {
+        const long long abs_idx = cnt - W + n;
+        int slot = h + n;
+        if (slot >= W) slot -= W;
+        const size_t wi = static_cast<size_t>(sd) * W;
+        float nhat = 0.f, cleaned = 0.f;
+        if (abs_idx >= 0) {
+            const float p = __ldg(a.pred + wi + (a.pred_ring ? slot : n));
+            if (a.agg == 0) {
+                const float prev = (n >= W - S) ? 0.f : a.acc[wi + slot];
+                const float acc = fmaf(__ldg(a.hann + n), p, prev);
+                a.acc[wi + slot] = acc;
+                nhat = acc * __ldg(a.inv_wsum + n);
+            } else {
+                if (n >= W - a.delta) nhat = 0.f;
+                else if (n >= W - S - a.delta) { nhat = p; a.acc[wi + slot] = p; }
+                else nhat = a.acc[wi + slot];
+            }
+            if (a.agg == 0 || n < W - a.delta)                 // post-processing: estimate back to strain units
+                nhat = fmaf(__ldg(a.post + 2 * d), nhat, __ldg(a.post + 2 * d + 1));
+            const float strain = __ldg(a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot);
+            cleaned = strain - nhat;
         }
-        if (a.agg == 0 || n < W - a.delta)                 // post-processing: estimate back to strain units
-            nhat = fmaf(__ldg(a.post + 2 * d), nhat, __ldg(a.post + 2 * d + 1));
-        const float strain = __ldg(a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot);
-        cleaned = strain - nhat;
+        if (a.running_out) a.running_out[wi + n] = cleaned;
+        if (a.nhat_out) a.nhat_out[wi + n] = nhat;
+        if (a.final_out) {
+            const int f0 = (a.agg == 0) ? 0 : W - S - a.delta;
+            const int i = n - f0;
+            if (i >= 0 && i < S) a.final_out[static_cast<size_t>(sd) * S + i] = cleaned;
+        }
+        if (a.clf_in) {
+            const int i = n - (W - a.delta - a.Lb);
+            if (i >= 0 && i < a.Lb) a.clf_in[static_cast<size_t>(sd) * a.Lb + i] = cleaned;
+        }
     }
-    if (a.running_out) a.running_out[wi + n] = cleaned;
-    if (a.nhat_out) a.nhat_out[wi + n] = nhat;
-    if (a.final_out) {
-        const int f0 = (a.agg == 0) ? 0 : W - S - a.delta;
-        const int i = n - f0;
-        if (i >= 0 && i < S) a.final_out[static_cast<size_t>(sd) * S + i] = cleaned;
-    }
-    if (a.clf_in) {
-        const int i = n - (W - a.delta - a.Lb);
-        if (i >= 0 && i < a.Lb) a.clf_in[static_cast<size_t>(sd) * a.Lb + i] = cleaned;
-    }
+    __syncthreads();
+    stamp_end(a.stamp);
 }
 
 // The same, four consecutive samples per thread with 128-bit accesses.  Requires W, S, delta, Lb multiples
@@ -547,51 +589,55 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
 // four, so a group never straddles the wrap, the newest stride, the final block or the classifier window.
 // (The scalar kernel spent its time on per-sample index arithmetic: ncu SM throughput 72 %, 1.9 TB/s.)
 __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
+    stamp_begin(a.stamp);
     const long long cnt = *a.count;
     const int W = a.W, S = a.S;
     const int h = static_cast<int>(cnt % W);
     const int sd = blockIdx.y;
     const int s = sd / a.n_det, d = sd % a.n_det;
     const int n = 4 * (blockIdx.x * blockDim.x + threadIdx.x);
-    if (n >= W) return;
-    const long long abs_idx = cnt - W + n;                 // cnt, W, n multiples of 4: the group is all >= 0 or all < 0
-    int slot = h + n;
-    if (slot >= W) slot -= W;
-    const size_t wi = static_cast<size_t>(sd) * W;
-    float4 nhat = make_float4(0.f, 0.f, 0.f, 0.f), cleaned = nhat;
-    if (abs_idx >= 0) {
-        const float4 p = __ldg(reinterpret_cast<const float4*>(a.pred + wi + n));
-        float4* accp = reinterpret_cast<float4*>(a.acc + wi + slot);
-        if (a.agg == 0) {
-            const float4 prev = (n >= W - S) ? make_float4(0.f, 0.f, 0.f, 0.f) : *accp;
-            const float4 hw = __ldg(reinterpret_cast<const float4*>(a.hann + n));
-            const float4 iw = __ldg(reinterpret_cast<const float4*>(a.inv_wsum + n));
-            const float4 acc = make_float4(fmaf(hw.x, p.x, prev.x), fmaf(hw.y, p.y, prev.y), fmaf(hw.z, p.z, prev.z), fmaf(hw.w, p.w, prev.w));
-            *accp = acc;
-            nhat = make_float4(acc.x * iw.x, acc.y * iw.y, acc.z * iw.z, acc.w * iw.w);
-        } else {
-            if (n >= W - a.delta) nhat = make_float4(0.f, 0.f, 0.f, 0.f);
-            else if (n >= W - S - a.delta) { nhat = p; *accp = p; }
-            else nhat = *accp;
+    if (n < W) {
+        const long long abs_idx = cnt - W + n;                 // cnt, W, n multiples of 4: the group is all >= 0 or all < 0
+        int slot = h + n;
+        if (slot >= W) slot -= W;
+        const size_t wi = static_cast<size_t>(sd) * W;
+        float4 nhat = make_float4(0.f, 0.f, 0.f, 0.f), cleaned = nhat;
+        if (abs_idx >= 0) {
+            const float4 p = __ldg(reinterpret_cast<const float4*>(a.pred + wi + (a.pred_ring ? slot : n)));
+            float4* accp = reinterpret_cast<float4*>(a.acc + wi + slot);
+            if (a.agg == 0) {
+                const float4 prev = (n >= W - S) ? make_float4(0.f, 0.f, 0.f, 0.f) : *accp;
+                const float4 hw = __ldg(reinterpret_cast<const float4*>(a.hann + n));
+                const float4 iw = __ldg(reinterpret_cast<const float4*>(a.inv_wsum + n));
+                const float4 acc = make_float4(fmaf(hw.x, p.x, prev.x), fmaf(hw.y, p.y, prev.y), fmaf(hw.z, p.z, prev.z), fmaf(hw.w, p.w, prev.w));
+                *accp = acc;
+                nhat = make_float4(acc.x * iw.x, acc.y * iw.y, acc.z * iw.z, acc.w * iw.w);
+            } else {
+                if (n >= W - a.delta) nhat = make_float4(0.f, 0.f, 0.f, 0.f);
+                else if (n >= W - S - a.delta) { nhat = p; *accp = p; }
+                else nhat = *accp;
+            }
+            if (a.agg == 0 || n < W - a.delta) {               // post-processing: estimate back to strain units
+                const float ps = __ldg(a.post + 2 * d), pm = __ldg(a.post + 2 * d + 1);
+                nhat = make_float4(fmaf(ps, nhat.x, pm), fmaf(ps, nhat.y, pm), fmaf(ps, nhat.z, pm), fmaf(ps, nhat.w, pm));
+            }
+            const float4 st4 = __ldg(reinterpret_cast<const float4*>(
+                a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot));
+            cleaned = make_float4(st4.x - nhat.x, st4.y - nhat.y, st4.z - nhat.z, st4.w - nhat.w);
         }
-        if (a.agg == 0 || n < W - a.delta) {               // post-processing: estimate back to strain units
-            const float ps = __ldg(a.post + 2 * d), pm = __ldg(a.post + 2 * d + 1);
-            nhat = make_float4(fmaf(ps, nhat.x, pm), fmaf(ps, nhat.y, pm), fmaf(ps, nhat.z, pm), fmaf(ps, nhat.w, pm));
+        if (a.running_out) *reinterpret_cast<float4*>(a.running_out + wi + n) = cleaned;
+        if (a.nhat_out) *reinterpret_cast<float4*>(a.nhat_out + wi + n) = nhat;
+        if (a.final_out) {
+            const int i = n - ((a.agg == 0) ? 0 : W - S - a.delta);
+            if (i >= 0 && i < S) *reinterpret_cast<float4*>(a.final_out + static_cast<size_t>(sd) * S + i) = cleaned;
         }
-        const float4 st4 = __ldg(reinterpret_cast<const float4*>(
-            a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot));
-        cleaned = make_float4(st4.x - nhat.x, st4.y - nhat.y, st4.z - nhat.z, st4.w - nhat.w);
+        if (a.clf_in) {
+            const int i = n - (W - a.delta - a.Lb);
+            if (i >= 0 && i < a.Lb) *reinterpret_cast<float4*>(a.clf_in + static_cast<size_t>(sd) * a.Lb + i) = cleaned;
+        }
     }
-    if (a.running_out) *reinterpret_cast<float4*>(a.running_out + wi + n) = cleaned;
-    if (a.nhat_out) *reinterpret_cast<float4*>(a.nhat_out + wi + n) = nhat;
-    if (a.final_out) {
-        const int i = n - ((a.agg == 0) ? 0 : W - S - a.delta);
-        if (i >= 0 && i < S) *reinterpret_cast<float4*>(a.final_out + static_cast<size_t>(sd) * S + i) = cleaned;
-    }
-    if (a.clf_in) {
-        const int i = n - (W - a.delta - a.Lb);
-        if (i >= 0 && i < a.Lb) *reinterpret_cast<float4*>(a.clf_in + static_cast<size_t>(sd) * a.Lb + i) = cleaned;
-    }
+    __syncthreads();
+    stamp_end(a.stamp);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -627,15 +673,20 @@ __global__ void __launch_bounds__(256) k_ola_offline(const float* __restrict__ p
     if (nhat_out) nhat_out[static_cast<size_t>(d) * T + a] = nhat;
 }
 
-void launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann, const double* cum,
-                        float* cleaned, float* nhat_out, int B, int n_det, int W, int S, long long T, const float* post,
-                        cudaStream_t st) {
+cudaError_t launch_ola_offline(const float* pred, const float* seg, const int* strain_rows, const float* hann,
+                               const double* cum, float* cleaned, float* nhat_out, int B, int n_det, int W, int S,
+                               long long T, const float* post, cudaStream_t st) {
     dim3 grid(static_cast<unsigned>((T + 255) / 256), n_det);
     k_ola_offline<<<grid, 256, 0, st>>>(pred, seg, strain_rows, hann, cum, cleaned, nhat_out, B, n_det, W, S, T, post);
-    ++g_kernel_launches;
+    count_launch();
+    return cudaGetLastError();
 }
 
-void launch_aggregate(const AggParams& a, cudaStream_t st) {
+bool is_aggregate_kernel(const void* func) {
+    return func == reinterpret_cast<const void*>(&k_aggregate) || func == reinterpret_cast<const void*>(&k_aggregate_v4);
+}
+
+cudaError_t launch_aggregate(const AggParams& a, cudaStream_t st) {
     auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };   // null counts as aligned
     const bool vec = a.W % 4 == 0 && a.S % 4 == 0 && a.delta % 4 == 0 && (a.clf_in == nullptr || a.Lb % 4 == 0) &&
                      al16(a.pred) && al16(a.acc) && al16(a.ring) && al16(a.hann) && al16(a.inv_wsum) && al16(a.final_out) &&
@@ -647,7 +698,8 @@ void launch_aggregate(const AggParams& a, cudaStream_t st) {
         dim3 grid((a.W + 255) / 256, a.n_streams * a.n_det);
         k_aggregate<<<grid, 256, 0, st>>>(a);
     }
-    ++g_kernel_launches;
+    count_launch();
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -671,8 +723,10 @@ constexpr int kC1Span = kC1Q * 4 + 12;
 template <int CIN>
 __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ x, const float* __restrict__ w,
                                                       const float* __restrict__ bias, void* __restrict__ out,
-                                                      int L, int cout, int cpad, int K, int pad_l, int fmt) {
+                                                      int L, int cout, int cpad, int K, int pad_l, int fmt,
+                                                      unsigned long long* stamp) {
     constexpr int cin = CIN;
+    stamp_begin(stamp);
     __shared__ __align__(16) float xs[kC1MaxCin][kC1Span];
     __shared__ __align__(16) float ws[32][kC1MaxCin][8];      // this block's 32 channels, zero where unused
     __shared__ float bs[32];
@@ -736,22 +790,25 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
             *reinterpret_cast<uint4*>(reinterpret_cast<uint16_t*>(out) + (static_cast<size_t>(b) * Lq + q) * cpad + cbase + cg * 8) = o;
         }
     }
+    __syncthreads();
+    stamp_end(stamp);
 }
 
-void launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
-                      int cout, int cpad, int K, int pad_l, int pool, int fmt, cudaStream_t st) {
+cudaError_t launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
+                             int cout, int cpad, int K, int pad_l, int pool, int fmt, Stamp stamp, cudaStream_t st) {
     (void)pool;                                        // validated == 4 at create time
     const int Lq = L / 4;
     int tiles = (Lq + kC1Q - 1) / kC1Q;
     if (static_cast<long long>(tiles) * batch >= 148 * 8) tiles = (tiles + 3) / 4;   // enough blocks: four tiles per block
     dim3 grid(tiles, batch, cpad / 32);
     switch (n_det) {                                   // cin = number of detectors (validated <= 4 at create time)
-        case 1: k_bbh_conv1<1><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
-        case 2: k_bbh_conv1<2><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
-        case 3: k_bbh_conv1<3><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
-        default: k_bbh_conv1<4><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt); break;
+        case 1: k_bbh_conv1<1><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
+        case 2: k_bbh_conv1<2><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
+        case 3: k_bbh_conv1<3><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
+        default: k_bbh_conv1<4><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
     }
-    ++g_kernel_launches;
+    count_launch();
+    return cudaGetLastError();
 }
 
 }  // namespace gw

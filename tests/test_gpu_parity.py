@@ -41,15 +41,12 @@ def test_snapshot_bit_exact(n, C, W, S_):
 
 # --------------------------------------------------------------------- DeepClean streaming (C0)
 def _run_streaming(cfg, dtype, n_up, white, agg=S.AGG_HANN_OLA, delta=0, check_scores=True, impl=gw.GW_IMPL_UMMA,
-                   use_graph=False):
-    gw.set_conv_impl(impl)
-    try:
-        st_spec = cfg.stream
-        dc_params, bbh_params = util.make_params(cfg)
-        x = synth.multi_stream(cfg.seed, st_spec, n_up * st_spec.stride, white=white)
-        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, agg, delta)
-    finally:
-        gw.set_conv_impl(gw.GW_IMPL_UMMA)
+                   use_graph=False, incremental=False):
+    st_spec = cfg.stream
+    dc_params, bbh_params = util.make_params(cfg)
+    x = synth.multi_stream(cfg.seed, st_spec, n_up * st_spec.stride, white=white)
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, agg, delta,
+                                              gw.Options(conv_impl=impl, incremental=incremental))
     oracles = [util.make_stream_oracle(cfg, dc_params, bbh_params, dtype, n_up, agg, delta)
                for _ in range(st_spec.n_streams)]
     xd = _dev(x)
@@ -141,11 +138,7 @@ def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype, fuse):
     dc_params, _ = util.make_params(cfg)
     dc_params2 = [dc_params[0]]
     st = gw.Stream(cfg.stream)
-    gw.set_fuse_tail(fuse)
-    try:
-        dc = gw.DeepClean(st, cfg.dc_layers, dc_params2, dtype)
-    finally:
-        gw.set_fuse_tail(True)
+    dc = gw.DeepClean(st, cfg.dc_layers, dc_params2, dtype, opts=gw.Options(fuse_tail=fuse))
     if fuse:
         with pytest.raises(gw.GwError) as e:
             dc.activation(len(cfg.dc_layers) - 2)
@@ -258,6 +251,78 @@ def test_small_ensemble_latency_offset_through_the_graph():
     _run_streaming(cfg, gw.GW_FP16, cfg.n_updates, white=False, agg=S.AGG_LAST_STRIDE, delta=256, use_graph=True)
 
 
+# ------------------------------------------------ D13 incremental path (gw_options.incremental)
+@pytest.mark.parametrize("W,S_,n,dtype", [(2048, 256, 3, gw.GW_FP16), (8192, 512, 2, gw.GW_BF16), (32768, 512, 2, gw.GW_FP16),
+                                          (4096, 16, 1, gw.GW_FP16)])
+def test_incremental_path_is_bit_identical_to_full_recompute(W, S_, n, dtype):
+    """DESIGN.md D13: with gw_options.incremental every layer's activations live in rings
+    over absolute position and an update recomputes only the rows near the two window edges (tests/test_oracle_pins.py
+    pins which).  The result must be the SAME NUMBERS as full recomputation: raw prediction, final cleaned samples and
+    scores compared with array_equal over more than 2 W/S updates, warm-up included (the first update fills the rings
+    with whole windows), through the CUDA graph; the stored activations of every layer as well at the end."""
+    cfg0 = S.config_c3(n, S_, W)
+    Lb = min(4096, W // 2)
+    cfg = S.Config("inc", cfg0.stream, cfg0.dc_layers, cfg0.bbh_convs, cfg0.bbh_dense, Lb, 0, 11)
+    sp = cfg.stream
+    k = W // S_
+    n_up = min(2 * k + 5, 300)
+    dc_params, bbh_params = util.make_params(cfg)
+    x = synth.multi_stream(cfg.seed, sp, n_up * S_)
+    xc = torch.from_numpy(np.ascontiguousarray(x.reshape(n, sp.channels, n_up, S_).transpose(2, 0, 1, 3))).cuda()
+    outs, acts = {}, {}
+    for inc in (0, 1):
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, opts=gw.Options(incremental=inc))
+        cs = torch.cuda.Stream()
+        sc = torch.zeros(n, device="cuda")
+        fin = torch.zeros((n, sp.n_det, S_), device="cuda")
+        torch.cuda.synchronize()
+        res = []
+        for t in range(n_up):
+            pipe.step(xc[t], sc, fin, cs)
+            cs.synchronize()
+            if t < 4 or t % 7 == 0 or t >= n_up - 3:
+                res.append((t, dc.noise().cpu().numpy(), fin.cpu().numpy().copy(), sc.cpu().numpy().copy()))
+        outs[inc] = res
+        acts[inc] = [dc.activation(li).cpu().view(torch.int16).numpy() for li in range(-1, len(cfg.dc_layers) - 2)]
+        if inc:
+            assert pipe.graph_nodes() == outs_nodes, "same kernels per step either way"
+        else:
+            outs_nodes = pipe.graph_nodes()
+    for (t, p0, f0, s0), (_, p1, f1, s1) in zip(outs[0], outs[1]):
+        assert np.array_equal(p0, p1), ("pred", t, np.argwhere(p0 != p1)[:4])
+        assert np.array_equal(f0, f1), ("final", t)
+        assert np.array_equal(s0, s1), ("scores", t)
+    for li, (a0, a1) in enumerate(zip(acts[0], acts[1])):
+        assert np.array_equal(a0, a1), ("activation after layer", li - 1)
+
+
+@pytest.mark.parametrize("dtype", [gw.GW_FP16, gw.GW_BF16])
+def test_incremental_path_matches_oracle_eager_and_graph(dtype):
+    """The oracle parity suite of the small ensemble with the incremental path switched on (the oracle is unchanged:
+    it recomputes every window from scratch)."""
+    cfg = S.config_small_ensemble(2)
+    _run_streaming(cfg, dtype, cfg.n_updates, white=False, incremental=True)
+    _run_streaming(cfg, dtype, cfg.n_updates, white=False, incremental=True, use_graph=True)
+    _run_streaming(cfg, dtype, cfg.n_updates, white=False, incremental=True, agg=S.AGG_LAST_STRIDE, delta=256)
+
+
+def test_incremental_path_rejects_shapes_it_cannot_serve():
+    cfg = S.config_c0()                                  # W = 512: not a multiple of 128 * 2^3
+    dc_params, _ = util.make_params(cfg)
+    st = gw.Stream(cfg.stream)
+    with pytest.raises(gw.GwError) as e:
+        gw.DeepClean(st, cfg.dc_layers, dc_params, gw.GW_FP16, opts=gw.Options(incremental=1))
+    assert e.value.code == gw.GW_EINVAL and "incremental" in str(e.value)
+    cfg2 = S.Config("odd", S.StreamSpec(1, 2, 4096, 2048, 200), S.config_c1().dc_layers, seed=1)   # 200 % 16 != 0
+    st2 = gw.Stream(cfg2.stream)
+    with pytest.raises(gw.GwError):
+        gw.DeepClean(st2, cfg2.dc_layers, [synth.deepclean_params(d, cfg2.dc_layers) for d in range(2)], gw.GW_FP16,
+                     agg=S.AGG_LAST_STRIDE, opts=gw.Options(incremental=1))
+    with pytest.raises(gw.GwError):
+        gw.DeepClean(st2, cfg2.dc_layers, [synth.deepclean_params(d, cfg2.dc_layers) for d in range(2)], gw.GW_FP16,
+                     agg=S.AGG_LAST_STRIDE, opts=gw.Options(incremental=1, conv_impl=gw.GW_IMPL_SIMT))
+
+
 def test_results_do_not_depend_on_batching():
     """updates are serial per stream, streams are independent: stream i's results are
     bit-identical whether it runs alone or batched with others."""
@@ -331,8 +396,9 @@ def test_call_order_is_enforced():
 
 # ------------------------------------------------- full size: the launch configuration bench.py times
 @pytest.mark.gpu
-@pytest.mark.parametrize("dtype,n,full_chain", [(gw.GW_FP16, 128, True), (gw.GW_BF16, 128, False), (gw.GW_FP16, 512, False)])
-def test_full_size_c4_sampled_streams_match_oracle(dtype, n, full_chain):
+@pytest.mark.parametrize("dtype,n,full_chain,incremental", [(gw.GW_FP16, 128, True, False), (gw.GW_BF16, 128, False, False),
+                                                           (gw.GW_FP16, 512, False, False), (gw.GW_FP16, 128, False, True)])
+def test_full_size_c4_sampled_streams_match_oracle(dtype, n, full_chain, incremental):
     """BASELINE.json configs[4] as bench.py runs it: n = 128 (and 512) streams x 2 detectors, W = 32768, S = 512, one
     CUDA-graph launch per stride -- every CTA of the persistent conv GEMMs walks many tiles, weight blocks stream
     through the pair-mode ring, both MMA warps and PDL are live -- compared with the oracle on FULLY POPULATED windows:
@@ -352,7 +418,7 @@ def test_full_size_c4_sampled_streams_match_oracle(dtype, n, full_chain):
     base = np.stack([synth.stream_channels(cfg.seed + i, one, n_up * sp.stride) for i in range(3)])
     sampled = {0: 0, 77: 1, n - 1: 2}                    # stream index -> which base signal it carries
     which = np.array([sampled.get(i, i % 3) for i in range(n)])
-    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype)
+    stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, opts=gw.Options(incremental=incremental))
     oracles = {i: util.make_stream_oracle(S.config_c3(1, 512, 32768), dc_params, bbh_params, dtype, n_up) for i in sampled}
     base_d = _dev(base)
     which_d = torch.from_numpy(which).cuda()
@@ -400,7 +466,7 @@ def test_full_size_c4_sampled_streams_match_oracle(dtype, n, full_chain):
                 j = {0: 0, 1: 77, 2: n - 1}[which[i]]
                 assert np.array_equal(pred[i], pred[j]), (t, i, j)
                 assert np.array_equal(final[i], final[j]) and scores[i] == scores[j], (t, i, j)
-    print(f"full size n={n} dtype={'bf16' if dtype == gw.GW_BF16 else 'fp16'}: fully populated windows, worst |d|/RMS "
+    print(f"full size n={n} dtype={'bf16' if dtype == gw.GW_BF16 else 'fp16'}{' incremental' if incremental else ''}: fully populated windows, worst |d|/RMS "
           f"pred {worst['pred']:.3e} final {worst['final']:.3e}, worst |d score| {worst['score']:.2e}")
 
 
@@ -756,6 +822,51 @@ def test_c3_ten_minute_stream_first_and_late_blocks():
 
 
 @pytest.mark.gpu
+def test_step_profile_decomposes_the_graph_step_and_outputs_rotate_without_recapture():
+    """gwstream_diag.h: gw_step_profile stamps every kernel INSIDE the replayed graph; the exclusive shares add up to
+    the device span of the step, and the profiled step computes the same numbers as a plain gw_step.  Also the
+    ADVICE item: new output buffers are node-parameter updates (results land in the buffer passed to THAT call)."""
+    cfg = S.config_small_ensemble(3)
+    sp = cfg.stream
+    dc_params, bbh_params = util.make_params(cfg)
+    n_up = 8
+    x = synth.multi_stream(cfg.seed, sp, n_up * sp.stride)
+    xc = torch.from_numpy(np.ascontiguousarray(x.reshape(sp.n_streams, sp.channels, n_up, sp.stride).transpose(2, 0, 1, 3))).cuda()
+    res = {}
+    for mode in ("plain", "profiled"):
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, gw.GW_FP16)
+        cs = torch.cuda.Stream()
+        scs = [torch.zeros(sp.n_streams, device="cuda") for _ in range(3)]
+        fins = [torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda") for _ in range(3)]
+        torch.cuda.synchronize()
+        out = []
+        for t in range(n_up):
+            b = t % 3                                    # rotate output buffers every step
+            if mode == "profiled" and t >= 2:
+                rows = pipe.step_profile(xc[t], scs[b], fins[b], cs)
+                labels = [r["label"] for r in rows]
+                assert labels[0] == "snapshot_append" and "aggregate" in labels and labels[-1].startswith("gemm.bbh")
+                assert len(rows) == pipe.graph_nodes() == 12
+                prev_end, span = 0.0, 0.0
+                for r in rows:
+                    assert r["end_us"] > r["begin_us"] >= 0.0, r
+                    span += max(0.0, r["end_us"] - max(r["begin_us"], prev_end))
+                    prev_end = max(prev_end, r["end_us"])
+                # exclusive shares + idle gaps between kernels = end of the last kernel
+                assert 0.5 * prev_end < span <= prev_end + 1e-6 and prev_end < 5000.0, (span, prev_end)
+                assert sum(r["flops"] for r in rows if r["label"].startswith("gemm.dc")) > 1e9
+            else:
+                pipe.step(xc[t], scs[b], fins[b], cs)
+            cs.synchronize()
+            out.append((fins[b].cpu().numpy().copy(), scs[b].cpu().numpy().copy()))
+        res[mode] = out
+    for t in range(n_up):
+        assert np.array_equal(res["plain"][t][0], res["profiled"][t][0]), t
+        assert np.array_equal(res["plain"][t][1], res["profiled"][t][1]), t
+    assert any(np.any(res["plain"][t][0] != res["plain"][t + 1][0]) for t in range(n_up - 1))
+
+
+@pytest.mark.gpu
 def test_mma_probe_reports_the_operand_read_law():
     """gw_probe_mma_cycles: the measured cycles per tcgen05.mma follow max(N/2, 32 + N/4) within 15 % on this class of
     device (the thin layers' shared-memory roofline in DESIGN.md rests on it); bad N is rejected."""
@@ -810,7 +921,7 @@ def test_handles_release_their_device_memory():
 
 @pytest.mark.gpu
 def test_scheduling_switches_are_bit_identical():
-    """include/gwstream.h promises that gw_set_pdl / _snake / _two_sm / _skip_zeros change scheduling (or skip exact
+    """include/gwstream.h promises that gw_options.pdl / snake / two_sm / skip_zeros change scheduling (or skip exact
     zeros) only.  C3-shaped layers at full window length (the CTA-pair kernel needs an even number of 128-row tiles),
     three streams so that CTAs walk several work items; every switch off in turn, compared bitwise with all on."""
     cfg = S.config_c3(3, 512, 32768)
@@ -819,10 +930,10 @@ def test_scheduling_switches_are_bit_identical():
     n_up = 2
     xc = torch.from_numpy(np.ascontiguousarray(
         synth.multi_stream(cfg.seed, sp, n_up * sp.stride).reshape(sp.n_streams, sp.channels, n_up, sp.stride).transpose(2, 0, 1, 3))).cuda()
-    switches = {"pdl": gw.set_pdl, "snake": gw.set_snake, "two_sm": gw.set_two_sm, "skip_zeros": gw.set_skip_zeros}
+    switches = ("pdl", "snake", "two_sm", "skip_zeros")
 
-    def run():
-        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, gw.GW_FP16)
+    def run(opts=None):
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, gw.GW_FP16, opts=opts)
         cs = torch.cuda.Stream()
         sc = torch.zeros(sp.n_streams, device="cuda")
         fin = torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda")
@@ -835,12 +946,8 @@ def test_scheduling_switches_are_bit_identical():
         return out
 
     base = run()
-    for name, setter in switches.items():
-        setter(False)
-        try:
-            got = run()
-        finally:
-            setter(True)
+    for name in switches:
+        got = run(gw.Options(**{name: 0}))
         for t in range(n_up):
             for a, b, what in zip(got[t], base[t], ("pred", "final", "scores")):
                 assert np.array_equal(a, b), (name, t, what)

@@ -513,6 +513,38 @@ def test_classifier_window_with_latency_offset_is_the_delayed_strain_slice(agg, 
     assert seen_real, "the test must reach windows that lie entirely inside the stream"
 
 
+# ------------------------------------------------ D13 incremental path: which rows change between updates
+@pytest.mark.parametrize("W,S_", [(1024, 64), (2048, 256), (512, 16)])
+def test_incremental_zones_are_exactly_the_rows_that_change_between_overlapping_windows(W, S_):
+    """DESIGN.md D13 (only floor(fs/r) samples are new per update): the oracle run on two overlapping
+    windows [0, W) and [S, S + W) of the same data.  At every layer, output position l of the second window equals
+    position l + S_i of the first one BIT FOR BIT except at the first `left[i]` positions (receptive field reaches the
+    zero-padded left edge) and the last `right[i]` (new samples / right edge); and the bounds are tight: the positions
+    just inside each zone do differ.  left / right come from the engine's host-side recurrence (gw_incremental_zones),
+    so a wrong receptive-field count there fails here, without a GPU."""
+    from paper_2108_12430_b200 import binding
+    layers = S.deepclean_layers([21, 4, 6, 5, 8], bn=False)        # C1's layer kinds, k, strides; narrow for speed
+    left, right = binding.incremental_zones(layers, S_)
+    assert left == [2, 3, 3, 3, 8, 18, 38, 78]
+    assert right == [S_ // 2 + 1, S_ // 4 + 2, S_ // 8 + 2, S_ // 16 + 2, S_ // 8 + 7, S_ // 4 + 17, S_ // 2 + 37, S_ + 77]
+    params = synth.deepclean_params(5, layers)
+    prepared = [oracle.prepare_conv(l, p, oracle.DT_FP16) for l, p in zip(layers, params)]
+    x = RNG.standard_normal((21, W + S_))
+    _, a = oracle.deepclean_forward(x[:, :W], layers, prepared, return_all=True)
+    _, b = oracle.deepclean_forward(x[:, S_:], layers, prepared, return_all=True)
+    for i, (ya, yb) in enumerate(zip(a, b)):
+        L = ya.shape[1]
+        sh = S_ * L // W
+        same = np.all(yb[:, :L - sh] == ya[:, sh:], axis=0)        # per position, all channels
+        lo, hi = left[i], L - right[i]
+        if lo < hi:
+            assert np.all(same[lo:hi]), (i, np.flatnonzero(~same[lo:hi])[:5] + lo)
+        if lo <= L - sh:
+            assert not same[lo - 1], f"layer {i}: left zone {lo} is not tight"
+        if hi >= 0 and hi < L - sh:
+            assert not same[hi], f"layer {i}: right zone {right[i]} is not tight"
+
+
 # ------------------------------------------------------------- error budget of 16-bit storage
 
 def test_bf16_activation_storage_alone_exceeds_the_elementwise_bar():
