@@ -73,6 +73,12 @@ struct ConvGemmParams {
     // new samples or the right window edge).  Full recomputation: v_tiles = v_left = tiles_m.
     int v_tiles, v_left;
     int pred_ring;                 // EPI_FINAL: pred is a ring over absolute sample index mod 4 M (no mirror: row stores)
+    // CTA-pair kernel on a ring input: one tensor map PER WINDOW HEAD (device array of a_ring_W / head_div maps, the
+    // map of head h based at the ring row where that window starts and a_rows rows tall), so that rows outside the
+    // window are TMA's zero fill exactly as for a plain activation tensor -- no zeroing in shared memory, which the
+    // pair kernel (the peer's slab is consumed by the leader's MMAs) has no warp in the right place for.
+    const CUtensorMap* tmA_heads;
+    int head_div;                  // head index = (*a_count mod a_ring_W) / head_div  (= the stride S)
     unsigned long long* stamp;     // profiling graph: [0] = min %globaltimer at CTA start, [1] = max at CTA end; else null
     // EPI_FINAL: this layer (ConvTranspose1d -> 32 channels, tanh) and the network's last layer
     // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel.  The

@@ -67,8 +67,9 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     if (p.two_sm) {
         // CTA-pair kernel: N = 256 store layers with an even number of tiles; half weight blocks of 16 KiB
         const int pairs = sm_count / 2;
-        bool ok = p.epi == EPI_STORE && p.N == 256 && p.a_count == nullptr && p.out_ring_div == 0 && p.tiles_m % 2 == 0 &&
-                  p.v_tiles == p.tiles_m && pairs >= p.n_det;
+        // ring input (incremental path): needs the per-head tensor maps; the pair works on virtual tiles 2u, 2u + 1
+        bool ok = p.epi == EPI_STORE && p.N == 256 && (p.a_count == nullptr || p.tmA_heads != nullptr) && p.v_tiles % 2 == 0 &&
+                  pairs >= p.n_det;
         for (int ob = 2; ok && ob >= 1; --ob) {
             const int fixed = kFixedSmem + ob * kOutStage;
             const int sa = p.n_cb < 2 ? 2 : (p.n_cb > 8 ? 8 : p.n_cb);
@@ -818,7 +819,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
     const int det = cid % p.n_det;
     const int cworker = cid / p.n_det;
     const int n_cw = (gridDim.x / 2) / p.n_det;
-    const int half_tiles = p.tiles_m / 2;                                    // tile pairs per batch item
+    const int half_tiles = p.v_tiles / 2;                                    // (virtual) tile pairs per batch item
     const int total = n_items * half_tiles;
 
     if (warp == 0) {
@@ -850,6 +851,8 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
         // only forced -- blocking -- to have issued slab (item, cb) before the first weight block of that column
         // block (otherwise the weight ring could fill while the MMA warp waits for the slab).
         griddep_wait();
+        // ring input: this update's window has its own tensor map (rows outside the window are zero fill)
+        const CUtensorMap* tmA = p.tmA_heads ? p.tmA_heads + static_cast<int>(*p.a_count % p.a_ring_W) / p.head_div : &p.tmA;
         const uint32_t lead_a_full = mapa_u32(smem_u32(a_full), 0), lead_b_full = mapa_u32(smem_u32(b_full), 0);
         unsigned long long cbstart = 0;
         {
@@ -872,9 +875,9 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
             else if (!__shfl_sync(0xffffffffu, mbar_test_wait(&a_empty[stage], aph ^ 1) ? 1 : 0, 0)) return false;
             if (lane == 0) {
                 const int u = p.reverse ? total - 1 - aw : aw;
-                const int m0 = ((u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
+                const int m0 = map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
                 if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.slab_rows * 128);
-                tma_load_3d_2sm(smem_a + stage * sl, &p.tmA, lead_a_full + 8u * stage, acb * kSegK, m0 + p.a_min,
+                tma_load_3d_2sm(smem_a + stage * sl, tmA, lead_a_full + 8u * stage, acb * kSegK, m0 + p.a_min,
                                 (u / half_tiles) * p.n_det + det);
             }
             if (++stage == sa) { stage = 0; aph ^= 1; }
@@ -953,6 +956,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
         asm volatile("bar.sync 1, 256;" ::: "memory");
         const uint32_t bias_u32 = smem_u32(bias_s);
         griddep_wait();
+        const int out_off = p.out_ring_div ? static_cast<int>(*p.a_count % p.a_ring_W) / p.out_ring_div : 0;
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;
         const uint32_t empty_addr[2] = {mapa_u32(smem_u32(&tmem_empty[0]), 0), mapa_u32(smem_u32(&tmem_empty[1]), 0)};
         int ostep = 0;
@@ -962,7 +966,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
             const int u = p.reverse ? total - 1 - w : w;
             const int acc = it & 1;
             const int batch = (u / half_tiles) * p.n_det + det;
-            const int mt = (u % half_tiles) * 2 + static_cast<int>(rank);
+            const int mt = map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank));
             TR_WAIT(0, mbar_wait(&tmem_full[acc], (it >> 1) & 1))
             tc_fence_after();
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * kAccCols;
@@ -1005,9 +1009,24 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) {
-                    if (mt < p.tiles_m) tma_store_3d(&p.tmOut, stg, col, mt * kTileM + quad * 32, batch);
-                    tma_store_commit();
+                {
+                    // mirror ring (incremental path): ring row r and its twin r +- M; see store_box in k_conv_gemm_umma
+                    const int r = out_off + mt * kTileM + quad * 32;
+                    if (lane == 0) {
+                        tma_store_3d(&p.tmOut, stg, col, r, batch);
+                        if (p.out_ring_div) {
+                            if (r >= p.M) tma_store_3d(&p.tmOut, stg, col, r - p.M, batch);
+                            else tma_store_3d(&p.tmOut, stg, col, r + p.M, batch);
+                        }
+                        tma_store_commit();
+                    }
+                    if (p.out_ring_div && r < p.M && r + 31 >= p.M && r + lane >= p.M) {
+                        uint8_t* dst = reinterpret_cast<uint8_t*>(p.out) +
+                                       ((static_cast<size_t>(batch) * 2 * p.M + (r + lane - p.M)) * p.N + col) * 2;
+#pragma unroll
+                        for (int uu = 0; uu < 8; ++uu)
+                            *reinterpret_cast<float4*>(dst + 16 * uu) = lds_f4(stg + lane * 128 + ((uu ^ (lane & 7)) << 4));
+                    }
                 }
             }
         }
@@ -1157,7 +1176,7 @@ cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     cudaError_t e;
     if (g.p.two_sm) {
         int cw = g.grid / 2 / g.p.n_det;                         // clusters per detector
-        const int units = n_items * (g.p.tiles_m / 2);
+        const int units = n_items * (g.p.v_tiles / 2);
         if (cw > units) cw = units;
         cudaLaunchConfig_t cfg2 = {};
         cfg2.gridDim = dim3(2 * cw * g.p.n_det);

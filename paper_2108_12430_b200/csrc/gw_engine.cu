@@ -269,6 +269,7 @@ struct GemmLayer {
     bool has_inc = false;
     void* d_B = nullptr;
     float* d_bias = nullptr;
+    CUtensorMap* d_heads = nullptr;              // incremental path, CTA-pair layers: one input tensor map per window head
     int impl = GW_IMPL_UMMA;
     std::string name;                            // profiler label, e.g. "gemm.dc3"
     double flops = 0.0;                          // algorithmic FLOPs per batch item, whole window (real channels and taps only)
@@ -410,7 +411,7 @@ extern "C" int gw_incremental_zones(const gw_conv_layer* layers, int n_layers, i
 static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, int n_det, int fmt, const gw_options& opt,
                             const void* in, int in_L, int cin_p, void* out, int cout_p, int batch, int epi,
                             int head_hidden = 0, const long long* ring_count = nullptr, int ring_W = 0,
-                            bool out_ring = false, long long seg_T = 0, int seg_S = 0) {
+                            bool out_ring = false, long long seg_T = 0, int seg_S = 0, int ring_S = 0) {
     const HostLayer& H0 = dets[0];
     ConvGemmParams& p = gl.g.p;
     memset(&p, 0, sizeof p);
@@ -537,6 +538,21 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
         const uint64_t out_rows = out_ring ? 2 * static_cast<uint64_t>(p.M) : p.M;
         if (int rc = make_tmap(&p.tmOut, out, fmt, p.N, out_rows, batch, p.N, out_rows * p.N, 32, p.N >= 64 ? 64 : 32)) return rc;
     }
+    if (out_ring && p.N == 256 && opt.two_sm && ring_S > 0 && ring_W % ring_S == 0) {
+        // CTA-pair kernel on a ring input: a tensor map per window head (see ConvGemmParams::tmA_heads)
+        const int n_heads = ring_W / ring_S;
+        std::vector<CUtensorMap> heads(n_heads);
+        for (int h = 0; h < n_heads; ++h) {
+            const size_t off_rows = static_cast<size_t>(h) * ring_S / p.a_ring_div;
+            const uint16_t* base = static_cast<const uint16_t*>(in) + off_rows * p.a_cols;
+            if (int rc = make_tmap(&heads[h], base, fmt, p.a_cols, p.a_rows, batch, p.a_cols,
+                                   static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, p.slab_rows)) return rc;
+        }
+        CU_TRY(cudaMalloc(&gl.d_heads, sizeof(CUtensorMap) * n_heads));
+        CU_TRY(cudaMemcpy(gl.d_heads, heads.data(), sizeof(CUtensorMap) * n_heads, cudaMemcpyHostToDevice));
+        p.tmA_heads = gl.d_heads;
+        p.head_div = ring_S;
+    }
     gl.g.batch = batch;
     gl.g.pdl = opt.pdl;
     p.head_hidden = head_hidden;
@@ -571,7 +587,10 @@ static void make_incremental_variant(GemmLayer& gl, int left_rows, int right_row
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    conv_gemm_plan(gl.gi, sms);                         // same operand layout; only the tiles-per-stage choice may differ
+    // same operand layout (resident / streamed weights, CTA pair or not: the weight tensor map depends on it); only the
+    // tiles-per-stage choice may differ.  A pair layer whose zones give an odd tile count gets one more left tile.
+    if (p.two_sm && (p.v_tiles & 1)) { p.v_left += 1; p.v_tiles += 1; }
+    conv_gemm_plan(gl.gi, sms);
     gl.has_inc = true;
 }
 
@@ -636,8 +655,8 @@ static void run_gemm(const GemmLayer& gl, LaunchCtx& cx, bool inc = false, int b
 }
 
 static void free_gemm(GemmLayer& gl) {
-    cudaFree(gl.d_B); cudaFree(gl.d_bias);
-    gl.d_B = nullptr; gl.d_bias = nullptr;
+    cudaFree(gl.d_B); cudaFree(gl.d_bias); cudaFree(gl.d_heads);
+    gl.d_B = nullptr; gl.d_bias = nullptr; gl.d_heads = nullptr;
 }
 
 // =============================================================================== snapshotter
@@ -838,7 +857,7 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         if (int rc = build_gemm_layer(dc->gemm[i], gk, per_det.data(), nd, dc->fmt, opt, in,
                                       len[i], cpad[i], dc->act[i + 1], cpad[i + 1], batch, fin ? EPI_FINAL : EPI_STORE, 0,
                                       from_ring ? s->d_count : nullptr, from_ring ? W : 0, dc->inc && !fin,
-                                      from_seg ? dc->off_T : 0, from_seg ? S : 0))
+                                      from_seg ? dc->off_T : 0, from_seg ? S : 0, S))
             return rc;
         dc->gemm[i].g.p.reverse = opt.snake ? (i & 1) : 0;
         dc->gemm[i].name = "gemm.dc" + std::to_string(i);
