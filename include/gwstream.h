@@ -232,6 +232,24 @@ int gw_deepclean_set_scaling(gw_deepclean *dc, const float *wit_mean, const floa
 int gw_offline_set_scaling(gw_offline *o, const float *wit_mean, const float *wit_std, const float *strain_mean,
                            const float *strain_std);
 
+/* Band-limiting of the predicted noise and whitening of the classifier input ("the noise frame ... is
+ * postprocessed then subtracted from the associated strain", :212 "the cleaned strains are combined and postprocessed
+ * then passed to BBHnet"; the paper defines neither operation: DESIGN.md D11, D12 fix them as causal FIR filters whose
+ * taps the caller supplies -- a band-pass for D11, a whitening filter for D12).
+ * gw_deepclean_set_postfilter (D11): the STREAM of emitted estimate samples e[a] (HANN_OLA: the samples that become
+ *   final, LAST_STRIDE: the kept stride; unscaled, 0 before the stream start) is filtered causally with state carried
+ *   from update to update, e~[a] = sum_{j < n_taps} taps[j] e[a - j], and the final cleaned samples (GW_FINAL,
+ *   gw_step's cleaned_final) become strain - (strain_std * e~ + strain_mean).  Running values (GW_RUNNING,
+ *   gw_noise_estimate, the classifier input) are provisional values inside the window and are not filtered.
+ *   taps_host: [n_taps] host floats, copied; 1 <= n_taps <= 64 and n_taps - 1 <= stride; NULL or 0 taps switches it off;
+ *   taps = {1} is a bit-exact no-op.  Before the first update (GW_ESTATE otherwise).
+ * gw_bbh_set_whitening (D12): the classifier sees y_d[i] = sum_{j < n_taps} taps[d][j] x_d[i - j], x_d[i < 0] = 0 (zero
+ *   initial state at the start of the classifier window), for gw_bbh_score, gw_bbh_score_batch and gw_step alike.
+ *   taps_host: [n_det][n_taps], copied; 1 <= n_taps <= 64; NULL or 0 switches it off.  Call it before the first
+ *   gw_step (a captured graph keeps the setting it was captured with). */
+int gw_deepclean_set_postfilter(gw_deepclean *dc, const float *taps_host, int n_taps);
+int gw_bbh_set_whitening(gw_bbh *b, const float *taps_host, int n_taps);
+
 /* ---- offline / non-streaming mode (PAPER.md:174 "adjacent frames ... in parallel", :202 offline regime, :216
  * non-streaming ensemble; D9) ---------------------------------------------------
  * One launch sequence cleans an ARCHIVAL segment of ONE stream: T = window + (n_windows - 1) * stride samples per

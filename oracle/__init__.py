@@ -197,6 +197,22 @@ def hann(W: int) -> np.ndarray:
     return w
 
 
+def fir_causal(x, taps) -> np.ndarray:
+    """D11 / D12: causal FIR with zero initial state along the last axis, y[i] = sum_{j < len(taps)} taps[j] x[i - j],
+    x[i < 0] = 0.  Written out as the definition (one shifted, scaled copy of x per tap), float64.
+    (DESIGN.md readings: PAPER.md:198 "the noise frame is postprocessed then subtracted", :212 "cleaned strains are
+    combined and postprocessed then passed to BBHnet"; the paper defines neither operation.)"""
+    x = _d(x)
+    taps = _d(taps).reshape(-1)
+    y = np.zeros_like(x)
+    n = x.shape[-1]
+    for j in range(len(taps)):
+        if j >= n:
+            break
+        y[..., j:] += taps[j] * x[..., :n - j]
+    return y
+
+
 # ------------------------------------------------------------------------------------- models
 
 def prepare_conv(layer, params: Dict[str, np.ndarray], dtype: int):
@@ -281,7 +297,13 @@ class StreamOracle:
     """
 
     def __init__(self, channels: int, W: int, S: int, rows, dc, bbh=None, agg: int = AGG_HANN_OLA,
-                 delta: int = 0, max_updates: int = 64, scaling=None):
+                 delta: int = 0, max_updates: int = 64, scaling=None, postfilter=None, whiten=None):
+        # postfilter (D11): None or FIR taps [Lh] applied, causally and with carried state, to the
+        # STREAM of emitted (final) estimate samples before rescaling and subtraction; running values are not filtered.
+        # whiten (D12): None or FIR taps [D][Lg] applied to each detector's classifier window with zero
+        # initial state at the window start.
+        self.postfilter = None if postfilter is None else _d(postfilter).reshape(-1)
+        self.whiten = None if whiten is None else _d(whiten)
         # scaling (reading A14): None or (wit_mean [D][n_wit], wit_std [D][n_wit],
         # strain_mean [D], strain_std [D]): the network sees (x - mean) / std of every witness and the
         # aggregated estimate is subtracted as strain_std * nhat + strain_mean.
@@ -294,6 +316,7 @@ class StreamOracle:
         ndet = len(rows)
         self.acc = np.zeros((ndet, self.T), dtype=np.float64)
         self.wsum = np.zeros((ndet, self.T), dtype=np.float64)
+        self.emitted = np.zeros((ndet, self.T), dtype=np.float64)   # D11: emitted estimate samples over absolute index
         self.w = hann(W)
 
     def _cleaned(self, d: int, strain_all: np.ndarray, a0: int, a1: int):
@@ -308,6 +331,33 @@ class StreamOracle:
             has[ok] = self.wsum[d][a[ok]] > 0
             nh = np.where(has, float(self.scaling[3][d]) * nh + float(self.scaling[2][d]), nh)
             cl = np.where(has, strain_all[np.clip(a, 0, self.T - 1)].astype(np.float64) - nh, cl)
+        return nh, cl
+
+    def _final_postfiltered(self, d: int, strain_all: np.ndarray, fin0: int, S: int):
+        """D11: this update's emitted block joins the stream of emitted estimate samples (unscaled, zeros before the
+        stream start); the stream is FIR-filtered causally (carried state = the earlier emitted samples), then rescaled
+        (A14) and subtracted.  Samples with negative absolute index give 0 (A12)."""
+        saved, self.scaling = self.scaling, None
+        raw, _ = self._cleaned(d, strain_all, fin0, fin0 + S)              # unscaled estimate of the emitted block
+        self.scaling = saved
+        nh = np.zeros(S); cl = np.zeros(S)
+        for i in range(S):
+            a = fin0 + i
+            if a < 0:
+                continue
+            self.emitted[d][a] = raw[i]
+        for i in range(S):
+            a = fin0 + i
+            if a < 0:
+                continue
+            acc = 0.0
+            for j, hj in enumerate(self.postfilter):
+                if a - j >= 0:
+                    acc += hj * self.emitted[d][a - j]
+            if self.scaling is not None:
+                acc = float(self.scaling[3][d]) * acc + float(self.scaling[2][d])
+            nh[i] = acc
+            cl[i] = float(strain_all[a]) - acc
         return nh, cl
 
     def skip(self, new: np.ndarray) -> None:
@@ -351,6 +401,8 @@ class StreamOracle:
                 acc, wsum = self.acc[d], self.wsum[d]
                 fin0 = a0
             nh, cl = self._cleaned(d, strain_all, fin0, fin0 + S)
+            if self.postfilter is not None:                                         # D11
+                nh, cl = self._final_postfiltered(d, strain_all, fin0, S)
             out["nhat_final"].append(nh); out["cleaned_final"].append(cl)
             nhr, clr = self._cleaned(d, strain_all, first, first + W)
             out["nhat_running"].append(nhr); out["cleaned_running"].append(clr)
@@ -360,6 +412,8 @@ class StreamOracle:
             xin = np.zeros((len(self.rows), Lb), dtype=np.float64)
             for d, (wit, srow) in enumerate(self.rows):
                 _, xin[d] = self._cleaned(d, np.ascontiguousarray(self.x[srow]), a1 - Lb, a1)
+            if self.whiten is not None:                                             # D12
+                xin = np.stack([fir_causal(xin[d], self.whiten[d]) for d in range(len(self.rows))])
             out["bbh_input"] = xin
             out["score"] = bbh_forward(xin, convs, pc, pd)
         return out

@@ -27,7 +27,7 @@ EXPORTS = [          # include/gwstream.h
     "gw_cleaned_strain", "gw_noise_estimate", "gw_deepclean_activation",
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
     "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_step_host_async", "gw_pipeline_graph_nodes",
-    "gw_deepclean_set_scaling", "gw_offline_set_scaling", "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
+    "gw_deepclean_set_scaling", "gw_offline_set_scaling", "gw_deepclean_set_postfilter", "gw_bbh_set_whitening", "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
 ]
 DIAG_EXPORTS = [     # include/gwstream_diag.h (measurement and diagnostics, not the product interface)
     "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes", "gw_probe_mma_cycles",
@@ -125,6 +125,8 @@ def lib():
         L.gw_step_host_async.argtypes = [vp, vp, vp, vp, vp]
         L.gw_deepclean_set_scaling.argtypes = [vp, vp, vp, vp, vp]
         L.gw_offline_set_scaling.argtypes = [vp, vp, vp, vp, vp]
+        L.gw_deepclean_set_postfilter.argtypes = [vp, vp, i]
+        L.gw_bbh_set_whitening.argtypes = [vp, vp, i]
         L.gw_offline_create.argtypes = [C.POINTER(vp), vp, i, i, i, i, i, i, C.POINTER(Options)]
         L.gw_offline_destroy.argtypes = [vp]
         L.gw_offline_samples.argtypes = [vp]
@@ -286,6 +288,14 @@ class DeepClean:
         None = identity.  Before the first update."""
         _check(lib().gw_deepclean_set_scaling(self.h, *_scaling_args(wit_mean, wit_std, strain_mean, strain_std)), self.h)
 
+    def set_postfilter(self, taps) -> None:
+        """D11: causal FIR over the stream of emitted (final) estimate samples; None switches it off.  Before the first update."""
+        if taps is None:
+            _check(lib().gw_deepclean_set_postfilter(self.h, None, 0), self.h)
+            return
+        t = np.ascontiguousarray(taps, dtype=np.float32).reshape(-1)
+        _check(lib().gw_deepclean_set_postfilter(self.h, C.c_void_p(t.ctypes.data), len(t)), self.h)
+
     def forward(self, stream=None) -> None:
         _check(lib().gw_deepclean_forward(self.h, _stream_ptr(stream)), self.h)
 
@@ -353,6 +363,15 @@ class Bbh:
         self.h = C.c_void_p()
         _check(lib().gw_bbh_create(C.byref(self.h), dc.h if dc is not None else None, C.byref(spec), dtype,
                                    n_det, max_batch, _opt_ptr(opts)))
+
+    def set_whitening(self, taps) -> None:
+        """D12: causal FIR whitening of each detector's classifier window, taps [n_det][n_taps]; None switches it off."""
+        if taps is None:
+            _check(lib().gw_bbh_set_whitening(self.h, None, 0), self.h)
+            return
+        t = np.ascontiguousarray(taps, dtype=np.float32)
+        assert t.ndim == 2 and t.shape[0] == self.n_det, t.shape
+        _check(lib().gw_bbh_set_whitening(self.h, C.c_void_p(t.ctypes.data), t.shape[1]), self.h)
 
     def score(self, stream=None):
         import torch

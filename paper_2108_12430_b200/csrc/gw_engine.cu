@@ -307,6 +307,9 @@ struct gw_deepclean {
     float* d_pre = nullptr;                      // [n_det][n_wit][2] witness standardisation (mean, 1/std); identity (0, 1)
     float* d_post = nullptr;                     // [n_det][2] estimate back to strain units (std, mean); identity (1, 0)
     float* final_buf = nullptr;                  // [batch][S]
+    float* d_fir = nullptr;                      // D11: post-filter taps [fir_n] (null: off)
+    float* d_hist = nullptr;                     // D11: [2][batch][kMaxFir - 1] emitted samples carried between updates
+    int fir_n = 0;
     float* clf_in = nullptr;                     // owned by the attached gw_bbh
     int Lb = 0;
     gw_bbh* bbh = nullptr;
@@ -328,6 +331,8 @@ struct gw_bbh {
     float *d_hw1 = nullptr, *d_hb1 = nullptr, *d_hw2 = nullptr, *d_hb2 = nullptr;
     float* pooled_dbg = nullptr;
     float* scores_buf = nullptr;
+    float* d_whiten = nullptr;                   // D12: whitening taps [n_det][whiten_n] (null: off)
+    int whiten_n = 0;
     int64_t scored_for = 0;
 };
 
@@ -646,12 +651,6 @@ static void run_gemm(const GemmLayer& gl, LaunchCtx& cx, bool inc = false, int b
     const double frac = rows >= g.p.M ? 1.0 : rows / g.p.M;
     g.p.stamp = cx.next(gl.name, gl.flops * g.batch * frac, gemm_smem_bytes(g, g.batch));
     cx.check(gl.impl == GW_IMPL_UMMA ? launch_conv_gemm_umma(g, cx.st) : launch_conv_gemm_simt(g, cx.st));
-    if (getenv("GW_DEBUG_SYNC")) {               // bring-up aid: name the launch that faults (never set in production)
-        const cudaError_t e = cudaStreamSynchronize(cx.st);
-        fprintf(stderr, "[gw debug] %s %s: v_tiles %d/%d left %d N %d M %d out_ring_div %d a_ring_div %d G %d resident %d sa %d -> %s\n",
-                gl.name.c_str(), inc ? "zones" : "full", g.p.v_tiles, g.p.tiles_m, g.p.v_left, g.p.N, g.p.M, g.p.out_ring_div,
-                g.p.a_ring_div, g.p.g_tiles, g.p.b_resident, g.p.sa_stages, cudaGetErrorString(e));
-    }
 }
 
 static void free_gemm(GemmLayer& gl) {
@@ -754,7 +753,7 @@ extern "C" int gw_deepclean_destroy(gw_deepclean* dc) {
     cudaFree(dc->d_wt_final); cudaFree(dc->d_b_final); cudaFree(dc->d_fin_B); cudaFree(dc->pred); cudaFree(dc->acc); cudaFree(dc->nhat);
     cudaFree(dc->d_hann); cudaFree(dc->d_inv_wsum); cudaFree(dc->d_rows_map); cudaFree(dc->d_strain_rows);
     cudaFree(dc->d_pre); cudaFree(dc->d_post);
-    cudaFree(dc->final_buf);
+    cudaFree(dc->final_buf); cudaFree(dc->d_fir); cudaFree(dc->d_hist);
     if (dc->s && dc->s->dc == dc) dc->s->dc = nullptr;
     dc->base.magic = 0;
     delete dc;
@@ -996,6 +995,33 @@ extern "C" int gw_deepclean_set_scaling(gw_deepclean* dc, const float* wit_mean,
     if (dc->s && dc->s->updates != 0)
         return fail(GW_ESTATE, "gw_deepclean_set_scaling: must be called before the first update (the state holds converted samples)");
     return set_scaling(dc, wit_mean, wit_std, strain_mean, strain_std);
+}
+
+// D11: causal FIR over the stream of emitted (final) estimate samples.
+extern "C" int gw_deepclean_set_postfilter(gw_deepclean* dc, const float* taps_host, int n_taps) {
+    if (!dc) return fail(GW_EINVAL, "gw_deepclean_set_postfilter: NULL handle");
+    CallScope scope(dc);
+    if (dc->offline) return fail(GW_EINVAL, "gw_deepclean_set_postfilter: streaming handles only");
+    if (dc->s && dc->s->updates != 0)
+        return fail(GW_ESTATE, "gw_deepclean_set_postfilter: must be called before the first update (the filter carries state)");
+    if (!taps_host || n_taps == 0) {             // off
+        cudaFree(dc->d_fir); cudaFree(dc->d_hist);
+        dc->d_fir = nullptr; dc->d_hist = nullptr; dc->fir_n = 0;
+        return GW_OK;
+    }
+    if (n_taps < 1 || n_taps > kMaxFir || n_taps - 1 > dc->s->S)
+        return fail(GW_EINVAL, "post-filter needs 1 <= n_taps <= %d and n_taps - 1 <= stride", kMaxFir);
+    for (int i = 0; i < n_taps; ++i)
+        if (!isfinite(taps_host[i])) return fail(GW_EINVAL, "post-filter taps must be finite");
+    cudaFree(dc->d_fir); cudaFree(dc->d_hist);
+    dc->d_fir = nullptr; dc->d_hist = nullptr;
+    const size_t hbytes = 2 * static_cast<size_t>(dc->batch) * (kMaxFir - 1) * sizeof(float);
+    CU_TRY(cudaMalloc(&dc->d_fir, n_taps * sizeof(float)));
+    CU_TRY(cudaMemcpy(dc->d_fir, taps_host, n_taps * sizeof(float), cudaMemcpyHostToDevice));
+    CU_TRY(cudaMalloc(&dc->d_hist, hbytes));
+    CU_TRY(cudaMemset(dc->d_hist, 0, hbytes));
+    dc->fir_n = n_taps;
+    return GW_OK;
 }
 
 extern "C" int gw_deepclean_create(gw_deepclean** out, gw_stream* s, const gw_dc_spec* spec, int dtype, const gw_options* opts) {
@@ -1241,6 +1267,7 @@ static AggParams make_agg(gw_deepclean* dc, float* final_out, float* running_out
     a.n_streams = s->n; a.n_det = dc->n_det; a.channels = s->C; a.W = s->W; a.S = s->S; a.Lb = dc->Lb;
     a.delta = dc->delta; a.agg = dc->agg;
     a.pred_ring = dc->inc ? 1 : 0;
+    a.fir = dc->d_fir; a.hist = dc->d_hist; a.fir_n = dc->fir_n;
     return a;
 }
 
@@ -1285,7 +1312,7 @@ extern "C" int gw_bbh_destroy(gw_bbh* b) {
     for (void* a : b->act) cudaFree(a);
     cudaFree(b->d_w1); cudaFree(b->d_b1); cudaFree(b->in_buf);
     cudaFree(b->d_hw1); cudaFree(b->d_hb1); cudaFree(b->d_hw2); cudaFree(b->d_hb2);
-    cudaFree(b->pooled_dbg); cudaFree(b->scores_buf);
+    cudaFree(b->pooled_dbg); cudaFree(b->scores_buf); cudaFree(b->d_whiten);
     if (b->dc && b->dc->bbh == b) { b->dc->bbh = nullptr; b->dc->clf_in = nullptr; b->dc->Lb = 0; }
     b->base.magic = 0;
     delete b;
@@ -1400,9 +1427,26 @@ extern "C" int gw_bbh_create(gw_bbh** out, gw_deepclean* dc, const gw_bbh_spec* 
     return GW_OK;
 }
 
+// D12: causal FIR whitening of every detector's classifier window, zero initial state.
+extern "C" int gw_bbh_set_whitening(gw_bbh* b, const float* taps_host, int n_taps) {
+    if (!b) return fail(GW_EINVAL, "gw_bbh_set_whitening: NULL handle");
+    CallScope scope(b);
+    cudaFree(b->d_whiten);
+    b->d_whiten = nullptr; b->whiten_n = 0;
+    if (!taps_host || n_taps == 0) return GW_OK;
+    if (n_taps < 1 || n_taps > kMaxFir) return fail(GW_EINVAL, "whitening needs 1 <= n_taps <= %d", kMaxFir);
+    const size_t n = static_cast<size_t>(b->n_det) * n_taps;
+    for (size_t i = 0; i < n; ++i)
+        if (!isfinite(taps_host[i])) return fail(GW_EINVAL, "whitening taps must be finite");
+    CU_TRY(cudaMalloc(&b->d_whiten, n * sizeof(float)));
+    CU_TRY(cudaMemcpy(b->d_whiten, taps_host, n * sizeof(float), cudaMemcpyHostToDevice));
+    b->whiten_n = n_taps;
+    return GW_OK;
+}
+
 static void bbh_enqueue(gw_bbh* b, const float* in, int batch, LaunchCtx& cx) {
     cx.check(launch_bbh_conv1(in, b->d_w1, b->d_b1, b->act[0], batch, b->n_det, b->L, b->c1.cout, b->c1_cpad, b->c1.k,
-                              b->c1.pad_l, b->c1.pool, b->fmt, cx.next("bbh_conv1"), cx.st));
+                              b->c1.pad_l, b->c1.pool, b->fmt, b->d_whiten, b->whiten_n, cx.next("bbh_conv1"), cx.st));
     for (auto& g : b->gemm) run_gemm(g, cx, false, batch);
 }
 

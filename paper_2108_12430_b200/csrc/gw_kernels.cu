@@ -537,6 +537,35 @@ cudaError_t launch_final_convt(const void* x, const float* wt, const float* bias
 // Samples with a < 0 (before the stream started) are written as 0 and never touch the state.
 // Algorithmic traffic: read p, acc, strain; write acc, cleaned  = 20 bytes per sample.
 // ---------------------------------------------------------------------------------------------
+// D11 helpers.  emitted_at: the unscaled estimate that window position n of batch item `wi / W` emits THIS update (n in
+// the final block): HANN -- the accumulator value before this update plus this window's term, normalised (the same
+// operations as the main path, so the same bits); LAST_STRIDE -- the prediction itself.  0 before the stream start.
+__device__ __forceinline__ float emitted_at(const AggParams& a, size_t wi, int n, int h, long long cnt) {
+    if (cnt - a.W + n < 0) return 0.f;
+    int slot = h + n;
+    if (slot >= a.W) slot -= a.W;
+    const float p = __ldg(a.pred + wi + (a.pred_ring ? slot : n));
+    if (a.agg != 0) return p;
+    return fmaf(__ldg(a.hann + n), p, a.acc[wi + slot]) * __ldg(a.inv_wsum + n);   // final block: never the newest stride
+}
+// Final (emitted) index i of batch item sd: FIR over the emitted stream, state carried in `hist`; writes the history
+// the next update needs.  Returns the filtered, unscaled estimate.
+__device__ __forceinline__ float postfiltered(const AggParams& a, int sd, size_t wi, int f0, int i, int h, long long cnt) {
+    const int HL = a.fir_n - 1;
+    const int parity = static_cast<int>((cnt / a.S) & 1);
+    const size_t hsz = static_cast<size_t>(a.n_streams) * a.n_det * (kMaxFir - 1);
+    const float* prev = a.hist + (parity ^ 1) * hsz + static_cast<size_t>(sd) * (kMaxFir - 1);
+    float* cur = a.hist + parity * hsz + static_cast<size_t>(sd) * (kMaxFir - 1);
+    float s = 0.f;
+    for (int j = 0; j < a.fir_n; ++j) {
+        const int i2 = i - j;
+        const float e = i2 >= 0 ? emitted_at(a, wi, f0 + i2, h, cnt) : prev[HL + i2];
+        s = fmaf(__ldg(a.fir + j), e, s);
+    }
+    if (i >= a.S - HL) cur[i - (a.S - HL)] = emitted_at(a, wi, f0 + i, h, cnt);
+    return s;
+}
+
 __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
     stamp_begin(a.stamp);
     const long long cnt = *a.count;
@@ -556,7 +585,9 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
             if (a.agg == 0) {
                 const float prev = (n >= W - S) ? 0.f : a.acc[wi + slot];
                 const float acc = fmaf(__ldg(a.hann + n), p, prev);
-                a.acc[wi + slot] = acc;
+                // D11: the final block's accumulators are read by neighbouring threads (emitted_at) and never needed
+                // again (their slots are reset when the ring reuses them): leave them as they were
+                if (!(a.fir && n < S)) a.acc[wi + slot] = acc;
                 nhat = acc * __ldg(a.inv_wsum + n);
             } else {
                 if (n >= W - a.delta) nhat = 0.f;
@@ -570,10 +601,21 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
         }
         if (a.running_out) a.running_out[wi + n] = cleaned;
         if (a.nhat_out) a.nhat_out[wi + n] = nhat;
-        if (a.final_out) {
+        {
             const int f0 = (a.agg == 0) ? 0 : W - S - a.delta;
             const int i = n - f0;
-            if (i >= 0 && i < S) a.final_out[static_cast<size_t>(sd) * S + i] = cleaned;
+            if (i >= 0 && i < S) {
+                float cf = cleaned;                            // the running / classifier outputs keep the unfiltered value
+                if (a.fir) {                                   // D11: band-limited estimate of the emitted stream
+                    const float e = postfiltered(a, sd, wi, f0, i, h, cnt);
+                    if (abs_idx >= 0) {
+                        const float nh = fmaf(__ldg(a.post + 2 * d), e, __ldg(a.post + 2 * d + 1));
+                        const float strain = __ldg(a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot);
+                        cf = strain - nh;
+                    }
+                }
+                if (a.final_out) a.final_out[static_cast<size_t>(sd) * S + i] = cf;
+            }
         }
         if (a.clf_in) {
             const int i = n - (W - a.delta - a.Lb);
@@ -610,7 +652,7 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
                 const float4 hw = __ldg(reinterpret_cast<const float4*>(a.hann + n));
                 const float4 iw = __ldg(reinterpret_cast<const float4*>(a.inv_wsum + n));
                 const float4 acc = make_float4(fmaf(hw.x, p.x, prev.x), fmaf(hw.y, p.y, prev.y), fmaf(hw.z, p.z, prev.z), fmaf(hw.w, p.w, prev.w));
-                *accp = acc;
+                if (!(a.fir && n < S)) *accp = acc;            // D11: see k_aggregate
                 nhat = make_float4(acc.x * iw.x, acc.y * iw.y, acc.z * iw.z, acc.w * iw.w);
             } else {
                 if (n >= W - a.delta) nhat = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -627,9 +669,25 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
         }
         if (a.running_out) *reinterpret_cast<float4*>(a.running_out + wi + n) = cleaned;
         if (a.nhat_out) *reinterpret_cast<float4*>(a.nhat_out + wi + n) = nhat;
-        if (a.final_out) {
-            const int i = n - ((a.agg == 0) ? 0 : W - S - a.delta);
-            if (i >= 0 && i < S) *reinterpret_cast<float4*>(a.final_out + static_cast<size_t>(sd) * S + i) = cleaned;
+        {
+            const int f0 = (a.agg == 0) ? 0 : W - S - a.delta;
+            const int i = n - f0;
+            if (i >= 0 && i < S) {
+                float4 cf = cleaned;
+                if (a.fir) {                                   // D11 (see k_aggregate)
+                    float e[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) e[q] = postfiltered(a, sd, wi, f0, i + q, h, cnt);
+                    if (abs_idx >= 0) {
+                        const float ps = __ldg(a.post + 2 * d), pm = __ldg(a.post + 2 * d + 1);
+                        const float4 st4 = __ldg(reinterpret_cast<const float4*>(
+                            a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot));
+                        cf = make_float4(st4.x - fmaf(ps, e[0], pm), st4.y - fmaf(ps, e[1], pm), st4.z - fmaf(ps, e[2], pm),
+                                         st4.w - fmaf(ps, e[3], pm));
+                    }
+                }
+                if (a.final_out) *reinterpret_cast<float4*>(a.final_out + static_cast<size_t>(sd) * S + i) = cf;
+            }
         }
         if (a.clf_in) {
             const int i = n - (W - a.delta - a.Lb);
@@ -724,10 +782,13 @@ template <int CIN>
 __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ x, const float* __restrict__ w,
                                                       const float* __restrict__ bias, void* __restrict__ out,
                                                       int L, int cout, int cpad, int K, int pad_l, int fmt,
+                                                      const float* __restrict__ whiten, int whiten_n,
                                                       unsigned long long* stamp) {
     constexpr int cin = CIN;
     stamp_begin(stamp);
     __shared__ __align__(16) float xs[kC1MaxCin][kC1Span];
+    __shared__ float xr[kC1MaxCin][kC1Span + kMaxFir];        // D12: raw samples of the tile + the filter's history
+    __shared__ float gs[kC1MaxCin][kMaxFir];                  // D12: whitening taps per input channel
     __shared__ __align__(16) float ws[32][kC1MaxCin][8];      // this block's 32 channels, zero where unused
     __shared__ float bs[32];
     const int b = blockIdx.y;
@@ -739,14 +800,34 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
         (&ws[0][0][0])[i] = (c < cout && ci < cin && j < K) ? __ldg(w + (static_cast<size_t>(c) * cin + ci) * K + j) : 0.f;
     }
     if (threadIdx.x < 32) bs[threadIdx.x] = cbase + threadIdx.x < cout ? __ldg(bias + cbase + threadIdx.x) : 0.f;
+    if (whiten)
+        for (int i = threadIdx.x; i < cin * whiten_n; i += blockDim.x) gs[i / whiten_n][i % whiten_n] = __ldg(whiten + i);
     const int pg = wrp & 1;                               // position group: pooled positions [32 pg, +32) of the tile
     const int cg = wrp >> 1;                              // channel group: channels [8 cg, +8) of the block's 32
     for (int q0 = blockIdx.x * kC1Q; q0 < Lq; q0 += gridDim.x * kC1Q) {
         const int l0 = q0 * 4 - pad_l;                    // first input position of the tile
-        __syncthreads();                                  // the previous tile has been consumed (and ws / bs are written)
-        for (int i = threadIdx.x; i < cin * kC1Span; i += blockDim.x) {
-            const int ci = i / kC1Span, l = l0 + i % kC1Span;
-            xs[ci][i % kC1Span] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+        __syncthreads();                                  // the previous tile has been consumed (and ws / bs / gs are written)
+        if (whiten) {
+            // D12: the block sees the WHITENED window y[l] = sum_j g[j] x[l - j] (x[l < 0] = 0: zero initial state at the
+            // window start); outside [0, L) it is the conv's zero padding as before
+            const int hl = whiten_n - 1, span = kC1Span + hl;
+            for (int i = threadIdx.x; i < cin * span; i += blockDim.x) {
+                const int ci = i / span, l = l0 - hl + i % span;
+                xr[ci][i % span] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+            }
+            __syncthreads();
+            for (int i = threadIdx.x; i < cin * kC1Span; i += blockDim.x) {
+                const int ci = i / kC1Span, q = i % kC1Span, l = l0 + q;
+                float v = 0.f;
+                if (l >= 0 && l < L)
+                    for (int j = 0; j < whiten_n; ++j) v = fmaf(gs[ci][j], xr[ci][q + hl - j], v);
+                xs[ci][q] = v;
+            }
+        } else {
+            for (int i = threadIdx.x; i < cin * kC1Span; i += blockDim.x) {
+                const int ci = i / kC1Span, l = l0 + i % kC1Span;
+                xs[ci][i % kC1Span] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+            }
         }
         __syncthreads();
         const int ql = pg * 32 + lane;                    // pooled position inside the tile
@@ -795,17 +876,18 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
 }
 
 cudaError_t launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
-                             int cout, int cpad, int K, int pad_l, int pool, int fmt, Stamp stamp, cudaStream_t st) {
+                             int cout, int cpad, int K, int pad_l, int pool, int fmt, const float* whiten, int whiten_n,
+                             Stamp stamp, cudaStream_t st) {
     (void)pool;                                        // validated == 4 at create time
     const int Lq = L / 4;
     int tiles = (Lq + kC1Q - 1) / kC1Q;
     if (static_cast<long long>(tiles) * batch >= 148 * 8) tiles = (tiles + 3) / 4;   // enough blocks: four tiles per block
     dim3 grid(tiles, batch, cpad / 32);
     switch (n_det) {                                   // cin = number of detectors (validated <= 4 at create time)
-        case 1: k_bbh_conv1<1><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
-        case 2: k_bbh_conv1<2><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
-        case 3: k_bbh_conv1<3><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
-        default: k_bbh_conv1<4><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, stamp); break;
+        case 1: k_bbh_conv1<1><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
+        case 2: k_bbh_conv1<2><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
+        case 3: k_bbh_conv1<3><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
+        default: k_bbh_conv1<4><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
     }
     count_launch();
     return cudaGetLastError();

@@ -251,6 +251,96 @@ def test_small_ensemble_latency_offset_through_the_graph():
     _run_streaming(cfg, gw.GW_FP16, cfg.n_updates, white=False, agg=S.AGG_LAST_STRIDE, delta=256, use_graph=True)
 
 
+# ------------------------------------------------ D11 / D12: band-limited emitted estimate, whitened classifier input
+@pytest.mark.parametrize("agg,delta,incremental", [(S.AGG_HANN_OLA, 0, False), (S.AGG_LAST_STRIDE, 256, False),
+                                                   (S.AGG_HANN_OLA, 0, True)])
+def test_postfilter_and_whitening_match_oracle(agg, delta, incremental):
+    """DESIGN.md D11: a causal FIR over the STREAM of emitted estimate samples, state carried from
+    update to update; D12: FIR whitening of the classifier window.  Final cleaned samples (through the
+    graph) and scores against the oracle; the identity filters are bit-exact no-ops; running values stay unfiltered."""
+    cfg = S.config_small_ensemble(2)
+    sp = cfg.stream
+    dc_params, bbh_params = util.make_params(cfg)
+    n_up = 14
+    rng = np.random.default_rng(77)
+    h = (0.3 * rng.standard_normal(17)).astype(np.float32)
+    g = (0.2 * rng.standard_normal((sp.n_det, 12))).astype(np.float32)
+    g[:, 0] += 1.0
+    x = synth.multi_stream(cfg.seed, sp, n_up * sp.stride)
+    xc = torch.from_numpy(np.ascontiguousarray(x.reshape(sp.n_streams, sp.channels, n_up, sp.stride).transpose(2, 0, 1, 3))).cuda()
+    dtype = gw.GW_FP16
+    outs = {}
+    for name, pf, wh in (("none", None, None), ("ident", np.ones(1, np.float32), np.ones((sp.n_det, 1), np.float32)), ("filt", h, g)):
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, agg, delta, gw.Options(incremental=incremental))
+        if pf is not None:
+            dc.set_postfilter(pf)
+            bbh.set_whitening(wh)
+        cs = torch.cuda.Stream()
+        sc = torch.zeros(sp.n_streams, device="cuda")
+        fin = torch.zeros((sp.n_streams, sp.n_det, sp.stride), device="cuda")
+        torch.cuda.synchronize()
+        res = []
+        for t in range(n_up):
+            pipe.step(xc[t], sc, fin, cs)
+            cs.synchronize()
+            res.append((fin.cpu().numpy().copy(), sc.cpu().numpy().copy()))
+        outs[name] = res
+        if name == "filt":
+            with pytest.raises(gw.GwError) as e:
+                dc.set_postfilter(h)                        # after the first update: the filter carries state
+            assert e.value.code == gw.GW_ESTATE
+    for t in range(n_up):
+        assert np.array_equal(outs["none"][t][0], outs["ident"][t][0]) and np.array_equal(outs["none"][t][1], outs["ident"][t][1]), t
+    oracles = [util.make_stream_oracle(cfg, dc_params, bbh_params, dtype, n_up, agg, delta) for _ in range(sp.n_streams)]
+    for o in oracles:
+        o.postfilter = np.asarray(h, np.float64)
+        o.whiten = np.asarray(g, np.float64)
+    worst = 0.0
+    differs = False
+    for t in range(n_up):
+        fin_t, sc_t = outs["filt"][t]
+        differs = differs or not np.array_equal(fin_t, outs["none"][t][0])
+        for i, orc in enumerate(oracles):
+            ref = orc.update(x[i][:, t * sp.stride:(t + 1) * sp.stride])
+            for d in range(sp.n_det):
+                _, w = util.check_network_output(fin_t[i, d], ref["cleaned_final"][d], f"post-filtered final update {t} stream {i} det {d}",
+                                                 rms_ref=ref["pred"][d])
+                worst = max(worst, w)
+            assert abs(float(sc_t[i]) - ref["score"]) <= util.SCORE_ABS, (t, i, float(sc_t[i]), ref["score"])
+            assert abs(util.logit(sc_t[i]) - util.logit(ref["score"])) <= util.LOGIT_ABS, (t, i, float(sc_t[i]), ref["score"])
+    assert differs, "the filters must change something"
+    print(f"D11/D12 agg={agg} delta={delta} incremental={incremental}: worst |d final|/RMS(pred) {worst:.3e}")
+
+
+def test_whitened_batch_classifier_and_filter_argument_checks():
+    cfg = S.config_c2()
+    L, batch = 1024, 6
+    cp, dp = util.centred_bbh_params(202, cfg.bbh_convs, cfg.bbh_dense, L)
+    bbh = gw.Bbh(None, cfg.bbh_convs, cp, dp, L, gw.GW_BF16, n_det=2, max_batch=8)
+    x = synth.bbh_windows(2, batch, L)
+    g = np.array([[1.0, -0.6, 0.25, 0.0, 0.1], [0.9, 0.3, -0.2, 0.05, 0.0]], np.float32)
+    bbh.set_whitening(g)
+    got = bbh.score_batch(_dev(x)).cpu().numpy()
+    pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    ref = np.array([oracle.bbh_forward(np.stack([oracle.fir_causal(x[i][d], g[d]) for d in range(2)]), cfg.bbh_convs, pc, pd)
+                    for i in range(batch)])
+    assert np.max(np.abs(got - ref)) <= util.SCORE_ABS, (got, ref)
+    assert np.max(np.abs(util.logit(got) - util.logit(ref))) <= util.LOGIT_ABS, (got, ref)
+    bbh.set_whitening(None)
+    plain = bbh.score_batch(_dev(x)).cpu().numpy()
+    assert not np.array_equal(plain, got)
+    with pytest.raises(gw.GwError):
+        bbh.set_whitening(np.ones((2, 65), np.float32))      # more than 64 taps
+    c0 = S.config_c0()
+    st = gw.Stream(c0.stream)
+    dc = gw.DeepClean(st, c0.dc_layers, util.make_params(c0)[0], gw.GW_FP16)
+    with pytest.raises(gw.GwError):
+        dc.set_postfilter(np.ones(66, np.float32))           # n_taps - 1 > stride (64) and > 64 taps
+    with pytest.raises(gw.GwError):
+        dc.set_postfilter(np.array([1.0, np.nan], np.float32))
+
+
 # ------------------------------------------------ D13 incremental path (gw_options.incremental)
 @pytest.mark.parametrize("W,S_,n,dtype", [(2048, 256, 3, gw.GW_FP16), (8192, 512, 2, gw.GW_BF16), (32768, 512, 2, gw.GW_FP16),
                                           (4096, 16, 1, gw.GW_FP16)])

@@ -513,6 +513,79 @@ def test_classifier_window_with_latency_offset_is_the_delayed_strain_slice(agg, 
     assert seen_real, "the test must reach windows that lie entirely inside the stream"
 
 
+# ------------------------------------------------ D11 / D12: band-limiting of the emitted estimate, whitening
+def test_fir_causal_impulse_identity_linearity_and_library_routine():
+    """fir_causal is y[i] = sum_j h[j] x[i-j] with zero initial state: an impulse reproduces the taps (unreversed, from
+    the impulse position on), the identity filter is a bit-exact no-op, the map is linear, and it agrees with
+    scipy.signal.lfilter(h, [1], x) (a library routine, not a retyped formula)."""
+    from scipy.signal import lfilter
+    h = RNG.standard_normal(9)
+    x = np.zeros(40); x[5] = 1.0
+    y = oracle.fir_causal(x, h)
+    assert np.array_equal(y[5:14], h) and np.all(y[:5] == 0) and np.all(y[14:] == 0)
+    z = RNG.standard_normal((3, 50))
+    assert np.array_equal(oracle.fir_causal(z, [1.0]), z)
+    assert np.array_equal(oracle.fir_causal(z, [0.0, 1.0])[:, 1:], z[:, :-1])        # a pure delay: the sign of the lag
+    z2 = RNG.standard_normal((3, 50))
+    assert np.allclose(oracle.fir_causal(2 * z - z2, h), 2 * oracle.fir_causal(z, h) - oracle.fir_causal(z2, h), atol=1e-13)
+    assert np.allclose(oracle.fir_causal(z, h), lfilter(h, [1.0], z, axis=-1), atol=1e-13)
+
+
+@pytest.mark.parametrize("agg", [oracle.AGG_HANN_OLA, oracle.AGG_LAST_STRIDE])
+def test_postfilter_acts_on_the_stream_of_emitted_samples_and_whitening_on_the_classifier_window(monkeypatch, agg):
+    """D11: with scripted predictions the emitted (final) estimate stream is known in closed form; the final cleaned
+    samples must be strain - lfilter(h, 1, emitted stream) evaluated over the WHOLE stream (state carried across
+    updates, zeros before the first emitted sample), the identity filter must change nothing bitwise, and running
+    values stay unfiltered.  D12: the classifier input is lfilter(g_d, 1, unwhitened window) per detector."""
+    from scipy.signal import lfilter
+    cfg = S.config_small_ensemble(1)
+    st = cfg.stream
+    W, S_, Lb = st.window, st.stride, cfg.bbh_len
+    n_up = 14
+    g_true = RNG.standard_normal(n_up * S_ + W)                    # the "true" noise over absolute index a + W
+    rows = [(st.witness_rows(d), st.strain_row(d)) for d in range(2)]
+    cp, dp = synth.bbh_params(1, cfg.bbh_convs, cfg.bbh_dense)
+    pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
+    pd = [oracle.prepare_dense(p) for p in dp]
+    h = RNG.standard_normal(17) * 0.3
+    gw_taps = RNG.standard_normal((2, 12)) * 0.3
+    x = synth.white_channels(4, st.channels, n_up * S_)
+    state = {"t": -1}
+
+    def fake(xin, layers, prepared):                                # consistent predictions: p_t[n] = g[a0_t + n]
+        t = state["t"]
+        a0 = (t + 1) * S_ - W
+        return g_true[a0 + W:a0 + 2 * W].copy()
+
+    monkeypatch.setattr(oracle, "deepclean_forward", fake)
+    outs = {}
+    for name, pf, wh in (("plain", None, None), ("ident", [1.0], np.array([[1.0], [1.0]])), ("filt", h, gw_taps)):
+        so = oracle.StreamOracle(st.channels, W, S_, rows, [(cfg.dc_layers, None)] * 2, (cfg.bbh_convs, pc, pd, Lb),
+                                 agg=agg, max_updates=n_up, postfilter=pf, whiten=wh)
+        res = []
+        for t in range(n_up):
+            state["t"] = t
+            res.append(so.update(x[:, t * S_:(t + 1) * S_]))
+        outs[name] = res
+    k = W // S_
+    for t in range(n_up):
+        a, b, c = outs["plain"][t], outs["ident"][t], outs["filt"][t]
+        for d in range(2):
+            assert np.array_equal(a["cleaned_final"][d], b["cleaned_final"][d])      # identity filter: bit-exact no-op
+            assert np.array_equal(a["cleaned_running"][d], c["cleaned_running"][d])  # running values are not filtered
+        assert np.array_equal(a["bbh_input"], b["bbh_input"])
+        assert np.allclose(c["bbh_input"], np.stack([lfilter(gw_taps[d], [1.0], a["bbh_input"][d]) for d in range(2)]), atol=1e-12)
+        # emitted stream in closed form: consistent predictions => the emitted estimate at absolute a >= 0 is g[a]
+        fin0 = (t + 1) * S_ - W if agg == oracle.AGG_HANN_OLA else t * S_
+        if fin0 >= 0:
+            emitted = g_true[W:W + fin0 + S_].copy()               # g at absolute 0 .. fin0 + S - 1
+            filt = lfilter(h, [1.0], emitted)[fin0:fin0 + S_]
+            for d in range(2):
+                strain = x[st.strain_row(d), fin0:fin0 + S_].astype(np.float64)
+                assert np.allclose(c["cleaned_final"][d], strain - filt, atol=1e-9), (t, d)
+                assert np.allclose(c["nhat_final"][d], filt, atol=1e-9)
+
+
 # ------------------------------------------------ D13 incremental path: which rows change between updates
 @pytest.mark.parametrize("W,S_", [(1024, 64), (2048, 256), (512, 16)])
 def test_incremental_zones_are_exactly_the_rows_that_change_between_overlapping_windows(W, S_):
