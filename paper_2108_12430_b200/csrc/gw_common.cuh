@@ -180,10 +180,10 @@ struct AggParams {
     int fir_n;
 };
 constexpr int kMaxFir = 64;        // taps of the post-filter (D11) and of the whitening filter (D12)
-cudaError_t launch_aggregate(const AggParams& a, cudaStream_t st);
+cudaError_t launch_aggregate(const AggParams& a, int pdl, cudaStream_t st);
 cudaError_t launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
                              int cout, int cpad, int K, int pad_l, int pool, int fmt, const float* whiten, int whiten_n,
-                             Stamp stamp, cudaStream_t st);
+                             int pdl, Stamp stamp, cudaStream_t st);
 
 cudaError_t launch_stamp_init(unsigned long long* stamps, int n, cudaStream_t st);   // begin slots = max, end slots = 0
 void count_launch();               // one more kernel launched (or captured) by this library: atomic process-wide counter

@@ -1274,7 +1274,7 @@ static AggParams make_agg(gw_deepclean* dc, float* final_out, float* running_out
 static AggParams cleaned_enqueue(gw_deepclean* dc, float* final_out, float* running_out, float* nhat_out, LaunchCtx& cx) {
     AggParams a = make_agg(dc, final_out, running_out, nhat_out);
     a.stamp = cx.next("aggregate");
-    cx.check(launch_aggregate(a, cx.st));
+    cx.check(launch_aggregate(a, dc->opt.pdl, cx.st));
     return a;
 }
 
@@ -1446,7 +1446,7 @@ extern "C" int gw_bbh_set_whitening(gw_bbh* b, const float* taps_host, int n_tap
 
 static void bbh_enqueue(gw_bbh* b, const float* in, int batch, LaunchCtx& cx) {
     cx.check(launch_bbh_conv1(in, b->d_w1, b->d_b1, b->act[0], batch, b->n_det, b->L, b->c1.cout, b->c1_cpad, b->c1.k,
-                              b->c1.pad_l, b->c1.pool, b->fmt, b->d_whiten, b->whiten_n, cx.next("bbh_conv1"), cx.st));
+                              b->c1.pad_l, b->c1.pool, b->fmt, b->d_whiten, b->whiten_n, b->opt.pdl, cx.next("bbh_conv1"), cx.st));
     for (auto& g : b->gemm) run_gemm(g, cx, false, batch);
 }
 

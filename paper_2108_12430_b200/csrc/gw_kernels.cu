@@ -8,8 +8,27 @@
 #include <atomic>
 
 #include "gw_common.cuh"
+#include "gw_ptx.cuh"
 
 namespace gw {
+
+// Programmatic dependent launch (gw_options.pdl): the kernels below trigger their dependents at once (the next kernel's
+// prologue -- barrier init, TMEM allocation, weight loads -- then overlaps this kernel) and, where they are launched as
+// dependents themselves, wait with griddepcontrol.wait before touching anything their predecessor wrote.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, int pdl, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
 
 static std::atomic<long long> g_kernel_launches{0};
 void count_launch() { g_kernel_launches.fetch_add(1, std::memory_order_relaxed); }
@@ -63,6 +82,7 @@ __global__ void __launch_bounds__(256) k_append(float* __restrict__ ring, const 
                                                 long long* count, unsigned* ticket, int n_rows, int W, int S,
                                                 unsigned long long* stamp) {
     stamp_begin(stamp);
+    griddep_launch_dependents();
     const long long cnt = *count;
     const int h = static_cast<int>(cnt % W);
     const int per_row = S / VEC;
@@ -152,6 +172,7 @@ __global__ void __launch_bounds__(256) k_gather(const float* __restrict__ ring, 
                                                 unsigned long long* stamp) {
     __shared__ float tile[32][kGatherPos + 1];
     stamp_begin(stamp);
+    griddep_launch_dependents();
     const int h = seg_T > 0 ? 0 : static_cast<int>(*count % W);
     const int sd = blockIdx.y;                       // stream * n_det + det
     const int s = sd / n_det, d = sd % n_det;
@@ -223,6 +244,7 @@ __global__ void __launch_bounds__(256) k_ring16_append(const float* __restrict__
                                                        int fmt, const float* __restrict__ pre, unsigned long long* stamp) {
     __shared__ float tile[32][kGatherPos + 1];
     stamp_begin(stamp);
+    griddep_launch_dependents();
     const int h0 = static_cast<int>((*count - S) % W);   // ring slot of this update's first sample
     const int sd = blockIdx.y;
     const int s = sd / n_det, d = sd % n_det;
@@ -283,6 +305,7 @@ __global__ void __launch_bounds__(256) k_snapshot_append(float* __restrict__ rin
                                                          int fmt, unsigned long long* stamp) {
     __shared__ float tile[32][kGatherPos + 1];
     stamp_begin(stamp);
+    griddep_launch_dependents();
     const long long cnt = *count;
     const int h0 = static_cast<int>(cnt % W);              // ring slot of this update's first sample
     const int sd = blockIdx.y;
@@ -566,6 +589,9 @@ __device__ __forceinline__ float postfiltered(const AggParams& a, int sd, size_t
     return s;
 }
 
+// FIR: the D11 post-filter path is compiled into its own instantiation, so that the default kernel keeps its 32
+// registers per thread (8 CTAs per SM; with the filter code inline it took 48 and lost 6 us at n = 128).
+template <bool FIR>
 __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
     stamp_begin(a.stamp);
     const long long cnt = *a.count;
@@ -587,7 +613,7 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
                 const float acc = fmaf(__ldg(a.hann + n), p, prev);
                 // D11: the final block's accumulators are read by neighbouring threads (emitted_at) and never needed
                 // again (their slots are reset when the ring reuses them): leave them as they were
-                if (!(a.fir && n < S)) a.acc[wi + slot] = acc;
+                if (!(FIR && n < S)) a.acc[wi + slot] = acc;
                 nhat = acc * __ldg(a.inv_wsum + n);
             } else {
                 if (n >= W - a.delta) nhat = 0.f;
@@ -606,7 +632,7 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
             const int i = n - f0;
             if (i >= 0 && i < S) {
                 float cf = cleaned;                            // the running / classifier outputs keep the unfiltered value
-                if (a.fir) {                                   // D11: band-limited estimate of the emitted stream
+                if (FIR) {                                     // D11: band-limited estimate of the emitted stream
                     const float e = postfiltered(a, sd, wi, f0, i, h, cnt);
                     if (abs_idx >= 0) {
                         const float nh = fmaf(__ldg(a.post + 2 * d), e, __ldg(a.post + 2 * d + 1));
@@ -630,8 +656,12 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
 // of 4: the ring head (count mod W, count a multiple of S) and every region boundary then fall on a group of
 // four, so a group never straddles the wrap, the newest stride, the final block or the classifier window.
 // (The scalar kernel spent its time on per-sample index arithmetic: ncu SM throughput 72 %, 1.9 TB/s.)
+template <bool FIR>
 __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
     stamp_begin(a.stamp);
+    // An ordinary launch, neither a programmatic dependent nor a trigger (both measured, n = 128): as a dependent its
+    // 8192 short CTAs each pay griddepcontrol.wait (+14 us); triggering the first classifier block early lets that
+    // kernel's CTAs take thread slots from this bandwidth kernel's last waves (+6 us) to save 1 us downstream.
     const long long cnt = *a.count;
     const int W = a.W, S = a.S;
     const int h = static_cast<int>(cnt % W);
@@ -652,7 +682,7 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
                 const float4 hw = __ldg(reinterpret_cast<const float4*>(a.hann + n));
                 const float4 iw = __ldg(reinterpret_cast<const float4*>(a.inv_wsum + n));
                 const float4 acc = make_float4(fmaf(hw.x, p.x, prev.x), fmaf(hw.y, p.y, prev.y), fmaf(hw.z, p.z, prev.z), fmaf(hw.w, p.w, prev.w));
-                if (!(a.fir && n < S)) *accp = acc;            // D11: see k_aggregate
+                if (!(FIR && n < S)) *accp = acc;              // D11: see k_aggregate
                 nhat = make_float4(acc.x * iw.x, acc.y * iw.y, acc.z * iw.z, acc.w * iw.w);
             } else {
                 if (n >= W - a.delta) nhat = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -674,7 +704,7 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
             const int i = n - f0;
             if (i >= 0 && i < S) {
                 float4 cf = cleaned;
-                if (a.fir) {                                   // D11 (see k_aggregate)
+                if (FIR) {                                     // D11 (see k_aggregate)
                     float e[4];
 #pragma unroll
                     for (int q = 0; q < 4; ++q) e[q] = postfiltered(a, sd, wi, f0, i + q, h, cnt);
@@ -741,23 +771,25 @@ cudaError_t launch_ola_offline(const float* pred, const float* seg, const int* s
 }
 
 bool is_aggregate_kernel(const void* func) {
-    return func == reinterpret_cast<const void*>(&k_aggregate) || func == reinterpret_cast<const void*>(&k_aggregate_v4);
+    return func == reinterpret_cast<const void*>(&k_aggregate<false>) || func == reinterpret_cast<const void*>(&k_aggregate<true>) ||
+           func == reinterpret_cast<const void*>(&k_aggregate_v4<false>) || func == reinterpret_cast<const void*>(&k_aggregate_v4<true>);
 }
 
-cudaError_t launch_aggregate(const AggParams& a, cudaStream_t st) {
+cudaError_t launch_aggregate(const AggParams& a, int /*pdl*/, cudaStream_t st) {
     auto al16 = [](const void* q) { return (reinterpret_cast<uintptr_t>(q) & 15) == 0; };   // null counts as aligned
     const bool vec = a.W % 4 == 0 && a.S % 4 == 0 && a.delta % 4 == 0 && (a.clf_in == nullptr || a.Lb % 4 == 0) &&
                      al16(a.pred) && al16(a.acc) && al16(a.ring) && al16(a.hann) && al16(a.inv_wsum) && al16(a.final_out) &&
                      al16(a.running_out) && al16(a.nhat_out) && al16(a.clf_in);
+    cudaError_t e;
     if (vec) {
         dim3 grid((a.W / 4 + 255) / 256, a.n_streams * a.n_det);
-        k_aggregate_v4<<<grid, 256, 0, st>>>(a);
+        e = a.fir ? launch_pdl(k_aggregate_v4<true>, grid, dim3(256), 0, st, a) : launch_pdl(k_aggregate_v4<false>, grid, dim3(256), 0, st, a);
     } else {
         dim3 grid((a.W + 255) / 256, a.n_streams * a.n_det);
-        k_aggregate<<<grid, 256, 0, st>>>(a);
+        e = a.fir ? launch_pdl(k_aggregate<true>, grid, dim3(256), 0, st, a) : launch_pdl(k_aggregate<false>, grid, dim3(256), 0, st, a);
     }
     count_launch();
-    return cudaGetLastError();
+    return e;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -802,6 +834,8 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
     if (threadIdx.x < 32) bs[threadIdx.x] = cbase + threadIdx.x < cout ? __ldg(bias + cbase + threadIdx.x) : 0.f;
     if (whiten)
         for (int i = threadIdx.x; i < cin * whiten_n; i += blockDim.x) gs[i / whiten_n][i % whiten_n] = __ldg(whiten + i);
+    griddep_wait();                                       // the weights above are constants; x is the predecessor's output
+    griddep_launch_dependents();
     const int pg = wrp & 1;                               // position group: pooled positions [32 pg, +32) of the tile
     const int cg = wrp >> 1;                              // channel group: channels [8 cg, +8) of the block's 32
     for (int q0 = blockIdx.x * kC1Q; q0 < Lq; q0 += gridDim.x * kC1Q) {
@@ -877,20 +911,21 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
 
 cudaError_t launch_bbh_conv1(const float* x, const float* w, const float* b, void* out, int batch, int n_det, int L,
                              int cout, int cpad, int K, int pad_l, int pool, int fmt, const float* whiten, int whiten_n,
-                             Stamp stamp, cudaStream_t st) {
+                             int pdl, Stamp stamp, cudaStream_t st) {
     (void)pool;                                        // validated == 4 at create time
     const int Lq = L / 4;
     int tiles = (Lq + kC1Q - 1) / kC1Q;
     if (static_cast<long long>(tiles) * batch >= 148 * 8) tiles = (tiles + 3) / 4;   // enough blocks: four tiles per block
     dim3 grid(tiles, batch, cpad / 32);
+    cudaError_t e;
     switch (n_det) {                                   // cin = number of detectors (validated <= 4 at create time)
-        case 1: k_bbh_conv1<1><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
-        case 2: k_bbh_conv1<2><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
-        case 3: k_bbh_conv1<3><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
-        default: k_bbh_conv1<4><<<grid, 256, 0, st>>>(x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
+        case 1: e = launch_pdl(k_bbh_conv1<1>, grid, dim3(256), pdl, st, x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
+        case 2: e = launch_pdl(k_bbh_conv1<2>, grid, dim3(256), pdl, st, x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
+        case 3: e = launch_pdl(k_bbh_conv1<3>, grid, dim3(256), pdl, st, x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
+        default: e = launch_pdl(k_bbh_conv1<4>, grid, dim3(256), pdl, st, x, w, b, out, L, cout, cpad, K, pad_l, fmt, whiten, whiten_n, stamp); break;
     }
     count_launch();
-    return cudaGetLastError();
+    return e;
 }
 
 }  // namespace gw
