@@ -633,10 +633,13 @@ def run_sweep(args):
                 with open(args.sweep, "a") as f:
                     f.write(line + "\n")
                 d = json.loads(line)
+                inc = d.get("incremental") or {}
                 rows.append((dtype, n, stride, d["value"], d["ms_per_step"], d["latency"]["p50_ms"], d["latency"]["p99_ms"],
-                             d["latency"]["realtime_budget_ms"], d["roofline"]["frac"], d["e2e"]["value"]))
-                log("%-5s n=%4d S=%5d  %9.1f data-s/s  %7.3f ms/step  p50 %7.3f  p99 %7.3f (budget %6.1f ms)  tensor %.3f  e2e %9.1f"
-                    % rows[-1])
+                             d["latency"]["realtime_budget_ms"], d["roofline"]["frac_sustained"], d["roofline"]["frac_nominal"],
+                             d["e2e"]["value"], inc.get("value", float("nan")), inc.get("ms_per_step", float("nan")),
+                             (inc.get("latency") or {}).get("p50_ms", float("nan")), (inc.get("latency") or {}).get("p99_ms", float("nan"))))
+                log("%-5s n=%4d S=%5d  full: %9.1f data-s/s  %7.3f ms/step  p50 %7.3f  p99 %7.3f (budget %6.1f ms)  tensor %.3f of sustained %.3f of nominal  "
+                    "e2e %9.1f | incremental: %9.1f data-s/s  %7.3f ms/step  p50 %7.3f  p99 %7.3f" % rows[-1])
 
 
 def main():

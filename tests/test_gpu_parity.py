@@ -343,7 +343,7 @@ def test_whitened_batch_classifier_and_filter_argument_checks():
 
 # ------------------------------------------------ D13 incremental path (gw_options.incremental)
 @pytest.mark.parametrize("W,S_,n,dtype", [(2048, 256, 3, gw.GW_FP16), (8192, 512, 2, gw.GW_BF16), (32768, 512, 2, gw.GW_FP16),
-                                          (4096, 16, 1, gw.GW_FP16)])
+                                          (4096, 16, 1, gw.GW_FP16), (32768, 1024, 1, gw.GW_BF16), (32768, 256, 1, gw.GW_FP16)])
 def test_incremental_path_is_bit_identical_to_full_recompute(W, S_, n, dtype):
     """DESIGN.md D13: with gw_options.incremental every layer's activations live in rings
     over absolute position and an update recomputes only the rows near the two window edges (tests/test_oracle_pins.py
