@@ -552,38 +552,37 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 // instruction: measured 65 % L1TEX utilisation and ~60 % of HBM rate on the thin layers).
                 // Rows past M are clipped by the tensor map.
                 const bool wide = p.N >= 64;
-                // All four 32-column chunks of this warp are pulled out of TMEM at once (128 registers) and the stage is
-                // handed back BEFORE any of the arithmetic: the MMA warps get their accumulator stage a whole epilogue
-                // earlier (they waited for it 15-26 % of their time in e2, e3, d2), and the warp pays one TMEM load
-                // latency per stage instead of two.  The bias is read from shared memory where it is used (caching it in
-                // registers would not leave room for the four chunks).
-                uint32_t r0a[32], r0b[32], r1a[32], r1b[32];
-                tmem_ld_32x32(taddr + 32 * (2 * hsel), r0a);
-                tmem_ld_32x32(taddr + 32 * (2 * hsel + 1), r0b);
-                tmem_ld_32x32(taddr + 32 * (4 + 2 * hsel), r1a);
-                tmem_ld_32x32(taddr + 32 * (4 + 2 * hsel + 1), r1b);
-                tmem_ld_wait();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&tmem_empty[acc]);
-#pragma unroll
                 for (int cp = 0; cp < 2; ++cp) {
+                    const int ca = 4 * cp + 2 * hsel, cbk = ca + 1;              // chunk indices
+                    uint32_t ra[32], rb[32];
+                    tmem_ld_32x32(taddr + 32 * ca, ra);
+                    tmem_ld_32x32(taddr + 32 * cbk, rb);
+                    float4 bia[2][8];                          // bias of both chunks, fetched under the TMEM latency
+#pragma unroll
+                    for (int which = 0; which < 2; ++which)
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) bia[which][j] = lds_f4(bias_u32 + 4u * (ch_col[2 * cp + which] + 4 * j));
                     const uint32_t stg = stage_u32 + ((ostep % p.out_bufs) << 15);
                     if (lane == 0) {                           // the store that last read this buffer has drained it
                         TR_WAIT(1, if (p.out_bufs == 2) tma_store_wait_read<1>(); else tma_store_wait_read<0>())
                     }
                     ++ostep;
+                    tmem_ld_wait();
+                    if (cp == 1) {                             // last reads of this stage: hand it back
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(&tmem_empty[acc]);
+                    }
                     __syncwarp();
 #pragma unroll
                     for (int which = 0; which < 2; ++which) {
-                        const uint32_t* r = cp == 0 ? (which == 0 ? r0a : r0b) : (which == 0 ? r1a : r1b);
-                        const uint32_t bias_c = bias_u32 + 4u * ch_col[2 * cp + which];
+                        const uint32_t* r = which == 0 ? ra : rb;
 #pragma unroll
                         for (int jj = 0; jj < 4; ++jj) {       // 16-byte units of this chunk's 64-byte row
                             uint32_t o[4];
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
-                                const float4 b4 = lds_f4(bias_c + 4u * (8 * jj + 4 * h));
+                                const float4 b4 = bia[which][2 * jj + h];
                                 o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
                                 o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
                             }
