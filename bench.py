@@ -296,7 +296,8 @@ class Engine:
                 continue
             prev_end = 0.0
             for r in rows:
-                a = acc.setdefault(r["label"], {"us": 0.0, "excl_us": 0.0, "flops": 0.0, "smem_bytes": 0.0})
+                a = acc.setdefault(r["label"], {"us": 0.0, "excl_us": 0.0, "flops": 0.0, "smem_bytes": 0.0, "sm_mhz": 0.0})
+                a["sm_mhz"] += r.get("sm_mhz", 0.0) / reps
                 if r["label"] not in order:
                     order.append(r["label"])
                 a["us"] += (r["end_us"] - r["begin_us"]) / reps
@@ -330,14 +331,18 @@ def kernel_table(eng, order, acc, pk, sm_mhz, sms):
     out = {}
     for k in order:
         a = acc[k]
-        row = {"us": round(a["us"], 2), "excl_us": round(a["excl_us"], 2)}
+        row = {"us": round(a["us"], 2), "excl_us": round(a["excl_us"], 2), "sm_mhz": round(a["sm_mhz"])}
         t = a["excl_us"] * 1e-6
+        mhz = a["sm_mhz"] or sm_mhz                    # the clock THIS kernel ran at (clock64 / %globaltimer of its CTA 0)
         if a["flops"] and t > 0:
             row["tflops"] = round(a["flops"] / t / 1e12, 1)
             row["tflops_own_span"] = round(a["flops"] / (a["us"] * 1e-6) / 1e12, 1)
+            # against what the tensor cores can do AT THAT CLOCK: 8192 dense 16-bit FLOP per clock per SM (2.25 PFLOP/s
+            # nominal = 148 SMs x 8192 x 1.855 GHz)
+            row["frac_of_tensor_peak_at_clock"] = round(a["flops"] / t / (sms * 8192.0 * mhz * 1e6), 3)
         if a["smem_bytes"] and a["us"] > 0:
             gbs = a["smem_bytes"] / (a["us"] * 1e-6) / 1e9
-            row.update({"smem_gbs": round(gbs, 1), "smem_frac": round(gbs / smem_peak_gbs, 3)})
+            row.update({"smem_gbs": round(gbs, 1), "smem_frac": round(gbs / (sms * 128 * mhz * 1e6 / 1e9), 3)})
         if k in hbm_bytes and a["us"] > 0:
             gbs = hbm_bytes[k] / (a["us"] * 1e-6) / 1e9
             row.update({"gbs": round(gbs, 1), "hbm_frac": round(gbs / pk["hbm_gbs"], 3),

@@ -19,13 +19,16 @@ extern "C" {
  *  the start of the step's first kernel.  Kernels overlap under PDL (a successor's prologue runs under its
  *  predecessor's tail), so the decomposition of the step is excl_i = end_i - max(begin_i, end_{i-1}); their sum is
  *  the span of the step on the device and cannot exceed the step time measured around the graph launch.
+ *  sm_mhz[i] (host, may be NULL): the SM clock kernel i actually ran at = the kernel's length in SM cycles (clock64 of its
+ *  CTA 0) over its length in ns (%globaltimer of the same CTA).  nvidia-smi samples every 25 ms at best; a kernel lasts
+ *  0.01-0.2 ms and the power cap moves the clock from one kernel to the next.
  *  gw_profile_label(p, i): kernel i's name ("snapshot_append", "gemm.dc0", ... "aggregate", "bbh_conv1", "gemm.bbh1", ...).
  *  gw_profile_flops(p, i): algorithmic FLOPs kernel i EXECUTED in that step (real channels and taps only, whole
  *  batch; with gw_options.incremental: the rows of the tiles that were recomputed); 0 for non-GEMM kernels.
  *  gw_profile_smem_bytes(p, i): shared-memory traffic of conv GEMM kernel i by the accounting of DESIGN.md section 7
  *  (MMA operand reads + TMA fills + epilogue staging, all SMs); 0 for other kernels. */
 int gw_step_profile(gw_pipeline *p, const float *new_samples_dev, float *scores_dev, float *cleaned_final_dev,
-                    void *stream, int max_kernels, double *begin_us, double *end_us, int *n_out);
+                    void *stream, int max_kernels, double *begin_us, double *end_us, double *sm_mhz, int *n_out);
 const char *gw_profile_label(const gw_pipeline *p, int i);
 double gw_profile_flops(const gw_pipeline *p, int i);
 double gw_profile_smem_bytes(const gw_pipeline *p, int i);

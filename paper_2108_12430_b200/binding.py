@@ -134,7 +134,8 @@ def lib():
         L.gw_offline_run.argtypes = [vp, vp, vp, vp, vp]
         L.gw_offline_predictions.argtypes = [vp, vp, vp]
         L.gw_pipeline_graph_nodes.argtypes = [vp]
-        L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(i)]
+        L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_double), C.POINTER(C.c_double),
+                                      C.POINTER(C.c_double), C.POINTER(i)]
         L.gw_profile_label.argtypes = [vp, i]
         L.gw_profile_label.restype = C.c_char_p
         L.gw_profile_flops.argtypes = [vp, i]
@@ -434,11 +435,12 @@ class Pipeline:
         %globaltimer at its first CTA's start and last CTA's end.  -> [dict(label, begin_us, end_us, flops, smem_bytes)]
         in launch order; begin/end are relative to the start of the step's first kernel."""
         n_max = 32
-        b, e = (C.c_double * n_max)(), (C.c_double * n_max)()
+        b, e, mhz = (C.c_double * n_max)(), (C.c_double * n_max)(), (C.c_double * n_max)()
         n = C.c_int(0)
         _check(lib().gw_step_profile(self.h, _ptr(new_samples), _ptr(scores), _ptr(cleaned_final),
-                                     _stream_ptr(stream), n_max, b, e, C.byref(n)), self.h)
+                                     _stream_ptr(stream), n_max, b, e, mhz, C.byref(n)), self.h)
         return [{"label": lib().gw_profile_label(self.h, i).decode(), "begin_us": float(b[i]), "end_us": float(e[i]),
+                 "sm_mhz": float(mhz[i]),
                  "flops": float(lib().gw_profile_flops(self.h, i)), "smem_bytes": float(lib().gw_profile_smem_bytes(self.h, i))}
                 for i in range(min(n.value, n_max))]
 

@@ -196,11 +196,22 @@ __device__ __forceinline__ unsigned long long gw_globaltimer() {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
+// Slots per kernel: [0] min begin (ns) over CTAs, [1] max end (ns) over CTAs, and for CTA 0 alone its own begin / end in
+// SM cycles ([2], [3]: clock64) and in ns ([4], [5]): cycles / ns = the SM clock that kernel actually ran at.
+constexpr int kStampSlots = 6;
 __device__ __forceinline__ void stamp_begin(unsigned long long* s) {
-    if (s != nullptr && threadIdx.x == 0) atomicMin(s, gw_globaltimer());
+    if (s != nullptr && threadIdx.x == 0) {
+        const unsigned long long t = gw_globaltimer();
+        atomicMin(s, t);
+        if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) { s[2] = static_cast<unsigned long long>(clock64()); s[4] = t; }
+    }
 }
 __device__ __forceinline__ void stamp_end(unsigned long long* s) {   // call after a __syncthreads() of the whole CTA
-    if (s != nullptr && threadIdx.x == 0) atomicMax(s + 1, gw_globaltimer());
+    if (s != nullptr && threadIdx.x == 0) {
+        const unsigned long long t = gw_globaltimer();
+        atomicMax(s + 1, t);
+        if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) { s[3] = static_cast<unsigned long long>(clock64()); s[5] = t; }
+    }
 }
 
 }  // namespace gw

@@ -232,7 +232,7 @@ struct Prof {
 };
 struct LaunchCtx {
     cudaStream_t st = nullptr;
-    unsigned long long* stamps = nullptr;          // device [kMaxStamps][2] (begin, end) or null
+    unsigned long long* stamps = nullptr;          // device [kMaxStamps][kStampSlots] or null
     Prof* prof = nullptr;
     cudaError_t err = cudaSuccess;
     explicit LaunchCtx(cudaStream_t s) : st(s) {}
@@ -241,7 +241,7 @@ struct LaunchCtx {
         const int i = static_cast<int>(prof->labels.size());
         if (i >= kMaxStamps) return nullptr;
         prof->labels.push_back(label); prof->flops.push_back(flops); prof->smem.push_back(smem);
-        return stamps + 2 * i;
+        return stamps + kStampSlots * i;
     }
     void check(cudaError_t e) { if (err == cudaSuccess && e != cudaSuccess) err = e; }
 };
@@ -1524,7 +1524,7 @@ static int pipeline_capture(gw_pipeline* p, GraphVar& v, bool zones, bool stampe
     graphvar_reset(v);
     LaunchCtx cx(st);
     if (stamped) {
-        if (!p->d_stamps) CU_TRY(cudaMalloc(&p->d_stamps, kMaxStamps * 2 * sizeof(unsigned long long)));
+        if (!p->d_stamps) CU_TRY(cudaMalloc(&p->d_stamps, kMaxStamps * kStampSlots * sizeof(unsigned long long)));
         cx.stamps = p->d_stamps;
         cx.prof = &v.prof;
     }
@@ -1647,7 +1647,7 @@ extern "C" int gw_step(gw_pipeline* p, const float* new_samples_dev, float* scor
 // One update through the PROFILING graph: the same kernels and launch attributes as gw_step, each stamping
 // %globaltimer at its first CTA's start and its last CTA's end; synchronises.
 extern "C" int gw_step_profile(gw_pipeline* p, const float* new_samples_dev, float* scores_dev, float* cleaned_final_dev,
-                               void* stream, int max_kernels, double* begin_us, double* end_us, int* n_out) {
+                               void* stream, int max_kernels, double* begin_us, double* end_us, double* sm_mhz, int* n_out) {
     if (!p || !new_samples_dev || !cleaned_final_dev || !begin_us || !end_us || !n_out || (p->bbh && !scores_dev))
         return fail(GW_EINVAL, "gw_step_profile: NULL argument");
     CallScope scope(p);
@@ -1660,15 +1660,17 @@ extern "C" int gw_step_profile(gw_pipeline* p, const float* new_samples_dev, flo
     for (auto& g : p->dc->gemm) trace_report(g);
     if (p->bbh) for (auto& g : p->bbh->gemm) trace_report(g);
 #endif
-    unsigned long long h[kMaxStamps * 2];
+    unsigned long long h[kMaxStamps * kStampSlots];
     CU_TRY(cudaMemcpy(h, p->d_stamps, sizeof h, cudaMemcpyDeviceToHost));
     const int nk = static_cast<int>(v->prof.labels.size());
     unsigned long long t0 = ~0ull;
-    for (int i = 0; i < nk; ++i) if (h[2 * i] < t0) t0 = h[2 * i];
+    for (int i = 0; i < nk; ++i) if (h[kStampSlots * i] < t0) t0 = h[kStampSlots * i];
     *n_out = nk;
     for (int i = 0; i < nk && i < max_kernels; ++i) {
-        begin_us[i] = static_cast<double>(h[2 * i] - t0) * 1e-3;
-        end_us[i] = static_cast<double>(h[2 * i + 1] - t0) * 1e-3;
+        const unsigned long long* s = h + kStampSlots * i;
+        begin_us[i] = static_cast<double>(s[0] - t0) * 1e-3;
+        end_us[i] = static_cast<double>(s[1] - t0) * 1e-3;
+        if (sm_mhz) sm_mhz[i] = s[5] > s[4] ? static_cast<double>(s[3] - s[2]) / static_cast<double>(s[5] - s[4]) * 1e3 : 0.0;
     }
     p->last_prof = &v->prof;
     return GW_OK;

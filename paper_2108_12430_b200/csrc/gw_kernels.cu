@@ -64,7 +64,10 @@ __device__ __forceinline__ void unpack16x8(const uint4& q, float (&f)[8], int fm
 // Profiling graph only: reset the %globaltimer stamps (begin = min over CTAs -> start from the maximum; end = max).
 __global__ void k_stamp_init(unsigned long long* stamps, int n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) { stamps[2 * i] = ~0ull; stamps[2 * i + 1] = 0ull; }
+    if (i < n) {
+        stamps[kStampSlots * i] = ~0ull;
+        for (int j = 1; j < kStampSlots; ++j) stamps[kStampSlots * i + j] = 0ull;
+    }
 }
 cudaError_t launch_stamp_init(unsigned long long* stamps, int n, cudaStream_t st) {
     k_stamp_init<<<(n + 63) / 64, 64, 0, st>>>(stamps, n);

@@ -940,6 +940,7 @@ def test_step_profile_decomposes_the_graph_step_and_outputs_rotate_without_recap
                 prev_end, span = 0.0, 0.0
                 for r in rows:
                     assert r["end_us"] > r["begin_us"] >= 0.0, r
+                    assert 300.0 < r["sm_mhz"] < 2500.0, r       # clock64 / %globaltimer of the kernel's CTA 0
                     span += max(0.0, r["end_us"] - max(r["begin_us"], prev_end))
                     prev_end = max(prev_end, r["end_us"])
                 # exclusive shares + idle gaps between kernels = end of the last kernel
