@@ -716,6 +716,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     // dense(hidden -> 1), sigmoid: fused into this (last) conv block's epilogue.
                     float* gap_s = pool_s + 64 * pstride;                    // [half]
                     float* hid_s = gap_s + half;                             // [hidden]
+                    // this warp's rows of the first dense layer (hidden <= 64, half <= 128: 8 rows x 4 values per lane),
+                    // requested NOW so that their L2 latency runs under the pooling barriers instead of once per row
+                    const bool pre_w = p.head_hidden <= 8 * kEpiWarps && half <= 128;
+                    float wreg[8][4];
+                    if (pre_w) {
+#pragma unroll
+                        for (int rr = 0; rr < 8; ++rr) {
+                            const int hrow = warp - 2 + rr * kEpiWarps;
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) {
+                                const int c = lane + 32 * k;
+                                wreg[rr][k] = (hrow < p.head_hidden && c < half) ? __ldg(p.hw1 + static_cast<size_t>(hrow) * half + c) : 0.f;
+                            }
+                        }
+                    }
                     asm volatile("bar.sync 1, 256;" ::: "memory");
                     for (int c = et; c < half; c += kEpiWarps * 32) {
                         float s = 0.f;
@@ -725,13 +740,29 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     asm volatile("bar.sync 1, 256;" ::: "memory");
                     // one warp per hidden unit, lanes stride over the inputs: the weight row is read with coalesced
                     // 128-byte requests (one thread per row walked 128 dependent, uncoalesced loads: ~15 us per launch)
-                    for (int hrow = warp - 2; hrow < p.head_hidden; hrow += kEpiWarps) {
-                        const float* wr = p.hw1 + static_cast<size_t>(hrow) * half;
-                        float s = 0.f;
-                        for (int c = lane; c < half; c += 32) s = fmaf(__ldg(wr + c), gap_s[c], s);
+                    if (pre_w) {
+                        float gv[4];
 #pragma unroll
-                        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-                        if (lane == 0) hid_s[hrow] = fmaxf(s + __ldg(p.hb1 + hrow), 0.f);
+                        for (int k = 0; k < 4; ++k) gv[k] = lane + 32 * k < half ? gap_s[lane + 32 * k] : 0.f;
+#pragma unroll
+                        for (int rr = 0; rr < 8; ++rr) {
+                            const int hrow = warp - 2 + rr * kEpiWarps;
+                            float s = 0.f;
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) s = fmaf(wreg[rr][k], gv[k], s);      // same order as the loop below
+#pragma unroll
+                            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+                            if (lane == 0 && hrow < p.head_hidden) hid_s[hrow] = fmaxf(s + __ldg(p.hb1 + hrow), 0.f);
+                        }
+                    } else {
+                        for (int hrow = warp - 2; hrow < p.head_hidden; hrow += kEpiWarps) {
+                            const float* wr = p.hw1 + static_cast<size_t>(hrow) * half;
+                            float s = 0.f;
+                            for (int c = lane; c < half; c += 32) s = fmaf(__ldg(wr + c), gap_s[c], s);
+#pragma unroll
+                            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+                            if (lane == 0) hid_s[hrow] = fmaxf(s + __ldg(p.hb1 + hrow), 0.f);
+                        }
                     }
                     asm volatile("bar.sync 1, 256;" ::: "memory");
                     if (et < 32) {

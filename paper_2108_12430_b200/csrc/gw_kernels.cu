@@ -821,7 +821,7 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
                                                       unsigned long long* stamp) {
     constexpr int cin = CIN;
     stamp_begin(stamp);
-    __shared__ __align__(16) float xs[kC1MaxCin][kC1Span];
+    __shared__ __align__(16) float xs2[2][kC1MaxCin][kC1Span];   // double-buffered input tile
     __shared__ float xr[kC1MaxCin][kC1Span + kMaxFir];        // D12: raw samples of the tile + the filter's history
     __shared__ float gs[kC1MaxCin][kMaxFir];                  // D12: whitening taps per input channel
     __shared__ __align__(16) float ws[32][kC1MaxCin][8];      // this block's 32 channels, zero where unused
@@ -841,9 +841,32 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
     griddep_launch_dependents();
     const int pg = wrp & 1;                               // position group: pooled positions [32 pg, +32) of the tile
     const int cg = wrp >> 1;                              // channel group: channels [8 cg, +8) of the block's 32
+    // Plain path: the NEXT tile's samples are fetched into registers before the current tile is computed and stored into
+    // the other buffer afterwards, so a block pays the global-load latency once, not once per tile (one barrier per tile).
+    constexpr int kPre = (CIN * kC1Span + 255) / 256;     // elements of a tile per thread
+    float nxt[kPre];
+    auto fetch = [&](int q0f) {
+        const int l0f = q0f * 4 - pad_l;
+#pragma unroll
+        for (int e = 0; e < kPre; ++e) {
+            const int i = threadIdx.x + e * 256;
+            const int ci = i / kC1Span, l = l0f + i % kC1Span;
+            nxt[e] = (i < cin * kC1Span && l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
+        }
+    };
+    auto stash = [&](int bufi) {
+#pragma unroll
+        for (int e = 0; e < kPre; ++e) {
+            const int i = threadIdx.x + e * 256;
+            if (i < cin * kC1Span) xs2[bufi][i / kC1Span][i % kC1Span] = nxt[e];
+        }
+    };
+    int buf = 0;
+    if (!whiten && blockIdx.x * kC1Q < Lq) { fetch(blockIdx.x * kC1Q); stash(0); }
     for (int q0 = blockIdx.x * kC1Q; q0 < Lq; q0 += gridDim.x * kC1Q) {
         const int l0 = q0 * 4 - pad_l;                    // first input position of the tile
-        __syncthreads();                                  // the previous tile has been consumed (and ws / bs / gs are written)
+        float (*xs)[kC1Span] = xs2[buf];
+        __syncthreads();                                  // this tile is in xs; the previous one has been consumed
         if (whiten) {
             // D12: the block sees the WHITENED window y[l] = sum_j g[j] x[l - j] (x[l < 0] = 0: zero initial state at the
             // window start); outside [0, L) it is the conv's zero padding as before
@@ -860,13 +883,10 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
                     for (int j = 0; j < whiten_n; ++j) v = fmaf(gs[ci][j], xr[ci][q + hl - j], v);
                 xs[ci][q] = v;
             }
-        } else {
-            for (int i = threadIdx.x; i < cin * kC1Span; i += blockDim.x) {
-                const int ci = i / kC1Span, l = l0 + i % kC1Span;
-                xs[ci][i % kC1Span] = (l >= 0 && l < L) ? __ldg(x + (static_cast<size_t>(b) * cin + ci) * L + l) : 0.f;
-            }
+            __syncthreads();
+        } else if (q0 + gridDim.x * kC1Q < Lq) {
+            fetch(q0 + gridDim.x * kC1Q);                 // in flight while this tile is computed
         }
-        __syncthreads();
         const int ql = pg * 32 + lane;                    // pooled position inside the tile
         const int q = q0 + ql;
         float v[CIN][12];
@@ -906,6 +926,10 @@ __global__ void __launch_bounds__(256, 4) k_bbh_conv1(const float* __restrict__ 
             o.x = pack16(res[0], res[1], fmt); o.y = pack16(res[2], res[3], fmt);
             o.z = pack16(res[4], res[5], fmt); o.w = pack16(res[6], res[7], fmt);
             *reinterpret_cast<uint4*>(reinterpret_cast<uint16_t*>(out) + (static_cast<size_t>(b) * Lq + q) * cpad + cbase + cg * 8) = o;
+        }
+        if (!whiten) {
+            if (q0 + gridDim.x * kC1Q < Lq) stash(buf ^ 1);   // the other buffer: its last readers passed this tile's barrier
+            buf ^= 1;
         }
     }
     __syncthreads();
