@@ -124,9 +124,16 @@ typedef struct {
  *              the new samples or one of the two window edges; every other row IS the previous update's value.
  *              Results are bit-identical to full recomputation.  Needs stride and window to be multiples of
  *              2^(encoder depth), window a multiple of 128 * 2^(encoder depth), the fused tail and GW_IMPL_UMMA
- *              (GW_EINVAL otherwise). */
+ *              (GW_EINVAL otherwise).
+ *  fuse_bbh    1 (default): the whole classifier (three conv blocks, pooling, dense head, sigmoid) runs as ONE kernel
+ *              with one CTA per window and every activation in shared memory, when its shape is three blocks of k = 8,
+ *              pad_l = 3 with at most 32 / 64 and exactly 128 output channels, at most 2 detectors, a window that is a
+ *              multiple of 512 in [512, 4096] and a dense hidden width <= 64 (BASELINE.json configs[2]); other shapes,
+ *              fuse_bbh = 0 and GW_IMPL_SIMT take the three-kernel path (first block on CUDA cores, blocks 2 and 3 as
+ *              conv GEMMs with activations in global memory).  Both paths keep the fp32 input unrounded; they agree
+ *              within rounding (different summation order). */
 typedef struct {
-    int conv_impl, fuse_tail, pdl, snake, two_sm, skip_zeros, incremental;
+    int conv_impl, fuse_tail, pdl, snake, two_sm, skip_zeros, incremental, fuse_bbh;
 } gw_options;
 void gw_options_default(gw_options *o);
 

@@ -185,6 +185,28 @@ cudaError_t launch_bbh_conv1(const float* x, const float* w, const float* b, voi
                              int cout, int cpad, int K, int pad_l, int pool, int fmt, const float* whiten, int whiten_n,
                              int pdl, Stamp stamp, cudaStream_t st);
 
+// The whole classifier (three conv blocks + pooling + dense head) as ONE kernel, one CTA per window, every activation in
+// shared memory (gw_bbh_fused.cu).  The weight images are built on the host in the exact shared-memory byte layout of the
+// UMMA operands (K-major, SWIZZLE_128B) so that plain bulk copies load them:
+//   w1img  [128 rows n = phase*32 + cout][64 k = (cin*2 + part)*16 + i]   block 1 as a Toeplitz matrix over 11 input samples
+//   w2img  [4 tap pairs][64 rows cout][64 k = (tap & 1)*32 + cin]
+//   w3img  [8 taps][128 rows cout][64 k = cin]
+struct BbhFusedParams {
+    const float* x;                // [batch][cin][L] fp32
+    const uint8_t *w1img, *w2img, *w3img;
+    const float *b1, *b2, *b3;     // [32], [64], [128] fp32 (channels past cout: 0)
+    const float *hw1, *hb1, *hw2, *hb2;   // dense head: [hidden][128], [hidden], [hidden], [1]
+    const float* whiten;           // D12: [cin][whiten_n] or null
+    int whiten_n;
+    float* scores;                 // [batch]
+    int L, cin, hidden;
+    Stamp stamp;
+};
+constexpr int kBbhW1Bytes = 128 * 128, kBbhW2Bytes = 4 * 64 * 128, kBbhW3Bytes = 8 * 128 * 128;
+bool bbh_fused_supported(int L, int cin, int hidden);
+cudaError_t bbh_fused_prepare();
+cudaError_t launch_bbh_fused(const BbhFusedParams& p, int batch, int fmt, int pdl, cudaStream_t st);
+
 cudaError_t launch_stamp_init(unsigned long long* stamps, int n, cudaStream_t st);   // begin slots = max, end slots = 0
 void count_launch();               // one more kernel launched (or captured) by this library: atomic process-wide counter
 long long kernel_launches();

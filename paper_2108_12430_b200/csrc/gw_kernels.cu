@@ -660,7 +660,7 @@ __global__ void __launch_bounds__(256) k_aggregate(const AggParams a) {
 // four, so a group never straddles the wrap, the newest stride, the final block or the classifier window.
 // (The scalar kernel spent its time on per-sample index arithmetic: ncu SM throughput 72 %, 1.9 TB/s.)
 template <bool FIR>
-__global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
+__global__ void __launch_bounds__(256, FIR ? 4 : 8) k_aggregate_v4(const AggParams a) {
     stamp_begin(a.stamp);
     // An ordinary launch, neither a programmatic dependent nor a trigger (both measured, n = 128): as a dependent its
     // 8192 short CTAs each pay griddepcontrol.wait (+14 us); triggering the first classifier block early lets that
@@ -678,9 +678,13 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
         const size_t wi = static_cast<size_t>(sd) * W;
         float4 nhat = make_float4(0.f, 0.f, 0.f, 0.f), cleaned = nhat;
         if (abs_idx >= 0) {
-            const float4 p = __ldg(reinterpret_cast<const float4*>(a.pred + wi + (a.pred_ring ? slot : n)));
+            // the strain is read (and the estimate mapped back to strain units) only where a cleaned sample leaves the
+            // kernel: inside the step that is the S final samples and the classifier window, not the whole window
+            const int f0o = (a.agg == 0) ? 0 : W - S - a.delta, c0o = W - a.delta - a.Lb;
+            const bool wanted = a.running_out || a.nhat_out || (n >= f0o && n < f0o + S) || (a.clf_in && n >= c0o && n < c0o + a.Lb);
             float4* accp = reinterpret_cast<float4*>(a.acc + wi + slot);
             if (a.agg == 0) {
+                const float4 p = __ldg(reinterpret_cast<const float4*>(a.pred + wi + (a.pred_ring ? slot : n)));
                 const float4 prev = (n >= W - S) ? make_float4(0.f, 0.f, 0.f, 0.f) : *accp;
                 const float4 hw = __ldg(reinterpret_cast<const float4*>(a.hann + n));
                 const float4 iw = __ldg(reinterpret_cast<const float4*>(a.inv_wsum + n));
@@ -689,16 +693,20 @@ __global__ void __launch_bounds__(256) k_aggregate_v4(const AggParams a) {
                 nhat = make_float4(acc.x * iw.x, acc.y * iw.y, acc.z * iw.z, acc.w * iw.w);
             } else {
                 if (n >= W - a.delta) nhat = make_float4(0.f, 0.f, 0.f, 0.f);
-                else if (n >= W - S - a.delta) { nhat = p; *accp = p; }
-                else nhat = *accp;
+                else if (n >= W - S - a.delta) {
+                    nhat = __ldg(reinterpret_cast<const float4*>(a.pred + wi + (a.pred_ring ? slot : n)));
+                    *accp = nhat;
+                } else if (wanted) nhat = *accp;
             }
-            if (a.agg == 0 || n < W - a.delta) {               // post-processing: estimate back to strain units
-                const float ps = __ldg(a.post + 2 * d), pm = __ldg(a.post + 2 * d + 1);
-                nhat = make_float4(fmaf(ps, nhat.x, pm), fmaf(ps, nhat.y, pm), fmaf(ps, nhat.z, pm), fmaf(ps, nhat.w, pm));
+            if (wanted) {
+                if (a.agg == 0 || n < W - a.delta) {           // post-processing: estimate back to strain units
+                    const float ps = __ldg(a.post + 2 * d), pm = __ldg(a.post + 2 * d + 1);
+                    nhat = make_float4(fmaf(ps, nhat.x, pm), fmaf(ps, nhat.y, pm), fmaf(ps, nhat.z, pm), fmaf(ps, nhat.w, pm));
+                }
+                const float4 st4 = __ldg(reinterpret_cast<const float4*>(
+                    a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot));
+                cleaned = make_float4(st4.x - nhat.x, st4.y - nhat.y, st4.z - nhat.z, st4.w - nhat.w);
             }
-            const float4 st4 = __ldg(reinterpret_cast<const float4*>(
-                a.ring + (static_cast<size_t>(s) * a.channels + __ldg(a.strain_rows + d)) * W + slot));
-            cleaned = make_float4(st4.x - nhat.x, st4.y - nhat.y, st4.z - nhat.z, st4.w - nhat.w);
         }
         if (a.running_out) *reinterpret_cast<float4*>(a.running_out + wi + n) = cleaned;
         if (a.nhat_out) *reinterpret_cast<float4*>(a.nhat_out + wi + n) = nhat;

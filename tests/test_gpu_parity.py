@@ -201,11 +201,13 @@ def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype, fuse):
 
 
 # ----------------------------------------------------------------------------- classifier (C2)
+@pytest.mark.parametrize("fuse", [1, 0])
 @pytest.mark.parametrize("length,batch", [(4096, 24), (1024, 5)])
-def test_bbh_batch_matches_oracle(length, batch):
+def test_bbh_batch_matches_oracle(length, batch, fuse):
+    """fuse = 1: the one-kernel, shared-memory-resident classifier (gw_options.fuse_bbh, the default); 0: three kernels."""
     cfg = S.config_c2()
     cp, dp = util.centred_bbh_params(202, cfg.bbh_convs, cfg.bbh_dense, length)
-    bbh = gw.Bbh(None, cfg.bbh_convs, cp, dp, length, gw.GW_BF16, n_det=2, max_batch=32)
+    bbh = gw.Bbh(None, cfg.bbh_convs, cp, dp, length, gw.GW_BF16, n_det=2, max_batch=32, opts=gw.Options(fuse_bbh=fuse))
     x = synth.bbh_windows(2, batch, length)
     got = bbh.score_batch(_dev(x)).cpu().numpy()
     pc = [oracle.prepare_conv(l, p, oracle.DT_BF16) for l, p in zip(cfg.bbh_convs, cp)]
@@ -216,6 +218,46 @@ def test_bbh_batch_matches_oracle(length, batch):
     assert 0.2 < np.mean(ref) < 0.8 and np.std(ref) > 1e-2, "scores should not be degenerate"
     print("bbh scores: max |d| %.2e, max |d logit| %.2e, ref range %.3f..%.3f" % (
         np.max(np.abs(got - ref)), np.max(np.abs(util.logit(got) - util.logit(ref))), ref.min(), ref.max()))
+
+
+@pytest.mark.parametrize("dtype", [gw.GW_FP16, gw.GW_BF16])
+@pytest.mark.parametrize("length,n_det,scale,white", [(512, 2, 1.0, False), (2048, 1, 1.0, True), (1536, 2, 2.0 ** -12, False),
+                                                     (4096, 2, 2.0 ** 17, True), (3584, 2, 1.0, False)])
+def test_bbh_fused_kernel_shapes_scales_and_whitening(length, n_det, scale, white, dtype):
+    """The one-kernel classifier at every window length it accepts (tile counts 1..8, one and two block-2 tiles), with one
+    detector, with D12 whitening (64 taps: the longest history), and with inputs far outside fp16 range in either direction
+    (its first block feeds the tensor core a power-of-two-scaled (hi, lo) pair per sample): against the oracle, and
+    against the three-kernel path, which computes the first block in fp32 on CUDA cores."""
+    convs = S.bbh_layers((n_det, 32, 64, 128))
+    dense = (128, 64, 1)
+    od = oracle.DT_BF16 if dtype == gw.GW_BF16 else oracle.DT_FP16
+    rng = np.random.default_rng(length + n_det)
+    g = None
+    if white:
+        g = (rng.standard_normal((n_det, 64)) * np.exp(-np.arange(64) / 6.0)).astype(np.float32)
+        g[:, 0] = 1.0
+    x = (synth.bbh_windows(7, 6, length)[:, :n_det] * scale).astype(np.float32)
+    xw = x if g is None else np.stack([np.stack([oracle.fir_causal(x[i][d], g[d]) for d in range(n_det)]) for i in range(len(x))])
+    # centre the logits on THESE inputs (weights of the first block absorb the input scale)
+    cp, dp = synth.bbh_params(303, convs, dense)
+    cp[0]["w"] = (cp[0]["w"] / np.float32(scale)).astype(np.float32)
+    pc = [oracle.prepare_conv(l, p, od) for l, p in zip(convs, cp)]
+    mean_logit = float(np.mean([oracle.bbh_forward(xw[i], convs, pc, [oracle.prepare_dense(p) for p in dp], return_logit=True)
+                                for i in range(len(x))]))
+    dp[-1]["b"] = (dp[-1]["b"] - np.float32(mean_logit)).astype(np.float32)
+    pd = [oracle.prepare_dense(p) for p in dp]
+    ref = np.array([oracle.bbh_forward(xw[i], convs, pc, pd) for i in range(len(x))])
+    got = {}
+    for fuse in (1, 0):
+        bbh = gw.Bbh(None, convs, cp, dp, length, dtype, n_det=n_det, max_batch=8, opts=gw.Options(fuse_bbh=fuse))
+        if g is not None:
+            bbh.set_whitening(g)
+        got[fuse] = bbh.score_batch(_dev(x)).cpu().numpy()
+        assert np.max(np.abs(got[fuse] - ref)) <= util.SCORE_ABS, (fuse, got[fuse], ref)
+        assert np.max(np.abs(util.logit(got[fuse]) - util.logit(ref))) <= util.LOGIT_ABS, (fuse, got[fuse], ref)
+    assert np.std(ref) > 1e-3, "scores should not be degenerate"
+    print("fused classifier L=%d D=%d scale=%g white=%s: max |d| vs oracle %.2e (three kernels %.2e), fused vs three kernels %.2e" % (
+        length, n_det, scale, white, np.max(np.abs(got[1] - ref)), np.max(np.abs(got[0] - ref)), np.max(np.abs(got[1] - got[0]))))
 
 
 # -------------------------------------------------------------------- end-to-end small ensemble
@@ -935,8 +977,8 @@ def test_step_profile_decomposes_the_graph_step_and_outputs_rotate_without_recap
             if mode == "profiled" and t >= 2:
                 rows = pipe.step_profile(xc[t], scs[b], fins[b], cs)
                 labels = [r["label"] for r in rows]
-                assert labels[0] == "snapshot_append" and "aggregate" in labels and labels[-1].startswith("gemm.bbh")
-                assert len(rows) == pipe.graph_nodes() == 12
+                assert labels[0] == "snapshot_append" and "aggregate" in labels and labels[-1] == "bbh_fused"
+                assert len(rows) == pipe.graph_nodes() == 10
                 prev_end, span = 0.0, 0.0
                 for r in rows:
                     assert r["end_us"] > r["begin_us"] >= 0.0, r
