@@ -172,6 +172,7 @@ struct AggParams {
     float* clf_in;             // [n][D][Lb] or null
     int n_streams, n_det, channels, W, S, Lb, delta, agg;
     int pred_ring;
+    int trigger;               // 1: let the next kernel of the stream (launched as a programmatic dependent) start early
     Stamp stamp;
     // D11: causal FIR over the stream of emitted (final) estimate samples.  fir: [fir_n] taps or null; hist: [2][n*D][kMaxFir-1]
     // the last fir_n - 1 emitted samples of the previous update (double-buffered by update parity).

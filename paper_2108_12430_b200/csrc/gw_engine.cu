@@ -1274,6 +1274,9 @@ static AggParams make_agg(gw_deepclean* dc, float* final_out, float* running_out
     a.n_streams = s->n; a.n_det = dc->n_det; a.channels = s->C; a.W = s->W; a.S = s->S; a.Lb = dc->Lb;
     a.delta = dc->delta; a.agg = dc->agg;
     a.pred_ring = dc->inc ? 1 : 0;
+    // the one-kernel classifier is one CTA of 288 threads per SM: as a programmatic dependent its prologue (barriers, TMEM,
+    // weight loads) runs under this kernel's last wave without taking its thread slots
+    a.trigger = (dc->bbh && dc->bbh->fused && dc->opt.pdl && dc->bbh->opt.pdl) ? 1 : 0;
     a.fir = dc->d_fir; a.hist = dc->d_hist; a.fir_n = dc->fir_n;
     return a;
 }

@@ -665,6 +665,7 @@ __global__ void __launch_bounds__(256, FIR ? 4 : 8) k_aggregate_v4(const AggPara
     // An ordinary launch, neither a programmatic dependent nor a trigger (both measured, n = 128): as a dependent its
     // 8192 short CTAs each pay griddepcontrol.wait (+14 us); triggering the first classifier block early lets that
     // kernel's CTAs take thread slots from this bandwidth kernel's last waves (+6 us) to save 1 us downstream.
+    if (a.trigger) griddep_launch_dependents();
     const long long cnt = *a.count;
     const int W = a.W, S = a.S;
     const int h = static_cast<int>(cnt % W);
