@@ -322,10 +322,12 @@ def kernel_table(eng, order, acc, pk, sm_mhz, sms):
         "append": sp.n_streams * sp.channels * sp.stride * 8,                       # read new + write ring
         "ring16_append": sp.n_streams * nd * sp.stride * (nw * 4 + 2 * 32 * 2),     # read fp32, write both mirror copies
         "snapshot_append": sp.n_streams * (sp.channels * sp.stride * 8 + nd * sp.stride * 2 * 32 * 2),  # a1 + a2 fused
-        # a5 as launched inside the step: reads p_t, acc, strain (12 W), writes acc (4 W) + the S final samples + the
-        # L_b classifier samples per detector-window; the running cleaned window is NOT written on this path
-        "aggregate": sp.n_streams * nd * (sp.window * 16 + (sp.stride + cfg.bbh_len) * 4),
+        # a5 as launched inside the step: reads p_t and acc (8 W - 4 S: the newest stride's accumulators start from zero),
+        # writes acc (4 W); the strain is read only where a cleaned sample leaves the kernel -- the S final samples and the
+        # L_b classifier samples (8 (S + L_b) read + written); the running cleaned window is NOT written on this path
+        "aggregate": sp.n_streams * nd * (sp.window * 12 + sp.stride * 4 + cfg.bbh_len * 8),
         "bbh_conv1": sp.n_streams * (nd * cfg.bbh_len * 4 + (cfg.bbh_len // 4) * 32 * 2),
+        "bbh_fused": sp.n_streams * (nd * cfg.bbh_len * 4 + 4),                      # the window in, one score out
     }
     smem_peak_gbs = sms * 128 * sm_mhz * 1e6 / 1e9
     out = {}
