@@ -63,13 +63,13 @@ __host__ __device__ __forceinline__ int head_scratch_bytes(int N, int hidden) {
 bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
     ConvGemmParams& p = g.p;
     const int b_block = p.N * 128;
-    const int sl = slab_bytes_of(p.slab_rows);
+    const int sl = slab_bytes_of(p.slab_rows + (p.two_sm ? p.pk_nl : 0));
     if (p.two_sm) {
         // CTA-pair kernel: N = 256 store layers with an even number of tiles; half weight blocks of 16 KiB
         const int pairs = sm_count / 2;
         // ring input (incremental path): needs the per-head tensor maps; the pair works on virtual tiles 2u, 2u + 1
-        bool ok = p.epi == EPI_STORE && p.N == 256 && (p.a_count == nullptr || p.tmA_heads != nullptr) && p.v_tiles % 2 == 0 &&
-                  pairs >= p.n_det;
+        bool ok = p.epi == EPI_STORE && p.N == 256 && (p.a_count == nullptr || p.tmA_heads != nullptr) &&
+                  (p.pk_nl ? (g.batch / p.n_det) % 2 == 0 && p.tmA_heads_left != nullptr : p.v_tiles % 2 == 0) && pairs >= p.n_det;
         for (int ob = 2; ok && ob >= 1; --ob) {
             const int fixed = kFixedSmem + ob * kOutStage;
             const int sa = p.n_cb < 2 ? 2 : (p.n_cb > 8 ? 8 : p.n_cb);
@@ -82,6 +82,7 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
             return true;
         }
         p.two_sm = 0;
+        p.pk_nl = 0;                                   // packing exists in the pair kernel only
     }
     // EPI_STORE stages its output through shared memory for TMA stores: one 4 KiB buffer per epilogue warp,
     // two when the operands leave room (thin layers)
@@ -826,7 +827,12 @@ template <int ACT, int FMT>
 __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid_constant__ ConvGemmParams p, int n_items) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int sl = slab_bytes_of(p.slab_rows);
+    // Packed zones (incremental path, p.pk_nl > 0): ONE tile per batch item holds both recomputed zones -- slab rows
+    // [0, pk_nl) are the input rows of the left zone (outputs 0 .. pk_left-1), slab rows [pk_nl, pk_nl + slab_rows) those of
+    // the right zone (tile rows pk_nl .. pk_nl + pk_right - 1 = the layer's LAST pk_right rows); the tile rows in between
+    // mix the two and are dropped.  The two CTAs of a pair then work on two consecutive batch items.
+    const bool packed = p.pk_nl > 0;
+    const int sl = slab_bytes_of(p.slab_rows + p.pk_nl);
     const int sa = p.sa_stages, sb = p.sb_stages;
     uint8_t* smem_out = smem;                                                // [out_bufs][8 warps][4 KiB]
     uint8_t* smem_b = smem + p.out_bufs * kOutStage;                         // [sb][16 KiB]
@@ -850,8 +856,8 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
     const int det = cid % p.n_det;
     const int cworker = cid / p.n_det;
     const int n_cw = (gridDim.x / 2) / p.n_det;
-    const int half_tiles = p.v_tiles / 2;                                    // (virtual) tile pairs per batch item
-    const int total = n_items * half_tiles;
+    const int half_tiles = packed ? 1 : p.v_tiles / 2;                       // (virtual) tile pairs per batch item
+    const int total = packed ? n_items / 2 : n_items * half_tiles;           // packed: one pair = two batch items
 
     if (warp == 0) {
         if (lane == 0) {
@@ -883,7 +889,9 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
         // block (otherwise the weight ring could fill while the MMA warp waits for the slab).
         griddep_wait();
         // ring input: this update's window has its own tensor map (rows outside the window are zero fill)
-        const CUtensorMap* tmA = p.tmA_heads ? p.tmA_heads + static_cast<int>(*p.a_count % p.a_ring_W) / p.head_div : &p.tmA;
+        const int head = p.tmA_heads ? static_cast<int>(*p.a_count % p.a_ring_W) / p.head_div : 0;
+        const CUtensorMap* tmA = p.tmA_heads ? p.tmA_heads + head : &p.tmA;
+        const CUtensorMap* tmA_left = packed ? p.tmA_heads_left + head : nullptr;   // box of pk_nl rows
         const uint32_t lead_a_full = mapa_u32(smem_u32(a_full), 0), lead_b_full = mapa_u32(smem_u32(b_full), 0);
         unsigned long long cbstart = 0;
         {
@@ -906,10 +914,18 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
             else if (!__shfl_sync(0xffffffffu, mbar_test_wait(&a_empty[stage], aph ^ 1) ? 1 : 0, 0)) return false;
             if (lane == 0) {
                 const int u = p.reverse ? total - 1 - aw : aw;
-                const int m0 = map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
-                if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.slab_rows * 128);
-                tma_load_3d_2sm(smem_a + stage * sl, tmA, lead_a_full + 8u * stage, acb * kSegK, m0 + p.a_min,
-                                (u / half_tiles) * p.n_det + det);
+                if (packed) {
+                    const int batch = (2 * u + static_cast<int>(rank)) * p.n_det + det;
+                    if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * (p.slab_rows + p.pk_nl) * 128);
+                    tma_load_3d_2sm(smem_a + stage * sl, tmA_left, lead_a_full + 8u * stage, acb * kSegK, p.a_min, batch);
+                    tma_load_3d_2sm(smem_a + stage * sl + p.pk_nl * 128, tmA, lead_a_full + 8u * stage, acb * kSegK,
+                                    p.M - p.pk_right + p.a_min, batch);
+                } else {
+                    const int m0 = map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
+                    if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.slab_rows * 128);
+                    tma_load_3d_2sm(smem_a + stage * sl, tmA, lead_a_full + 8u * stage, acb * kSegK, m0 + p.a_min,
+                                    (u / half_tiles) * p.n_det + det);
+                }
             }
             if (++stage == sa) { stage = 0; aph ^= 1; }
             if (++acb == n_cb) { acb = 0; aw += n_cw; }
@@ -996,11 +1012,52 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
         for (int w = cworker; w < total; w += n_cw, ++it) {
             const int u = p.reverse ? total - 1 - w : w;
             const int acc = it & 1;
-            const int batch = (u / half_tiles) * p.n_det + det;
-            const int mt = map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank));
+            const int batch = packed ? (2 * u + static_cast<int>(rank)) * p.n_det + det : (u / half_tiles) * p.n_det + det;
+            const int mt = packed ? 0 : map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank));
             TR_WAIT(0, mbar_wait(&tmem_full[acc], (it >> 1) & 1))
             tc_fence_after();
             const uint32_t taddr = tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + acc * kAccCols;
+            if (packed) {
+                // this lane's tile row: a row of the left zone, of the right zone, or one of the mixed rows in between;
+                // the few live rows go straight from registers to their ring row and its twin (r +- M)
+                const int i = quad * 32 + lane;
+                const int lrow = i < p.pk_left ? i : (i >= p.pk_nl && i < p.pk_nl + p.pk_right) ? p.M - p.pk_right + i - p.pk_nl : -1;
+                const int r = out_off + lrow, r2 = r >= p.M ? r - p.M : r + p.M;
+                uint8_t* row1 = reinterpret_cast<uint8_t*>(p.out) + (static_cast<size_t>(batch) * 2 * p.M + r) * 512;
+                uint8_t* row2 = reinterpret_cast<uint8_t*>(p.out) + (static_cast<size_t>(batch) * 2 * p.M + r2) * 512;
+                for (int cp = 0; cp < 2; ++cp) {
+                    const int col = 32 * (4 * cp + 2 * hsel);
+                    uint32_t ra[32], rb[32];
+                    tmem_ld_32x32(taddr + col, ra);
+                    tmem_ld_32x32(taddr + col + 32, rb);
+                    tmem_ld_wait();
+                    if (cp == 1) {
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive_cluster(empty_addr[acc]);
+                    }
+                    if (lrow >= 0) {
+#pragma unroll
+                        for (int which = 0; which < 2; ++which) {
+                            const uint32_t* rr = which == 0 ? ra : rb;
+#pragma unroll
+                            for (int jj = 0; jj < 4; ++jj) {
+                                uint32_t o[4];
+#pragma unroll
+                                for (int h = 0; h < 2; ++h) {
+                                    const float4 b4 = lds_f4(bias_u32 + 4u * (col + 32 * which + 8 * jj + 4 * h));
+                                    o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(rr[8 * jj + 4 * h]) + b4.x, __uint_as_float(rr[8 * jj + 4 * h + 1]) + b4.y);
+                                    o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(rr[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(rr[8 * jj + 4 * h + 3]) + b4.w);
+                                }
+                                const int off = (col + 32 * which + 8 * jj) * 2;
+                                *reinterpret_cast<uint4*>(row1 + off) = make_uint4(o[0], o[1], o[2], o[3]);
+                                *reinterpret_cast<uint4*>(row2 + off) = make_uint4(o[0], o[1], o[2], o[3]);
+                            }
+                        }
+                    }
+                }
+                continue;
+            }
             for (int cp = 0; cp < 2; ++cp) {
                 const int col = 32 * (4 * cp + 2 * hsel);                    // 64 adjacent columns: two 32-column chunks
                 uint32_t ra[32], rb[32];
@@ -1207,7 +1264,7 @@ cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     cudaError_t e;
     if (g.p.two_sm) {
         int cw = g.grid / 2 / g.p.n_det;                         // clusters per detector
-        const int units = n_items * (g.p.v_tiles / 2);
+        const int units = g.p.pk_nl ? n_items / 2 : n_items * (g.p.v_tiles / 2);
         if (cw > units) cw = units;
         cudaLaunchConfig_t cfg2 = {};
         cfg2.gridDim = dim3(2 * cw * g.p.n_det);

@@ -271,6 +271,7 @@ struct GemmLayer {
     void* d_B = nullptr;
     float* d_bias = nullptr;
     CUtensorMap* d_heads = nullptr;              // incremental path, CTA-pair layers: one input tensor map per window head
+    CUtensorMap* d_heads_left = nullptr;         // the same with a box of pk_nl rows (zones packed into one tile)
     int impl = GW_IMPL_UMMA;
     std::string name;                            // profiler label, e.g. "gemm.dc3"
     double flops = 0.0;                          // algorithmic FLOPs per batch item, whole window (real channels and taps only)
@@ -586,9 +587,34 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
 
 // Incremental variant of a built layer: the same operands, work list = the tiles that cover the first `left_rows`
 // and the last `right_rows` GEMM rows of every batch item (all tiles when the two zones meet).
-static void make_incremental_variant(GemmLayer& gl, int left_rows, int right_rows) {
+static int make_incremental_variant(GemmLayer& gl, int left_rows, int right_rows) {
     gl.gi = gl.g;
     ConvGemmParams& p = gl.gi.p;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    // CTA-pair layers (ring input through per-head tensor maps): both zones in ONE tile per batch item when they fit, the
+    // pair working on two batch items -- half the tiles (and half the streamed weights) of a tile per zone
+    if (p.two_sm && p.tmA_heads && (gl.g.batch / p.n_det) % 2 == 0) {
+        const int nl = round_up(left_rows + p.n_shift - 1, 8);
+        if (nl + right_rows <= kTileM && left_rows + right_rows < p.M) {
+            const int n_heads = p.a_ring_W / p.head_div;
+            std::vector<CUtensorMap> heads(n_heads);
+            for (int h = 0; h < n_heads; ++h) {
+                const size_t off_rows = static_cast<size_t>(h) * p.head_div / p.a_ring_div;
+                const uint16_t* base = static_cast<const uint16_t*>(p.A) + off_rows * p.a_cols;
+                if (int rc = make_tmap(&heads[h], base, p.fmt, p.a_cols, p.a_rows, gl.g.batch, p.a_cols,
+                                       static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, nl)) return rc;
+            }
+            CU_TRY(cudaMalloc(&gl.d_heads_left, sizeof(CUtensorMap) * n_heads));
+            CU_TRY(cudaMemcpy(gl.d_heads_left, heads.data(), sizeof(CUtensorMap) * n_heads, cudaMemcpyHostToDevice));
+            p.tmA_heads_left = gl.d_heads_left;
+            p.pk_nl = nl; p.pk_left = left_rows; p.pk_right = right_rows;
+            p.v_left = 0; p.v_tiles = 1;                // one (packed) tile per batch item
+            if (conv_gemm_plan(gl.gi, sms) && gl.gi.p.two_sm) { gl.has_inc = true; return GW_OK; }
+            gl.gi = gl.g;                               // does not fit: the unpacked work list below
+        }
+    }
     const int ts = p.tile_stride;                       // tile t produces rows [t ts, t ts + ts)
     int v_left = (left_rows + ts - 1) / ts;
     int first_right = (p.M - right_rows) / ts;
@@ -596,14 +622,12 @@ static void make_incremental_variant(GemmLayer& gl, int left_rows, int right_row
     if (v_left > p.tiles_m) v_left = p.tiles_m;
     if (first_right <= v_left) { p.v_left = p.v_tiles = p.tiles_m; }
     else { p.v_left = v_left; p.v_tiles = v_left + (p.tiles_m - first_right); }
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     // same operand layout (resident / streamed weights, CTA pair or not: the weight tensor map depends on it); only the
     // tiles-per-stage choice may differ.  A pair layer whose zones give an odd tile count gets one more left tile.
     if (p.two_sm && (p.v_tiles & 1)) { p.v_left += 1; p.v_tiles += 1; }
     conv_gemm_plan(gl.gi, sms);
     gl.has_inc = true;
+    return GW_OK;
 }
 
 #ifdef GW_TRACE
@@ -661,8 +685,8 @@ static void run_gemm(const GemmLayer& gl, LaunchCtx& cx, bool inc = false, int b
 }
 
 static void free_gemm(GemmLayer& gl) {
-    cudaFree(gl.d_B); cudaFree(gl.d_bias); cudaFree(gl.d_heads);
-    gl.d_B = nullptr; gl.d_bias = nullptr; gl.d_heads = nullptr;
+    cudaFree(gl.d_B); cudaFree(gl.d_bias); cudaFree(gl.d_heads); cudaFree(gl.d_heads_left);
+    gl.d_B = nullptr; gl.d_bias = nullptr; gl.d_heads = nullptr; gl.d_heads_left = nullptr;
 }
 
 // =============================================================================== snapshotter
@@ -930,7 +954,7 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
             const bool fin = i == nl - 2;
             const int per_row = fin ? 4 : (dc->host[i].kind == GW_CONV ? 1 : 2);
             const int zl = fin ? z_left[nl - 1] : z_left[i], zr = fin ? z_right[nl - 1] : z_right[i];
-            make_incremental_variant(dc->gemm[i], (zl + per_row - 1) / per_row, (zr + per_row - 1) / per_row);
+            if (int rc = make_incremental_variant(dc->gemm[i], (zl + per_row - 1) / per_row, (zr + per_row - 1) / per_row)) return rc;
         }
     }
     CU_TRY(cudaMalloc(&dc->acc, wbytes));
