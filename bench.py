@@ -584,6 +584,31 @@ def run_native(args):
         snapshotter["what"] = ("gw_stream_update alone, eager launches of k_append on one stream, 2000 updates, CUDA events; "
                                "real time needs realtime_rate_hz updates per second")
 
+    # BASELINE.json configs[2] on its own: 256 windows x 2 detectors x 4096 samples through the stateless classifier
+    classifier = None
+    if not args.no_offline:
+        c2 = S.config_c2()
+        cp2, dp2 = synth.bbh_params(c2.seed * 100 + 50, c2.bbh_convs, c2.bbh_dense)
+        wins = torch.from_numpy(synth.bbh_windows(c2.seed, 256, c2.bbh_len)).cuda()
+        classifier = {"windows": 256, "what": "gw_bbh_score_batch (stateless), device-resident windows, CUDA events over 50 calls; "
+                                              "one_kernel = gw_options.fuse_bbh (default), three_kernels = fuse_bbh 0"}
+        for name, fuse in (("one_kernel", 1), ("three_kernels", 0)):
+            bb = gw.Bbh(None, c2.bbh_convs, cp2, dp2, c2.bbh_len, dtype, n_det=2, max_batch=256, opts=gw.Options(fuse_bbh=fuse))
+            with torch.cuda.stream(cs):
+                for _ in range(5):
+                    bb.score_batch(wins, cs)
+                c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                c0.record(cs)
+                for _ in range(50):
+                    bb.score_batch(wins, cs)
+                c1.record(cs)
+            torch.cuda.synchronize()
+            us = 1e3 * c0.elapsed_time(c1) / 50
+            classifier[name] = {"us_per_batch": round(us, 2), "windows_per_s": round(256 / (us * 1e-6)),
+                                "data_seconds_per_s": round(256 * c2.bbh_len / FS / (us * 1e-6), 1)}
+            bb.close()
+        del wins
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
@@ -615,7 +640,7 @@ def run_native(args):
             "sustained": sustained, "latency": latency, "e2e": e2e, "gpu_launches": int(launches),
             "graph_nodes": graph_nodes,
             "roofline": roofline, "smem_peak_gbs": round(smem_peak_gbs, 1), "kernels": kernels, "clocks": clocks,
-            "incremental": incremental, "largest": largest, "cpu_baseline": cpu, "offline": offline, "snapshotter": snapshotter,
+            "incremental": incremental, "largest": largest, "cpu_baseline": cpu, "offline": offline, "classifier_c2": classifier, "snapshotter": snapshotter,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

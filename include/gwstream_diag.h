@@ -22,7 +22,8 @@ extern "C" {
  *  sm_mhz[i] (host, may be NULL): the SM clock kernel i actually ran at = the kernel's length in SM cycles (clock64 of its
  *  CTA 0) over its length in ns (%globaltimer of the same CTA).  nvidia-smi samples every 25 ms at best; a kernel lasts
  *  0.01-0.2 ms and the power cap moves the clock from one kernel to the next.
- *  gw_profile_label(p, i): kernel i's name ("snapshot_append", "gemm.dc0", ... "aggregate", "bbh_conv1", "gemm.bbh1", ...).
+ *  gw_profile_label(p, i): kernel i's name ("snapshot_append", "gemm.dc0", ... "aggregate", "bbh_fused" -- or, as three
+ *  kernels, "bbh_conv1", "gemm.bbh1", "gemm.bbh2").
  *  gw_profile_flops(p, i): algorithmic FLOPs kernel i EXECUTED in that step (real channels and taps only, whole
  *  batch; with gw_options.incremental: the rows of the tiles that were recomputed); 0 for non-GEMM kernels.
  *  gw_profile_smem_bytes(p, i): shared-memory traffic of conv GEMM kernel i by the accounting of DESIGN.md section 7
@@ -46,6 +47,19 @@ int gw_probe_mma_cycles(int N, float *issue_cycles, float *complete_cycles);
  * recomputes those rows (rounded up to tiles) and keeps every other row.  tests/test_oracle_pins.py checks the numbers
  * against the oracle run on two overlapping windows. */
 int gw_incremental_zones(const gw_conv_layer *layers, int n_layers, int stride, int *left, int *right);
+
+/* Host only (no CUDA device needed): the tensor-core operand images of the one-kernel classifier (gw_options.fuse_bbh)
+ * exactly as gw_bbh_create uploads them, so that their construction can be checked without a GPU.  All three are
+ * K-major SWIZZLE_128B matrices of 16-bit storage values (rows of 64 values = 128 bytes; the 16-byte chunk c of row r sits
+ * at chunk c ^ (r & 7)):
+ *   w1 [128 rows][64]:           row = phase q * 32 + cout, k = (cin * 2 + part) * 16 + i holds tap j = i - q of
+ *                                w[cout][cin][.] (i = 0..10: input sample 4r - 3 + i of im2col row r; part 0 multiplies
+ *                                the 16-bit head of a sample, part 1 what that rounding lost) -- block 1 as a Toeplitz matrix;
+ *   w2 [4 tap pairs][64 rows][64]:  block j / 2, row = cout, k = (j & 1) * 32 + cin;
+ *   w3 [8 taps][128 rows][64]:      block j, row = cout, k = cin.
+ * Sizes in 16-bit values: 8192, 16384, 65536.  GW_EINVAL if the spec is not a shape that kernel takes (gwstream.h,
+ * gw_options.fuse_bbh). */
+int gw_bbh_fused_images(const gw_bbh_spec *spec, int dtype, uint16_t *w1, uint16_t *w2, uint16_t *w3);
 
 #ifdef __cplusplus
 }

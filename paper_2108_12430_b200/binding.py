@@ -31,7 +31,7 @@ EXPORTS = [          # include/gwstream.h
 ]
 DIAG_EXPORTS = [     # include/gwstream_diag.h (measurement and diagnostics, not the product interface)
     "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes", "gw_probe_mma_cycles",
-    "gw_incremental_zones",
+    "gw_incremental_zones", "gw_bbh_fused_images",
 ]
 
 _FP = C.POINTER(C.c_float)
@@ -103,6 +103,7 @@ def lib():
         L.gw_options_default.restype = None
         L.gw_probe_mma_cycles.argtypes = [i, C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.gw_incremental_zones.argtypes = [C.POINTER(_ConvLayer), i, i, C.POINTER(i), C.POINTER(i)]
+        L.gw_bbh_fused_images.argtypes = [C.POINTER(_BbhSpec), i, vp, vp, vp]
         L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
         L.gw_stream_destroy.argtypes = [vp]
         L.gw_stream_update.argtypes = [vp, vp, vp]
@@ -155,6 +156,19 @@ def _check(rc: int, handle=None) -> None:
 
 def kernel_launches() -> int:
     return int(lib().gw_kernel_launches())
+
+
+def bbh_fused_images(convs: Sequence[S.ConvSpec], conv_params, dense_dims: Sequence[int], length: int, dtype: int):
+    """Host only: the operand images (uint16 arrays w1 [128][64], w2 [4][64][64], w3 [8][128][64], still swizzled) of the
+    one-kernel classifier as gw_bbh_create builds them (gwstream_diag.h)."""
+    keep: list = []
+    arr = _marshal_layers(convs, conv_params, keep)
+    dims_c = (C.c_int * len(dense_dims))(*dense_dims)
+    spec = _BbhSpec(len(convs), arr, len(dense_dims) - 1, dims_c, None, None, length)
+    w1 = np.zeros((128, 64), np.uint16); w2 = np.zeros((4, 64, 64), np.uint16); w3 = np.zeros((8, 128, 64), np.uint16)
+    _check(lib().gw_bbh_fused_images(C.byref(spec), dtype, C.c_void_p(w1.ctypes.data), C.c_void_p(w2.ctypes.data),
+                                     C.c_void_p(w3.ctypes.data)))
+    return w1, w2, w3
 
 
 def incremental_zones(layer_specs: Sequence[S.ConvSpec], stride: int):

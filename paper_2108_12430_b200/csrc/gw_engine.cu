@@ -1365,10 +1365,20 @@ static void put_sw128(std::vector<uint16_t>& img, size_t block_elems, int row, i
     img[block_elems + static_cast<size_t>(row) * 64 + (((k >> 3) ^ (row & 7)) << 3) + (k & 7)] = bits;
 }
 
-// gw_options.fuse_bbh: operand images of the one-kernel classifier (layouts: BbhFusedParams in gw_common.cuh).
-static int bbh_build_fused(gw_bbh* b, const std::vector<HostLayer>& H, int hidden) {
+// gw_options.fuse_bbh: is this classifier one the one-kernel form takes (gw_bbh_fused.cu)?
+static bool bbh_fused_shape(const std::vector<HostLayer>& H, int L, int hidden) {
+    if (H.size() != 3) return false;
+    for (const HostLayer& h : H)
+        if (h.kind != GW_CONV || h.k != 8 || h.pad_l != 3 || h.stride != 1 || h.pool != 4) return false;
+    return H[0].cout <= 32 && H[1].cin <= 32 && H[1].cout <= 64 && H[2].cin <= 64 && H[2].cout == 128 &&
+           bbh_fused_supported(L, H[0].cin, hidden);
+}
+
+// Its operand images, host only (layouts: BbhFusedParams in gw_common.cuh).
+static void bbh_fused_images(const std::vector<HostLayer>& H, int fmt, std::vector<uint16_t>& w1, std::vector<uint16_t>& w2,
+                             std::vector<uint16_t>& w3) {
     const HostLayer &A = H[0], &B = H[1], &C = H[2];
-    std::vector<uint16_t> w1(kBbhW1Bytes / 2, 0), w2(kBbhW2Bytes / 2, 0), w3(kBbhW3Bytes / 2, 0);
+    w1.assign(kBbhW1Bytes / 2, 0); w2.assign(kBbhW2Bytes / 2, 0); w3.assign(kBbhW3Bytes / 2, 0);
     // block 1: row n = phase q x 32 + cout, k = (cin x 2 + part) x 16 + i; input sample i of the row (position 4r - 3 + i)
     // is tap j = i - q of output phase q; the same weights multiply the hi and the lo part of a sample
     for (int q = 0; q < 4; ++q)
@@ -1376,15 +1386,35 @@ static int bbh_build_fused(gw_bbh* b, const std::vector<HostLayer>& H, int hidde
             for (int ci = 0; ci < A.cin; ++ci)
                 for (int j = 0; j < 8; ++j)
                     for (int part = 0; part < 2; ++part)
-                        put_sw128(w1, 0, q * 32 + co, (ci * 2 + part) * 16 + j + q, to_storage_bits(A.W(co, ci, j), b->fmt));
+                        put_sw128(w1, 0, q * 32 + co, (ci * 2 + part) * 16 + j + q, to_storage_bits(A.W(co, ci, j), fmt));
     for (int j = 0; j < 8; ++j)
         for (int co = 0; co < B.cout; ++co)
             for (int ci = 0; ci < B.cin; ++ci)
-                put_sw128(w2, static_cast<size_t>(j >> 1) * 64 * 64, co, (j & 1) * 32 + ci, to_storage_bits(B.W(co, ci, j), b->fmt));
+                put_sw128(w2, static_cast<size_t>(j >> 1) * 64 * 64, co, (j & 1) * 32 + ci, to_storage_bits(B.W(co, ci, j), fmt));
     for (int j = 0; j < 8; ++j)
         for (int co = 0; co < C.cout; ++co)
             for (int ci = 0; ci < C.cin; ++ci)
-                put_sw128(w3, static_cast<size_t>(j) * 128 * 64, co, ci, to_storage_bits(C.W(co, ci, j), b->fmt));
+                put_sw128(w3, static_cast<size_t>(j) * 128 * 64, co, ci, to_storage_bits(C.W(co, ci, j), fmt));
+}
+
+extern "C" int gw_bbh_fused_images(const gw_bbh_spec* spec, int dtype, uint16_t* w1, uint16_t* w2, uint16_t* w3) {
+    if (!spec || !spec->convs || !spec->dense_dims || !w1 || !w2 || !w3) return fail(GW_EINVAL, "gw_bbh_fused_images: NULL argument");
+    if (dtype != GW_BF16 && dtype != GW_FP16) return fail(GW_EINVAL, "dtype must be GW_BF16 or GW_FP16");
+    if (spec->n_convs != 3 || spec->n_dense != 2) return fail(GW_EINVAL, "gw_bbh_fused_images: not a shape the one-kernel classifier takes");
+    std::vector<HostLayer> H(3);
+    for (int i = 0; i < 3; ++i)
+        if (int rc = fold_layer(spec->convs[i], H[i])) return rc;
+    if (!bbh_fused_shape(H, spec->length, spec->dense_dims[1])) return fail(GW_EINVAL, "gw_bbh_fused_images: not a shape the one-kernel classifier takes");
+    std::vector<uint16_t> a, b, c;
+    bbh_fused_images(H, dtype == GW_BF16 ? FMT_BF16 : FMT_FP16, a, b, c);
+    memcpy(w1, a.data(), a.size() * 2); memcpy(w2, b.data(), b.size() * 2); memcpy(w3, c.data(), c.size() * 2);
+    return GW_OK;
+}
+
+static int bbh_build_fused(gw_bbh* b, const std::vector<HostLayer>& H, int hidden) {
+    const HostLayer &A = H[0], &B = H[1], &C = H[2];
+    std::vector<uint16_t> w1, w2, w3;
+    bbh_fused_images(H, b->fmt, w1, w2, w3);
     auto up16 = [](uint8_t** dst, const std::vector<uint16_t>& v) -> cudaError_t {
         cudaError_t e = cudaMalloc(dst, v.size() * 2);
         return e != cudaSuccess ? e : cudaMemcpy(*dst, v.data(), v.size() * 2, cudaMemcpyHostToDevice);
@@ -1433,10 +1463,7 @@ static int bbh_build(gw_bbh* b, const gw_bbh_spec* spec) {
         for (int i = 0; i < nc; ++i) { b->flops += 2.0 * l * H[i].k * H[i].cin * H[i].cout; l /= 4; }
     }
     // the whole classifier as one kernel when its shape is the one that kernel is written for (BASELINE.json configs[2])
-    if (b->opt.fuse_bbh && b->opt.conv_impl == GW_IMPL_UMMA && nc == 3 && H[0].k == 8 && H[1].k == 8 && H[2].k == 8 &&
-        H[0].pad_l == 3 && H[1].pad_l == 3 && H[2].pad_l == 3 && H[0].cout <= 32 && H[1].cin <= 32 && H[1].cout <= 64 &&
-        H[2].cin <= 64 && H[2].cout == 128 && bbh_fused_supported(L, H[0].cin, hidden))
-        return bbh_build_fused(b, H, hidden);
+    if (b->opt.fuse_bbh && b->opt.conv_impl == GW_IMPL_UMMA && bbh_fused_shape(H, L, hidden)) return bbh_build_fused(b, H, hidden);
     // first block on CUDA cores (its cin * k taps live in registers)
     if (H[0].cin > 4 || H[0].k > 8 || H[0].pad_l > 4 || H[0].k - 1 - H[0].pad_l > 4)
         return fail(GW_EINVAL, "first classifier block: needs cin <= 4, k <= 8, pad_l <= 4, pad_r <= 4");

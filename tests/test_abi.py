@@ -76,3 +76,60 @@ def test_missing_library_raises(monkeypatch, tmp_path):
     monkeypatch.setattr(binding, "LIB_PATH", str(tmp_path / "nope.so"))
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         binding.lib()
+
+
+def test_fused_classifier_operand_images_hold_every_weight_where_the_kernel_reads_it():
+    """Host logic of the one-kernel classifier (no GPU): gw_bbh_fused_images returns the three tensor-core operand images
+    gw_bbh_create uploads.  Unswizzled by the rule the header states, every weight must sit -- rounded to the storage type
+    exactly as the oracle rounds it -- at the (row, k) the kernel's index arithmetic reads it from, and nothing else may be
+    non-zero: block 1 as a Toeplitz matrix over the 11 samples of an im2col row (tap j of output phase q at sample j + q,
+    once for the head and once for the tail of a sample), blocks 2 and 3 as [tap][cout][cin]."""
+    import numpy as np
+    import oracle
+    from paper_2108_12430_b200 import specs as S
+    from paper_2108_12430_b200 import synth
+
+    def unswizzle(img):                                   # [..., rows, 64] -> the logical K order
+        out = np.empty_like(img)
+        rows = img.shape[-2]
+        for r in range(rows):
+            for c in range(8):
+                out[..., r, 8 * c:8 * c + 8] = img[..., r, 8 * (c ^ (r & 7)):8 * (c ^ (r & 7)) + 8]
+        return out
+
+    def to_float(bits, dtype):
+        if dtype == binding.GW_FP16:
+            return bits.view(np.float16).astype(np.float64)
+        return (bits.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+    for dtype, od in ((binding.GW_FP16, oracle.DT_FP16), (binding.GW_BF16, oracle.DT_BF16)):
+        for n_det, widths in ((2, (2, 32, 64, 128)), (1, (1, 24, 48, 128))):
+            convs = S.bbh_layers(widths)
+            cp, _ = synth.bbh_params(9, convs, (128, 64, 1))
+            w1, w2, w3 = binding.bbh_fused_images(convs, cp, (128, 64, 1), 2048, dtype)
+            w1, w2, w3 = (to_float(unswizzle(w), dtype) for w in (w1, w2, w3))
+            wq = [oracle.round_storage(p["w"], od) for p in cp]              # [cout][cin][8] on the storage grid
+            e1 = np.zeros((128, 64))
+            for q in range(4):
+                for part in range(2):
+                    for ci in range(widths[0]):
+                        for j in range(8):
+                            e1[q * 32:q * 32 + widths[1], (ci * 2 + part) * 16 + j + q] = wq[0][:, ci, j]
+            assert np.array_equal(w1, e1)
+            e2 = np.zeros((4, 64, 64))
+            for j in range(8):
+                e2[j // 2, :widths[2], (j % 2) * 32:(j % 2) * 32 + widths[1]] = wq[1][:, :, j]
+            assert np.array_equal(w2, e2)
+            e3 = np.zeros((8, 128, 64))
+            for j in range(8):
+                e3[j, :, :widths[2]] = wq[2][:, :, j]
+            assert np.array_equal(w3, e3)
+    # shapes that kernel does not take are refused, not mangled
+    convs = S.bbh_layers((2, 32, 64, 96))
+    cp, _ = synth.bbh_params(9, convs, (96, 64, 1))
+    with pytest.raises(binding.GwError):
+        binding.bbh_fused_images(convs, cp, (96, 64, 1), 2048, binding.GW_FP16)
+    convs = S.bbh_layers((2, 32, 64, 128))
+    cp, _ = synth.bbh_params(9, convs, (128, 64, 1))
+    with pytest.raises(binding.GwError):
+        binding.bbh_fused_images(convs, cp, (128, 64, 1), 1000, binding.GW_FP16)   # window not a multiple of 512
