@@ -4,7 +4,7 @@
 // but the 32 KiB input window, the weights (L2-resident constants) and one score per window touches global memory.
 //
 // All three conv blocks run on the tensor cores (tcgen05.mma, accumulators in TMEM):
-//   block 1 (cin <= 2 -> 32, M = 4 conv positions per row)   A = an im2col tile built by four warps: row r holds the 11
+//   block 1 (cin <= 2 -> 32, M = 4 conv positions per row)   A = an im2col tile built by the worker warps: row r holds the 11
 //            input samples [4r-3, 4r+7] of each channel as a (hi, lo) pair of 16-bit values (x = hi + lo to ~2^-22, so the
 //            fp32 input is NOT rounded to the storage type: D8's numerics are kept), pre-scaled by a power of two that
 //            brings the window into fp16 range; B = the 8-tap filter as a Toeplitz matrix with N = 4 phases x 32 channels.
@@ -17,7 +17,9 @@
 //            row-shifted per tap (N = 256 positions), so a thread owns one output channel and all positions: max-pool,
 //            ReLU and the global average pool are column arithmetic in registers.
 // then the dense head and the sigmoid (fp32, CUDA cores).  Roles: warp 0 loads weights (bulk copies) and issues every MMA;
-// warps 1-4 build the im2col tiles, warps 5-8 drain block 1's accumulators; all eight drain blocks 2 and 3.
+// the eight worker warps stage the window, build block 1's im2col tiles and drain its accumulators one tile apart, then
+// drain blocks 2 and 3.  The MMAs of block 2's first tile are issued between block 1's last tiles (the tensor pipe idles
+// through most of block 1).
 // Shared memory is time-shared: [act1 | later taps 4-7 of block 3's weights] [im2col x 2 | later act2] [W2]
 // [W1 + input staging | later taps 0-3 of block 3's weights].
 #include <stdio.h>
