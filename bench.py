@@ -520,6 +520,11 @@ def run_native(args):
                        "frac_sustained": gemm_fl * 4 / (ms_l / n_l * 1e-3) / 1e12 / pk["tensor_tflops"],
                        "frac_nominal": gemm_fl * 4 / (ms_l / n_l * 1e-3) / 1e12 / NOMINAL_TFLOPS,
                        "what": "full recompute, whole step time (all kernels) against the conv FLOPs of 4 x the n=128 step"}
+            # the bandwidth kernels at the size where they are no longer launch-latency-scale (north_star: achieved HBM GB/s
+            # of the snapshot and overlap-add kernels): per-kernel stamps of the same step
+            order_l, acc_l = le.profile(reps=4, prewarm_s=0.3, ms_per_step=ms_l / n_l)
+            kern_l, _ = kernel_table(le, order_l, acc_l, pk, (c4 or {}).get("sm_mhz") or 1700.0, sms)
+            largest["bandwidth_kernels"] = {k: v for k, v in kern_l.items() if "gbs" in v}
             le.close()
             del le
         except Exception as ex:                      # e.g. a smaller box: report, do not fail the bench line

@@ -307,32 +307,97 @@ __global__ void __launch_bounds__(256) k_snapshot_append(float* __restrict__ rin
                                                          int channels, int n_det, int n_wit, int W, int S, int cpad,
                                                          int fmt, unsigned long long* stamp) {
     __shared__ float tile[32][kGatherPos + 1];
+    __shared__ long long cnt_s;
     stamp_begin(stamp);
     griddep_launch_dependents();
-    const long long cnt = *count;
+    // The counter is advanced by whichever block is the LAST TO HAVE READ IT (a ticket taken right after the read), not
+    // the last to finish: nothing in this launch reads the new value, and consumers run after the grid has completed.
+    // (Taking the ticket after the block's stores needed a __threadfence per block: every block then idled until its
+    // stores had drained, holding its slot.)
+    if (threadIdx.x == 0) {
+        const long long c = *reinterpret_cast<volatile long long*>(count);
+        cnt_s = c;
+        __threadfence();                                   // the read is performed before the ticket is taken
+        const unsigned t = atomicAdd(ticket, 1u);
+        if (t == gridDim.x * gridDim.y - 1) {
+            *count = c + S;
+            *ticket = 0;
+        }
+    }
+    __syncthreads();
+    const long long cnt = cnt_s;
     const int h0 = static_cast<int>(cnt % W);              // ring slot of this update's first sample
     const int sd = blockIdx.y;
     const int s = sd / n_det, d = sd % n_det;
     const int i0 = blockIdx.x * kGatherPos;
     const int tid = threadIdx.x;
-    // fp32 ring rows owned by this block: 32 float4 per row and tile
-    {
-        const int n_mine = (channels - d + n_det - 1) / n_det;
-        for (int idx = tid; idx < n_mine * 32; idx += 256) {
-            const int row = s * channels + d + (idx >> 5) * n_det;
-            const int i = i0 + (idx & 31) * 4;
-            if (i < S) {
-                int slot = h0 + i;
-                if (slot >= W) slot -= W;
-                *reinterpret_cast<float4*>(ring + static_cast<size_t>(row) * W + slot) =
-                    __ldg(reinterpret_cast<const float4*>(src + static_cast<size_t>(row) * S + i));
+    // Every global load of the block is requested before the first store (a block moves ~75 KB through a handful of
+    // dependent phases; with one 4- or 16-byte load in flight per thread it sat at 0.42-0.54 of the HBM rate at n = 512):
+    // (1) the fp32 ring rows owned by this block, 32 float4 per row and tile: up to three per thread;
+    // (2) this detector's witness samples, one float4 of four positions per (channel, thread): channel = warp + 8 j.
+    constexpr int kRingMax = 3;                            // float4 per thread: covers 24 owned rows (channels <= 24 n_det)
+    const int n_mine = (channels - d + n_det - 1) / n_det;
+    float4 rv[kRingMax];
+#pragma unroll
+    for (int e = 0; e < kRingMax; ++e) {
+        const int idx = tid + e * 256;
+        const int row = s * channels + d + (idx >> 5) * n_det;
+        const int i = i0 + (idx & 31) * 4;
+        rv[e] = (idx < n_mine * 32 && i < S) ? __ldg(reinterpret_cast<const float4*>(src + static_cast<size_t>(row) * S + i))
+                                             : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    const int wq = tid >> 5, f4 = tid & 31;                // warp, float4 index inside the 128-position tile
+    const bool wide = cpad == 32 && n_mine <= kRingMax * 8;
+    float4 wv[4];
+    if (wide) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int c = wq + 8 * j;
+            const int i = i0 + 4 * f4;
+            wv[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (c < n_wit && i < S) {
+                const int row = s * channels + __ldg(rows_map + d * n_wit + c);
+                wv[j] = __ldg(reinterpret_cast<const float4*>(src + static_cast<size_t>(row) * S + i));
             }
+        }
+    }
+    for (int idx = tid + kRingMax * 256; idx < n_mine * 32; idx += 256) {      // more than 24 owned rows: the rest, plainly
+        const int row = s * channels + d + (idx >> 5) * n_det;
+        const int i = i0 + (idx & 31) * 4;
+        if (i < S) {
+            int slot = h0 + i;
+            if (slot >= W) slot -= W;
+            *reinterpret_cast<float4*>(ring + static_cast<size_t>(row) * W + slot) =
+                __ldg(reinterpret_cast<const float4*>(src + static_cast<size_t>(row) * S + i));
+        }
+    }
+#pragma unroll
+    for (int e = 0; e < kRingMax; ++e) {
+        const int idx = tid + e * 256;
+        const int row = s * channels + d + (idx >> 5) * n_det;
+        const int i = i0 + (idx & 31) * 4;
+        if (idx < n_mine * 32 && i < S) {
+            int slot = h0 + i;
+            if (slot >= W) slot -= W;
+            *reinterpret_cast<float4*>(ring + static_cast<size_t>(row) * W + slot) = rv[e];
         }
     }
     // 16-bit mirror ring, 32 channels at a time through the transpose tile
     for (int cb = 0; cb < cpad; cb += 32) {
         __syncthreads();
-        {
+        if (wide) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int c = wq + 8 * j;
+                float2 ms = make_float2(0.f, 1.f);
+                if (c < n_wit) ms = __ldg(reinterpret_cast<const float2*>(pre) + d * n_wit + c);   // (mean, 1/std)
+                const bool live = c < n_wit && i0 + 4 * f4 < S;
+                tile[c][4 * f4 + 0] = live ? (wv[j].x - ms.x) * ms.y : 0.f;
+                tile[c][4 * f4 + 1] = live ? (wv[j].y - ms.x) * ms.y : 0.f;
+                tile[c][4 * f4 + 2] = live ? (wv[j].z - ms.x) * ms.y : 0.f;
+                tile[c][4 * f4 + 3] = live ? (wv[j].w - ms.x) * ms.y : 0.f;
+            }
+        } else {
             const int pos = tid % kGatherPos;
             const int cg = tid / kGatherPos;
             const int i = i0 + pos;
@@ -368,16 +433,7 @@ __global__ void __launch_bounds__(256) k_snapshot_append(float* __restrict__ rin
             }
         }
     }
-    __threadfence();
     __syncthreads();
-    if (tid == 0) {
-        const unsigned t = atomicAdd(ticket, 1u);
-        if (t == gridDim.x * gridDim.y - 1) {
-            *count = cnt + S;
-            *ticket = 0;
-            __threadfence();
-        }
-    }
     stamp_end(stamp);
 }
 
