@@ -314,8 +314,11 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             int ib = 0;
             int rs0 = 0, rs1 = 0; uint32_t rp0 = 0, rp1 = 0;                 // position and phase in each sub-ring
             TR_DECL
-            // mirror-ring source: the window starts at ring row (count mod W) / div (see ConvGemmParams)
-            const int row_off = p.a_count ? static_cast<int>((*p.a_count % p.a_ring_W) / p.a_ring_div) : 0;
+            // mirror-ring source: the window starts at ring row (count mod W) / div (see ConvGemmParams); with a tensor map
+            // per window head the map itself is based there (and rows outside the window are zero fill)
+            const int ring_h0 = p.a_count ? static_cast<int>(*p.a_count % p.a_ring_W) : 0;
+            const CUtensorMap* tmA = p.tmA_heads ? p.tmA_heads + ring_h0 / p.head_div : &p.tmA;
+            const int row_off = (p.a_count && !p.tmA_heads) ? ring_h0 / p.a_ring_div : 0;
             for (int w = worker; w < total; w += n_workers) {
                 const int u = p.reverse ? total - 1 - w : w;
                 const int batch = (u / spi) * p.n_det + det;
@@ -329,7 +332,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                         TR_WAIT(0, mbar_wait(&a_empty[stage], (second ? rp1 : rp0) ^ 1))
                         mbar_arrive_expect_tx(&a_full[stage], p.slab_rows * 128);
                         if (p.a_4d) tma_load_4d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min, det, u / spi);
-                        else tma_load_3d(smem_a + stage * sl, &p.tmA, &a_full[stage], cb * kSegK, m0 + p.a_min + row_off, batch);
+                        else tma_load_3d(smem_a + stage * sl, tmA, &a_full[stage], cb * kSegK, m0 + p.a_min + row_off, batch);
                         if (second) { if (++rs1 == sa - ring0) { rs1 = 0; rp1 ^= 1; } }
                         else if (++rs0 == ring0) { rs0 = 0; rp0 ^= 1; }
                         if (!p.b_resident) {
@@ -361,7 +364,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         if (p.b_resident) mbar_wait(bres_bar, 0);
         const uint32_t smem_a_u32 = smem_u32(smem_a), smem_b_u32 = smem_u32(smem_b);
         const bool resident = p.b_resident != 0;
-        const bool ring = p.a_count != nullptr;
+        const bool ring = p.a_count != nullptr && p.tmA_heads == nullptr;   // window-edge rows must be cleared by hand
         const int n_cb = p.n_cb, n_shift = p.n_shift;
         const uint32_t b_step = static_cast<uint32_t>(b_block) >> 4;       // descriptor units per B K-block
         const uint32_t idesc_half = umma_idesc_f16(FMT, kTileM, p.N / 2);

@@ -551,8 +551,11 @@ static int build_gemm_layer(GemmLayer& gl, GemmKind gk, const HostLayer* dets, i
         const uint64_t out_rows = out_ring ? 2 * static_cast<uint64_t>(p.M) : p.M;
         if (int rc = make_tmap(&p.tmOut, out, fmt, p.N, out_rows, batch, p.N, out_rows * p.N, 32, p.N >= 64 ? 64 : 32)) return rc;
     }
-    if (out_ring && p.N == 256 && opt.two_sm && ring_S > 0 && ring_W % ring_S == 0) {
-        // CTA-pair kernel on a ring input: a tensor map per window head (see ConvGemmParams::tmA_heads)
+    if (ring_count && ring_S > 0 && ring_W % ring_S == 0 && ring_S % p.a_ring_div == 0 && seg_T == 0) {
+        // ring input: a tensor map per window head (see ConvGemmParams::tmA_heads), so that rows outside the window are
+        // TMA's zero fill.  The CTA-pair kernel needs them; the one-CTA kernel would otherwise clear those rows in shared
+        // memory from its MMA warp, with a proxy fence per column block in front of the MMAs -- every tile of a zone launch
+        // lies on a window edge and paid it (GW_TRACE at n = 512: 12.7 k cycles per tile in the MMA warp against 2.4 k)
         const int n_heads = ring_W / ring_S;
         std::vector<CUtensorMap> heads(n_heads);
         for (int h = 0; h < n_heads; ++h) {
