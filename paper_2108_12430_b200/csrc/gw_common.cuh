@@ -72,6 +72,10 @@ struct ConvGemmParams {
     // receptive field reaches the LEFT window edge) and the rest are the LAST v_tiles - v_left tiles (rows that see the
     // new samples or the right window edge).  Full recomputation: v_tiles = v_left = tiles_m.
     int v_tiles, v_left;
+    // Zone launches, EPI_STORE: the recomputed rows are the first z_left and the last z_right rows of the layer; an epilogue
+    // warp whose 32-row quadrant of a tile holds none of them skips it (the ring keeps those rows' values, which ARE the
+    // values the tile would store again).  0 / 0: every row is live.
+    int z_left, z_right;
     int pred_ring;                 // EPI_FINAL: pred is a ring over absolute sample index mod 4 M (no mirror: row stores)
     // CTA-pair kernel on a ring input: one tensor map PER WINDOW HEAD (device array of a_ring_W / head_div maps, the
     // map of head h based at the ring row where that window starts and a_rows rows tall), so that rows outside the

@@ -535,6 +535,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 }
             }
         };
+        // zone launches (EPI_STORE): rows [r0, r0 + 32) of the layer hold a recomputed row iff they reach into the first
+        // z_left or the last z_right rows
+        auto quad_live = [&](int vt) -> bool {
+            if ((p.z_left | p.z_right) == 0) return true;
+            const int r0 = map_tile(p, vt) * kTileM + quad * 32;
+            return r0 < p.z_left || r0 + 32 > p.M - p.z_right;
+        };
         const float fin_bias = EPI == EPI_FINAL ? __ldg(p.fin_b + det) : 0.f;
         int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL: the tile whose second chain is in flight
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;   // + 32 KiB for the second buffer
@@ -558,6 +565,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 const bool wide = p.N >= 64;
                 for (int cp = 0; cp < 2; ++cp) {
                     const int ca = 4 * cp + 2 * hsel, cbk = ca + 1;              // chunk indices
+                    // zone launches: does this warp's quadrant of the chunk's tile hold a recomputed row at all?
+                    const int vta = (u % spi) * G + ch_g[2 * cp], vtb = (u % spi) * G + ch_g[2 * cp + 1];
+                    const bool la = ch_g[2 * cp] < G && vta < p.v_tiles && quad_live(vta);
+                    const bool lb = wide ? la : (ch_g[2 * cp + 1] < G && vtb < p.v_tiles && quad_live(vtb));
+                    if (!la && !lb) {
+                        if (cp == 1) {                         // nothing read from this stage by this warp: hand it back
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(&tmem_empty[acc]);
+                        }
+                        continue;
+                    }
                     uint32_t ra[32], rb[32];
                     tmem_ld_32x32(taddr + 32 * ca, ra);
                     tmem_ld_32x32(taddr + 32 * cbk, rb);
@@ -600,16 +619,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     {
                         const int row0 = quad * 32;
                         if (wide) {                            // both chunks: one tile, 64 adjacent columns
-                            const int vt = (u % spi) * G + ch_g[2 * cp];
-                            if (ch_g[2 * cp] < G && vt < p.v_tiles)
-                                store_box(stg, ch_col[2 * cp], map_tile(p, vt) * kTileM + row0, batch, 128);
+                            if (la) store_box(stg, ch_col[2 * cp], map_tile(p, vta) * kTileM + row0, batch, 128);
                         } else {                               // N = 32: the chunks are two consecutive tiles
-#pragma unroll
-                            for (int which = 0; which < 2; ++which) {
-                                const int vt = (u % spi) * G + ch_g[2 * cp + which];
-                                if (ch_g[2 * cp + which] < G && vt < p.v_tiles)
-                                    store_box(stg + which * 2048, 0, map_tile(p, vt) * kTileM + row0, batch, 64);
-                            }
+                            if (la) store_box(stg, 0, map_tile(p, vta) * kTileM + row0, batch, 64);
+                            if (lb) store_box(stg + 2048, 0, map_tile(p, vtb) * kTileM + row0, batch, 64);
                         }
                         if (lane == 0) tma_store_commit();
                     }
