@@ -83,12 +83,15 @@ struct ConvGemmParams {
     // pair kernel (the peer's slab is consumed by the leader's MMAs) has no warp in the right place for.
     const CUtensorMap* tmA_heads;
     int head_div;                  // head index = (*a_count mod a_ring_W) / head_div  (= the stride S)
-    // CTA-pair kernel, zones packed into ONE tile per batch item (k_conv_gemm_2sm): the left zone's pk_left output rows
-    // are tile rows [0, pk_left) and read slab rows [0, pk_nl) (loaded through tmA_heads_left: the same per-head maps
-    // with a box of pk_nl rows, pk_nl = pk_left + n_shift - 1 rounded up to 8); the right zone's pk_right rows are tile
-    // rows [pk_nl, pk_nl + pk_right) and read slab rows from pk_nl on.  pk_nl = 0: not packed.
+    // CTA-pair kernel, zones packed (k_conv_gemm_2sm): a tile holds pk_k consecutive batch items, one segment of
+    // pk_nl + pk_nr rows each.  Inside a segment the left zone's pk_left output rows are rows [0, pk_left) and read slab
+    // rows [0, pk_nl) (loaded through tmA_heads_left: the per-head maps with a box of pk_nl rows, pk_nl = pk_left +
+    // n_shift - 1 rounded up to 8); the right zone's pk_right rows are rows [pk_nl, pk_nl + pk_right) and read the
+    // pk_nr slab rows from pk_nl on (tmA_heads_right: box of pk_nr = pk_right + n_shift - 1 rounded up to 8 rows).
+    // pk_k (pk_nl + pk_nr) <= 128.  pk_nl = 0: not packed.
     const CUtensorMap* tmA_heads_left;
-    int pk_nl, pk_left, pk_right;
+    const CUtensorMap* tmA_heads_right;
+    int pk_nl, pk_nr, pk_k, pk_left, pk_right;
     unsigned long long* stamp;     // profiling graph: [0] = min %globaltimer at CTA start, [1] = max at CTA end; else null
     // EPI_FINAL: this layer (ConvTranspose1d -> 32 channels, tanh) and the network's last layer
     // (ConvTranspose1d 32 -> 1, k = 7, stride 2, pad 3, output_padding 1, linear) in one kernel.  The

@@ -69,7 +69,8 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
         const int pairs = sm_count / 2;
         // ring input (incremental path): needs the per-head tensor maps; the pair works on virtual tiles 2u, 2u + 1
         bool ok = p.epi == EPI_STORE && p.N == 256 && (p.a_count == nullptr || p.tmA_heads != nullptr) &&
-                  (p.pk_nl ? (g.batch / p.n_det) % 2 == 0 && p.tmA_heads_left != nullptr : p.v_tiles % 2 == 0) && pairs >= p.n_det;
+                  (p.pk_nl ? (g.batch / p.n_det) % (2 * p.pk_k) == 0 && p.tmA_heads_left != nullptr && p.tmA_heads_right != nullptr
+                           : p.v_tiles % 2 == 0) && pairs >= p.n_det;
         for (int ob = 2; ok && ob >= 1; --ob) {
             const int fixed = kFixedSmem + ob * kOutStage;
             const int sa = p.n_cb < 2 ? 2 : (p.n_cb > 8 ? 8 : p.n_cb);
@@ -843,10 +844,11 @@ template <int ACT, int FMT>
 __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid_constant__ ConvGemmParams p, int n_items) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    // Packed zones (incremental path, p.pk_nl > 0): ONE tile per batch item holds both recomputed zones -- slab rows
-    // [0, pk_nl) are the input rows of the left zone (outputs 0 .. pk_left-1), slab rows [pk_nl, pk_nl + slab_rows) those of
-    // the right zone (tile rows pk_nl .. pk_nl + pk_right - 1 = the layer's LAST pk_right rows); the tile rows in between
-    // mix the two and are dropped.  The two CTAs of a pair then work on two consecutive batch items.
+    // Packed zones (incremental path, p.pk_nl > 0): a tile holds both recomputed zones of pk_k consecutive batch items, one
+    // segment of pk_seg = pk_nl + pk_nr rows each -- slab rows [0, pk_nl) of a segment are the input rows of the left zone
+    // (outputs 0 .. pk_left-1), the next pk_nr rows those of the right zone (tile rows pk_nl .. pk_nl + pk_right - 1 of the
+    // segment = the layer's LAST pk_right rows); the tile rows in between mix neighbours and are dropped.  The two CTAs
+    // of a pair then work on 2 pk_k consecutive batch items.
     const bool packed = p.pk_nl > 0;
     const int sl = slab_bytes_of(p.slab_rows + p.pk_nl);
     const int sa = p.sa_stages, sb = p.sb_stages;
@@ -873,7 +875,8 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
     const int cworker = cid / p.n_det;
     const int n_cw = (gridDim.x / 2) / p.n_det;
     const int half_tiles = packed ? 1 : p.v_tiles / 2;                       // (virtual) tile pairs per batch item
-    const int total = packed ? n_items / 2 : n_items * half_tiles;           // packed: one pair = two batch items
+    const int pk_seg = p.pk_nl + p.pk_nr;
+    const int total = packed ? n_items / (2 * p.pk_k) : n_items * half_tiles; // packed: one pair = 2 pk_k batch items
 
     if (warp == 0) {
         if (lane == 0) {
@@ -908,6 +911,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
         const int head = p.tmA_heads ? static_cast<int>(*p.a_count % p.a_ring_W) / p.head_div : 0;
         const CUtensorMap* tmA = p.tmA_heads ? p.tmA_heads + head : &p.tmA;
         const CUtensorMap* tmA_left = packed ? p.tmA_heads_left + head : nullptr;   // box of pk_nl rows
+        const CUtensorMap* tmA_right = packed ? p.tmA_heads_right + head : nullptr; // box of pk_nr rows
         const uint32_t lead_a_full = mapa_u32(smem_u32(a_full), 0), lead_b_full = mapa_u32(smem_u32(b_full), 0);
         unsigned long long cbstart = 0;
         {
@@ -931,11 +935,14 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
             if (lane == 0) {
                 const int u = p.reverse ? total - 1 - aw : aw;
                 if (packed) {
-                    const int batch = (2 * u + static_cast<int>(rank)) * p.n_det + det;
-                    if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * (p.slab_rows + p.pk_nl) * 128);
-                    tma_load_3d_2sm(smem_a + stage * sl, tmA_left, lead_a_full + 8u * stage, acb * kSegK, p.a_min, batch);
-                    tma_load_3d_2sm(smem_a + stage * sl + p.pk_nl * 128, tmA, lead_a_full + 8u * stage, acb * kSegK,
-                                    p.M - p.pk_right + p.a_min, batch);
+                    if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.pk_k * pk_seg * 128);
+                    for (int w = 0; w < p.pk_k; ++w) {
+                        const int batch = ((2 * u + static_cast<int>(rank)) * p.pk_k + w) * p.n_det + det;
+                        uint8_t* seg = smem_a + stage * sl + w * pk_seg * 128;
+                        tma_load_3d_2sm(seg, tmA_left, lead_a_full + 8u * stage, acb * kSegK, p.a_min, batch);
+                        tma_load_3d_2sm(seg + p.pk_nl * 128, tmA_right, lead_a_full + 8u * stage, acb * kSegK,
+                                        p.M - p.pk_right + p.a_min, batch);
+                    }
                 } else {
                     const int m0 = map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank)) * kTileM;
                     if (rank == 0) mbar_arrive_expect_tx(&a_full[stage], 2 * p.slab_rows * 128);
@@ -1028,7 +1035,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
         for (int w = cworker; w < total; w += n_cw, ++it) {
             const int u = p.reverse ? total - 1 - w : w;
             const int acc = it & 1;
-            const int batch = packed ? (2 * u + static_cast<int>(rank)) * p.n_det + det : (u / half_tiles) * p.n_det + det;
+            const int batch = packed ? 0 : (u / half_tiles) * p.n_det + det;      // packed: per segment, below
             const int mt = packed ? 0 : map_tile(p, (u % half_tiles) * 2 + static_cast<int>(rank));
             TR_WAIT(0, mbar_wait(&tmem_full[acc], (it >> 1) & 1))
             tc_fence_after();
@@ -1037,10 +1044,13 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
                 // this lane's tile row: a row of the left zone, of the right zone, or one of the mixed rows in between;
                 // the few live rows go straight from registers to their ring row and its twin (r +- M)
                 const int i = quad * 32 + lane;
-                const int lrow = i < p.pk_left ? i : (i >= p.pk_nl && i < p.pk_nl + p.pk_right) ? p.M - p.pk_right + i - p.pk_nl : -1;
+                const int w = i / pk_seg, j = i - w * pk_seg;       // segment (batch item of this CTA) and row inside it
+                const int lrow = w >= p.pk_k ? -1 : j < p.pk_left ? j
+                               : (j >= p.pk_nl && j < p.pk_nl + p.pk_right) ? p.M - p.pk_right + j - p.pk_nl : -1;
+                const int pbatch = ((2 * u + static_cast<int>(rank)) * p.pk_k + w) * p.n_det + det;
                 const int r = out_off + lrow, r2 = r >= p.M ? r - p.M : r + p.M;
-                uint8_t* row1 = reinterpret_cast<uint8_t*>(p.out) + (static_cast<size_t>(batch) * 2 * p.M + r) * 512;
-                uint8_t* row2 = reinterpret_cast<uint8_t*>(p.out) + (static_cast<size_t>(batch) * 2 * p.M + r2) * 512;
+                uint8_t* row1 = reinterpret_cast<uint8_t*>(p.out) + (static_cast<size_t>(pbatch) * 2 * p.M + r) * 512;
+                uint8_t* row2 = reinterpret_cast<uint8_t*>(p.out) + (static_cast<size_t>(pbatch) * 2 * p.M + r2) * 512;
                 for (int cp = 0; cp < 2; ++cp) {
                     const int col = 32 * (4 * cp + 2 * hsel);
                     uint32_t ra[32], rb[32];
@@ -1280,7 +1290,7 @@ cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     cudaError_t e;
     if (g.p.two_sm) {
         int cw = g.grid / 2 / g.p.n_det;                         // clusters per detector
-        const int units = g.p.pk_nl ? n_items / 2 : n_items * (g.p.v_tiles / 2);
+        const int units = g.p.pk_nl ? n_items / (2 * g.p.pk_k) : n_items * (g.p.v_tiles / 2);
         if (cw > units) cw = units;
         cudaLaunchConfig_t cfg2 = {};
         cfg2.gridDim = dim3(2 * cw * g.p.n_det);

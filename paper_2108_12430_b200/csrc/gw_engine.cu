@@ -272,6 +272,7 @@ struct GemmLayer {
     float* d_bias = nullptr;
     CUtensorMap* d_heads = nullptr;              // incremental path, CTA-pair layers: one input tensor map per window head
     CUtensorMap* d_heads_left = nullptr;         // the same with a box of pk_nl rows (zones packed into one tile)
+    CUtensorMap* d_heads_right = nullptr;        // ... and of pk_nr rows
     int impl = GW_IMPL_UMMA;
     std::string name;                            // profiler label, e.g. "gemm.dc3"
     double flops = 0.0;                          // algorithmic FLOPs per batch item, whole window (real channels and taps only)
@@ -599,21 +600,29 @@ static int make_incremental_variant(GemmLayer& gl, int left_rows, int right_rows
     // CTA-pair layers (ring input through per-head tensor maps): both zones in ONE tile per batch item when they fit, the
     // pair working on two batch items -- half the tiles (and half the streamed weights) of a tile per zone
     if (p.two_sm && p.tmA_heads && (gl.g.batch / p.n_det) % 2 == 0) {
-        const int nl = round_up(left_rows + p.n_shift - 1, 8);
-        if (nl + right_rows <= kTileM && left_rows + right_rows < p.M) {
+        const int nl = round_up(left_rows + p.n_shift - 1, 8), nr = round_up(right_rows + p.n_shift - 1, 8);
+        if (nl + nr <= kTileM && left_rows + right_rows < p.M) {
+            // as many batch items per tile as fit (and as divide the batch): 2 at S = 512, 4 at S = 256
+            int k = kTileM / (nl + nr);
+            while (k > 1 && (gl.g.batch / p.n_det) % (2 * k)) --k;
             const int n_heads = p.a_ring_W / p.head_div;
-            std::vector<CUtensorMap> heads(n_heads);
+            std::vector<CUtensorMap> heads(n_heads), heads_r(n_heads);
             for (int h = 0; h < n_heads; ++h) {
                 const size_t off_rows = static_cast<size_t>(h) * p.head_div / p.a_ring_div;
                 const uint16_t* base = static_cast<const uint16_t*>(p.A) + off_rows * p.a_cols;
                 if (int rc = make_tmap(&heads[h], base, p.fmt, p.a_cols, p.a_rows, gl.g.batch, p.a_cols,
                                        static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, nl)) return rc;
+                if (int rc = make_tmap(&heads_r[h], base, p.fmt, p.a_cols, p.a_rows, gl.g.batch, p.a_cols,
+                                       static_cast<uint64_t>(p.a_rows_tm) * p.a_cols, nr)) return rc;
             }
             CU_TRY(cudaMalloc(&gl.d_heads_left, sizeof(CUtensorMap) * n_heads));
             CU_TRY(cudaMemcpy(gl.d_heads_left, heads.data(), sizeof(CUtensorMap) * n_heads, cudaMemcpyHostToDevice));
+            CU_TRY(cudaMalloc(&gl.d_heads_right, sizeof(CUtensorMap) * n_heads));
+            CU_TRY(cudaMemcpy(gl.d_heads_right, heads_r.data(), sizeof(CUtensorMap) * n_heads, cudaMemcpyHostToDevice));
             p.tmA_heads_left = gl.d_heads_left;
-            p.pk_nl = nl; p.pk_left = left_rows; p.pk_right = right_rows;
-            p.v_left = 0; p.v_tiles = 1;                // one (packed) tile per batch item
+            p.tmA_heads_right = gl.d_heads_right;
+            p.pk_nl = nl; p.pk_nr = nr; p.pk_k = k; p.pk_left = left_rows; p.pk_right = right_rows;
+            p.v_left = 0; p.v_tiles = 1;                // one (packed) tile per pk_k batch items
             if (conv_gemm_plan(gl.gi, sms) && gl.gi.p.two_sm) { gl.has_inc = true; return GW_OK; }
             gl.gi = gl.g;                               // does not fit: the unpacked work list below
         }
@@ -675,7 +684,7 @@ static double gemm_smem_bytes(const GemmLaunch& g, int batch) {
     double epi = 0.0;
     if (p.epi == EPI_STORE) epi = 2.0 * 128.0 * p.N * 2.0;                            // staged once, read once by the TMA store
     if (p.epi == EPI_FINAL) { epi = 128.0 * 128.0; mma += 10.0 * (4096.0 + 32.0 * 16); }   // activated tile + second chain
-    return (mma + fill + epi) * static_cast<double>(p.v_tiles) * n_items * p.n_det;
+    return (mma + fill + epi) * static_cast<double>(p.v_tiles) * n_items * p.n_det / (p.pk_k > 1 ? p.pk_k : 1);
 }
 
 static void run_gemm(const GemmLayer& gl, LaunchCtx& cx, bool inc = false, int batch_override = 0) {
@@ -683,14 +692,15 @@ static void run_gemm(const GemmLayer& gl, LaunchCtx& cx, bool inc = false, int b
     if (batch_override) g.batch = batch_override;
     // algorithmic FLOPs this launch executes: the rows of its tiles (all of them, or the recomputed zones)
     const double rows = static_cast<double>(g.p.v_tiles) * g.p.tile_stride;
-    const double frac = rows >= g.p.M ? 1.0 : rows / g.p.M;
+    double frac = rows >= g.p.M ? 1.0 : rows / g.p.M;
+    if (g.p.pk_k > 1) frac /= g.p.pk_k;                 // packed zones: one tile per pk_k batch items
     g.p.stamp = cx.next(gl.name, gl.flops * g.batch * frac, gemm_smem_bytes(g, g.batch));
     cx.check(gl.impl == GW_IMPL_UMMA ? launch_conv_gemm_umma(g, cx.st) : launch_conv_gemm_simt(g, cx.st));
 }
 
 static void free_gemm(GemmLayer& gl) {
-    cudaFree(gl.d_B); cudaFree(gl.d_bias); cudaFree(gl.d_heads); cudaFree(gl.d_heads_left);
-    gl.d_B = nullptr; gl.d_bias = nullptr; gl.d_heads = nullptr; gl.d_heads_left = nullptr;
+    cudaFree(gl.d_B); cudaFree(gl.d_bias); cudaFree(gl.d_heads); cudaFree(gl.d_heads_left); cudaFree(gl.d_heads_right);
+    gl.d_B = nullptr; gl.d_bias = nullptr; gl.d_heads = nullptr; gl.d_heads_left = nullptr; gl.d_heads_right = nullptr;
 }
 
 // =============================================================================== snapshotter

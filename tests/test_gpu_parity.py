@@ -386,15 +386,15 @@ def test_whitened_batch_classifier_and_filter_argument_checks():
 # ------------------------------------------------ D13 incremental path (gw_options.incremental)
 @pytest.mark.parametrize("W,S_,n,dtype", [(2048, 256, 3, gw.GW_FP16), (8192, 512, 2, gw.GW_BF16), (32768, 512, 2, gw.GW_FP16),
                                           (4096, 16, 1, gw.GW_FP16), (32768, 1024, 1, gw.GW_BF16), (32768, 256, 1, gw.GW_FP16),
-                                          (8192, 1024, 6, gw.GW_FP16), (16384, 256, 4, gw.GW_BF16)])
+                                          (8192, 1024, 6, gw.GW_FP16), (16384, 256, 4, gw.GW_BF16), (8192, 256, 8, gw.GW_FP16)])
 def test_incremental_path_is_bit_identical_to_full_recompute(W, S_, n, dtype):
     """DESIGN.md D13: with gw_options.incremental every layer's activations live in rings
     over absolute position and an update recomputes only the rows near the two window edges (tests/test_oracle_pins.py
     pins which).  The result must be the SAME NUMBERS as full recomputation: raw prediction, final cleaned samples and
     scores compared with array_equal over more than 2 W/S updates, warm-up included (the first update fills the rings
     with whole windows), through the CUDA graph; the stored activations of every layer as well at the end.
-    Even stream counts take the CTA-pair layers' packed form (both zones in one tile per window, a pair = two windows),
-    odd ones the tile-per-zone form."""
+    Even stream counts take the CTA-pair layers' packed form (both zones of one, two or four windows in one tile: stride
+    1024 / 512 / 256 with stream counts that divide), odd ones the tile-per-zone form."""
     cfg0 = S.config_c3(n, S_, W)
     Lb = min(4096, W // 2)
     cfg = S.Config("inc", cfg0.stream, cfg0.dc_layers, cfg0.bbh_convs, cfg0.bbh_dense, Lb, 0, 11)
