@@ -543,6 +543,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             const int r0 = map_tile(p, vt) * kTileM + quad * 32;
             return r0 < p.z_left || r0 + 32 > p.M - p.z_right;
         };
+        auto fin_row_live = [&](int orow) -> bool {            // EPI_FINAL zone launches: is this output row recomputed?
+            return (p.z_left | p.z_right) == 0 || orow < p.z_left || orow >= p.M - p.z_right;
+        };
         const float fin_bias = EPI == EPI_FINAL ? __ldg(p.fin_b + det) : 0.f;
         int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL: the tile whose second chain is in flight
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;   // + 32 KiB for the second buffer
@@ -639,30 +642,39 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 // PREVIOUS tile are read back one iteration later, when its chain has long retired.
                 const int vt = (u % spi) * G + hsel;
                 const int mt = vt < p.v_tiles ? map_tile(p, vt) : p.tiles_m;   // tiles_m: no such tile
+                // zone launches: this warp's 32 rows matter only if one of them, or a neighbour the second chain reads with
+                // it, is a recomputed row (the first z_left / last z_right rows of the layer); else the stale shared-memory
+                // rows stay and feed nothing but outputs that are not stored
+                const int qr0 = mt * p.tile_stride + p.tile_row0 + quad * 32;
+                const bool qlive = (p.z_left | p.z_right) == 0 || qr0 < p.z_left + 1 || qr0 + 32 > p.M - p.z_right - 1;
                 uint32_t ra[32], rb[32];
-                tmem_ld_32x32(taddr + 64 * hsel, ra);
-                tmem_ld_32x32(taddr + 64 * hsel + 32, rb);
-                tmem_ld_wait();
+                if (qlive) {
+                    tmem_ld_32x32(taddr + 64 * hsel, ra);
+                    tmem_ld_32x32(taddr + 64 * hsel + 32, rb);
+                    tmem_ld_wait();
+                }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&tmem_empty[acc]);
                 const int row = mt * p.tile_stride + p.tile_row0 + row_in_tile;
                 const bool inside = mt < p.tiles_m && row >= 0 && row < p.M;
                 const uint32_t tile_u32 = smem_u32(smem_out) + (acc * 2 + hsel) * kFinTile + quad * 4096;
+                if (qlive) {
 #pragma unroll
-                for (int which = 0; which < 2; ++which) {
-                    const uint32_t* r = which == 0 ? ra : rb;
+                    for (int which = 0; which < 2; ++which) {
+                        const uint32_t* r = which == 0 ? ra : rb;
 #pragma unroll
-                    for (int jj = 0; jj < 4; ++jj) {
-                        uint32_t o[4];
+                        for (int jj = 0; jj < 4; ++jj) {
+                            uint32_t o[4];
 #pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const float4 b4 = lds_f4(bias_u32 + 4u * (32 * which + 8 * jj + 4 * h));
-                            o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
-                            o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
+                            for (int h = 0; h < 2; ++h) {
+                                const float4 b4 = lds_f4(bias_u32 + 4u * (32 * which + 8 * jj + 4 * h));
+                                o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
+                                o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
+                            }
+                            if (!inside) o[0] = o[1] = o[2] = o[3] = 0u;
+                            sts_u4(tile_u32 + lane * 128 + (((4 * which + jj) ^ (lane & 7)) << 4), o[0], o[1], o[2], o[3]);
                         }
-                        if (!inside) o[0] = o[1] = o[2] = o[3] = 0u;
-                        sts_u4(tile_u32 + lane * 128 + (((4 * which + jj) ^ (lane & 7)) << 4), o[0], o[1], o[2], o[3]);
                     }
                 }
                 fence_proxy_async();
@@ -676,7 +688,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     tmem_ld_32x4(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + hsel * kFinN, y);
                     tmem_ld_wait();
                     const int orow = prev_mt * p.tile_stride + row_in_tile;     // D row i = tile row i + 1
-                    if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M) {
+                    if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M && fin_row_live(orow)) {
                         int o4 = 4 * orow;                                      // window position of y[4 orow]
                         if (p.pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }   // ring slot (absolute index mod W)
                         *reinterpret_cast<float4*>(p.pred + static_cast<size_t>(prev_batch) * p.M * 4 + o4) =
@@ -805,7 +817,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             tmem_ld_32x4(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + hsel * kFinN, y);
             tmem_ld_wait();
             const int orow = prev_mt * p.tile_stride + row_in_tile;
-            if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M) {
+            if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M && fin_row_live(orow)) {
                 int o4 = 4 * orow;
                 if (p.pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }
                 *reinterpret_cast<float4*>(p.pred + static_cast<size_t>(prev_batch) * p.M * 4 + o4) =
@@ -840,7 +852,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
 constexpr int kGemm2Threads = 64 + kEpiWarps * 32;
 constexpr int kHalfB = 128 * 128;                    // half of one weight K block: 128 rows x 128 bytes
 
-template <int ACT, int FMT>
+// PACKED is a template parameter so that the whole-window instantiation (the two heaviest launches of the full step)
+// compiles without a trace of the zone packing: with the packing as a run-time branch it took 164 registers instead of 151
+// and ran 15 % slower per cycle.
+template <int ACT, int FMT, bool PACKED>
 __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid_constant__ ConvGemmParams p, int n_items) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -849,8 +864,8 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
     // (outputs 0 .. pk_left-1), the next pk_nr rows those of the right zone (tile rows pk_nl .. pk_nl + pk_right - 1 of the
     // segment = the layer's LAST pk_right rows); the tile rows in between mix neighbours and are dropped.  The two CTAs
     // of a pair then work on 2 pk_k consecutive batch items.
-    const bool packed = p.pk_nl > 0;
-    const int sl = slab_bytes_of(p.slab_rows + p.pk_nl);
+    constexpr bool packed = PACKED;
+    const int sl = slab_bytes_of(p.slab_rows + (PACKED ? p.pk_nl : 0));
     const int sa = p.sa_stages, sb = p.sb_stages;
     uint8_t* smem_out = smem;                                                // [out_bufs][8 warps][4 KiB]
     uint8_t* smem_b = smem + p.out_bufs * kOutStage;                         // [sb][16 KiB]
@@ -875,7 +890,7 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
     const int cworker = cid / p.n_det;
     const int n_cw = (gridDim.x / 2) / p.n_det;
     const int half_tiles = packed ? 1 : p.v_tiles / 2;                       // (virtual) tile pairs per batch item
-    const int pk_seg = p.pk_nl + p.pk_nr;
+    const int pk_seg = PACKED ? p.pk_nl + p.pk_nr : 1;
     const int total = packed ? n_items / (2 * p.pk_k) : n_items * half_tiles; // packed: one pair = 2 pk_k batch items
 
     if (warp == 0) {
@@ -1155,10 +1170,14 @@ __global__ void __launch_bounds__(kGemm2Threads, 1) k_conv_gemm_2sm(const __grid
 }
 
 typedef void (*Gemm2Kernel)(const ConvGemmParams, int);
-static Gemm2Kernel pick_kernel_2sm(int act, int fmt) {
-    if (act == ACT_TANH) return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_TANH, FMT_BF16> : k_conv_gemm_2sm<ACT_TANH, FMT_FP16>;
-    if (act == ACT_RELU) return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_RELU, FMT_BF16> : k_conv_gemm_2sm<ACT_RELU, FMT_FP16>;
-    return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_NONE, FMT_BF16> : k_conv_gemm_2sm<ACT_NONE, FMT_FP16>;
+template <bool PACKED>
+static Gemm2Kernel pick_kernel_2sm_t(int act, int fmt) {
+    if (act == ACT_TANH) return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_TANH, FMT_BF16, PACKED> : k_conv_gemm_2sm<ACT_TANH, FMT_FP16, PACKED>;
+    if (act == ACT_RELU) return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_RELU, FMT_BF16, PACKED> : k_conv_gemm_2sm<ACT_RELU, FMT_FP16, PACKED>;
+    return fmt == FMT_BF16 ? k_conv_gemm_2sm<ACT_NONE, FMT_BF16, PACKED> : k_conv_gemm_2sm<ACT_NONE, FMT_FP16, PACKED>;
+}
+static Gemm2Kernel pick_kernel_2sm(int act, int fmt, bool packed) {
+    return packed ? pick_kernel_2sm_t<true>(act, fmt) : pick_kernel_2sm_t<false>(act, fmt);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1271,9 +1290,11 @@ cudaError_t conv_gemm_prepare() {
         }
     for (int act = 0; act < 3; ++act)
         for (int fmt = 0; fmt < 2; ++fmt) {
-            cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel_2sm(act, fmt)),
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-            if (e != cudaSuccess) return e;
+            for (int pk = 0; pk < 2; ++pk) {
+                cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel_2sm(act, fmt, pk != 0)),
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+                if (e != cudaSuccess) return e;
+            }
         }
     g_prepared = true;
     return cudaSuccess;
@@ -1304,7 +1325,7 @@ cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
         at2[1].val.programmaticStreamSerializationAllowed = g.pdl ? 1 : 0;
         cfg2.attrs = at2;
         cfg2.numAttrs = 2;
-        e = cudaLaunchKernelEx(&cfg2, pick_kernel_2sm(g.p.act, g.p.fmt), g.p, n_items);
+        e = cudaLaunchKernelEx(&cfg2, pick_kernel_2sm(g.p.act, g.p.fmt, g.p.pk_nl > 0), g.p, n_items);
         count_launch();
         return e;
     }

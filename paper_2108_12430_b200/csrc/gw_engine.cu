@@ -637,7 +637,7 @@ static int make_incremental_variant(GemmLayer& gl, int left_rows, int right_rows
     // same operand layout (resident / streamed weights, CTA pair or not: the weight tensor map depends on it); only the
     // tiles-per-stage choice may differ.  A pair layer whose zones give an odd tile count gets one more left tile.
     if (p.two_sm && (p.v_tiles & 1)) { p.v_left += 1; p.v_tiles += 1; }
-    if (p.epi == EPI_STORE && p.v_tiles < p.tiles_m) { p.z_left = left_rows; p.z_right = right_rows; }
+    if ((p.epi == EPI_STORE || p.epi == EPI_FINAL) && p.v_tiles < p.tiles_m) { p.z_left = left_rows; p.z_right = right_rows; }
     conv_gemm_plan(gl.gi, sms);
     gl.has_inc = true;
     return GW_OK;
