@@ -218,9 +218,13 @@ __device__ __forceinline__ uint32_t pack_pair(float a, float b, int fmt) {
 // One accumulator stage is kAccCols = 256 TMEM columns and holds G = 256 / N consecutive output tiles
 // (EPI_STORE; G = 1 for the pooled epilogues), so that thin layers (N = 32, 64) hand over 8 or 4 tiles
 // per mbarrier round trip instead of one.  Two stages (512 columns) double-buffer MMA against epilogue.
-template <int EPI, int ACT, int FMT>
+// ZONE: the incremental path's output forms (mirror-ring stores, prediction ring, dead-quadrant skipping) exist in their
+// own instantiation, so that the whole-window kernels of the full step carry none of it.
+template <int EPI, int ACT, int FMT, bool ZONE>
 __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid_constant__ ConvGemmParams p,
                                                                     int n_items) {
+    const int out_ring_div = ZONE ? p.out_ring_div : 0, pred_ring = ZONE ? p.pred_ring : 0;
+    const int z_left = ZONE ? p.z_left : 0, z_right = ZONE ? p.z_right : 0;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     const int b_block = p.N * 128;
@@ -510,8 +514,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         griddep_wait();                                        // before the first global store of this grid
         // incremental path: window start inside the output mirror ring / the prediction ring (the append kernel of
         // this update has advanced the counter; nothing changes it while the conv kernels run)
-        const int ring_h = (p.out_ring_div || p.pred_ring) ? static_cast<int>(*p.a_count % p.a_ring_W) : 0;
-        const int out_off = p.out_ring_div ? ring_h / p.out_ring_div : 0;
+        const int ring_h = (out_ring_div || pred_ring) ? static_cast<int>(*p.a_count % p.a_ring_W) : 0;
+        const int out_off = out_ring_div ? ring_h / out_ring_div : 0;
         // One 32-row box of this tile at window row `row` (whole warp calls it; lane 0 issues the TMA stores).  Mirror
         // ring: ring row r = out_off + row, and every row is stored a second time at its twin r +- M.  A box that
         // straddles row M has twins on both sides: those of its rows below M go out with a TMA store that the tensor
@@ -521,12 +525,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             const int r = out_off + row;
             if (lane == 0) {
                 tma_store_3d(&p.tmOut, src, col, r, b);
-                if (p.out_ring_div) {
+                if (out_ring_div) {
                     if (r >= p.M) tma_store_3d(&p.tmOut, src, col, r - p.M, b);
                     else tma_store_3d(&p.tmOut, src, col, r + p.M, b);
                 }
             }
-            if (p.out_ring_div && r < p.M && r + 31 >= p.M && r + lane >= p.M) {
+            if (out_ring_div && r < p.M && r + 31 >= p.M && r + lane >= p.M) {
                 uint8_t* dst = reinterpret_cast<uint8_t*>(p.out) +
                                ((static_cast<size_t>(b) * 2 * p.M + (r + lane - p.M)) * p.N + col) * 2;
                 const int units = row_bytes / 16;
@@ -539,12 +543,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         // zone launches (EPI_STORE): rows [r0, r0 + 32) of the layer hold a recomputed row iff they reach into the first
         // z_left or the last z_right rows
         auto quad_live = [&](int vt) -> bool {
-            if ((p.z_left | p.z_right) == 0) return true;
+            if ((z_left | z_right) == 0) return true;
             const int r0 = map_tile(p, vt) * kTileM + quad * 32;
-            return r0 < p.z_left || r0 + 32 > p.M - p.z_right;
+            return r0 < z_left || r0 + 32 > p.M - z_right;
         };
         auto fin_row_live = [&](int orow) -> bool {            // EPI_FINAL zone launches: is this output row recomputed?
-            return (p.z_left | p.z_right) == 0 || orow < p.z_left || orow >= p.M - p.z_right;
+            return (z_left | z_right) == 0 || orow < z_left || orow >= p.M - z_right;
         };
         const float fin_bias = EPI == EPI_FINAL ? __ldg(p.fin_b + det) : 0.f;
         int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL: the tile whose second chain is in flight
@@ -646,7 +650,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 // it, is a recomputed row (the first z_left / last z_right rows of the layer); else the stale shared-memory
                 // rows stay and feed nothing but outputs that are not stored
                 const int qr0 = mt * p.tile_stride + p.tile_row0 + quad * 32;
-                const bool qlive = (p.z_left | p.z_right) == 0 || qr0 < p.z_left + 1 || qr0 + 32 > p.M - p.z_right - 1;
+                const bool qlive = (z_left | z_right) == 0 || qr0 < z_left + 1 || qr0 + 32 > p.M - z_right - 1;
                 uint32_t ra[32], rb[32];
                 if (qlive) {
                     tmem_ld_32x32(taddr + 64 * hsel, ra);
@@ -690,7 +694,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     const int orow = prev_mt * p.tile_stride + row_in_tile;     // D row i = tile row i + 1
                     if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M && fin_row_live(orow)) {
                         int o4 = 4 * orow;                                      // window position of y[4 orow]
-                        if (p.pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }   // ring slot (absolute index mod W)
+                        if (pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }   // ring slot (absolute index mod W)
                         *reinterpret_cast<float4*>(p.pred + static_cast<size_t>(prev_batch) * p.M * 4 + o4) =
                             make_float4(__uint_as_float(y[0]) + fin_bias, __uint_as_float(y[1]) + fin_bias,
                                         __uint_as_float(y[2]) + fin_bias, __uint_as_float(y[3]) + fin_bias);
@@ -819,7 +823,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             const int orow = prev_mt * p.tile_stride + row_in_tile;
             if (row_in_tile < p.tile_stride && prev_mt < p.tiles_m && orow < p.M && fin_row_live(orow)) {
                 int o4 = 4 * orow;
-                if (p.pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }
+                if (pred_ring) { o4 += ring_h; if (o4 >= 4 * p.M) o4 -= 4 * p.M; }
                 *reinterpret_cast<float4*>(p.pred + static_cast<size_t>(prev_batch) * p.M * 4 + o4) =
                     make_float4(__uint_as_float(y[0]) + fin_bias, __uint_as_float(y[1]) + fin_bias,
                                 __uint_as_float(y[2]) + fin_bias, __uint_as_float(y[3]) + fin_bias);
@@ -1264,9 +1268,11 @@ cudaError_t probe_mma_cycles(int N, float* issue, float* complete) {
 
 typedef void (*GemmKernel)(const ConvGemmParams, int);
 
-static GemmKernel pick_kernel(int epi, int act, int fmt) {
+static GemmKernel pick_kernel(int epi, int act, int fmt, bool zone) {
 #define GW_PICK(E, A)                                                                                         \
-    if (epi == E && act == A) return fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16> : k_conv_gemm_umma<E, A, FMT_FP16>;
+    if (epi == E && act == A)                                                                                 \
+        return zone ? (fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16, true> : k_conv_gemm_umma<E, A, FMT_FP16, true>)   \
+                    : (fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16, false> : k_conv_gemm_umma<E, A, FMT_FP16, false>);
     GW_PICK(EPI_STORE, ACT_TANH)
     GW_PICK(EPI_STORE, ACT_NONE)
     GW_PICK(EPI_STORE, ACT_RELU)
@@ -1284,9 +1290,11 @@ cudaError_t conv_gemm_prepare() {
     const int acts[6] = {ACT_TANH, ACT_NONE, ACT_RELU, ACT_RELU, ACT_RELU, ACT_TANH};
     for (int i = 0; i < 6; ++i)
         for (int fmt = 0; fmt < 2; ++fmt) {
-            cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel(epis[i], acts[i], fmt)),
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-            if (e != cudaSuccess) return e;
+            for (int zone = 0; zone < 2; ++zone) {
+                cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel(epis[i], acts[i], fmt, zone != 0)),
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+                if (e != cudaSuccess) return e;
+            }
         }
     for (int act = 0; act < 3; ++act)
         for (int fmt = 0; fmt < 2; ++fmt) {
@@ -1306,7 +1314,10 @@ cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     const int total = n_items * ((g.p.v_tiles + per_unit - 1) / per_unit);   // work units per detector
     int workers = g.grid / g.p.n_det;
     if (workers > total) workers = total;
-    GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt);
+    // the store epilogue without the zone forms is 9-11 % faster on e2 / e3 / d2 (measured, n = 128); the fused tail is
+    // 5 % SLOWER without them (code placement), so it always runs the instantiation that has them (inert in whole windows)
+    const bool zone = g.p.epi == EPI_FINAL || g.p.out_ring_div || g.p.pred_ring || g.p.z_left || g.p.z_right;
+    GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt, zone);
     if (!k) return cudaErrorInvalidDeviceFunction;           // no kernel for this (epilogue, activation) pair
     cudaError_t e;
     if (g.p.two_sm) {
