@@ -220,14 +220,18 @@ __device__ __forceinline__ uint32_t pack_pair(float a, float b, int fmt) {
 // per mbarrier round trip instead of one.  Two stages (512 columns) double-buffer MMA against epilogue.
 // ZONE: the incremental path's output forms (mirror-ring stores, prediction ring, dead-quadrant skipping) exist in their
 // own instantiation, so that the whole-window kernels of the full step carry none of it.
-template <int EPI, int ACT, int FMT, bool ZONE>
+// NT: GEMM N as a compile-time constant (0: read from the parameters) -- the whole-window DeepClean layers get their own
+// instantiation per width, so that the instruction descriptor, the weight-block stride and the epilogue's chunk -> tile
+// map are constants.
+template <int EPI, int ACT, int FMT, bool ZONE, int NT>
 __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid_constant__ ConvGemmParams p,
                                                                     int n_items) {
+    const int pN = NT ? NT : p.N;
     const int out_ring_div = ZONE ? p.out_ring_div : 0, pred_ring = ZONE ? p.pred_ring : 0;
     const int z_left = ZONE ? p.z_left : 0, z_right = ZONE ? p.z_right : 0;
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    const int b_block = p.N * 128;
+    const int b_block = pN * 128;
     const int sl = slab_bytes_of(p.slab_rows);
     const int sa = p.sa_stages, sb = p.sb_stages;
     uint8_t* smem_out = smem;                                                // [out_bufs][8 warps][4 KiB]
@@ -256,7 +260,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int det = blockIdx.x % p.n_det;
     const int worker = blockIdx.x / p.n_det;
     const int n_workers = gridDim.x / p.n_det;
-    const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / p.N) : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
+    const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / pN) : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
     const int spi = (p.v_tiles + G - 1) / G;                                 // super-tiles per batch item (virtual tiles:
                                                                              // all of them, or the two recomputed zones)
     // Two MMA-issuing warps share a stage when it holds several tiles (even tiles: warp 1, odd tiles: warp
@@ -305,7 +309,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                         const int s = p.seg_of[cb][sh];
                         if (s < 0) continue;
                         if ((p.mask_nu >> (cb * kMaxShift + sh)) & 1ull) {
-                            tma_load_3d(smem_b + off, &p.tmBh, bres_bar, s * kSegK, p.N / 2, det);
+                            tma_load_3d(smem_b + off, &p.tmBh, bres_bar, s * kSegK, pN / 2, det);
                             off += b_block / 2;
                         } else {
                             tma_load_3d(smem_b + off, &p.tmB, bres_bar, s * kSegK, 0, det);
@@ -365,14 +369,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         // it to uniform registers one R2UR at a time; clock64 stamps put that block at ~330 cycles fixed
         // plus ~40 per MMA, which bounded every layer with N <= 128 (an MMA there executes in 16..64 cycles).
         // Which shifts exist for column block cb is a 6-bit field of the register `shmask`.
-        const uint32_t idesc = umma_idesc_f16(FMT, kTileM, p.N);
+        const uint32_t idesc = umma_idesc_f16(FMT, kTileM, pN);
         if (p.b_resident) mbar_wait(bres_bar, 0);
         const uint32_t smem_a_u32 = smem_u32(smem_a), smem_b_u32 = smem_u32(smem_b);
         const bool resident = p.b_resident != 0;
         const bool ring = p.a_count != nullptr && p.tmA_heads == nullptr;   // window-edge rows must be cleared by hand
         const int n_cb = p.n_cb, n_shift = p.n_shift;
         const uint32_t b_step = static_cast<uint32_t>(b_block) >> 4;       // descriptor units per B K-block
-        const uint32_t idesc_half = umma_idesc_f16(FMT, kTileM, p.N / 2);
+        const uint32_t idesc_half = umma_idesc_f16(FMT, kTileM, pN / 2);
         const unsigned long long mask_k2 = p.mask_k2, mask_nu = p.mask_nu;
         unsigned long long shmask = 0;
         for (int cb = 0; cb < n_cb; ++cb)
@@ -418,7 +422,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             const int g_end = min(G, p.v_tiles - (u % spi) * G);
             for (int g = 0; g < g_end; ++g) {
                 if (n_mma == 2 && (g & 1) != mw) continue;                 // the other warp's tile
-                const uint32_t d_tmem = tmem_base + acc * kAccCols + g * p.N;
+                const uint32_t d_tmem = tmem_base + acc * kAccCols + g * pN;
                 uint32_t accumulate = 0;
                 uint32_t b_lo = umma_desc_lo(smem_b_u32);                  // resident: block 0 of B
                 for (int cb = 0; cb < n_cb; ++cb) {
@@ -451,7 +455,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             if ((mnu >> sh) & 1u) {                        // weights in the upper half of N only (half-size block)
 #pragma unroll
                                 for (int k = 0; k < kSegK / 16; ++k)
-                                    umma_f16_if(leader, d_tmem + p.N / 2, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc_half, 1u);
+                                    umma_f16_if(leader, d_tmem + pN / 2, umma_desc_make(a_lo_s + 2 * k), umma_desc_make(bl + 2 * k), idesc_half, 1u);
                                 bl += b_step / 2;
                             } else if ((mk2 >> sh) & 1u) {                 // K steps 0, 1 hold no weight
 #pragma unroll
@@ -500,7 +504,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         const int hsel = (warp - 2) / 4;                       // which half of the 32-column chunks
         const int row_in_tile = quad * 32 + lane;
         const int et = threadIdx.x - 64;                       // 0..255
-        for (int i = et; i < p.N; i += kEpiWarps * 32) bias_s[i] = __ldg(p.bias + static_cast<size_t>(det) * p.N + i);
+        for (int i = et; i < pN; i += kEpiWarps * 32) bias_s[i] = __ldg(p.bias + static_cast<size_t>(det) * pN + i);
         asm volatile("bar.sync 1, 256;" ::: "memory");
         // the four 32-column chunks this warp owns in every stage: tile-in-stage g and first column col0
         int ch_g[4], ch_col[4];
@@ -508,8 +512,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             const int c = 4 * (i / 2) + 2 * hsel + (i % 2);    // pairs of ADJACENT chunks: 128 contiguous bytes per row
-            ch_g[i] = (32 * c) / p.N;
-            ch_col[i] = (32 * c) % p.N;
+            ch_g[i] = (32 * c) / pN;
+            ch_col[i] = (32 * c) % pN;
         }
         griddep_wait();                                        // before the first global store of this grid
         // incremental path: window start inside the output mirror ring / the prediction ring (the append kernel of
@@ -532,7 +536,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             }
             if (out_ring_div && r < p.M && r + 31 >= p.M && r + lane >= p.M) {
                 uint8_t* dst = reinterpret_cast<uint8_t*>(p.out) +
-                               ((static_cast<size_t>(b) * 2 * p.M + (r + lane - p.M)) * p.N + col) * 2;
+                               ((static_cast<size_t>(b) * 2 * p.M + (r + lane - p.M)) * pN + col) * 2;
                 const int units = row_bytes / 16;
                 for (int u = 0; u < units; ++u) {
                     const int su = row_bytes == 128 ? (u ^ (lane & 7)) : (u ^ ((lane >> 1) & 3));
@@ -570,7 +574,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 // 32-row x 128-byte box (per-lane row stores would touch 32 lines with 16 bytes each per
                 // instruction: measured 65 % L1TEX utilisation and ~60 % of HBM rate on the thin layers).
                 // Rows past M are clipped by the tensor map.
-                const bool wide = p.N >= 64;
+                const bool wide = pN >= 64;
                 for (int cp = 0; cp < 2; ++cp) {
                     const int ca = 4 * cp + 2 * hsel, cbk = ca + 1;              // chunk indices
                     // zone launches: does this warp's quadrant of the chunk's tile hold a recomputed row at all?
@@ -706,7 +710,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 // (cols [N/2,N)); pooled row q = m/2 is the max over both halves of rows 2q and 2q+1.
                 const int m0 = (u % spi) * kTileM;
                 const int row = m0 + row_in_tile;
-                const int half = p.N / 2;
+                const int half = pN / 2;
                 const int Mq = p.M / 2;
                 const int pstride = half + 1;
                 float* pool_s = head_s;                        // [64][half+1] fp32 (EPI_POOL_HEAD only)
@@ -1268,11 +1272,17 @@ cudaError_t probe_mma_cycles(int N, float* issue, float* complete) {
 
 typedef void (*GemmKernel)(const ConvGemmParams, int);
 
-static GemmKernel pick_kernel(int epi, int act, int fmt, bool zone) {
+static GemmKernel pick_kernel(int epi, int act, int fmt, bool zone, int N = 0) {
+    // whole-window DeepClean layers (store epilogue, tanh): N is a template parameter
+    if (epi == EPI_STORE && act == ACT_TANH && !zone) {
+        if (N == 32) return fmt == FMT_BF16 ? k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_BF16, false, 32> : k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_FP16, false, 32>;
+        if (N == 64) return fmt == FMT_BF16 ? k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_BF16, false, 64> : k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_FP16, false, 64>;
+        if (N == 128) return fmt == FMT_BF16 ? k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_BF16, false, 128> : k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_FP16, false, 128>;
+    }
 #define GW_PICK(E, A)                                                                                         \
     if (epi == E && act == A)                                                                                 \
-        return zone ? (fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16, true> : k_conv_gemm_umma<E, A, FMT_FP16, true>)   \
-                    : (fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16, false> : k_conv_gemm_umma<E, A, FMT_FP16, false>);
+        return zone ? (fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16, true, 0> : k_conv_gemm_umma<E, A, FMT_FP16, true, 0>)   \
+                    : (fmt == FMT_BF16 ? k_conv_gemm_umma<E, A, FMT_BF16, false, 0> : k_conv_gemm_umma<E, A, FMT_FP16, false, 0>);
     GW_PICK(EPI_STORE, ACT_TANH)
     GW_PICK(EPI_STORE, ACT_NONE)
     GW_PICK(EPI_STORE, ACT_RELU)
@@ -1290,11 +1300,12 @@ cudaError_t conv_gemm_prepare() {
     const int acts[6] = {ACT_TANH, ACT_NONE, ACT_RELU, ACT_RELU, ACT_RELU, ACT_TANH};
     for (int i = 0; i < 6; ++i)
         for (int fmt = 0; fmt < 2; ++fmt) {
-            for (int zone = 0; zone < 2; ++zone) {
-                cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel(epis[i], acts[i], fmt, zone != 0)),
-                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-                if (e != cudaSuccess) return e;
-            }
+            for (int zone = 0; zone < 2; ++zone)
+                for (int N = 0; N <= 128; N = N ? 2 * N : 32) {
+                    cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel(epis[i], acts[i], fmt, zone != 0, N)),
+                                                         cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+                    if (e != cudaSuccess) return e;
+                }
         }
     for (int act = 0; act < 3; ++act)
         for (int fmt = 0; fmt < 2; ++fmt) {
@@ -1317,7 +1328,7 @@ cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     // the store epilogue without the zone forms is 9-11 % faster on e2 / e3 / d2 (measured, n = 128); the fused tail is
     // 5 % SLOWER without them (code placement), so it always runs the instantiation that has them (inert in whole windows)
     const bool zone = g.p.epi == EPI_FINAL || g.p.out_ring_div || g.p.pred_ring || g.p.z_left || g.p.z_right;
-    GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt, zone);
+    GemmKernel k = pick_kernel(g.p.epi, g.p.act, g.p.fmt, zone, g.p.N);
     if (!k) return cudaErrorInvalidDeviceFunction;           // no kernel for this (epilogue, activation) pair
     cudaError_t e;
     if (g.p.two_sm) {
