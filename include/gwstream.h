@@ -131,9 +131,15 @@ typedef struct {
  *              multiple of 512 in [512, 4096] and a dense hidden width <= 64 (BASELINE.json configs[2]); other shapes,
  *              fuse_bbh = 0 and GW_IMPL_SIMT take the three-kernel path (first block on CUDA cores, blocks 2 and 3 as
  *              conv GEMMs with activations in global memory).  Both paths keep the fp32 input unrounded; they agree
- *              within rounding (different summation order). */
+ *              within rounding (different summation order).
+ *  fuse_head   1 (default): the first two DeepClean layers (stride-2 Conv1d -> 32 and -> 64 channels, tanh) run as one
+ *              kernel: two tiles of layer 0 are activated into shared memory as one operand tile of layer 1, a second
+ *              chain of tcgen05.mma produces layer 1's rows, and layer 0's activation is never written (or read back) --
+ *              a quarter of the two layers' HBM traffic (gw_deepclean_activation returns GW_ESTATE for layer 0).  Whole
+ *              windows only (not with `incremental`), GW_IMPL_UMMA.  The same products in the same order: BIT-identical
+ *              to fuse_head = 0. */
 typedef struct {
-    int conv_impl, fuse_tail, pdl, snake, two_sm, skip_zeros, incremental, fuse_bbh;
+    int conv_impl, fuse_tail, pdl, snake, two_sm, skip_zeros, incremental, fuse_bbh, fuse_head;
 } gw_options;
 void gw_options_default(gw_options *o);
 

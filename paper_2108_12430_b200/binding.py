@@ -42,13 +42,14 @@ class Options(C.Structure):
     Defaults: tensor-core kernels, fused tail, PDL, snake order, CTA pairs, zero skipping on; incremental off; the
     classifier as one shared-memory-resident kernel (fuse_bbh) on."""
     _fields_ = [("conv_impl", C.c_int), ("fuse_tail", C.c_int), ("pdl", C.c_int), ("snake", C.c_int),
-                ("two_sm", C.c_int), ("skip_zeros", C.c_int), ("incremental", C.c_int), ("fuse_bbh", C.c_int)]
+                ("two_sm", C.c_int), ("skip_zeros", C.c_int), ("incremental", C.c_int), ("fuse_bbh", C.c_int), ("fuse_head", C.c_int)]
 
     def __init__(self, **kw):
         super().__init__()
         self.conv_impl, self.fuse_tail, self.pdl, self.snake, self.two_sm, self.skip_zeros, self.incremental = \
             GW_IMPL_UMMA, 1, 1, 1, 1, 1, 0
         self.fuse_bbh = 1
+        self.fuse_head = 1
         for k, v in kw.items():
             if k not in dict(self._fields_):
                 raise TypeError(f"unknown option {k}")

@@ -13,7 +13,7 @@ constexpr int kTileM = 128;        // UMMA M: one TMEM lane per output row
 constexpr int kSegK = 64;          // 64 x 16-bit = one 128-byte swizzle row
 
 enum { FMT_FP16 = 0, FMT_BF16 = 1 };                       // UMMA instruction-descriptor encoding
-enum { EPI_STORE = 0, EPI_POOL = 1, EPI_POOL_HEAD = 2, EPI_FINAL = 3 };
+enum { EPI_STORE = 0, EPI_POOL = 1, EPI_POOL_HEAD = 2, EPI_FINAL = 3, EPI_CHAIN = 4 };
 enum { ACT_NONE = 0, ACT_TANH = 1, ACT_RELU = 2 };
 
 constexpr int kMaxCb = 8;          // 64-column blocks of the A view (a_cols <= 512)
@@ -98,6 +98,16 @@ struct ConvGemmParams {
     // epilogue writes each activated accumulator row (positions 2m, 2m+1 x 32 channels = one 128-byte
     // row) to a shared-memory tile in the swizzled K-major layout, and a SECOND chain of tcgen05.mma
     // (M 128, N 16, K 3 x 64: rows m-1, m, m+1) turns it into the 4 predictions y[4m .. 4m+3].
+    // EPI_CHAIN: the first two encoder layers (Conv1d 21 -> 32 and 32 -> 64, k 7, stride 2, tanh) in one kernel.  Two
+    // consecutive tiles of this layer (2 x 128 positions x 32 channels) ARE one A tile of the next layer (128 position
+    // pairs x 64): the epilogue writes them, activated, into shared memory in the swizzled K-major layout, a second
+    // chain of tcgen05.mma (M 128, N 64, K 4 x 64: pair rows l-2 .. l+1) produces 125 rows of the next layer (super-tiles
+    // overlap by three pair rows), and a second epilogue stores those.  This layer's activation never exists in memory.
+    // tmF: the next layer's B operand, box (64, 64, 1); tmOut: ITS output, box (32, 32, 1); bias2 [n_det][64]; out2 / M2:
+    // its output tensor [batch][M2][64] and rows per batch item; chain_k2: bit sh = K steps 0, 1 of shift sh hold no weight.
+    const float* bias2;
+    void* out2;
+    int M2, chain_k2;
     CUtensorMap tmF;               // last layer as a B operand: 3-D (K = 3 x 64, N = 16, n_det), box (64, 16, 1)
     const float* fin_b;            // [n_det]
     float* pred;                   // [batch][4 M] fp32

@@ -54,6 +54,16 @@ constexpr int kFinTile = kTileM * 128;               // EPI_FINAL: one activated
 constexpr int kFinN = 16;                            // EPI_FINAL: N of the second MMA chain (4 real columns)
 constexpr int kFinCol = 128;                         // EPI_FINAL: TMEM column of the second chain's accumulators in a stage
 constexpr int kOutStage = kEpiWarps * 4096;          // output staging: 32 rows x 128 bytes per epilogue warp
+constexpr int kChainRows = 125;                      // EPI_CHAIN: rows of the second layer one super-tile produces
+constexpr int kChainTile = kTileM * 128;             // EPI_CHAIN: the second layer's A tile (two activated tiles of this layer)
+constexpr int kChainStg = 2 * kChainTile + 1024;     // EPI_CHAIN: offset of the second epilogue's staging (2 KiB per warp) behind
+                                                     // the two A tiles and 1 KiB the shifted reads of the last rows run into
+constexpr int kChainOut = kChainStg + kEpiWarps * 2048;
+constexpr int kChainBlock = 64 * 128;                // EPI_CHAIN: one K block of the second layer's B operand (N = 64 rows)
+constexpr int kChainScratch = 4 * kChainBlock;
+// first row (position) of this layer's virtual tile vt in chain mode: super-tile s = vt / 2 covers the second layer's rows
+// [125 s, 125 s + 125), which read its input pair rows 125 s - 2 .. 125 s + 125, i.e. positions from 250 s - 4 on
+__host__ __device__ __forceinline__ int chain_m0(int vt) { return (vt >> 1) * (2 * kChainRows) - 4 + (vt & 1) * kTileM; }
 
 __host__ __device__ __forceinline__ int slab_bytes_of(int slab_rows) { return (slab_rows * 128 + 1023) & ~1023; }
 __host__ __device__ __forceinline__ int head_scratch_bytes(int N, int hidden) {
@@ -97,7 +107,8 @@ bool conv_gemm_plan(GemmLaunch& g, int sm_count) {
         p.out_bufs = (kFixedSmem + 2 * kOutStage + b_need + 4 * sl <= kSmemBudget) ? 2 : 1;
     }
     const int fixed = kFixedSmem + (p.epi == EPI_POOL_HEAD ? head_scratch_bytes(p.N, p.head_hidden) : 0) +
-                      (p.epi == EPI_FINAL ? kFinalScratch : 0) + p.out_bufs * kOutStage;
+                      (p.epi == EPI_FINAL ? kFinalScratch : 0) + (p.epi == EPI_CHAIN ? kChainScratch + kChainOut : 0) +
+                      p.out_bufs * kOutStage;
     int b_bytes;
     int n_half = 0;
     for (unsigned long long m = p.mask_nu; m; m &= m - 1) ++n_half;
@@ -235,7 +246,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int sl = slab_bytes_of(p.slab_rows);
     const int sa = p.sa_stages, sb = p.sb_stages;
     uint8_t* smem_out = smem;                                                // [out_bufs][8 warps][4 KiB]
-    uint8_t* smem_b = smem + p.out_bufs * kOutStage;
+    uint8_t* smem_b = smem + (EPI == EPI_CHAIN ? kChainOut : p.out_bufs * kOutStage);
     uint8_t* smem_a = smem_b + (p.b_resident ? p.b_res_bytes : sb * b_block);
     uint8_t* after_a = smem_a + sa * sl;
     float* bias_s = reinterpret_cast<float*>(after_a);                       // [N]
@@ -260,7 +271,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int det = blockIdx.x % p.n_det;
     const int worker = blockIdx.x / p.n_det;
     const int n_workers = gridDim.x / p.n_det;
-    const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / pN) : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
+    const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / pN) : (EPI == EPI_FINAL || EPI == EPI_CHAIN) ? 2 : 1;   // tiles per accumulator stage
     const int spi = (p.v_tiles + G - 1) / G;                                 // super-tiles per batch item (virtual tiles:
                                                                              // all of them, or the two recomputed zones)
     // Two MMA-issuing warps share a stage when it holds several tiles (even tiles: warp 1, odd tiles: warp
@@ -278,12 +289,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         if (lane == 0) {
             tma_prefetch_desc(&p.tmA);
             tma_prefetch_desc(&p.tmB);
-            if (EPI == EPI_FINAL) tma_prefetch_desc(&p.tmF);
+            if (EPI == EPI_FINAL || EPI == EPI_CHAIN) tma_prefetch_desc(&p.tmF);
             for (int i = 0; i < sa; ++i) { mbar_init(&a_full[i], 1); mbar_init(&a_empty[i], 1); }
             for (int i = 0; i < sb; ++i) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
             mbar_init(bres_bar, 1);
             for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full[i], n_mma); mbar_init(&tmem_empty[i], kEpiWarps); }
-            for (int i = 0; i < 4; ++i) { mbar_init(&stg_full[i], 4); mbar_init(&fin_full[i], 1); }
+            for (int i = 0; i < 4; ++i) { mbar_init(&stg_full[i], EPI == EPI_CHAIN ? kEpiWarps : 4); mbar_init(&fin_full[i], 1); }
             fence_barrier_init();
         }
         __syncwarp();
@@ -302,7 +313,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         // ------------------------------------------------------------------------ TMA producer
         if (lane == 0) {
             if (p.b_resident) {
-                mbar_arrive_expect_tx(bres_bar, p.b_res_bytes + (EPI == EPI_FINAL ? kFinalScratch : 0));
+                mbar_arrive_expect_tx(bres_bar, p.b_res_bytes + (EPI == EPI_FINAL ? kFinalScratch : 0) + (EPI == EPI_CHAIN ? kChainScratch : 0));
                 int off = 0;                                   // blocks in issue order (cb outer, shift inner)
                 for (int cb = 0; cb < p.n_cb; ++cb)
                     for (int sh = 0; sh < p.n_shift; ++sh) {
@@ -318,6 +329,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     }
                 if (EPI == EPI_FINAL)
                     for (int s = 0; s < 3; ++s) tma_load_3d(smem_fin + s * kFinBlock, &p.tmF, bres_bar, s * kSegK, 0, det);
+                if (EPI == EPI_CHAIN)
+                    for (int s = 0; s < 4; ++s) tma_load_3d(smem_fin + s * kChainBlock, &p.tmF, bres_bar, s * kSegK, 0, det);
             }
             griddep_wait();
             int ib = 0;
@@ -334,7 +347,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 for (int g = 0; g < G; ++g) {
                     const int vt = (u % spi) * G + g;
                     if (vt >= p.v_tiles) break;
-                    const int m0 = map_tile(p, vt) * p.tile_stride + p.tile_row0;
+                    const int m0 = EPI == EPI_CHAIN ? chain_m0(vt) : map_tile(p, vt) * p.tile_stride + p.tile_row0;
                     for (int cb = 0; cb < p.n_cb; ++cb) {
                         const bool second = n_mma == 2 && (g & 1);
                         const int stage = second ? ring0 + rs1 : rs0;
@@ -414,6 +427,33 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 umma_commit_if(leader, &fin_full[accp * 2 + h]);
             }
         };
+        // EPI_CHAIN: the second layer on super-tile `itp`: D row i = pair rows i .. i + 3 of the activated A tile (input pair
+        // rows l - 2 .. l + 1 of output row l = 125 s + i) times the second layer's four K blocks; the same K steps in the
+        // same order as that layer's own kernel issues them (chain_k2: K steps 0, 1 of a block hold no weight).
+        const uint32_t idesc_ch = umma_idesc_f16(FMT, kTileM, 64);
+        auto issue_chain = [&](int itp) {
+            const int accp = itp & 1;
+            TR_WAIT(3, mbar_wait(&stg_full[accp], (itp >> 1) & 1))
+            tc_fence_after();
+            const uint32_t d_ch = tmem_base + accp * kAccCols + kFinCol;
+            const uint32_t a_t = stg_lo + static_cast<uint32_t>(accp * kChainTile >> 4);
+            uint32_t first = 0;
+#pragma unroll
+            for (int sh = 0; sh < 4; ++sh) {
+                const uint32_t bl = fin_lo + static_cast<uint32_t>(sh * kChainBlock >> 4);
+                if ((p.chain_k2 >> sh) & 1) {
+#pragma unroll
+                    for (int k = 2; k < kSegK / 16; ++k)
+                        umma_f16_if(leader, d_ch, umma_desc_make(a_t + 8u * sh + 2 * k), umma_desc_make(bl + 2 * k), idesc_ch, first | (k - 2));
+                } else {
+#pragma unroll
+                    for (int k = 0; k < kSegK / 16; ++k)
+                        umma_f16_if(leader, d_ch, umma_desc_make(a_t + 8u * sh + 2 * k), umma_desc_make(bl + 2 * k), idesc_ch, first | k);
+                }
+                first = 1;
+            }
+            umma_commit_if(leader, &fin_full[accp]);
+        };
         for (int w = worker; w < total; w += n_workers, ++it) {
             const int u = p.reverse ? total - 1 - w : w;
             const int acc = it & 1;
@@ -433,7 +473,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     if (ring) {
                         // window-edge zero padding: slab rows whose logical row is outside [0, M) hold
                         // neighbouring ring samples; clear them (whole 128-byte rows: swizzle-agnostic)
-                        const int lo = map_tile(p, (u % spi) * G + g) * p.tile_stride + p.tile_row0 + p.a_min;
+                        const int lo = (EPI == EPI_CHAIN ? chain_m0((u % spi) * G + g) : map_tile(p, (u % spi) * G + g) * p.tile_stride + p.tile_row0) + p.a_min;
                         if (lo < 0 || lo + p.slab_rows > p.a_rows) {
                             uint8_t* slab = smem_a + astage * sl;
                             for (int idx = lane; idx < p.slab_rows * 8; idx += 32) {
@@ -495,8 +535,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             }
             umma_commit_if(leader, &tmem_full[acc]);                       // accumulator stage complete
             if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);           // behind this stage's MMAs in the pipe
+            if (EPI == EPI_CHAIN && it > 0 && mw == 0) issue_chain(it - 1);
         }
         if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);
+        if (EPI == EPI_CHAIN && it > 0 && mw == 0) issue_chain(it - 1);
         if (mw == 0) { TR_FLUSH(3, 4) }
     } else if (warp < kMmaWarp2) {
         // ------------------------------------------------------------- epilogue warps 2..9 (8 warps)
@@ -505,6 +547,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         const int row_in_tile = quad * 32 + lane;
         const int et = threadIdx.x - 64;                       // 0..255
         for (int i = et; i < pN; i += kEpiWarps * 32) bias_s[i] = __ldg(p.bias + static_cast<size_t>(det) * pN + i);
+        if (EPI == EPI_CHAIN && et < 64) bias_s[64 + et] = __ldg(p.bias2 + static_cast<size_t>(det) * 64 + et);   // second layer's
         asm volatile("bar.sync 1, 256;" ::: "memory");
         // the four 32-column chunks this warp owns in every stage: tile-in-stage g and first column col0
         int ch_g[4], ch_col[4];
@@ -555,7 +598,52 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             return (z_left | z_right) == 0 || orow < z_left || orow >= p.M - z_right;
         };
         const float fin_bias = EPI == EPI_FINAL ? __ldg(p.fin_b + det) : 0.f;
-        int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL: the tile whose second chain is in flight
+        // EPI_CHAIN, second epilogue: the 125 rows super-tile `s_prev` of batch item `b_prev` produced (its chain was issued
+        // one iteration ago and has long retired).  Warp (quad, hsel): rows [32 quad, +32), channels [32 hsel, +32); bias,
+        // tanh, 16-bit, through this warp's 2 KiB staging buffer; quadrants 0-2 leave with one TMA store (32 rows x 64 bytes,
+        // clipped at the tensor's last row), quadrant 3 holds 29 live rows, which its lanes copy out themselves.
+        const uint32_t chain_stg = smem_u32(smem_out) + kChainStg + (warp - 2) * 2048;
+        auto chain_emit = [&](int accp, uint32_t parity, int b_prev, int s_prev) {
+            mbar_wait(&fin_full[accp], parity);
+            tc_fence_after();
+            uint32_t r[32];
+            tmem_ld_32x32(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + 32 * hsel, r);
+            if (lane == 0) tma_store_wait_read<0>();           // this warp's previous box has left the staging buffer
+            tmem_ld_wait();
+            __syncwarp();
+            const uint32_t bias_c = bias_u32 + 4u * (64 + 32 * hsel);
+#pragma unroll
+            for (int jj = 0; jj < 4; ++jj) {
+                uint32_t o[4];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const float4 b4 = lds_f4(bias_c + 16u * (2 * jj + h));
+                    o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
+                    o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
+                }
+                sts_u4(chain_stg + lane * 64 + ((jj ^ ((lane >> 1) & 3)) << 4), o[0], o[1], o[2], o[3]);
+            }
+            const int l0 = s_prev * kChainRows;                // first output row of the super-tile
+            if (quad < 3) {
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) {
+                    tma_store_3d(&p.tmOut, chain_stg, 32 * hsel, l0 + quad * 32, b_prev);
+                    tma_store_commit();
+                }
+            } else {
+                __syncwarp();
+                const int l = l0 + row_in_tile;
+                if (row_in_tile < kChainRows && l < p.M2) {
+                    uint8_t* dst = reinterpret_cast<uint8_t*>(p.out2) + ((static_cast<size_t>(b_prev) * p.M2 + l) * 64 + 32 * hsel) * 2;
+#pragma unroll
+                    for (int uq = 0; uq < 4; ++uq)
+                        *reinterpret_cast<float4*>(dst + 16 * uq) = lds_f4(chain_stg + lane * 64 + ((uq ^ ((lane >> 1) & 3)) << 4));
+                }
+                __syncwarp();                                  // the buffer is rewritten in the next call
+            }
+        };
+        int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL / EPI_CHAIN: the tile whose second chain is in flight
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;   // + 32 KiB for the second buffer
         int ostep = 0;
         int it = 0;
@@ -639,6 +727,39 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                         if (lane == 0) tma_store_commit();
                     }
                 }
+            } else if (EPI == EPI_CHAIN) {
+                // N = 32, two tiles per stage: tile g = hsel holds positions chain_m0(vt) + [0, 128) of this layer x 32
+                // channels; position pair r of the super-tile (the next layer's A row r = 64 g + position / 2) takes the
+                // position's 64 bytes in its even or odd half.  Zero outside this layer's rows (the next layer's padding).
+                const int s_cur = u % spi;
+                const int vt = s_cur * G + hsel;
+                uint32_t ra[32];
+                tmem_ld_32x32(taddr + 32 * hsel, ra);
+                tmem_ld_wait();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tmem_empty[acc]);
+                const int pos = chain_m0(vt) + row_in_tile;
+                const bool inside = vt < p.v_tiles && pos >= 0 && pos < p.M;
+                const int arow = 64 * hsel + (row_in_tile >> 1);
+                const uint32_t row_u32 = smem_u32(smem_out) + acc * kChainTile + arow * 128;
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    uint32_t o[4];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const float4 b4 = lds_f4(bias_u32 + 16u * (2 * jj + h));
+                        o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(ra[8 * jj + 4 * h]) + b4.x, __uint_as_float(ra[8 * jj + 4 * h + 1]) + b4.y);
+                        o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(ra[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(ra[8 * jj + 4 * h + 3]) + b4.w);
+                    }
+                    if (!inside) o[0] = o[1] = o[2] = o[3] = 0u;
+                    sts_u4(row_u32 + ((((row_in_tile & 1) * 4 + jj) ^ (arow & 7)) << 4), o[0], o[1], o[2], o[3]);
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&stg_full[acc]);
+                if (it > 0) chain_emit(acc ^ 1, ((it - 1) >> 1) & 1, prev_batch, prev_mt);
+                prev_batch = batch; prev_mt = s_cur;
             } else if (EPI == EPI_FINAL) {
                 // N = 64, two tiles per stage: accumulator row i of tile g is input position m = mt * 126 - 1 + i of
                 // this layer and holds its outputs x[2m][0..32) | x[2m+1][0..32) = one 128-byte row of the last
@@ -817,6 +938,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 }
             }
         }
+        if (EPI == EPI_CHAIN && it > 0) chain_emit((it - 1) & 1, ((it - 1) >> 1) & 1, prev_batch, prev_mt);
         if (EPI == EPI_FINAL && it > 0) {                      // the last tile's second chain
             const int accp = (it - 1) & 1;
             mbar_wait(&fin_full[accp * 2 + hsel], ((it - 1) >> 1) & 1);
@@ -835,7 +957,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         }
         if (warp == 2) { TR_FLUSH(8, 3) }
     }
-    if (EPI == EPI_STORE && warp >= 2 && warp < kMmaWarp2 && lane == 0) tma_store_wait_all<0>();   // staging buffers are still being read
+    if ((EPI == EPI_STORE || EPI == EPI_CHAIN) && warp >= 2 && warp < kMmaWarp2 && lane == 0) tma_store_wait_all<0>();   // staging buffers are still being read
     tc_fence_before();
     __syncthreads();
     stamp_end(p.stamp);
@@ -1273,6 +1395,8 @@ cudaError_t probe_mma_cycles(int N, float* issue, float* complete) {
 typedef void (*GemmKernel)(const ConvGemmParams, int);
 
 static GemmKernel pick_kernel(int epi, int act, int fmt, bool zone, int N = 0) {
+    if (epi == EPI_CHAIN && act == ACT_TANH)
+        return fmt == FMT_BF16 ? k_conv_gemm_umma<EPI_CHAIN, ACT_TANH, FMT_BF16, false, 32> : k_conv_gemm_umma<EPI_CHAIN, ACT_TANH, FMT_FP16, false, 32>;
     // whole-window DeepClean layers (store epilogue, tanh): N is a template parameter
     if (epi == EPI_STORE && act == ACT_TANH && !zone) {
         if (N == 32) return fmt == FMT_BF16 ? k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_BF16, false, 32> : k_conv_gemm_umma<EPI_STORE, ACT_TANH, FMT_FP16, false, 32>;
@@ -1307,6 +1431,11 @@ cudaError_t conv_gemm_prepare() {
                     if (e != cudaSuccess) return e;
                 }
         }
+    for (int fmt = 0; fmt < 2; ++fmt) {
+        cudaError_t e = cudaFuncSetAttribute(reinterpret_cast<const void*>(pick_kernel(EPI_CHAIN, ACT_TANH, fmt, false, 32)),
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+        if (e != cudaSuccess) return e;
+    }
     for (int act = 0; act < 3; ++act)
         for (int fmt = 0; fmt < 2; ++fmt) {
             for (int pk = 0; pk < 2; ++pk) {
@@ -1321,7 +1450,8 @@ cudaError_t conv_gemm_prepare() {
 
 cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     const int n_items = g.batch / g.p.n_det;
-    const int per_unit = g.p.epi == EPI_STORE ? (g.p.g_tiles ? g.p.g_tiles : kAccCols / g.p.N) : g.p.epi == EPI_FINAL ? 2 : 1;
+    const int per_unit = g.p.epi == EPI_STORE ? (g.p.g_tiles ? g.p.g_tiles : kAccCols / g.p.N)
+                                              : (g.p.epi == EPI_FINAL || g.p.epi == EPI_CHAIN) ? 2 : 1;
     const int total = n_items * ((g.p.v_tiles + per_unit - 1) / per_unit);   // work units per detector
     int workers = g.grid / g.p.n_det;
     if (workers > total) workers = total;

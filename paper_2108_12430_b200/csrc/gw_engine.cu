@@ -68,6 +68,7 @@ extern "C" void gw_options_default(gw_options* o) {
     o->fuse_tail = 1; o->pdl = 1; o->snake = 1; o->two_sm = 1; o->skip_zeros = 1;
     o->incremental = 0;
     o->fuse_bbh = 1;
+    o->fuse_head = 1;
 }
 static int take_options(gw_options& dst, const gw_options* src) {
     gw_options_default(&dst);
@@ -75,7 +76,7 @@ static int take_options(gw_options& dst, const gw_options* src) {
     if (src->conv_impl != GW_IMPL_UMMA && src->conv_impl != GW_IMPL_SIMT) return fail(GW_EINVAL, "unknown conv impl %d", src->conv_impl);
     dst = *src;
     dst.fuse_tail = !!src->fuse_tail; dst.pdl = !!src->pdl; dst.snake = !!src->snake; dst.two_sm = !!src->two_sm;
-    dst.skip_zeros = !!src->skip_zeros; dst.incremental = !!src->incremental; dst.fuse_bbh = !!src->fuse_bbh;
+    dst.skip_zeros = !!src->skip_zeros; dst.incremental = !!src->incremental; dst.fuse_bbh = !!src->fuse_bbh; dst.fuse_head = !!src->fuse_head;
     return GW_OK;
 }
 
@@ -294,6 +295,8 @@ struct gw_deepclean {
     bool mirror = false;                         // first layer reads the window from ring16 (no per-update gather)
     bool fused_tail = false;                     // last GEMM layer + final ConvTranspose1d run as one kernel (EPI_FINAL)
     bool inc = false;                            // incremental path: act[i] are mirror rings [batch][2 L_i][C_i], pred a ring
+    bool has_chain = false;                      // gw_options.fuse_head: layers 0 and 1 run as ONE kernel (EPI_CHAIN); act[1] is
+    GemmLayer chain;                             // never written.  Operands are those of gemm[0] / gemm[1] (not owned here)
     std::vector<void*> act;                      // act[0] = gathered window (null when `mirror`), act[i+1] = output of layer i
     std::vector<int> act_rows, act_cols;
     float* d_wt_final = nullptr;                 // [n_det][K][cpad]
@@ -961,6 +964,46 @@ static int deepclean_build(gw_deepclean* dc, gw_stream* s, const gw_dc_spec* spe
         p.fin_b = dc->d_b_final; p.pred = dc->pred;
         p.pred_ring = dc->inc ? 1 : 0;
     }
+    // gw_options.fuse_head: the first two encoder layers as one kernel (EPI_CHAIN, gw_conv_gemm.cu) -- whole-window
+    // streaming handles whose layers 0 / 1 are the stride-2 Conv1d pair that kernel is written for (GEMM N 32 and 64, one
+    // 64-column block, four row shifts from -2, resident weights, window edges as TMA zero fill)
+    if (opt.fuse_head && !dc->inc && !dc->offline && opt.conv_impl == GW_IMPL_UMMA && nl >= 4 &&
+        dc->host[0].kind == GW_CONV && dc->host[1].kind == GW_CONV) {
+        const ConvGemmParams &p0 = dc->gemm[0].g.p, &p1 = dc->gemm[1].g.p;
+        const bool edge_ok = p0.a_count == nullptr || p0.tmA_heads != nullptr;
+        if (p0.epi == EPI_STORE && p1.epi == EPI_STORE && p0.act == ACT_TANH && p1.act == ACT_TANH && p0.N == 32 && p1.N == 64 &&
+            p0.n_cb == 1 && p1.n_cb == 1 && p0.n_shift == 4 && p1.n_shift == 4 && p0.a_min == -2 && p1.a_min == -2 &&
+            p0.b_resident && p1.b_resident && p1.n_seg == 4 && p1.mask_nu == 0 && p0.mask_nu == 0 && !p0.a_4d && edge_ok &&
+            p1.a_rows * 2 == p0.M && p0.M % 2 == 0) {
+            dc->chain = dc->gemm[0];                    // operands, segment table, input tensor maps of layer 0
+            GemmLayer& c = dc->chain;
+            c.has_inc = false;
+            ConvGemmParams& p = c.g.p;
+            p.epi = EPI_CHAIN;
+            p.M2 = p1.M;
+            const int n_super = (p.M2 + 124) / 125;
+            p.tiles_m = p.v_tiles = p.v_left = 2 * n_super;
+            p.tile_stride = kTileM; p.tile_row0 = 0;
+            p.g_tiles = 0; p.out_bufs = 0;
+            p.bias2 = dc->gemm[1].d_bias;
+            p.out2 = dc->act[2];
+            p.chain_k2 = static_cast<int>(p1.mask_k2 & ((1ull << kMaxShift) - 1));
+            p.reverse = opt.snake ? 1 : 0;              // layer 2 walks forwards: end where it starts
+            const size_t ktot2 = static_cast<size_t>(p1.n_seg) * kSegK;
+            if (int rc = make_tmap(&p.tmF, dc->gemm[1].d_B, dc->fmt, ktot2, 64, nd, ktot2, 64 * ktot2, 64)) return rc;
+            if (int rc = make_tmap(&p.tmOut, dc->act[2], dc->fmt, 64, p.M2, batch, 64, static_cast<uint64_t>(p.M2) * 64, 32, 32)) return rc;
+            int dev = 0, sms = 148;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            p.two_sm = 0;
+            if (conv_gemm_plan(c.g, sms) && c.g.p.b_resident) {
+                c.name = "gemm.dc0+1";
+                c.flops = dc->gemm[0].flops + dc->gemm[1].flops;
+                c.d_B = nullptr; c.d_bias = nullptr; c.d_heads = nullptr; c.d_heads_left = nullptr; c.d_heads_right = nullptr;
+                dc->has_chain = true;
+            }
+        }
+    }
     if (dc->inc) {
         // zones in GEMM rows: an encoder row is one output position, a decoder row two (even | odd output), a row of the
         // fused tail four positions of the network output
@@ -1118,7 +1161,9 @@ static void deepclean_forward_enqueue(gw_deepclean* dc, LaunchCtx& cx, bool zone
     if (!dc->mirror)
         cx.check(launch_gather(s->ring, dc->act[0], s->d_count, dc->d_rows_map, s->n, s->C, dc->n_det, dc->n_wit, s->W,
                                dc->act_cols[0], dc->fmt, dc->d_pre, cx.next("gather"), cx.st));
-    for (auto& g : dc->gemm) run_gemm(g, cx, zones && dc->inc);
+    size_t first = 0;
+    if (dc->has_chain) { run_gemm(dc->chain, cx); first = 2; }    // layers 0 and 1 in one launch
+    for (size_t i = first; i < dc->gemm.size(); ++i) run_gemm(dc->gemm[i], cx, zones && dc->inc);
     if (!dc->fused_tail)
         cx.check(launch_final_convt(dc->act[dc->n_layers - 1], dc->d_wt_final, dc->d_b_final, dc->pred, dc->batch, dc->n_det,
                                     dc->final_L, dc->final_cpad, dc->final_K, dc->final_pad, dc->fmt, cx.next("final_convt"), cx.st));
@@ -1282,6 +1327,8 @@ extern "C" int gw_deepclean_activation(gw_deepclean* dc, int layer, void* out_de
     const int i = layer + 1;
     if (i == dc->n_layers - 1 && dc->fused_tail && out_dev)
         return fail(GW_ESTATE, "layer %d's output is not materialised: it is fused with the final layer (gw_options.fuse_tail = 0 to inspect it)", layer);
+    if (i == 1 && dc->has_chain && out_dev)
+        return fail(GW_ESTATE, "layer 0's output is not materialised: layers 0 and 1 run as one kernel (gw_options.fuse_head = 0 to inspect it)");
     if (rows) *rows = dc->act_rows[i];
     if (cols) *cols = dc->act_cols[i];
     const int64_t bytes = static_cast<int64_t>(dc->batch) * dc->act_rows[i] * dc->act_cols[i] * 2;

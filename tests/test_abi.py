@@ -36,9 +36,9 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 def test_options_defaults_and_per_handle_errors():
     L = binding.lib()
-    o = binding.Options(conv_impl=5, fuse_tail=0, pdl=0, snake=0, two_sm=0, skip_zeros=0, incremental=1, fuse_bbh=0)
+    o = binding.Options(conv_impl=5, fuse_tail=0, pdl=0, snake=0, two_sm=0, skip_zeros=0, incremental=1, fuse_bbh=0, fuse_head=0)
     L.gw_options_default(C.byref(o))
-    assert (o.conv_impl, o.fuse_tail, o.pdl, o.snake, o.two_sm, o.skip_zeros, o.incremental, o.fuse_bbh) == (0, 1, 1, 1, 1, 1, 0, 1)
+    assert (o.conv_impl, o.fuse_tail, o.pdl, o.snake, o.two_sm, o.skip_zeros, o.incremental, o.fuse_bbh, o.fuse_head) == (0, 1, 1, 1, 1, 1, 0, 1, 1)
     # a failing call without a handle is reported for the calling thread: gw_last_error(NULL)
     h = C.c_void_p()
     assert L.gw_stream_create(C.byref(h), 0, 22, 512, 512, 64) == binding.GW_EINVAL

@@ -132,16 +132,17 @@ def test_c0_last_stride_mode_and_latency_offset():
 def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype, fuse):
     """The full C1 network (21->32->64->128->256 and back, folded BatchNorm) on a 4096-sample window:
     every stored activation against the oracle's, several M tiles and all channel widths.  fuse=True is
-    the production path (last tensor-core layer + final ConvTranspose1d in one kernel: the activation
-    between them is not materialised); fuse=False stores and checks that activation as well."""
+    the production path (layers 0 + 1 in one kernel, last tensor-core layer + final ConvTranspose1d in one kernel: the
+    activations inside those kernels are not materialised); fuse=False stores and checks those activations as well."""
     cfg = S.Config("C1-short", S.StreamSpec(2, 1, 4096, 4096, 512), S.config_c1().dc_layers, seed=1)
     dc_params, _ = util.make_params(cfg)
     dc_params2 = [dc_params[0]]
     st = gw.Stream(cfg.stream)
-    dc = gw.DeepClean(st, cfg.dc_layers, dc_params2, dtype, opts=gw.Options(fuse_tail=fuse))
-    if fuse:
+    dc = gw.DeepClean(st, cfg.dc_layers, dc_params2, dtype, opts=gw.Options(fuse_tail=fuse, fuse_head=fuse))
+    fused_layers = (0, len(cfg.dc_layers) - 2) if fuse else ()     # fuse_head: layer 0's output, fuse_tail: the last stored one
+    for li in fused_layers:
         with pytest.raises(gw.GwError) as e:
-            dc.activation(len(cfg.dc_layers) - 2)
+            dc.activation(li)
         assert e.value.code == gw.GW_ESTATE
     od, et = util.oracle_dtype(dtype), util.elem_tol(dtype)
     n_up = 8
@@ -157,7 +158,7 @@ def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype, fuse):
         ref_p, acts = oracle.deepclean_forward(snap[cfg.stream.witness_rows(0)].astype(np.float64), cfg.dc_layers,
                                                prepared, return_all=True)
         for li, (layer, ref) in enumerate(zip(cfg.dc_layers[:-1], acts[:-1])):
-            if fuse and li == len(cfg.dc_layers) - 2:
+            if li in fused_layers:
                 continue
             got = dc.activation(li).float().cpu().numpy()[i, 0]          # [L][Cp]
             assert got.shape[0] == ref.shape[1]
@@ -177,7 +178,7 @@ def test_c1_shaped_layers_match_oracle_layer_by_layer(dtype, fuse):
                                       elem=util.ELEM_RMS, rel_l2=3e-3)
         worst_layer = 0.0
         for li, (layer, ref) in enumerate(zip(cfg.dc_layers[:-1], acts_r[:-1])):
-            if fuse and li == len(cfg.dc_layers) - 2:
+            if li in fused_layers:
                 continue
             got = dc.activation(li).float().cpu().numpy()[i, 0]
             # stored 16-bit values: a rounding that flips costs one unit in the last place of the value's binade (bf16:
@@ -406,7 +407,8 @@ def test_incremental_path_is_bit_identical_to_full_recompute(W, S_, n, dtype):
     xc = torch.from_numpy(np.ascontiguousarray(x.reshape(n, sp.channels, n_up, S_).transpose(2, 0, 1, 3))).cuda()
     outs, acts = {}, {}
     for inc in (0, 1):
-        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, opts=gw.Options(incremental=inc))
+        # fuse_head = 0: the whole-window engine stores layer 0's output, so that every layer can be compared
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, opts=gw.Options(incremental=inc, fuse_head=0))
         cs = torch.cuda.Stream()
         sc = torch.zeros(n, device="cuda")
         fin = torch.zeros((n, sp.n_det, S_), device="cuda")
@@ -981,7 +983,7 @@ def test_step_profile_decomposes_the_graph_step_and_outputs_rotate_without_recap
                 rows = pipe.step_profile(xc[t], scs[b], fins[b], cs)
                 labels = [r["label"] for r in rows]
                 assert labels[0] == "snapshot_append" and "aggregate" in labels and labels[-1] == "bbh_fused"
-                assert len(rows) == pipe.graph_nodes() == 10
+                assert len(rows) == pipe.graph_nodes() == 9            # append, 6 DeepClean kernels (layers 0 + 1 and the tail fused), overlap-add, classifier
                 prev_end, span = 0.0, 0.0
                 for r in rows:
                     assert r["end_us"] > r["begin_us"] >= 0.0, r
@@ -1053,6 +1055,43 @@ def test_handles_release_their_device_memory():
     gc.collect(); torch.cuda.synchronize(); torch.cuda.empty_cache()
     free1, _ = torch.cuda.mem_get_info()
     assert free0 - free1 < 8 * 2**20, (free0, free1)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("W,S_,n,dtype", [(2048, 256, 3, gw.GW_FP16), (4096, 512, 2, gw.GW_BF16), (32768, 512, 3, gw.GW_FP16)])
+def test_first_two_layers_as_one_kernel_are_bit_identical(W, S_, n, dtype):
+    """gw_options.fuse_head (default): layers 0 and 1 run as one kernel -- two tiles of layer 0 become, activated and in
+    shared memory, one operand tile of layer 1 (super-tiles of 125 rows overlapping by three position pairs; 17 to 66 of them
+    per window here, walked backwards under the snake order).  The same products in the same order as the two kernels:
+    prediction, final samples, scores and every stored activation from layer 1 on must be array_equal, and the graph has one
+    kernel fewer."""
+    cfg0 = S.config_c3(n, S_, W)
+    cfg = S.Config("head", cfg0.stream, cfg0.dc_layers, cfg0.bbh_convs, cfg0.bbh_dense, min(4096, W // 2), 0, 31)
+    sp = cfg.stream
+    n_up = 6
+    dc_params, bbh_params = util.make_params(cfg)
+    x = synth.multi_stream(cfg.seed, sp, n_up * S_)
+    xc = torch.from_numpy(np.ascontiguousarray(x.reshape(n, sp.channels, n_up, S_).transpose(2, 0, 1, 3))).cuda()
+    outs, acts, nodes = {}, {}, {}
+    for fuse in (1, 0):
+        stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, opts=gw.Options(fuse_head=fuse))
+        cs = torch.cuda.Stream()
+        sc = torch.zeros(n, device="cuda")
+        fin = torch.zeros((n, sp.n_det, S_), device="cuda")
+        torch.cuda.synchronize()
+        res = []
+        for t in range(n_up):
+            pipe.step(xc[t], sc, fin, cs)
+            cs.synchronize()
+            res.append((dc.noise().cpu().numpy(), fin.cpu().numpy().copy(), sc.cpu().numpy().copy()))
+        outs[fuse], nodes[fuse] = res, pipe.graph_nodes()
+        acts[fuse] = [dc.activation(li).cpu().view(torch.int16).numpy() for li in range(1, len(cfg.dc_layers) - 2)]
+    assert nodes[1] == nodes[0] - 1, nodes
+    for li, (a1, a0) in enumerate(zip(acts[1], acts[0])):
+        assert np.array_equal(a1, a0), ("activation after layer", li + 1, np.argwhere(a1 != a0)[:4])
+    for t in range(n_up):
+        for a, b, what in zip(outs[1][t], outs[0][t], ("pred", "final", "scores")):
+            assert np.array_equal(a, b), (t, what)
 
 
 @pytest.mark.gpu
