@@ -56,9 +56,10 @@ constexpr int kFinCol = 128;                         // EPI_FINAL: TMEM column o
 constexpr int kOutStage = kEpiWarps * 4096;          // output staging: 32 rows x 128 bytes per epilogue warp
 constexpr int kChainRows = 125;                      // EPI_CHAIN: rows of the second layer one super-tile produces
 constexpr int kChainTile = kTileM * 128;             // EPI_CHAIN: the second layer's A tile (two activated tiles of this layer)
-constexpr int kChainStg = 2 * kChainTile + 1024;     // EPI_CHAIN: offset of the second epilogue's staging (2 KiB per warp) behind
-                                                     // the two A tiles and 1 KiB the shifted reads of the last rows run into
-constexpr int kChainOut = kChainStg + kEpiWarps * 2048;
+constexpr int kChainStg = 4 * kChainTile + 1024;     // EPI_CHAIN: offset of the second epilogue's staging (2 x 2 KiB per warp) behind
+                                                     // the four A tiles ([stage][super-tile of the stage]) and 1 KiB the shifted
+                                                     // reads of the last rows run into
+constexpr int kChainOut = kChainStg + kEpiWarps * 4096;
 constexpr int kChainBlock = 64 * 128;                // EPI_CHAIN: one K block of the second layer's B operand (N = 64 rows)
 constexpr int kChainScratch = 4 * kChainBlock;
 // first row (position) of this layer's virtual tile vt in chain mode: super-tile s = vt / 2 covers the second layer's rows
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
     const int det = blockIdx.x % p.n_det;
     const int worker = blockIdx.x / p.n_det;
     const int n_workers = gridDim.x / p.n_det;
-    const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / pN) : (EPI == EPI_FINAL || EPI == EPI_CHAIN) ? 2 : 1;   // tiles per accumulator stage
+    const int G = EPI == EPI_STORE ? (p.g_tiles ? p.g_tiles : kAccCols / pN) : EPI == EPI_CHAIN ? 4 : EPI == EPI_FINAL ? 2 : 1;   // tiles per accumulator stage
     const int spi = (p.v_tiles + G - 1) / G;                                 // super-tiles per batch item (virtual tiles:
                                                                              // all of them, or the two recomputed zones)
     // Two MMA-issuing warps share a stage when it holds several tiles (even tiles: warp 1, odd tiles: warp
@@ -432,11 +433,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         // same order as that layer's own kernel issues them (chain_k2: K steps 0, 1 of a block hold no weight).
         const uint32_t idesc_ch = umma_idesc_f16(FMT, kTileM, 64);
         auto issue_chain = [&](int itp) {
-            const int accp = itp & 1;
-            TR_WAIT(3, mbar_wait(&stg_full[accp], (itp >> 1) & 1))
+          const int accp = itp & 1;
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {                    // the stage's two super-tiles: one per MMA warp
+            if (n_mma == 2 && j != mw) continue;
+            TR_WAIT(3, mbar_wait(&stg_full[accp * 2 + j], (itp >> 1) & 1))
             tc_fence_after();
-            const uint32_t d_ch = tmem_base + accp * kAccCols + kFinCol;
-            const uint32_t a_t = stg_lo + static_cast<uint32_t>(accp * kChainTile >> 4);
+            const uint32_t d_ch = tmem_base + accp * kAccCols + kFinCol + j * 64;
+            const uint32_t a_t = stg_lo + static_cast<uint32_t>((accp * 2 + j) * kChainTile >> 4);
             uint32_t first = 0;
 #pragma unroll
             for (int sh = 0; sh < 4; ++sh) {
@@ -452,7 +456,8 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                 }
                 first = 1;
             }
-            umma_commit_if(leader, &fin_full[accp]);
+            umma_commit_if(leader, &fin_full[accp * 2 + j]);
+          }
         };
         for (int w = worker; w < total; w += n_workers, ++it) {
             const int u = p.reverse ? total - 1 - w : w;
@@ -535,10 +540,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             }
             umma_commit_if(leader, &tmem_full[acc]);                       // accumulator stage complete
             if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);           // behind this stage's MMAs in the pipe
-            if (EPI == EPI_CHAIN && it > 0 && mw == 0) issue_chain(it - 1);
+            if (EPI == EPI_CHAIN && it > 0) issue_chain(it - 1);
         }
         if (EPI == EPI_FINAL && it > 0) issue_final(it - 1);
-        if (EPI == EPI_CHAIN && it > 0 && mw == 0) issue_chain(it - 1);
+        if (EPI == EPI_CHAIN && it > 0) issue_chain(it - 1);
         if (mw == 0) { TR_FLUSH(3, 4) }
     } else if (warp < kMmaWarp2) {
         // ------------------------------------------------------------- epilogue warps 2..9 (8 warps)
@@ -598,49 +603,60 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             return (z_left | z_right) == 0 || orow < z_left || orow >= p.M - z_right;
         };
         const float fin_bias = EPI == EPI_FINAL ? __ldg(p.fin_b + det) : 0.f;
-        // EPI_CHAIN, second epilogue: the 125 rows super-tile `s_prev` of batch item `b_prev` produced (its chain was issued
-        // one iteration ago and has long retired).  Warp (quad, hsel): rows [32 quad, +32), channels [32 hsel, +32); bias,
-        // tanh, 16-bit, through this warp's 2 KiB staging buffer; quadrants 0-2 leave with one TMA store (32 rows x 64 bytes,
-        // clipped at the tensor's last row), quadrant 3 holds 29 live rows, which its lanes copy out themselves.
-        const uint32_t chain_stg = smem_u32(smem_out) + kChainStg + (warp - 2) * 2048;
+        // EPI_CHAIN, second epilogue: the 2 x 125 rows the two super-tiles `s_prev`, `s_prev + 1` of batch item `b_prev`
+        // produced (their chains were issued one iteration ago and have long retired).  Warp (quad, hsel): rows [32 quad, +32),
+        // channels [32 hsel, +32) of both; bias, tanh, 16-bit, through this warp's two 2 KiB staging buffers; quadrants 0-2 leave
+        // with one TMA store each (32 rows x 64 bytes, clipped at the tensor's last row), quadrant 3 holds 29 live rows, which
+        // its lanes copy out themselves.
+        const uint32_t chain_stg = smem_u32(smem_out) + kChainStg + (warp - 2) * 4096;   // two 2 KiB boxes: one per super-tile of the stage
         auto chain_emit = [&](int accp, uint32_t parity, int b_prev, int s_prev) {
-            mbar_wait(&fin_full[accp], parity);
-            tc_fence_after();
-            uint32_t r[32];
-            tmem_ld_32x32(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + 32 * hsel, r);
-            if (lane == 0) tma_store_wait_read<0>();           // this warp's previous box has left the staging buffer
+            uint32_t r[2][32];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                mbar_wait(&fin_full[accp * 2 + j], parity);
+                tc_fence_after();
+                tmem_ld_32x32(tmem_base + (static_cast<uint32_t>(quad * 32) << 16) + accp * kAccCols + kFinCol + 64 * j + 32 * hsel, r[j]);
+            }
+            if (lane == 0) tma_store_wait_read<0>();           // this warp's previous boxes have left the staging buffers
             tmem_ld_wait();
             __syncwarp();
             const uint32_t bias_c = bias_u32 + 4u * (64 + 32 * hsel);
 #pragma unroll
-            for (int jj = 0; jj < 4; ++jj) {
-                uint32_t o[4];
+            for (int j = 0; j < 2; ++j)
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const float4 b4 = lds_f4(bias_c + 16u * (2 * jj + h));
-                    o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
-                    o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
+                for (int jj = 0; jj < 4; ++jj) {
+                    uint32_t o[4];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const float4 b4 = lds_f4(bias_c + 16u * (2 * jj + h));
+                        o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj + 4 * h]) + b4.x, __uint_as_float(r[j][8 * jj + 4 * h + 1]) + b4.y);
+                        o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[j][8 * jj + 4 * h + 3]) + b4.w);
+                    }
+                    sts_u4(chain_stg + j * 2048 + lane * 64 + ((jj ^ ((lane >> 1) & 3)) << 4), o[0], o[1], o[2], o[3]);
                 }
-                sts_u4(chain_stg + lane * 64 + ((jj ^ ((lane >> 1) & 3)) << 4), o[0], o[1], o[2], o[3]);
-            }
-            const int l0 = s_prev * kChainRows;                // first output row of the super-tile
             if (quad < 3) {
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) {
-                    tma_store_3d(&p.tmOut, chain_stg, 32 * hsel, l0 + quad * 32, b_prev);
+#pragma unroll
+                    for (int j = 0; j < 2; ++j)
+                        if ((s_prev + j) * kChainRows < p.M2)
+                            tma_store_3d(&p.tmOut, chain_stg + j * 2048, 32 * hsel, (s_prev + j) * kChainRows + quad * 32, b_prev);
                     tma_store_commit();
                 }
             } else {
                 __syncwarp();
-                const int l = l0 + row_in_tile;
-                if (row_in_tile < kChainRows && l < p.M2) {
-                    uint8_t* dst = reinterpret_cast<uint8_t*>(p.out2) + ((static_cast<size_t>(b_prev) * p.M2 + l) * 64 + 32 * hsel) * 2;
 #pragma unroll
-                    for (int uq = 0; uq < 4; ++uq)
-                        *reinterpret_cast<float4*>(dst + 16 * uq) = lds_f4(chain_stg + lane * 64 + ((uq ^ ((lane >> 1) & 3)) << 4));
+                for (int j = 0; j < 2; ++j) {
+                    const int l = (s_prev + j) * kChainRows + row_in_tile;
+                    if (row_in_tile < kChainRows && l < p.M2) {
+                        uint8_t* dst = reinterpret_cast<uint8_t*>(p.out2) + ((static_cast<size_t>(b_prev) * p.M2 + l) * 64 + 32 * hsel) * 2;
+#pragma unroll
+                        for (int uq = 0; uq < 4; ++uq)
+                            *reinterpret_cast<float4*>(dst + 16 * uq) = lds_f4(chain_stg + j * 2048 + lane * 64 + ((uq ^ ((lane >> 1) & 3)) << 4));
+                    }
                 }
-                __syncwarp();                                  // the buffer is rewritten in the next call
+                __syncwarp();                                  // the buffers are rewritten in the next call
             }
         };
         int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL / EPI_CHAIN: the tile whose second chain is in flight
@@ -728,36 +744,41 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     }
                 }
             } else if (EPI == EPI_CHAIN) {
-                // N = 32, two tiles per stage: tile g = hsel holds positions chain_m0(vt) + [0, 128) of this layer x 32
-                // channels; position pair r of the super-tile (the next layer's A row r = 64 g + position / 2) takes the
-                // position's 64 bytes in its even or odd half.  Zero outside this layer's rows (the next layer's padding).
-                const int s_cur = u % spi;
-                const int vt = s_cur * G + hsel;
-                uint32_t ra[32];
-                tmem_ld_32x32(taddr + 32 * hsel, ra);
+                // N = 32, four tiles per stage = two super-tiles: tile g holds positions chain_m0(vt) + [0, 128) of this layer
+                // x 32 channels; this warp drains tiles g = hsel and hsel + 2 (super-tile j = 0, 1 of the stage).  Position
+                // pair r of a super-tile (the next layer's A row r = 64 (g & 1) + position / 2) takes the position's 64 bytes
+                // in its even or odd half.  Zero outside this layer's rows (the next layer's padding).
+                const int s_cur = (u % spi) * 2;               // first super-tile of the stage
+                uint32_t ra[2][32];
+                tmem_ld_32x32(taddr + 32 * hsel, ra[0]);
+                tmem_ld_32x32(taddr + 32 * (hsel + 2), ra[1]);
                 tmem_ld_wait();
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&tmem_empty[acc]);
-                const int pos = chain_m0(vt) + row_in_tile;
-                const bool inside = vt < p.v_tiles && pos >= 0 && pos < p.M;
                 const int arow = 64 * hsel + (row_in_tile >> 1);
-                const uint32_t row_u32 = smem_u32(smem_out) + acc * kChainTile + arow * 128;
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) {
-                    uint32_t o[4];
+                for (int j = 0; j < 2; ++j) {
+                    const int vt = (u % spi) * G + hsel + 2 * j;
+                    const int pos = chain_m0(vt) + row_in_tile;
+                    const bool inside = vt < p.v_tiles && pos >= 0 && pos < p.M;
+                    const uint32_t row_u32 = smem_u32(smem_out) + (acc * 2 + j) * kChainTile + arow * 128;
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const float4 b4 = lds_f4(bias_u32 + 16u * (2 * jj + h));
-                        o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(ra[8 * jj + 4 * h]) + b4.x, __uint_as_float(ra[8 * jj + 4 * h + 1]) + b4.y);
-                        o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(ra[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(ra[8 * jj + 4 * h + 3]) + b4.w);
+                    for (int jj = 0; jj < 4; ++jj) {
+                        uint32_t o[4];
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+                            const float4 b4 = lds_f4(bias_u32 + 16u * (2 * jj + h));
+                            o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(ra[j][8 * jj + 4 * h]) + b4.x, __uint_as_float(ra[j][8 * jj + 4 * h + 1]) + b4.y);
+                            o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(ra[j][8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(ra[j][8 * jj + 4 * h + 3]) + b4.w);
+                        }
+                        if (!inside) o[0] = o[1] = o[2] = o[3] = 0u;
+                        sts_u4(row_u32 + ((((row_in_tile & 1) * 4 + jj) ^ (arow & 7)) << 4), o[0], o[1], o[2], o[3]);
                     }
-                    if (!inside) o[0] = o[1] = o[2] = o[3] = 0u;
-                    sts_u4(row_u32 + ((((row_in_tile & 1) * 4 + jj) ^ (arow & 7)) << 4), o[0], o[1], o[2], o[3]);
                 }
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&stg_full[acc]);
+                if (lane == 0) { mbar_arrive(&stg_full[acc * 2]); mbar_arrive(&stg_full[acc * 2 + 1]); }
                 if (it > 0) chain_emit(acc ^ 1, ((it - 1) >> 1) & 1, prev_batch, prev_mt);
                 prev_batch = batch; prev_mt = s_cur;
             } else if (EPI == EPI_FINAL) {
@@ -1451,7 +1472,7 @@ cudaError_t conv_gemm_prepare() {
 cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st) {
     const int n_items = g.batch / g.p.n_det;
     const int per_unit = g.p.epi == EPI_STORE ? (g.p.g_tiles ? g.p.g_tiles : kAccCols / g.p.N)
-                                              : (g.p.epi == EPI_FINAL || g.p.epi == EPI_CHAIN) ? 2 : 1;
+                                              : g.p.epi == EPI_CHAIN ? 4 : g.p.epi == EPI_FINAL ? 2 : 1;
     const int total = n_items * ((g.p.v_tiles + per_unit - 1) / per_unit);   // work units per detector
     int workers = g.grid / g.p.n_det;
     if (workers > total) workers = total;
