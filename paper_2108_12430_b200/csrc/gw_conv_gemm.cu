@@ -22,6 +22,9 @@
 //              TMA store, overlapping the next stage's MMAs
 // CTA c serves detector c % n_det (each detector has its own weights) and walks that detector's tiles
 // with stride gridDim.x / n_det.  k_conv_gemm_2sm (further down) is the CTA-pair variant for N = 256.
+// Two epilogues chain a SECOND layer onto the first through shared memory and a second run of tcgen05.mma: EPI_FINAL
+// (the network's last two layers: the 1-channel ConvTranspose1d rides on the 32-channel one) and EPI_CHAIN (its first
+// two: two tiles of layer 0 are one operand tile of layer 1); neither intermediate activation is ever stored.
 // Kernels of a step are chained with programmatic dependent launch (griddepcontrol).
 #include <stdio.h>
 
