@@ -625,18 +625,18 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             __syncwarp();
             const uint32_t bias_c = bias_u32 + 4u * (64 + 32 * hsel);
 #pragma unroll
-            for (int j = 0; j < 2; ++j)
+            for (int jj = 0; jj < 4; ++jj) {                   // one bias fetch serves both super-tiles (the kernel is bound by
+                const float4 b0 = lds_f4(bias_c + 32u * jj), b1 = lds_f4(bias_c + 32u * jj + 16u);   // shared-memory wavefronts)
 #pragma unroll
-                for (int jj = 0; jj < 4; ++jj) {
+                for (int j = 0; j < 2; ++j) {
                     uint32_t o[4];
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const float4 b4 = lds_f4(bias_c + 16u * (2 * jj + h));
-                        o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj + 4 * h]) + b4.x, __uint_as_float(r[j][8 * jj + 4 * h + 1]) + b4.y);
-                        o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[j][8 * jj + 4 * h + 3]) + b4.w);
-                    }
+                    o[0] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj]) + b0.x, __uint_as_float(r[j][8 * jj + 1]) + b0.y);
+                    o[1] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj + 2]) + b0.z, __uint_as_float(r[j][8 * jj + 3]) + b0.w);
+                    o[2] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj + 4]) + b1.x, __uint_as_float(r[j][8 * jj + 5]) + b1.y);
+                    o[3] = act_pack_t<ACT, FMT>(__uint_as_float(r[j][8 * jj + 6]) + b1.z, __uint_as_float(r[j][8 * jj + 7]) + b1.w);
                     sts_u4(chain_stg + j * 2048 + lane * 64 + ((jj ^ ((lane >> 1) & 3)) << 4), o[0], o[1], o[2], o[3]);
                 }
+            }
             if (quad < 3) {
                 fence_proxy_async();
                 __syncwarp();
@@ -663,6 +663,16 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
             }
         };
         int prev_batch = 0, prev_mt = 0;                       // EPI_FINAL / EPI_CHAIN: the tile whose second chain is in flight
+        // EPI_CHAIN: this layer's 32 biases stay in registers (every lane needs all of them for every tile; read from shared
+        // memory they were 128 of the ~2600 shared-memory wavefronts per super-tile that bound the kernel)
+        float chain_bias[EPI == EPI_CHAIN ? 32 : 1];
+        if (EPI == EPI_CHAIN) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const float4 b4 = lds_f4(bias_u32 + 16u * i);
+                chain_bias[4 * i] = b4.x; chain_bias[4 * i + 1] = b4.y; chain_bias[4 * i + 2] = b4.z; chain_bias[4 * i + 3] = b4.w;
+            }
+        }
         const uint32_t stage_u32 = smem_u32(smem_out) + (warp - 2) * 4096;   // + 32 KiB for the second buffer
         int ostep = 0;
         int it = 0;
@@ -770,11 +780,11 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     for (int jj = 0; jj < 4; ++jj) {
                         uint32_t o[4];
 #pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const float4 b4 = lds_f4(bias_u32 + 16u * (2 * jj + h));
-                            o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(ra[j][8 * jj + 4 * h]) + b4.x, __uint_as_float(ra[j][8 * jj + 4 * h + 1]) + b4.y);
-                            o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(ra[j][8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(ra[j][8 * jj + 4 * h + 3]) + b4.w);
-                        }
+                        for (int h = 0; h < 2; ++h)
+#pragma unroll
+                            for (int q = 0; q < 2; ++q)
+                                o[2 * h + q] = act_pack_t<ACT, FMT>(__uint_as_float(ra[j][8 * jj + 4 * h + 2 * q]) + chain_bias[8 * jj + 4 * h + 2 * q],
+                                                                    __uint_as_float(ra[j][8 * jj + 4 * h + 2 * q + 1]) + chain_bias[8 * jj + 4 * h + 2 * q + 1]);
                         if (!inside) o[0] = o[1] = o[2] = o[3] = 0u;
                         sts_u4(row_u32 + ((((row_in_tile & 1) * 4 + jj) ^ (arow & 7)) << 4), o[0], o[1], o[2], o[3]);
                     }
