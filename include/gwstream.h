@@ -284,6 +284,28 @@ int64_t gw_offline_samples(const gw_offline *o);
 int gw_offline_run(gw_offline *o, const float *samples_dev, float *cleaned_dev, float *noise_dev, void *stream);
 int gw_offline_predictions(gw_offline *o, float *out_dev, void *stream);
 
+/* ---- The entry point that allocates nothing (csrc/gw_noalloc.cu) -------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the offline overlap-add above (D9) on per-window predictions the caller
+ * already holds, with no handle and no allocation.  It calls no cudaMalloc, cudaFree or allocating library routine: the
+ * Hann window and the summed-weight table it needs live in a fixed __device__ array inside the library (640 KiB, held by
+ * every GPU that loads the library until the process exits), whose device address is looked up once per device on the
+ * first call made with that device current.
+ *   pred_dev    [n_windows][n_det][window] fp32, window j = samples [j*stride, j*stride + window) of the segment
+ *   strain_dev  [n_det][T] fp32, T = window + (n_windows - 1) * stride
+ *   cleaned_dev [n_det][T] fp32 out: strain - estimate;  noise_dev [n_det][T] out or NULL: the estimate
+ *   post_dev    [n_det][2] fp32 (scale, offset) applied to the normalised estimate, or NULL for (1, 0)
+ * All are device pointers owned by the caller, none may alias an output.  Asynchronous on `stream` (three kernels).
+ * Same arithmetic as gw_offline_run's overlap-add (tables computed on the device instead of the host).
+ * Limits: window <= GW_OLA_NOALLOC_MAX_WINDOW, window % stride == 0, window / stride >= 2, n_det <= 65535; anything
+ * else returns GW_EINVAL and launches nothing.  GW_ECUDA: no device / launch failure (there is no CPU fallback).
+ * The scratch array is shared by all calls on a device and keeps the last call's tables; every call rewrites what it
+ * reads.  Calls on one stream are ordered; calls that OVERLAP on the GPU (different streams or threads) race on it
+ * unless they use the same (window, stride). */
+#define GW_OLA_NOALLOC_MAX_WINDOW 32768
+int gw_ola_offline_noalloc(const float *pred_dev, const float *strain_dev, float *cleaned_dev, float *noise_dev,
+                           const float *post_dev, int n_windows, int n_det, int window, int stride, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -28,6 +28,7 @@ EXPORTS = [          # include/gwstream.h
     "gw_bbh_create", "gw_bbh_destroy", "gw_bbh_score", "gw_bbh_score_batch",
     "gw_pipeline_create", "gw_pipeline_destroy", "gw_step", "gw_step_host", "gw_step_host_async", "gw_pipeline_graph_nodes",
     "gw_deepclean_set_scaling", "gw_offline_set_scaling", "gw_deepclean_set_postfilter", "gw_bbh_set_whitening", "gw_offline_create", "gw_offline_destroy", "gw_offline_samples", "gw_offline_run", "gw_offline_predictions",
+    "gw_ola_offline_noalloc",
 ]
 DIAG_EXPORTS = [     # include/gwstream_diag.h (measurement and diagnostics, not the product interface)
     "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes", "gw_probe_mma_cycles",
@@ -137,6 +138,7 @@ def lib():
         L.gw_offline_samples.restype = i64
         L.gw_offline_run.argtypes = [vp, vp, vp, vp, vp]
         L.gw_offline_predictions.argtypes = [vp, vp, vp]
+        L.gw_ola_offline_noalloc.argtypes = [vp, vp, vp, vp, vp, C.c_int, C.c_int, C.c_int, C.c_int, vp]
         L.gw_pipeline_graph_nodes.argtypes = [vp]
         L.gw_step_profile.argtypes = [vp, vp, vp, vp, vp, i, C.POINTER(C.c_double), C.POINTER(C.c_double),
                                       C.POINTER(C.c_double), C.POINTER(i)]
@@ -522,6 +524,31 @@ class Offline:
                 self.h = C.c_void_p()
         except Exception:
             pass
+
+
+GW_OLA_NOALLOC_MAX_WINDOW = 32768
+
+
+def ola_offline_noalloc(pred, strain, stride: int, cleaned=None, noise=None, post=None, stream=None):
+    """gw_ola_offline_noalloc (include/gwstream.h): the offline Hann overlap-add with the library's built-in scratch,
+    no handle and no allocation inside the library.  pred: CUDA float32 [B][D][W]; strain: [D][T], T = W + (B-1)*stride;
+    post: optional [D][2] (scale, offset).  Pass `cleaned` (and `noise`) to keep this wrapper from allocating as well.
+    Returns (cleaned, noise)."""
+    import torch
+    B, D, W = (int(v) for v in pred.shape)
+    T = W + (B - 1) * int(stride)
+    assert pred.is_contiguous() and pred.dtype == torch.float32
+    assert tuple(strain.shape) == (D, T) and strain.is_contiguous() and strain.dtype == torch.float32
+    if cleaned is None:
+        cleaned = torch.empty((D, T), dtype=torch.float32, device=pred.device)
+    assert tuple(cleaned.shape) == (D, T) and cleaned.is_contiguous()
+    if noise is not None:
+        assert tuple(noise.shape) == (D, T) and noise.is_contiguous()
+    if post is not None:
+        assert tuple(post.shape) == (D, 2) and post.is_contiguous() and post.dtype == torch.float32
+    _check(lib().gw_ola_offline_noalloc(_ptr(pred), _ptr(strain), _ptr(cleaned), _ptr(noise), _ptr(post), B, D, W, int(stride),
+                                        _stream_ptr(stream)))
+    return cleaned, noise
 
 
 def build_ensemble(cfg: S.Config, dc_params_per_det, bbh_params=None, dtype: int = GW_BF16,

@@ -14,7 +14,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgwstream.so")
-SOURCES = ["gw_engine.cu", "gw_kernels.cu", "gw_conv_gemm.cu", "gw_bbh_fused.cu"]
+SOURCES = ["gw_engine.cu", "gw_kernels.cu", "gw_conv_gemm.cu", "gw_bbh_fused.cu", "gw_noalloc.cu"]
 HEADERS = ["gw_common.cuh", "gw_ptx.cuh", os.path.join("..", "..", "include", "gwstream.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared"]

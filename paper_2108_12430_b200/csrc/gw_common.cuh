@@ -232,6 +232,7 @@ cudaError_t bbh_fused_prepare();
 cudaError_t launch_bbh_fused(const BbhFusedParams& p, int batch, int fmt, int pdl, cudaStream_t st);
 
 cudaError_t launch_stamp_init(unsigned long long* stamps, int n, cudaStream_t st);   // begin slots = max, end slots = 0
+int report_error(int code, const char* msg);   // records `msg` as the calling thread's gw_last_error (gw_engine.cu), returns `code`
 void count_launch();               // one more kernel launched (or captured) by this library: atomic process-wide counter
 long long kernel_launches();
 void uncount_launches(long long n);   // captured, not launched

@@ -45,6 +45,8 @@ static int fail(int code, const char* fmt, ...) {
     if (g_cur && g_cur->magic == kHandleMagic) g_cur->err = buf;
     return code;
 }
+// fail() for the library's other translation units (gw_noalloc.cu): a finished message, no formatting
+int gw::report_error(int code, const char* msg) { return fail(code, "%s", msg); }
 #define CU_TRY(expr)                                                                              \
     do {                                                                                          \
         cudaError_t _e = (expr);                                                                  \
