@@ -1126,3 +1126,60 @@ def test_scheduling_switches_are_bit_identical():
         for t in range(n_up):
             for a, b, what in zip(got[t], base[t], ("pred", "final", "scores")):
                 assert np.array_equal(a, b), (name, t, what)
+
+
+@pytest.mark.gpu
+def test_random_shapes_and_option_combinations_are_bit_identical():
+    """Seeded draws of (window, stride, streams, dtype) and of every gw_options switch at once, against the plain path
+    (nothing fused, full recompute, no PDL / snake / CTA pairs / zero skipping) with the same fuse_tail -- the one switch
+    the header states as 'within rounding'.  Prediction and final samples array_equal on warm-up and steady-state updates;
+    scores array_equal with the three-kernel classifier, within the score bar with the one-kernel one (other arithmetic)."""
+    import random
+    rng = random.Random(20260)
+    cases = 0
+    for _ in range(10):
+        W = rng.choice([2048, 4096, 6144, 8192, 16384])
+        S_ = rng.choice([s for s in (16, 64, 128, 256, 512, 1024, 2048) if s <= W // 2 and W % s == 0])
+        n = rng.choice([1, 2, 3, 4, 5, 8])
+        dtype = rng.choice([gw.GW_FP16, gw.GW_BF16])
+        cfg0 = S.config_c3(n, S_, W)
+        cfg = S.Config("mix", cfg0.stream, cfg0.dc_layers, cfg0.bbh_convs, cfg0.bbh_dense, 512 * max(1, min(4096, W // 2) // 512), 0,
+                       rng.randrange(1000))
+        sp = cfg.stream
+        n_up = min(W // S_ + 4, 24)
+        dc_params, bbh_params = util.make_params(cfg)
+        xc = torch.from_numpy(np.ascontiguousarray(
+            synth.multi_stream(cfg.seed, sp, n_up * S_).reshape(n, sp.channels, n_up, S_).transpose(2, 0, 1, 3))).cuda()
+
+        def run(opts):
+            stream, dc, bbh, pipe = gw.build_ensemble(cfg, dc_params, bbh_params, dtype, opts=opts)
+            cs = torch.cuda.Stream()
+            sc = torch.zeros(n, device="cuda")
+            fin = torch.zeros((n, sp.n_det, S_), device="cuda")
+            torch.cuda.synchronize()
+            out = []
+            for t in range(n_up):
+                pipe.step(xc[t], sc, fin, cs)
+                cs.synchronize()
+                if t < 2 or t % 4 == 0 or t >= n_up - 2:
+                    out.append((dc.noise().cpu().numpy(), fin.cpu().numpy().copy(), sc.cpu().numpy().copy()))
+            return out
+
+        plain = {ft: run(gw.Options(fuse_tail=ft, fuse_head=0, fuse_bbh=0, incremental=0, snake=0, pdl=0, two_sm=0, skip_zeros=0))
+                 for ft in (0, 1)}
+        for trial in range(3):
+            o = {name: rng.randint(0, 1) for name in ("fuse_tail", "fuse_head", "fuse_bbh", "incremental", "snake", "pdl", "two_sm", "skip_zeros")}
+            if trial == 0:
+                o = dict(fuse_tail=1, fuse_head=1, fuse_bbh=1, incremental=1, snake=1, pdl=1, two_sm=1, skip_zeros=1)
+            if o["incremental"] and (W % 2048 or S_ % 16 or not o["fuse_tail"]):
+                o["incremental"] = 0                     # shapes / combinations the incremental path refuses (tested elsewhere)
+            got = run(gw.Options(**o))
+            cases += 1
+            for (p0, f0, s0), (p1, f1, s1) in zip(plain[o["fuse_tail"]], got):
+                assert np.array_equal(p0, p1), ("pred", W, S_, n, dtype, o)
+                assert np.array_equal(f0, f1), ("final", W, S_, n, dtype, o)
+                if o["fuse_bbh"]:
+                    assert np.abs(s0 - s1).max() <= 5e-3, ("scores", W, S_, n, dtype, o)
+                else:
+                    assert np.array_equal(s0, s1), ("scores", W, S_, n, dtype, o)
+    assert cases == 30
