@@ -312,7 +312,7 @@ class Engine:
         del self.chunks_d
 
 
-def kernel_table(eng, order, acc, pk, sm_mhz, sms):
+def kernel_table(eng, order, acc, pk, sm_mhz, sms, full=True):
     """Per-kernel dict for the bench line: duration and exclusive share (us, from the graph-replay stamps), TFLOP/s on
     the exclusive time for the conv GEMMs (executed algorithmic FLOPs), GB/s for the bandwidth kernels."""
     sp, cfg = eng.sp, eng.cfg
@@ -330,6 +330,19 @@ def kernel_table(eng, order, acc, pk, sm_mhz, sms):
         "bbh_fused": sp.n_streams * (nd * cfg.bbh_len * 4 + 4),                      # the window in, one score out
     }
     smem_peak_gbs = sms * 128 * sm_mhz * 1e6 / 1e9
+    # MUFU operations of a whole-window DeepClean launch: one per tanh (fp16: tanh.approx.f32) or two (bf16: ex2 + rcp); the
+    # pipe retires 16 per clock per SM (measured: 15.99 with 512-1024 threads per SM, any operand width -- f16x2 / bf16x2 are
+    # two operations).  Zone launches (incremental path) are not counted: their rows are a fraction of the layer.
+    mufu_ops = {}
+    if full:
+        per_tanh = 2 if eng.dtype_name == "bf16" else 1
+        lens, tanh = [sp.window], []
+        for l in cfg.dc_layers:
+            lens.append(l.lout(lens[-1]))
+            tanh.append(sp.n_streams * nd * lens[-1] * l.cout * per_tanh if l.act == S.ACT_TANH else 0)
+        for k in order:
+            if k.startswith("gemm.dc"):
+                mufu_ops[k] = sum(tanh[int(i)] for i in k[len("gemm.dc"):].split("+"))   # the fused tail's last layer is linear
     out = {}
     for k in order:
         a = acc[k]
@@ -345,6 +358,8 @@ def kernel_table(eng, order, acc, pk, sm_mhz, sms):
         if a["smem_bytes"] and a["us"] > 0:
             gbs = a["smem_bytes"] / (a["us"] * 1e-6) / 1e9
             row.update({"smem_gbs": round(gbs, 1), "smem_frac": round(gbs / (sms * 128 * mhz * 1e6 / 1e9), 3)})
+        if mufu_ops.get(k) and a["us"] > 0:
+            row.update({"mufu_ops": mufu_ops[k], "mufu_frac": round(mufu_ops[k] / (a["us"] * 1e-6) / (sms * 16.0 * mhz * 1e6), 3)})
         if k in hbm_bytes and a["us"] > 0:
             gbs = hbm_bytes[k] / (a["us"] * 1e-6) / 1e9
             row.update({"gbs": round(gbs, 1), "hbm_frac": round(gbs / pk["hbm_gbs"], 3),
@@ -426,6 +441,11 @@ def run_native(args):
     sm_mhz_sus = (clocks_profile or {}).get("sm_mhz") or ((sustained or {}).get("clocks") or {}).get("sm_mhz") or 1700.0
     sms = torch.cuda.get_device_properties(local).multi_processor_count
     kernels, smem_peak_gbs = kernel_table(eng, order, acc, pk, sm_mhz_sus, sms)
+    mufu_total = sum(r.get("mufu_ops", 0) for r in kernels.values())
+    mufu = {"unit": "MUFU operations (tanh of the DeepClean epilogues)", "ops_per_step": mufu_total, "peak_per_clock_per_sm": 16,
+            "us_at_the_profiled_clock": round(mufu_total / (sms * 16.0 * sm_mhz_sus), 1),
+            "what": "time the step's tanh evaluations occupy the MUFU pipe of every SM at the profiled steps' clock: a second floor "
+                    "under the conv kernels beside the tensor pipe (per kernel: kernels[..].mufu_frac)"}
     gemm_us = sum(a["excl_us"] for k, a in acc.items() if k.startswith("gemm."))
     gemm_fl = sum(a["flops"] for k, a in acc.items() if k.startswith("gemm."))
     span_us = sum(a["excl_us"] for a in acc.values())
@@ -478,7 +498,7 @@ def run_native(args):
         lat_i = ie.latency(min(max(K, 50), 2000))
         e2e_i = ie.e2e(K, world)
         order_i, acc_i = ie.profile(ms_per_step=ms_i / n_i)
-        kern_i, _ = kernel_table(ie, order_i, acc_i, pk, (c3 or {}).get("sm_mhz") or 1700.0, sms)
+        kern_i, _ = kernel_table(ie, order_i, acc_i, pk, (c3 or {}).get("sm_mhz") or 1700.0, sms, full=False)
         fl_i = sum(a["flops"] for k, a in acc_i.items() if k.startswith("gemm."))
         us_i = sum(a["excl_us"] for k, a in acc_i.items() if k.startswith("gemm."))
         incremental = {"value": world * n_i * ie.ds_per_step / (ms_i / 1e3), "unit": UNIT, "steps": n_i,
@@ -644,7 +664,7 @@ def run_native(args):
                              "is re-read every step", "precision": f"{args.dtype} storage, fp32 accumulate"},
             "sustained": sustained, "latency": latency, "e2e": e2e, "gpu_launches": int(launches),
             "graph_nodes": graph_nodes,
-            "roofline": roofline, "smem_peak_gbs": round(smem_peak_gbs, 1), "kernels": kernels, "clocks": clocks,
+            "roofline": roofline, "smem_peak_gbs": round(smem_peak_gbs, 1), "mufu": mufu, "kernels": kernels, "clocks": clocks,
             "incremental": incremental, "largest": largest, "cpu_baseline": cpu, "offline": offline, "classifier_c2": classifier, "snapshotter": snapshotter,
         }
         print(json.dumps(line), flush=True)

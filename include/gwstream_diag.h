@@ -40,6 +40,14 @@ double gw_profile_smem_bytes(const gw_pipeline *p, int i);
  * one has retired, per MMA (host pointers).  Synchronises the device. */
 int gw_probe_mma_cycles(int N, float *issue_cycles, float *complete_cycles);
 
+/* Measured rate of the DeepClean epilogues' activation instruction on the current device, in results per clock per SM
+ * (host pointer), with `threads` threads per SM (multiple of 32, <= 1024) running eight independent chains each:
+ * mode 0 tanh.approx.f32 (fp16 engine: one MUFU operation per tanh), 1 tanh.approx.f16x2 (two results per instruction --
+ * and two MUFU operations: no gain), 2 ex2.approx + rcp.approx (bf16 engine's exact tanh: *result counts tanh evaluations,
+ * two MUFU operations each).  The MUFU pipe is the second floor under the thin conv layers: a layer
+ * evaluates rows x channels tanh per window.  Synchronises the device. */
+int gw_probe_mufu_rate(int mode, int threads, float *results_per_clock_per_sm);
+
 /* The arithmetic behind gw_options.incremental (D13), host only: for a stack of stride-2 layers
  * (kind, k as in gw_conv_layer; weights are not read) and `stride` new samples per update, left[i] / right[i] = how
  * many OUTPUT positions of layer i at the left / right end of the window differ from the previous update's value at

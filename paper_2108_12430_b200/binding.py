@@ -31,7 +31,7 @@ EXPORTS = [          # include/gwstream.h
     "gw_ola_offline_noalloc",
 ]
 DIAG_EXPORTS = [     # include/gwstream_diag.h (measurement and diagnostics, not the product interface)
-    "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes", "gw_probe_mma_cycles",
+    "gw_step_profile", "gw_profile_label", "gw_profile_flops", "gw_profile_smem_bytes", "gw_probe_mma_cycles", "gw_probe_mufu_rate",
     "gw_incremental_zones", "gw_bbh_fused_images",
 ]
 
@@ -104,6 +104,7 @@ def lib():
         L.gw_options_default.argtypes = [C.POINTER(Options)]
         L.gw_options_default.restype = None
         L.gw_probe_mma_cycles.argtypes = [i, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+        L.gw_probe_mufu_rate.argtypes = [i, i, C.POINTER(C.c_float)]
         L.gw_incremental_zones.argtypes = [C.POINTER(_ConvLayer), i, i, C.POINTER(i), C.POINTER(i)]
         L.gw_bbh_fused_images.argtypes = [C.POINTER(_BbhSpec), i, vp, vp, vp]
         L.gw_stream_create.argtypes = [C.POINTER(vp), i, i, i, i, i]
@@ -197,6 +198,13 @@ def probe_mma_cycles(n_values=(16, 32, 64, 128, 256)):
         _check(lib().gw_probe_mma_cycles(int(n), C.byref(a), C.byref(b)))
         out[int(n)] = (float(a.value), float(b.value))
     return out
+
+
+def probe_mufu_rate(mode: int = 0, threads: int = 512) -> float:
+    """Diagnostic: activation results per clock per SM (gwstream_diag.h; mode 0 tanh.f32, 1 tanh.f16x2, 2 ex2 + rcp)."""
+    r = C.c_float(0)
+    _check(lib().gw_probe_mufu_rate(int(mode), int(threads), C.byref(r)))
+    return float(r.value)
 
 
 def print_mma_probe() -> None:

@@ -152,6 +152,7 @@ cudaError_t launch_conv_gemm_umma(const GemmLaunch& g, cudaStream_t st);
 cudaError_t launch_conv_gemm_simt(const GemmLaunch& g, cudaStream_t st);
 // Chooses resident/streaming B, ring depths and the shared-memory size for a layer; false if it cannot fit.
 bool conv_gemm_plan(GemmLaunch& g, int sm_count);
+cudaError_t probe_mufu_rate(int mode, int threads, float* results_per_clock_per_sm);   // diagnostic: activation results per clock per SM
 cudaError_t probe_mma_cycles(int N, float* issue, float* complete);   // diagnostic: cycles per tcgen05.mma, N in {16..256}
 cudaError_t conv_gemm_prepare();   // opt-in shared-memory attribute
 

@@ -98,6 +98,15 @@ extern "C" int gw_probe_mma_cycles(int N, float* issue_cycles, float* complete_c
     return GW_OK;
 }
 
+extern "C" int gw_probe_mufu_rate(int mode, int threads, float* results_per_clock_per_sm) {
+    if (!results_per_clock_per_sm) return fail(GW_EINVAL, "gw_probe_mufu_rate: NULL argument");
+    if (mode < 0 || mode > 2) return fail(GW_EINVAL, "gw_probe_mufu_rate: mode must be 0 (tanh.f32), 1 (tanh.f16x2) or 2 (ex2 + rcp)");
+    if (threads < 32 || threads > 1024 || threads % 32) return fail(GW_EINVAL, "gw_probe_mufu_rate: threads must be a multiple of 32 in [32, 1024]");
+    if (int rc = check_device()) return rc;
+    CU_TRY(probe_mufu_rate(mode, threads, results_per_clock_per_sm));
+    return GW_OK;
+}
+
 // ------------------------------------------------------------------------- TMA descriptor encode
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                     const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,

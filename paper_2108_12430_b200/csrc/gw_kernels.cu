@@ -838,6 +838,69 @@ cudaError_t launch_ola_offline(const float* pred, const float* seg, const int* s
     return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------------------
+// Diagnostic (gwstream_diag.h, gw_probe_mufu_rate): results per clock per SM of the epilogues' activation instruction --
+// mode 0 tanh.approx.f32 (the fp16 engine's tanh), 1 tanh.approx.f16x2 (two results per instruction), 2 ex2.approx + rcp.approx
+// (the bf16 engine's exact form: two MUFU operations per tanh) -- with `threads` threads resident per SM and eight independent
+// chains per thread.  One block per SM; block 0 reports its own clock64 span.
+// ---------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void k_probe_mufu(unsigned* sink, int reps, long long* cycles) {
+    float f[8];
+    unsigned h[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { f[i] = 0.1f * i + threadIdx.x * 1e-3f; h[i] = 0x30003400u + threadIdx.x * 8 + i; }
+    __syncthreads();
+    const long long t0 = clock64();
+    for (int r = 0; r < reps; ++r) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            if (MODE == 0) asm volatile("tanh.approx.f32 %0, %0;" : "+f"(f[i]));
+            if (MODE == 1) asm volatile("tanh.approx.f16x2 %0, %0;" : "+r"(h[i]));
+            if (MODE == 2) {
+                asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(f[i]));
+                f[i] += 1.f;                               // as in the epilogue: 1 / (1 + e^2x); keeps ptxas from folding rcp(ex2)
+                asm volatile("rcp.approx.ftz.f32 %0, %0;" : "+f"(f[i]));
+            }
+        }
+    }
+    __syncthreads();
+    const long long t1 = clock64();
+    unsigned s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += h[i] + __float_as_uint(f[i]);
+    sink[blockIdx.x * blockDim.x + threadIdx.x] = s;
+    if (blockIdx.x == 0 && threadIdx.x == 0) *cycles = t1 - t0;
+}
+
+cudaError_t probe_mufu_rate(int mode, int threads, float* results_per_clock_per_sm) {
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    unsigned* sink = nullptr;
+    long long* cyc = nullptr;
+    e = cudaMalloc(&sink, static_cast<size_t>(sms) * threads * 4);
+    if (e == cudaSuccess) e = cudaMalloc(&cyc, 8);
+    const int reps = 2048;
+    for (int pass = 0; pass < 2 && e == cudaSuccess; ++pass) {      // the first pass warms up
+        if (mode == 0) k_probe_mufu<0><<<sms, threads>>>(sink, reps, cyc);
+        if (mode == 1) k_probe_mufu<1><<<sms, threads>>>(sink, reps, cyc);
+        if (mode == 2) k_probe_mufu<2><<<sms, threads>>>(sink, reps, cyc);
+        count_launch();
+        e = cudaDeviceSynchronize();
+    }
+    long long c = 0;
+    if (e == cudaSuccess) e = cudaMemcpy(&c, cyc, 8, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && c > 0) {
+        const double per_thread = 8.0 * reps * (mode == 1 ? 2.0 : 1.0);      // results (mode 2: tanh evaluations) per thread
+        *results_per_clock_per_sm = static_cast<float>(per_thread * threads / static_cast<double>(c));
+    }
+    cudaFree(sink);
+    cudaFree(cyc);
+    return e;
+}
+
 bool is_aggregate_kernel(const void* func) {
     return func == reinterpret_cast<const void*>(&k_aggregate<false>) || func == reinterpret_cast<const void*>(&k_aggregate<true>) ||
            func == reinterpret_cast<const void*>(&k_aggregate_v4<false>) || func == reinterpret_cast<const void*>(&k_aggregate_v4<true>);

@@ -1183,3 +1183,19 @@ def test_random_shapes_and_option_combinations_are_bit_identical():
                 else:
                     assert np.array_equal(s0, s1), ("scores", W, S_, n, dtype, o)
     assert cases == 30
+
+
+@pytest.mark.gpu
+def test_mufu_probe_reports_sixteen_results_per_clock_per_sm():
+    """gw_probe_mufu_rate: tanh.approx.f32 retires 16 per clock per SM once the SM holds >= 256 threads, the packed f16x2
+    form gives the same 16 RESULTS per clock (two operations per instruction), the bf16 engine's ex2 + rcp form 8 tanh per
+    clock: the MUFU floor under the thin layers (bench.py's mufu_frac) rests on these."""
+    for threads in (256, 512):
+        r = gw.probe_mufu_rate(0, threads)
+        assert 15.0 <= r <= 16.2, (threads, r)
+    assert 15.0 <= gw.probe_mufu_rate(1, 512) <= 16.2
+    assert 7.5 <= gw.probe_mufu_rate(2, 512) <= 8.1
+    with pytest.raises(gw.GwError):
+        gw.probe_mufu_rate(3, 512)
+    with pytest.raises(gw.GwError):
+        gw.probe_mufu_rate(0, 100)
