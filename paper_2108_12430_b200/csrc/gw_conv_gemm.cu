@@ -666,6 +666,24 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
         // EPI_CHAIN: this layer's 32 biases stay in registers (every lane needs all of them for every tile; read from shared
         // memory they were 128 of the ~2600 shared-memory wavefronts per super-tile that bound the kernel)
         float chain_bias[EPI == EPI_CHAIN ? 32 : 1];
+        // EPI_STORE with N a constant (32, 64, 128: whole-window DeepClean layers): a warp's chunk pair covers the same 64 (32)
+        // columns in every stage -- 32 (4 cp + 2 hsel + which) mod N does not depend on cp -- so their biases are read once.  A
+        // broadcast ld.shared.v4 costs four wavefronts of the shared-memory data stage (its 512 bytes of return traffic), and
+        // per stage they were two thirds of the epilogue's wavefronts on the stage that bounds these layers.  Same for the 64
+        // columns of EPI_FINAL.
+        constexpr bool kStoreBiasRegs = EPI == EPI_STORE && NT != 0;
+        float4 store_bias[kStoreBiasRegs ? 2 : 1][kStoreBiasRegs ? 8 : 1];
+        if (kStoreBiasRegs) {
+#pragma unroll
+            for (int which = 0; which < 2; ++which)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) store_bias[which][j] = lds_f4(bias_u32 + 4u * (ch_col[which] + 4 * j));
+        }
+        float4 final_bias[EPI == EPI_FINAL ? 16 : 1];
+        if (EPI == EPI_FINAL) {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) final_bias[j] = lds_f4(bias_u32 + 16u * j);
+        }
         if (EPI == EPI_CHAIN) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
@@ -710,10 +728,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                     tmem_ld_32x32(taddr + 32 * ca, ra);
                     tmem_ld_32x32(taddr + 32 * cbk, rb);
                     float4 bia[2][8];                          // bias of both chunks, fetched under the TMEM latency
+                    if (NT == 0) {
 #pragma unroll
-                    for (int which = 0; which < 2; ++which)
+                        for (int which = 0; which < 2; ++which)
 #pragma unroll
-                        for (int j = 0; j < 8; ++j) bia[which][j] = lds_f4(bias_u32 + 4u * (ch_col[2 * cp + which] + 4 * j));
+                            for (int j = 0; j < 8; ++j) bia[which][j] = lds_f4(bias_u32 + 4u * (ch_col[2 * cp + which] + 4 * j));
+                    }
                     const uint32_t stg = stage_u32 + ((ostep % p.out_bufs) << 15);
                     if (lane == 0) {                           // the store that last read this buffer has drained it
                         TR_WAIT(1, if (p.out_bufs == 2) tma_store_wait_read<1>(); else tma_store_wait_read<0>())
@@ -734,7 +754,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             uint32_t o[4];
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
-                                const float4 b4 = bia[which][2 * jj + h];
+                                const float4 b4 = NT ? store_bias[which][2 * jj + h] : bia[which][2 * jj + h];
                                 o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
                                 o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
                             }
@@ -831,7 +851,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) k_conv_gemm_umma(const __grid
                             uint32_t o[4];
 #pragma unroll
                             for (int h = 0; h < 2; ++h) {
-                                const float4 b4 = lds_f4(bias_u32 + 4u * (32 * which + 8 * jj + 4 * h));
+                                const float4 b4 = final_bias[8 * which + 2 * jj + h];
                                 o[2 * h] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h]) + b4.x, __uint_as_float(r[8 * jj + 4 * h + 1]) + b4.y);
                                 o[2 * h + 1] = act_pack_t<ACT, FMT>(__uint_as_float(r[8 * jj + 4 * h + 2]) + b4.z, __uint_as_float(r[8 * jj + 4 * h + 3]) + b4.w);
                             }
