@@ -156,6 +156,11 @@ def run_reference(args):
     if rank != 0:
         return
     cfg = S.config_c3(args.streams, args.stride, WINDOW)
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1 and os.environ.get("OMP_NUM_THREADS") == "1":
+        # torchrun pins every rank to one OpenMP thread; the other ranks do no work here, so rank 0 takes the host's cores
+        # as in the N = 1 run (the line's `cores` says what was used)
+        import oracle
+        oracle.set_num_threads(len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
     times, cores = oracle_rate(cfg, args.dtype, args.warmup + args.steps, budget_s=args.reference_budget)
     timed = times[args.warmup:] if len(times) > args.warmup else times[-1:]
     sec = sum(timed)
